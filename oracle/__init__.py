@@ -1,0 +1,143 @@
+"""TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+ctypes wrapper around ``oracle_vesnet.c`` -- the plain long-double CPU statement of
+VesNet's far-field single-layer sum (PAPER.md:129-136 eqs 2.8/2.9, :173 trapezoid rule,
+:140-144 who contributes, :163-169 spectral derivative).  Only ``tests/``,
+``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` / ``--impl reference``
+legs may import this package.  It imports nothing from ``paper_2606_25569_b200`` and
+that package imports nothing from here.
+
+All arrays are float64 numpy arrays on the host; results are float64.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "oracle_vesnet.c")
+_LIB = os.path.join(_HERE, "liboracle_vesnet.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (-O2, no FMA contraction, OpenMP over targets only)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared",
+               "-o", _LIB, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        lib = ctypes.CDLL(_LIB)
+        d = ctypes.POINTER(ctypes.c_double)
+        i64 = ctypes.c_int64
+        u8 = ctypes.POINTER(ctypes.c_ubyte)
+        lib.oracle_num_threads.restype = ctypes.c_int
+        lib.oracle_farfield.argtypes = [d, d, d, i64, i64, ctypes.c_double, d]
+        lib.oracle_farfield_subset.argtypes = [d, d, d, i64, i64, ctypes.c_double,
+                                               ctypes.POINTER(i64), i64, d]
+        lib.oracle_farfield_targets.argtypes = [d, d, d, i64, i64, ctypes.c_double, d, i64, d]
+        lib.oracle_weights.argtypes = [d, i64, i64, d, d]
+        lib.oracle_near_mask.argtypes = [d, d, i64, i64, u8]
+        lib.oracle_farfield_masked.argtypes = [d, d, d, i64, i64, ctypes.c_double, u8, d]
+        _lib = lib
+    return _lib
+
+
+def _c(a, shape=None):
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    if shape is not None and a.shape != tuple(shape):
+        raise ValueError(f"expected shape {shape}, got {a.shape}")
+    return a
+
+
+def _p(a):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+
+
+def num_threads() -> int:
+    return int(_load().oracle_num_threads())
+
+
+def farfield(X, F, W, mu=1.0):
+    """U[nves,npts,2]: eq 2.8/2.9 by the trapezoid rule over every other vesicle."""
+    X = _c(X); nves, npts, _ = X.shape
+    F = _c(F, X.shape); W = _c(W, (nves, npts))
+    U = np.empty_like(X)
+    rc = _load().oracle_farfield(_p(X), _p(F), _p(W), nves, npts, float(mu), _p(U))
+    if rc:
+        raise ValueError(f"oracle_farfield rc={rc}")
+    return U
+
+
+def farfield_subset(X, F, W, idx, mu=1.0):
+    """U at the flat point indices ``idx`` only -> [len(idx), 2]."""
+    X = _c(X); nves, npts, _ = X.shape
+    F = _c(F, X.shape); W = _c(W, (nves, npts))
+    idx = np.ascontiguousarray(idx, dtype=np.int64)
+    Us = np.empty((idx.size, 2), dtype=np.float64)
+    rc = _load().oracle_farfield_subset(_p(X), _p(F), _p(W), nves, npts, float(mu),
+                                        idx.ctypes.data_as(ctypes.POINTER(ctypes.c_int64)),
+                                        idx.size, _p(Us))
+    if rc:
+        raise ValueError(f"oracle_farfield_subset rc={rc}")
+    return Us
+
+
+def farfield_targets(X, F, W, xt, mu=1.0):
+    """Velocity at free points xt[nt,2] induced by all vesicles -> [nt,2]."""
+    X = _c(X); nves, npts, _ = X.shape
+    F = _c(F, X.shape); W = _c(W, (nves, npts))
+    xt = _c(xt)
+    Ut = np.empty_like(xt)
+    rc = _load().oracle_farfield_targets(_p(X), _p(F), _p(W), nves, npts, float(mu),
+                                         _p(xt), xt.shape[0], _p(Ut))
+    if rc:
+        raise ValueError(f"oracle_farfield_targets rc={rc}")
+    return Ut
+
+
+def weights(X, return_derivative=False):
+    """W[nves,npts] = (2 pi/N) |dX/dalpha| by explicit DFT -> ik -> inverse DFT."""
+    X = _c(X); nves, npts, _ = X.shape
+    W = np.empty((nves, npts), dtype=np.float64)
+    dX = np.empty_like(X) if return_derivative else None
+    rc = _load().oracle_weights(_p(X), nves, npts, _p(W), _p(dX) if dX is not None else None)
+    if rc:
+        raise ValueError(f"oracle_weights rc={rc}")
+    return (W, dX) if return_derivative else W
+
+
+def near_mask(X, W):
+    """near[P, nves] (uint8): vesicle vp within its arclength spacing of point t."""
+    X = _c(X); nves, npts, _ = X.shape
+    W = _c(W, (nves, npts))
+    near = np.empty((nves * npts, nves), dtype=np.uint8)
+    rc = _load().oracle_near_mask(_p(X), _p(W), nves, npts,
+                                  near.ctypes.data_as(ctypes.POINTER(ctypes.c_ubyte)))
+    if rc:
+        raise ValueError(f"oracle_near_mask rc={rc}")
+    return near
+
+
+def farfield_masked(X, F, W, near, mu=1.0):
+    """Direct sum with near vesicles' contribution set to zero."""
+    X = _c(X); nves, npts, _ = X.shape
+    F = _c(F, X.shape); W = _c(W, (nves, npts))
+    near = np.ascontiguousarray(near, dtype=np.uint8)
+    if near.shape != (nves * npts, nves):
+        raise ValueError("near mask shape")
+    U = np.empty_like(X)
+    rc = _load().oracle_farfield_masked(_p(X), _p(F), _p(W), nves, npts, float(mu),
+                                        near.ctypes.data_as(ctypes.POINTER(ctypes.c_ubyte)), _p(U))
+    if rc:
+        raise ValueError(f"oracle_farfield_masked rc={rc}")
+    return U

@@ -1,0 +1,315 @@
+"""Pins for the oracle (CPU only).  Each test fixes the oracle against something other
+than itself: a closed form, a continuous integral computed by mpmath (tests/golden/),
+an identity of the Stokes kernel, a library routine (numpy.fft), or a brute-force pair
+loop written independently here.  A dropped term, wrong sign, transposed index or wrong
+exclusion set fails at least one of them (see test_wrong_kernels_are_caught)."""
+import math
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+
+FOURPI = 4.0 * math.pi
+
+
+def _load(golden_dir, name):
+    rows = []
+    with open(os.path.join(golden_dir, name)) as fh:
+        for line in fh:
+            if line.startswith("#") or not line.strip():
+                continue
+            rows.append([float(t) for t in line.split()])
+    return np.array(rows)
+
+
+def _rot(th):
+    return np.array([[math.cos(th), -math.sin(th)], [math.sin(th), math.cos(th)]])
+
+
+def _ellipse(a, b, n, th=0.0, c=(0.0, 0.0)):
+    al = 2 * np.pi * np.arange(n) / n
+    P = np.stack([a * np.cos(al), b * np.sin(al)], -1) @ _rot(th).T + np.asarray(c)
+    return P, al
+
+
+def _random_problem(rng, nves, npts, spread=3.0):
+    """Well separated blobs of random points (not curves: the sum does not care)."""
+    X = rng.normal(size=(nves, npts, 2)) * 0.3 + spread * rng.normal(size=(nves, 1, 2))
+    F = rng.normal(size=(nves, npts, 2))
+    W = rng.uniform(0.5, 1.5, size=(nves, npts))
+    return X, F, W
+
+
+# ----------------------------------------------------------------------------- kernel values
+def test_point_stokeslet_closed_form(golden_dir):
+    """eq 2.9 for one source: nves=2, npts=1, second vesicle carries no force."""
+    for x, y, gx, gy, ex, ey in _load(golden_dir, "point_stokeslet.txt"):
+        X = np.array([[[0.0, 0.0]], [[x, y]]])
+        F = np.array([[[gx, gy]], [[0.0, 0.0]]])
+        W = np.ones((2, 1))
+        U = oracle.farfield(X, F, W, mu=1.0)
+        assert np.allclose(FOURPI * U[1, 0], [ex, ey], rtol=0, atol=2e-15)
+        assert np.all(U[0, 0] == 0.0)           # the only other vesicle has zero density
+
+
+def test_mu_scaling_and_prefactor():
+    rng = np.random.default_rng(1)
+    X, F, W = _random_problem(rng, 3, 5)
+    U1 = oracle.farfield(X, F, W, mu=1.0)
+    U2 = oracle.farfield(X, F, W, mu=2.5)
+    assert np.allclose(U2 * 2.5, U1, rtol=1e-15, atol=0)
+
+
+# ----------------------------------------------------------------------------- whole operator vs exact integrals
+def test_constant_density_on_circle(golden_dir):
+    """Trapezoid sum vs closed form / mpmath quadrature of eq 2.8."""
+    N = 64
+    for R, ex, ey, x, y, cx, cy, qx, qy in _load(golden_dir, "circle_constant_density.txt"):
+        src, _ = _ellipse(R, R, N)
+        X = np.stack([src, np.tile([[x, y]], (N, 1))])
+        F = np.stack([np.tile([[ex, ey]], (N, 1)), np.zeros((N, 2))])
+        W = np.stack([np.full(N, 2 * np.pi * R / N), np.ones(N)])
+        U = oracle.farfield(X, F, W)
+        assert np.allclose(FOURPI * U[1, 0], [cx, cy], rtol=0, atol=5e-15)
+        assert abs(cx - qx) < 1e-20 and abs(cy - qy) < 1e-20
+
+
+def test_smooth_density_on_rotated_ellipse_uses_oracle_weights(golden_dir):
+    """General density, general shape: oracle.weights + oracle.farfield together reproduce
+    the continuous integral (spectral convergence for far targets)."""
+    N = 128
+    src, al = _ellipse(1.0, 0.4, N, th=0.35, c=(0.2, -0.1))
+    f = np.stack([0.5 + np.cos(2 * al) - 0.3 * np.sin(al),
+                  -0.2 + 0.7 * np.sin(3 * al) + 0.4 * np.cos(al)], -1)
+    rows = _load(golden_dir, "ellipse_smooth_density.txt")
+    tg = np.zeros((N, 2)); tg[:] = rows[0, :2]; tg[:len(rows)] = rows[:, :2]
+    X = np.stack([src, tg])
+    F = np.stack([f, np.zeros((N, 2))])
+    W = oracle.weights(X)
+    W[1] = 1.0
+    U = oracle.farfield(X, F, W)
+    assert np.allclose(FOURPI * U[1, :len(rows)], rows[:, 2:4], rtol=0, atol=3e-14)
+
+
+@pytest.mark.parametrize("a,b", [(1.0, 1.0), (1.0, 0.4)])
+def test_single_layer_of_normal_vanishes_outside(a, b):
+    """S[n](x) = 0 outside a closed curve (Stokeslet is divergence free).  With the paper's
+    printed '+log' and no identity the residual is O(0.1): this pins reading A1."""
+    N = 128
+    src, al = _ellipse(a, b, N, th=0.6, c=(0.3, 0.2))
+    tx, ty = -a * np.sin(al), b * np.cos(al)                     # dX/dalpha in the body frame
+    sa = np.sqrt(tx ** 2 + ty ** 2)
+    nrm = np.stack([ty / sa, -tx / sa], -1) @ _rot(0.6).T        # outward unit normal
+    tg, _ = _ellipse(a + 1.0, b + 1.0, N, th=0.6, c=(0.3, 0.2))   # targets at distance >= 1
+    X = np.stack([src, tg]); F = np.stack([nrm, np.zeros((N, 2))])
+    W = np.stack([sa * 2 * np.pi / N, np.ones(N)])
+    U = oracle.farfield(X, F, W)
+    assert np.abs(U[1]).max() < 1e-15
+
+
+def test_single_layer_of_normal_spectral_decay_N32():
+    """N=32: residual decays with distance like the trapezoid rule's (R/rho)^N."""
+    N = 32
+    src, al = _ellipse(1.0, 1.0, N)
+    res = []
+    for d in (0.5, 1.0, 2.0):
+        tg, _ = _ellipse(1.0 + d, 1.0 + d, N)
+        X = np.stack([src, tg]); F = np.stack([src.copy(), np.zeros((N, 2))])
+        W = np.stack([np.full(N, 2 * np.pi / N), np.ones(N)])
+        res.append(np.abs(oracle.farfield(X, F, W)[1]).max())
+    assert 1e-8 < res[0] < 1e-5 and res[1] < 1e-9 and res[2] < 1e-14
+
+
+# ----------------------------------------------------------------------------- identities
+def test_scaling_identity_pins_log_and_exclusion():
+    """X -> sX, W -> sW  =>  U -> s [ U - ln(s)/(4 pi mu) (G_tot - G_own) ],  G_v = sum_j F W."""
+    rng = np.random.default_rng(2)
+    X, F, W = _random_problem(rng, 4, 6)
+    s, mu = 1.7, 0.9
+    U = oracle.farfield(X, F, W, mu)
+    Us = oracle.farfield(s * X, F, s * W, mu)
+    G = (F * W[..., None]).sum(1)                                 # [nves, 2]
+    corr = (G.sum(0)[None, :] - G)[:, None, :]                    # other vesicles only
+    assert np.allclose(Us, s * (U - math.log(s) / (FOURPI * mu) * corr), rtol=0, atol=1e-14)
+
+
+def test_adjoint_identity():
+    """<a, S g> = <S a, g> with W = 1: G(r) = G(-r) = G^T and a symmetric exclusion set."""
+    rng = np.random.default_rng(3)
+    X, _, _ = _random_problem(rng, 5, 7)
+    a = rng.normal(size=X.shape); g = rng.normal(size=X.shape)
+    W = np.ones(X.shape[:2])
+    lhs = (a * oracle.farfield(X, g, W)).sum()
+    rhs = (oracle.farfield(X, a, W) * g).sum()
+    assert abs(lhs - rhs) < 1e-13 * max(1.0, abs(lhs))
+
+
+def test_brute_force_symmetric_pair_sum():
+    """Independent loop over unordered cross-vesicle pairs, K built once per pair and
+    scattered both ways (different loop structure, numpy float64)."""
+    rng = np.random.default_rng(4)
+    nves, npts = 4, 5
+    X, F, W = _random_problem(rng, nves, npts)
+    g = (F * W[..., None]).reshape(-1, 2); P = X.reshape(-1, 2)
+    ves = np.repeat(np.arange(nves), npts)
+    U = np.zeros_like(P)
+    for i in range(len(P)):
+        for j in range(i + 1, len(P)):
+            if ves[i] == ves[j]:
+                continue
+            r = P[i] - P[j]
+            K = -0.5 * math.log(r @ r) * np.eye(2) + np.outer(r, r) / (r @ r)
+            U[i] += K @ g[j]
+            U[j] += K @ g[i]
+    U /= FOURPI
+    assert np.allclose(oracle.farfield(X, F, W).reshape(-1, 2), U, rtol=0, atol=1e-14)
+
+
+def test_translation_rotation_linearity_superposition():
+    rng = np.random.default_rng(5)
+    X, F, W = _random_problem(rng, 4, 6)
+    U = oracle.farfield(X, F, W)
+    # translation: only differences enter
+    assert np.allclose(oracle.farfield(X + np.array([3.0, -2.0]), F, W), U, rtol=0, atol=1e-14)
+    # rotation equivariance
+    R = _rot(0.83)
+    assert np.allclose(oracle.farfield(X @ R.T, F @ R.T, W), U @ R.T, rtol=0, atol=1e-14)
+    # linearity in F and dependence on F, W only through F*W
+    F2 = rng.normal(size=F.shape)
+    assert np.allclose(oracle.farfield(X, 2 * F - 3 * F2, W),
+                       2 * U - 3 * oracle.farfield(X, F2, W), rtol=0, atol=1e-13)
+    assert np.allclose(oracle.farfield(X, F * W[..., None], np.ones_like(W)), U, rtol=0, atol=1e-14)
+    # superposition over source vesicles: U = sum over "only vesicle s carries force"
+    acc = np.zeros_like(U)
+    for s in range(X.shape[0]):
+        Fs = np.zeros_like(F); Fs[s] = F[s]
+        Us = oracle.farfield(X, Fs, W)
+        assert np.all(Us[s] == 0.0)                               # a vesicle never acts on itself
+        acc += Us
+    assert np.allclose(acc, U, rtol=0, atol=1e-14)
+
+
+def test_permutation_equivariance():
+    rng = np.random.default_rng(6)
+    X, F, W = _random_problem(rng, 5, 4)
+    U = oracle.farfield(X, F, W)
+    pv = rng.permutation(5)
+    assert np.allclose(oracle.farfield(X[pv], F[pv], W[pv]), U[pv], rtol=0, atol=1e-14)
+    pp = rng.permutation(4)
+    assert np.allclose(oracle.farfield(X[:, pp], F[:, pp], W[:, pp]), U[:, pp], rtol=0, atol=1e-14)
+
+
+def test_single_vesicle_is_zero_and_errors():
+    rng = np.random.default_rng(7)
+    X, F, W = _random_problem(rng, 1, 9)
+    assert np.all(oracle.farfield(X, F, W) == 0.0)
+    with pytest.raises(ValueError):
+        oracle.farfield(X, F, W, mu=0.0)
+
+
+def test_subset_and_free_targets_agree_with_full():
+    rng = np.random.default_rng(8)
+    X, F, W = _random_problem(rng, 4, 6)
+    U = oracle.farfield(X, F, W, mu=1.3).reshape(-1, 2)
+    idx = np.array([0, 7, 23, 11])
+    assert np.array_equal(oracle.farfield_subset(X, F, W, idx, mu=1.3), U[idx])
+    # free targets see every vesicle: U_free(x) = sum over all; check against superposition of
+    # a 5-vesicle problem whose extra vesicle holds the targets and no force
+    xt = rng.normal(size=(6, 2)) * 5
+    X5 = np.concatenate([X, xt[None]], 0); F5 = np.concatenate([F, np.zeros((1, 6, 2))], 0)
+    W5 = np.concatenate([W, np.ones((1, 6))], 0)
+    assert np.allclose(oracle.farfield_targets(X, F, W, xt, mu=1.3),
+                       oracle.farfield(X5, F5, W5, mu=1.3)[4], rtol=0, atol=1e-15)
+
+
+def test_wrong_kernels_are_caught():
+    """The pins are sharp: the paper's printed kernel (+log, no I) and a transposed dyad
+    both violate S[n] = 0 by O(0.1) on the same input where the oracle gives < 1e-15."""
+    N = 128
+    src, al = _ellipse(1.0, 0.4, N)
+    tx, ty = -np.sin(al), 0.4 * np.cos(al)
+    sa = np.hypot(tx, ty)
+    g = np.stack([ty / sa, -tx / sa], -1) * (sa * 2 * np.pi / N)[:, None]
+    x = np.array([1.5, 1.2])
+    r = x - src; r2 = (r ** 2).sum(1)
+    printed = (0.5 * np.log(r2)[:, None] * g + ((r * g).sum(1) / r2)[:, None] * r).sum(0)
+    nodyad = (-0.5 * np.log(r2)[:, None] * g).sum(0)
+    assert np.abs(printed).max() > 0.05 and np.abs(nodyad).max() > 0.05
+
+
+# ----------------------------------------------------------------------------- weights
+def test_weights_circle_and_ellipse_pointwise(golden_dir):
+    for N in (32, 33, 128):
+        for (a, b, th, c) in [(0.8, 0.8, 0.0, (0, 0)), (1.0, 0.4, 0.9, (2.0, -1.0))]:
+            P, al = _ellipse(a, b, N, th, c)
+            W = oracle.weights(P[None])[0]
+            exact = (2 * np.pi / N) * np.sqrt(a * a * np.sin(al) ** 2 + b * b * np.cos(al) ** 2)
+            assert np.allclose(W, exact, rtol=0, atol=2e-15)
+    per = _load(golden_dir, "ellipse_perimeter.txt")[0, 0]
+    P, _ = _ellipse(1.0, 0.4, 128)
+    assert abs(oracle.weights(P[None]).sum() - per) < 1e-14
+    P, _ = _ellipse(1.0, 0.4, 32)
+    assert 1e-9 < abs(oracle.weights(P[None]).sum() - per) < 1e-6      # N=32: -4.7e-8 (not yet converged)
+
+
+@pytest.mark.parametrize("N", [1, 2, 3, 8, 31, 32, 33, 100, 128, 129])
+def test_weights_match_numpy_fft(N):
+    """Library routine: derivative via numpy.fft with the Nyquist mode zeroed (reading A4)."""
+    rng = np.random.default_rng(100 + N)
+    X = rng.normal(size=(3, N, 2))
+    k = np.fft.fftfreq(N, 1.0 / N)
+    if N % 2 == 0:
+        k[N // 2] = 0.0
+    d = np.fft.ifft(1j * k[None, :, None] * np.fft.fft(X, axis=1), axis=1).real
+    W, dX = oracle.weights(X, return_derivative=True)
+    assert np.allclose(dX, d, rtol=0, atol=1e-12 * max(1, N))
+    assert np.allclose(W, (2 * np.pi / N) * np.hypot(d[..., 0], d[..., 1]), rtol=0, atol=1e-12 * max(1, N))
+
+
+def test_weights_invariances_and_circulant_form():
+    rng = np.random.default_rng(9)
+    N = 16
+    X = rng.normal(size=(2, N, 2))
+    W = oracle.weights(X)
+    assert np.allclose(oracle.weights(X @ _rot(1.1).T + 4.0), W, rtol=0, atol=1e-14)
+    assert np.allclose(oracle.weights(2.5 * X), 2.5 * W, rtol=0, atol=1e-14)
+    # circulant differentiation matrix D_jk = 1/2 (-1)^(j-k) cot((j-k) pi / N), even N (textbook form)
+    j = np.arange(N)[:, None]; k = np.arange(N)[None, :]
+    with np.errstate(divide="ignore"):
+        D = 0.5 * (-1.0) ** (j - k) / np.tan((j - k) * np.pi / N)
+    D[np.arange(N), np.arange(N)] = 0.0
+    d = np.einsum("jk,vkc->vjc", D, X)
+    assert np.allclose(W, (2 * np.pi / N) * np.hypot(d[..., 0], d[..., 1]), rtol=0, atol=1e-13)
+
+
+# ----------------------------------------------------------------------------- near-field mask variant
+def test_near_mask_and_masked_sum():
+    """Two ellipses 0.03 apart (closer than the arclength spacing) and one far away."""
+    N = 32
+    A, _ = _ellipse(1.0, 0.4, N, c=(0.0, 0.0))
+    B, _ = _ellipse(1.0, 0.4, N, c=(0.0, 0.83))          # gap 0.03 at the minor-axis tips
+    C, _ = _ellipse(1.0, 0.4, N, c=(6.0, 0.0))
+    X = np.stack([A, B, C])
+    W = oracle.weights(X)
+    rng = np.random.default_rng(10)
+    F = rng.normal(size=X.shape)
+    near = oracle.near_mask(X, W)
+    h = W.max(1)
+    # brute-force definition: dist(point, vesicle) <= arclength spacing of that vesicle
+    P = X.reshape(-1, 2)
+    for t in range(3 * N):
+        for vp in range(3):
+            d = np.sqrt(((P[t] - X[vp]) ** 2).sum(1)).min()
+            assert near[t, vp] == (1 if (vp != t // N and d <= h[vp]) else 0)
+    assert near[:N, 1].any() and near[N:2 * N, 0].any() and not near[:, 2].any() and not near[2 * N:].any()
+    # masked sum = full sum minus the masked vesicles' contributions (superposition)
+    U = oracle.farfield(X, F, W)
+    Um = oracle.farfield_masked(X, F, W, near)
+    FB = np.zeros_like(F); FB[1] = F[1]
+    UB = oracle.farfield(X, FB, W)                       # vesicle B's contribution everywhere
+    rows = near[:N, 1].astype(bool)
+    assert np.allclose(Um[0][rows], (U[0] - UB[0])[rows], rtol=0, atol=1e-13)
+    assert np.allclose(Um[0][~rows], U[0][~rows], rtol=0, atol=0)
+    assert np.array_equal(Um[2], U[2])
