@@ -1,0 +1,98 @@
+/*
+ * vesnet_farfield.h -- C-ABI boundary of the B200-native far-field module of VesNet
+ * (arxiv/paper_2606_25569).  Plain C, no CUDA or torch types in any signature.
+ *
+ * The module is the one conventional, data-parallel piece VesNet keeps beside its
+ * networks: "DirectSingleLayerIntegral(X, f)" (Alg. 4 line 3), the
+ * O((MN)^2) direct evaluation of the single-layer integral between vesicles that is
+ * "done without any approximation" and dominates the time step.
+ *
+ * Mathematics (PAPER.md:129-136 eqs 2.8/2.9, :173 trapezoid rule, :140-144 eq 2.10):
+ *
+ *   U[v,i,:] = 1/(4 pi mu) * sum_{v' != v} sum_{j<npts}
+ *                  ( -log|r| I + r r^T / |r|^2 ) F[v',j,:] W[v',j],   r = X[v,i,:] - X[v',j,:]
+ *
+ * (the extracted paper text prints "+log|r|" and drops the identity; see DESIGN.md
+ * reading A1).  W are the trapezoid arclength weights ds = |dX/dalpha| 2 pi / npts with
+ * the derivative taken spectrally.
+ *
+ * Conventions for every call:
+ *  - Arrays are contiguous, row-major, interleaved (x, y): X, F, U are [nves, npts, 2],
+ *    W is [nves, npts].  `precision` selects storage AND arithmetic: VN_F32 -> float,
+ *    VN_F64 -> double for every array of the call.  mu is a host double.
+ *  - "device pointer" = memory of the CURRENT CUDA device, owned by the caller, never
+ *    freed or retained by the library.  X, F, U must be aligned to one (x, y) pair
+ *    (8 B fp32 / 16 B fp64), W to one element.  Outputs are overwritten and must not
+ *    alias inputs.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Device
+ *    calls only enqueue work and return; scratch memory is stream-ordered
+ *    (cudaMallocAsync / cudaFreeAsync on `stream`), so back-to-back calls on one stream
+ *    need no host synchronisation.
+ *  - Errors are return codes only; nothing is printed, thrown or aborted.
+ *      VN_ERR_INVALID_ARG  null pointer, nves < 1, npts < 1, nves*npts >= 2^31,
+ *                          mu not finite or <= 0, bad enum, misaligned pointer
+ *      VN_ERR_UNSUPPORTED  current device is not compute capability 10.x (there is no
+ *                          fallback of any kind, by design)
+ *      VN_ERR_CUDA         a CUDA runtime call failed (allocation, launch)
+ *    Argument checks happen before any CUDA call, so they work without a GPU.
+ *  - Input values are not validated: NaN/Inf propagate.  Points of DIFFERENT vesicles
+ *    are assumed distinct; a coincident cross-vesicle pair gives a non-finite value at
+ *    that target only (reading A5).  nves == 1 is valid and yields U == 0.
+ */
+#ifndef VESNET_FARFIELD_H
+#define VESNET_FARFIELD_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    VN_OK = 0,
+    VN_ERR_INVALID_ARG = 1,
+    VN_ERR_UNSUPPORTED = 2,
+    VN_ERR_CUDA = 3
+} vn_status;
+
+typedef enum { VN_F32 = 0, VN_F64 = 1 } vn_precision;
+
+/* Far-field single-layer potential at every membrane point, own vesicle excluded
+ * (north_star).  All pointers are DEVICE pointers.
+ * Steps run on the device: pack g = F*W, pair sum over all other vesicles' points,
+ * two-level accumulation, scale by 1/(4 pi mu), store.  U is overwritten. */
+vn_status vn_farfield(const void *X, const void *F, const void *W,
+                      int64_t nves, int64_t npts, double mu,
+                      void *U, vn_precision precision, void *stream);
+
+/* Trapezoid arclength weights W[v,j] = (2 pi / npts) |dX_v/dalpha (alpha_j)|,
+ * alpha_j = 2 pi j / npts, derivative by Fourier differentiation with the unmatched
+ * k = npts/2 mode dropped for even npts (reading A4).
+ * X, W are DEVICE pointers.  W is overwritten. */
+vn_status vn_arclength_weights(const void *X, int64_t nves, int64_t npts,
+                               void *W, vn_precision precision, void *stream);
+
+/* The whole hot path from HOST buffers: copies X, F (and W when W != NULL) to the
+ * device, computes W with vn_arclength_weights when W == NULL, runs vn_farfield and
+ * copies U back; returns after U is complete (synchronous).  X, F, W, U are HOST
+ * pointers (pinned memory makes the copies asynchronous to the host but is not
+ * required).  Device buffers are cached per process and grown on demand. */
+vn_status vn_farfield_host(const void *X, const void *F, const void *W,
+                           int64_t nves, int64_t npts, double mu,
+                           void *U, vn_precision precision);
+
+/* Number of kernels of this library launched by the calling process so far
+ * (all entry points, all streams).  Used by bench.py to report gpu_launches. */
+int64_t vn_launch_count(void);
+
+/* Static, NUL-terminated description of a status code. */
+const char *vn_status_string(vn_status s);
+
+/* Library version: major*10000 + minor*100 + patch. */
+int vn_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+
+#endif /* VESNET_FARFIELD_H */

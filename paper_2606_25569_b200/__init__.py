@@ -1,0 +1,167 @@
+"""paper_2606_25569_b200 -- B200-native far-field module of VesNet (arxiv/paper_2606_25569).
+
+Thin Python binding over the C-ABI library ``libvesnet_farfield.so`` (include/vesnet_farfield.h).
+The functions below carry the same names as the C entry points and do argument marshalling only:
+every step of the path (weights, packing, pair sum, reduction, scaling) runs in the library's
+sm_100a kernels.  PyTorch is used for device memory and streams, nothing else.  There is no CPU
+or PyTorch fallback: if the library is missing or the device is not a B200-class GPU the call
+raises.
+
+    W = vn_arclength_weights(X)                 # X: [nves, npts, 2] cuda tensor, fp32 or fp64
+    U = vn_farfield(X, F, W, mu=1.0)            # U: [nves, npts, 2]
+    U = vn_farfield_host(X, F, None, mu=1.0)    # host (numpy / pinned torch) buffers, whole path
+
+`inputs` (seeded synthetic suspensions) is importable without the library.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+VN_F32, VN_F64 = 0, 1
+VN_OK, VN_ERR_INVALID_ARG, VN_ERR_UNSUPPORTED, VN_ERR_CUDA = 0, 1, 2, 3
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libvesnet_farfield.so")
+_lib = None
+
+
+class VesnetError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        msg = lib().vn_status_string(status).decode()
+        super().__init__(f"{where}: {msg} (vn_status {status})")
+
+
+def lib():
+    """Load the C-ABI library (built in-tree by ``python -m paper_2606_25569_b200.build``)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_2606_25569_b200.build` "
+                              "(nvcc, sm_100a). There is no fallback path.")
+        L = ctypes.CDLL(LIB_PATH)
+        vp, i64, dbl, ci = ctypes.c_void_p, ctypes.c_int64, ctypes.c_double, ctypes.c_int
+        L.vn_farfield.argtypes = [vp, vp, vp, i64, i64, dbl, vp, ci, vp]
+        L.vn_farfield.restype = ci
+        L.vn_arclength_weights.argtypes = [vp, i64, i64, vp, ci, vp]
+        L.vn_arclength_weights.restype = ci
+        L.vn_farfield_host.argtypes = [vp, vp, vp, i64, i64, dbl, vp, ci]
+        L.vn_farfield_host.restype = ci
+        L.vn_launch_count.argtypes = []
+        L.vn_launch_count.restype = i64
+        L.vn_status_string.argtypes = [ci]
+        L.vn_status_string.restype = ctypes.c_char_p
+        L.vn_version.argtypes = []
+        L.vn_version.restype = ci
+        _lib = L
+    return _lib
+
+
+def _prec(t):
+    import torch
+    if t.dtype == torch.float32:
+        return VN_F32
+    if t.dtype == torch.float64:
+        return VN_F64
+    raise TypeError(f"dtype must be float32 or float64, got {t.dtype}")
+
+
+def _check_dev(name, t, shape=None, dtype=None):
+    if not t.is_cuda:
+        raise ValueError(f"{name} must be a CUDA tensor (device calls take device pointers)")
+    if not t.is_contiguous():
+        raise ValueError(f"{name} must be contiguous")
+    if shape is not None and tuple(t.shape) != tuple(shape):
+        raise ValueError(f"{name}: expected shape {tuple(shape)}, got {tuple(t.shape)}")
+    if dtype is not None and t.dtype != dtype:
+        raise TypeError(f"{name}: expected dtype {dtype}, got {t.dtype}")
+
+
+def _stream_ptr(stream):
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return ctypes.c_void_p(s.cuda_stream)
+
+
+def vn_farfield(X, F, W, mu: float = 1.0, out=None, stream=None):
+    """U = far-field single-layer potential (device tensors; enqueues on the current stream)."""
+    import torch
+    nves, npts, two = X.shape
+    if two != 2:
+        raise ValueError("X must be [nves, npts, 2]")
+    _check_dev("X", X)
+    _check_dev("F", F, X.shape, X.dtype)
+    _check_dev("W", W, (nves, npts), X.dtype)
+    if out is None:
+        out = torch.empty_like(X)
+    _check_dev("out", out, X.shape, X.dtype)
+    with torch.cuda.device(X.device):
+        rc = lib().vn_farfield(X.data_ptr(), F.data_ptr(), W.data_ptr(), nves, npts, float(mu),
+                               out.data_ptr(), _prec(X), _stream_ptr(stream))
+    if rc != VN_OK:
+        raise VesnetError(rc, "vn_farfield")
+    return out
+
+
+def vn_arclength_weights(X, out=None, stream=None):
+    """W[v, j] = (2 pi / npts) |dX_v/dalpha| (device tensors; enqueues on the current stream)."""
+    import torch
+    nves, npts, two = X.shape
+    if two != 2:
+        raise ValueError("X must be [nves, npts, 2]")
+    _check_dev("X", X)
+    if out is None:
+        out = torch.empty((nves, npts), dtype=X.dtype, device=X.device)
+    _check_dev("out", out, (nves, npts), X.dtype)
+    with torch.cuda.device(X.device):
+        rc = lib().vn_arclength_weights(X.data_ptr(), nves, npts, out.data_ptr(), _prec(X), _stream_ptr(stream))
+    if rc != VN_OK:
+        raise VesnetError(rc, "vn_arclength_weights")
+    return out
+
+
+def _host_ptr(name, a, shape, dtype_name):
+    """numpy array or CPU torch tensor -> (pointer, keepalive)."""
+    import numpy as np
+    if hasattr(a, "data_ptr"):                      # torch CPU tensor (possibly pinned)
+        if a.is_cuda or not a.is_contiguous():
+            raise ValueError(f"{name} must be a contiguous HOST tensor")
+        if tuple(a.shape) != tuple(shape) or str(a.dtype).split(".")[-1] != dtype_name:
+            raise ValueError(f"{name}: expected {dtype_name}{tuple(shape)}")
+        return a.data_ptr(), a
+    a = np.asarray(a)
+    if not a.flags["C_CONTIGUOUS"] or a.shape != tuple(shape) or a.dtype.name != dtype_name:
+        raise ValueError(f"{name}: expected C-contiguous {dtype_name}{tuple(shape)}")
+    return a.ctypes.data, a
+
+
+def vn_farfield_host(X, F, W=None, mu: float = 1.0, out=None):
+    """Whole hot path from host buffers (numpy arrays or CPU torch tensors); synchronous.
+    W=None computes the arclength weights on the device from X."""
+    import numpy as np
+    nves, npts, two = X.shape
+    if two != 2:
+        raise ValueError("X must be [nves, npts, 2]")
+    dtype_name = str(X.dtype).split(".")[-1]
+    if dtype_name not in ("float32", "float64"):
+        raise TypeError("dtype must be float32 or float64")
+    prec = VN_F32 if dtype_name == "float32" else VN_F64
+    pX, kX = _host_ptr("X", X, (nves, npts, 2), dtype_name)
+    pF, kF = _host_ptr("F", F, (nves, npts, 2), dtype_name)
+    pW, kW = (None, None) if W is None else _host_ptr("W", W, (nves, npts), dtype_name)
+    if out is None:
+        out = np.empty((nves, npts, 2), dtype=dtype_name)
+    pU, kU = _host_ptr("out", out, (nves, npts, 2), dtype_name)
+    rc = lib().vn_farfield_host(pX, pF, pW, nves, npts, float(mu), pU, prec)
+    if rc != VN_OK:
+        raise VesnetError(rc, "vn_farfield_host")
+    return out
+
+
+def vn_launch_count() -> int:
+    return int(lib().vn_launch_count())
+
+
+def vn_version() -> int:
+    return int(lib().vn_version())

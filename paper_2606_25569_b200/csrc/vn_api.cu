@@ -1,0 +1,166 @@
+// vn_api.cu -- the extern "C" boundary declared in include/vesnet_farfield.h: argument checks
+// (before any CUDA call), device check (sm_100 family only, no fallback), dispatch by precision,
+// and the host-buffer entry point.
+#include <math.h>
+
+#include <mutex>
+
+#include "vn_common.cuh"
+
+namespace vn {
+
+unsigned long long g_launches = 0;
+
+vn_status farfield_f32(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, double mu,
+                       void *U, cudaStream_t st);
+vn_status farfield_f64(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, double mu,
+                       void *U, cudaStream_t st);
+vn_status arclength_weights(const void *X, int64_t nves, int64_t npts, void *W, vn_precision prec, cudaStream_t st);
+
+Split choose_split(long long P, int targets_per_block, int slots, int min_tiles)
+{
+    Split sp;
+    sp.n_tb = (int)((P + targets_per_block - 1) / targets_per_block);
+    sp.n_tiles = (int)((P + kTile - 1) / kTile);
+    int max_chunks = sp.n_tiles / min_tiles;
+    if (max_chunks < 1) max_chunks = 1;
+    if (max_chunks > 32) max_chunks = 32;      // bounds the partial-sum scratch to 32 * P results
+    double best = -1.0;
+    sp.n_chunks = 1;
+    for (int c = 1; c <= max_chunks; ++c) {
+        const long long blocks = (long long)sp.n_tb * c;
+        const long long waves = (blocks + slots - 1) / slots;
+        const double eff = (double)blocks / (double)(waves * slots);
+        if (eff > best + 1e-3) { best = eff; sp.n_chunks = c; }
+        else if (eff > best - 1e-3 && c > sp.n_chunks) { sp.n_chunks = c; if (eff > best) best = eff; }
+    }
+    return sp;
+}
+
+static vn_status check_device()
+{
+    static int ok = -1;   // -1 unknown, 1 ok, 0 unsupported
+    if (ok < 0) {
+        int dev = 0, major = 0;
+        VN_CUDA(cudaGetDevice(&dev));
+        VN_CUDA(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+        ok = (major == 10) ? 1 : 0;
+        if (ok) {
+            // keep freed stream-ordered scratch cached in the pool instead of returning it to the OS
+            cudaMemPool_t pool;
+            if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+                unsigned long long thr = ~0ull;
+                (void)cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
+            }
+        }
+    }
+    return ok ? VN_OK : VN_ERR_UNSUPPORTED;
+}
+
+static bool misaligned(const void *p, size_t a) { return ((uintptr_t)p % a) != 0; }
+
+static vn_status check_shape(int64_t nves, int64_t npts, vn_precision prec)
+{
+    if (prec != VN_F32 && prec != VN_F64) return VN_ERR_INVALID_ARG;
+    if (nves < 1 || npts < 1) return VN_ERR_INVALID_ARG;
+    if (npts >= (1ll << 31) || nves >= (1ll << 31) || nves * npts >= (1ll << 31)) return VN_ERR_INVALID_ARG;
+    return VN_OK;
+}
+
+}  // namespace vn
+
+using namespace vn;
+
+extern "C" {
+
+vn_status vn_farfield(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, double mu,
+                      void *U, vn_precision precision, void *stream)
+{
+    if (!X || !F || !W || !U) return VN_ERR_INVALID_ARG;
+    if (check_shape(nves, npts, precision) != VN_OK) return VN_ERR_INVALID_ARG;
+    if (!isfinite(mu) || !(mu > 0.0)) return VN_ERR_INVALID_ARG;
+    const size_t pair = precision == VN_F32 ? 8 : 16;
+    if (misaligned(X, pair) || misaligned(F, pair) || misaligned(U, pair) || misaligned(W, pair / 2))
+        return VN_ERR_INVALID_ARG;
+    if (U == X || U == F || U == W) return VN_ERR_INVALID_ARG;
+    const vn_status ds = check_device();
+    if (ds != VN_OK) return ds;
+    cudaStream_t st = (cudaStream_t)stream;
+    return precision == VN_F32 ? farfield_f32(X, F, W, nves, npts, mu, U, st)
+                               : farfield_f64(X, F, W, nves, npts, mu, U, st);
+}
+
+vn_status vn_arclength_weights(const void *X, int64_t nves, int64_t npts, void *W, vn_precision precision,
+                               void *stream)
+{
+    if (!X || !W) return VN_ERR_INVALID_ARG;
+    if (check_shape(nves, npts, precision) != VN_OK) return VN_ERR_INVALID_ARG;
+    const size_t pair = precision == VN_F32 ? 8 : 16;
+    if (misaligned(X, pair) || misaligned(W, pair / 2) || W == X) return VN_ERR_INVALID_ARG;
+    const vn_status ds = check_device();
+    if (ds != VN_OK) return ds;
+    return arclength_weights(X, nves, npts, W, precision, (cudaStream_t)stream);
+}
+
+vn_status vn_farfield_host(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, double mu,
+                           void *U, vn_precision precision)
+{
+    if (!X || !F || !U) return VN_ERR_INVALID_ARG;
+    if (check_shape(nves, npts, precision) != VN_OK) return VN_ERR_INVALID_ARG;
+    if (!isfinite(mu) || !(mu > 0.0)) return VN_ERR_INVALID_ARG;
+    if (U == X || U == F || U == W) return VN_ERR_INVALID_ARG;
+    const vn_status ds = check_device();
+    if (ds != VN_OK) return ds;
+
+    // process-wide cached device buffers and stream, grown on demand
+    static std::mutex mtx;
+    static cudaStream_t st = nullptr;
+    static char *buf = nullptr;
+    static size_t cap = 0;
+    std::lock_guard<std::mutex> lock(mtx);
+    if (!st) VN_CUDA(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking));
+    const size_t P = (size_t)(nves * npts);
+    const size_t es = precision == VN_F32 ? 4 : 8;
+    const size_t bX = 2 * es * P, bW = es * P;
+    auto up = [](size_t b) { return (b + 255) & ~(size_t)255; };
+    const size_t need = 3 * up(bX) + up(bW);
+    if (need > cap) {
+        if (buf) VN_CUDA(cudaFree(buf));
+        buf = nullptr; cap = 0;
+        VN_CUDA(cudaMalloc((void **)&buf, need));
+        cap = need;
+    }
+    char *dX = buf, *dF = dX + up(bX), *dU = dF + up(bX), *dW = dU + up(bX);
+    VN_CUDA(cudaMemcpyAsync(dX, X, bX, cudaMemcpyHostToDevice, st));
+    VN_CUDA(cudaMemcpyAsync(dF, F, bX, cudaMemcpyHostToDevice, st));
+    vn_status rc;
+    if (W) {
+        VN_CUDA(cudaMemcpyAsync(dW, W, bW, cudaMemcpyHostToDevice, st));
+    } else {
+        rc = arclength_weights(dX, nves, npts, dW, precision, st);
+        if (rc != VN_OK) return rc;
+    }
+    rc = precision == VN_F32 ? farfield_f32(dX, dF, dW, nves, npts, mu, dU, st)
+                             : farfield_f64(dX, dF, dW, nves, npts, mu, dU, st);
+    if (rc != VN_OK) return rc;
+    VN_CUDA(cudaMemcpyAsync(U, dU, bX, cudaMemcpyDeviceToHost, st));
+    VN_CUDA(cudaStreamSynchronize(st));
+    return VN_OK;
+}
+
+int64_t vn_launch_count(void) { return (int64_t)__atomic_load_n(&g_launches, __ATOMIC_RELAXED); }
+
+const char *vn_status_string(vn_status s)
+{
+    switch (s) {
+        case VN_OK: return "ok";
+        case VN_ERR_INVALID_ARG: return "invalid argument";
+        case VN_ERR_UNSUPPORTED: return "unsupported device (needs compute capability 10.x, sm_100a build)";
+        case VN_ERR_CUDA: return "CUDA runtime error";
+    }
+    return "unknown status";
+}
+
+int vn_version(void) { return 100; }
+
+}  // extern "C"

@@ -1,0 +1,49 @@
+"""The C-ABI library loads on a CPU-only box, exports every symbol the header declares, and
+rejects bad arguments before touching CUDA (no compute calls here)."""
+import ctypes
+import os
+import re
+
+import paper_2606_25569_b200 as vn
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _declared():
+    text = open(os.path.join(ROOT, "include", "vesnet_farfield.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(vn_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_library_exports_every_declared_symbol():
+    from paper_2606_25569_b200 import build
+    build.build()
+    L = vn.lib()
+    names = _declared()
+    assert {"vn_farfield", "vn_arclength_weights", "vn_farfield_host", "vn_status_string",
+            "vn_version", "vn_launch_count"} <= set(names)
+    for n in names:
+        assert hasattr(L, n), n
+    assert vn.vn_version() >= 100
+    assert L.vn_status_string(0) == b"ok" and b"invalid" in L.vn_status_string(1)
+
+
+def test_argument_validation_needs_no_gpu():
+    L = vn.lib()
+    buf = (ctypes.c_double * 64)()
+    p = ctypes.addressof(buf)
+    q = p + 256 if False else ctypes.addressof((ctypes.c_double * 64)())
+    INV = vn.VN_ERR_INVALID_ARG
+    assert L.vn_farfield(None, p, p, 2, 4, 1.0, q, vn.VN_F64, None) == INV          # null
+    assert L.vn_farfield(p, p, p, 0, 4, 1.0, q, vn.VN_F64, None) == INV             # nves < 1
+    assert L.vn_farfield(p, p, p, 2, 0, 1.0, q, vn.VN_F64, None) == INV             # npts < 1
+    assert L.vn_farfield(p, p, p, 1 << 20, 1 << 12, 1.0, q, vn.VN_F32, None) == INV  # >= 2^31 points
+    assert L.vn_farfield(p, p, p, 2, 4, 0.0, q, vn.VN_F64, None) == INV             # mu <= 0
+    assert L.vn_farfield(p, p, p, 2, 4, float("nan"), q, vn.VN_F64, None) == INV    # mu not finite
+    assert L.vn_farfield(p, p, p, 2, 4, 1.0, q, 7, None) == INV                     # bad enum
+    assert L.vn_farfield(p + 4, p, p, 2, 4, 1.0, q, vn.VN_F32, None) == INV         # misaligned pair
+    assert L.vn_farfield(p, p, p, 2, 4, 1.0, p, vn.VN_F64, None) == INV             # U aliases X
+    assert L.vn_arclength_weights(None, 2, 4, q, vn.VN_F64, None) == INV
+    assert L.vn_arclength_weights(p, 2, -1, q, vn.VN_F64, None) == INV
+    assert L.vn_farfield_host(p, None, None, 2, 4, 1.0, q, vn.VN_F64) == INV
+    assert L.vn_farfield_host(p, p, None, 2, 4, -1.0, q, vn.VN_F64) == INV

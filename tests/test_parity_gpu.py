@@ -1,0 +1,240 @@
+"""Parity of the CUDA path with the oracle (run on the B200 box: pytest -m gpu).
+
+Every call goes through the C-ABI library via the thin binding.  Tolerances are north_star's:
+relative L2 <= 1e-12 (fp64) and <= 2e-5 (fp32), measured against the oracle on the same seeded
+inputs; for fp32 the oracle consumes the fp32-rounded inputs promoted to double, so the measured
+error is arithmetic, not input quantisation."""
+import numpy as np
+import pytest
+
+import oracle
+import paper_2606_25569_b200 as vn
+from paper_2606_25569_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+TOL = {np.float64: 1e-12, np.float32: 2e-5}
+_cache = {}
+
+
+def rel_l2(a, b):
+    a = np.asarray(a, dtype=np.float64).ravel()
+    b = np.asarray(b, dtype=np.float64).ravel()
+    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+def dev(a, dtype):
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=dtype)).cuda()
+
+
+def problem(index):
+    """Config `index` with oracle weights (fp64), cached for the session."""
+    if index not in _cache:
+        s = inputs.config(index)
+        _cache[index] = (s, oracle.weights(s.X))
+    return _cache[index]
+
+
+def gpu_farfield(X, F, W, mu, dtype):
+    U = vn.vn_farfield(dev(X, dtype), dev(F, dtype), dev(W, dtype), mu)
+    torch.cuda.synchronize()
+    return U.cpu().numpy()
+
+
+def oracle_inputs(X, F, W, dtype):
+    """What the GPU sees, promoted to double."""
+    return tuple(np.asarray(a, dtype=dtype).astype(np.float64) for a in (X, F, W))
+
+
+def sample_targets(P, n, seed):
+    rng = np.random.Generator(np.random.PCG64(seed))
+    # always include the first and last points and both ends of a tile / vesicle boundary
+    fixed = np.array([0, 1, 127, 128, P // 2, P - 129, P - 128, P - 1])
+    return np.unique(np.concatenate([fixed, rng.choice(P, size=n, replace=False)]))
+
+
+# ------------------------------------------------------------------------------------- full parity
+@pytest.mark.parametrize("index,dtype", [(0, np.float64), (0, np.float32), (1, np.float64), (1, np.float32)])
+def test_farfield_full_parity(index, dtype):
+    s, W = problem(index)
+    Xo, Fo, Wo = oracle_inputs(s.X, s.F, W, dtype)
+    ref = oracle.farfield(Xo, Fo, Wo, s.mu)
+    got = gpu_farfield(s.X, s.F, W, s.mu, dtype)
+    err = rel_l2(got, ref)
+    print(f"config{index} {np.dtype(dtype).name}: rel-L2 {err:.3e}")
+    assert err <= TOL[dtype]
+
+
+# ------------------------------------------------------------------------------------- full-size configs, sampled targets
+@pytest.mark.parametrize("index,dtype,nsample", [(2, np.float32, 4096), (2, np.float64, 4096),
+                                                 (3, np.float32, 3072), (3, np.float64, 3072)])
+def test_farfield_sampled_parity_large(index, dtype, nsample):
+    s, W = problem(index)
+    P = s.nves * s.npts
+    idx = sample_targets(P, nsample, 260625569 + 100)
+    Xo, Fo, Wo = oracle_inputs(s.X, s.F, W, dtype)
+    ref = oracle.farfield_subset(Xo, Fo, Wo, idx, s.mu)
+    got = gpu_farfield(s.X, s.F, W, s.mu, dtype).reshape(-1, 2)[idx]
+    err = rel_l2(got, ref)
+    print(f"config{index} {np.dtype(dtype).name}: sampled rel-L2 {err:.3e} over {len(idx)} targets")
+    assert err <= TOL[dtype]
+
+
+def test_config4_sequence_fp32():
+    """8,000 x 128, ten consecutive evaluations on one stream reusing the device buffers; the
+    oracle checks calls 0 and 9 on sampled targets, fp64-GPU checks call 0 on ALL targets."""
+    s, W = problem(4)
+    P = s.nves * s.npts
+    idx = sample_targets(P, 1024, 260625569 + 100)
+    seq = [dev(x, np.float32) for x in s.X_sequence]
+    Xd = torch.empty_like(seq[0])
+    Fd, Wd = dev(s.F, np.float32), dev(W, np.float32)
+    Ud = torch.empty_like(Xd)
+    outs = {}
+    for c in range(10):
+        Xd.copy_(seq[c])
+        vn.vn_farfield(Xd, Fd, Wd, s.mu, out=Ud)
+        if c in (0, 9):
+            outs[c] = Ud.clone()
+    torch.cuda.synchronize()
+    for c in (0, 9):
+        Xo, Fo, Wo = oracle_inputs(s.X_sequence[c], s.F, W, np.float32)
+        ref = oracle.farfield_subset(Xo, Fo, Wo, idx, s.mu)
+        err = rel_l2(outs[c].cpu().numpy().reshape(-1, 2)[idx], ref)
+        print(f"config4 call {c}: sampled rel-L2 {err:.3e}")
+        assert err <= TOL[np.float32]
+    # all targets: fp32 GPU vs fp64 GPU on the same fp32-rounded inputs
+    U64 = vn.vn_farfield(seq[0].double(), Fd.double(), Wd.double(), s.mu)
+    torch.cuda.synchronize()
+    err = rel_l2(outs[0].cpu().numpy(), U64.cpu().numpy())
+    print(f"config4 call 0: fp32 vs fp64 GPU over all targets rel-L2 {err:.3e}")
+    assert err <= TOL[np.float32]
+    # and the fp64 GPU result itself against the oracle on the sample
+    Xo, Fo, Wo = oracle_inputs(s.X_sequence[0], s.F, W, np.float32)
+    ref = oracle.farfield_subset(Xo, Fo, Wo, idx, s.mu)
+    assert rel_l2(U64.cpu().numpy().reshape(-1, 2)[idx], ref) <= TOL[np.float64]
+
+
+# ------------------------------------------------------------------------------------- edge shapes
+def _blobs(rng, nves, npts):
+    X = rng.normal(size=(nves, npts, 2)) * 0.3 + 4.0 * rng.normal(size=(nves, 1, 2))
+    F = rng.normal(size=(nves, npts, 2))
+    W = rng.uniform(0.5, 1.5, size=(nves, npts))
+    return X, F, W
+
+
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+@pytest.mark.parametrize("nves,npts", [(2, 1), (3, 2), (7, 3), (5, 31), (9, 32), (5, 33), (7, 100), (3, 129),
+                                       (2, 257), (37, 128), (11, 1000), (1030, 1), (3, 2049)])
+def test_edge_shapes(nves, npts, dtype):
+    rng = np.random.Generator(np.random.PCG64(1000 * nves + npts))
+    X, F, W = _blobs(rng, nves, npts)
+    mu = 0.7
+    Xo, Fo, Wo = oracle_inputs(X, F, W, dtype)
+    ref = oracle.farfield(Xo, Fo, Wo, mu)
+    got = gpu_farfield(X, F, W, mu, dtype)
+    assert got.shape == ref.shape and np.all(np.isfinite(got))
+    assert rel_l2(got, ref) <= TOL[dtype]
+
+
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+def test_single_vesicle_gives_zero(dtype):
+    rng = np.random.Generator(np.random.PCG64(5))
+    X, F, W = _blobs(rng, 1, 200)
+    got = gpu_farfield(X, F, W, 1.0, dtype)
+    assert np.all(got == 0.0)
+
+
+def test_mu_and_output_overwrite():
+    s, W = problem(0)
+    Xd, Fd, Wd = dev(s.X, np.float64), dev(s.F, np.float64), dev(W, np.float64)
+    out = torch.full_like(Xd, float("nan"))
+    U1 = vn.vn_farfield(Xd, Fd, Wd, 1.0, out=out)
+    U2 = vn.vn_farfield(Xd, Fd, Wd, 4.0)
+    torch.cuda.synchronize()
+    assert U1 is out and torch.isfinite(out).all()
+    assert torch.allclose(U2 * 4.0, U1, rtol=1e-14, atol=0)
+
+
+# ------------------------------------------------------------------------------------- weights (a-1)
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+@pytest.mark.parametrize("index", [0, 1, 3])
+def test_arclength_weights_parity(index, dtype):
+    s, _ = problem(index)
+    Xo = np.asarray(s.X, dtype=dtype).astype(np.float64)
+    ref = oracle.weights(Xo)
+    got = vn.vn_arclength_weights(dev(s.X, dtype))
+    torch.cuda.synchronize()
+    err = rel_l2(got.cpu().numpy(), ref)
+    print(f"weights config{index} {np.dtype(dtype).name}: rel-L2 {err:.3e}")
+    assert err <= TOL[dtype]
+
+
+@pytest.mark.parametrize("npts", [1, 2, 3, 8, 31, 32, 33, 100, 129, 257, 1500])
+def test_arclength_weights_edge_shapes(npts):
+    rng = np.random.Generator(np.random.PCG64(npts))
+    X = rng.normal(size=(5, npts, 2)) + 30.0
+    ref = oracle.weights(X)
+    got = vn.vn_arclength_weights(dev(X, np.float64))
+    torch.cuda.synchronize()
+    got = got.cpu().numpy()
+    if npts <= 2:
+        assert np.abs(got).max() < 1e-12          # only the mean and the dropped Nyquist mode exist
+    else:
+        assert rel_l2(got, ref) <= 1e-12
+
+
+# ------------------------------------------------------------------------------------- whole path, host buffers
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+def test_host_entry_point_whole_path(dtype):
+    s, _ = problem(1)
+    X = np.ascontiguousarray(s.X, dtype=dtype)
+    F = np.ascontiguousarray(s.F, dtype=dtype)
+    got = vn.vn_farfield_host(X, F, None, s.mu)                      # weights computed on the device
+    Xo, Fo = X.astype(np.float64), F.astype(np.float64)
+    idx = sample_targets(s.nves * s.npts, 2048, 3)
+    ref = oracle.farfield_subset(Xo, Fo, oracle.weights(Xo), idx, s.mu)
+    assert rel_l2(got.reshape(-1, 2)[idx], ref) <= TOL[dtype]
+    # pinned torch tensors and caller-supplied weights
+    Xp, Fp = torch.from_numpy(X).pin_memory(), torch.from_numpy(F).pin_memory()
+    Wp = torch.from_numpy(oracle.weights(Xo).astype(dtype)).pin_memory()
+    Up = torch.empty_like(Xp).pin_memory()
+    vn.vn_farfield_host(Xp, Fp, Wp, s.mu, out=Up)
+    assert rel_l2(Up.numpy().reshape(-1, 2)[idx], ref) <= TOL[dtype]
+
+
+# ------------------------------------------------------------------------------------- determinism, streams
+def test_determinism_bitwise():
+    s, W = problem(2)
+    Xd, Fd, Wd = dev(s.X, np.float32), dev(s.F, np.float32), dev(W, np.float32)
+    a = vn.vn_farfield(Xd, Fd, Wd).clone()
+    b = vn.vn_farfield(Xd, Fd, Wd)
+    torch.cuda.synchronize()
+    assert torch.equal(a, b)
+
+
+def test_side_stream_behind_producer():
+    """Enqueued on a non-default stream behind a producer kernel: no implicit device sync needed."""
+    s, W = problem(1)
+    Fd, Wd = dev(s.F, np.float64), dev(W, np.float64)
+    Xh = dev(s.X, np.float64)
+    ref = vn.vn_farfield(Xh, Fd, Wd)
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        Xd = torch.zeros_like(Xh)
+        for _ in range(20):                       # producer chain on the side stream
+            Xd = Xd * 0.5 + Xh * 0.5
+        Xd = Xd * 0 + Xh                          # ends exactly at Xh
+        got = vn.vn_farfield(Xd, Fd, Wd)
+    side.synchronize()
+    assert torch.equal(got, ref)
+
+
+def test_launch_counter_moves():
+    s, W = problem(0)
+    n0 = vn.vn_launch_count()
+    vn.vn_farfield(dev(s.X, np.float32), dev(s.F, np.float32), dev(W, np.float32))
+    torch.cuda.synchronize()
+    assert vn.vn_launch_count() >= n0 + 3
