@@ -35,9 +35,12 @@
  *                          fallback of any kind, by design)
  *      VN_ERR_CUDA         a CUDA runtime call failed (allocation, launch)
  *    Argument checks happen before any CUDA call, so they work without a GPU.
+ *  - VN_F32 shares one SFU reciprocal between two pairs (t = rcp(a*b), 1/a = t*b): squared
+ *    distances must keep a*b inside the fp32 normal range, i.e. 1e-9 < |r| < 1e9 in the
+ *    caller's units.  VN_F64 has no such restriction beyond normal doubles.
  *  - Input values are not validated: NaN/Inf propagate.  Points of DIFFERENT vesicles
- *    are assumed distinct; a coincident cross-vesicle pair gives a non-finite value at
- *    that target only (reading A5).  nves == 1 is valid and yields U == 0.
+ *    are assumed distinct; a coincident cross-vesicle pair gives an unspecified (possibly
+ *    non-finite) value at that target only (reading A5).  nves == 1 is valid and yields U == 0.
  */
 #ifndef VESNET_FARFIELD_H
 #define VESNET_FARFIELD_H
@@ -80,6 +83,14 @@ vn_status vn_arclength_weights(const void *X, int64_t nves, int64_t npts,
 vn_status vn_farfield_host(const void *X, const void *F, const void *W,
                            int64_t nves, int64_t npts, double mu,
                            void *U, vn_precision precision);
+
+/* Profiling aid (bench.py's roofline figure): while enabled, every vn_farfield /
+ * vn_farfield_host call records a CUDA event pair on its stream around the pair kernel
+ * alone (not the pack / finish kernels).  vn_profile_read waits for the recorded events,
+ * writes up to max_entries durations in milliseconds (oldest first) into the HOST array
+ * ms, forgets them, and returns how many it wrote (or -1 on a CUDA error). */
+vn_status vn_profile_enable(int enable);
+int64_t vn_profile_read(double *ms, int64_t max_entries);
 
 /* Number of kernels of this library launched by the calling process so far
  * (all entry points, all streams).  Used by bench.py to report gpu_launches. */

@@ -48,6 +48,10 @@ def lib():
         L.vn_arclength_weights.restype = ci
         L.vn_farfield_host.argtypes = [vp, vp, vp, i64, i64, dbl, vp, ci]
         L.vn_farfield_host.restype = ci
+        L.vn_profile_enable.argtypes = [ci]
+        L.vn_profile_enable.restype = ci
+        L.vn_profile_read.argtypes = [ctypes.POINTER(dbl), i64]
+        L.vn_profile_read.restype = i64
         L.vn_launch_count.argtypes = []
         L.vn_launch_count.restype = i64
         L.vn_status_string.argtypes = [ci]
@@ -157,6 +161,19 @@ def vn_farfield_host(X, F, W=None, mu: float = 1.0, out=None):
     if rc != VN_OK:
         raise VesnetError(rc, "vn_farfield_host")
     return out
+
+
+def vn_profile_enable(enable: bool) -> None:
+    lib().vn_profile_enable(1 if enable else 0)
+
+
+def vn_profile_read(max_entries: int = 4096):
+    """Durations (ms) of the pair kernel of every vn_farfield call since the last read."""
+    buf = (ctypes.c_double * max_entries)()
+    n = lib().vn_profile_read(buf, max_entries)
+    if n < 0:
+        raise VesnetError(VN_ERR_CUDA, "vn_profile_read")
+    return [buf[i] for i in range(n)]
 
 
 def vn_launch_count() -> int:

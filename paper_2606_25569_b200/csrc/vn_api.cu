@@ -4,12 +4,28 @@
 #include <math.h>
 
 #include <mutex>
+#include <vector>
 
 #include "vn_common.cuh"
 
 namespace vn {
 
 unsigned long long g_launches = 0;
+
+static bool g_profile = false;
+static std::mutex g_profile_mtx;
+static std::vector<cudaEvent_t> g_profile_events;   // begin, end, begin, end, ...
+
+void profile_mark(cudaStream_t st, bool begin)
+{
+    if (!g_profile) return;
+    std::lock_guard<std::mutex> lock(g_profile_mtx);
+    if (begin != (g_profile_events.size() % 2 == 0)) return;   // keep pairs well formed
+    cudaEvent_t ev;
+    if (cudaEventCreate(&ev) != cudaSuccess) return;
+    cudaEventRecord(ev, st);
+    g_profile_events.push_back(ev);
+}
 
 vn_status farfield_f32(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, double mu,
                        void *U, cudaStream_t st);
@@ -146,6 +162,32 @@ vn_status vn_farfield_host(const void *X, const void *F, const void *W, int64_t 
     VN_CUDA(cudaMemcpyAsync(U, dU, bX, cudaMemcpyDeviceToHost, st));
     VN_CUDA(cudaStreamSynchronize(st));
     return VN_OK;
+}
+
+vn_status vn_profile_enable(int enable)
+{
+    std::lock_guard<std::mutex> lock(g_profile_mtx);
+    g_profile = enable != 0;
+    return VN_OK;
+}
+
+int64_t vn_profile_read(double *ms, int64_t max_entries)
+{
+    std::lock_guard<std::mutex> lock(g_profile_mtx);
+    const int64_t pairs = (int64_t)(g_profile_events.size() / 2);
+    int64_t n = 0;
+    bool bad = false;
+    for (int64_t i = 0; i < pairs; ++i) {
+        cudaEvent_t a = g_profile_events[2 * i], b = g_profile_events[2 * i + 1];
+        float t = 0.f;
+        if (cudaEventSynchronize(b) != cudaSuccess || cudaEventElapsedTime(&t, a, b) != cudaSuccess) bad = true;
+        if (ms && n < max_entries) ms[n++] = (double)t;
+        cudaEventDestroy(a);
+        cudaEventDestroy(b);
+    }
+    for (size_t i = 2 * (size_t)pairs; i < g_profile_events.size(); ++i) cudaEventDestroy(g_profile_events[i]);
+    g_profile_events.clear();
+    return bad ? -1 : n;
 }
 
 int64_t vn_launch_count(void) { return (int64_t)__atomic_load_n(&g_launches, __ATOMIC_RELAXED); }

@@ -21,6 +21,9 @@ constexpr int kStages = 4;         // tiles in flight per block
 extern unsigned long long g_launches;
 inline void count_launch(int n = 1) { __atomic_fetch_add(&g_launches, (unsigned long long)n, __ATOMIC_RELAXED); }
 
+// optional event pair around the pair kernel (vn_profile_enable / vn_profile_read)
+void profile_mark(cudaStream_t st, bool begin);
+
 #define VN_CUDA(call)                                   \
     do {                                                \
         cudaError_t e_ = (call);                        \

@@ -214,8 +214,10 @@ vn_status farfield_f64(const void *X, const void *F, const void *W, int64_t nves
     VN_CUDA(cudaMallocAsync((void **)&part, (size_t)P * sizeof(double2) * (size_t)sp.n_chunks, st));
 
     pack_sources_f64<<<(P + 255) / 256, 256, 0, st>>>((const double2 *)X, (const double2 *)F, (const double *)W, P, src);
+    profile_mark(st, true);
     farfield_f64_kernel<<<sp.n_tb * sp.n_chunks, kThreads, 0, st>>>(src, (const double2 *)X, P, (int)npts, sp.n_tiles,
                                                                    sp.n_chunks, part);
+    profile_mark(st, false);
     finish_f64<<<(P + 255) / 256, 256, 0, st>>>(part, P, sp.n_chunks, 1.0 / (4.0 * 3.14159265358979323846 * mu),
                                                  (double2 *)U);
     count_launch(3);
