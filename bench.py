@@ -295,10 +295,13 @@ def main():
         peak_lane = SMS * lanes * sm_max * 1e6 / 1e12                     # T lane-instr/s at max clock
         k_ms = statistics.mean(kernel_ms) if kernel_ms else None
         achieved = LANE_OPS_PER_PAIR * susp.pairs / (k_ms * 1e-3) / 1e12 if k_ms else None
-        traffic = None
+        traffic = None                                   # dram bytes per launch from the committed ncu --set full capture
         try:
-            with open(os.path.join(ROOT, "profiles", "traffic.json")) as fh:
-                traffic = json.load(fh).get(f"config{args.workload}_{args.precision}")
+            import csv
+            with open(os.path.join(ROOT, "profiles", "traffic.csv")) as fh:
+                for row in csv.DictReader(fh):
+                    if row["workload"] == f"config{args.workload}" and row["precision"] == args.precision:
+                        traffic = int(row["dram_read_bytes"]) + int(row["dram_write_bytes"])
         except Exception:
             pass
         roofline = {"bound": "alu", "kernel": "farfield_%s_kernel" % args.precision,
