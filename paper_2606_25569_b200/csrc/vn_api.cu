@@ -53,6 +53,30 @@ Split choose_split(long long P, int targets_per_block, int slots, int min_tiles)
     return sp;
 }
 
+// Grid of the symmetric kernel: every super-tile walks a list of about sub*(n_st/2 + 1) source tiles,
+// cut into n_chunks chunks.  The run time is modelled as (waves of resident blocks) x (tiles of the
+// longest chunk); the chunk count minimising it wins, ties go to fewer chunks.
+SymSplit choose_sym_split(long long P, int super_tile, int slots, int min_tiles)
+{
+    SymSplit sp;
+    sp.n_st = (int)((P + super_tile - 1) / super_tile);
+    sp.n_tiles = (int)((P + kTile - 1) / kTile);
+    const int sub = super_tile / kTile;
+    const long long list = (long long)sub * (sp.n_st / 2 + 1);     // longest list over the super-tiles
+    long long max_chunks = list / min_tiles;
+    if (max_chunks < 1) max_chunks = 1;
+    if (max_chunks > 256) max_chunks = 256;
+    double best = 0.0;
+    sp.n_chunks = 1;
+    for (int c = 1; c <= (int)max_chunks; ++c) {
+        const long long blocks = (long long)sp.n_st * c;
+        const long long waves = (blocks + slots - 1) / slots;
+        const double cost = (double)waves * (double)((list + c - 1) / c);
+        if (c == 1 || cost < best * (1.0 - 1e-9)) { best = cost; sp.n_chunks = c; }
+    }
+    return sp;
+}
+
 static vn_status check_device()
 {
     static int ok = -1;   // -1 unknown, 1 ok, 0 unsupported

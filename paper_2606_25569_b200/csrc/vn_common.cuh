@@ -48,6 +48,15 @@ struct Split {
 // waves (wave quantisation) while each chunk keeps >= min_tiles tiles.
 Split choose_split(long long P, int targets_per_block, int slots, int min_tiles);
 
+// Symmetric (both-direction) decomposition of the fp32 kernel: block = (super-tile I, chunk c of I's
+// source-tile list); see vn_farfield_f32.cu.
+struct SymSplit {
+    int n_st;        // super-tiles (target blocks)
+    int n_tiles;     // source tiles of kTile points
+    int n_chunks;    // chunks of the per-super-tile list (grid = n_st * n_chunks)
+};
+SymSplit choose_sym_split(long long P, int super_tile, int slots, int min_tiles);
+
 // ---------------------------------------------------------------------------------------------
 // shared-memory / mbarrier / bulk-copy PTX
 __device__ __forceinline__ uint32_t smem_u32(const void *p)

@@ -3,41 +3,89 @@
 //   U_i = 1/(4 pi mu) sum_{j not in ves(i)} [ -log|r| g_j + (r.g_j)/|r|^2 r ],  r = x_i - y_j, g_j = f_j w_j
 //   (PAPER.md:129-136 eqs 2.8/2.9, :173 trapezoid rule, :425 DirectSingleLayerIntegral)
 //
-// Per pair, in the order the inner loop does it (canonical count 2 FADD + 3 FMUL + 6 FFMA + rcp + lg2):
-//   r = x - y; r2 = rx*rx + ry*ry; A += lg2(r2) * g; d = rx*gx + ry*gy; B += (d / r2) * r
+// The kernel matrix K(r) = -log|r| I + r r^T/|r|^2 is even in r and symmetric, so the unordered pair
+// {i, j} needs r, |r|^2, 1/|r|^2 and log|r|^2 ONCE and serves both U_i += K g_j and U_j += K g_i.
+// The kernel walks unordered pairs of point tiles and applies every pair in both directions:
+//   per unordered pair:  r = x - y; r2 = rx*rx + ry*ry; l = lg2(r2); inv = 1/r2           (shared)
+//   i <- j:  A_i += l * g_j;  B_i += ((r.g_j) * inv) * r                                     (7 FP32 instr)
+//   j <- i:  A_j += l * g_i;  B_j += ((r.g_i) * inv) * r                                     (7 FP32 instr)
 //   U = 1/(4 pi mu) * ( -(ln 2 / 2) * A + B )
-// Two targets share one packed register (FADD2/FMUL2/FFMA2) and one reciprocal:
-//   t = rcp(a*b), 1/a = t*b, 1/b = t*a   (a, b = the two r2 of the packed pair; 1.5 SFU ops per pair).
+// Two targets share one packed register (FADD2/FMUL2/FFMA2) and one SFU reciprocal:
+//   t = rcp(a*b), 1/a = t*b, 1/b = t*a   (a, b = the two r2 of the packed pair).
+// Per directed interaction this is 9.75 FP32 lane-instructions and 0.75 SFU ops against the canonical
+// 11 + 2 of a one-directional sum.
+//
+// Cross-block accumulation goes through 64-bit fixed-point atomics (integer addition is associative, so
+// the result is bitwise reproducible whatever the block order); see fixed_scale().
 #include "vn_common.cuh"
 
 namespace vn {
 
-// ------------------------------------------------------------------------------------------------
-// a-2: g = F*W, packed with the position into one 32-byte record per source, every value
-// duplicated so that one LDS.128 yields ready-made packed operands (yx,yx | yy,yy) and (gx,gx | gy,gy).
-__global__ void pack_sources_f32(const float2 *__restrict__ X, const float2 *__restrict__ F,
-                                 const float *__restrict__ W, int P, ulonglong2 *__restrict__ src)
+constexpr int kNP32 = 4;                          // packed target pairs per thread (8 targets)
+constexpr int kST32 = 2 * kNP32 * kThreads;       // points per super-tile (target block): 1024
+constexpr int kSub32 = kST32 / kTile;             // source tiles per super-tile: 8
+constexpr int kBatch = 8;                         // sources per cross-lane reduction batch
+
+// Power-of-two scale of the fixed-point accumulators.  gmax = max_j (|g_jx| + |g_jy|).  Every term of
+// the sum is bounded by (|ln2/2 * lg2 r2| + 1) |g_j| <= 64 gmax (|lg2| <= 150 over all positive fp32),
+// so every partial sum of any subset is below bnd = 64 P gmax; 2^(61-e) with 2^e <= bnd < 2^(e+1)
+// keeps |value * scale| < 2^62.
+__device__ __forceinline__ double fixed_scale(unsigned gmax_bits, int P)
 {
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= P) return;
-    const float2 y = X[s];
-    const float2 f = F[s];
-    const float w = W[s];
-    const float gx = f.x * w, gy = f.y * w;
-    src[2 * (size_t)s + 0] = make_ulonglong2(pk(y.x, y.x), pk(y.y, y.y));
-    src[2 * (size_t)s + 1] = make_ulonglong2(pk(gx, gx), pk(gy, gy));
+    const float gmax = __uint_as_float(gmax_bits);
+    if (!(gmax > 0.f) || !(gmax <= 3.4028234e38f)) return 1.0;   // all-zero (or non-finite) density
+    const double bnd = 64.0 * (double)P * (double)gmax;
+    const int e = ((__double2hiint(bnd) >> 20) & 0x7ff) - 1023;
+    return __hiloint2double((1023 + 61 - e) << 20, 0);
+}
+
+__device__ __forceinline__ void red_fixed(long long *addr, float v, double scale)
+{
+    const long long q = __double2ll_rn((double)v * scale);
+    atomicAdd((unsigned long long *)addr, (unsigned long long)q);
 }
 
 // ------------------------------------------------------------------------------------------------
-// a-3 / a-4: pair kernel.  Block = (target block, source chunk).  Each thread owns T = 2*NP targets
-// (NP packed pairs) in registers; source tiles of kTile points stream through a kStages-deep ring of
-// shared-memory buffers filled by 1-D bulk async copies (TMA) that complete on mbarriers.
-// A tile that cannot contain points of the block's own vesicles takes the fast path (no predicate
-// at all); the few tiles that overlap them, and a ragged last tile, take the predicated slow path.
+// a-2: g = F*W, packed with the position into one 32-byte record per source, every value
+// duplicated so that one LDS.128 yields ready-made packed operands (yx,yx | yy,yy) and (gx,gx | gy,gy).
+// Also gmax (bit pattern of a non-negative float orders like the float).
+__global__ void pack_sources_f32(const float2 *__restrict__ X, const float2 *__restrict__ F,
+                                 const float *__restrict__ W, int P, ulonglong2 *__restrict__ src,
+                                 unsigned *__restrict__ gmax_bits)
+{
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    float m = 0.f;
+    if (s < P) {
+        const float2 y = X[s];
+        const float2 f = F[s];
+        const float w = W[s];
+        const float gx = f.x * w, gy = f.y * w;
+        src[2 * (size_t)s + 0] = make_ulonglong2(pk(y.x, y.x), pk(y.y, y.y));
+        src[2 * (size_t)s + 1] = make_ulonglong2(pk(gx, gx), pk(gy, gy));
+        m = fabsf(gx) + fabsf(gy);
+        if (!(m <= 3.4028234e38f)) m = __int_as_float(0x7f800000);   // NaN / Inf -> +Inf
+    }
+    const unsigned wm = __reduce_max_sync(0xffffffffu, __float_as_uint(m));
+    if ((threadIdx.x & 31) == 0 && wm != 0u) atomicMax(gmax_bits, wm);
+}
+
+// ------------------------------------------------------------------------------------------------
+// a-3 / a-4: pair kernel.  Points are cut into super-tiles of kST32 = 1024 points.  Block (I, c) owns
+// super-tile I as targets (each thread 8 points in 4 packed register pairs, with their densities) and
+// walks chunk c of the source-tile list of I:
+//   s = 0            the 8 tiles of super-tile I itself: one-directional, own vesicle predicated out;
+//   s = 1 .. S_I     the tiles of super-tile (I + s) mod n_st: both directions.
+// With S_I = floor((n_st-1)/2) (+1 for I < n_st/2 when n_st is even) every unordered pair of super-tiles
+// is visited exactly once and every block has the same amount of work.
+// Source tiles of kTile points stream through a kStages-deep ring of shared-memory buffers filled by
+// 1-D bulk async copies (TMA) that complete on mbarriers.  A tile that cannot contain points of the
+// block's own vesicles takes the fast path (no predicate); tiles that overlap them and a ragged last
+// tile take the predicated path.
 template <int NP>
 __global__ void __launch_bounds__(kThreads, 4)
 farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict__ X, int P, int npts,
-                    int n_tiles, int n_chunks, float2 *__restrict__ part)
+                    int n_tiles, int n_st, int n_chunks, const unsigned *__restrict__ gmax_bits,
+                    long long *__restrict__ acc)
 {
     constexpr int T = 2 * NP;
     __shared__ __align__(128) ulonglong2 tile[kStages][kTile * 2];
@@ -45,10 +93,21 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
     __shared__ __align__(8) u64 empty_bar[kStages];
 
     const int tid = threadIdx.x;
-    const int tb = blockIdx.x / n_chunks;
-    const int sc = blockIdx.x - tb * n_chunks;
-    const int t_begin = chunk_tile_begin(n_tiles, n_chunks, sc);
-    const int nt = chunk_tile_begin(n_tiles, n_chunks, sc + 1) - t_begin;
+    const int lane = tid & 31;
+    const int I = blockIdx.x / n_chunks;
+    const int sc = blockIdx.x - I * n_chunks;
+    int S = (n_st - 1) / 2;
+    if ((n_st & 1) == 0 && I < n_st / 2) S += 1;
+    const int nu = kSub32 * (S + 1);
+    const int u_begin = chunk_tile_begin(nu, n_chunks, sc);
+    const int nt = chunk_tile_begin(nu, n_chunks, sc + 1) - u_begin;
+
+    auto tile_of = [&](int u) {        // source tile index of list entry u (may be >= n_tiles: empty)
+        const int s = u / kSub32;
+        int J = I + s;
+        if (J >= n_st) J -= n_st;
+        return J * kSub32 + (u - s * kSub32);
+    };
 
     if (tid == 0) {
 #pragma unroll
@@ -60,29 +119,45 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
     }
     __syncthreads();
 
-    auto issue = [&](int i) {   // one thread: tile i of this chunk -> stage i % kStages
+    auto issue = [&](int i) {   // one thread: list entry u_begin + i -> stage i % kStages
         const int s = i % kStages;
-        const int first = (t_begin + i) * kTile;
+        const int first = tile_of(u_begin + i) * kTile;
         const int cnt = min(kTile, P - first);
-        const uint32_t bytes = (uint32_t)cnt * 32u;
-        mbar_expect_tx(&full_bar[s], bytes);
-        bulk_g2s(&tile[s][0], src + 2 * (size_t)first, bytes, &full_bar[s]);
+        if (cnt > 0) {
+            const uint32_t bytes = (uint32_t)cnt * 32u;
+            mbar_expect_tx(&full_bar[s], bytes);
+            bulk_g2s(&tile[s][0], src + 2 * (size_t)first, bytes, &full_bar[s]);
+        } else {
+            mbar_arrive(&full_bar[s]);      // empty entry: complete the phase without a copy
+        }
     };
     if (tid == 0) {
         const int pre = nt < kStages ? nt : kStages;
         for (int i = 0; i < pre; ++i) issue(i);
     }
 
+    const double scale = fixed_scale(*gmax_bits, P);
+
     // targets: packed pair p holds points base + (2p)*kThreads + tid (low half) and
-    // base + (2p+1)*kThreads + tid (high half); indices past the end are clamped (never stored).
-    const int base = tb * (T * kThreads);
-    u64 tx[NP], ty[NP];
+    // base + (2p+1)*kThreads + tid (high half); indices past the end are clamped to P-1 and carry a
+    // zero density (their results are never stored, their contributions to others vanish).
+    const int base = I * kST32;
+    u64 tx[NP], ty[NP], hx[NP], hy[NP];          // positions and densities g_i of the targets
 #pragma unroll
     for (int p = 0; p < NP; ++p) {
-        const float2 a = X[min(base + (2 * p) * kThreads + tid, P - 1)];
-        const float2 b = X[min(base + (2 * p + 1) * kThreads + tid, P - 1)];
+        const int i0 = base + (2 * p) * kThreads + tid, i1 = i0 + kThreads;
+        const int c0 = min(i0, P - 1), c1 = min(i1, P - 1);
+        const float2 a = X[c0], b = X[c1];
         tx[p] = pk(a.x, b.x);
         ty[p] = pk(a.y, b.y);
+        float g0x, g0y, g1x, g1y, dum;
+        const ulonglong2 ga = src[2 * (size_t)c0 + 1], gb = src[2 * (size_t)c1 + 1];
+        upk(ga.x, g0x, dum); upk(ga.y, g0y, dum);
+        upk(gb.x, g1x, dum); upk(gb.y, g1y, dum);
+        if (i0 >= P) g0x = g0y = 0.f;
+        if (i1 >= P) g1x = g1y = 0.f;
+        hx[p] = pk(g0x, g1x);
+        hy[p] = pk(g0y, g1y);
     }
     // source index range occupied by the vesicles this block's targets belong to
     const int last_target = min(base + T * kThreads, P) - 1;
@@ -102,123 +177,170 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
         }
         mbar_wait(&full_bar[s], (i / kStages) & 1);
 
-        const int first = (t_begin + i) * kTile;
+        const int u = u_begin + i;
+        const bool both = u >= kSub32;                    // s >= 1: another super-tile, both directions
+        const int first = tile_of(u) * kTile;
+        const int cnt = min(kTile, P - first);
         const ulonglong2 *ts = tile[s];
-        const bool fast = (first >= span_end || first + kTile <= span_begin) && (first + kTile <= P);
+        const bool fast = both && (first >= span_end || first + kTile <= span_begin) && (cnt == kTile);
         if (fast) {
             u64 Ax[NP], Ay[NP], Bx[NP], By[NP];   // per-tile partial sums (two-level accumulation)
 #pragma unroll
             for (int p = 0; p < NP; ++p) Ax[p] = Ay[p] = Bx[p] = By[p] = 0ull;
-#pragma unroll 2
-            for (int j = 0; j < kTile; ++j) {
-                const ulonglong2 yy = ts[2 * j + 0];   // (yx,yx) (yy,yy)
-                const ulonglong2 gg = ts[2 * j + 1];   // (gx,gx) (gy,gy)
+            long long *accj = acc + 2 * (size_t)first + (lane >> 1);
+#pragma unroll 1
+            for (int jb = 0; jb < kTile; jb += kBatch) {
+                float c[2 * kBatch];              // this thread's contributions to the batch's sources
 #pragma unroll
-                for (int p = 0; p < NP; ++p) {
-                    const u64 rx = sub2(tx[p], yy.x);
-                    const u64 ry = sub2(ty[p], yy.y);
-                    const u64 r2 = fma2(rx, rx, mul2(ry, ry));
-                    float a, b;
-                    upk(r2, a, b);
-                    const float t = sfu_rcp(a * b);
-                    const u64 inv = pk(t * b, t * a);
-                    const u64 l = pk(sfu_lg2(a), sfu_lg2(b));
-                    Ax[p] = fma2(l, gg.x, Ax[p]);
-                    Ay[p] = fma2(l, gg.y, Ay[p]);
-                    const u64 d = fma2(rx, gg.x, mul2(ry, gg.y));
-                    const u64 q = mul2(d, inv);
-                    Bx[p] = fma2(q, rx, Bx[p]);
-                    By[p] = fma2(q, ry, By[p]);
+                for (int jj = 0; jj < kBatch; ++jj) {
+                    const ulonglong2 yy = ts[2 * (jb + jj) + 0];   // (yx,yx) (yy,yy)
+                    const ulonglong2 gg = ts[2 * (jb + jj) + 1];   // (gx,gx) (gy,gy)
+                    u64 cAx = 0ull, cAy = 0ull, cBx = 0ull, cBy = 0ull;
+#pragma unroll
+                    for (int p = 0; p < NP; ++p) {
+                        const u64 rx = sub2(tx[p], yy.x);
+                        const u64 ry = sub2(ty[p], yy.y);
+                        const u64 r2 = fma2(rx, rx, mul2(ry, ry));
+                        float a, b;
+                        upk(r2, a, b);
+                        const float t = sfu_rcp(a * b);
+                        const u64 inv = pk(t * b, t * a);
+                        const u64 l = pk(sfu_lg2(a), sfu_lg2(b));
+                        // i <- j
+                        Ax[p] = fma2(l, gg.x, Ax[p]);
+                        Ay[p] = fma2(l, gg.y, Ay[p]);
+                        const u64 q = mul2(fma2(rx, gg.x, mul2(ry, gg.y)), inv);
+                        Bx[p] = fma2(q, rx, Bx[p]);
+                        By[p] = fma2(q, ry, By[p]);
+                        // j <- i
+                        cAx = fma2(l, hx[p], cAx);
+                        cAy = fma2(l, hy[p], cAy);
+                        const u64 w = mul2(fma2(rx, hx[p], mul2(ry, hy[p])), inv);
+                        cBx = fma2(w, rx, cBx);
+                        cBy = fma2(w, ry, cBy);
+                    }
+                    float lo, hi;
+                    upk(fma2(KA, cAx, cBx), lo, hi);
+                    c[2 * jj + 0] = lo + hi;
+                    upk(fma2(KA, cAy, cBy), lo, hi);
+                    c[2 * jj + 1] = lo + hi;
                 }
+                // transpose-reduce over the warp: 16 values per lane -> lane L ends with the warp
+                // total of value (L >> 1); 16 shuffles instead of 16 x 5.
+#pragma unroll
+                for (int w = kBatch, m = 16; w >= 1; w >>= 1, m >>= 1) {
+                    const bool up = (lane & m) != 0;
+#pragma unroll
+                    for (int k = 0; k < w; ++k) {
+                        const float send = up ? c[k] : c[k + w];
+                        const float keep = up ? c[k + w] : c[k];
+                        c[k] = keep + __shfl_xor_sync(0xffffffffu, send, m);
+                    }
+                }
+                c[0] += __shfl_xor_sync(0xffffffffu, c[0], 1);
+                if ((lane & 1) == 0) red_fixed(accj + 2 * jb, c[0], scale);
             }
 #pragma unroll
             for (int p = 0; p < NP; ++p) {
                 Rx[p] = add2(Rx[p], fma2(KA, Ax[p], Bx[p]));
                 Ry[p] = add2(Ry[p], fma2(KA, Ay[p], By[p]));
             }
-        } else {
+        } else if (cnt > 0) {
             // predicated path: own-vesicle sources and the ragged tail are skipped per pair
-            const int cnt = min(kTile, P - first);
+            float ux[T], uy[T];
+            int own[T];
 #pragma unroll
-            for (int p = 0; p < NP; ++p) {
-                float x0, x1, y0, y1;
-                upk(tx[p], x0, x1);
-                upk(ty[p], y0, y1);
-                const int own0 = (min(base + (2 * p) * kThreads + tid, P - 1) / npts) * npts;
-                const int own1 = (min(base + (2 * p + 1) * kThreads + tid, P - 1) / npts) * npts;
-                float ax0 = 0.f, ay0 = 0.f, bx0 = 0.f, by0 = 0.f, ax1 = 0.f, ay1 = 0.f, bx1 = 0.f, by1 = 0.f;
+            for (int k = 0; k < T; ++k) {
+                ux[k] = uy[k] = 0.f;
+                own[k] = (min(base + k * kThreads + tid, P - 1) / npts) * npts;
+            }
 #pragma unroll 1
-                for (int j = 0; j < cnt; ++j) {
-                    const ulonglong2 yy = ts[2 * j + 0];
-                    const ulonglong2 gg = ts[2 * j + 1];
-                    float sx, sy, gx, gy, dum;
-                    upk(yy.x, sx, dum);
-                    upk(yy.y, sy, dum);
-                    upk(gg.x, gx, dum);
-                    upk(gg.y, gy, dum);
-                    const int jg = first + j;
-                    {
-                        const float rx = x0 - sx, ry = y0 - sy;
+            for (int j = 0; j < cnt; ++j) {
+                const ulonglong2 yy = ts[2 * j + 0];
+                const ulonglong2 gg = ts[2 * j + 1];
+                float sx, sy, gx, gy, dum;
+                upk(yy.x, sx, dum);
+                upk(yy.y, sy, dum);
+                upk(gg.x, gx, dum);
+                upk(gg.y, gy, dum);
+                const int jg = first + j;
+                float cx = 0.f, cy = 0.f;
+#pragma unroll
+                for (int k = 0; k < T; ++k) {
+                    float x0, x1, y0, y1, h0x, h1x, h0y, h1y;
+                    upk(tx[k >> 1], x0, x1);
+                    upk(ty[k >> 1], y0, y1);
+                    upk(hx[k >> 1], h0x, h1x);
+                    upk(hy[k >> 1], h0y, h1y);
+                    const float xk = (k & 1) ? x1 : x0, yk = (k & 1) ? y1 : y0;
+                    const float hkx = (k & 1) ? h1x : h0x, hky = (k & 1) ? h1y : h0y;
+                    if ((unsigned)(jg - own[k]) >= (unsigned)npts) {
+                        const float rx = xk - sx, ry = yk - sy;
                         const float r2 = fmaf(rx, rx, ry * ry);
-                        const float l = sfu_lg2(r2);
-                        const float q = fmaf(rx, gx, ry * gy) * sfu_rcp(r2);
-                        if ((unsigned)(jg - own0) >= (unsigned)npts) {
-                            ax0 = fmaf(l, gx, ax0); ay0 = fmaf(l, gy, ay0);
-                            bx0 = fmaf(q, rx, bx0); by0 = fmaf(q, ry, by0);
-                        }
-                    }
-                    {
-                        const float rx = x1 - sx, ry = y1 - sy;
-                        const float r2 = fmaf(rx, rx, ry * ry);
-                        const float l = sfu_lg2(r2);
-                        const float q = fmaf(rx, gx, ry * gy) * sfu_rcp(r2);
-                        if ((unsigned)(jg - own1) >= (unsigned)npts) {
-                            ax1 = fmaf(l, gx, ax1); ay1 = fmaf(l, gy, ay1);
-                            bx1 = fmaf(q, rx, bx1); by1 = fmaf(q, ry, by1);
-                        }
+                        const float l = -0.34657359027997264f * sfu_lg2(r2);
+                        const float inv = sfu_rcp(r2);
+                        const float q = fmaf(rx, gx, ry * gy) * inv;
+                        ux[k] += fmaf(l, gx, q * rx);
+                        uy[k] += fmaf(l, gy, q * ry);
+                        const float w = fmaf(rx, hkx, ry * hky) * inv;
+                        cx += fmaf(l, hkx, w * rx);
+                        cy += fmaf(l, hky, w * ry);
                     }
                 }
-                Rx[p] = add2(Rx[p], fma2(KA, pk(ax0, ax1), pk(bx0, bx1)));
-                Ry[p] = add2(Ry[p], fma2(KA, pk(ay0, ay1), pk(by0, by1)));
+                if (both) {
+#pragma unroll
+                    for (int m = 16; m >= 1; m >>= 1) {
+                        cx += __shfl_xor_sync(0xffffffffu, cx, m);
+                        cy += __shfl_xor_sync(0xffffffffu, cy, m);
+                    }
+                    if (lane == 0) {
+                        red_fixed(acc + 2 * (size_t)jg + 0, cx, scale);
+                        red_fixed(acc + 2 * (size_t)jg + 1, cy, scale);
+                    }
+                }
+            }
+#pragma unroll
+            for (int p = 0; p < NP; ++p) {
+                Rx[p] = add2(Rx[p], pk(ux[2 * p], ux[2 * p + 1]));
+                Ry[p] = add2(Ry[p], pk(uy[2 * p], uy[2 * p + 1]));
             }
         }
         __syncwarp();
-        if ((tid & 31) == 0) mbar_arrive(&empty_bar[s]);
+        if (lane == 0) mbar_arrive(&empty_bar[s]);
     }
 
-    // per-chunk partial results; a-5 finishes them
-    float2 *out = part + (size_t)sc * (size_t)P;
+    // this block's one-directional sums for its own targets
 #pragma unroll
     for (int p = 0; p < NP; ++p) {
         float x0, x1, y0, y1;
         upk(Rx[p], x0, x1);
         upk(Ry[p], y0, y1);
         const int i0 = base + (2 * p) * kThreads + tid;
-        const int i1 = base + (2 * p + 1) * kThreads + tid;
-        if (i0 < P) out[i0] = make_float2(x0, y0);
-        if (i1 < P) out[i1] = make_float2(x1, y1);
+        const int i1 = i0 + kThreads;
+        if (i0 < P) {
+            red_fixed(acc + 2 * (size_t)i0 + 0, x0, scale);
+            red_fixed(acc + 2 * (size_t)i0 + 1, y0, scale);
+        }
+        if (i1 < P) {
+            red_fixed(acc + 2 * (size_t)i1 + 0, x1, scale);
+            red_fixed(acc + 2 * (size_t)i1 + 1, y1, scale);
+        }
     }
 }
 
 // ------------------------------------------------------------------------------------------------
-// a-5: sum the chunk partials in a fixed order (deterministic), scale by 1/(4 pi mu), store U.
-__global__ void finish_f32(const float2 *__restrict__ part, int P, int n_chunks, double scale,
-                           float2 *__restrict__ U)
+// a-5: fixed point -> float, scale by 1/(4 pi mu), store U.
+__global__ void finish_f32(const long long *__restrict__ acc, int P, const unsigned *__restrict__ gmax_bits,
+                           double prefactor, float2 *__restrict__ U)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= P) return;
-    double sx = 0.0, sy = 0.0;
-    for (int c = 0; c < n_chunks; ++c) {
-        const float2 v = part[(size_t)c * (size_t)P + i];
-        sx += (double)v.x;
-        sy += (double)v.y;
-    }
-    U[i] = make_float2((float)(scale * sx), (float)(scale * sy));
+    const double f = prefactor / fixed_scale(*gmax_bits, P);
+    const longlong2 v = *reinterpret_cast<const longlong2 *>(acc + 2 * (size_t)i);
+    U[i] = make_float2((float)(f * (double)v.x), (float)(f * (double)v.y));
 }
 
 // ------------------------------------------------------------------------------------------------
-constexpr int kNP32 = 4;   // 8 targets per thread
-
 vn_status farfield_f32(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, double mu,
                        void *U, cudaStream_t st)
 {
@@ -231,24 +353,26 @@ vn_status farfield_f32(const void *X, const void *F, const void *W, int64_t nves
         VN_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, farfield_f32_kernel<kNP32>, kThreads, 0));
         slots = sms * (occ > 0 ? occ : 1);
     }
-    const Split sp = choose_split(P, 2 * kNP32 * kThreads, slots, 16);
+    const SymSplit sp = choose_sym_split(P, kST32, slots, 16);
 
-    ulonglong2 *src = nullptr;
-    float2 *part = nullptr;
-    VN_CUDA(cudaMallocAsync((void **)&src, (size_t)P * 32, st));
-    VN_CUDA(cudaMallocAsync((void **)&part, (size_t)P * sizeof(float2) * (size_t)sp.n_chunks, st));
+    // scratch: packed sources | fixed-point accumulators | gmax
+    const size_t b_src = (size_t)P * 32, b_acc = (size_t)P * 16;
+    char *scratch = nullptr;
+    VN_CUDA(cudaMallocAsync((void **)&scratch, b_src + b_acc + 16, st));
+    ulonglong2 *src = (ulonglong2 *)scratch;
+    long long *acc = (long long *)(scratch + b_src);
+    unsigned *gmax = (unsigned *)(scratch + b_src + b_acc);
+    VN_CUDA(cudaMemsetAsync(acc, 0, b_acc + 16, st));
 
-    pack_sources_f32<<<(P + 255) / 256, 256, 0, st>>>((const float2 *)X, (const float2 *)F, (const float *)W, P, src);
+    pack_sources_f32<<<(P + 255) / 256, 256, 0, st>>>((const float2 *)X, (const float2 *)F, (const float *)W, P, src, gmax);
     profile_mark(st, true);
-    farfield_f32_kernel<kNP32><<<sp.n_tb * sp.n_chunks, kThreads, 0, st>>>(src, (const float2 *)X, P, (int)npts,
-                                                                          sp.n_tiles, sp.n_chunks, part);
+    farfield_f32_kernel<kNP32><<<sp.n_st * sp.n_chunks, kThreads, 0, st>>>(src, (const float2 *)X, P, (int)npts,
+                                                                          sp.n_tiles, sp.n_st, sp.n_chunks, gmax, acc);
     profile_mark(st, false);
-    finish_f32<<<(P + 255) / 256, 256, 0, st>>>(part, P, sp.n_chunks, 1.0 / (4.0 * 3.14159265358979323846 * mu),
-                                                 (float2 *)U);
+    finish_f32<<<(P + 255) / 256, 256, 0, st>>>(acc, P, gmax, 1.0 / (4.0 * 3.14159265358979323846 * mu), (float2 *)U);
     count_launch(3);
     const cudaError_t e = cudaGetLastError();
-    VN_CUDA(cudaFreeAsync(src, st));
-    VN_CUDA(cudaFreeAsync(part, st));
+    VN_CUDA(cudaFreeAsync(scratch, st));
     return e == cudaSuccess ? VN_OK : VN_ERR_CUDA;
 }
 
