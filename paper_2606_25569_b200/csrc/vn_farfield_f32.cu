@@ -5,14 +5,15 @@
 //
 // The kernel matrix K(r) = -log|r| I + r r^T/|r|^2 is even in r and symmetric, so the unordered pair
 // {i, j} needs r, |r|^2, 1/|r|^2 and log|r|^2 ONCE and serves both U_i += K g_j and U_j += K g_i.
-// The kernel walks unordered pairs of point tiles and applies every pair in both directions:
-//   per unordered pair:  r = x - y; r2 = rx*rx + ry*ry; l = lg2(r2); inv = 1/r2           (shared)
-//   i <- j:  A_i += l * g_j;  B_i += ((r.g_j) * inv) * r                                     (7 FP32 instr)
-//   j <- i:  A_j += l * g_i;  B_j += ((r.g_i) * inv) * r                                     (7 FP32 instr)
-//   U = 1/(4 pi mu) * ( -(ln 2 / 2) * A + B )
+// The kernel walks unordered pairs of point tiles and applies every pair in both directions.  With
+// KA = -(ln 2)/2 it builds M' = K / KA once per unordered pair,
+//   r = x - y; r2 = rx*rx + ry*ry; inv = 1/(KA r2); l = lg2(r2);  u = r * inv
+//   M'xx = l + ux*rx;  M'xy = ux*ry;  M'yy = l + uy*ry                                 (shared)
+//   i <- j:  U'_i += M' g_j      j <- i:  U'_j += M' g_i                                (4 FP32 instr each)
+//   U = 1/(4 pi mu) * KA * U'
 // Two targets share one packed register (FADD2/FMUL2/FFMA2) and one SFU reciprocal:
-//   t = rcp(a*b), 1/a = t*b, 1/b = t*a   (a, b = the two r2 of the packed pair).
-// Per directed interaction this is 9.75 FP32 lane-instructions and 0.75 SFU ops against the canonical
+//   t = rcp(KA*a*b), 1/(KA a) = t*b, 1/(KA b) = t*a   (a, b = the two r2 of the packed pair).
+// Per directed interaction this is 9.5 FP32 lane-instructions and 0.75 SFU ops against the canonical
 // 11 + 2 of a one-directional sum.
 //
 // Cross-block accumulation goes through 64-bit fixed-point atomics (integer addition is associative, so
@@ -184,9 +185,10 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
         const ulonglong2 *ts = tile[s];
         const bool fast = both && (first >= span_end || first + kTile <= span_begin) && (cnt == kTile);
         if (fast) {
-            u64 Ax[NP], Ay[NP], Bx[NP], By[NP];   // per-tile partial sums (two-level accumulation)
+            // per-tile partial sums (two-level accumulation), in units of -(ln2/2): U' = U / KA
+            u64 Ux[NP], Uy[NP];
 #pragma unroll
-            for (int p = 0; p < NP; ++p) Ax[p] = Ay[p] = Bx[p] = By[p] = 0ull;
+            for (int p = 0; p < NP; ++p) Ux[p] = Uy[p] = 0ull;
             long long *accj = acc + 2 * (size_t)first + (lane >> 1);
 #pragma unroll 1
             for (int jb = 0; jb < kTile; jb += kBatch) {
@@ -195,34 +197,41 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
                 for (int jj = 0; jj < kBatch; ++jj) {
                     const ulonglong2 yy = ts[2 * (jb + jj) + 0];   // (yx,yx) (yy,yy)
                     const ulonglong2 gg = ts[2 * (jb + jj) + 1];   // (gx,gx) (gy,gy)
-                    u64 cAx = 0ull, cAy = 0ull, cBx = 0ull, cBy = 0ull;
+                    u64 rx[NP], ry[NP], l[NP], inv[NP];
 #pragma unroll
                     for (int p = 0; p < NP; ++p) {
-                        const u64 rx = sub2(tx[p], yy.x);
-                        const u64 ry = sub2(ty[p], yy.y);
-                        const u64 r2 = fma2(rx, rx, mul2(ry, ry));
+                        rx[p] = sub2(tx[p], yy.x);
+                        ry[p] = sub2(ty[p], yy.y);
+                        const u64 r2 = fma2(rx[p], rx[p], mul2(ry[p], ry[p]));
                         float a, b;
                         upk(r2, a, b);
-                        const float t = sfu_rcp(a * b);
-                        const u64 inv = pk(t * b, t * a);
-                        const u64 l = pk(sfu_lg2(a), sfu_lg2(b));
-                        // i <- j
-                        Ax[p] = fma2(l, gg.x, Ax[p]);
-                        Ay[p] = fma2(l, gg.y, Ay[p]);
-                        const u64 q = mul2(fma2(rx, gg.x, mul2(ry, gg.y)), inv);
-                        Bx[p] = fma2(q, rx, Bx[p]);
-                        By[p] = fma2(q, ry, By[p]);
-                        // j <- i
-                        cAx = fma2(l, hx[p], cAx);
-                        cAy = fma2(l, hy[p], cAy);
-                        const u64 w = mul2(fma2(rx, hx[p], mul2(ry, hy[p])), inv);
-                        cBx = fma2(w, rx, cBx);
-                        cBy = fma2(w, ry, cBy);
+                        const float t = sfu_rcp((a * b) * -0.34657359027997264f);   // 1/(KA a b)
+                        inv[p] = pk(t * b, t * a);                                   // 1/(KA r2)
+                        l[p] = pk(sfu_lg2(a), sfu_lg2(b));
+                    }
+                    u64 cUx = 0ull, cUy = 0ull;
+#pragma unroll
+                    for (int p = 0; p < NP; ++p) {
+                        // M' = K / KA = lg2(r2) I + r r^T / (KA r2)
+                        const u64 ux = mul2(rx[p], inv[p]);
+                        const u64 uy = mul2(ry[p], inv[p]);
+                        const u64 Mxy = mul2(ux, ry[p]);
+                        const u64 Mxx = fma2(ux, rx[p], l[p]);
+                        const u64 Myy = fma2(uy, ry[p], l[p]);
+                        // one chain through all eight products: neighbours share an operand slot
+                        Ux[p] = fma2(Mxx, gg.x, Ux[p]);
+                        cUx = fma2(Mxx, hx[p], cUx);
+                        cUy = fma2(Mxy, hx[p], cUy);
+                        cUx = fma2(Mxy, hy[p], cUx);
+                        cUy = fma2(Myy, hy[p], cUy);
+                        Uy[p] = fma2(Myy, gg.y, Uy[p]);
+                        Ux[p] = fma2(Mxy, gg.y, Ux[p]);
+                        Uy[p] = fma2(Mxy, gg.x, Uy[p]);
                     }
                     float lo, hi;
-                    upk(fma2(KA, cAx, cBx), lo, hi);
+                    upk(cUx, lo, hi);
                     c[2 * jj + 0] = lo + hi;
-                    upk(fma2(KA, cAy, cBy), lo, hi);
+                    upk(cUy, lo, hi);
                     c[2 * jj + 1] = lo + hi;
                 }
                 // transpose-reduce over the warp: 16 values per lane -> lane L ends with the warp
@@ -238,12 +247,12 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
                     }
                 }
                 c[0] += __shfl_xor_sync(0xffffffffu, c[0], 1);
-                if ((lane & 1) == 0) red_fixed(accj + 2 * jb, c[0], scale);
+                if ((lane & 1) == 0) red_fixed(accj + 2 * jb, c[0] * -0.34657359027997264f, scale);
             }
 #pragma unroll
             for (int p = 0; p < NP; ++p) {
-                Rx[p] = add2(Rx[p], fma2(KA, Ax[p], Bx[p]));
-                Ry[p] = add2(Ry[p], fma2(KA, Ay[p], By[p]));
+                Rx[p] = fma2(KA, Ux[p], Rx[p]);
+                Ry[p] = fma2(KA, Uy[p], Ry[p]);
             }
         } else if (cnt > 0) {
             // predicated path: own-vesicle sources and the ragged tail are skipped per pair
