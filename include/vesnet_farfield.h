@@ -84,9 +84,61 @@ vn_status vn_farfield_host(const void *X, const void *F, const void *W,
                            int64_t nves, int64_t npts, double mu,
                            void *U, vn_precision precision);
 
+/* ---- row f-1: the paper's DirectSingleLayerIntegral with its near-field mask ------------------
+ *
+ * Near-field relation ("A vesicle is considered in the near-field of the point x if
+ * the distance of x to the vesicle is less than or equal to the arclength spacing", :248 |d| <= h,
+ * :426 Alg. 4 line 4 FindNearFieldPoints):
+ *
+ *   near(t, v')  <=>  v' != ves(t)  and  min_j |X[t] - X[v',j]| <= h_v',   h_v' = max_j W[v',j]
+ *
+ * (h = the largest trapezoid weight of the source vesicle, reading N1; the distance to
+ * the membrane is the distance to its nearest discretisation point.)  The decision is taken in
+ * double arithmetic on the stored values for both precisions.  Output is CSR over the P = nves*npts
+ * target points t = v*npts + i, all DEVICE pointers:
+ *   near_ptr[P+1]  int64, near_ptr[0] = 0, near_ptr[P] = number of near (point, vesicle) pairs
+ *   near_ves[...]  int32, for each t the near vesicles v' in ascending order
+ * `capacity` is the number of int32 entries near_ves can hold; entries at positions >= capacity are
+ * not written (near_ptr is always complete, so the caller detects overflow by near_ptr[P] >
+ * capacity and calls again).  near_ves may be NULL with capacity 0: count only. */
+vn_status vn_near_pairs(const void *X, const void *W, int64_t nves, int64_t npts,
+                        int64_t *near_ptr, int32_t *near_ves, int64_t capacity,
+                        vn_precision precision, void *stream);
+
+/* vn_farfield with the contribution of every near vesicle set to zero ("direct
+ * integration with boolean masks to set neighboring vesicles' contribution to zero", :425 Alg. 4
+ * line 3):
+ *
+ *   U[t,:] = 1/(4 pi mu) sum_{v' != ves(t), v' not near t} sum_j K(X[t]-X[v',j]) F[v',j,:] W[v',j]
+ *
+ * near_ptr / near_ves: the CSR relation as written by vn_near_pairs (DEVICE pointers, complete:
+ * near_ptr[P] entries readable in near_ves; near_ves may be NULL only if near_ptr[P] == 0).  Any
+ * relation in that format is accepted (v' == ves(t) entries are a caller error, not checked).
+ * The near contributions are evaluated in double and leave the accumulators before the final
+ * rounding.  Other arguments as vn_farfield. */
+vn_status vn_farfield_masked(const void *X, const void *F, const void *W,
+                             int64_t nves, int64_t npts, double mu,
+                             const int64_t *near_ptr, const int32_t *near_ves,
+                             void *U, vn_precision precision, void *stream);
+
+/* ---- row f-4: free targets ------------------------------------------------------------------
+ * Velocity induced at nt points Xt[nt,2] that lie on no membrane by ALL vesicles (eq 2.8 summed
+ * over every vesicle with the trapezoid rule; the velocity-field
+ * evaluation behind the paper's streamline figures):
+ *
+ *   Ut[q,:] = 1/(4 pi mu) sum_{v'} sum_j K(Xt[q]-X[v',j]) F[v',j,:] W[v',j]
+ *
+ * No vesicle is excluded; a target closer to a membrane than its point spacing gets the plain
+ * trapezoid value (inaccurate there by the nature of the rule).  Xt, Ut: DEVICE
+ * pointers, [nt,2] interleaved, pair-aligned; nt == 0 is valid and does nothing.  Ut overwritten. */
+vn_status vn_farfield_targets(const void *Xt, int64_t nt,
+                              const void *X, const void *F, const void *W,
+                              int64_t nves, int64_t npts, double mu,
+                              void *Ut, vn_precision precision, void *stream);
+
 /* Profiling aid (bench.py's roofline figure): while enabled, every vn_farfield /
- * vn_farfield_host call records a CUDA event pair on its stream around the pair kernel
- * alone (not the pack / finish kernels).  vn_profile_read waits for the recorded events,
+ * vn_farfield_host / vn_farfield_masked / vn_farfield_targets call records a CUDA event pair on its
+ * stream around the pair kernel alone (not the pack / finish / correction kernels).  vn_profile_read waits for the recorded events,
  * writes up to max_entries durations in milliseconds (oldest first) into the HOST array
  * ms, forgets them, and returns how many it wrote (or -1 on a CUDA error). */
 vn_status vn_profile_enable(int enable);

@@ -48,6 +48,9 @@ def _load():
         lib.oracle_weights.argtypes = [d, i64, i64, d, d]
         lib.oracle_near_mask.argtypes = [d, d, i64, i64, u8]
         lib.oracle_farfield_masked.argtypes = [d, d, d, i64, i64, ctypes.c_double, u8, d]
+        lib.oracle_near_mask_subset.argtypes = [d, d, i64, i64, ctypes.POINTER(i64), i64, u8]
+        lib.oracle_farfield_masked_subset.argtypes = [d, d, d, i64, i64, ctypes.c_double,
+                                                      ctypes.POINTER(i64), i64, u8, d]
         _lib = lib
     return _lib
 
@@ -141,3 +144,34 @@ def farfield_masked(X, F, W, near, mu=1.0):
     if rc:
         raise ValueError(f"oracle_farfield_masked rc={rc}")
     return U
+
+
+def near_mask_subset(X, W, idx):
+    """Rows ``idx`` of the near mask -> [len(idx), nves] (uint8)."""
+    X = _c(X); nves, npts, _ = X.shape
+    W = _c(W, (nves, npts))
+    idx = np.ascontiguousarray(idx, dtype=np.int64)
+    near = np.empty((idx.size, nves), dtype=np.uint8)
+    rc = _load().oracle_near_mask_subset(_p(X), _p(W), nves, npts,
+                                         idx.ctypes.data_as(ctypes.POINTER(ctypes.c_int64)), idx.size,
+                                         near.ctypes.data_as(ctypes.POINTER(ctypes.c_ubyte)))
+    if rc:
+        raise ValueError(f"oracle_near_mask_subset rc={rc}")
+    return near
+
+
+def farfield_masked_subset(X, F, W, idx, near_rows, mu=1.0):
+    """Masked direct sum at the flat point indices ``idx``; near_rows: [len(idx), nves]."""
+    X = _c(X); nves, npts, _ = X.shape
+    F = _c(F, X.shape); W = _c(W, (nves, npts))
+    idx = np.ascontiguousarray(idx, dtype=np.int64)
+    near_rows = np.ascontiguousarray(near_rows, dtype=np.uint8)
+    if near_rows.shape != (idx.size, nves):
+        raise ValueError("near_rows shape")
+    Us = np.empty((idx.size, 2), dtype=np.float64)
+    rc = _load().oracle_farfield_masked_subset(_p(X), _p(F), _p(W), nves, npts, float(mu),
+                                               idx.ctypes.data_as(ctypes.POINTER(ctypes.c_int64)), idx.size,
+                                               near_rows.ctypes.data_as(ctypes.POINTER(ctypes.c_ubyte)), _p(Us))
+    if rc:
+        raise ValueError(f"oracle_farfield_masked_subset rc={rc}")
+    return Us

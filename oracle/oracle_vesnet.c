@@ -251,3 +251,60 @@ int oracle_farfield_masked(const double *X, const double *F, const double *W,
     }
     return 0;
 }
+
+/* Rows idx[0..nidx) of the near mask only (same definition; for suspensions whose full
+ * [P, nves] mask would not fit).  near: [nidx, nves] bytes. */
+int oracle_near_mask_subset(const double *X, const double *W, int64_t nves, int64_t npts,
+                            const int64_t *idx, int64_t nidx, unsigned char *near)
+{
+    if (!X || !W || !near || !idx || nves < 1 || npts < 1 || nidx < 0) return 1;
+    const int64_t P = nves * npts;
+    for (int64_t q = 0; q < nidx; ++q)
+        if (idx[q] < 0 || idx[q] >= P) return 1;
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t q = 0; q < nidx; ++q) {
+        const int64_t t = idx[q];
+        const int64_t v = t / npts;
+        for (int64_t vp = 0; vp < nves; ++vp) {
+            unsigned char flag = 0;
+            if (vp != v) {
+                ld h = 0.0L;
+                for (int64_t j = 0; j < npts; ++j)
+                    if ((ld)W[vp * npts + j] > h) h = (ld)W[vp * npts + j];
+                ld dmin2 = INFINITY;
+                for (int64_t j = 0; j < npts; ++j) {
+                    const ld rx = (ld)X[2 * t + 0] - (ld)X[2 * (vp * npts + j) + 0];
+                    const ld ry = (ld)X[2 * t + 1] - (ld)X[2 * (vp * npts + j) + 1];
+                    const ld d2 = rx * rx + ry * ry;
+                    if (d2 < dmin2) dmin2 = d2;
+                }
+                flag = (dmin2 <= h * h) ? 1 : 0;
+            }
+            near[q * nves + vp] = flag;
+        }
+    }
+    return 0;
+}
+
+/* The masked direct sum at the listed targets only; near: [nidx, nves] rows for those targets. */
+int oracle_farfield_masked_subset(const double *X, const double *F, const double *W,
+                                  int64_t nves, int64_t npts, double mu,
+                                  const int64_t *idx, int64_t nidx,
+                                  const unsigned char *near, double *Usub)
+{
+    if (!X || !F || !W || !Usub || !near || !idx || nves < 1 || npts < 1 || !(mu > 0.0)) return 1;
+    const ld scale = 1.0L / (4.0L * ORACLE_PI * (ld)mu);
+    const int64_t P = nves * npts;
+    for (int64_t q = 0; q < nidx; ++q)
+        if (idx[q] < 0 || idx[q] >= P) return 1;
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t q = 0; q < nidx; ++q) {
+        const int64_t t = idx[q];
+        ld ux, uy;
+        farfield_one_target(X, F, W, nves, npts, t / npts,
+                            (ld)X[2 * t + 0], (ld)X[2 * t + 1], near + q * nves, &ux, &uy);
+        Usub[2 * q + 0] = (double)(scale * ux);
+        Usub[2 * q + 1] = (double)(scale * uy);
+    }
+    return 0;
+}

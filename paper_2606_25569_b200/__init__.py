@@ -10,6 +10,9 @@ raises.
     W = vn_arclength_weights(X)                 # X: [nves, npts, 2] cuda tensor, fp32 or fp64
     U = vn_farfield(X, F, W, mu=1.0)            # U: [nves, npts, 2]
     U = vn_farfield_host(X, F, None, mu=1.0)    # host (numpy / pinned torch) buffers, whole path
+    ptr, ves = vn_near_pairs(X, W)              # near-field relation (CSR)
+    U = vn_farfield_masked(X, F, W, ptr, ves)   # the paper's DirectSingleLayerIntegral
+    Ut = vn_farfield_targets(Xt, X, F, W)       # velocity at free points Xt[nt, 2]
 
 `inputs` (seeded synthetic suspensions) is importable without the library.
 """
@@ -48,6 +51,12 @@ def lib():
         L.vn_arclength_weights.restype = ci
         L.vn_farfield_host.argtypes = [vp, vp, vp, i64, i64, dbl, vp, ci]
         L.vn_farfield_host.restype = ci
+        L.vn_near_pairs.argtypes = [vp, vp, i64, i64, vp, vp, i64, ci, vp]
+        L.vn_near_pairs.restype = ci
+        L.vn_farfield_masked.argtypes = [vp, vp, vp, i64, i64, dbl, vp, vp, vp, ci, vp]
+        L.vn_farfield_masked.restype = ci
+        L.vn_farfield_targets.argtypes = [vp, i64, vp, vp, vp, i64, i64, dbl, vp, ci, vp]
+        L.vn_farfield_targets.restype = ci
         L.vn_profile_enable.argtypes = [ci]
         L.vn_profile_enable.restype = ci
         L.vn_profile_read.argtypes = [ctypes.POINTER(dbl), i64]
@@ -122,6 +131,82 @@ def vn_arclength_weights(X, out=None, stream=None):
         rc = lib().vn_arclength_weights(X.data_ptr(), nves, npts, out.data_ptr(), _prec(X), _stream_ptr(stream))
     if rc != VN_OK:
         raise VesnetError(rc, "vn_arclength_weights")
+    return out
+
+
+def vn_near_pairs(X, W, near_ptr=None, near_ves=None, stream=None):
+    """Near-field relation in CSR form (device tensors).  With near_ves=None the binding makes the
+    count-only call, reads near_ptr[P] (one host synchronisation), allocates near_ves of exactly
+    that size and calls again; pass both tensors to stay asynchronous.  Returns (near_ptr, near_ves)."""
+    import torch
+    nves, npts, two = X.shape
+    if two != 2:
+        raise ValueError("X must be [nves, npts, 2]")
+    _check_dev("X", X)
+    _check_dev("W", W, (nves, npts), X.dtype)
+    P = nves * npts
+    if near_ptr is None:
+        near_ptr = torch.empty(P + 1, dtype=torch.int64, device=X.device)
+    _check_dev("near_ptr", near_ptr, (P + 1,), torch.int64)
+    L = lib()
+    with torch.cuda.device(X.device):
+        if near_ves is None:
+            rc = L.vn_near_pairs(X.data_ptr(), W.data_ptr(), nves, npts, near_ptr.data_ptr(), None, 0,
+                                 _prec(X), _stream_ptr(stream))
+            if rc != VN_OK:
+                raise VesnetError(rc, "vn_near_pairs")
+            near_ves = torch.empty(int(near_ptr[P].item()), dtype=torch.int32, device=X.device)
+        _check_dev("near_ves", near_ves, None, torch.int32)
+        if near_ves.numel() > 0:
+            rc = L.vn_near_pairs(X.data_ptr(), W.data_ptr(), nves, npts, near_ptr.data_ptr(), near_ves.data_ptr(),
+                                 near_ves.numel(), _prec(X), _stream_ptr(stream))
+            if rc != VN_OK:
+                raise VesnetError(rc, "vn_near_pairs")
+    return near_ptr, near_ves
+
+
+def vn_farfield_masked(X, F, W, near_ptr, near_ves, mu: float = 1.0, out=None, stream=None):
+    """The paper's DirectSingleLayerIntegral: vn_farfield with the near vesicles' contribution zeroed."""
+    import torch
+    nves, npts, two = X.shape
+    if two != 2:
+        raise ValueError("X must be [nves, npts, 2]")
+    _check_dev("X", X)
+    _check_dev("F", F, X.shape, X.dtype)
+    _check_dev("W", W, (nves, npts), X.dtype)
+    _check_dev("near_ptr", near_ptr, (nves * npts + 1,), torch.int64)
+    _check_dev("near_ves", near_ves, None, torch.int32)
+    if out is None:
+        out = torch.empty_like(X)
+    _check_dev("out", out, X.shape, X.dtype)
+    with torch.cuda.device(X.device):
+        rc = lib().vn_farfield_masked(X.data_ptr(), F.data_ptr(), W.data_ptr(), nves, npts, float(mu),
+                                      near_ptr.data_ptr(), near_ves.data_ptr() if near_ves.numel() else None,
+                                      out.data_ptr(), _prec(X), _stream_ptr(stream))
+    if rc != VN_OK:
+        raise VesnetError(rc, "vn_farfield_masked")
+    return out
+
+
+def vn_farfield_targets(Xt, X, F, W, mu: float = 1.0, out=None, stream=None):
+    """Velocity at free points Xt[nt, 2] induced by all vesicles (device tensors)."""
+    import torch
+    nves, npts, two = X.shape
+    if two != 2 or Xt.dim() != 2 or Xt.shape[1] != 2:
+        raise ValueError("X must be [nves, npts, 2] and Xt [nt, 2]")
+    _check_dev("X", X)
+    _check_dev("F", F, X.shape, X.dtype)
+    _check_dev("W", W, (nves, npts), X.dtype)
+    _check_dev("Xt", Xt, None, X.dtype)
+    if out is None:
+        out = torch.empty_like(Xt)
+    _check_dev("out", out, Xt.shape, X.dtype)
+    with torch.cuda.device(X.device):
+        rc = lib().vn_farfield_targets(Xt.data_ptr() if Xt.numel() else None, Xt.shape[0], X.data_ptr(), F.data_ptr(),
+                                       W.data_ptr(), nves, npts, float(mu),
+                                       out.data_ptr() if Xt.numel() else None, _prec(X), _stream_ptr(stream))
+    if rc != VN_OK:
+        raise VesnetError(rc, "vn_farfield_targets")
     return out
 
 

@@ -28,19 +28,25 @@ void profile_mark(cudaStream_t st, bool begin)
 }
 
 vn_status farfield_f32(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, double mu,
-                       void *U, cudaStream_t st);
+                       void *U, cudaStream_t st, const int64_t *near_ptr, const int32_t *near_ves);
 vn_status farfield_f64(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, double mu,
-                       void *U, cudaStream_t st);
+                       void *U, cudaStream_t st, const int64_t *near_ptr, const int32_t *near_ves);
+vn_status farfield_targets_f32(const void *Xt, int64_t nt, const void *X, const void *F, const void *W,
+                               int64_t nves, int64_t npts, double mu, void *Ut, cudaStream_t st);
+vn_status farfield_targets_f64(const void *Xt, int64_t nt, const void *X, const void *F, const void *W,
+                               int64_t nves, int64_t npts, double mu, void *Ut, cudaStream_t st);
+vn_status near_pairs(const void *X, const void *W, int64_t nves, int64_t npts, int64_t *near_ptr,
+                     int32_t *near_ves, int64_t capacity, vn_precision prec, cudaStream_t st);
 vn_status arclength_weights(const void *X, int64_t nves, int64_t npts, void *W, vn_precision prec, cudaStream_t st);
 
-Split choose_split(long long P, int targets_per_block, int slots, int min_tiles)
+Split choose_split_for(int n_tb, int n_tiles, int slots, int min_tiles)
 {
     Split sp;
-    sp.n_tb = (int)((P + targets_per_block - 1) / targets_per_block);
-    sp.n_tiles = (int)((P + kTile - 1) / kTile);
+    sp.n_tb = n_tb;
+    sp.n_tiles = n_tiles;
     int max_chunks = sp.n_tiles / min_tiles;
     if (max_chunks < 1) max_chunks = 1;
-    if (max_chunks > 32) max_chunks = 32;      // bounds the partial-sum scratch to 32 * P results
+    if (max_chunks > 32) max_chunks = 32;
     double best = -1.0;
     sp.n_chunks = 1;
     for (int c = 1; c <= max_chunks; ++c) {
@@ -126,8 +132,62 @@ vn_status vn_farfield(const void *X, const void *F, const void *W, int64_t nves,
     const vn_status ds = check_device();
     if (ds != VN_OK) return ds;
     cudaStream_t st = (cudaStream_t)stream;
-    return precision == VN_F32 ? farfield_f32(X, F, W, nves, npts, mu, U, st)
-                               : farfield_f64(X, F, W, nves, npts, mu, U, st);
+    return precision == VN_F32 ? farfield_f32(X, F, W, nves, npts, mu, U, st, nullptr, nullptr)
+                               : farfield_f64(X, F, W, nves, npts, mu, U, st, nullptr, nullptr);
+}
+
+vn_status vn_near_pairs(const void *X, const void *W, int64_t nves, int64_t npts, int64_t *near_ptr,
+                        int32_t *near_ves, int64_t capacity, vn_precision precision, void *stream)
+{
+    if (!X || !W || !near_ptr) return VN_ERR_INVALID_ARG;
+    if (check_shape(nves, npts, precision) != VN_OK) return VN_ERR_INVALID_ARG;
+    if (capacity < 0 || (capacity > 0 && !near_ves)) return VN_ERR_INVALID_ARG;
+    const size_t pair = precision == VN_F32 ? 8 : 16;
+    if (misaligned(X, pair) || misaligned(W, pair / 2) || misaligned(near_ptr, 8) || misaligned(near_ves, 4))
+        return VN_ERR_INVALID_ARG;
+    const vn_status ds = check_device();
+    if (ds != VN_OK) return ds;
+    return near_pairs(X, W, nves, npts, near_ptr, near_ves, capacity, precision, (cudaStream_t)stream);
+}
+
+vn_status vn_farfield_masked(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, double mu,
+                             const int64_t *near_ptr, const int32_t *near_ves, void *U, vn_precision precision,
+                             void *stream)
+{
+    if (!X || !F || !W || !U || !near_ptr) return VN_ERR_INVALID_ARG;
+    if (check_shape(nves, npts, precision) != VN_OK) return VN_ERR_INVALID_ARG;
+    if (!isfinite(mu) || !(mu > 0.0)) return VN_ERR_INVALID_ARG;
+    const size_t pair = precision == VN_F32 ? 8 : 16;
+    if (misaligned(X, pair) || misaligned(F, pair) || misaligned(U, pair) || misaligned(W, pair / 2) ||
+        misaligned(near_ptr, 8) || misaligned(near_ves, 4))
+        return VN_ERR_INVALID_ARG;
+    if (U == X || U == F || U == W) return VN_ERR_INVALID_ARG;
+    const vn_status ds = check_device();
+    if (ds != VN_OK) return ds;
+    cudaStream_t st = (cudaStream_t)stream;
+    return precision == VN_F32 ? farfield_f32(X, F, W, nves, npts, mu, U, st, near_ptr, near_ves)
+                               : farfield_f64(X, F, W, nves, npts, mu, U, st, near_ptr, near_ves);
+}
+
+vn_status vn_farfield_targets(const void *Xt, int64_t nt, const void *X, const void *F, const void *W,
+                              int64_t nves, int64_t npts, double mu, void *Ut, vn_precision precision, void *stream)
+{
+    if (!X || !F || !W) return VN_ERR_INVALID_ARG;
+    if (check_shape(nves, npts, precision) != VN_OK) return VN_ERR_INVALID_ARG;
+    if (nt < 0 || nt >= (1ll << 31)) return VN_ERR_INVALID_ARG;
+    if (!isfinite(mu) || !(mu > 0.0)) return VN_ERR_INVALID_ARG;
+    if (nt == 0) return VN_OK;
+    if (!Xt || !Ut) return VN_ERR_INVALID_ARG;
+    const size_t pair = precision == VN_F32 ? 8 : 16;
+    if (misaligned(X, pair) || misaligned(F, pair) || misaligned(Xt, pair) || misaligned(Ut, pair) ||
+        misaligned(W, pair / 2))
+        return VN_ERR_INVALID_ARG;
+    if (Ut == X || Ut == F || Ut == W || Ut == Xt) return VN_ERR_INVALID_ARG;
+    const vn_status ds = check_device();
+    if (ds != VN_OK) return ds;
+    cudaStream_t st = (cudaStream_t)stream;
+    return precision == VN_F32 ? farfield_targets_f32(Xt, nt, X, F, W, nves, npts, mu, Ut, st)
+                               : farfield_targets_f64(Xt, nt, X, F, W, nves, npts, mu, Ut, st);
 }
 
 vn_status vn_arclength_weights(const void *X, int64_t nves, int64_t npts, void *W, vn_precision precision,
@@ -180,8 +240,8 @@ vn_status vn_farfield_host(const void *X, const void *F, const void *W, int64_t 
         rc = arclength_weights(dX, nves, npts, dW, precision, st);
         if (rc != VN_OK) return rc;
     }
-    rc = precision == VN_F32 ? farfield_f32(dX, dF, dW, nves, npts, mu, dU, st)
-                             : farfield_f64(dX, dF, dW, nves, npts, mu, dU, st);
+    rc = precision == VN_F32 ? farfield_f32(dX, dF, dW, nves, npts, mu, dU, st, nullptr, nullptr)
+                             : farfield_f64(dX, dF, dW, nves, npts, mu, dU, st, nullptr, nullptr);
     if (rc != VN_OK) return rc;
     VN_CUDA(cudaMemcpyAsync(U, dU, bX, cudaMemcpyDeviceToHost, st));
     VN_CUDA(cudaStreamSynchronize(st));
@@ -227,6 +287,6 @@ const char *vn_status_string(vn_status s)
     return "unknown status";
 }
 
-int vn_version(void) { return 100; }
+int vn_version(void) { return 200; }
 
 }  // extern "C"

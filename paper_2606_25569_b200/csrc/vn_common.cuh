@@ -46,7 +46,7 @@ struct Split {
 
 // Choose the number of source chunks so that the grid fills `slots` resident blocks in whole
 // waves (wave quantisation) while each chunk keeps >= min_tiles tiles.
-Split choose_split(long long P, int targets_per_block, int slots, int min_tiles);
+Split choose_split_for(int n_tb, int n_tiles, int slots, int min_tiles);
 
 // Symmetric (both-direction) decomposition of the fp32 kernel: block = (super-tile I, chunk c of I's
 // source-tile list); see vn_farfield_f32.cu.
@@ -103,6 +103,80 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
                  "l"(src), "r"(bytes), "r"(smem_u32(bar))
                  : "memory");
 }
+
+// ---------------------------------------------------------------------------------------------
+// 64-bit fixed-point accumulation of fp32 results across blocks (bitwise reproducible).
+// Power-of-two scale of the fixed-point accumulators.  gmax = max_j (|g_jx| + |g_jy|).  Every term of
+// the sum is bounded by (|ln2/2 * lg2 r2| + 1) |g_j| <= 64 gmax (|lg2| <= 150 over all positive fp32),
+// so every partial sum of any subset is below bnd = 64 P gmax; 2^(61-e) with 2^e <= bnd < 2^(e+1)
+// keeps |value * scale| < 2^62.
+__device__ __forceinline__ double fixed_scale(unsigned gmax_bits, int P)
+{
+    const float gmax = __uint_as_float(gmax_bits);
+    if (!(gmax > 0.f) || !(gmax <= 3.4028234e38f)) return 1.0;   // all-zero (or non-finite) density
+    const double bnd = 64.0 * (double)P * (double)gmax;
+    const int e = ((__double2hiint(bnd) >> 20) & 0x7ff) - 1023;
+    return __hiloint2double((1023 + 61 - e) << 20, 0);
+}
+
+__device__ __forceinline__ void red_fixed(long long *addr, float v, double scale)
+{
+    const long long q = __double2ll_rn((double)v * scale);
+    atomicAdd((unsigned long long *)addr, (unsigned long long)q);
+}
+
+// fp64 results: two 64-bit words per value.  The high word counts units of 1/s_hi (s_hi as above, with
+// the term bound 512 gmax because |ln r2|/2 <= 355 over all positive doubles), the low word counts
+// units of 2^-40/s_hi and receives the EXACT remainder v - hi/s_hi (an fma), rounded to that unit.
+// A contribution therefore enters with an absolute error <= 2^-102 of the bound -- far below double
+// rounding of the sum -- and, integer addition being associative, the total is bitwise reproducible.
+// The remainder is below 2^39 units per contribution, so 2^23 contributions cannot overflow the low word.
+struct Fixed2 {
+    double s_hi, inv_s_hi, s_lo;
+};
+__device__ __forceinline__ Fixed2 fixed2_scale(unsigned long long gmax_bits, int P)
+{
+    const double gmax = __longlong_as_double((long long)gmax_bits);
+    Fixed2 f;
+    int ex = 1023 + 61;
+    if (gmax > 0.0 && gmax <= 1.0e300) {
+        const double bnd = 512.0 * (double)P * gmax;
+        ex = 1023 + 61 - (((__double2hiint(bnd) >> 20) & 0x7ff) - 1023);
+        ex = ex < 1 ? 1 : (ex > 2000 ? 2000 : ex);
+    }
+    f.s_hi = __hiloint2double(ex << 20, 0);
+    f.inv_s_hi = __hiloint2double((2046 - ex) << 20, 0);
+    f.s_lo = __hiloint2double((ex + 40) << 20, 0);
+    return f;
+}
+// which = 0: the high word of v, which = 1: the low word
+__device__ __forceinline__ long long fixed2_word(double v, const Fixed2 &f, int which)
+{
+    const long long qh = __double2ll_rn(v * f.s_hi);
+    if (which == 0) return qh;
+    const double rem = fma(-(double)qh, f.inv_s_hi, v);
+    return __double2ll_rn(rem * f.s_lo);
+}
+__device__ __forceinline__ void red_fixed2(long long *addr, double v, const Fixed2 &f)   // addr[0] hi, addr[1] lo
+{
+    atomicAdd((unsigned long long *)addr + 0, (unsigned long long)fixed2_word(v, f, 0));
+    atomicAdd((unsigned long long *)addr + 1, (unsigned long long)fixed2_word(v, f, 1));
+}
+__device__ __forceinline__ double fixed2_value(long long hi, long long lo, const Fixed2 &f)
+{
+    const long long carry = lo >> 40;               // move whole high units out of the low word
+    hi += carry;
+    lo -= carry << 40;
+    return (double)hi * f.inv_s_hi + ((double)lo * f.inv_s_hi) * 9.094947017729282379e-13;   // 2^-40
+}
+
+// near-field correction (vn_near.cu), used by the masked variants of both precisions: subtracts the
+// near vesicles' contributions from the fixed-point accumulators before the final rounding
+vn_status near_correction_f32(const void *X, const void *F, const void *W, int P, int npts, const int64_t *near_ptr,
+                              const int32_t *near_ves, long long *acc, const unsigned *gmax_bits, cudaStream_t st);
+vn_status near_correction_f64(const void *X, const void *F, const void *W, int P, int npts, const int64_t *near_ptr,
+                              const int32_t *near_ves, long long *acc, const unsigned long long *gmax_bits,
+                              cudaStream_t st);
 
 // ---------------------------------------------------------------------------------------------
 // packed fp32 pairs (sm_100 FADD2 / FMUL2 / FFMA2) and single-instruction SFU ops

@@ -27,25 +27,6 @@ constexpr int kST32 = 2 * kNP32 * kThreads;       // points per super-tile (targ
 constexpr int kSub32 = kST32 / kTile;             // source tiles per super-tile: 8
 constexpr int kBatch = 8;                         // sources per cross-lane reduction batch
 
-// Power-of-two scale of the fixed-point accumulators.  gmax = max_j (|g_jx| + |g_jy|).  Every term of
-// the sum is bounded by (|ln2/2 * lg2 r2| + 1) |g_j| <= 64 gmax (|lg2| <= 150 over all positive fp32),
-// so every partial sum of any subset is below bnd = 64 P gmax; 2^(61-e) with 2^e <= bnd < 2^(e+1)
-// keeps |value * scale| < 2^62.
-__device__ __forceinline__ double fixed_scale(unsigned gmax_bits, int P)
-{
-    const float gmax = __uint_as_float(gmax_bits);
-    if (!(gmax > 0.f) || !(gmax <= 3.4028234e38f)) return 1.0;   // all-zero (or non-finite) density
-    const double bnd = 64.0 * (double)P * (double)gmax;
-    const int e = ((__double2hiint(bnd) >> 20) & 0x7ff) - 1023;
-    return __hiloint2double((1023 + 61 - e) << 20, 0);
-}
-
-__device__ __forceinline__ void red_fixed(long long *addr, float v, double scale)
-{
-    const long long q = __double2ll_rn((double)v * scale);
-    atomicAdd((unsigned long long *)addr, (unsigned long long)q);
-}
-
 // ------------------------------------------------------------------------------------------------
 // a-2: g = F*W, packed with the position into one 32-byte record per source, every value
 // duplicated so that one LDS.128 yields ready-made packed operands (yx,yx | yy,yy) and (gx,gx | gy,gy).
@@ -339,11 +320,11 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
 
 // ------------------------------------------------------------------------------------------------
 // a-5: fixed point -> float, scale by 1/(4 pi mu), store U.
-__global__ void finish_f32(const long long *__restrict__ acc, int P, const unsigned *__restrict__ gmax_bits,
+__global__ void finish_f32(const long long *__restrict__ acc, int n, int P, const unsigned *__restrict__ gmax_bits,
                            double prefactor, float2 *__restrict__ U)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= P) return;
+    if (i >= n) return;
     const double f = prefactor / fixed_scale(*gmax_bits, P);
     const longlong2 v = *reinterpret_cast<const longlong2 *>(acc + 2 * (size_t)i);
     U[i] = make_float2((float)(f * (double)v.x), (float)(f * (double)v.y));
@@ -351,7 +332,7 @@ __global__ void finish_f32(const long long *__restrict__ acc, int P, const unsig
 
 // ------------------------------------------------------------------------------------------------
 vn_status farfield_f32(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, double mu,
-                       void *U, cudaStream_t st)
+                       void *U, cudaStream_t st, const int64_t *near_ptr, const int32_t *near_ves)
 {
     const int P = (int)(nves * npts);
     static int slots = 0;
@@ -378,7 +359,173 @@ vn_status farfield_f32(const void *X, const void *F, const void *W, int64_t nves
     farfield_f32_kernel<kNP32><<<sp.n_st * sp.n_chunks, kThreads, 0, st>>>(src, (const float2 *)X, P, (int)npts,
                                                                           sp.n_tiles, sp.n_st, sp.n_chunks, gmax, acc);
     profile_mark(st, false);
-    finish_f32<<<(P + 255) / 256, 256, 0, st>>>(acc, P, gmax, 1.0 / (4.0 * 3.14159265358979323846 * mu), (float2 *)U);
+    if (near_ptr) {   // row f-1: take the near vesicles' contributions out again before the final rounding
+        const vn_status rc = near_correction_f32(X, F, W, P, (int)npts, near_ptr, near_ves, acc, gmax, st);
+        if (rc != VN_OK) { (void)cudaFreeAsync(scratch, st); return rc; }
+    }
+    finish_f32<<<(P + 255) / 256, 256, 0, st>>>(acc, P, P, gmax, 1.0 / (4.0 * 3.14159265358979323846 * mu), (float2 *)U);
+    count_launch(3);
+    const cudaError_t e = cudaGetLastError();
+    VN_CUDA(cudaFreeAsync(scratch, st));
+    return e == cudaSuccess ? VN_OK : VN_ERR_CUDA;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Row f-4: free targets.  Velocity induced at nt points that lie on no membrane by ALL vesicles
+// (eq 2.8 summed over every vesicle, trapezoid rule; the velocity-field
+// evaluation behind the streamline plots).  Targets and sources are different sets, so
+// there is no symmetry to use: one-directional sum, per pair
+//   r = x - y; r2 = rx*rx + ry*ry; A += lg2(r2) * g; d = rx*gx + ry*gy; B += (d / r2) * r
+// (2 FADD + 3 FMUL + 6 FFMA + 1.5 MUFU with the shared reciprocal), 8 targets per thread as packed
+// pairs, the same tile ring, per-tile partial sums folded into running sums, fixed-point atomics out.
+template <int NP>
+__global__ void __launch_bounds__(kThreads, 4)
+targets_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict__ Xt, int nt_pts, int P,
+                   int n_tiles, int n_chunks, const unsigned *__restrict__ gmax_bits, long long *__restrict__ acc)
+{
+    constexpr int T = 2 * NP;
+    __shared__ __align__(128) ulonglong2 tile[kStages][kTile * 2];
+    __shared__ __align__(8) u64 full_bar[kStages];
+    __shared__ __align__(8) u64 empty_bar[kStages];
+
+    const int tid = threadIdx.x;
+    const int tb = blockIdx.x / n_chunks;
+    const int sc = blockIdx.x - tb * n_chunks;
+    const int t_begin = chunk_tile_begin(n_tiles, n_chunks, sc);
+    const int nt = chunk_tile_begin(n_tiles, n_chunks, sc + 1) - t_begin;
+
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < kStages; ++s) {
+            mbar_init(&full_bar[s], 1);
+            mbar_init(&empty_bar[s], kThreads / 32);
+        }
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    auto issue = [&](int i) {
+        const int s = i % kStages;
+        const int first = (t_begin + i) * kTile;
+        const uint32_t bytes = (uint32_t)min(kTile, P - first) * 32u;
+        mbar_expect_tx(&full_bar[s], bytes);
+        bulk_g2s(&tile[s][0], src + 2 * (size_t)first, bytes, &full_bar[s]);
+    };
+    if (tid == 0) {
+        const int pre = nt < kStages ? nt : kStages;
+        for (int i = 0; i < pre; ++i) issue(i);
+    }
+
+    const int base = tb * (T * kThreads);
+    u64 tx[NP], ty[NP], Rx[NP], Ry[NP];
+#pragma unroll
+    for (int p = 0; p < NP; ++p) {
+        const float2 a = Xt[min(base + (2 * p) * kThreads + tid, nt_pts - 1)];
+        const float2 b = Xt[min(base + (2 * p + 1) * kThreads + tid, nt_pts - 1)];
+        tx[p] = pk(a.x, b.x);
+        ty[p] = pk(a.y, b.y);
+        Rx[p] = Ry[p] = 0ull;
+    }
+    const u64 KA = pk(-0.34657359027997264f, -0.34657359027997264f);   // -(ln 2)/2
+
+    for (int i = 0; i < nt; ++i) {
+        const int s = i % kStages;
+        if (tid == 0 && i >= 1 && i - 1 + kStages < nt) {
+            mbar_wait(&empty_bar[(i - 1) % kStages], ((i - 1) / kStages) & 1);
+            issue(i - 1 + kStages);
+        }
+        mbar_wait(&full_bar[s], (i / kStages) & 1);
+
+        const int cnt = min(kTile, P - (t_begin + i) * kTile);
+        const ulonglong2 *ts = tile[s];
+        u64 Ax[NP], Ay[NP], Bx[NP], By[NP];   // per-tile partial sums (two-level accumulation)
+#pragma unroll
+        for (int p = 0; p < NP; ++p) Ax[p] = Ay[p] = Bx[p] = By[p] = 0ull;
+        auto pair = [&](int j) {
+            const ulonglong2 yy = ts[2 * j + 0];   // (yx,yx) (yy,yy)
+            const ulonglong2 gg = ts[2 * j + 1];   // (gx,gx) (gy,gy)
+#pragma unroll
+            for (int p = 0; p < NP; ++p) {
+                const u64 rx = sub2(tx[p], yy.x);
+                const u64 ry = sub2(ty[p], yy.y);
+                const u64 r2 = fma2(rx, rx, mul2(ry, ry));
+                float a, b;
+                upk(r2, a, b);
+                const float t = sfu_rcp(a * b);
+                const u64 inv = pk(t * b, t * a);
+                const u64 l = pk(sfu_lg2(a), sfu_lg2(b));
+                Ax[p] = fma2(l, gg.x, Ax[p]);
+                Ay[p] = fma2(l, gg.y, Ay[p]);
+                const u64 d = fma2(rx, gg.x, mul2(ry, gg.y));
+                const u64 q = mul2(d, inv);
+                Bx[p] = fma2(q, rx, Bx[p]);
+                By[p] = fma2(q, ry, By[p]);
+            }
+        };
+        if (cnt == kTile) {
+#pragma unroll 2
+            for (int j = 0; j < kTile; ++j) pair(j);
+        } else {
+#pragma unroll 1
+            for (int j = 0; j < cnt; ++j) pair(j);
+        }
+#pragma unroll
+        for (int p = 0; p < NP; ++p) {
+            Rx[p] = add2(Rx[p], fma2(KA, Ax[p], Bx[p]));
+            Ry[p] = add2(Ry[p], fma2(KA, Ay[p], By[p]));
+        }
+        __syncwarp();
+        if ((tid & 31) == 0) mbar_arrive(&empty_bar[s]);
+    }
+
+    const double scale = fixed_scale(*gmax_bits, P);
+#pragma unroll
+    for (int p = 0; p < NP; ++p) {
+        float x0, x1, y0, y1;
+        upk(Rx[p], x0, x1);
+        upk(Ry[p], y0, y1);
+        const int i0 = base + (2 * p) * kThreads + tid;
+        const int i1 = i0 + kThreads;
+        if (i0 < nt_pts) {
+            red_fixed(acc + 2 * (size_t)i0 + 0, x0, scale);
+            red_fixed(acc + 2 * (size_t)i0 + 1, y0, scale);
+        }
+        if (i1 < nt_pts) {
+            red_fixed(acc + 2 * (size_t)i1 + 0, x1, scale);
+            red_fixed(acc + 2 * (size_t)i1 + 1, y1, scale);
+        }
+    }
+}
+
+vn_status farfield_targets_f32(const void *Xt, int64_t nt, const void *X, const void *F, const void *W,
+                               int64_t nves, int64_t npts, double mu, void *Ut, cudaStream_t st)
+{
+    const int P = (int)(nves * npts), n = (int)nt;
+    static int slots = 0;
+    if (slots == 0) {
+        int dev = 0, sms = 0, occ = 0;
+        VN_CUDA(cudaGetDevice(&dev));
+        VN_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+        VN_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, targets_f32_kernel<kNP32>, kThreads, 0));
+        slots = sms * (occ > 0 ? occ : 1);
+    }
+    // target blocks come from the free targets, chunks from the sources
+    const Split sp = choose_split_for((n + kST32 - 1) / kST32, (P + kTile - 1) / kTile, slots, 16);
+
+    const size_t b_src = (size_t)P * 32, b_acc = (size_t)n * 16;
+    char *scratch = nullptr;
+    VN_CUDA(cudaMallocAsync((void **)&scratch, b_src + b_acc + 16, st));
+    ulonglong2 *src = (ulonglong2 *)scratch;
+    long long *acc = (long long *)(scratch + b_src);
+    unsigned *gmax = (unsigned *)(scratch + b_src + b_acc);
+    VN_CUDA(cudaMemsetAsync(acc, 0, b_acc + 16, st));
+
+    pack_sources_f32<<<(P + 255) / 256, 256, 0, st>>>((const float2 *)X, (const float2 *)F, (const float *)W, P, src, gmax);
+    profile_mark(st, true);
+    targets_f32_kernel<kNP32><<<sp.n_tb * sp.n_chunks, kThreads, 0, st>>>(src, (const float2 *)Xt, n, P, sp.n_tiles,
+                                                                         sp.n_chunks, gmax, acc);
+    profile_mark(st, false);
+    finish_f32<<<(n + 255) / 256, 256, 0, st>>>(acc, n, P, gmax, 1.0 / (4.0 * 3.14159265358979323846 * mu), (float2 *)Ut);
     count_launch(3);
     const cudaError_t e = cudaGetLastError();
     VN_CUDA(cudaFreeAsync(scratch, st));

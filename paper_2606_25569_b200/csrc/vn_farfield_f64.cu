@@ -1,76 +1,346 @@
-// vn_farfield_f64.cu -- fp64 far-field Stokeslet sum for sm_100a (parity-grade variant).
+// vn_farfield_f64.cu -- fp64 far-field Stokeslet sum for sm_100a (parity-grade variant, steps a-2 .. a-5).
 //
-// Same decomposition as the fp32 kernel (vn_farfield_f32.cu): block = (target block, source chunk),
-// source tiles through a ring of shared-memory stages filled by bulk async copies, own-vesicle
-// tiles on a predicated path.  Arithmetic is plain double: per pair
-//   r = x - y; r2 = rx*rx + ry*ry; acc += -(1/2) log(r2) * g + ((r.g)/r2) * r
-// (eqs 2.8/2.9).  There is no SFU log/rcp in double; see pair_f64().
+//   U_i = 1/(4 pi mu) sum_{j not in ves(i)} [ -log|r| g_j + (r.g_j)/|r|^2 r ],  r = x_i - y_j, g_j = f_j w_j
+//   (PAPER.md:129-136 eqs 2.8/2.9, :173 trapezoid rule, :425 DirectSingleLayerIntegral)
+//
+// Same decomposition as the fp32 kernel (vn_farfield_f32.cu): K(r) = -log|r| I + r r^T/|r|^2 is even
+// and symmetric, so every unordered pair of points is evaluated once,
+//   r = x - y; r2 = rx*rx + ry*ry; ml = -(1/2) ln r2; inv = 1/r2; u = r * inv
+//   Kxx = ml + ux*rx;  Kxy = ux*ry;  Kyy = ml + uy*ry
+// and applied in both directions, U_i += K g_j and U_j += K g_i: 28 DP instructions per unordered pair
+// (14 per directed interaction) instead of about 36 per directed pair of a one-directional sum.
+// The FP64 pipe (64 lanes/clk/SM) is the bound, so the instruction count is what matters: there is no
+// SFU log or reciprocal in double, see log_rcp_f64().
+// Cross-block accumulation goes through 2 x 64-bit fixed-point atomics per value (Fixed2 in
+// vn_common.cuh): exact to 2^-102 of the term bound and bitwise reproducible.
 #include "vn_common.cuh"
 
 namespace vn {
 
-constexpr int kT64 = 4;   // targets per thread
+constexpr int kT64 = 4;                       // targets per thread
+constexpr int kST64 = kT64 * kThreads;        // points per super-tile (target block): 512
+constexpr int kSub64 = kST64 / kTile;         // source tiles per super-tile: 4
+constexpr int kBatch64 = 4;                   // sources per cross-lane reduction batch
+constexpr int kLogTab = 513;                  // (1/2) ln(rc) for the 9-bit reciprocals rc in [1/2, 1]
 
-// a-2: one 32-byte record (yx, yy, gx, gy) per source, g = F*W.
+// a-2: one 32-byte record (yx, yy, gx, gy) per source, g = F*W; also gmax = max_j (|gx| + |gy|)
+// (the bit pattern of a non-negative double orders like the double).
 __global__ void pack_sources_f64(const double2 *__restrict__ X, const double2 *__restrict__ F,
-                                 const double *__restrict__ W, int P, double4 *__restrict__ src)
+                                 const double *__restrict__ W, int P, double4 *__restrict__ src,
+                                 unsigned long long *__restrict__ gmax_bits)
 {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= P) return;
-    const double2 y = X[s];
-    const double2 f = F[s];
-    const double w = W[s];
-    src[s] = make_double4(y.x, y.y, f.x * w, f.y * w);
+    double m = 0.0;
+    if (s < P) {
+        const double2 y = X[s];
+        const double2 f = F[s];
+        const double w = W[s];
+        const double gx = f.x * w, gy = f.y * w;
+        src[s] = make_double4(y.x, y.y, gx, gy);
+        m = fabs(gx) + fabs(gy);
+        if (!(m <= 1.7976931348623157e308)) m = __longlong_as_double(0x7ff0000000000000ll);   // NaN / Inf -> +Inf
+    }
+#pragma unroll
+    for (int k = 16; k >= 1; k >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, k));
+    if ((threadIdx.x & 31) == 0 && m != 0.0) atomicMax(gmax_bits, (unsigned long long)__double_as_longlong(m));
 }
 
-// -(1/2) log(r2) and 1/r2 in double.  One reciprocal serves both: with r2 = m * 2^e, m in
-// [sqrt(1/2), sqrt(2)), s = (m-1)/(m+1) and log m = 2 atanh(s); 1/(m (m+1)) gives 1/m and 1/(m+1)
-// (same trick as the packed fp32 pair).  Series error < 2e-17 for |s| <= 0.1716.
-__device__ __forceinline__ void log_rcp_f64(double r2, double &mhalf_log, double &inv)
+// -(1/2) ln(r2) and 1/r2 in double, 11 DP instructions + one MUFU.RCP64H + one I2F + one 8-byte
+// shared-memory load.  r2 = m 2^e with m in [1, 2).
+//   t0  = hardware reciprocal seed of m (about 20 bits);  1/m = t0 (1 + d + d^2), d = 1 - m t0  (cubic step)
+//   rc  = t0 rounded to 9 mantissa bits, eps = m rc - 1 (one fma; |eps| <= 2^-10 + 2^-19)
+//   ln m = -ln rc + log1p(eps),  log1p by its series through eps^5 (next term <= 2e-19)
+//   tab[k] = (1/2) ln(rc_k), rc_k = 1/2 + k/1024 (k = 0 .. 512), built by every block at start-up
+// r2 must be a positive normal double whose reciprocal is normal too (the header's precondition).
+__device__ __forceinline__ void log_rcp_f64(double r2, const double *__restrict__ tab, double &mhalf_log, double &inv)
 {
-    int hi = __double2hiint(r2);
+    const int hi = __double2hiint(r2);
     const int lo = __double2loint(r2);
-    int e = (hi >> 20) - 1023;                      // r2 is a positive normal number (precondition)
-    hi = (hi & 0x000fffff) | 0x3ff00000;            // mantissa in [1, 2)
-    if (hi >= 0x3ff6a09f) { hi -= 0x00100000; e += 1; }   // -> [sqrt(1/2), sqrt(2))
-    const double m = __hiloint2double(hi, lo);
-    const double mp1 = m + 1.0;
-    const double prod = m * mp1;
-    // reciprocal of prod: hardware seed + two Newton steps
-    double t;
-    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(t) : "d"(prod));
-    t = fma(fma(-prod, t, 1.0), t, t);
-    t = fma(fma(-prod, t, 1.0), t, t);
-    t = fma(fma(-prod, t, 1.0), t, t);
-    const double inv_m = t * mp1;                   // 1/m
-    const double s = (m - 1.0) * (t * m);           // (m-1)/(m+1)
-    const double z = s * s;
-    // atanh(s)/s = 1 + z/3 + z^2/5 + ... + z^10/21
-    double p = 1.0 / 21.0;
-    p = fma(p, z, 1.0 / 19.0);
-    p = fma(p, z, 1.0 / 17.0);
-    p = fma(p, z, 1.0 / 15.0);
-    p = fma(p, z, 1.0 / 13.0);
-    p = fma(p, z, 1.0 / 11.0);
-    p = fma(p, z, 1.0 / 9.0);
-    p = fma(p, z, 1.0 / 7.0);
-    p = fma(p, z, 1.0 / 5.0);
-    p = fma(p, z, 1.0 / 3.0);
-    p = fma(p, z, 1.0);
-    // -(1/2) log(r2) = -(1/2) e ln2 - s p
-    mhalf_log = fma((double)e, -0.34657359027997265471, -(s * p));
-    // 1/r2 = 2^-e / m
-    inv = __hiloint2double(__double2hiint(inv_m) - (e << 20), __double2loint(inv_m));
+    const int e = (hi >> 20) - 1023;
+    const double m = __hiloint2double((hi & 0x000fffff) | 0x3ff00000, lo);
+    double t0;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(t0) : "d"(m));                 // MUFU.RCP64H: 1/m in (1/2, 1]
+    const int rch = (__double2hiint(t0) + 0x400) & 0xfffff800;              // round to 9 mantissa bits
+    const double rc = __hiloint2double(rch, 0);
+    const double half_ln_rc = tab[(rch - 0x3fe00000) >> 11];
+    // reciprocal
+    const double d = fma(-m, t0, 1.0);
+    const double p = fma(d, d, d);
+    const double t = fma(t0, p, t0);
+    inv = __hiloint2double(__double2hiint(t) - (e << 20), __double2loint(t));   // 2^-e / m
+    // logarithm: -(1/2) ln r2 = -(1/2) e ln2 + (1/2) ln rc - (1/2) log1p(eps)
+    const double eps = fma(m, rc, -1.0);
+    const double z = eps * eps;
+    double q = -0.1;                                   // -(1/2) (-1/2 + eps/3 - eps^2/4 + eps^3/5)
+    q = fma(q, eps, 0.125);
+    q = fma(q, eps, -1.0 / 6.0);
+    q = fma(q, eps, 0.25);
+    const double base = fma((double)e, -0.34657359027997265471, half_ln_rc);
+    mhalf_log = fma(eps, -0.5, fma(z, q, base));
 }
 
+// a-3 / a-4: pair kernel; block (I, c) = super-tile I as targets x chunk c of I's list of source tiles
+// (own super-tile one-directional with the own vesicle predicated out, then the tiles of super-tiles
+// I+1 .. I+S_I in both directions) -- the same walk as farfield_f32_kernel.
 __global__ void __launch_bounds__(kThreads, 4)
 farfield_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__ X, int P, int npts,
-                    int n_tiles, int n_chunks, double2 *__restrict__ part)
+                    int n_tiles, int n_st, int n_chunks, const unsigned long long *__restrict__ gmax_bits,
+                    long long *__restrict__ acc)
+{
+    constexpr int T = kT64;
+    constexpr int B = kBatch64;
+    constexpr int kDup = 32 / (2 * B);              // lanes that end up with the same reduced value
+    __shared__ __align__(128) double4 tile[kStages][kTile];
+    __shared__ __align__(8) u64 full_bar[kStages];
+    __shared__ __align__(8) u64 empty_bar[kStages];
+    __shared__ double tab[kLogTab];
+
+    const int tid = threadIdx.x;
+    const int lane = tid & 31;
+    const int I = blockIdx.x / n_chunks;
+    const int sc = blockIdx.x - I * n_chunks;
+    int S = (n_st - 1) / 2;
+    if ((n_st & 1) == 0 && I < n_st / 2) S += 1;
+    const int nu = kSub64 * (S + 1);
+    const int u_begin = chunk_tile_begin(nu, n_chunks, sc);
+    const int nt = chunk_tile_begin(nu, n_chunks, sc + 1) - u_begin;
+
+    auto tile_of = [&](int u) {        // source tile index of list entry u (may be >= n_tiles: empty)
+        const int s = u / kSub64;
+        int J = I + s;
+        if (J >= n_st) J -= n_st;
+        return J * kSub64 + (u - s * kSub64);
+    };
+
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < kStages; ++s) {
+            mbar_init(&full_bar[s], 1);
+            mbar_init(&empty_bar[s], kThreads / 32);
+        }
+        mbar_fence_init();
+    }
+    for (int k = tid; k < kLogTab; k += kThreads) tab[k] = 0.5 * log(0.5 + (double)k * (1.0 / 1024.0));
+    __syncthreads();
+
+    auto issue = [&](int i) {   // one thread: list entry u_begin + i -> stage i % kStages
+        const int s = i % kStages;
+        const int first = tile_of(u_begin + i) * kTile;
+        const int cnt = min(kTile, P - first);
+        if (cnt > 0) {
+            const uint32_t bytes = (uint32_t)cnt * 32u;
+            mbar_expect_tx(&full_bar[s], bytes);
+            bulk_g2s(&tile[s][0], src + first, bytes, &full_bar[s]);
+        } else {
+            mbar_arrive(&full_bar[s]);      // empty entry: complete the phase without a copy
+        }
+    };
+    if (tid == 0) {
+        const int pre = nt < kStages ? nt : kStages;
+        for (int i = 0; i < pre; ++i) issue(i);
+    }
+
+    const Fixed2 fx = fixed2_scale(*gmax_bits, P);
+
+    // targets: point base + k*kThreads + tid; indices past the end are clamped to P-1 and carry a zero
+    // density (their results are never stored, their contributions to others vanish).
+    const int base = I * kST64;
+    double tx[T], ty[T], hx[T], hy[T], Ux[T], Uy[T];
+#pragma unroll
+    for (int k = 0; k < T; ++k) {
+        const int i0 = base + k * kThreads + tid;
+        const double4 a = src[min(i0, P - 1)];
+        tx[k] = a.x;
+        ty[k] = a.y;
+        hx[k] = i0 < P ? a.z : 0.0;
+        hy[k] = i0 < P ? a.w : 0.0;
+        Ux[k] = Uy[k] = 0.0;
+    }
+    const int last_target = min(base + T * kThreads, P) - 1;
+    const int span_begin = (base / npts) * npts;
+    const int span_end = (last_target / npts + 1) * npts;
+
+    for (int i = 0; i < nt; ++i) {
+        const int s = i % kStages;
+        if (tid == 0 && i >= 1 && i - 1 + kStages < nt) {   // refill the stage drained last iteration
+            mbar_wait(&empty_bar[(i - 1) % kStages], ((i - 1) / kStages) & 1);
+            issue(i - 1 + kStages);
+        }
+        mbar_wait(&full_bar[s], (i / kStages) & 1);
+
+        const int u = u_begin + i;
+        const bool both = u >= kSub64;                    // another super-tile: both directions
+        const int first = tile_of(u) * kTile;
+        const int cnt = min(kTile, P - first);
+        const double4 *ts = tile[s];
+        const bool fast = both && (first >= span_end || first + kTile <= span_begin) && (cnt == kTile);
+        if (fast) {
+            // lane L ends a batch holding the warp total of value L / kDup (value = 2*source + component);
+            // sub-lane 0 adds its high word, sub-lane 1 its low word
+            long long *accj = acc + 4 * (size_t)first + 2 * (lane / kDup) + (lane % kDup);
+#pragma unroll 1
+            for (int jb = 0; jb < kTile; jb += B) {
+                double c[2 * B];
+#pragma unroll
+                for (int jj = 0; jj < B; ++jj) {
+                    const double4 sj = ts[jb + jj];
+                    double cx = 0.0, cy = 0.0;
+#pragma unroll
+                    for (int k = 0; k < T; ++k) {
+                        const double rx = tx[k] - sj.x, ry = ty[k] - sj.y;
+                        const double r2 = fma(rx, rx, ry * ry);
+                        double ml, inv;
+                        log_rcp_f64(r2, tab, ml, inv);
+                        const double ux = rx * inv, uy = ry * inv;
+                        const double Kxy = ux * ry;
+                        const double Kxx = fma(ux, rx, ml);
+                        const double Kyy = fma(uy, ry, ml);
+                        Ux[k] = fma(Kxx, sj.z, fma(Kxy, sj.w, Ux[k]));
+                        Uy[k] = fma(Kxy, sj.z, fma(Kyy, sj.w, Uy[k]));
+                        cx = fma(Kxx, hx[k], fma(Kxy, hy[k], cx));
+                        cy = fma(Kxy, hx[k], fma(Kyy, hy[k], cy));
+                    }
+                    c[2 * jj + 0] = cx;
+                    c[2 * jj + 1] = cy;
+                }
+                // transpose-reduce over the warp: 2B values per lane -> one warp total per lane
+                int m = 16;
+#pragma unroll
+                for (int w = B; w >= 1; w >>= 1, m >>= 1) {
+                    const bool up = (lane & m) != 0;
+#pragma unroll
+                    for (int k = 0; k < w; ++k) {
+                        const double send = up ? c[k] : c[k + w];
+                        const double keep = up ? c[k + w] : c[k];
+                        c[k] = keep + __shfl_xor_sync(0xffffffffu, send, m);
+                    }
+                }
+#pragma unroll
+                for (; m >= 1; m >>= 1) c[0] += __shfl_xor_sync(0xffffffffu, c[0], m);
+                if ((lane % kDup) < 2)
+                    atomicAdd((unsigned long long *)(accj + 4 * jb),
+                              (unsigned long long)fixed2_word(c[0], fx, lane % kDup));
+            }
+        } else if (cnt > 0) {
+            // predicated path: own-vesicle sources and the ragged tail are skipped per pair
+            int own[T];
+#pragma unroll
+            for (int k = 0; k < T; ++k) own[k] = (min(base + k * kThreads + tid, P - 1) / npts) * npts;
+#pragma unroll 1
+            for (int j = 0; j < cnt; ++j) {
+                const double4 sj = ts[j];
+                const int jg = first + j;
+                double cx = 0.0, cy = 0.0;
+#pragma unroll
+                for (int k = 0; k < T; ++k) {
+                    if ((unsigned)(jg - own[k]) >= (unsigned)npts) {
+                        const double rx = tx[k] - sj.x, ry = ty[k] - sj.y;
+                        const double r2 = fma(rx, rx, ry * ry);
+                        double ml, inv;
+                        log_rcp_f64(r2, tab, ml, inv);
+                        const double ux = rx * inv, uy = ry * inv;
+                        const double Kxy = ux * ry;
+                        const double Kxx = fma(ux, rx, ml);
+                        const double Kyy = fma(uy, ry, ml);
+                        Ux[k] = fma(Kxx, sj.z, fma(Kxy, sj.w, Ux[k]));
+                        Uy[k] = fma(Kxy, sj.z, fma(Kyy, sj.w, Uy[k]));
+                        cx = fma(Kxx, hx[k], fma(Kxy, hy[k], cx));
+                        cy = fma(Kxy, hx[k], fma(Kyy, hy[k], cy));
+                    }
+                }
+                if (both) {
+#pragma unroll
+                    for (int m = 16; m >= 1; m >>= 1) {
+                        cx += __shfl_xor_sync(0xffffffffu, cx, m);
+                        cy += __shfl_xor_sync(0xffffffffu, cy, m);
+                    }
+                    if (lane < 4) {   // lanes 0..3: x hi, x lo, y hi, y lo
+                        const double v = (lane & 2) ? cy : cx;
+                        atomicAdd((unsigned long long *)(acc + 4 * (size_t)jg + lane),
+                                  (unsigned long long)fixed2_word(v, fx, lane & 1));
+                    }
+                }
+            }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty_bar[s]);
+    }
+
+    // this block's sums for its own targets
+#pragma unroll
+    for (int k = 0; k < T; ++k) {
+        const int i0 = base + k * kThreads + tid;
+        if (i0 < P) {
+            red_fixed2(acc + 4 * (size_t)i0 + 0, Ux[k], fx);
+            red_fixed2(acc + 4 * (size_t)i0 + 2, Uy[k], fx);
+        }
+    }
+}
+
+// a-5: fixed point -> double, scale by 1/(4 pi mu), store U.
+__global__ void finish_f64(const long long *__restrict__ acc, int n, int P, const unsigned long long *__restrict__ gmax_bits,
+                           double prefactor, double2 *__restrict__ U)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const Fixed2 fx = fixed2_scale(*gmax_bits, P);
+    const longlong2 a = *reinterpret_cast<const longlong2 *>(acc + 4 * (size_t)i);
+    const longlong2 b = *reinterpret_cast<const longlong2 *>(acc + 4 * (size_t)i + 2);
+    U[i] = make_double2(prefactor * fixed2_value(a.x, a.y, fx), prefactor * fixed2_value(b.x, b.y, fx));
+}
+
+vn_status farfield_f64(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, double mu,
+                       void *U, cudaStream_t st, const int64_t *near_ptr, const int32_t *near_ves)
+{
+    const int P = (int)(nves * npts);
+    static int slots = 0;
+    if (slots == 0) {
+        int dev = 0, sms = 0, occ = 0;
+        VN_CUDA(cudaGetDevice(&dev));
+        VN_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+        VN_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, farfield_f64_kernel, kThreads, 0));
+        slots = sms * (occ > 0 ? occ : 1);
+    }
+    const SymSplit sp = choose_sym_split(P, kST64, slots, 8);
+
+    // scratch: packed sources | fixed-point accumulators (hi, lo per component) | gmax
+    const size_t b_src = (size_t)P * 32, b_acc = (size_t)P * 32;
+    char *scratch = nullptr;
+    VN_CUDA(cudaMallocAsync((void **)&scratch, b_src + b_acc + 16, st));
+    double4 *src = (double4 *)scratch;
+    long long *acc = (long long *)(scratch + b_src);
+    unsigned long long *gmax = (unsigned long long *)(scratch + b_src + b_acc);
+    VN_CUDA(cudaMemsetAsync(acc, 0, b_acc + 16, st));
+
+    pack_sources_f64<<<(P + 255) / 256, 256, 0, st>>>((const double2 *)X, (const double2 *)F, (const double *)W, P, src, gmax);
+    profile_mark(st, true);
+    farfield_f64_kernel<<<sp.n_st * sp.n_chunks, kThreads, 0, st>>>(src, (const double2 *)X, P, (int)npts, sp.n_tiles,
+                                                                   sp.n_st, sp.n_chunks, gmax, acc);
+    profile_mark(st, false);
+    if (near_ptr) {   // row f-1: take the near vesicles' contributions out again before the final rounding
+        const vn_status rc = near_correction_f64(X, F, W, P, (int)npts, near_ptr, near_ves, acc, gmax, st);
+        if (rc != VN_OK) { (void)cudaFreeAsync(scratch, st); return rc; }
+    }
+    finish_f64<<<(P + 255) / 256, 256, 0, st>>>(acc, P, P, gmax, 1.0 / (4.0 * 3.14159265358979323846 * mu), (double2 *)U);
+    count_launch(3);
+    const cudaError_t e = cudaGetLastError();
+    VN_CUDA(cudaFreeAsync(scratch, st));
+    return e == cudaSuccess ? VN_OK : VN_ERR_CUDA;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Row f-4: free targets in double (see targets_f32_kernel): one-directional sum over ALL vesicles,
+// 4 targets per thread, per pair  acc += ml * g + ((r.g) inv) * r  (22 DP instructions).
+__global__ void __launch_bounds__(kThreads, 4)
+targets_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__ Xt, int nt_pts, int P,
+                   int n_tiles, int n_chunks, const unsigned long long *__restrict__ gmax_bits,
+                   long long *__restrict__ acc)
 {
     constexpr int T = kT64;
     __shared__ __align__(128) double4 tile[kStages][kTile];
     __shared__ __align__(8) u64 full_bar[kStages];
     __shared__ __align__(8) u64 empty_bar[kStages];
+    __shared__ double tab[kLogTab];
 
     const int tid = threadIdx.x;
     const int tb = blockIdx.x / n_chunks;
@@ -86,13 +356,13 @@ farfield_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__
         }
         mbar_fence_init();
     }
+    for (int k = tid; k < kLogTab; k += kThreads) tab[k] = 0.5 * log(0.5 + (double)k * (1.0 / 1024.0));
     __syncthreads();
 
     auto issue = [&](int i) {
         const int s = i % kStages;
         const int first = (t_begin + i) * kTile;
-        const int cnt = min(kTile, P - first);
-        const uint32_t bytes = (uint32_t)cnt * 32u;
+        const uint32_t bytes = (uint32_t)min(kTile, P - first) * 32u;
         mbar_expect_tx(&full_bar[s], bytes);
         bulk_g2s(&tile[s][0], src + first, bytes, &full_bar[s]);
     };
@@ -105,14 +375,11 @@ farfield_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__
     double tx[T], ty[T], ux[T], uy[T];
 #pragma unroll
     for (int k = 0; k < T; ++k) {
-        const double2 a = X[min(base + k * kThreads + tid, P - 1)];
+        const double2 a = Xt[min(base + k * kThreads + tid, nt_pts - 1)];
         tx[k] = a.x;
         ty[k] = a.y;
         ux[k] = uy[k] = 0.0;
     }
-    const int last_target = min(base + T * kThreads, P) - 1;
-    const int span_begin = (base / npts) * npts;
-    const int span_end = (last_target / npts + 1) * npts;
 
     for (int i = 0; i < nt; ++i) {
         const int s = i % kStages;
@@ -121,109 +388,68 @@ farfield_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__
             issue(i - 1 + kStages);
         }
         mbar_wait(&full_bar[s], (i / kStages) & 1);
-
-        const int first = (t_begin + i) * kTile;
+        const int cnt = min(kTile, P - (t_begin + i) * kTile);
         const double4 *ts = tile[s];
-        const bool fast = (first >= span_end || first + kTile <= span_begin) && (first + kTile <= P);
-        if (fast) {
-            double px[T], py[T];
-#pragma unroll
-            for (int k = 0; k < T; ++k) px[k] = py[k] = 0.0;
 #pragma unroll 2
-            for (int j = 0; j < kTile; ++j) {
-                const double4 sj = ts[j];
-#pragma unroll
-                for (int k = 0; k < T; ++k) {
-                    const double rx = tx[k] - sj.x, ry = ty[k] - sj.y;
-                    const double r2 = fma(rx, rx, ry * ry);
-                    double ml, inv;
-                    log_rcp_f64(r2, ml, inv);
-                    const double q = fma(rx, sj.z, ry * sj.w) * inv;
-                    px[k] = fma(ml, sj.z, fma(q, rx, px[k]));
-                    py[k] = fma(ml, sj.w, fma(q, ry, py[k]));
-                }
-            }
-#pragma unroll
-            for (int k = 0; k < T; ++k) { ux[k] += px[k]; uy[k] += py[k]; }
-        } else {
-            const int cnt = min(kTile, P - first);
+        for (int j = 0; j < cnt; ++j) {
+            const double4 sj = ts[j];
 #pragma unroll
             for (int k = 0; k < T; ++k) {
-                const int own = (min(base + k * kThreads + tid, P - 1) / npts) * npts;
-                double px = 0.0, py = 0.0;
-#pragma unroll 1
-                for (int j = 0; j < cnt; ++j) {
-                    const double4 sj = ts[j];
-                    const double rx = tx[k] - sj.x, ry = ty[k] - sj.y;
-                    const double r2 = fma(rx, rx, ry * ry);
-                    if ((unsigned)(first + j - own) >= (unsigned)npts) {
-                        double ml, inv;
-                        log_rcp_f64(r2, ml, inv);
-                        const double q = fma(rx, sj.z, ry * sj.w) * inv;
-                        px = fma(ml, sj.z, fma(q, rx, px));
-                        py = fma(ml, sj.w, fma(q, ry, py));
-                    }
-                }
-                ux[k] += px;
-                uy[k] += py;
+                const double rx = tx[k] - sj.x, ry = ty[k] - sj.y;
+                const double r2 = fma(rx, rx, ry * ry);
+                double ml, inv;
+                log_rcp_f64(r2, tab, ml, inv);
+                const double q = fma(rx, sj.z, ry * sj.w) * inv;
+                ux[k] = fma(ml, sj.z, fma(q, rx, ux[k]));
+                uy[k] = fma(ml, sj.w, fma(q, ry, uy[k]));
             }
         }
         __syncwarp();
         if ((tid & 31) == 0) mbar_arrive(&empty_bar[s]);
     }
 
-    double2 *out = part + (size_t)sc * (size_t)P;
+    const Fixed2 fx = fixed2_scale(*gmax_bits, P);
 #pragma unroll
     for (int k = 0; k < T; ++k) {
         const int i0 = base + k * kThreads + tid;
-        if (i0 < P) out[i0] = make_double2(ux[k], uy[k]);
+        if (i0 < nt_pts) {
+            red_fixed2(acc + 4 * (size_t)i0 + 0, ux[k], fx);
+            red_fixed2(acc + 4 * (size_t)i0 + 2, uy[k], fx);
+        }
     }
 }
 
-__global__ void finish_f64(const double2 *__restrict__ part, int P, int n_chunks, double scale,
-                           double2 *__restrict__ U)
+vn_status farfield_targets_f64(const void *Xt, int64_t nt, const void *X, const void *F, const void *W,
+                               int64_t nves, int64_t npts, double mu, void *Ut, cudaStream_t st)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= P) return;
-    double sx = 0.0, sy = 0.0;
-    for (int c = 0; c < n_chunks; ++c) {
-        const double2 v = part[(size_t)c * (size_t)P + i];
-        sx += v.x;
-        sy += v.y;
-    }
-    U[i] = make_double2(scale * sx, scale * sy);
-}
-
-vn_status farfield_f64(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, double mu,
-                       void *U, cudaStream_t st)
-{
-    const int P = (int)(nves * npts);
+    const int P = (int)(nves * npts), n = (int)nt;
     static int slots = 0;
     if (slots == 0) {
         int dev = 0, sms = 0, occ = 0;
         VN_CUDA(cudaGetDevice(&dev));
         VN_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-        VN_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, farfield_f64_kernel, kThreads, 0));
+        VN_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, targets_f64_kernel, kThreads, 0));
         slots = sms * (occ > 0 ? occ : 1);
     }
-    const Split sp = choose_split(P, kT64 * kThreads, slots, 8);
+    const Split sp = choose_split_for((n + kST64 - 1) / kST64, (P + kTile - 1) / kTile, slots, 8);
 
-    double4 *src = nullptr;
-    double2 *part = nullptr;
-    VN_CUDA(cudaMallocAsync((void **)&src, (size_t)P * sizeof(double4), st));
-    VN_CUDA(cudaMallocAsync((void **)&part, (size_t)P * sizeof(double2) * (size_t)sp.n_chunks, st));
+    const size_t b_src = (size_t)P * 32, b_acc = (size_t)n * 32;
+    char *scratch = nullptr;
+    VN_CUDA(cudaMallocAsync((void **)&scratch, b_src + b_acc + 16, st));
+    double4 *src = (double4 *)scratch;
+    long long *acc = (long long *)(scratch + b_src);
+    unsigned long long *gmax = (unsigned long long *)(scratch + b_src + b_acc);
+    VN_CUDA(cudaMemsetAsync(acc, 0, b_acc + 16, st));
 
-    pack_sources_f64<<<(P + 255) / 256, 256, 0, st>>>((const double2 *)X, (const double2 *)F, (const double *)W, P, src);
+    pack_sources_f64<<<(P + 255) / 256, 256, 0, st>>>((const double2 *)X, (const double2 *)F, (const double *)W, P, src, gmax);
     profile_mark(st, true);
-    farfield_f64_kernel<<<sp.n_tb * sp.n_chunks, kThreads, 0, st>>>(src, (const double2 *)X, P, (int)npts, sp.n_tiles,
-                                                                   sp.n_chunks, part);
+    targets_f64_kernel<<<sp.n_tb * sp.n_chunks, kThreads, 0, st>>>(src, (const double2 *)Xt, n, P, sp.n_tiles,
+                                                                  sp.n_chunks, gmax, acc);
     profile_mark(st, false);
-    finish_f64<<<(P + 255) / 256, 256, 0, st>>>(part, P, sp.n_chunks, 1.0 / (4.0 * 3.14159265358979323846 * mu),
-                                                 (double2 *)U);
+    finish_f64<<<(n + 255) / 256, 256, 0, st>>>(acc, n, P, gmax, 1.0 / (4.0 * 3.14159265358979323846 * mu), (double2 *)Ut);
     count_launch(3);
     const cudaError_t e = cudaGetLastError();
-    VN_CUDA(cudaFreeAsync(src, st));
-    VN_CUDA(cudaFreeAsync(part, st));
+    VN_CUDA(cudaFreeAsync(scratch, st));
     return e == cudaSuccess ? VN_OK : VN_ERR_CUDA;
 }
 

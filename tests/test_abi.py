@@ -21,7 +21,8 @@ def test_library_exports_every_declared_symbol():
     L = vn.lib()
     names = _declared()
     assert {"vn_farfield", "vn_arclength_weights", "vn_farfield_host", "vn_status_string",
-            "vn_version", "vn_launch_count"} <= set(names)
+            "vn_version", "vn_launch_count", "vn_near_pairs", "vn_farfield_masked",
+            "vn_farfield_targets"} <= set(names)
     for n in names:
         assert hasattr(L, n), n
     assert vn.vn_version() >= 100
@@ -45,5 +46,17 @@ def test_argument_validation_needs_no_gpu():
     assert L.vn_farfield(p, p, p, 2, 4, 1.0, p, vn.VN_F64, None) == INV             # U aliases X
     assert L.vn_arclength_weights(None, 2, 4, q, vn.VN_F64, None) == INV
     assert L.vn_arclength_weights(p, 2, -1, q, vn.VN_F64, None) == INV
+    # NEXT rows
+    assert L.vn_near_pairs(p, None, 2, 4, q, None, 0, vn.VN_F64, None) == INV          # null W
+    assert L.vn_near_pairs(p, p, 2, 4, None, None, 0, vn.VN_F64, None) == INV          # null near_ptr
+    assert L.vn_near_pairs(p, p, 2, 4, q, None, 5, vn.VN_F64, None) == INV             # capacity without buffer
+    assert L.vn_near_pairs(p, p, 2, 4, q, q, -1, vn.VN_F64, None) == INV               # negative capacity
+    assert L.vn_near_pairs(p, p, 2, 4, q + 4, None, 0, vn.VN_F64, None) == INV         # misaligned near_ptr
+    assert L.vn_farfield_masked(p, p, p, 2, 4, 1.0, None, None, q, vn.VN_F64, None) == INV
+    assert L.vn_farfield_masked(p, p, p, 2, 4, -2.0, q, None, q, vn.VN_F64, None) == INV
+    assert L.vn_farfield_targets(None, 3, p, p, p, 2, 4, 1.0, q, vn.VN_F64, None) == INV
+    assert L.vn_farfield_targets(q, -1, p, p, p, 2, 4, 1.0, q, vn.VN_F64, None) == INV
+    assert L.vn_farfield_targets(q, 3, p, p, p, 2, 4, 1.0, q, vn.VN_F64, None) == INV   # Ut aliases Xt
+    assert L.vn_farfield_targets(None, 0, p, p, p, 2, 4, 1.0, None, vn.VN_F64, None) == vn.VN_OK   # nt == 0: nothing to do
     assert L.vn_farfield_host(p, None, None, 2, 4, 1.0, q, vn.VN_F64) == INV
     assert L.vn_farfield_host(p, p, None, 2, 4, -1.0, q, vn.VN_F64) == INV

@@ -1,0 +1,303 @@
+"""Parity of the NEXT rows (DESIGN.md f-1 near-field mask variant, f-4 free targets) with the oracle
+(run on the B200 box: pytest -m gpu).  Every call goes through the C-ABI library via the binding.
+
+Index work (the near relation) must match the oracle exactly; the decision d^2 <= h^2 is taken in
+double by the kernel and in long double by the oracle on the same stored values, and every test
+checks that no pair sits within 1e-9 (relative) of the threshold, so that the comparison is
+meaningful.  Floating point: rel-L2 <= 1e-12 (fp64), <= 2e-5 (fp32) as for vn_farfield."""
+import numpy as np
+import pytest
+
+import oracle
+import paper_2606_25569_b200 as vn
+from paper_2606_25569_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+TOL = {np.float64: 1e-12, np.float32: 2e-5}
+_cache = {}
+
+
+def rel_l2(a, b):
+    a = np.asarray(a, dtype=np.float64).ravel()
+    b = np.asarray(b, dtype=np.float64).ravel()
+    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+def dev(a, dtype):
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=dtype)).cuda()
+
+
+def stored(a, dtype):
+    """What the GPU sees, promoted to double."""
+    return np.asarray(a, dtype=dtype).astype(np.float64)
+
+
+def crowded(index, shrink):
+    """Config `index` with the vesicle centres pulled together by `shrink` (shapes unchanged): gaps
+    fall below the arclength spacing, so many points get near vesicles."""
+    key = (index, shrink)
+    if key not in _cache:
+        s = inputs.config(index)
+        c = s.X.mean(1, keepdims=True)
+        X = (s.X - c) + c * shrink
+        _cache[key] = (X, s.F, oracle.weights(X), s.mu)
+    return _cache[key]
+
+
+def three_circles(npts=16):
+    """Three unit circles on a triangle of side 2.05: points facing the middle are near TWO vesicles."""
+    al = 2 * np.pi * np.arange(npts) / npts
+    body = np.stack([np.cos(al), np.sin(al)], -1)
+    cen = np.array([[0.0, 0.0], [2.05, 0.0], [1.025, 1.7753]])
+    X = body[None] + cen[:, None, :]
+    rng = np.random.Generator(np.random.PCG64(77))
+    F = rng.normal(size=X.shape)
+    return X, F, oracle.weights(X), 0.9
+
+
+def csr_to_dense(ptr, ves, nves):
+    P = len(ptr) - 1
+    dense = np.zeros((P, nves), dtype=np.uint8)
+    rows = np.repeat(np.arange(P), np.diff(ptr))
+    dense[rows, ves] = 1
+    return dense
+
+
+def margin_ok(X, W, near_rows, idx):
+    """No (target, vesicle) pair within 1e-9 relative of the threshold d^2 = h^2."""
+    nves, npts, _ = X.shape
+    P = X.reshape(-1, 2)
+    h2 = W.max(1) ** 2
+    for q, t in enumerate(idx):
+        cand = np.flatnonzero(near_rows[q])
+        for vp in cand:
+            d2 = ((P[t] - X[vp]) ** 2).sum(1).min()
+            if abs(d2 - h2[vp]) <= 1e-9 * h2[vp]:
+                return False
+    return True
+
+
+def gpu_near(X, W, dtype):
+    ptr, ves = vn.vn_near_pairs(dev(X, dtype), dev(W, dtype))
+    torch.cuda.synchronize()
+    return ptr.cpu().numpy(), ves.cpu().numpy()
+
+
+# ------------------------------------------------------------------------------------- near relation (index work: exact)
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+@pytest.mark.parametrize("case", ["three_circles", "config0", "config1", "crowded1"])
+def test_near_pairs_exact(case, dtype):
+    if case == "three_circles":
+        X, F, W, mu = three_circles()
+    elif case == "config0":
+        s = inputs.config(0); X, W = s.X, oracle.weights(s.X)
+    elif case == "config1":
+        s = inputs.config(1); X, W = s.X, oracle.weights(s.X)
+    else:
+        X, F, W, mu = crowded(1, 0.94)
+    Xo, Wo = stored(X, dtype), stored(W, dtype)
+    ref = oracle.near_mask(Xo, Wo)
+    nves, npts, _ = X.shape
+    assert margin_ok(Xo, Wo, ref, np.arange(nves * npts))
+    ptr, ves = gpu_near(X, W, dtype)
+    assert ptr[0] == 0 and ptr[-1] == len(ves) == ref.sum() and np.all(np.diff(ptr) >= 0)
+    got = csr_to_dense(ptr, ves, nves)
+    assert np.array_equal(got, ref)
+    for t in np.flatnonzero(np.diff(ptr) > 1):                 # ascending vesicle order inside a row
+        assert np.all(np.diff(ves[ptr[t]:ptr[t + 1]]) > 0)
+    if case == "three_circles":
+        assert np.diff(ptr).max() == 2
+    if case == "crowded1":
+        assert ref.sum() > 300
+    print(f"{case} {np.dtype(dtype).name}: {ref.sum()} near pairs")
+
+
+def test_near_pairs_capacity_and_count_only():
+    X, F, W, mu = crowded(1, 0.94)
+    Xd, Wd = dev(X, np.float64), dev(W, np.float64)
+    P = X.shape[0] * X.shape[1]
+    ptr_full, ves_full = vn.vn_near_pairs(Xd, Wd)
+    n = ves_full.numel()
+    # a too-small buffer: the pointer array is still complete, only the first `capacity` entries are written
+    small = torch.full((n + 16,), -7, dtype=torch.int32, device="cuda")
+    ptr = torch.empty(P + 1, dtype=torch.int64, device="cuda")
+    rc = vn.lib().vn_near_pairs(Xd.data_ptr(), Wd.data_ptr(), X.shape[0], X.shape[1], ptr.data_ptr(),
+                                small.data_ptr(), n // 2, vn.VN_F64, None)
+    torch.cuda.synchronize()
+    assert rc == vn.VN_OK and torch.equal(ptr, ptr_full)
+    assert torch.equal(small[:n // 2], ves_full[:n // 2]) and bool((small[n // 2:] == -7).all())
+
+
+@pytest.mark.parametrize("nves,npts", [(2, 1), (5, 3), (9, 31), (4, 129), (3, 300), (130, 7), (300, 2)])
+def test_near_pairs_edge_shapes(nves, npts):
+    rng = np.random.Generator(np.random.PCG64(31 * nves + npts))
+    X = rng.normal(size=(nves, npts, 2)) * 0.3 + 1.5 * rng.normal(size=(nves, 1, 2))
+    W = rng.uniform(0.02, 0.25, size=(nves, npts))
+    ref = oracle.near_mask(X, W)
+    assert margin_ok(X, W, ref, np.arange(nves * npts))
+    ptr, ves = gpu_near(X, W, np.float64)
+    assert np.array_equal(csr_to_dense(ptr, ves, nves), ref)
+    assert ref.sum() > 0 or nves * npts < 1000          # the larger cases all contain near pairs
+
+
+def test_near_pairs_large_sampled():
+    """Config 3 (2,000 x 128): the oracle checks 2,048 sampled rows; the total count is checked against
+    the relation's own CSR invariants."""
+    s = inputs.config(3)
+    W = oracle.weights(s.X)
+    P = s.nves * s.npts
+    rng = np.random.Generator(np.random.PCG64(260625569 + 200))
+    ptr, ves = gpu_near(s.X, W, np.float32)
+    Xo, Wo = stored(s.X, np.float32), stored(W, np.float32)
+    hot = np.flatnonzero(np.diff(ptr) > 0)
+    idx = np.unique(np.concatenate([rng.choice(P, size=1536, replace=False), hot[:512]]))
+    ref = oracle.near_mask_subset(Xo, Wo, idx)
+    assert margin_ok(Xo, Wo, ref, idx)
+    got = csr_to_dense(ptr, ves, s.nves)[idx] if P * s.nves <= 1 << 29 else None
+    if got is None:
+        got = np.zeros_like(ref)
+        for q, t in enumerate(idx):
+            got[q, ves[ptr[t]:ptr[t + 1]]] = 1
+    assert np.array_equal(got, ref)
+    assert ves.min() >= 0 and ves.max() < s.nves and np.all(ves != np.repeat(np.arange(P), np.diff(ptr)) // s.npts)
+    print(f"config3: {len(ves)} near pairs, {len(hot)} points with a near vesicle")
+
+
+# ------------------------------------------------------------------------------------- masked sum
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+@pytest.mark.parametrize("case", ["three_circles", "crowded1"])
+def test_farfield_masked_full_parity(case, dtype):
+    X, F, W, mu = three_circles() if case == "three_circles" else crowded(1, 0.94)
+    Xo, Fo, Wo = stored(X, dtype), stored(F, dtype), stored(W, dtype)
+    near = oracle.near_mask(Xo, Wo)
+    ref = oracle.farfield_masked(Xo, Fo, Wo, near, mu)
+    Xd, Fd, Wd = dev(X, dtype), dev(F, dtype), dev(W, dtype)
+    ptr, ves = vn.vn_near_pairs(Xd, Wd)
+    got = vn.vn_farfield_masked(Xd, Fd, Wd, ptr, ves, mu)
+    torch.cuda.synchronize()
+    got = got.cpu().numpy()
+    err = rel_l2(got, ref)
+    rows = near.sum(1) > 0                                           # the corrected targets on their own
+    err_rows = rel_l2(got.reshape(-1, 2)[rows], ref.reshape(-1, 2)[rows])
+    print(f"masked {case} {np.dtype(dtype).name}: rel-L2 {err:.3e} (corrected rows only {err_rows:.3e}, {rows.sum()} rows)")
+    assert err <= TOL[dtype] and err_rows <= TOL[dtype]
+    # the mask matters: the unmasked sum differs on those rows by far more than the tolerance
+    full = oracle.farfield(Xo, Fo, Wo, mu).reshape(-1, 2)
+    assert rel_l2(full[rows], ref.reshape(-1, 2)[rows]) > 1e3 * TOL[dtype]
+
+
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+def test_farfield_masked_empty_relation_equals_plain(dtype):
+    s = inputs.config(0)
+    W = oracle.weights(s.X)
+    Xd, Fd, Wd = dev(s.X, dtype), dev(s.F, dtype), dev(W, dtype)
+    ptr, ves = vn.vn_near_pairs(Xd, Wd)
+    assert ves.numel() == 0
+    a = vn.vn_farfield_masked(Xd, Fd, Wd, ptr, ves, s.mu)
+    b = vn.vn_farfield(Xd, Fd, Wd, s.mu)
+    torch.cuda.synchronize()
+    assert torch.equal(a, b)
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_farfield_masked_large_sampled(dtype):
+    """Config 3 pulled together by 3 %: thousands of near pairs; oracle on sampled targets, half of
+    them rows that carry a correction."""
+    X, F, W, mu = crowded(3, 0.97)
+    nves, npts, _ = X.shape
+    P = nves * npts
+    Xd, Fd, Wd = dev(X, dtype), dev(F, dtype), dev(W, dtype)
+    ptr, ves = vn.vn_near_pairs(Xd, Wd)
+    got = vn.vn_farfield_masked(Xd, Fd, Wd, ptr, ves, mu)
+    torch.cuda.synchronize()
+    ptr_h = ptr.cpu().numpy()
+    hot = np.flatnonzero(np.diff(ptr_h) > 0)
+    rng = np.random.Generator(np.random.PCG64(260625569 + 300))
+    idx = np.unique(np.concatenate([rng.choice(P, size=1024, replace=False),
+                                    rng.choice(hot, size=min(1024, len(hot)), replace=False)]))
+    Xo, Fo, Wo = stored(X, dtype), stored(F, dtype), stored(W, dtype)
+    rows = oracle.near_mask_subset(Xo, Wo, idx)
+    ref = oracle.farfield_masked_subset(Xo, Fo, Wo, idx, rows, mu)
+    err = rel_l2(got.cpu().numpy().reshape(-1, 2)[idx], ref)
+    print(f"masked config3 x0.97 {np.dtype(dtype).name}: {len(hot)} corrected points, sampled rel-L2 {err:.3e}")
+    assert len(hot) > 1000 and err <= TOL[dtype]
+
+
+def test_farfield_masked_deterministic():
+    X, F, W, mu = crowded(1, 0.94)
+    Xd, Fd, Wd = dev(X, np.float32), dev(F, np.float32), dev(W, np.float32)
+    ptr, ves = vn.vn_near_pairs(Xd, Wd)
+    a = vn.vn_farfield_masked(Xd, Fd, Wd, ptr, ves, mu).clone()
+    b = vn.vn_farfield_masked(Xd, Fd, Wd, ptr, ves, mu)
+    torch.cuda.synchronize()
+    assert torch.equal(a, b)
+
+
+# ------------------------------------------------------------------------------------- free targets
+def grid_targets(X, n, seed, keep_away=0.25):
+    """Random points of the suspension's bounding box that stay `keep_away` from every membrane point."""
+    from scipy.spatial import cKDTree
+    P = X.reshape(-1, 2)
+    rng = np.random.Generator(np.random.PCG64(seed))
+    lo, hi = P.min(0) - 1.0, P.max(0) + 1.0
+    xt = rng.uniform(lo, hi, size=(3 * n, 2))
+    d, _ = cKDTree(P).query(xt)
+    return xt[d >= keep_away][:n]
+
+
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+@pytest.mark.parametrize("index,nt", [(0, 1), (0, 777), (1, 5000)])
+def test_farfield_targets_parity(index, nt, dtype):
+    s = inputs.config(index)
+    W = oracle.weights(s.X)
+    xt = grid_targets(s.X, nt, 900 + index)
+    assert len(xt) == nt
+    ref = oracle.farfield_targets(stored(s.X, dtype), stored(s.F, dtype), stored(W, dtype), stored(xt, dtype), s.mu)
+    got = vn.vn_farfield_targets(dev(xt, dtype), dev(s.X, dtype), dev(s.F, dtype), dev(W, dtype), s.mu)
+    torch.cuda.synchronize()
+    err = rel_l2(got.cpu().numpy(), ref)
+    print(f"targets config{index} nt={nt} {np.dtype(dtype).name}: rel-L2 {err:.3e}")
+    assert err <= TOL[dtype]
+
+
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+def test_farfield_targets_large_sampled(dtype):
+    """Config 3 sources, 100,000 free targets (several target blocks and a ragged tail), oracle on 1,500 of them."""
+    s = inputs.config(3)
+    W = oracle.weights(s.X)
+    xt = grid_targets(s.X, 100_000, 903)
+    got = vn.vn_farfield_targets(dev(xt, dtype), dev(s.X, dtype), dev(s.F, dtype), dev(W, dtype), s.mu)
+    torch.cuda.synchronize()
+    rng = np.random.Generator(np.random.PCG64(904))
+    idx = np.unique(np.concatenate([[0, 1023, 1024, len(xt) - 1], rng.choice(len(xt), size=1500, replace=False)]))
+    ref = oracle.farfield_targets(stored(s.X, dtype), stored(s.F, dtype), stored(W, dtype), stored(xt, dtype)[idx], s.mu)
+    err = rel_l2(got.cpu().numpy()[idx], ref)
+    print(f"targets config3 nt={len(xt)} {np.dtype(dtype).name}: sampled rel-L2 {err:.3e}")
+    assert err <= TOL[dtype]
+
+
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+def test_farfield_targets_on_a_membrane_free_vesicle_equals_farfield(dtype):
+    """Targets = the points of a force-free extra vesicle: vn_farfield's value there (own vesicle
+    excluded, and it carries no force anyway) equals the free-target value."""
+    s = inputs.config(0)
+    X = np.concatenate([s.X, s.X[:1] + np.array([1.5, 1.5])])     # a 17th ellipse between grid rows
+    F = np.concatenate([s.F, np.zeros_like(s.F[:1])])
+    W = oracle.weights(X)
+    Xd, Fd, Wd = dev(X, dtype), dev(F, dtype), dev(W, dtype)
+    a = vn.vn_farfield(Xd, Fd, Wd, s.mu)[-1]
+    # sources for the free-target call: the 16 force-carrying vesicles only (a target must not coincide
+    # with a source point)
+    b = vn.vn_farfield_targets(Xd[-1].clone(), Xd[:-1].contiguous(), Fd[:-1].contiguous(), Wd[:-1].contiguous(), s.mu)
+    torch.cuda.synchronize()
+    assert rel_l2(b.cpu().numpy(), a.cpu().numpy()) <= TOL[dtype]
+
+
+def test_farfield_targets_empty():
+    s = inputs.config(0)
+    W = oracle.weights(s.X)
+    xt = torch.empty((0, 2), dtype=torch.float64, device="cuda")
+    out = vn.vn_farfield_targets(xt, dev(s.X, np.float64), dev(s.F, np.float64), dev(W, np.float64), s.mu)
+    assert out.shape == (0, 2)

@@ -313,3 +313,12 @@ def test_near_mask_and_masked_sum():
     assert np.allclose(Um[0][rows], (U[0] - UB[0])[rows], rtol=0, atol=1e-13)
     assert np.allclose(Um[0][~rows], U[0][~rows], rtol=0, atol=0)
     assert np.array_equal(Um[2], U[2])
+    # subset variants are the same rows
+    idx = np.array([0, 5, N - 1, N, N + 7, 2 * N, 3 * N - 1])
+    rows_sub = oracle.near_mask_subset(X, W, idx)
+    assert np.array_equal(rows_sub, near[idx])
+    assert np.array_equal(oracle.farfield_masked_subset(X, F, W, idx, rows_sub), Um.reshape(-1, 2)[idx])
+    # the relation is not symmetric in general (h belongs to the SOURCE vesicle): shrink B's weights
+    W2 = W.copy(); W2[1] *= 0.1
+    near2 = oracle.near_mask(X, W2)
+    assert near2[N:2 * N, 0].any() and not near2[:N, 1].any()
