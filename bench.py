@@ -101,13 +101,24 @@ def nvml_index(local_rank):
 def make_workload(index, rank):
     """Suspension for this rank: rank 0 gets BASELINE.json's seed, rank r the same recipe with seed + 1000 r."""
     from paper_2606_25569_b200 import inputs
+    from paper_2606_25569_b200 import multi
     if rank == 0 or index == 0:
         return inputs.config(index)
     kw = dict(inputs._CONFIGS[index])
-    return inputs.suspension(seed=inputs.BASE_SEED + index + 1000 * rank, **kw)
+    return inputs.suspension(seed=multi.shard_seed(inputs.BASE_SEED, index, rank), **kw)
 
 
-def oracle_rate(susp, np_dtype, seconds, rng_seed):
+def target_grid(susp, n_side, np_dtype):
+    """n_side x n_side velocity-field grid over the suspension's bounding box plus a margin of 1
+    (row f-4).  Grid points that fall close to a membrane simply get the plain trapezoid value."""
+    P = susp.X.reshape(-1, 2)
+    lo, hi = P.min(0) - 1.0, P.max(0) + 1.0
+    gx = np.linspace(lo[0], hi[0], n_side)
+    gy = np.linspace(lo[1], hi[1], n_side)
+    return np.ascontiguousarray(np.stack(np.meshgrid(gx, gy, indexing="ij"), -1).reshape(-1, 2), dtype=np_dtype)
+
+
+def oracle_rate(susp, np_dtype, seconds, rng_seed, path="farfield"):
     """Times the oracle (as it stands) on a bounded random sample of targets x ALL sources of the
     same workload; returns (GInt/s, cores, description)."""
     import oracle
@@ -115,16 +126,25 @@ def oracle_rate(susp, np_dtype, seconds, rng_seed):
     F = np.asarray(susp.F, dtype=np_dtype).astype(np.float64)
     W = oracle.weights(X)
     P = susp.nves * susp.npts
-    per_target = P - susp.npts
     rng = np.random.Generator(np.random.PCG64(rng_seed))
-    probe = rng.choice(P, size=min(P, 64 * oracle.num_threads()), replace=False)
+    if path == "targets":
+        xt = target_grid(susp, 512, np_dtype).astype(np.float64)
+        pool, per_target = len(xt), P
+        run = lambda idx: oracle.farfield_targets(X, F, W, xt[idx], susp.mu)
+    elif path == "masked":
+        pool, per_target = P, P - susp.npts
+        run = lambda idx: oracle.farfield_masked_subset(X, F, W, idx, oracle.near_mask_subset(X, W, idx), susp.mu)
+    else:
+        pool, per_target = P, P - susp.npts
+        run = lambda idx: oracle.farfield_subset(X, F, W, idx, susp.mu)
+    probe = rng.choice(pool, size=min(pool, 64 * oracle.num_threads()), replace=False)
     t0 = time.perf_counter()
-    oracle.farfield_subset(X, F, W, probe, susp.mu)
+    run(probe)
     rate = len(probe) * per_target / (time.perf_counter() - t0)
-    n = int(max(len(probe), min(P, rate * seconds / per_target)))
-    idx = rng.choice(P, size=n, replace=False)
+    n = int(max(len(probe), min(pool, rate * seconds / per_target)))
+    idx = rng.choice(pool, size=n, replace=False)
     t0 = time.perf_counter()
-    oracle.farfield_subset(X, F, W, idx, susp.mu)
+    run(idx)
     dt = time.perf_counter() - t0
     return n * per_target / dt / 1e9, oracle.num_threads(), f"{n} random targets x all {P} sources ({n * per_target:.3e} pairs, {dt:.1f} s)"
 
@@ -140,15 +160,16 @@ def run_reference(args):
     per_step = max(2.0, min(30.0, 150.0 / total))
     rates, cores, sample = [], 0, ""
     for s in range(total):
-        r, cores, sample = oracle_rate(susp, np_dtype, per_step, 7000 + s)
+        r, cores, sample = oracle_rate(susp, np_dtype, per_step, 7000 + s, args.path)
         if s >= args.warmup:
             rates.append(r)
     value = statistics.mean(rates)
     P = susp.nves * susp.npts
     evals = 10 if args.workload == 4 else 1
+    pairs_eval = 512 * 512 * P if args.path == "targets" else susp.pairs
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": evals * susp.pairs / (value * 1e9) * 1e3, "higher_is_better": True, "scaling": "weak",
+            "ms_per_step": evals * pairs_eval / (value * 1e9) * 1e3, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": workload_config(args, susp, "oracle on host cores; ms_per_step extrapolated from the sampled rate"),
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
@@ -158,11 +179,18 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+PATHS = {"farfield": "rows a-1..a-5: vn_arclength_weights + vn_farfield",
+         "masked": "row f-1: vn_arclength_weights + vn_near_pairs + vn_farfield_masked (the paper's DirectSingleLayerIntegral)",
+         "targets": "row f-4: vn_arclength_weights + vn_farfield_targets on a 512x512 grid of free targets"}
+
+
 def workload_config(args, susp, note=""):
     evals = 10 if args.workload == 4 else 1
-    return {"workload": f"BASELINE.json configs[{args.workload}]: {susp.name}",
-            "nves": susp.nves, "npts": susp.npts, "points": susp.nves * susp.npts,
-            "pairs_per_evaluation": susp.pairs, "evaluations_per_step": evals,
+    P = susp.nves * susp.npts
+    return {"workload": f"BASELINE.json configs[{args.workload}]: {susp.name}", "path": PATHS[args.path],
+            "nves": susp.nves, "npts": susp.npts, "points": P,
+            "pairs_per_evaluation": 512 * 512 * P if args.path == "targets" else susp.pairs,
+            "evaluations_per_step": evals,
             "precision": args.precision, "l2": "flushed between timed steps (256 MiB write); inputs < L2",
             "parallelism": f"{args.gpus} independent suspensions (one per GPU)" if args.gpus > 1 else "single GPU",
             "note": note}
@@ -176,6 +204,9 @@ def main():
     ap.add_argument("--workload", type=int, default=4, choices=[0, 1, 2, 3, 4])
     ap.add_argument("--precision", default="f32", choices=["f32", "f64"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--path", default="farfield", choices=["farfield", "masked", "targets"],
+                    help="farfield: rows a-1..a-5 (the headline); masked: row f-1 (vn_near_pairs + "
+                         "vn_farfield_masked); targets: row f-4 (vn_farfield_targets on a 512x512 grid)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -205,7 +236,8 @@ def main():
     seq_np = susp.X_sequence if susp.X_sequence else [susp.X]
     evals = len(seq_np)
     P = susp.nves * susp.npts
-    pairs_step = evals * susp.pairs
+    pairs_eval = 512 * 512 * P if args.path == "targets" else susp.pairs
+    pairs_step = evals * pairs_eval
 
     # ---- device-resident inputs (value) and pinned host inputs (e2e)
     seq_h = [torch.from_numpy(np.ascontiguousarray(x, dtype=np_dtype)).pin_memory() for x in seq_np]
@@ -218,19 +250,50 @@ def main():
     U_d = torch.empty_like(X_d)
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")
 
+    if args.path == "masked":                          # CSR buffers sized once (4 near vesicles per point is generous)
+        near_ptr = torch.empty(P + 1, dtype=torch.int64, device="cuda")
+        near_ves = torch.empty(4 * P, dtype=torch.int32, device="cuda")
+    if args.path == "targets":
+        Xt_h = torch.from_numpy(target_grid(susp, 512, np_dtype)).pin_memory()
+        Xt_d = Xt_h.cuda()
+        Ut_d = torch.empty_like(Xt_d)
+        Ut_h = torch.empty_like(Xt_h).pin_memory()
+
+    def evaluate():
+        vn.vn_arclength_weights(X_d, out=W_d)          # a-1
+        if args.path == "farfield":
+            vn.vn_farfield(X_d, F_d, W_d, susp.mu, out=U_d)   # a-2 .. a-5
+        elif args.path == "masked":
+            vn.vn_near_pairs(X_d, W_d, near_ptr, near_ves)
+            vn.vn_farfield_masked(X_d, F_d, W_d, near_ptr, near_ves, susp.mu, out=U_d)
+        else:
+            vn.vn_farfield_targets(Xt_d, X_d, F_d, W_d, susp.mu, out=Ut_d)
+
     def step_device():
         for c in range(evals):
             X_d.copy_(seq_d[c])                        # device-to-device, same stream
-            vn.vn_arclength_weights(X_d, out=W_d)      # a-1
-            vn.vn_farfield(X_d, F_d, W_d, susp.mu, out=U_d)   # a-2 .. a-5
+            evaluate()
 
     def step_host():
         for c in range(evals):
-            vn.vn_farfield_host(seq_h[c], F_h, None, susp.mu, out=U_h)
+            if args.path == "farfield":
+                vn.vn_farfield_host(seq_h[c], F_h, None, susp.mu, out=U_h)
+            else:                                      # no host entry point for the NEXT rows: explicit copies
+                X_d.copy_(seq_h[c], non_blocking=True)
+                F_d.copy_(F_h, non_blocking=True)
+                if args.path == "targets":
+                    Xt_d.copy_(Xt_h, non_blocking=True)
+                evaluate()
+                if args.path == "targets":
+                    Ut_h.copy_(Ut_d, non_blocking=True)
+                else:
+                    U_h.copy_(U_d, non_blocking=True)
+                torch.cuda.synchronize()
+
+    from paper_2606_25569_b200 import multi
 
     def barrier():
-        if world > 1:
-            dist.barrier()
+        multi.barrier()
         torch.cuda.synchronize()
 
     def timed(step_fn, steps, use_events):
@@ -271,48 +334,49 @@ def main():
 
     t_e2e = None
     if not args.no_e2e:
-        for _ in range(3):
-            vn.vn_farfield_host(seq_h[0], F_h, None, susp.mu, out=U_h)
+        for _ in range(3 if args.path == "farfield" else 1):
+            step_host()
         t_e2e = timed(step_host, max(1, min(args.steps, 2)), False) / max(1, min(args.steps, 2)) * args.steps
 
-    def max_over_ranks(x):
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
-
-    t_dev = max_over_ranks(t_dev)
+    if args.path == "masked":
+        torch.cuda.synchronize()
+        n_near = int(near_ptr[P].item())
+        if n_near > near_ves.numel():
+            raise SystemExit(f"near relation has {n_near} pairs, buffer holds {near_ves.numel()}")
+    # whole-job numbers: work summed over ranks, time = the slowest rank (paper_2606_25569_b200/multi.py)
+    rate_dev, t_dev, _ = multi.whole_job_rate(args.steps * pairs_step, t_dev, "cuda")
     if t_e2e is not None:
-        t_e2e = max_over_ranks(t_e2e)
+        rate_e2e, t_e2e, _ = multi.whole_job_rate(args.steps * pairs_step, t_e2e, "cuda")
 
     if rank == 0:
-        value = world * args.steps * pairs_step / t_dev / 1e9
+        value = rate_dev / 1e9
         clocks = sampler.summary()
         peaks = measured_peaks()
         sm_max = clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz") or 1965.0
         lanes = FP32_LANES if args.precision == "f32" else FP64_LANES
         peak_lane = SMS * lanes * sm_max * 1e6 / 1e12                     # T lane-instr/s at max clock
         k_ms = statistics.mean(kernel_ms) if kernel_ms else None
-        achieved = LANE_OPS_PER_PAIR * susp.pairs / (k_ms * 1e-3) / 1e12 if k_ms else None
+        achieved = LANE_OPS_PER_PAIR * pairs_eval / (k_ms * 1e-3) / 1e12 if k_ms else None
         traffic = None                                   # dram bytes per launch from the committed ncu --set full capture
         try:
             import csv
             with open(os.path.join(ROOT, "profiles", "traffic.csv")) as fh:
                 for row in csv.DictReader(fh):
-                    if row["workload"] == f"config{args.workload}" and row["precision"] == args.precision:
+                    if (row["workload"] == f"config{args.workload}" and row["precision"] == args.precision
+                            and row.get("path", "farfield") == args.path):
                         traffic = int(row["dram_read_bytes"]) + int(row["dram_write_bytes"])
         except Exception:
             pass
-        roofline = {"bound": "alu", "kernel": "farfield_%s_kernel" % args.precision,
+        roofline = {"bound": "alu",
+                    "kernel": ("targets_%s_kernel" if args.path == "targets" else "farfield_%s_kernel") % args.precision,
                     "achieved": achieved, "peak": peak_lane,
                     "unit": "T lane-instr/s (%s pipe; 11 canonical instr per pair)" % ("FP32" if args.precision == "f32" else "FP64"),
                     "frac": achieved / peak_lane if achieved else None,
                     "peak_source": "derived: 148 SMs x %d lanes x %.0f MHz (guide unit counts, clocks.max.sm); "
                                    "MEASURED_PEAKS.json holds only HBM/bf16 peaks" % (lanes, sm_max),
                     "kernel_ms_avg": k_ms, "kernel_launches_timed": len(kernel_ms),
-                    "kernel_ginteractions_per_s": susp.pairs / (k_ms * 1e-3) / 1e9 if k_ms else None,
-                    "flop_frac": (FLOP_PER_PAIR * susp.pairs / (k_ms * 1e-3) / 1e12) / (2 * peak_lane) if k_ms else None,
+                    "kernel_ginteractions_per_s": pairs_eval / (k_ms * 1e-3) / 1e9 if k_ms else None,
+                    "flop_frac": (FLOP_PER_PAIR * pairs_eval / (k_ms * 1e-3) / 1e12) / (2 * peak_lane) if k_ms else None,
                     "frac_at_sampled_clock": (achieved / (SMS * lanes * clocks["sm_mhz"] * 1e6 / 1e12)
                                               if achieved and clocks.get("sm_mhz") else None),
                     "hbm_algorithmic_bytes": 28 * P if args.precision == "f32" else 56 * P,
@@ -324,11 +388,17 @@ def main():
                 "roofline": roofline}
         if t_e2e is not None:
             es = 4 if args.precision == "f32" else 8
-            line["e2e"] = {"value": world * args.steps * pairs_step / t_e2e / 1e9, "unit": UNIT,
-                           "h2d_bytes_per_step": evals * 2 * (2 * es * P), "d2h_bytes_per_step": evals * 2 * es * P,
-                           "api": "vn_farfield_host (pinned host buffers; weights computed on device)"}
+            nt = 512 * 512
+            line["e2e"] = {"value": rate_e2e / 1e9, "unit": UNIT,
+                           "h2d_bytes_per_step": evals * 2 * es * (2 * P + (nt if args.path == "targets" else 0)),
+                           "d2h_bytes_per_step": evals * 2 * es * (nt if args.path == "targets" else P),
+                           "api": "vn_farfield_host (pinned host buffers; weights computed on device)"
+                                  if args.path == "farfield" else
+                                  "pinned host buffers -> device copies -> the path's C-ABI calls -> copy back, synchronised"}
+        if args.path == "masked":
+            line["config"]["near_pairs"] = n_near
         if world == 1 and not args.no_cpu_baseline:
-            v, cores, sample = oracle_rate(susp, np_dtype, 15.0, 4242)
+            v, cores, sample = oracle_rate(susp, np_dtype, 15.0, 4242, args.path)
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
         print(json.dumps(line), flush=True)
 

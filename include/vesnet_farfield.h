@@ -136,6 +136,23 @@ vn_status vn_farfield_targets(const void *Xt, int64_t nt,
                               int64_t nves, int64_t npts, double mu,
                               void *Ut, vn_precision precision, void *stream);
 
+/* ---- row f-2: the elastic membrane force (the producer of F) -----------------------------------
+ * PAPER.md:123 eq 2.7, :319 Fig. 5b:
+ *
+ *   F[v,j,:] = -kappa_b X_ssss + (sigma X_s)_s   at point j of vesicle v,
+ *   d/ds = |dX/dalpha|^-1 d/dalpha, d/dalpha = Fourier derivative with the unmatched
+ *   k = npts/2 mode dropped, the four arclength derivatives applied one after the other without
+ *   filtering (readings A4, E1).
+ *
+ * X[nves,npts,2], sigma[nves,npts] (membrane tension per point), F[nves,npts,2]: DEVICE pointers in
+ * the call's precision; kappa_b: host double (bending stiffness, one value for all vesicles, any
+ * finite value).  Arithmetic is double inside for both precisions.  npts <= 1024 (one vesicle lives
+ * in one block's shared memory), else VN_ERR_INVALID_ARG.  F is overwritten and must not alias
+ * the inputs.  The result is conditioned like a fourth derivative: rounding of X is amplified by
+ * about (npts/2)^4 / |dX/dalpha|^4. */
+vn_status vn_elastic_force(const void *X, const void *sigma, int64_t nves, int64_t npts,
+                           double kappa_b, void *F, vn_precision precision, void *stream);
+
 /* Profiling aid (bench.py's roofline figure): while enabled, every vn_farfield /
  * vn_farfield_host / vn_farfield_masked / vn_farfield_targets call records a CUDA event pair on its
  * stream around the pair kernel alone (not the pack / finish / correction kernels).  vn_profile_read waits for the recorded events,

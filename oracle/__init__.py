@@ -51,6 +51,7 @@ def _load():
         lib.oracle_near_mask_subset.argtypes = [d, d, i64, i64, ctypes.POINTER(i64), i64, u8]
         lib.oracle_farfield_masked_subset.argtypes = [d, d, d, i64, i64, ctypes.c_double,
                                                       ctypes.POINTER(i64), i64, u8, d]
+        lib.oracle_elastic_force.argtypes = [d, d, i64, i64, ctypes.c_double, d]
         _lib = lib
     return _lib
 
@@ -175,3 +176,14 @@ def farfield_masked_subset(X, F, W, idx, near_rows, mu=1.0):
     if rc:
         raise ValueError(f"oracle_farfield_masked_subset rc={rc}")
     return Us
+
+
+def elastic_force(X, sigma, kappa_b=1.0):
+    """f = -kappa_b X_ssss + (sigma X_s)_s (eq 2.7), spectral arclength derivatives -> [nves,npts,2]."""
+    X = _c(X); nves, npts, _ = X.shape
+    sigma = _c(sigma, (nves, npts))
+    F = np.empty_like(X)
+    rc = _load().oracle_elastic_force(_p(X), _p(sigma), nves, npts, float(kappa_b), _p(F))
+    if rc:
+        raise ValueError(f"oracle_elastic_force rc={rc}")
+    return F

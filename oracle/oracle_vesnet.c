@@ -308,3 +308,79 @@ int oracle_farfield_masked_subset(const double *X, const double *F, const double
     }
     return 0;
 }
+
+/* ---------------------------------------------------------------------------------------------
+ * Row f-2: the elastic membrane force (PAPER.md:123 eq 2.7, :319 Fig. 5b)
+ *
+ *     f = -kappa_b X_ssss + (sigma X_s)_s ,      d/ds = |dX/dalpha|^-1 d/dalpha
+ *
+ * with every d/dalpha the Fourier derivative written out as in oracle_weights (forward DFT,
+ * multiply by i k, inverse DFT, unmatched k = N/2 mode dropped -- DESIGN.md reading A4) and the
+ * four arclength derivatives applied one after the other (reading E1: no filtering, no
+ * de-aliasing; the paper is silent).  kappa_b is one scalar, sigma a value per point. */
+static void fourier_derivative(const ld *f, int64_t N, const ld *ctab, const ld *stab, ld *df)
+{
+    const int64_t kmax = (N - 1) / 2;
+    for (int64_t j = 0; j < N; ++j) df[j] = 0.0L;
+    for (int64_t k = -kmax; k <= kmax; ++k) {
+        ld cre = 0.0L, cim = 0.0L;                        /* fhat_k = (1/N) sum_m f_m e^{-i k alpha_m} */
+        for (int64_t m = 0; m < N; ++m) {
+            int64_t a = (k * m) % N; if (a < 0) a += N;
+            cre += f[m] * ctab[a];
+            cim -= f[m] * stab[a];
+        }
+        cre /= (ld)N; cim /= (ld)N;
+        for (int64_t j = 0; j < N; ++j) {                 /* + Re( i k fhat_k e^{i k alpha_j} ) */
+            int64_t b = (k * j) % N; if (b < 0) b += N;
+            df[j] += (ld)k * (-cim * ctab[b] - cre * stab[b]);
+        }
+    }
+}
+
+int oracle_elastic_force(const double *X, const double *sigma, int64_t nves, int64_t npts,
+                         double kappa_b, double *F)
+{
+    if (!X || !sigma || !F || nves < 1 || npts < 1) return 1;
+    const int64_t N = npts;
+    ld *ctab = (ld *)malloc(sizeof(ld) * (size_t)N);
+    ld *stab = (ld *)malloc(sizeof(ld) * (size_t)N);
+    if (!ctab || !stab) { free(ctab); free(stab); return 2; }
+    for (int64_t m = 0; m < N; ++m) {
+        ctab[m] = cosl(2.0L * ORACLE_PI * (ld)m / (ld)N);
+        stab[m] = sinl(2.0L * ORACLE_PI * (ld)m / (ld)N);
+    }
+    int fail = 0;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t v = 0; v < nves; ++v) {
+        ld *w = (ld *)malloc(sizeof(ld) * 9 * (size_t)N);
+        if (!w) { fail = 1; continue; }
+        ld *x = w, *y = w + N, *dx = w + 2 * N, *dy = w + 3 * N, *sa = w + 4 * N;
+        ld *xs = w + 5 * N, *ys = w + 6 * N, *tx = w + 7 * N, *ty = w + 8 * N;
+        for (int64_t j = 0; j < N; ++j) { x[j] = (ld)X[2 * (v * N + j)]; y[j] = (ld)X[2 * (v * N + j) + 1]; }
+        fourier_derivative(x, N, ctab, stab, dx);
+        fourier_derivative(y, N, ctab, stab, dy);
+        for (int64_t j = 0; j < N; ++j) {
+            sa[j] = sqrtl(dx[j] * dx[j] + dy[j] * dy[j]);                 /* |dX/dalpha| */
+            xs[j] = dx[j] / sa[j]; ys[j] = dy[j] / sa[j];                 /* X_s */
+        }
+        /* (sigma X_s)_s */
+        for (int64_t j = 0; j < N; ++j) { x[j] = (ld)sigma[v * N + j] * xs[j]; y[j] = (ld)sigma[v * N + j] * ys[j]; }
+        fourier_derivative(x, N, ctab, stab, tx);
+        fourier_derivative(y, N, ctab, stab, ty);
+        for (int64_t j = 0; j < N; ++j) { tx[j] /= sa[j]; ty[j] /= sa[j]; }
+        /* X_ss, X_sss, X_ssss: three more arclength derivatives of X_s */
+        for (int64_t j = 0; j < N; ++j) { x[j] = xs[j]; y[j] = ys[j]; }
+        for (int rep = 0; rep < 3; ++rep) {
+            fourier_derivative(x, N, ctab, stab, dx);
+            fourier_derivative(y, N, ctab, stab, dy);
+            for (int64_t j = 0; j < N; ++j) { x[j] = dx[j] / sa[j]; y[j] = dy[j] / sa[j]; }
+        }
+        for (int64_t j = 0; j < N; ++j) {
+            F[2 * (v * N + j) + 0] = (double)(-(ld)kappa_b * x[j] + tx[j]);
+            F[2 * (v * N + j) + 1] = (double)(-(ld)kappa_b * y[j] + ty[j]);
+        }
+        free(w);
+    }
+    free(ctab); free(stab);
+    return fail ? 2 : 0;
+}

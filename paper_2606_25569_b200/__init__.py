@@ -13,6 +13,7 @@ raises.
     ptr, ves = vn_near_pairs(X, W)              # near-field relation (CSR)
     U = vn_farfield_masked(X, F, W, ptr, ves)   # the paper's DirectSingleLayerIntegral
     Ut = vn_farfield_targets(Xt, X, F, W)       # velocity at free points Xt[nt, 2]
+    F = vn_elastic_force(X, sigma, kappa_b)     # eq 2.7, the density the sums above consume
 
 `inputs` (seeded synthetic suspensions) is importable without the library.
 """
@@ -57,6 +58,8 @@ def lib():
         L.vn_farfield_masked.restype = ci
         L.vn_farfield_targets.argtypes = [vp, i64, vp, vp, vp, i64, i64, dbl, vp, ci, vp]
         L.vn_farfield_targets.restype = ci
+        L.vn_elastic_force.argtypes = [vp, vp, i64, i64, dbl, vp, ci, vp]
+        L.vn_elastic_force.restype = ci
         L.vn_profile_enable.argtypes = [ci]
         L.vn_profile_enable.restype = ci
         L.vn_profile_read.argtypes = [ctypes.POINTER(dbl), i64]
@@ -207,6 +210,25 @@ def vn_farfield_targets(Xt, X, F, W, mu: float = 1.0, out=None, stream=None):
                                        out.data_ptr() if Xt.numel() else None, _prec(X), _stream_ptr(stream))
     if rc != VN_OK:
         raise VesnetError(rc, "vn_farfield_targets")
+    return out
+
+
+def vn_elastic_force(X, sigma, kappa_b: float = 1.0, out=None, stream=None):
+    """F = -kappa_b X_ssss + (sigma X_s)_s (eq 2.7) for every vesicle (device tensors)."""
+    import torch
+    nves, npts, two = X.shape
+    if two != 2:
+        raise ValueError("X must be [nves, npts, 2]")
+    _check_dev("X", X)
+    _check_dev("sigma", sigma, (nves, npts), X.dtype)
+    if out is None:
+        out = torch.empty_like(X)
+    _check_dev("out", out, X.shape, X.dtype)
+    with torch.cuda.device(X.device):
+        rc = lib().vn_elastic_force(X.data_ptr(), sigma.data_ptr(), nves, npts, float(kappa_b), out.data_ptr(),
+                                    _prec(X), _stream_ptr(stream))
+    if rc != VN_OK:
+        raise VesnetError(rc, "vn_elastic_force")
     return out
 
 

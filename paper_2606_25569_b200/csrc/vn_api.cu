@@ -35,6 +35,8 @@ vn_status farfield_targets_f32(const void *Xt, int64_t nt, const void *X, const 
                                int64_t nves, int64_t npts, double mu, void *Ut, cudaStream_t st);
 vn_status farfield_targets_f64(const void *Xt, int64_t nt, const void *X, const void *F, const void *W,
                                int64_t nves, int64_t npts, double mu, void *Ut, cudaStream_t st);
+vn_status elastic_force(const void *X, const void *sigma, int64_t nves, int64_t npts, double kappa_b, void *F,
+                        vn_precision prec, cudaStream_t st);
 vn_status near_pairs(const void *X, const void *W, int64_t nves, int64_t npts, int64_t *near_ptr,
                      int32_t *near_ves, int64_t capacity, vn_precision prec, cudaStream_t st);
 vn_status arclength_weights(const void *X, int64_t nves, int64_t npts, void *W, vn_precision prec, cudaStream_t st);
@@ -200,6 +202,20 @@ vn_status vn_arclength_weights(const void *X, int64_t nves, int64_t npts, void *
     const vn_status ds = check_device();
     if (ds != VN_OK) return ds;
     return arclength_weights(X, nves, npts, W, precision, (cudaStream_t)stream);
+}
+
+vn_status vn_elastic_force(const void *X, const void *sigma, int64_t nves, int64_t npts, double kappa_b, void *F,
+                           vn_precision precision, void *stream)
+{
+    if (!X || !sigma || !F) return VN_ERR_INVALID_ARG;
+    if (check_shape(nves, npts, precision) != VN_OK) return VN_ERR_INVALID_ARG;
+    if (npts > 1024 || !isfinite(kappa_b)) return VN_ERR_INVALID_ARG;
+    const size_t pair = precision == VN_F32 ? 8 : 16;
+    if (misaligned(X, pair) || misaligned(F, pair) || misaligned(sigma, pair / 2) || F == X || F == sigma)
+        return VN_ERR_INVALID_ARG;
+    const vn_status ds = check_device();
+    if (ds != VN_OK) return ds;
+    return elastic_force(X, sigma, nves, npts, kappa_b, F, precision, (cudaStream_t)stream);
 }
 
 vn_status vn_farfield_host(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, double mu,
