@@ -20,7 +20,16 @@ namespace vn {
 constexpr int kT64 = 4;                       // targets per thread
 constexpr int kST64 = kT64 * kThreads;        // points per super-tile (target block): 512
 constexpr int kSub64 = kST64 / kTile;         // source tiles per super-tile: 4
-constexpr int kBatch64 = 4;                   // sources per cross-lane reduction batch
+#ifndef VN_F64_BATCH
+#define VN_F64_BATCH 8
+#endif
+#ifndef VN_F64_MINBLK
+#define VN_F64_MINBLK 4
+#endif
+#ifndef VN_F64_MINTILES
+#define VN_F64_MINTILES 32
+#endif
+constexpr int kBatch64 = VN_F64_BATCH;        // sources per cross-lane reduction batch
 constexpr int kLogTab = 513;                  // (1/2) ln(rc) for the 9-bit reciprocals rc in [1/2, 1]
 
 // a-2: one 32-byte record (yx, yy, gx, gy) per source, g = F*W; also gmax = max_j (|gx| + |gy|)
@@ -82,7 +91,7 @@ __device__ __forceinline__ void log_rcp_f64(double r2, const double *__restrict_
 // a-3 / a-4: pair kernel; block (I, c) = super-tile I as targets x chunk c of I's list of source tiles
 // (own super-tile one-directional with the own vesicle predicated out, then the tiles of super-tiles
 // I+1 .. I+S_I in both directions) -- the same walk as farfield_f32_kernel.
-__global__ void __launch_bounds__(kThreads, 4)
+__global__ void __launch_bounds__(kThreads, VN_F64_MINBLK)
 farfield_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__ X, int P, int npts,
                     int n_tiles, int n_st, int n_chunks, const unsigned long long *__restrict__ gmax_bits,
                     long long *__restrict__ acc)
@@ -301,7 +310,7 @@ vn_status farfield_f64(const void *X, const void *F, const void *W, int64_t nves
         VN_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, farfield_f64_kernel, kThreads, 0));
         slots = sms * (occ > 0 ? occ : 1);
     }
-    const SymSplit sp = choose_sym_split(P, kST64, slots, 8);
+    const SymSplit sp = choose_sym_split(P, kST64, slots, VN_F64_MINTILES);
 
     // scratch: packed sources | fixed-point accumulators (hi, lo per component) | gmax
     const size_t b_src = (size_t)P * 32, b_acc = (size_t)P * 32;

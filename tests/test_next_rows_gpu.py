@@ -301,3 +301,65 @@ def test_farfield_targets_empty():
     xt = torch.empty((0, 2), dtype=torch.float64, device="cuda")
     out = vn.vn_farfield_targets(xt, dev(s.X, np.float64), dev(s.F, np.float64), dev(W, np.float64), s.mu)
     assert out.shape == (0, 2)
+
+
+# ------------------------------------------------------------------------------------- elastic force (row f-2)
+def force_tol(npts, dtype):
+    """The operator is a fourth spectral derivative: each of the four d/dalpha amplifies the relative
+    rounding noise already present by up to npts/2 (highest retained wavenumber over the O(1)
+    wavenumbers that carry the signal).  The kernel works in double, the oracle in long double, on the
+    same stored inputs: bound 64 eps (npts/2)^4 (64 covers the npts-term sums), plus the rounding of
+    the result to the storage type."""
+    return max(TOL[dtype] if dtype == np.float32 else 0.0, 64 * 2.2e-16 * (npts / 2) ** 4, 1e-12)
+
+
+def tension(nves, npts, seed):
+    rng = np.random.Generator(np.random.PCG64(seed))
+    al = 2 * np.pi * np.arange(npts) / npts
+    sig = np.ones((nves, npts))
+    for k in range(1, 9):
+        sig += rng.normal(size=(nves, 1)) / k ** 2 * np.cos(k * al + rng.uniform(0, 2 * np.pi, size=(nves, 1)))
+    return sig
+
+
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+@pytest.mark.parametrize("index", [0, 1])
+def test_elastic_force_parity(index, dtype):
+    s = inputs.config(index)
+    sig = tension(s.nves, s.npts, 40 + index)
+    kb = 0.7
+    ref = oracle.elastic_force(stored(s.X, dtype), stored(sig, dtype), kb)
+    got = vn.vn_elastic_force(dev(s.X, dtype), dev(sig, dtype), kb)
+    torch.cuda.synchronize()
+    err = rel_l2(got.cpu().numpy(), ref)
+    print(f"elastic force config{index} {np.dtype(dtype).name}: rel-L2 {err:.3e} (tolerance {force_tol(s.npts, dtype):.1e})")
+    assert err <= force_tol(s.npts, dtype)
+
+
+@pytest.mark.parametrize("npts", [3, 8, 31, 32, 33, 100, 129, 257, 1024])
+def test_elastic_force_edge_shapes(npts):
+    rng = np.random.Generator(np.random.PCG64(npts))
+    al = 2 * np.pi * np.arange(npts) / npts
+    r = 1.0 + 0.2 * np.cos(2 * al + rng.uniform(0, 6.28, size=(5, 1)))
+    X = np.stack([r * np.cos(al), 0.7 * r * np.sin(al)], -1) + 10.0 * rng.normal(size=(5, 1, 2))
+    sig = tension(5, npts, npts)
+    ref = oracle.elastic_force(X, sig, 1.3)
+    got = vn.vn_elastic_force(dev(X, np.float64), dev(sig, np.float64), 1.3)
+    torch.cuda.synchronize()
+    assert rel_l2(got.cpu().numpy(), ref) <= force_tol(npts, np.float64)
+
+
+def test_elastic_force_rejects_long_vesicles_and_feeds_farfield():
+    s = inputs.config(0)
+    with pytest.raises(vn.VesnetError):
+        vn.vn_elastic_force(torch.zeros((1, 1025, 2), device="cuda"), torch.zeros((1, 1025), device="cuda"))
+    # the producer feeds the consumer on one stream: F = elastic force, U = far field of F
+    Xd = dev(s.X, np.float64)
+    sig = dev(tension(s.nves, s.npts, 7), np.float64)
+    Wd = vn.vn_arclength_weights(Xd)
+    Fd = vn.vn_elastic_force(Xd, sig, 0.5)
+    Ud = vn.vn_farfield(Xd, Fd, Wd, s.mu)
+    torch.cuda.synchronize()
+    Fo = oracle.elastic_force(s.X, sig.cpu().numpy(), 0.5)
+    ref = oracle.farfield(s.X, Fo, oracle.weights(s.X), s.mu)
+    assert rel_l2(Ud.cpu().numpy(), ref) <= force_tol(s.npts, np.float64)

@@ -322,3 +322,105 @@ def test_near_mask_and_masked_sum():
     W2 = W.copy(); W2[1] *= 0.1
     near2 = oracle.near_mask(X, W2)
     assert near2[N:2 * N, 0].any() and not near2[:N, 1].any()
+
+
+# ----------------------------------------------------------------------------- elastic force (row f-2)
+def _circle(R, N, c=(0.0, 0.0), warp=0.0):
+    al = 2 * np.pi * np.arange(N) / N
+    be = al + warp * np.sin(al)                      # warp != 0: same circle, points not equispaced in arclength
+    return np.asarray(c) + R * np.stack([np.cos(be), np.sin(be)], -1), be
+
+
+def test_elastic_force_circle_closed_form():
+    """Circle of radius R about c: X_ss = -(X-c)/R^2, X_ssss = (X-c)/R^4, so with constant tension
+    f = -kappa_b (X-c)/R^4 - sigma (X-c)/R^2 (eq 2.7).  A sign error in either term, a
+    missing 1/|X_alpha| or a wrong derivative count fails this."""
+    for N in (16, 32, 64):
+        X, _ = _circle(0.7, N)
+        F = oracle.elastic_force(X[None], np.full((1, N), 1.3), 0.4)[0]
+        ref = -0.4 * X / 0.7 ** 4 - 1.3 * X / 0.7 ** 2
+        assert np.abs(F - ref).max() <= 1e-16 * (N / 2) ** 4 * 64
+
+
+def test_elastic_force_warped_circle_variable_tension():
+    """Arclength derivatives do not depend on the parametrisation: a circle sampled at beta = alpha +
+    0.3 sin(alpha) with sigma = 1.3 + 0.5 cos(beta) has (sigma X_s)_s = sigma_s X_s + sigma X_ss,
+    sigma_s = -0.5 sin(beta)/R, X_s = (-sin beta, cos beta).  Error falls spectrally with N."""
+    R, kb = 0.7, 0.4
+    errs = []
+    for N in (12, 16, 32):
+        X, be = _circle(R, N, warp=0.3)
+        sig = 1.3 + 0.5 * np.cos(be)
+        Xs = np.stack([-np.sin(be), np.cos(be)], -1)
+        ref = -kb * X / R ** 4 + (-0.5 * np.sin(be) / R)[:, None] * Xs - sig[:, None] * X / R ** 2
+        errs.append(np.abs(oracle.elastic_force(X[None], sig[None], kb)[0] - ref).max())
+    assert errs[0] > 1e-5 and errs[1] < 0.2 * errs[0] and errs[2] < 1e-10, errs
+
+
+def test_elastic_force_ellipse_tension_is_curvature_times_normal():
+    """kappa_b = 0, sigma = const on an ellipse sampled uniformly in the parameter (NOT in arclength):
+    f = sigma X_ss = -sigma * curvature * outward normal, curvature = ab/(a^2 sin^2 + b^2 cos^2)^(3/2)."""
+    a, b, N = 1.0, 0.6, 128
+    t = 2 * np.pi * np.arange(N) / N
+    th = 0.4
+    R = np.array([[np.cos(th), -np.sin(th)], [np.sin(th), np.cos(th)]])
+    X = np.stack([a * np.cos(t), b * np.sin(t)], -1) @ R.T
+    q = np.sqrt(a * a * np.sin(t) ** 2 + b * b * np.cos(t) ** 2)
+    n = np.stack([b * np.cos(t), a * np.sin(t)], -1) / q[:, None] @ R.T
+    ref = -2.5 * (a * b / q ** 3)[:, None] * n
+    F = oracle.elastic_force(X[None], np.full((1, N), 2.5), 0.0)[0]
+    assert np.abs(F - ref).max() <= 1e-10
+
+
+def _random_vesicles(seed, nves, N):
+    rng = np.random.default_rng(seed)
+    al = 2 * np.pi * np.arange(N) / N
+    r = 1.0 + sum(rng.uniform(0, 0.1 / k, (nves, 1)) * np.cos(k * al + rng.uniform(0, 2 * np.pi, (nves, 1))) for k in (2, 3, 4))
+    X = np.stack([r * np.cos(al), 0.6 * r * np.sin(al)], -1) + rng.normal(size=(nves, 1, 2))
+    sig = 1.0 + sum(rng.normal(size=(nves, 1)) / k ** 2 * np.cos(k * al + rng.uniform(0, 2 * np.pi, (nves, 1))) for k in (1, 2, 3))
+    return X, sig
+
+
+def test_elastic_force_total_force_vanishes_and_symmetries():
+    N = 32
+    X, sig = _random_vesicles(5, 4, N)
+    kb = 0.3
+    F = oracle.elastic_force(X, sig, kb)
+    W = oracle.weights(X)
+    # sum_j f_j w_j = (2 pi/N) sum_j d/dalpha(...)_j = 0 exactly: a membrane exerts no net force
+    assert np.abs((F * W[..., None]).sum(1)).max() <= 1e-11
+    # net torque vanishes to spectral accuracy
+    tq = ((X[..., 0] * F[..., 1] - X[..., 1] * F[..., 0]) * W).sum(1)
+    assert np.abs(tq).max() <= 1e-6
+    # translation invariance, rotation equivariance
+    assert np.allclose(oracle.elastic_force(X + np.array([7.0, -3.0]), sig, kb), F, rtol=0, atol=1e-9)
+    th = 1.1
+    R = np.array([[np.cos(th), -np.sin(th)], [np.sin(th), np.cos(th)]])
+    assert np.allclose(oracle.elastic_force(X @ R.T, sig, kb), F @ R.T, rtol=0, atol=1e-9)
+    # linear in (kappa_b, sigma); bending scales like a^-3, tension like a^-1 under X -> a X
+    Fb = oracle.elastic_force(X, 0 * sig, 1.0)
+    Ft = oracle.elastic_force(X, sig, 0.0)
+    assert np.allclose(F, kb * Fb + Ft, rtol=0, atol=1e-10)
+    a = 1.7
+    assert np.allclose(oracle.elastic_force(a * X, sig, kb), kb * Fb / a ** 3 + Ft / a, rtol=0, atol=1e-9)
+    # each vesicle on its own
+    assert np.array_equal(oracle.elastic_force(X[2:3], sig[2:3], kb)[0], F[2])
+    # reversing the orientation of the curve changes nothing (even number of arclength derivatives)
+    rev = np.concatenate([[0], np.arange(N - 1, 0, -1)])
+    assert np.allclose(oracle.elastic_force(X[:, rev], sig[:, rev], kb)[:, rev], F, rtol=0, atol=1e-9)
+
+
+def test_elastic_force_matches_numpy_fft_route():
+    """Independent route: numpy's FFT for every derivative (library routine, double)."""
+    N = 32
+    X, sig = _random_vesicles(6, 3, N)
+    k = np.fft.fftfreq(N, 1.0 / N)
+    k[N // 2] = 0.0                                                     # reading A4
+    D = lambda f: np.real(np.fft.ifft(1j * k[None, :, None] * np.fft.fft(f, axis=1), axis=1))
+    dX = D(X)
+    sa = np.sqrt((dX ** 2).sum(-1, keepdims=True))
+    Xs = dX / sa
+    Xssss = D(D(D(Xs) / sa) / sa) / sa
+    ref = -0.8 * Xssss + D(sig[..., None] * Xs) / sa
+    F = oracle.elastic_force(X, sig, 0.8)
+    assert np.abs(F - ref).max() <= 1e-16 * (N / 2) ** 4 * 64 * np.abs(ref).max()
