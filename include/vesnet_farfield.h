@@ -153,6 +153,23 @@ vn_status vn_farfield_targets(const void *Xt, int64_t nt,
 vn_status vn_elastic_force(const void *X, const void *sigma, int64_t nves, int64_t npts,
                            double kappa_b, void *F, vn_precision precision, void *stream);
 
+/* ---- row f-3: redistributing points equally in arclength ----------------------------------------
+ * PAPER.md:331-335 (sec 4.2), called three times per time step.  Per vesicle:
+ *   1. trigonometric interpolation of X to M = 6 npts nodes ("upsample by a factor of 6");
+ *   2. arclength l_m at those nodes: |dX/dalpha| by Fourier differentiation, integrated through the
+ *      Fourier series of |dX/dalpha| on the fine grid; L = l_M the total length;
+ *   3. for k = 0 .. npts-1: target arclength k L / npts, located in the increasing sequence l_0..l_M,
+ *      Xnew[v,k,:] = linear interpolation of the two upsampled points that bracket it.
+ * (readings R1-R5 state what the paper leaves open: Nyquist handling, spectral
+ * integration, point 0 stays in place, positions interpolated with the same weight as arclength.)
+ * The new points are equispaced in arclength up to the piecewise-linear error of step 3
+ * (relative spacing error about 1e-4 at npts = 128) and lie on the chords of the upsampled
+ * polygon.  X, Xnew: DEVICE pointers, [nves,npts,2] in the call's precision (arithmetic is double
+ * inside); Xnew is overwritten and must not alias X.  3 <= npts <= 512, else VN_ERR_INVALID_ARG.
+ * The arclength sequence is assumed increasing (true whenever the curve is resolved). */
+vn_status vn_redistribute_arclength(const void *X, int64_t nves, int64_t npts, void *Xnew,
+                                    vn_precision precision, void *stream);
+
 /* Profiling aid (bench.py's roofline figure): while enabled, every vn_farfield /
  * vn_farfield_host / vn_farfield_masked / vn_farfield_targets call records a CUDA event pair on its
  * stream around the pair kernel alone (not the pack / finish / correction kernels).  vn_profile_read waits for the recorded events,

@@ -52,6 +52,7 @@ def _load():
         lib.oracle_farfield_masked_subset.argtypes = [d, d, d, i64, i64, ctypes.c_double,
                                                       ctypes.POINTER(i64), i64, u8, d]
         lib.oracle_elastic_force.argtypes = [d, d, i64, i64, ctypes.c_double, d]
+        lib.oracle_redistribute.argtypes = [d, i64, i64, d]
         _lib = lib
     return _lib
 
@@ -187,3 +188,13 @@ def elastic_force(X, sigma, kappa_b=1.0):
     if rc:
         raise ValueError(f"oracle_elastic_force rc={rc}")
     return F
+
+
+def redistribute(X):
+    """Points of every vesicle redistributed equally in arclength (sec 4.2) -> [nves,npts,2]."""
+    X = _c(X); nves, npts, _ = X.shape
+    Xn = np.empty_like(X)
+    rc = _load().oracle_redistribute(_p(X), nves, npts, _p(Xn))
+    if rc:
+        raise ValueError(f"oracle_redistribute rc={rc}")
+    return Xn

@@ -384,3 +384,112 @@ int oracle_elastic_force(const double *X, const double *sigma, int64_t nves, int
     free(ctab); free(stab);
     return fail ? 2 : 0;
 }
+
+/* ---------------------------------------------------------------------------------------------
+ * Row f-3: redistributing the points of a vesicle equally in arclength (sec 4.2).
+ * Step by step, in the paper's order, with DESIGN.md readings R1-R5 where the text is silent:
+ *   1. "we first upsample the membrane points by a factor of 6": trigonometric interpolation of X
+ *      to M = 6 N nodes alpha'_m = 2 pi m / M (an even N keeps its k = N/2 mode as cos(N alpha/2), so
+ *      the interpolant passes through the data; R1).
+ *   2. "we compute arclength {l_k}": sa_m = |dX/dalpha (alpha'_m)| (Fourier derivative, reading A4),
+ *      l(alpha) = int_0^alpha sa by integrating the Fourier series of sa on the fine grid term by
+ *      term, its k = M/2 mode dropped (R2: "the FFT in computing arclength").  l_M = L = 2 pi mean(sa).
+ *   3. "build a piece-wise linear interpolant, and then infer the corresponding alpha~_k for the
+ *      equispaced arclength": targets l~_k = k L / N, k = 0 .. N-1 (point 0 stays where it is; R3);
+ *      "a search in the increasing arclength sequence to locate the interval containing the target
+ *      arclength, then interpolate based on the two endpoints of the interval": the first m with
+ *      l_{m+1} > l~_k, theta = (l~_k - l_m)/(l_{m+1} - l_m), and the new point is the same linear
+ *      interpolation of the two upsampled points, Xnew_k = Xup_m + theta (Xup_{m+1} - Xup_m)   (R4).
+ * Xnew: [nves, npts, 2]. */
+int oracle_redistribute(const double *X, int64_t nves, int64_t npts, double *Xnew)
+{
+    if (!X || !Xnew || nves < 1 || npts < 1) return 1;
+    const int64_t N = npts, M = 6 * npts, K = (N - 1) / 2;
+    ld *cM = (ld *)malloc(sizeof(ld) * (size_t)M), *sM = (ld *)malloc(sizeof(ld) * (size_t)M);
+    ld *cN = (ld *)malloc(sizeof(ld) * (size_t)N), *sN = (ld *)malloc(sizeof(ld) * (size_t)N);
+    if (!cM || !sM || !cN || !sN) { free(cM); free(sM); free(cN); free(sN); return 2; }
+    for (int64_t m = 0; m < M; ++m) { cM[m] = cosl(2.0L * ORACLE_PI * (ld)m / (ld)M); sM[m] = sinl(2.0L * ORACLE_PI * (ld)m / (ld)M); }
+    for (int64_t m = 0; m < N; ++m) { cN[m] = cosl(2.0L * ORACLE_PI * (ld)m / (ld)N); sN[m] = sinl(2.0L * ORACLE_PI * (ld)m / (ld)N); }
+    int fail = 0;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t v = 0; v < nves; ++v) {
+        const double *Xv = X + 2 * v * N;
+        ld *w = (ld *)malloc(sizeof(ld) * (size_t)(4 * (2 * K + 1) + 2 + 4 * M + 1 + 2 * M));
+        if (!w) { fail = 1; continue; }
+        ld *coef = w;                                   /* (re_x, im_x, re_y, im_y) for k = -K..K */
+        ld *nyq = w + 4 * (2 * K + 1);                  /* k = N/2 coefficient of x, y (even N)   */
+        ld *xu = nyq + 2, *yu = xu + M, *sa = yu + M, *l = sa + M;   /* l has M + 1 entries */
+        ld *p = l + M + 1, *q = p + M;                  /* Fourier coefficients of sa             */
+        /* 1. coefficients of X, then the interpolant and its derivative on the fine grid */
+        for (int64_t k = -K; k <= K; ++k) {
+            ld rx = 0.0L, ix = 0.0L, ry = 0.0L, iy = 0.0L;
+            for (int64_t j = 0; j < N; ++j) {
+                int64_t a = (k * j) % N; if (a < 0) a += N;
+                rx += (ld)Xv[2 * j] * cN[a];     ix -= (ld)Xv[2 * j] * sN[a];
+                ry += (ld)Xv[2 * j + 1] * cN[a]; iy -= (ld)Xv[2 * j + 1] * sN[a];
+            }
+            ld *c = coef + 4 * (k + K);
+            c[0] = rx / (ld)N; c[1] = ix / (ld)N; c[2] = ry / (ld)N; c[3] = iy / (ld)N;
+        }
+        nyq[0] = nyq[1] = 0.0L;
+        if (N % 2 == 0) {
+            for (int64_t j = 0; j < N; ++j) {
+                const ld sgn = (j % 2) ? -1.0L : 1.0L;
+                nyq[0] += sgn * (ld)Xv[2 * j]; nyq[1] += sgn * (ld)Xv[2 * j + 1];
+            }
+            nyq[0] /= (ld)N; nyq[1] /= (ld)N;
+        }
+        for (int64_t m = 0; m < M; ++m) {
+            ld x = 0.0L, y = 0.0L, dx = 0.0L, dy = 0.0L;
+            for (int64_t k = -K; k <= K; ++k) {
+                const ld *c = coef + 4 * (k + K);
+                int64_t a = (k * m) % M; if (a < 0) a += M;
+                x += c[0] * cM[a] - c[1] * sM[a];
+                y += c[2] * cM[a] - c[3] * sM[a];
+                dx += (ld)k * (-c[1] * cM[a] - c[0] * sM[a]);
+                dy += (ld)k * (-c[3] * cM[a] - c[2] * sM[a]);
+            }
+            if (N % 2 == 0) {                                   /* cos(N alpha'/2) = cos(2 pi (N/2) m / M) */
+                const int64_t a = ((N / 2) * m) % M;
+                x += nyq[0] * cM[a]; y += nyq[1] * cM[a];
+            }
+            xu[m] = x; yu[m] = y;
+            sa[m] = sqrtl(dx * dx + dy * dy);
+        }
+        /* 2. arclength at the fine nodes by term-by-term integration of the Fourier series of sa */
+        ld s0 = 0.0L;
+        for (int64_t m = 0; m < M; ++m) s0 += sa[m];
+        s0 /= (ld)M;
+        for (int64_t k = 1; k <= M / 2 - 1; ++k) {              /* shat_k = p_k + i q_k */
+            ld pr = 0.0L, qi = 0.0L;
+            for (int64_t m = 0; m < M; ++m) {
+                const int64_t a = (k * m) % M;
+                pr += sa[m] * cM[a]; qi -= sa[m] * sM[a];
+            }
+            p[k] = pr / (ld)M; q[k] = qi / (ld)M;
+        }
+        for (int64_t m = 0; m < M; ++m) {
+            ld acc = s0 * (2.0L * ORACLE_PI * (ld)m / (ld)M);
+            for (int64_t k = 1; k <= M / 2 - 1; ++k) {
+                const int64_t a = (k * m) % M;
+                acc += 2.0L * (p[k] * sM[a] - q[k] * (1.0L - cM[a])) / (ld)k;
+            }
+            l[m] = acc;
+        }
+        const ld L = 2.0L * ORACLE_PI * s0;
+        l[M] = L;
+        /* 3. search + linear interpolation */
+        for (int64_t k = 0; k < N; ++k) {
+            const ld lt = (ld)k * L / (ld)N;
+            int64_t m = 0;
+            while (m < M - 1 && !(l[m + 1] > lt)) ++m;
+            const ld theta = (lt - l[m]) / (l[m + 1] - l[m]);
+            const int64_t m1 = (m + 1) % M;
+            Xnew[2 * (v * N + k) + 0] = (double)(xu[m] + theta * (xu[m1] - xu[m]));
+            Xnew[2 * (v * N + k) + 1] = (double)(yu[m] + theta * (yu[m1] - yu[m]));
+        }
+        free(w);
+    }
+    free(cM); free(sM); free(cN); free(sN);
+    return fail ? 2 : 0;
+}

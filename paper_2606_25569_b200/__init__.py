@@ -14,6 +14,7 @@ raises.
     U = vn_farfield_masked(X, F, W, ptr, ves)   # the paper's DirectSingleLayerIntegral
     Ut = vn_farfield_targets(Xt, X, F, W)       # velocity at free points Xt[nt, 2]
     F = vn_elastic_force(X, sigma, kappa_b)     # eq 2.7, the density the sums above consume
+    Xe = vn_redistribute_arclength(X)           # points equispaced in arclength, sec 4.2
 
 `inputs` (seeded synthetic suspensions) is importable without the library.
 """
@@ -60,6 +61,8 @@ def lib():
         L.vn_farfield_targets.restype = ci
         L.vn_elastic_force.argtypes = [vp, vp, i64, i64, dbl, vp, ci, vp]
         L.vn_elastic_force.restype = ci
+        L.vn_redistribute_arclength.argtypes = [vp, i64, i64, vp, ci, vp]
+        L.vn_redistribute_arclength.restype = ci
         L.vn_profile_enable.argtypes = [ci]
         L.vn_profile_enable.restype = ci
         L.vn_profile_read.argtypes = [ctypes.POINTER(dbl), i64]
@@ -229,6 +232,23 @@ def vn_elastic_force(X, sigma, kappa_b: float = 1.0, out=None, stream=None):
                                     _prec(X), _stream_ptr(stream))
     if rc != VN_OK:
         raise VesnetError(rc, "vn_elastic_force")
+    return out
+
+
+def vn_redistribute_arclength(X, out=None, stream=None):
+    """Points of every vesicle redistributed equally in arclength (sec 4.2; device tensors)."""
+    import torch
+    nves, npts, two = X.shape
+    if two != 2:
+        raise ValueError("X must be [nves, npts, 2]")
+    _check_dev("X", X)
+    if out is None:
+        out = torch.empty_like(X)
+    _check_dev("out", out, X.shape, X.dtype)
+    with torch.cuda.device(X.device):
+        rc = lib().vn_redistribute_arclength(X.data_ptr(), nves, npts, out.data_ptr(), _prec(X), _stream_ptr(stream))
+    if rc != VN_OK:
+        raise VesnetError(rc, "vn_redistribute_arclength")
     return out
 
 

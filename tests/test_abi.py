@@ -22,7 +22,7 @@ def test_library_exports_every_declared_symbol():
     names = _declared()
     assert {"vn_farfield", "vn_arclength_weights", "vn_farfield_host", "vn_status_string",
             "vn_version", "vn_launch_count", "vn_near_pairs", "vn_farfield_masked",
-            "vn_farfield_targets", "vn_elastic_force"} <= set(names)
+            "vn_farfield_targets", "vn_elastic_force", "vn_redistribute_arclength"} <= set(names)
     for n in names:
         assert hasattr(L, n), n
     assert vn.vn_version() >= 100
@@ -61,5 +61,9 @@ def test_argument_validation_needs_no_gpu():
     assert L.vn_elastic_force(p, None, 2, 4, 1.0, q, vn.VN_F64, None) == INV            # null sigma
     assert L.vn_elastic_force(p, p, 2, 1025, 1.0, q, vn.VN_F64, None) == INV            # npts > 1024
     assert L.vn_elastic_force(p, p, 2, 4, float("inf"), q, vn.VN_F64, None) == INV      # kappa_b not finite
+    assert L.vn_redistribute_arclength(None, 2, 4, q, vn.VN_F64, None) == INV
+    assert L.vn_redistribute_arclength(p, 2, 2, q, vn.VN_F64, None) == INV               # npts < 3
+    assert L.vn_redistribute_arclength(p, 2, 513, q, vn.VN_F64, None) == INV             # npts > 512
+    assert L.vn_redistribute_arclength(p, 2, 4, p, vn.VN_F64, None) == INV               # in place
     assert L.vn_farfield_host(p, None, None, 2, 4, 1.0, q, vn.VN_F64) == INV
     assert L.vn_farfield_host(p, p, None, 2, 4, -1.0, q, vn.VN_F64) == INV

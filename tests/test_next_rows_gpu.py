@@ -363,3 +363,63 @@ def test_elastic_force_rejects_long_vesicles_and_feeds_farfield():
     Fo = oracle.elastic_force(s.X, sig.cpu().numpy(), 0.5)
     ref = oracle.farfield(s.X, Fo, oracle.weights(s.X), s.mu)
     assert rel_l2(Ud.cpu().numpy(), ref) <= force_tol(s.npts, np.float64)
+
+
+# ------------------------------------------------------------------------------------- equal-arclength redistribution (row f-3)
+def shape_err(got, ref):
+    """Error relative to the size of the vesicles (not to their position in the box)."""
+    c = ref.mean(1, keepdims=True)
+    return float(np.linalg.norm(got - ref) / np.linalg.norm(ref - c))
+
+
+def redistribute_tol(X, dtype):
+    """fp64: 1e-12.  fp32: the result is rounded to float at box coordinates, 2^-24 max|X| per coordinate,
+    measured here against the vesicle size; at least north_star's 2e-5."""
+    if dtype == np.float64:
+        return 1e-12
+    size = np.sqrt(((X - X.mean(1, keepdims=True)) ** 2).sum(-1).mean())
+    return max(2e-5, 2.0 ** -24 * np.abs(X).max() / size)
+
+
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+@pytest.mark.parametrize("index", [0, 1, 3])
+def test_redistribute_parity(index, dtype):
+    s = inputs.config(index)
+    X = s.X if index < 3 else s.X[:500]                         # the oracle is O((6N)^2) per vesicle
+    ref = oracle.redistribute(stored(X, dtype))
+    got = vn.vn_redistribute_arclength(dev(X, dtype))
+    torch.cuda.synchronize()
+    err = shape_err(got.cpu().numpy().astype(np.float64), ref)
+    W0, W1 = oracle.weights(stored(X, dtype)), oracle.weights(got.cpu().numpy().astype(np.float64))
+    print(f"redistribute config{index} {np.dtype(dtype).name}: shape-relative L2 {err:.3e} (tolerance {redistribute_tol(X, dtype):.1e}); "
+          f"max/min spacing {np.max(W0.max(1) / W0.min(1)):.3f} -> {np.max(W1.max(1) / W1.min(1)):.4f}")
+    assert err <= redistribute_tol(X, dtype)
+
+
+@pytest.mark.parametrize("npts", [3, 4, 5, 8, 31, 33, 100, 129, 257, 512])
+def test_redistribute_edge_shapes(npts):
+    rng = np.random.Generator(np.random.PCG64(npts))
+    al = 2 * np.pi * np.arange(npts) / npts
+    be = al + 0.3 * np.sin(al + rng.uniform(0, 6.28, size=(4, 1)))
+    r = 1.0 + (0.2 if npts >= 8 else 0.0) * np.cos(2 * be)
+    X = np.stack([r * np.cos(be), 0.7 * r * np.sin(be)], -1) + 10.0 * rng.normal(size=(4, 1, 2))
+    ref = oracle.redistribute(X)
+    got = vn.vn_redistribute_arclength(dev(X, np.float64))
+    torch.cuda.synchronize()
+    assert shape_err(got.cpu().numpy(), ref) <= 1e-12
+
+
+def test_redistribute_rejects_bad_sizes_and_chains():
+    with pytest.raises(vn.VesnetError):
+        vn.vn_redistribute_arclength(torch.zeros((1, 2, 2), device="cuda", dtype=torch.float64))
+    with pytest.raises(vn.VesnetError):
+        vn.vn_redistribute_arclength(torch.zeros((1, 513, 2), device="cuda", dtype=torch.float64))
+    # redistribute -> weights -> far field on one stream equals the oracle's chain
+    s = inputs.config(0)
+    Xd = vn.vn_redistribute_arclength(dev(s.X, np.float64))
+    Wd = vn.vn_arclength_weights(Xd)
+    Ud = vn.vn_farfield(Xd, dev(s.F, np.float64), Wd, s.mu)
+    torch.cuda.synchronize()
+    Xo = oracle.redistribute(s.X)
+    ref = oracle.farfield(Xo, s.F, oracle.weights(Xo), s.mu)
+    assert rel_l2(Ud.cpu().numpy(), ref) <= 1e-12

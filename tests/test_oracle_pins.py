@@ -424,3 +424,101 @@ def test_elastic_force_matches_numpy_fft_route():
     ref = -0.8 * Xssss + D(sig[..., None] * Xs) / sa
     F = oracle.elastic_force(X, sig, 0.8)
     assert np.abs(F - ref).max() <= 1e-16 * (N / 2) ** 4 * 64 * np.abs(ref).max()
+
+
+# ----------------------------------------------------------------------------- equal-arclength redistribution (row f-3)
+def _np_redistribute(X):
+    """Independent route through numpy's FFT, searchsorted and interp (library routines, double)."""
+    nves, N, _ = X.shape
+    M = 6 * N
+    out = np.empty_like(X)
+    k = np.fft.fftfreq(N, 1.0 / N)
+    for v in range(nves):
+        Xh = np.fft.fft(X[v], axis=0) / N
+        pad = np.zeros((M, 2), dtype=complex)
+        K = (N - 1) // 2
+        pad[:K + 1] = Xh[:K + 1]
+        pad[M - K:] = Xh[N - K:]
+        dpad = pad * (1j * np.fft.fftfreq(M, 1.0 / M))[:, None]          # Nyquist mode not in it (reading A4)
+        if N % 2 == 0:                                                    # cos(N alpha / 2): split over +-N/2
+            pad[N // 2] = Xh[N // 2] / 2
+            pad[M - N // 2] = Xh[N // 2] / 2
+        Xu = np.real(np.fft.ifft(pad, axis=0)) * M
+        dXu = np.real(np.fft.ifft(dpad, axis=0)) * M
+        sa = np.sqrt((dXu ** 2).sum(1))
+        sh = np.fft.fft(sa) / M
+        kk = np.fft.fftfreq(M, 1.0 / M)
+        ih = np.zeros(M, dtype=complex)
+        nz = (kk != 0) & (np.abs(kk) != M // 2)
+        ih[nz] = sh[nz] / (1j * kk[nz])
+        prim = np.real(np.fft.ifft(ih)) * M
+        al = 2 * np.pi * np.arange(M) / M
+        l = np.real(sh[0]) * al + prim - prim[0]
+        L = 2 * np.pi * np.real(sh[0])
+        l = np.append(l, L)
+        lt = np.arange(N) * L / N
+        Xc = np.vstack([Xu, Xu[:1]])
+        out[v, :, 0] = np.interp(lt, l, Xc[:, 0])
+        out[v, :, 1] = np.interp(lt, l, Xc[:, 1])
+    return out
+
+
+def test_redistribute_fixed_point_and_warped_circle():
+    """A circle sampled equally in arclength is a fixed point.  The same circle sampled at beta = alpha +
+    0.4 sin(alpha) comes back equispaced in angle (the piecewise-linear error of the 6x-upsampled
+    polygon is O((2 pi / 6N)^2)), on the chords of that polygon, with point 0 exactly where it was."""
+    N, R = 32, 0.8
+    al = 2 * np.pi * np.arange(N) / N
+    X = R * np.stack([np.cos(al), np.sin(al)], -1)[None] + np.array([1.0, 2.0])
+    assert np.abs(oracle.redistribute(X) - X).max() <= 2e-15
+    be = al + 0.4 * np.sin(al)
+    Xw = R * np.stack([np.cos(be), np.sin(be)], -1)[None]
+    Y = oracle.redistribute(Xw)[0]
+    assert np.abs(Y[0] - Xw[0, 0]).max() <= 1e-16
+    ang = np.unwrap(np.arctan2(Y[:, 1], Y[:, 0]))
+    assert np.abs(ang - al).max() <= 5e-6
+    rad = np.hypot(Y[:, 0], Y[:, 1])
+    sag = R * (1 - np.cos(1.4 * np.pi / (6 * N)))            # largest chord sag: fine spacing stretched by <= 1.4
+    assert np.all(rad <= R + 1e-12) and np.all(rad >= R - sag * 1.01)
+    # reversed orientation gives the mirrored answer; a wrong sign in the integration would not
+    rev = np.concatenate([[0], np.arange(N - 1, 0, -1)])
+    assert np.allclose(oracle.redistribute(Xw[:, rev])[0][rev], Y, rtol=0, atol=1e-13)
+
+
+def test_redistribute_matches_numpy_route_and_equalises_spacing():
+    for N in (31, 32, 64):
+        X, _ = _random_vesicles(11 + N, 3, N)
+        # make the sampling uneven in arclength on purpose
+        al = 2 * np.pi * np.arange(N) / N
+        be = al + 0.5 * np.sin(al + 0.3)
+        kk = np.arange(-(N // 2) + 1, N // 2)
+        Xh = np.array([[np.exp(-1j * k * al) @ X[v] / N for k in kk] for v in range(3)])
+        Xw = np.real(np.einsum("jk,vkc->vjc", np.exp(1j * np.outer(be, kk)), Xh))
+        Y = oracle.redistribute(Xw)
+        assert np.abs(Y - _np_redistribute(Xw)).max() <= 1e-12
+        W0, W1 = oracle.weights(Xw), oracle.weights(Y)
+        assert (W0.max(1) / W0.min(1)).min() > 2.0                       # uneven before
+        if N >= 32:
+            assert (W1.max(1) / W1.min(1)).max() < 1.05                  # even after
+        # the perimeter is preserved up to the chord sag
+        assert np.allclose(W1.sum(1), W0.sum(1), rtol=2e-3)
+
+
+def test_redistribute_equivariances():
+    N = 32
+    X, _ = _random_vesicles(21, 3, N)
+    Y = oracle.redistribute(X)
+    th = 0.7
+    R = np.array([[np.cos(th), -np.sin(th)], [np.sin(th), np.cos(th)]])
+    assert np.allclose(oracle.redistribute(X + np.array([5.0, -9.0])), Y + np.array([5.0, -9.0]), rtol=0, atol=1e-13)
+    assert np.allclose(oracle.redistribute(X @ R.T), Y @ R.T, rtol=0, atol=1e-13)
+    assert np.allclose(oracle.redistribute(2.5 * X), 2.5 * Y, rtol=0, atol=1e-13)
+    assert np.array_equal(oracle.redistribute(X[1:2])[0], Y[1])
+    # cyclic relabelling of the input points: the new point 0 follows the old point 0, the curve does not change,
+    # so the new points are the same polygon's equal-arclength points started elsewhere -- still equispaced
+    W = oracle.weights(oracle.redistribute(np.roll(X, 5, axis=1)))
+    assert (W.max(1) / W.min(1)).max() < 1.05
+    # almost idempotent: a second pass moves the points by much less than the first
+    d1 = np.abs(Y - X).max()
+    d2 = np.abs(oracle.redistribute(Y) - Y).max()
+    assert d2 < 2e-2 * d1
