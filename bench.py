@@ -196,6 +196,100 @@ def workload_config(args, susp, note=""):
             "note": note}
 
 
+def run_aux(args, susp, vn, torch, tdtype, np_dtype, rank, world, local_rank):
+    """--path aux: a step = vn_redistribute_arclength -> vn_arclength_weights -> vn_elastic_force on the
+    workload's vesicles (rows f-3, a-1, f-2: everything O(P) that surrounds the pair sum in a time step).
+    Reported in membrane points per second; the roofline object describes the dominant kernel
+    (redistribute_kernel, FP64 pipe; algorithmic DFMA count per vesicle stated in DESIGN.md section 11)."""
+    from paper_2606_25569_b200 import multi
+    import oracle
+    P = susp.nves * susp.npts
+    X_h = torch.from_numpy(np.ascontiguousarray(susp.X, dtype=np_dtype)).pin_memory()
+    sig_h = torch.ones((susp.nves, susp.npts), dtype=tdtype).pin_memory()
+    X_d, sig_d = X_h.cuda(), sig_h.cuda()
+    Xe_d, F_d = torch.empty_like(X_d), torch.empty_like(X_d)
+    W_d = torch.empty((susp.nves, susp.npts), dtype=tdtype, device="cuda")
+    F_host = torch.empty_like(X_h).pin_memory()
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    parts = {"redistribute": [], "weights": [], "elastic_force": []}
+
+    def step(record):
+        e = [ev() for _ in range(4)]
+        e[0].record()
+        vn.vn_redistribute_arclength(X_d, out=Xe_d)
+        e[1].record()
+        vn.vn_arclength_weights(Xe_d, out=W_d)
+        e[2].record()
+        vn.vn_elastic_force(Xe_d, sig_d, 1.0, out=F_d)
+        e[3].record()
+        if record:
+            e[3].synchronize()
+            for k, name in enumerate(parts):
+                parts[name].append(e[k].elapsed_time(e[k + 1]))
+
+    for _ in range(max(args.warmup, 3)):
+        step(False)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(nvml_index(local_rank))
+    sampler.start()
+    n0 = vn.vn_launch_count()
+    t_dev = 0.0
+    for _ in range(args.steps):
+        flush.fill_(1)
+        multi.barrier(); torch.cuda.synchronize()
+        e0, e1 = ev(), ev()
+        e0.record(); step(True); e1.record(); e1.synchronize()
+        t_dev += e0.elapsed_time(e1) * 1e-3
+    launches = vn.vn_launch_count() - n0
+    t_e2e = 0.0
+    for _ in range(args.steps):
+        multi.barrier(); torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        X_d.copy_(X_h, non_blocking=True); sig_d.copy_(sig_h, non_blocking=True)
+        step(False)
+        F_host.copy_(F_d, non_blocking=True)
+        torch.cuda.synchronize()
+        t_e2e += time.perf_counter() - t0
+    sampler.stop_flag.set(); sampler.join()
+    rate, t_dev, _ = multi.whole_job_rate(args.steps * P, t_dev, "cuda")
+    rate_e2e, t_e2e, _ = multi.whole_job_rate(args.steps * P, t_e2e, "cuda")
+    if rank != 0:
+        return
+    N, M = susp.npts, 6 * susp.npts
+    K, H = (N - 1) // 2, M // 2 - 1
+    dfma_per_ves = 4 * (K + 1) * N + 8 * K * M + 2 * (H + 1) * M + 2 * H * M      # steps 1a, 1b, 2b, 2c
+    k_ms = statistics.mean(parts["redistribute"])
+    clocks = sampler.summary()
+    sm_max = clocks.get("sm_max_mhz") or 1965.0
+    peak = SMS * FP64_LANES * sm_max * 1e6 / 1e12
+    achieved = dfma_per_ves * susp.nves / (k_ms * 1e-3) / 1e12
+    es = 4 if args.precision == "f32" else 8
+    line = {"metric": "membrane points/s through redistribution + weights + elastic force", "value": rate,
+            "unit": "points/s", "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "ms_per_step": t_dev / args.steps * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"BASELINE.json configs[{args.workload}]: {susp.name}", "path": "rows f-3, a-1, f-2",
+                       "nves": susp.nves, "npts": susp.npts, "storage": args.precision,
+                       "l2": "flushed between timed steps (256 MiB write)"},
+            "clocks": clocks, "gpu_launches": int(launches),
+            "kernel_ms": {k: statistics.mean(v) for k, v in parts.items()},
+            "roofline": {"bound": "alu", "kernel": "redistribute_kernel", "achieved": achieved, "peak": peak,
+                         "unit": "T DFMA lane-instr/s (FP64 pipe)", "frac": achieved / peak,
+                         "peak_source": "derived: 148 SMs x 64 lanes x %.0f MHz" % sm_max,
+                         "dfma_per_vesicle": dfma_per_ves, "traffic": None},
+            "e2e": {"value": rate_e2e, "unit": "points/s", "h2d_bytes_per_step": 3 * es * P, "d2h_bytes_per_step": 2 * es * P}}
+    if world == 1 and not args.no_cpu_baseline:
+        Xo = np.asarray(susp.X, dtype=np_dtype).astype(np.float64)
+        nv = min(susp.nves, 64)
+        t0 = time.perf_counter()
+        Xe = oracle.redistribute(Xo[:nv]); oracle.weights(Xe); oracle.elastic_force(Xe, np.ones((nv, susp.npts)), 1.0)
+        dt = time.perf_counter() - t0
+        line["cpu_baseline"] = {"value": nv * susp.npts / dt, "unit": "points/s", "cores": oracle.num_threads(),
+                                "kind": "oracle", "sample": f"first {nv} vesicles ({dt:.1f} s)"}
+    print(json.dumps(line), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -204,9 +298,11 @@ def main():
     ap.add_argument("--workload", type=int, default=4, choices=[0, 1, 2, 3, 4])
     ap.add_argument("--precision", default="f32", choices=["f32", "f64"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--path", default="farfield", choices=["farfield", "masked", "targets"],
+    ap.add_argument("--path", default="farfield", choices=["farfield", "masked", "targets", "aux"],
                     help="farfield: rows a-1..a-5 (the headline); masked: row f-1 (vn_near_pairs + "
-                         "vn_farfield_masked); targets: row f-4 (vn_farfield_targets on a 512x512 grid)")
+                         "vn_farfield_masked); targets: row f-4 (vn_farfield_targets on a 512x512 grid); "
+                         "aux: the O(P) rows around the sum (f-3 redistribution, a-1 weights, f-2 elastic force), "
+                         "reported in points/s")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -233,6 +329,8 @@ def main():
     tdtype = torch.float32 if args.precision == "f32" else torch.float64
     np_dtype = np.float32 if args.precision == "f32" else np.float64
     susp = make_workload(args.workload, rank)
+    if args.path == "aux":
+        return run_aux(args, susp, vn, torch, tdtype, np_dtype, rank, world, local_rank)
     seq_np = susp.X_sequence if susp.X_sequence else [susp.X]
     evals = len(seq_np)
     P = susp.nves * susp.npts
