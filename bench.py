@@ -256,9 +256,8 @@ def run_aux(args, susp, vn, torch, tdtype, np_dtype, rank, world, local_rank):
     rate_e2e, t_e2e, _ = multi.whole_job_rate(args.steps * P, t_e2e, "cuda")
     if rank != 0:
         return
-    N, M = susp.npts, 6 * susp.npts
-    K, H = (N - 1) // 2, M // 2 - 1
-    dfma_per_ves = 4 * (K + 1) * N + 8 * K * M + 2 * (H + 1) * M + 2 * H * M      # steps 1a, 1b, 2b, 2c
+    N = susp.npts
+    dfma_per_ves = 24 * N * N + 36 * N * N      # interpolant + derivative (4 x 6N x N), integration (6N x 6N)
     k_ms = statistics.mean(parts["redistribute"])
     clocks = sampler.summary()
     sm_max = clocks.get("sm_max_mhz") or 1965.0
@@ -281,7 +280,7 @@ def run_aux(args, susp, vn, torch, tdtype, np_dtype, rank, world, local_rank):
             "e2e": {"value": rate_e2e, "unit": "points/s", "h2d_bytes_per_step": 3 * es * P, "d2h_bytes_per_step": 2 * es * P}}
     if world == 1 and not args.no_cpu_baseline:
         Xo = np.asarray(susp.X, dtype=np_dtype).astype(np.float64)
-        nv = min(susp.nves, 64)
+        nv = min(susp.nves, 4000)
         t0 = time.perf_counter()
         Xe = oracle.redistribute(Xo[:nv]); oracle.weights(Xe); oracle.elastic_force(Xe, np.ones((nv, susp.npts)), 1.0)
         dt = time.perf_counter() - t0
