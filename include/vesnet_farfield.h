@@ -35,9 +35,10 @@
  *                          fallback of any kind, by design)
  *      VN_ERR_CUDA         a CUDA runtime call failed (allocation, launch)
  *    Argument checks happen before any CUDA call, so they work without a GPU.
- *  - VN_F32 shares one SFU reciprocal between two pairs (t = rcp(a*b), 1/a = t*b): squared
- *    distances must keep a*b inside the fp32 normal range, i.e. 1e-9 < |r| < 1e9 in the
- *    caller's units.  VN_F64 has no such restriction beyond normal doubles.
+ *  - VN_F32 uses the SFU approximations rcp/lg2 (flush-to-zero): squared distances must be normal
+ *    fp32 numbers, and vn_farfield_targets additionally shares one reciprocal between two pairs
+ *    (t = rcp(a*b), 1/a = t*b), which needs a*b inside the fp32 normal range, i.e.
+ *    1e-9 < |r| < 1e9 in the caller's units.  VN_F64 needs normal doubles whose reciprocal is normal.
  *  - Input values are not validated: NaN/Inf propagate.  Points of DIFFERENT vesicles
  *    are assumed distinct; a coincident cross-vesicle pair gives an unspecified (possibly
  *    non-finite) value at that target only (reading A5).  nves == 1 is valid and yields U == 0.

