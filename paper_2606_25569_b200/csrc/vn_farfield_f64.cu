@@ -33,7 +33,8 @@ constexpr int kSub64 = kST64 / kTile;         // source tiles per super-tile: 4
 #define VN_F64_MINTILES 8
 #endif
 constexpr int kBatch64 = VN_F64_BATCH;        // sources per cross-lane reduction batch
-constexpr int kLogTab = 1025;                 // (1/2) ln(rc) for the 10-bit reciprocals rc in [1/2, 1]
+constexpr int kLogTab = 1024;                 // (1/2) ln of the 10-bit mantissas 1 + k/1024
+constexpr int kExpTab = 2048;                 // (1/2) ln2 (E - 1023) for every exponent field
 
 // a-2: one 32-byte record (yx, yy, gx, gy) per source, g = F*W; also gmax = max_j (|gx| + |gy|)
 // (the bit pattern of a non-negative double orders like the double).
@@ -57,37 +58,41 @@ __global__ void pack_sources_f64(const double2 *__restrict__ X, const double2 *_
     if ((threadIdx.x & 31) == 0 && m != 0.0) atomicMax(gmax_bits, (unsigned long long)__double_as_longlong(m));
 }
 
-// -(1/2) ln(r2) and 1/r2 in double, 9 DP instructions + one MUFU.RCP64H + one I2F + one 8-byte
-// shared-memory load.  r2 = m 2^e with m in [1, 2).
-//   t0  = hardware reciprocal seed of m (2^-20 accurate);  1/m = t0 (1 + d + d^2), d = 1 - m t0  (cubic step)
-//   rc  = t0 rounded to 10 mantissa bits, eps = m rc - 1 (one fma; |eps| <= 2^-11 + 2^-19)
-//   ln m = -ln rc + log1p(eps),  log1p by its series through eps^4 (next term <= 6e-18), Horner
-//   tab[k] = (1/2) ln(rc_k), rc_k = 1/2 + k/2048 (k = 0 .. 1024), built by every block at start-up
+// -(1/2) ln(r2) and 1/r2 in double: 9 DP instructions + one MUFU.RCP64H + two 8-byte shared-memory loads,
+// no exponent/mantissa surgery on r2 and no integer-to-double conversion (I2F.F64 occupies the FP64 pipe).
+//   t0  = hardware reciprocal seed of r2 (2^-20 accurate, full exponent range)
+//   1/r2 = t0 (1 + d + d^2), d = 1 - r2 t0                                     (one cubic step, 3 DP)
+//   rc  = t0 rounded to 10 mantissa bits = 2^(E-1023) (1 + k/1024);  eps = r2 rc - 1 (one fma; |eps| <= 2^-11 + 2^-19)
+//   -(1/2) ln r2 = (1/2) ln rc - (1/2) log1p(eps),  log1p by its series through eps^4 (next term <= 6e-18), Horner
+//   (1/2) ln rc = tabE[E] + tab[k]:  tab[k] = (1/2) ln(1 + k/1024), tabE[E] = (1/2) ln2 (E - 1023) for every
+//   exponent field E = 0 .. 2047; both built by every block at start-up (24 KB of shared memory).
 // r2 must be a positive normal double whose reciprocal is normal too (the header's precondition).
 __device__ __forceinline__ void log_rcp_f64(double r2, const double *__restrict__ tab, double &mhalf_log, double &inv)
 {
-    const int hi = __double2hiint(r2);
-    const int lo = __double2loint(r2);
-    const int e = (hi >> 20) - 1023;
-    const double m = __hiloint2double((hi & 0x000fffff) | 0x3ff00000, lo);
     double t0;
-    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(t0) : "d"(m));                 // MUFU.RCP64H: 1/m in (1/2, 1]
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(t0) : "d"(r2));                // MUFU.RCP64H
     const int rch = (__double2hiint(t0) + 0x200) & 0xfffffc00;              // round to 10 mantissa bits
     const double rc = __hiloint2double(rch, 0);
-    const double half_ln_rc = tab[(rch - 0x3fe00000) >> 10];
+    const int k = (rch >> 10) & 0x3ff;
+    const double base = tab[kLogTab + (rch >> 20)] + tab[k];
     // reciprocal
-    const double d = fma(-m, t0, 1.0);
+    const double d = fma(-r2, t0, 1.0);
     const double p = fma(d, d, d);
-    const double t = fma(t0, p, t0);
-    inv = __hiloint2double(__double2hiint(t) - (e << 20), __double2loint(t));   // 2^-e / m
-    // logarithm: -(1/2) ln r2 = -(1/2) e ln2 + (1/2) ln rc - (1/2) log1p(eps)
-    const double eps = fma(m, rc, -1.0);
+    inv = fma(t0, p, t0);
+    // logarithm
+    const double eps = fma(r2, rc, -1.0);
     double q = 0.125;                                  // -(1/2) (1 - eps/2 + eps^2/3 - eps^3/4)
     q = fma(q, eps, -1.0 / 6.0);
     q = fma(q, eps, 0.25);
     q = fma(q, eps, -0.5);
-    const double base = fma((double)e, -0.34657359027997265471, half_ln_rc);
     mhalf_log = fma(eps, q, base);
+}
+
+// the two tables of log_rcp_f64, consecutive in shared memory: tab[0 .. kLogTab) and tabE[0 .. kExpTab)
+__device__ __forceinline__ void build_log_tables(double *tab, int tid, int nthreads)
+{
+    for (int k = tid; k < kLogTab; k += nthreads) tab[k] = 0.5 * log1p((double)k * (1.0 / 1024.0));
+    for (int i = tid; i < kExpTab; i += nthreads) tab[kLogTab + i] = 0.34657359027997265471 * (double)(i - 1023);
 }
 
 // a-3 / a-4: pair kernel; block (I, c) = super-tile I as targets x chunk c of I's list of source tiles
@@ -104,7 +109,7 @@ farfield_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__
     __shared__ __align__(128) double4 tile[kStages][kTile];
     __shared__ __align__(8) u64 full_bar[kStages];
     __shared__ __align__(8) u64 empty_bar[kStages];
-    __shared__ double tab[kLogTab];
+    __shared__ double tab[kLogTab + kExpTab];
 
     const int tid = threadIdx.x;
     const int lane = tid & 31;
@@ -131,7 +136,7 @@ farfield_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__
         }
         mbar_fence_init();
     }
-    for (int k = tid; k < kLogTab; k += kThreads) tab[k] = 0.5 * log(0.5 + (double)k * (1.0 / 2048.0));
+    build_log_tables(tab, tid, kThreads);
     __syncthreads();
 
     auto issue = [&](int i) {   // one thread: list entry u_begin + i -> stage i % kStages
@@ -351,7 +356,7 @@ targets_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__ 
     __shared__ __align__(128) double4 tile[kStages][kTile];
     __shared__ __align__(8) u64 full_bar[kStages];
     __shared__ __align__(8) u64 empty_bar[kStages];
-    __shared__ double tab[kLogTab];
+    __shared__ double tab[kLogTab + kExpTab];
 
     const int tid = threadIdx.x;
     const int tb = blockIdx.x / n_chunks;
@@ -367,7 +372,7 @@ targets_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__ 
         }
         mbar_fence_init();
     }
-    for (int k = tid; k < kLogTab; k += kThreads) tab[k] = 0.5 * log(0.5 + (double)k * (1.0 / 2048.0));
+    build_log_tables(tab, tid, kThreads);
     __syncthreads();
 
     auto issue = [&](int i) {
