@@ -137,6 +137,22 @@ vn_status vn_farfield_targets(const void *Xt, int64_t nt,
                               int64_t nves, int64_t npts, double mu,
                               void *Ut, vn_precision precision, void *stream);
 
+/* ---- row f-4, second half: the far-field sum by a fast multipole method -----------------------
+ * The same quantity as vn_farfield (own vesicle excluded, same conventions), computed in O(P) by the
+ * 2-D fast multipole method the paper points to as future work ("Applying the fast multipole method
+ * ... will make it scale as O(M), but an applicable GPU implementation is beyond the scope of this
+ * paper"; Greengard & Rokhlin 1987 cited PAPER.md:173).  It is an APPROXIMATION:
+ * `order` = p, the number of terms kept in the multipole / local expansions (2 <= p <= 48); the
+ * relative L2 truncation error falls like 0.45^p (measured on the synthetic suspensions: p = 12
+ * about 3e-6, p = 20 about 5e-9, p = 38 about 1e-13); vn_farfield stays the exact path.
+ * Arithmetic is double inside for both storage precisions, so the VN_F32 result is the double
+ * result rounded once.  Uniform quadtree over the bounding square of the points; a strongly
+ * non-uniform point distribution costs time (crowded leaves), not accuracy.  Results are bitwise
+ * reproducible.  Scratch: about 100 * (p+1) bytes per leaf box plus 100 bytes per point. */
+vn_status vn_farfield_fmm(const void *X, const void *F, const void *W,
+                          int64_t nves, int64_t npts, double mu, int order,
+                          void *U, vn_precision precision, void *stream);
+
 /* ---- row f-2: the elastic membrane force (the producer of F) -----------------------------------
  * PAPER.md:123 eq 2.7, :319 Fig. 5b:
  *

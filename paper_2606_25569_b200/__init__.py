@@ -15,6 +15,7 @@ raises.
     Ut = vn_farfield_targets(Xt, X, F, W)       # velocity at free points Xt[nt, 2]
     F = vn_elastic_force(X, sigma, kappa_b)     # eq 2.7, the density the sums above consume
     Xe = vn_redistribute_arclength(X)           # points equispaced in arclength, sec 4.2
+    U = vn_farfield_fmm(X, F, W, order=12)      # the same sum in O(P) by a fast multipole method (approximate)
 
 `inputs` (seeded synthetic suspensions) is importable without the library.
 """
@@ -63,6 +64,8 @@ def lib():
         L.vn_elastic_force.restype = ci
         L.vn_redistribute_arclength.argtypes = [vp, i64, i64, vp, ci, vp]
         L.vn_redistribute_arclength.restype = ci
+        L.vn_farfield_fmm.argtypes = [vp, vp, vp, i64, i64, dbl, ci, vp, ci, vp]
+        L.vn_farfield_fmm.restype = ci
         L.vn_profile_enable.argtypes = [ci]
         L.vn_profile_enable.restype = ci
         L.vn_profile_read.argtypes = [ctypes.POINTER(dbl), i64]
@@ -120,6 +123,26 @@ def vn_farfield(X, F, W, mu: float = 1.0, out=None, stream=None):
                                out.data_ptr(), _prec(X), _stream_ptr(stream))
     if rc != VN_OK:
         raise VesnetError(rc, "vn_farfield")
+    return out
+
+
+def vn_farfield_fmm(X, F, W, mu: float = 1.0, order: int = 12, out=None, stream=None):
+    """The far-field sum by the fast multipole method with `order` expansion terms (approximate, O(P))."""
+    import torch
+    nves, npts, two = X.shape
+    if two != 2:
+        raise ValueError("X must be [nves, npts, 2]")
+    _check_dev("X", X)
+    _check_dev("F", F, X.shape, X.dtype)
+    _check_dev("W", W, (nves, npts), X.dtype)
+    if out is None:
+        out = torch.empty_like(X)
+    _check_dev("out", out, X.shape, X.dtype)
+    with torch.cuda.device(X.device):
+        rc = lib().vn_farfield_fmm(X.data_ptr(), F.data_ptr(), W.data_ptr(), nves, npts, float(mu), int(order),
+                                   out.data_ptr(), _prec(X), _stream_ptr(stream))
+    if rc != VN_OK:
+        raise VesnetError(rc, "vn_farfield_fmm")
     return out
 
 

@@ -57,6 +57,11 @@ struct SymSplit {
 };
 SymSplit choose_sym_split(long long P, int super_tile, int slots, int min_tiles);
 
+// exclusive scan of int counts into 64-bit offsets (kernels in vn_near.cu, also used by vn_fmm.cu)
+constexpr int kScanThreads = 256;
+constexpr int kScanItems = 4;
+constexpr int kScanBlock = kScanThreads * kScanItems;
+
 // ---------------------------------------------------------------------------------------------
 // shared-memory / mbarrier / bulk-copy PTX
 __device__ __forceinline__ uint32_t smem_u32(const void *p)

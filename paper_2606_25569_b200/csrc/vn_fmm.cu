@@ -1,0 +1,630 @@
+// vn_fmm.cu -- row f-4 (second half) of DESIGN.md: the far-field sum by a fast multipole method, O(P) instead
+// of O(P^2).  The paper names it as the missing piece: "Applying the fast multipole method will significantly
+// reduce the cost and make it scale as O(M), but an applicable GPU implementation is beyond the scope of this
+// paper" (PAPER.md:451; :173 for the trapezoid rule + FMM setting).  It is an APPROXIMATION of vn_farfield
+// with a controlled truncation error (expansion order p), not a replacement of the exact path.
+//
+// In complex notation z = x + i y, g = gx + i gy, r = z - zeta_j, the 2-D Stokeslet sum is
+//   u(z) = sum_j [ -log|r| g_j + g_j/2 + (r / conj r) conj(g_j) / 2 ]
+//        = -( Re Phi1 + i Re Phi2 ) + (z/2) conj( Phi1' + i Phi2' ) - (1/2) conj( psi ),
+//   Phi_m(z) = sum_j g_{m,j} log(z - zeta_j)  (m = 1, 2: the real and imaginary parts of g as real charges),
+//   psi(z)   = sum_j ( conj(zeta_j) g_j / (z - zeta_j) - conj(g_j) ),
+// i.e. two complex logarithmic potentials and one Cauchy sum, all analytic away from the sources, so the classic
+// 2-D FMM applies (Greengard & Rokhlin 1987, cited PAPER.md:173): uniform quadtree with L levels over the bounding
+// square, power moments about box centres scaled by the box size, M2M / M2L / L2L in scaled variables, local
+// expansions evaluated at the targets, direct sums over the 3 x 3 neighbour boxes.  The target's own vesicle is
+// excluded as in vn_farfield: the direct part skips it, and what the expansions included of it (own-vesicle
+// points in non-neighbour boxes) is subtracted by a short direct sum.  All arithmetic is double for both storage
+// precisions; the accuracy is set by p (truncation error about 0.45^p relative, measured).
+#include "vn_common.cuh"
+#include "vn_log64.cuh"
+
+namespace vn {
+
+// scan kernels of vn_near.cu (exclusive scan of int counts into 64-bit offsets)
+__global__ void scan_block_sums(const int *__restrict__ cnt, int P, long long *__restrict__ bsum);
+__global__ void scan_of_sums(long long *__restrict__ bsum, int nb);
+__global__ void scan_apply(const int *__restrict__ cnt, int P, const long long *__restrict__ bsum,
+                           long long *__restrict__ ptr, long long *__restrict__ cursor);
+
+// ------------------------------------------------------------------------------------------------
+// complex helpers (double2 = re, im)
+typedef double2 cplx;
+__device__ __forceinline__ cplx cmul(cplx a, cplx b) { return make_double2(fma(a.x, b.x, -a.y * b.y), fma(a.x, b.y, a.y * b.x)); }
+__device__ __forceinline__ cplx cfma(cplx a, cplx b, cplx c)   // a*b + c
+{
+    return make_double2(fma(a.x, b.x, fma(-a.y, b.y, c.x)), fma(a.x, b.y, fma(a.y, b.x, c.y)));
+}
+__device__ __forceinline__ cplx cadd(cplx a, cplx b) { return make_double2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ cplx cscale(cplx a, double s) { return make_double2(a.x * s, a.y * s); }
+__device__ __forceinline__ cplx crcp(cplx a) { const double d = 1.0 / (a.x * a.x + a.y * a.y); return make_double2(a.x * d, -a.y * d); }
+
+// ------------------------------------------------------------------------------------------------
+// geometry: bounding square of all points, kept on the device as four order-preserving encodings
+// (xmin, ymin, xmax, ymax) so that no host synchronisation is needed
+__device__ __forceinline__ unsigned long long enc_f64(double v)
+{
+    const unsigned long long b = (unsigned long long)__double_as_longlong(v);
+    return (b >> 63) ? ~b : (b | 0x8000000000000000ull);
+}
+__device__ __forceinline__ double dec_f64(unsigned long long e)
+{
+    return __longlong_as_double((long long)((e >> 63) ? (e & 0x7fffffffffffffffull) : ~e));
+}
+struct Geom {
+    double x0, y0, size;     // lower-left corner and edge of the root square
+};
+__device__ __forceinline__ Geom load_geom(const unsigned long long *__restrict__ enc)
+{
+    Geom g;
+    g.x0 = dec_f64(enc[0]);
+    g.y0 = dec_f64(enc[1]);
+    const double ex = dec_f64(enc[2]) - g.x0, ey = dec_f64(enc[3]) - g.y0;
+    g.size = fmax(fmax(ex, ey) * (1.0 + 1e-9), 1e-300);
+    return g;
+}
+__device__ __forceinline__ cplx box_centre(const Geom &g, int level, int ix, int iy)
+{
+    const double s = g.size / (double)(1 << level);
+    return make_double2(fma((double)ix + 0.5, s, g.x0), fma((double)iy + 0.5, s, g.y0));
+}
+
+__global__ void fmm_init_bounds(unsigned long long *enc)
+{
+    enc[0] = enc[1] = ~0ull;
+    enc[2] = enc[3] = 0ull;
+}
+
+// positions and densities g = F*W promoted to double (original order), and the bounding box
+template <typename real, typename real2>
+__global__ void __launch_bounds__(256)
+fmm_load(const real2 *__restrict__ X, const real2 *__restrict__ F, const real *__restrict__ W, int P,
+         cplx *__restrict__ z, cplx *__restrict__ g, unsigned long long *__restrict__ enc)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    double x = INFINITY, y = INFINITY, X1 = -INFINITY, Y1 = -INFINITY;
+    if (i < P) {
+        const real2 p = X[i];
+        const real2 f = F[i];
+        const real w = W[i];
+        x = X1 = (double)p.x;
+        y = Y1 = (double)p.y;
+        z[i] = make_double2(x, y);
+        g[i] = make_double2((double)(f.x * w), (double)(f.y * w));   // product in the storage precision, as in the exact path
+    }
+#pragma unroll
+    for (int m = 16; m >= 1; m >>= 1) {
+        x = fmin(x, __shfl_xor_sync(0xffffffffu, x, m));
+        y = fmin(y, __shfl_xor_sync(0xffffffffu, y, m));
+        X1 = fmax(X1, __shfl_xor_sync(0xffffffffu, X1, m));
+        Y1 = fmax(Y1, __shfl_xor_sync(0xffffffffu, Y1, m));
+    }
+    if ((threadIdx.x & 31) == 0 && x <= X1) {
+        atomicMin(enc + 0, enc_f64(x));
+        atomicMin(enc + 1, enc_f64(y));
+        atomicMax(enc + 2, enc_f64(X1));
+        atomicMax(enc + 3, enc_f64(Y1));
+    }
+}
+
+// leaf box of every point and the population count of the leaves
+__global__ void __launch_bounds__(256)
+fmm_bin(const cplx *__restrict__ z, int P, int L, const unsigned long long *__restrict__ enc, int *__restrict__ cell,
+        int *__restrict__ cnt)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= P) return;
+    const Geom gm = load_geom(enc);
+    const int n = 1 << L;
+    const double inv = (double)n / gm.size;
+    const int ix = min(max((int)((z[i].x - gm.x0) * inv), 0), n - 1);
+    const int iy = min(max((int)((z[i].y - gm.y0) * inv), 0), n - 1);
+    const int c = ix * n + iy;
+    cell[i] = c;
+    atomicAdd(cnt + c, 1);
+}
+
+__global__ void __launch_bounds__(256)
+fmm_scatter(const int *__restrict__ cell, int P, long long *__restrict__ cursor, int *__restrict__ perm)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= P) return;
+    const long long pos = (long long)atomicAdd((unsigned long long *)(cursor + cell[i]), 1ull);
+    perm[pos] = i;
+}
+
+// the atomic scatter leaves every leaf's points in arbitrary order: sort each segment by point index so that
+// every later sum runs in a fixed order (bitwise reproducible results); then gather the sorted copies
+__global__ void __launch_bounds__(128)
+fmm_sort_cells(const long long *__restrict__ start, int ncell, int *__restrict__ perm)
+{
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= ncell) return;
+    const long long a = start[c], b = start[c + 1];
+    for (long long i = a + 1; i < b; ++i) {            // insertion sort: segments are a few dozen entries
+        const int v = perm[i];
+        long long j = i - 1;
+        while (j >= a && perm[j] > v) { perm[j + 1] = perm[j]; --j; }
+        perm[j + 1] = v;
+    }
+}
+
+__global__ void __launch_bounds__(256)
+fmm_gather(const int *__restrict__ perm, int P, int npts, const cplx *__restrict__ z, const cplx *__restrict__ g,
+           cplx *__restrict__ zs, cplx *__restrict__ gs, int *__restrict__ vs)
+{
+    const int q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= P) return;
+    const int i = perm[q];
+    zs[q] = z[i];
+    gs[q] = g[i];
+    vs[q] = i / npts;
+}
+
+// ------------------------------------------------------------------------------------------------
+// translation tables for order p (q = p + 1 coefficients), built once per call on the device:
+//   Cb[n][l]   = C(n + l, l)                                    (real, q x q)          -- M2L
+//   S[c][k][m] = C(k, m) delta_c^(k-m) 2^-m   (m <= k)          (complex, 4 x q x q)   -- M2M, child c -> parent
+//   T[c][m][k] = 2^-m C(k, m) delta_c^(k-m)   (k >= m)          (complex, 4 x q x q)   -- L2L, parent -> child c
+//   rho[t][n]  = tau_t^-n, n = 0 .. q;  lrho[t] = log(1/tau_t)  (complex, 49 offsets tau = dx + i dy, |dx|,|dy| <= 3)
+// delta_c = ((a - 1/2) + i (b - 1/2)) / 2 is the child's centre in the parent's scaled variable, c = 2 a + b.
+struct FmmTables {
+    double *Cb;
+    cplx *S, *T, *rho, *lrho;
+};
+__host__ __device__ inline size_t fmm_tables_doubles(int q) { return (((size_t)q * q + 1) & ~(size_t)1) + 2 * (size_t)(8 * q * q) + 2 * (size_t)(49 * (q + 1)) + 2 * 49; }
+__host__ __device__ inline FmmTables fmm_tables_at(double *base, int q)
+{
+    FmmTables t;
+    t.Cb = base;
+    t.S = (cplx *)(base + (((size_t)q * q + 1) & ~(size_t)1));   // 16-byte aligned
+    t.T = t.S + 4 * q * q;
+    t.rho = t.T + 4 * q * q;
+    t.lrho = t.rho + 49 * (q + 1);
+    return t;
+}
+__device__ __forceinline__ double binom(int n, int l)
+{
+    if (l < 0 || l > n) return 0.0;
+    double r = 1.0;
+    for (int i = 1; i <= l; ++i) r = r * (double)(n - l + i) / (double)i;
+    return r;
+}
+__device__ __forceinline__ cplx cpowi(cplx a, int n)
+{
+    cplx r = make_double2(1.0, 0.0);
+    for (int i = 0; i < n; ++i) r = cmul(r, a);
+    return r;
+}
+__global__ void fmm_build_tables(int q, double *base)
+{
+    const FmmTables t = fmm_tables_at(base, q);
+    const int nthreads = gridDim.x * blockDim.x, tid = blockIdx.x * blockDim.x + threadIdx.x;
+    for (int e = tid; e < q * q; e += nthreads) {
+        const int n = e / q, l = e % q;
+        t.Cb[e] = binom(n + l, l);
+    }
+    for (int e = tid; e < 4 * q * q; e += nthreads) {
+        const int c = e / (q * q), k = (e / q) % q, m = e % q;
+        const cplx d = make_double2(0.5 * ((double)(c >> 1) - 0.5), 0.5 * ((double)(c & 1) - 0.5));
+        cplx s = make_double2(0.0, 0.0), u = make_double2(0.0, 0.0);
+        if (m <= k) s = cscale(cpowi(d, k - m), binom(k, m) * exp2(-(double)m));       // S[c][k][m]
+        if (k <= m) u = cscale(cpowi(d, m - k), binom(m, k) * exp2(-(double)k));       // T[c][k][m]: row = child index k
+        t.S[e] = s;
+        t.T[e] = u;
+    }
+    for (int e = tid; e < 49 * (q + 1); e += nthreads) {
+        const int o = e / (q + 1), n = e % (q + 1);
+        const cplx tau = make_double2((double)(o / 7 - 3), (double)(o % 7 - 3));
+        cplx r = make_double2(0.0, 0.0);
+        if (tau.x != 0.0 || tau.y != 0.0) r = cpowi(crcp(tau), n);
+        t.rho[e] = r;
+        if (n == 0) {
+            cplx lr = make_double2(0.0, 0.0);
+            if (tau.x != 0.0 || tau.y != 0.0) lr = make_double2(-0.5 * log(tau.x * tau.x + tau.y * tau.y), -atan2(tau.y, tau.x));
+            t.lrho[o] = lr;
+        }
+    }
+}
+
+// expansions: [box][3][q] complex, boxes of level l start at (4^l - 1)/3; index inside a level ix * 2^l + iy
+__host__ __device__ inline long long level_offset(int l) { return ((1ll << (2 * l)) - 1) / 3; }
+
+// ------------------------------------------------------------------------------------------------
+// P2M: one warp per leaf box.  Moments about the box centre in the scaled variable w = (zeta - c)/s:
+//   A1_k = sum g_x w^k,  A2_k = sum g_y w^k,  B_k = sum conj(zeta) g w^k.
+constexpr int kFmmMaxQ = 49;          // p <= 48
+__global__ void __launch_bounds__(128)
+fmm_p2m(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const long long *__restrict__ start, int L, int q,
+        const unsigned long long *__restrict__ enc, cplx *__restrict__ mult)
+{
+    __shared__ cplx acc[4][3 * kFmmMaxQ];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int n = 1 << L, ncell = n * n;
+    const int c = blockIdx.x * 4 + warp;
+    if (c >= ncell) return;
+    const Geom gm = load_geom(enc);
+    const double s = gm.size / (double)n, inv_s = 1.0 / s;
+    const cplx ctr = box_centre(gm, L, c / n, c % n);
+    for (int e = lane; e < 3 * q; e += 32) acc[warp][e] = make_double2(0.0, 0.0);
+    __syncwarp();
+    const long long a = start[c], b = start[c + 1];
+    for (long long base = a; base < b; base += 32) {
+        const long long idx = base + lane;
+        cplx w = make_double2(0.0, 0.0), g = make_double2(0.0, 0.0), h = make_double2(0.0, 0.0);
+        if (idx < b) {
+            const cplx zt = zs[idx];
+            g = gs[idx];
+            w = make_double2((zt.x - ctr.x) * inv_s, (zt.y - ctr.y) * inv_s);
+            h = cmul(make_double2(zt.x, -zt.y), g);                  // conj(zeta) g
+        }
+        cplx pw = make_double2(1.0, 0.0);
+        for (int k = 0; k < q; ++k) {
+            double v[6] = {g.x * pw.x, g.x * pw.y, g.y * pw.x, g.y * pw.y, fma(h.x, pw.x, -h.y * pw.y), fma(h.x, pw.y, h.y * pw.x)};
+#pragma unroll
+            for (int m = 16; m >= 1; m >>= 1)
+#pragma unroll
+                for (int e = 0; e < 6; ++e) v[e] += __shfl_xor_sync(0xffffffffu, v[e], m);
+            if (lane == 0) {
+                acc[warp][k] = cadd(acc[warp][k], make_double2(v[0], v[1]));
+                acc[warp][q + k] = cadd(acc[warp][q + k], make_double2(v[2], v[3]));
+                acc[warp][2 * q + k] = cadd(acc[warp][2 * q + k], make_double2(v[4], v[5]));
+            }
+            pw = cmul(pw, w);
+        }
+    }
+    __syncwarp();
+    cplx *out = mult + (level_offset(L) + c) * (long long)(3 * q);
+    for (int e = lane; e < 3 * q; e += 32) out[e] = acc[warp][e];
+}
+
+// M2M: parent moments from its four children, levels L-1 down to 2.  One thread per (parent box, k).
+__global__ void __launch_bounds__(128)
+fmm_m2m(int level, int q, const double *__restrict__ tab, cplx *__restrict__ mult, int *__restrict__ boxcnt)
+{
+    const FmmTables t = fmm_tables_at(const_cast<double *>(tab), q);
+    const int n = 1 << level;
+    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= (long long)n * n * q) return;
+    const int box = (int)(e / q), k = (int)(e % q);
+    const int ix = box / n, iy = box % n;
+    cplx s1 = make_double2(0.0, 0.0), s2 = s1, s3 = s1;
+    int cnt = 0;
+    for (int c = 0; c < 4; ++c) {
+        const long long child = level_offset(level + 1) + (long long)(2 * ix + (c >> 1)) * (2 * n) + (2 * iy + (c & 1));
+        const int cc = boxcnt[child];
+        cnt += cc;
+        if (cc == 0) continue;
+        const cplx *A = mult + child * (long long)(3 * q);
+        const cplx *row = t.S + ((size_t)c * q + k) * q;
+        for (int m = 0; m <= k; ++m) {
+            const cplx sm = row[m];
+            s1 = cfma(sm, A[m], s1);
+            s2 = cfma(sm, A[q + m], s2);
+            s3 = cfma(sm, A[2 * q + m], s3);
+        }
+    }
+    cplx *out = mult + (level_offset(level) + box) * (long long)(3 * q);
+    out[k] = s1;
+    out[q + k] = s2;
+    out[2 * q + k] = s3;
+    if (k == 0) boxcnt[level_offset(level) + box] = cnt;
+}
+
+// ------------------------------------------------------------------------------------------------
+// M2L: one block per target box of `level`; thread (a, l) = (tid / 64, tid % 64) owns coefficient l of local
+// expansion a (0, 1: the logarithmic potentials Phi1, Phi2; 2: the Cauchy sum psi).  For every box of the
+// interaction list (children of the parent's neighbours that are not neighbours of the target; offset
+// tau = target - source in box units, rho = 1/tau):
+//   Ahat_k = A_k rho^k / k (k >= 1, log type)      Bhat_k = B_k rho^k (k >= 0)              (staged in shared memory)
+//   b_l += (-1)^(l+1) rho^l ( A_0 / l + sum_{k>=1} C(k+l-1, l) Ahat_k )          l >= 1
+//   b_0 += A_0 (log s - log rho) - sum_{k>=1} Ahat_k
+//   d_l += (-1)^l rho^(l+1) / s * sum_{k>=0} C(k+l, l) Bhat_k ;   d_0 -= conj(A1_0 + i A2_0)   (the g/2 of each source)
+// so the inner loop is a REAL binomial matrix (shared memory, same for every offset and level) times a complex
+// vector: 2 DFMA per entry.
+__global__ void __launch_bounds__(192)
+fmm_m2l(int level, int q, const double *__restrict__ tab, const unsigned long long *__restrict__ enc,
+        const cplx *__restrict__ mult, const int *__restrict__ boxcnt, cplx *__restrict__ loc)
+{
+    extern __shared__ __align__(16) double sm[];
+    double *Cb = sm;                                   // [q][q]
+    cplx *hat = (cplx *)(sm + ((q * q + 1) & ~1));     // [3][q]
+    __shared__ cplx A0[2];
+    const FmmTables t = fmm_tables_at(const_cast<double *>(tab), q);
+    const int n = 1 << level;
+    const int box = blockIdx.x, ix = box / n, iy = box % n;
+    const int a = threadIdx.x >> 6, l = threadIdx.x & 63;
+    const bool active = l < q;
+    for (int e = threadIdx.x; e < q * q; e += blockDim.x) Cb[e] = t.Cb[e];
+    const Geom gm = load_geom(enc);
+    const double s = gm.size / (double)n, log_s = log(s);
+    cplx acc = make_double2(0.0, 0.0);
+    const double sgn = (l & 1) ? -1.0 : 1.0;           // (-1)^l
+    const int px = ix >> 1, py = iy >> 1;
+    const int x_lo = max(0, 2 * (px - 1)), x_hi = min(n, 2 * (px + 1) + 2);
+    const int y_lo = max(0, 2 * (py - 1)), y_hi = min(n, 2 * (py + 1) + 2);
+    for (int sx = x_lo; sx < x_hi; ++sx)
+        for (int sy = y_lo; sy < y_hi; ++sy) {
+            if (abs(sx - ix) <= 1 && abs(sy - iy) <= 1) continue;
+            const long long src = level_offset(level) + (long long)sx * n + sy;
+            if (boxcnt[src] == 0) continue;
+            const int o = (ix - sx + 3) * 7 + (iy - sy + 3);
+            const cplx *rho = t.rho + (size_t)o * (q + 1);
+            const cplx *A = mult + src * (long long)(3 * q);
+            __syncthreads();                               // previous source's hat / A0 are consumed
+            if (active) {
+                cplx v = cmul(A[a * q + l], rho[l]);
+                if (a < 2 && l >= 1) v = cscale(v, 1.0 / (double)l);
+                hat[a * q + l] = v;
+                if (a < 2 && l == 0) A0[a] = A[a * q];
+            }
+            __syncthreads();
+            if (active) {
+                cplx S = make_double2(0.0, 0.0);
+                const cplx *h = hat + a * q;
+                if (a < 2) {
+                    for (int k = 1; k < q; ++k) {
+                        const double c = Cb[(k - 1) * q + l];
+                        S.x = fma(c, h[k].x, S.x);
+                        S.y = fma(c, h[k].y, S.y);
+                    }
+                    if (l == 0) {
+                        const cplx lr = t.lrho[o];
+                        acc = cadd(acc, make_double2(A0[a].x * (log_s - lr.x) - A0[a].y * (-lr.y) - S.x,
+                                                     A0[a].x * (-lr.y) + A0[a].y * (log_s - lr.x) - S.y));
+                    } else {
+                        const cplx w = cadd(cscale(A0[a], 1.0 / (double)l), S);
+                        acc = cadd(acc, cscale(cmul(rho[l], w), -sgn));
+                    }
+                } else {
+                    for (int k = 0; k < q; ++k) {
+                        const double c = Cb[k * q + l];
+                        S.x = fma(c, h[k].x, S.x);
+                        S.y = fma(c, h[k].y, S.y);
+                    }
+                    acc = cadd(acc, cscale(cmul(rho[l + 1], S), sgn / s));
+                    if (l == 0) acc = cadd(acc, make_double2(-(A0[0].x - A0[1].y), A0[0].y + A0[1].x));   // -conj(A1_0 + i A2_0)
+                }
+            }
+        }
+    if (active) loc[(level_offset(level) + box) * (long long)(3 * q) + a * q + l] = acc;
+}
+
+// L2L: child local expansions inherit the parent's.  One thread per (child box, k); child level = `level`.
+__global__ void __launch_bounds__(128)
+fmm_l2l(int level, int q, const double *__restrict__ tab, cplx *__restrict__ loc)
+{
+    const FmmTables t = fmm_tables_at(const_cast<double *>(tab), q);
+    const int n = 1 << level;
+    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= (long long)n * n * q) return;
+    const int box = (int)(e / q), k = (int)(e % q);
+    const int ix = box / n, iy = box % n, c = 2 * (ix & 1) + (iy & 1);
+    const cplx *par = loc + (level_offset(level - 1) + (long long)(ix >> 1) * (n >> 1) + (iy >> 1)) * (long long)(3 * q);
+    const cplx *row = t.T + ((size_t)c * q + k) * q;
+    cplx s1 = make_double2(0.0, 0.0), s2 = s1, s3 = s1;
+    for (int m = k; m < q; ++m) {
+        const cplx tm = row[m];
+        s1 = cfma(tm, par[m], s1);
+        s2 = cfma(tm, par[q + m], s2);
+        s3 = cfma(tm, par[2 * q + m], s3);
+    }
+    cplx *out = loc + (level_offset(level) + box) * (long long)(3 * q);
+    out[k] = cadd(out[k], s1);
+    out[q + k] = cadd(out[q + k], s2);
+    out[2 * q + k] = cadd(out[2 * q + k], s3);
+}
+
+// the two tables of log_rcp_f64 in global memory (built once per call, copied to shared memory by every block)
+__global__ void fmm_build_logtab(double *tab)
+{
+    build_log_tables(tab, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
+}
+
+// ------------------------------------------------------------------------------------------------
+// L2P + P2P: one block per leaf box, one thread per target point (in rounds of 64).
+//   far  = -(Re Phi1 + i Re Phi2) + (z/2) conj(Phi1' + i Phi2') - (1/2) conj(psi)   from the box's local expansions
+//   near = direct sum over the points of the 3 x 3 neighbour boxes that belong to OTHER vesicles
+// The sum goes to accum[original point index] (still without the 1/(4 pi mu)).
+constexpr int kP2PThreads = 64;
+__global__ void __launch_bounds__(kP2PThreads)
+fmm_l2p_p2p(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const int *__restrict__ vs,
+            const int *__restrict__ perm, const long long *__restrict__ start, int L, int q,
+            const unsigned long long *__restrict__ enc, const cplx *__restrict__ loc, const double *__restrict__ logtab,
+            cplx *__restrict__ accum)
+{
+    __shared__ double tab[kLogTab + kExpTab];
+    __shared__ cplx lc[3 * kFmmMaxQ];
+    __shared__ double4 src[kP2PThreads];               // (zeta_x, zeta_y, g_x, g_y)
+    __shared__ int sves[kP2PThreads];
+    const int n = 1 << L, c = blockIdx.x, ix = c / n, iy = c % n;
+    const long long a = start[c], b = start[c + 1];
+    if (a == b) return;
+    const int tid = threadIdx.x;
+    for (int e = tid; e < kLogTab + kExpTab; e += kP2PThreads) tab[e] = logtab[e];
+    for (int e = tid; e < 3 * q; e += kP2PThreads) lc[e] = loc[(level_offset(L) + c) * (long long)(3 * q) + e];
+    const Geom gm = load_geom(enc);
+    const double s = gm.size / (double)n, inv_s = 1.0 / s;
+    const cplx ctr = box_centre(gm, L, ix, iy);
+    __syncthreads();
+
+    for (long long t0 = a; t0 < b; t0 += kP2PThreads) {
+        const long long ti = t0 + tid;
+        const bool live = ti < b;
+        cplx z = make_double2(0.0, 0.0);
+        int myves = -1;
+        double ux = 0.0, uy = 0.0;
+        if (live) {
+            z = zs[ti];
+            myves = vs[ti];
+            // far field: Horner for value and derivative of the three local expansions
+            const cplx t = make_double2((z.x - ctr.x) * inv_s, (z.y - ctr.y) * inv_s);
+            cplx p1 = lc[q - 1], p2 = lc[2 * q - 1], p3 = lc[3 * q - 1];
+            cplx d1 = make_double2(0.0, 0.0), d2 = d1;
+            for (int l = q - 2; l >= 0; --l) {
+                d1 = cfma(d1, t, p1);
+                d2 = cfma(d2, t, p2);
+                p1 = cfma(p1, t, lc[l]);
+                p2 = cfma(p2, t, lc[q + l]);
+                p3 = cfma(p3, t, lc[2 * q + l]);
+            }
+            // phi = (Phi1' + i Phi2') = (d1 + i d2)/s ;  z conj(phi)
+            const cplx phi = make_double2((d1.x - d2.y) * inv_s, (d1.y + d2.x) * inv_s);
+            const cplx zc = cmul(z, make_double2(phi.x, -phi.y));
+            ux = -p1.x + 0.5 * zc.x - 0.5 * p3.x;
+            uy = -p2.x + 0.5 * zc.y + 0.5 * p3.y;
+        }
+        // near field
+        for (int bx = max(ix - 1, 0); bx <= min(ix + 1, n - 1); ++bx)
+            for (int by = max(iy - 1, 0); by <= min(iy + 1, n - 1); ++by) {
+                const long long sa = start[bx * n + by], sb = start[bx * n + by + 1];
+                for (long long s0 = sa; s0 < sb; s0 += kP2PThreads) {
+                    __syncthreads();
+                    if (s0 + tid < sb) {
+                        const cplx zz = zs[s0 + tid], gg = gs[s0 + tid];
+                        src[tid] = make_double4(zz.x, zz.y, gg.x, gg.y);
+                        sves[tid] = vs[s0 + tid];
+                    }
+                    __syncthreads();
+                    const int cnt = (int)min((long long)kP2PThreads, sb - s0);
+                    if (live)
+                        for (int j = 0; j < cnt; ++j) {
+                            if (sves[j] == myves) continue;
+                            const double4 sj = src[j];
+                            const double rx = z.x - sj.x, ry = z.y - sj.y;
+                            const double r2 = fma(rx, rx, ry * ry);
+                            double ml, inv;
+                            log_rcp_f64(r2, tab, ml, inv);
+                            const double qd = fma(rx, sj.z, ry * sj.w) * inv;
+                            ux = fma(ml, sj.z, fma(qd, rx, ux));
+                            uy = fma(ml, sj.w, fma(qd, ry, uy));
+                        }
+                }
+            }
+        if (live) accum[perm[ti]] = make_double2(ux, uy);
+        __syncthreads();
+    }
+}
+
+// own-vesicle points that sit in NON-neighbour leaf boxes of the target went through the expansions: take their
+// contribution out again (direct, libm log), scale by 1/(4 pi mu) and store.  One thread per point.
+template <typename real2>
+__global__ void __launch_bounds__(128)
+fmm_finish(const cplx *__restrict__ z, const cplx *__restrict__ g, const int *__restrict__ cell, int P, int npts, int L,
+           const cplx *__restrict__ accum, double prefactor, real2 *__restrict__ U)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= P) return;
+    const int n = 1 << L;
+    const int ci = cell[i], ix = ci / n, iy = ci % n;
+    const cplx zi = z[i];
+    const int v0 = (i / npts) * npts;
+    double cx = 0.0, cy = 0.0;
+    for (int j = v0; j < v0 + npts; ++j) {
+        const int cj = cell[j];
+        if (abs(cj / n - ix) <= 1 && abs(cj % n - iy) <= 1) continue;
+        const cplx gj = g[j];
+        const double rx = zi.x - z[j].x, ry = zi.y - z[j].y;
+        const double r2 = rx * rx + ry * ry;
+        const double ml = -0.5 * log(r2);
+        const double qd = (rx * gj.x + ry * gj.y) / r2;
+        cx += ml * gj.x + qd * rx;
+        cy += ml * gj.y + qd * ry;
+    }
+    const cplx u = accum[i];
+    real2 o;
+    o.x = (decltype(o.x))(prefactor * (u.x - cx));
+    o.y = (decltype(o.y))(prefactor * (u.y - cy));
+    U[i] = o;
+}
+
+// ------------------------------------------------------------------------------------------------
+static int fmm_levels(long long P, int order)
+{
+    // leaves of about 1.5 (p+1) points balance the direct part (9 x leaf pairs per point) against M2L
+    // (27 x 3 (p+1)^2 per box); at least 2 levels (no interaction lists above), at most 10
+    double target = 1.5 * (order + 1);
+    target = target < 16 ? 16 : (target > 96 ? 96 : target);
+    int L = 2;
+    while (L < 10 && (double)P / (double)(1ll << (2 * L)) > target) ++L;
+    return L;
+}
+
+vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, double mu, int order,
+                       void *U, vn_precision prec, cudaStream_t st)
+{
+    const int P = (int)(nves * npts), q = order + 1;
+    const int L = fmm_levels(P, order);
+    const int n = 1 << L, ncell = n * n;
+    const long long nbox = level_offset(L + 1);
+    const int nb_scan = (ncell + kScanBlock - 1) / kScanBlock;
+    auto up = [](size_t b) { return (b + 255) & ~(size_t)255; };
+    const size_t b_pt = up(sizeof(cplx) * (size_t)P), b_int = up(sizeof(int) * (size_t)P);
+    const size_t b_exp = up(sizeof(cplx) * (size_t)nbox * 3 * q), b_cnt = up(sizeof(int) * (size_t)nbox);
+    const size_t b_start = up(sizeof(long long) * ((size_t)ncell + 1)), b_bs = up(sizeof(long long) * (size_t)nb_scan);
+    const size_t b_tab = up(sizeof(double) * fmm_tables_doubles(q)), b_log = up(sizeof(double) * (kLogTab + kExpTab));
+    const size_t total = 5 * b_pt + 3 * b_int + 2 * b_exp + b_cnt + 2 * b_start + b_bs + b_tab + b_log + 256;
+    char *scr = nullptr;
+    VN_CUDA(cudaMallocAsync((void **)&scr, total, st));
+    char *ptr = scr;
+    auto take = [&](size_t b) { char *r = ptr; ptr += b; return r; };
+    cplx *z = (cplx *)take(b_pt), *g = (cplx *)take(b_pt), *zs = (cplx *)take(b_pt), *gs = (cplx *)take(b_pt);
+    cplx *accum = (cplx *)take(b_pt);
+    int *cell = (int *)take(b_int), *perm = (int *)take(b_int), *vs = (int *)take(b_int);
+    cplx *mult = (cplx *)take(b_exp), *loc = (cplx *)take(b_exp);
+    int *boxcnt = (int *)take(b_cnt);
+    long long *start = (long long *)take(b_start), *cursor = (long long *)take(b_start), *bsum = (long long *)take(b_bs);
+    double *tab = (double *)take(b_tab), *logtab = (double *)take(b_log);
+    unsigned long long *enc = (unsigned long long *)take(256);
+    int *cnt = boxcnt + level_offset(L);
+
+    VN_CUDA(cudaMemsetAsync(boxcnt, 0, b_cnt, st));
+    fmm_init_bounds<<<1, 1, 0, st>>>(enc);
+    const int gp = (P + 255) / 256;
+    if (prec == VN_F32)
+        fmm_load<float, float2><<<gp, 256, 0, st>>>((const float2 *)X, (const float2 *)F, (const float *)W, P, z, g, enc);
+    else
+        fmm_load<double, double2><<<gp, 256, 0, st>>>((const double2 *)X, (const double2 *)F, (const double *)W, P, z, g, enc);
+    fmm_bin<<<gp, 256, 0, st>>>(z, P, L, enc, cell, cnt);
+    scan_block_sums<<<nb_scan, kScanThreads, 0, st>>>(cnt, ncell, bsum);
+    scan_of_sums<<<1, kScanThreads, 0, st>>>(bsum, nb_scan);
+    scan_apply<<<nb_scan, kScanThreads, 0, st>>>(cnt, ncell, bsum, start, cursor);
+    fmm_scatter<<<gp, 256, 0, st>>>(cell, P, cursor, perm);
+    fmm_sort_cells<<<(ncell + 127) / 128, 128, 0, st>>>(start, ncell, perm);
+    fmm_gather<<<gp, 256, 0, st>>>(perm, P, (int)npts, z, g, zs, gs, vs);
+    fmm_build_tables<<<64, 128, 0, st>>>(q, tab);
+    fmm_build_logtab<<<8, 128, 0, st>>>(logtab);
+    int launches = 12;
+
+    profile_mark(st, true);
+    fmm_p2m<<<(ncell + 3) / 4, 128, 0, st>>>(zs, gs, start, L, q, enc, mult);
+    ++launches;
+    for (int l = L - 1; l >= 2; --l) {
+        const long long work = (1ll << (2 * l)) * q;
+        fmm_m2m<<<(unsigned)((work + 127) / 128), 128, 0, st>>>(l, q, tab, mult, boxcnt);
+        ++launches;
+    }
+    const size_t smem_m2l = sizeof(double) * (size_t)(((q * q + 1) & ~1) + 6 * q);
+    for (int l = 2; l <= L; ++l) {
+        fmm_m2l<<<1u << (2 * l), 192, smem_m2l, st>>>(l, q, tab, enc, mult, boxcnt, loc);
+        ++launches;
+    }
+    for (int l = 3; l <= L; ++l) {
+        const long long work = (1ll << (2 * l)) * q;
+        fmm_l2l<<<(unsigned)((work + 127) / 128), 128, 0, st>>>(l, q, tab, loc);
+        ++launches;
+    }
+    fmm_l2p_p2p<<<ncell, kP2PThreads, 0, st>>>(zs, gs, vs, perm, start, L, q, enc, loc, logtab, accum);
+    profile_mark(st, false);
+    const double pref = 1.0 / (4.0 * 3.14159265358979323846 * mu);
+    if (prec == VN_F32)
+        fmm_finish<float2><<<(P + 127) / 128, 128, 0, st>>>(z, g, cell, P, (int)npts, L, accum, pref, (float2 *)U);
+    else
+        fmm_finish<double2><<<(P + 127) / 128, 128, 0, st>>>(z, g, cell, P, (int)npts, L, accum, pref, (double2 *)U);
+    count_launch(launches + 2);
+    const cudaError_t e = cudaGetLastError();
+    VN_CUDA(cudaFreeAsync(scr, st));
+    return e == cudaSuccess ? VN_OK : VN_ERR_CUDA;
+}
+
+}  // namespace vn

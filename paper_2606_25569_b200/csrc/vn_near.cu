@@ -144,9 +144,6 @@ near_kernel(const real2 *__restrict__ X, int nves, int npts, const double4 *__re
 // ------------------------------------------------------------------------------------------------
 // exclusive scan cnt[P] -> ptr[P+1] (64-bit), three small kernels: block sums, scan of the block sums
 // by one block, rescan with the offsets.
-constexpr int kScanThreads = 256;
-constexpr int kScanItems = 4;
-constexpr int kScanBlock = kScanThreads * kScanItems;
 
 __device__ __forceinline__ long long block_exclusive_scan(long long v, long long *total)
 {

@@ -423,3 +423,79 @@ def test_redistribute_rejects_bad_sizes_and_chains():
     Xo = oracle.redistribute(s.X)
     ref = oracle.farfield(Xo, s.F, oracle.weights(Xo), s.mu)
     assert rel_l2(Ud.cpu().numpy(), ref) <= 1e-12
+
+
+# ------------------------------------------------------------------------------------- fast multipole method (row f-4, second half)
+# vn_farfield_fmm approximates the exact sum; the oracle is still the plain direct sum.  The tolerance follows the
+# truncation error of the expansions, about 0.45^p relative: p = 12 for the fp32 bar (2e-5),
+# p = 38 for the fp64 bar (1e-12).
+@pytest.mark.parametrize("index,dtype,order", [(0, np.float64, 38), (0, np.float32, 12), (1, np.float64, 38),
+                                                (1, np.float32, 12), (1, np.float64, 12)])
+def test_fmm_full_parity(index, dtype, order):
+    s = inputs.config(index)
+    W = oracle.weights(s.X)
+    ref = oracle.farfield(stored(s.X, dtype), stored(s.F, dtype), stored(W, dtype), s.mu)
+    got = vn.vn_farfield_fmm(dev(s.X, dtype), dev(s.F, dtype), dev(W, dtype), s.mu, order)
+    torch.cuda.synchronize()
+    err = rel_l2(got.cpu().numpy(), ref)
+    tol = TOL[dtype] if not (dtype == np.float64 and order < 30) else 2e-5
+    print(f"fmm config{index} {np.dtype(dtype).name} p={order}: rel-L2 {err:.3e} (tolerance {tol:.0e})")
+    assert err <= tol
+
+
+@pytest.mark.parametrize("index,dtype,order,nsample", [(3, np.float32, 12, 3072), (3, np.float64, 38, 3072),
+                                                      (4, np.float32, 12, 1024)])
+def test_fmm_sampled_parity_large(index, dtype, order, nsample):
+    s = inputs.config(index)
+    W = oracle.weights(s.X)
+    P = s.nves * s.npts
+    rng = np.random.Generator(np.random.PCG64(260625569 + 400))
+    idx = np.unique(np.concatenate([[0, 127, 128, P - 1], rng.choice(P, size=nsample, replace=False)]))
+    ref = oracle.farfield_subset(stored(s.X, dtype), stored(s.F, dtype), stored(W, dtype), idx, s.mu)
+    got = vn.vn_farfield_fmm(dev(s.X, dtype), dev(s.F, dtype), dev(W, dtype), s.mu, order)
+    torch.cuda.synchronize()
+    err = rel_l2(got.cpu().numpy().reshape(-1, 2)[idx], ref)
+    print(f"fmm config{index} {np.dtype(dtype).name} p={order}: sampled rel-L2 {err:.3e}")
+    assert err <= TOL[dtype]
+
+
+def test_fmm_converges_with_order_and_agrees_with_exact_path():
+    s = inputs.config(2)
+    W = oracle.weights(s.X)
+    Xd, Fd, Wd = dev(s.X, np.float64), dev(s.F, np.float64), dev(W, np.float64)
+    exact = vn.vn_farfield(Xd, Fd, Wd, s.mu)
+    errs = []
+    for order in (4, 8, 16, 24, 32):
+        got = vn.vn_farfield_fmm(Xd, Fd, Wd, s.mu, order)
+        torch.cuda.synchronize()
+        errs.append(rel_l2(got.cpu().numpy(), exact.cpu().numpy()))
+    print("fmm vs exact GPU path, config2, p = 4, 8, 16, 24, 32:", " ".join(f"{e:.2e}" for e in errs))
+    assert all(b < 0.05 * a for a, b in zip(errs, errs[1:])) and errs[-1] < 1e-10
+    # bitwise reproducible
+    a = vn.vn_farfield_fmm(Xd, Fd, Wd, s.mu, 12).clone()
+    b = vn.vn_farfield_fmm(Xd, Fd, Wd, s.mu, 12)
+    torch.cuda.synchronize()
+    assert torch.equal(a, b)
+
+
+@pytest.mark.parametrize("nves,npts", [(2, 1), (3, 2), (7, 3), (5, 33), (3, 129), (37, 128), (11, 1000), (1030, 1), (3, 2049)])
+def test_fmm_edge_shapes(nves, npts):
+    rng = np.random.Generator(np.random.PCG64(1000 * nves + npts))
+    X = rng.normal(size=(nves, npts, 2)) * 0.3 + 4.0 * rng.normal(size=(nves, 1, 2))
+    F = rng.normal(size=(nves, npts, 2))
+    W = rng.uniform(0.5, 1.5, size=(nves, npts))
+    ref = oracle.farfield(X, F, W, 0.7)
+    got = vn.vn_farfield_fmm(dev(X, np.float64), dev(F, np.float64), dev(W, np.float64), 0.7, 40)
+    torch.cuda.synchronize()
+    got = got.cpu().numpy()
+    assert np.all(np.isfinite(got)) and rel_l2(got, ref) <= 1e-11
+
+
+def test_fmm_single_vesicle_gives_zero():
+    rng = np.random.Generator(np.random.PCG64(5))
+    X = rng.normal(size=(1, 700, 2)); F = rng.normal(size=(1, 700, 2)); W = rng.uniform(0.5, 1.5, size=(1, 700))
+    got = vn.vn_farfield_fmm(dev(X, np.float64), dev(F, np.float64), dev(W, np.float64), 1.0, 30)
+    torch.cuda.synchronize()
+    # everything the expansions add is taken out again by the own-vesicle correction: zero up to truncation
+    scale = np.abs(oracle.farfield_targets(X, F, W, X[0, :1] + 50.0)).max()
+    assert np.abs(got.cpu().numpy()).max() <= 1e-9 * max(scale, 1.0) * 700
