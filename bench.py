@@ -180,6 +180,7 @@ def run_reference(args):
 
 
 PATHS = {"farfield": "rows a-1..a-5: vn_arclength_weights + vn_farfield",
+         "fmm": "row f-4b: vn_arclength_weights + vn_farfield_fmm (fast multipole, APPROXIMATE; value = the direct sum's pair count / time)",
          "masked": "row f-1: vn_arclength_weights + vn_near_pairs + vn_farfield_masked (the paper's DirectSingleLayerIntegral)",
          "targets": "row f-4: vn_arclength_weights + vn_farfield_targets on a 512x512 grid of free targets"}
 
@@ -297,11 +298,13 @@ def main():
     ap.add_argument("--workload", type=int, default=4, choices=[0, 1, 2, 3, 4])
     ap.add_argument("--precision", default="f32", choices=["f32", "f64"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--path", default="farfield", choices=["farfield", "masked", "targets", "aux"],
+    ap.add_argument("--path", default="farfield", choices=["farfield", "masked", "targets", "aux", "fmm"],
                     help="farfield: rows a-1..a-5 (the headline); masked: row f-1 (vn_near_pairs + "
                          "vn_farfield_masked); targets: row f-4 (vn_farfield_targets on a 512x512 grid); "
                          "aux: the O(P) rows around the sum (f-3 redistribution, a-1 weights, f-2 elastic force), "
-                         "reported in points/s")
+                         "reported in points/s; fmm: vn_farfield_fmm (approximate, O(P)), reported in the direct sum's "
+                         "interactions per second so that it compares with --path farfield")
+    ap.add_argument("--order", type=int, default=0, help="expansion order of --path fmm (default 12 for f32, 38 for f64)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -347,6 +350,7 @@ def main():
     U_d = torch.empty_like(X_d)
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")
 
+    fmm_order = args.order or (12 if args.precision == "f32" else 38)
     if args.path == "masked":                          # CSR buffers sized once (4 near vesicles per point is generous)
         near_ptr = torch.empty(P + 1, dtype=torch.int64, device="cuda")
         near_ves = torch.empty(4 * P, dtype=torch.int32, device="cuda")
@@ -360,6 +364,8 @@ def main():
         vn.vn_arclength_weights(X_d, out=W_d)          # a-1
         if args.path == "farfield":
             vn.vn_farfield(X_d, F_d, W_d, susp.mu, out=U_d)   # a-2 .. a-5
+        elif args.path == "fmm":
+            vn.vn_farfield_fmm(X_d, F_d, W_d, susp.mu, fmm_order, out=U_d)
         elif args.path == "masked":
             vn.vn_near_pairs(X_d, W_d, near_ptr, near_ves)
             vn.vn_farfield_masked(X_d, F_d, W_d, near_ptr, near_ves, susp.mu, out=U_d)
@@ -465,7 +471,8 @@ def main():
         except Exception:
             pass
         roofline = {"bound": "alu",
-                    "kernel": ("targets_%s_kernel" if args.path == "targets" else "farfield_%s_kernel") % args.precision,
+                    "kernel": ("fmm kernels (P2M, M2M, M2L, L2L, L2P+P2P)" if args.path == "fmm" else
+                               ("targets_%s_kernel" if args.path == "targets" else "farfield_%s_kernel") % args.precision),
                     "achieved": achieved, "peak": peak_lane,
                     "unit": "T lane-instr/s (%s pipe; 11 canonical instr per pair)" % ("FP32" if args.precision == "f32" else "FP64"),
                     "frac": achieved / peak_lane if achieved else None,
@@ -494,6 +501,10 @@ def main():
                                   "pinned host buffers -> device copies -> the path's C-ABI calls -> copy back, synchronised"}
         if args.path == "masked":
             line["config"]["near_pairs"] = n_near
+        if args.path == "fmm":
+            line["config"]["order"] = fmm_order
+            line["roofline"]["note"] = ("approximate algorithm: 'achieved' counts the interactions of the direct sum it replaces, "
+                                        "not executed work; kernel_ms_avg spans P2M..P2P (all FMM kernels)")
         if world == 1 and not args.no_cpu_baseline:
             v, cores, sample = oracle_rate(susp, np_dtype, 15.0, 4242, args.path)
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}

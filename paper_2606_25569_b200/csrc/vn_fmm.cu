@@ -312,7 +312,7 @@ fmm_m2m(int level, int q, const double *__restrict__ tab, cplx *__restrict__ mul
 }
 
 // ------------------------------------------------------------------------------------------------
-// M2L: one block per target box of `level`; thread (a, l) = (tid / 64, tid % 64) owns coefficient l of local
+// M2L: one block per target box of `level`; thread (a, l) = (tid / q, tid % q) owns coefficient l of local
 // expansion a (0, 1: the logarithmic potentials Phi1, Phi2; 2: the Cauchy sum psi).  For every box of the
 // interaction list (children of the parent's neighbours that are not neighbours of the target; offset
 // tau = target - source in box units, rho = 1/tau):
@@ -322,71 +322,84 @@ fmm_m2m(int level, int q, const double *__restrict__ tab, cplx *__restrict__ mul
 //   d_l += (-1)^l rho^(l+1) / s * sum_{k>=0} C(k+l, l) Bhat_k ;   d_0 -= conj(A1_0 + i A2_0)   (the g/2 of each source)
 // so the inner loop is a REAL binomial matrix (shared memory, same for every offset and level) times a complex
 // vector: 2 DFMA per entry.
-__global__ void __launch_bounds__(192)
+__global__ void __launch_bounds__(160)
 fmm_m2l(int level, int q, const double *__restrict__ tab, const unsigned long long *__restrict__ enc,
         const cplx *__restrict__ mult, const int *__restrict__ boxcnt, cplx *__restrict__ loc)
 {
     extern __shared__ __align__(16) double sm[];
     double *Cb = sm;                                   // [q][q]
-    cplx *hat = (cplx *)(sm + ((q * q + 1) & ~1));     // [3][q]
-    __shared__ cplx A0[2];
+    cplx *hat = (cplx *)(sm + ((q * q + 1) & ~1));     // [2][3][q]: double-buffered, one barrier per source
+    __shared__ cplx A0[2][2];
+    __shared__ int list_src[27], list_off[27], list_n;
     const FmmTables t = fmm_tables_at(const_cast<double *>(tab), q);
     const int n = 1 << level;
     const int box = blockIdx.x, ix = box / n, iy = box % n;
-    const int a = threadIdx.x >> 6, l = threadIdx.x & 63;
-    const bool active = l < q;
+    const int a = threadIdx.x / q, l = threadIdx.x - a * q;       // blockDim.x = 3 q rounded up to a warp
+    const bool active = a < 3;
     for (int e = threadIdx.x; e < q * q; e += blockDim.x) Cb[e] = t.Cb[e];
+    if (threadIdx.x == 0) {                            // interaction list: non-empty boxes, fixed order
+        const int px = ix >> 1, py = iy >> 1;
+        int cnt = 0;
+        for (int sx = max(0, 2 * (px - 1)); sx < min(n, 2 * (px + 1) + 2); ++sx)
+            for (int sy = max(0, 2 * (py - 1)); sy < min(n, 2 * (py + 1) + 2); ++sy) {
+                if (abs(sx - ix) <= 1 && abs(sy - iy) <= 1) continue;
+                if (boxcnt[level_offset(level) + (long long)sx * n + sy] == 0) continue;
+                list_src[cnt] = sx * n + sy;
+                list_off[cnt] = (ix - sx + 3) * 7 + (iy - sy + 3);
+                ++cnt;
+            }
+        list_n = cnt;
+    }
     const Geom gm = load_geom(enc);
     const double s = gm.size / (double)n, log_s = log(s);
     cplx acc = make_double2(0.0, 0.0);
     const double sgn = (l & 1) ? -1.0 : 1.0;           // (-1)^l
-    const int px = ix >> 1, py = iy >> 1;
-    const int x_lo = max(0, 2 * (px - 1)), x_hi = min(n, 2 * (px + 1) + 2);
-    const int y_lo = max(0, 2 * (py - 1)), y_hi = min(n, 2 * (py + 1) + 2);
-    for (int sx = x_lo; sx < x_hi; ++sx)
-        for (int sy = y_lo; sy < y_hi; ++sy) {
-            if (abs(sx - ix) <= 1 && abs(sy - iy) <= 1) continue;
-            const long long src = level_offset(level) + (long long)sx * n + sy;
-            if (boxcnt[src] == 0) continue;
-            const int o = (ix - sx + 3) * 7 + (iy - sy + 3);
-            const cplx *rho = t.rho + (size_t)o * (q + 1);
-            const cplx *A = mult + src * (long long)(3 * q);
-            __syncthreads();                               // previous source's hat / A0 are consumed
-            if (active) {
-                cplx v = cmul(A[a * q + l], rho[l]);
-                if (a < 2 && l >= 1) v = cscale(v, 1.0 / (double)l);
-                hat[a * q + l] = v;
-                if (a < 2 && l == 0) A0[a] = A[a * q];
-            }
-            __syncthreads();
-            if (active) {
-                cplx S = make_double2(0.0, 0.0);
-                const cplx *h = hat + a * q;
-                if (a < 2) {
-                    for (int k = 1; k < q; ++k) {
-                        const double c = Cb[(k - 1) * q + l];
-                        S.x = fma(c, h[k].x, S.x);
-                        S.y = fma(c, h[k].y, S.y);
-                    }
-                    if (l == 0) {
-                        const cplx lr = t.lrho[o];
-                        acc = cadd(acc, make_double2(A0[a].x * (log_s - lr.x) - A0[a].y * (-lr.y) - S.x,
-                                                     A0[a].x * (-lr.y) + A0[a].y * (log_s - lr.x) - S.y));
-                    } else {
-                        const cplx w = cadd(cscale(A0[a], 1.0 / (double)l), S);
-                        acc = cadd(acc, cscale(cmul(rho[l], w), -sgn));
-                    }
-                } else {
-                    for (int k = 0; k < q; ++k) {
-                        const double c = Cb[k * q + l];
-                        S.x = fma(c, h[k].x, S.x);
-                        S.y = fma(c, h[k].y, S.y);
-                    }
-                    acc = cadd(acc, cscale(cmul(rho[l + 1], S), sgn / s));
-                    if (l == 0) acc = cadd(acc, make_double2(-(A0[0].x - A0[1].y), A0[0].y + A0[1].x));   // -conj(A1_0 + i A2_0)
+    __syncthreads();
+    const int ns = list_n;
+    const cplx *Mlev = mult + level_offset(level) * (long long)(3 * q);
+    cplx nextA = make_double2(0.0, 0.0);
+    if (active && ns > 0) nextA = Mlev[(long long)list_src[0] * (3 * q) + a * q + l];
+    for (int it = 0; it < ns; ++it) {
+        const int o = list_off[it];
+        const cplx *rho = t.rho + (size_t)o * (q + 1);
+        cplx *hb = hat + (it & 1) * 3 * q;
+        if (active) {
+            cplx v = cmul(nextA, rho[l]);
+            if (a < 2 && l >= 1) v = cscale(v, 1.0 / (double)l);
+            hb[a * q + l] = v;
+            if (a < 2 && l == 0) A0[it & 1][a] = nextA;
+            if (it + 1 < ns) nextA = Mlev[(long long)list_src[it + 1] * (3 * q) + a * q + l];   // prefetch
+        }
+        __syncthreads();
+        if (active) {
+            cplx S = make_double2(0.0, 0.0);
+            const cplx *h = hb + a * q;
+            const cplx a0 = A0[it & 1][a < 2 ? a : 0], a1 = A0[it & 1][1];
+            if (a < 2) {
+                for (int k = 1; k < q; ++k) {
+                    const double c = Cb[(k - 1) * q + l];
+                    S.x = fma(c, h[k].x, S.x);
+                    S.y = fma(c, h[k].y, S.y);
                 }
+                if (l == 0) {
+                    const cplx lr = t.lrho[o];
+                    acc = cadd(acc, make_double2(a0.x * (log_s - lr.x) + a0.y * lr.y - S.x,
+                                                 -a0.x * lr.y + a0.y * (log_s - lr.x) - S.y));
+                } else {
+                    const cplx w = cadd(cscale(a0, 1.0 / (double)l), S);
+                    acc = cadd(acc, cscale(cmul(rho[l], w), -sgn));
+                }
+            } else {
+                for (int k = 0; k < q; ++k) {
+                    const double c = Cb[k * q + l];
+                    S.x = fma(c, h[k].x, S.x);
+                    S.y = fma(c, h[k].y, S.y);
+                }
+                acc = cadd(acc, cscale(cmul(rho[l + 1], S), sgn / s));
+                if (l == 0) acc = cadd(acc, make_double2(-(a0.x - a1.y), a0.y + a1.x));   // -conj(A1_0 + i A2_0)
             }
         }
+    }
     if (active) loc[(level_offset(level) + box) * (long long)(3 * q) + a * q + l] = acc;
 }
 
@@ -422,11 +435,13 @@ __global__ void fmm_build_logtab(double *tab)
 }
 
 // ------------------------------------------------------------------------------------------------
-// L2P + P2P: one block per leaf box, one thread per target point (in rounds of 64).
+// L2P + P2P: one block per leaf box; kP2PSplit threads share one target (each takes every kP2PSplit-th source,
+// fixed-order shuffle reduction), targets in rounds of kP2PThreads / kP2PSplit.
 //   far  = -(Re Phi1 + i Re Phi2) + (z/2) conj(Phi1' + i Phi2') - (1/2) conj(psi)   from the box's local expansions
 //   near = direct sum over the points of the 3 x 3 neighbour boxes that belong to OTHER vesicles
 // The sum goes to accum[original point index] (still without the 1/(4 pi mu)).
 constexpr int kP2PThreads = 64;
+constexpr int kP2PSplit = 4;
 __global__ void __launch_bounds__(kP2PThreads)
 fmm_l2p_p2p(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const int *__restrict__ vs,
             const int *__restrict__ perm, const long long *__restrict__ start, int L, int q,
@@ -437,10 +452,11 @@ fmm_l2p_p2p(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const int 
     __shared__ cplx lc[3 * kFmmMaxQ];
     __shared__ double4 src[kP2PThreads];               // (zeta_x, zeta_y, g_x, g_y)
     __shared__ int sves[kP2PThreads];
+    constexpr int kRound = kP2PThreads / kP2PSplit;
     const int n = 1 << L, c = blockIdx.x, ix = c / n, iy = c % n;
     const long long a = start[c], b = start[c + 1];
     if (a == b) return;
-    const int tid = threadIdx.x;
+    const int tid = threadIdx.x, slot = tid / kP2PSplit, part = tid % kP2PSplit;
     for (int e = tid; e < kLogTab + kExpTab; e += kP2PThreads) tab[e] = logtab[e];
     for (int e = tid; e < 3 * q; e += kP2PThreads) lc[e] = loc[(level_offset(L) + c) * (long long)(3 * q) + e];
     const Geom gm = load_geom(enc);
@@ -448,8 +464,8 @@ fmm_l2p_p2p(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const int 
     const cplx ctr = box_centre(gm, L, ix, iy);
     __syncthreads();
 
-    for (long long t0 = a; t0 < b; t0 += kP2PThreads) {
-        const long long ti = t0 + tid;
+    for (long long t0 = a; t0 < b; t0 += kRound) {
+        const long long ti = t0 + slot;
         const bool live = ti < b;
         cplx z = make_double2(0.0, 0.0);
         int myves = -1;
@@ -457,6 +473,8 @@ fmm_l2p_p2p(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const int 
         if (live) {
             z = zs[ti];
             myves = vs[ti];
+        }
+        if (live && part == 0) {
             // far field: Horner for value and derivative of the three local expansions
             const cplx t = make_double2((z.x - ctr.x) * inv_s, (z.y - ctr.y) * inv_s);
             cplx p1 = lc[q - 1], p2 = lc[2 * q - 1], p3 = lc[3 * q - 1];
@@ -488,7 +506,7 @@ fmm_l2p_p2p(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const int 
                     __syncthreads();
                     const int cnt = (int)min((long long)kP2PThreads, sb - s0);
                     if (live)
-                        for (int j = 0; j < cnt; ++j) {
+                        for (int j = part; j < cnt; j += kP2PSplit) {
                             if (sves[j] == myves) continue;
                             const double4 sj = src[j];
                             const double rx = z.x - sj.x, ry = z.y - sj.y;
@@ -501,7 +519,12 @@ fmm_l2p_p2p(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const int 
                         }
                 }
             }
-        if (live) accum[perm[ti]] = make_double2(ux, uy);
+#pragma unroll
+        for (int m = 1; m < kP2PSplit; m <<= 1) {
+            ux += __shfl_xor_sync(0xffffffffu, ux, m);
+            uy += __shfl_xor_sync(0xffffffffu, uy, m);
+        }
+        if (live && part == 0) accum[perm[ti]] = make_double2(ux, uy);
         __syncthreads();
     }
 }
@@ -516,13 +539,13 @@ fmm_finish(const cplx *__restrict__ z, const cplx *__restrict__ g, const int *__
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= P) return;
     const int n = 1 << L;
-    const int ci = cell[i], ix = ci / n, iy = ci % n;
+    const int ci = cell[i], ix = ci >> L, iy = ci & (n - 1);
     const cplx zi = z[i];
     const int v0 = (i / npts) * npts;
     double cx = 0.0, cy = 0.0;
     for (int j = v0; j < v0 + npts; ++j) {
         const int cj = cell[j];
-        if (abs(cj / n - ix) <= 1 && abs(cj % n - iy) <= 1) continue;
+        if (abs((cj >> L) - ix) <= 1 && abs((cj & (n - 1)) - iy) <= 1) continue;
         const cplx gj = g[j];
         const double rx = zi.x - z[j].x, ry = zi.y - z[j].y;
         const double r2 = rx * rx + ry * ry;
@@ -604,9 +627,10 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
         fmm_m2m<<<(unsigned)((work + 127) / 128), 128, 0, st>>>(l, q, tab, mult, boxcnt);
         ++launches;
     }
-    const size_t smem_m2l = sizeof(double) * (size_t)(((q * q + 1) & ~1) + 6 * q);
+    const size_t smem_m2l = sizeof(double) * (size_t)(((q * q + 1) & ~1) + 12 * q);
+    const int thr_m2l = (3 * q + 31) & ~31;
     for (int l = 2; l <= L; ++l) {
-        fmm_m2l<<<1u << (2 * l), 192, smem_m2l, st>>>(l, q, tab, enc, mult, boxcnt, loc);
+        fmm_m2l<<<1u << (2 * l), thr_m2l, smem_m2l, st>>>(l, q, tab, enc, mult, boxcnt, loc);
         ++launches;
     }
     for (int l = 3; l <= L; ++l) {
