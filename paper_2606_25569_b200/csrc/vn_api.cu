@@ -94,7 +94,9 @@ SymSplit choose_sym_split(long long P, int super_tile, int slots, int min_tiles)
 
 static vn_status check_device()
 {
-    static int ok = -1;   // -1 unknown, 1 ok, 0 unsupported
+    static int state_dev[kMaxDevices] = {0};   // 0 unknown, 1 ok, 2 unsupported
+    int &state = state_dev[current_device()];
+    int ok = state == 0 ? -1 : (state == 1 ? 1 : 0);
     if (ok < 0) {
         int dev = 0, major = 0;
         VN_CUDA(cudaGetDevice(&dev));
@@ -109,6 +111,7 @@ static vn_status check_device()
             }
         }
     }
+    state = ok ? 1 : 2;
     return ok ? VN_OK : VN_ERR_UNSUPPORTED;
 }
 
@@ -268,7 +271,12 @@ vn_status vn_farfield_host(const void *X, const void *F, const void *W, int64_t 
     static cudaStream_t st = nullptr;
     static char *buf = nullptr;
     static size_t cap = 0;
+    static int owner = -1;                          // device the cached stream and buffer belong to
     std::lock_guard<std::mutex> lock(mtx);
+    if (owner != current_device()) {                // first call, or the caller switched devices: start afresh
+        st = nullptr; buf = nullptr; cap = 0;       // (the old device's stream and buffer are left to that context)
+        owner = current_device();
+    }
     if (!st) VN_CUDA(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking));
     const size_t P = (size_t)(nves * npts);
     const size_t es = precision == VN_F32 ? 4 : 8;

@@ -21,6 +21,15 @@ constexpr int kStages = 4;         // tiles in flight per block
 extern unsigned long long g_launches;
 inline void count_launch(int n = 1) { __atomic_fetch_add(&g_launches, (unsigned long long)n, __ATOMIC_RELAXED); }
 
+// per-device caches (occupancy, function attributes, capability check) are indexed by the current device
+constexpr int kMaxDevices = 64;
+inline int current_device()
+{
+    int d = 0;
+    if (cudaGetDevice(&d) != cudaSuccess || d < 0 || d >= kMaxDevices) d = 0;
+    return d;
+}
+
 // optional event pair around the pair kernel (vn_profile_enable / vn_profile_read)
 void profile_mark(cudaStream_t st, bool begin);
 

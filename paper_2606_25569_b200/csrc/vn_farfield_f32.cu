@@ -373,7 +373,8 @@ vn_status farfield_f32(const void *X, const void *F, const void *W, int64_t nves
                        void *U, cudaStream_t st, const int64_t *near_ptr, const int32_t *near_ves)
 {
     const int P = (int)(nves * npts);
-    static int slots = 0;
+    static int slots_dev[kMaxDevices] = {0};
+    int &slots = slots_dev[current_device()];
     if (slots == 0) {
         int dev = 0, sms = 0, occ = 0;
         VN_CUDA(cudaGetDevice(&dev));
@@ -416,8 +417,11 @@ vn_status farfield_f32(const void *X, const void *F, const void *W, int64_t nves
 //   r = x - y; r2 = rx*rx + ry*ry; A += lg2(r2) * g; d = rx*gx + ry*gy; B += (d / r2) * r
 // (2 FADD + 3 FMUL + 6 FFMA + 1.5 MUFU with the shared reciprocal), 8 targets per thread as packed
 // pairs, the same tile ring, per-tile partial sums folded into running sums, fixed-point atomics out.
+#ifndef VN_F32_TGT_MINBLK
+#define VN_F32_TGT_MINBLK 4
+#endif
 template <int NP>
-__global__ void __launch_bounds__(kThreads, 4)
+__global__ void __launch_bounds__(kThreads, VN_F32_TGT_MINBLK)
 targets_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict__ Xt, int nt_pts, int P,
                    int n_tiles, int n_chunks, const unsigned *__restrict__ gmax_bits, long long *__restrict__ acc)
 {
@@ -539,7 +543,8 @@ vn_status farfield_targets_f32(const void *Xt, int64_t nt, const void *X, const 
                                int64_t nves, int64_t npts, double mu, void *Ut, cudaStream_t st)
 {
     const int P = (int)(nves * npts), n = (int)nt;
-    static int slots = 0;
+    static int slots_dev[kMaxDevices] = {0};
+    int &slots = slots_dev[current_device()];
     if (slots == 0) {
         int dev = 0, sms = 0, occ = 0;
         VN_CUDA(cudaGetDevice(&dev));

@@ -271,7 +271,8 @@ vn_status farfield_f64(const void *X, const void *F, const void *W, int64_t nves
                        void *U, cudaStream_t st, const int64_t *near_ptr, const int32_t *near_ves)
 {
     const int P = (int)(nves * npts);
-    static int slots = 0;
+    static int slots_dev[kMaxDevices] = {0};
+    int &slots = slots_dev[current_device()];
     if (slots == 0) {
         int dev = 0, sms = 0, occ = 0;
         VN_CUDA(cudaGetDevice(&dev));
@@ -309,7 +310,10 @@ vn_status farfield_f64(const void *X, const void *F, const void *W, int64_t nves
 // ------------------------------------------------------------------------------------------------
 // Row f-4: free targets in double (see targets_f32_kernel): one-directional sum over ALL vesicles,
 // 4 targets per thread, per pair  acc += ml * g + ((r.g) inv) * r  (22 DP instructions).
-__global__ void __launch_bounds__(kThreads, 4)
+#ifndef VN_F64_TGT_MINBLK
+#define VN_F64_TGT_MINBLK 4
+#endif
+__global__ void __launch_bounds__(kThreads, VN_F64_TGT_MINBLK)
 targets_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__ Xt, int nt_pts, int P,
                    int n_tiles, int n_chunks, const unsigned long long *__restrict__ gmax_bits,
                    long long *__restrict__ acc)
@@ -401,7 +405,8 @@ vn_status farfield_targets_f64(const void *Xt, int64_t nt, const void *X, const 
                                int64_t nves, int64_t npts, double mu, void *Ut, cudaStream_t st)
 {
     const int P = (int)(nves * npts), n = (int)nt;
-    static int slots = 0;
+    static int slots_dev[kMaxDevices] = {0};
+    int &slots = slots_dev[current_device()];
     if (slots == 0) {
         int dev = 0, sms = 0, occ = 0;
         VN_CUDA(cudaGetDevice(&dev));

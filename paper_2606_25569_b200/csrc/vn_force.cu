@@ -103,7 +103,8 @@ vn_status elastic_force(const void *X, const void *sigma, int64_t nves, int64_t 
 {
     const int N = (int)npts;
     const size_t smem = sizeof(double) * 8 * (size_t)N;
-    static bool attr_set = false;
+    static bool attr_dev[kMaxDevices] = {false};
+    bool &attr_set = attr_dev[current_device()];
     if (!attr_set) {
         VN_CUDA(cudaFuncSetAttribute(elastic_force_kernel<float, float2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024));
         VN_CUDA(cudaFuncSetAttribute(elastic_force_kernel<double, double2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024));

@@ -182,7 +182,8 @@ vn_status redistribute(const void *X, int64_t nves, int64_t npts, void *Xnew, vn
 {
     const int N = (int)npts, M = kUp * N;
     const size_t smem = redistribute_smem(N);
-    static bool attr_set = false;
+    static bool attr_dev[kMaxDevices] = {false};
+    bool &attr_set = attr_dev[current_device()];
     if (!attr_set) {
         const int cap = (int)redistribute_smem(512);
         VN_CUDA(cudaFuncSetAttribute(redistribute_kernel<float, float2>, cudaFuncAttributeMaxDynamicSharedMemorySize, cap));
