@@ -304,7 +304,8 @@ def main():
                          "aux: the O(P) rows around the sum (f-3 redistribution, a-1 weights, f-2 elastic force), "
                          "reported in points/s; fmm: vn_farfield_fmm (approximate, O(P)), reported in the direct sum's "
                          "interactions per second so that it compares with --path farfield")
-    ap.add_argument("--order", type=int, default=0, help="expansion order of --path fmm (default 12 for f32, 38 for f64)")
+    ap.add_argument("--order", type=int, default=0, help="expansion order of --path fmm (default 12 for f32, 38 for f64); with --path targets a value > 0 "
+                         "selects vn_farfield_targets_fmm")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -370,7 +371,7 @@ def main():
             vn.vn_near_pairs(X_d, W_d, near_ptr, near_ves)
             vn.vn_farfield_masked(X_d, F_d, W_d, near_ptr, near_ves, susp.mu, out=U_d)
         else:
-            vn.vn_farfield_targets(Xt_d, X_d, F_d, W_d, susp.mu, out=Ut_d)
+            vn.vn_farfield_targets(Xt_d, X_d, F_d, W_d, susp.mu, out=Ut_d, fmm_order=args.order)   # --order > 0: FMM
 
     def step_device():
         for c in range(evals):
@@ -501,6 +502,10 @@ def main():
                                   "pinned host buffers -> device copies -> the path's C-ABI calls -> copy back, synchronised"}
         if args.path == "masked":
             line["config"]["near_pairs"] = n_near
+        if args.path == "targets" and args.order > 0:
+            line["config"]["order"] = args.order
+            line["roofline"]["kernel"] = "fmm kernels (P2M, M2M, M2L, L2L, L2P+P2P)"
+            line["roofline"]["note"] = "approximate algorithm (vn_farfield_targets_fmm): 'achieved' counts the direct sum's interactions"
         if args.path == "fmm":
             line["config"]["order"] = fmm_order
             line["roofline"]["note"] = ("approximate algorithm: 'achieved' counts the interactions of the direct sum it replaces, "

@@ -148,10 +148,22 @@ vn_status vn_farfield_targets(const void *Xt, int64_t nt,
  * Arithmetic is double inside for both storage precisions, so the VN_F32 result is the double
  * result rounded once.  Uniform quadtree over the bounding square of the points; a strongly
  * non-uniform point distribution costs time (crowded leaves), not accuracy.  Results are bitwise
- * reproducible.  Scratch: about 100 * (p+1) bytes per leaf box plus 100 bytes per point. */
+ * reproducible.  Scratch: about 100 * (p+1) bytes per leaf box plus 100 bytes per point.
+ * near_ptr / near_ves: NULL for the plain sum (vn_farfield's quantity), or the CSR near-field
+ * relation of vn_near_pairs: then the listed vesicles' contributions are zeroed as in
+ * vn_farfield_masked (the paper's DirectSingleLayerIntegral in O(P)). */
 vn_status vn_farfield_fmm(const void *X, const void *F, const void *W,
                           int64_t nves, int64_t npts, double mu, int order,
+                          const int64_t *near_ptr, const int32_t *near_ves,
                           void *U, vn_precision precision, void *stream);
+
+/* vn_farfield_targets (free targets, all vesicles contribute) by the same fast multipole method: the
+ * sources build the tree and the local expansions, the nt targets are sorted into the same leaves.
+ * Same approximation and `order` semantics as vn_farfield_fmm, same conventions as vn_farfield_targets. */
+vn_status vn_farfield_targets_fmm(const void *Xt, int64_t nt,
+                                  const void *X, const void *F, const void *W,
+                                  int64_t nves, int64_t npts, double mu, int order,
+                                  void *Ut, vn_precision precision, void *stream);
 
 /* ---- row f-2: the elastic membrane force (the producer of F) -----------------------------------
  * PAPER.md:123 eq 2.7, :319 Fig. 5b:

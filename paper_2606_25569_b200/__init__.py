@@ -64,8 +64,10 @@ def lib():
         L.vn_elastic_force.restype = ci
         L.vn_redistribute_arclength.argtypes = [vp, i64, i64, vp, ci, vp]
         L.vn_redistribute_arclength.restype = ci
-        L.vn_farfield_fmm.argtypes = [vp, vp, vp, i64, i64, dbl, ci, vp, ci, vp]
+        L.vn_farfield_fmm.argtypes = [vp, vp, vp, i64, i64, dbl, ci, vp, vp, vp, ci, vp]
         L.vn_farfield_fmm.restype = ci
+        L.vn_farfield_targets_fmm.argtypes = [vp, i64, vp, vp, vp, i64, i64, dbl, ci, vp, ci, vp]
+        L.vn_farfield_targets_fmm.restype = ci
         L.vn_profile_enable.argtypes = [ci]
         L.vn_profile_enable.restype = ci
         L.vn_profile_read.argtypes = [ctypes.POINTER(dbl), i64]
@@ -126,8 +128,9 @@ def vn_farfield(X, F, W, mu: float = 1.0, out=None, stream=None):
     return out
 
 
-def vn_farfield_fmm(X, F, W, mu: float = 1.0, order: int = 12, out=None, stream=None):
-    """The far-field sum by the fast multipole method with `order` expansion terms (approximate, O(P))."""
+def vn_farfield_fmm(X, F, W, mu: float = 1.0, order: int = 12, out=None, stream=None, near_ptr=None, near_ves=None):
+    """The far-field sum by the fast multipole method with `order` expansion terms (approximate, O(P));
+    with the CSR relation of vn_near_pairs the near vesicles' contributions are zeroed as in vn_farfield_masked."""
     import torch
     nves, npts, two = X.shape
     if two != 2:
@@ -139,7 +142,12 @@ def vn_farfield_fmm(X, F, W, mu: float = 1.0, order: int = 12, out=None, stream=
         out = torch.empty_like(X)
     _check_dev("out", out, X.shape, X.dtype)
     with torch.cuda.device(X.device):
+        if near_ptr is not None:
+            _check_dev("near_ptr", near_ptr, (nves * npts + 1,), torch.int64)
+            _check_dev("near_ves", near_ves, None, torch.int32)
         rc = lib().vn_farfield_fmm(X.data_ptr(), F.data_ptr(), W.data_ptr(), nves, npts, float(mu), int(order),
+                                   None if near_ptr is None else near_ptr.data_ptr(),
+                                   None if near_ptr is None or near_ves.numel() == 0 else near_ves.data_ptr(),
                                    out.data_ptr(), _prec(X), _stream_ptr(stream))
     if rc != VN_OK:
         raise VesnetError(rc, "vn_farfield_fmm")
@@ -217,8 +225,9 @@ def vn_farfield_masked(X, F, W, near_ptr, near_ves, mu: float = 1.0, out=None, s
     return out
 
 
-def vn_farfield_targets(Xt, X, F, W, mu: float = 1.0, out=None, stream=None):
-    """Velocity at free points Xt[nt, 2] induced by all vesicles (device tensors)."""
+def vn_farfield_targets(Xt, X, F, W, mu: float = 1.0, out=None, stream=None, fmm_order: int = 0):
+    """Velocity at free points Xt[nt, 2] induced by all vesicles (device tensors); fmm_order > 0 selects
+    vn_farfield_targets_fmm with that expansion order (approximate, O(P + nt))."""
     import torch
     nves, npts, two = X.shape
     if two != 2 or Xt.dim() != 2 or Xt.shape[1] != 2:
@@ -231,9 +240,13 @@ def vn_farfield_targets(Xt, X, F, W, mu: float = 1.0, out=None, stream=None):
         out = torch.empty_like(Xt)
     _check_dev("out", out, Xt.shape, X.dtype)
     with torch.cuda.device(X.device):
-        rc = lib().vn_farfield_targets(Xt.data_ptr() if Xt.numel() else None, Xt.shape[0], X.data_ptr(), F.data_ptr(),
-                                       W.data_ptr(), nves, npts, float(mu),
-                                       out.data_ptr() if Xt.numel() else None, _prec(X), _stream_ptr(stream))
+        pt, po = (Xt.data_ptr(), out.data_ptr()) if Xt.numel() else (None, None)
+        if fmm_order > 0:
+            rc = lib().vn_farfield_targets_fmm(pt, Xt.shape[0], X.data_ptr(), F.data_ptr(), W.data_ptr(), nves, npts,
+                                               float(mu), int(fmm_order), po, _prec(X), _stream_ptr(stream))
+        else:
+            rc = lib().vn_farfield_targets(pt, Xt.shape[0], X.data_ptr(), F.data_ptr(), W.data_ptr(), nves, npts,
+                                           float(mu), po, _prec(X), _stream_ptr(stream))
     if rc != VN_OK:
         raise VesnetError(rc, "vn_farfield_targets")
     return out

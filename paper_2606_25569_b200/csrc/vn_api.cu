@@ -39,7 +39,9 @@ vn_status elastic_force(const void *X, const void *sigma, int64_t nves, int64_t 
                         vn_precision prec, cudaStream_t st);
 vn_status redistribute(const void *X, int64_t nves, int64_t npts, void *Xnew, vn_precision prec, cudaStream_t st);
 vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, double mu, int order,
-                       void *U, vn_precision prec, cudaStream_t st);
+                       const int64_t *near_ptr, const int32_t *near_ves, void *U, vn_precision prec, cudaStream_t st);
+vn_status farfield_targets_fmm(const void *Xt, int64_t nt, const void *X, const void *F, const void *W, int64_t nves,
+                               int64_t npts, double mu, int order, void *Ut, vn_precision prec, cudaStream_t st);
 vn_status near_pairs(const void *X, const void *W, int64_t nves, int64_t npts, int64_t *near_ptr,
                      int32_t *near_ves, int64_t capacity, vn_precision prec, cudaStream_t st);
 vn_status arclength_weights(const void *X, int64_t nves, int64_t npts, void *W, vn_precision prec, cudaStream_t st);
@@ -242,8 +244,10 @@ vn_status vn_redistribute_arclength(const void *X, int64_t nves, int64_t npts, v
 }
 
 vn_status vn_farfield_fmm(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, double mu,
-                          int order, void *U, vn_precision precision, void *stream)
+                          int order, const int64_t *near_ptr, const int32_t *near_ves, void *U,
+                          vn_precision precision, void *stream)
 {
+    if (misaligned(near_ptr, 8) || misaligned(near_ves, 4)) return VN_ERR_INVALID_ARG;
     if (!X || !F || !W || !U) return VN_ERR_INVALID_ARG;
     if (check_shape(nves, npts, precision) != VN_OK) return VN_ERR_INVALID_ARG;
     if (!isfinite(mu) || !(mu > 0.0) || order < 2 || order > 48) return VN_ERR_INVALID_ARG;
@@ -253,7 +257,27 @@ vn_status vn_farfield_fmm(const void *X, const void *F, const void *W, int64_t n
     if (U == X || U == F || U == W) return VN_ERR_INVALID_ARG;
     const vn_status ds = check_device();
     if (ds != VN_OK) return ds;
-    return farfield_fmm(X, F, W, nves, npts, mu, order, U, precision, (cudaStream_t)stream);
+    return farfield_fmm(X, F, W, nves, npts, mu, order, near_ptr, near_ves, U, precision, (cudaStream_t)stream);
+}
+
+vn_status vn_farfield_targets_fmm(const void *Xt, int64_t nt, const void *X, const void *F, const void *W,
+                                  int64_t nves, int64_t npts, double mu, int order, void *Ut,
+                                  vn_precision precision, void *stream)
+{
+    if (!X || !F || !W) return VN_ERR_INVALID_ARG;
+    if (check_shape(nves, npts, precision) != VN_OK) return VN_ERR_INVALID_ARG;
+    if (nt < 0 || nt >= (1ll << 31) || order < 2 || order > 48) return VN_ERR_INVALID_ARG;
+    if (!isfinite(mu) || !(mu > 0.0)) return VN_ERR_INVALID_ARG;
+    if (nt == 0) return VN_OK;
+    if (!Xt || !Ut) return VN_ERR_INVALID_ARG;
+    const size_t pair = precision == VN_F32 ? 8 : 16;
+    if (misaligned(X, pair) || misaligned(F, pair) || misaligned(Xt, pair) || misaligned(Ut, pair) ||
+        misaligned(W, pair / 2))
+        return VN_ERR_INVALID_ARG;
+    if (Ut == X || Ut == F || Ut == W || Ut == Xt) return VN_ERR_INVALID_ARG;
+    const vn_status ds = check_device();
+    if (ds != VN_OK) return ds;
+    return farfield_targets_fmm(Xt, nt, X, F, W, nves, npts, mu, order, Ut, precision, (cudaStream_t)stream);
 }
 
 vn_status vn_farfield_host(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, double mu,

@@ -188,6 +188,8 @@ __device__ __forceinline__ double fixed2_value(long long hi, long long lo, const
 // near vesicles' contributions from the fixed-point accumulators before the final rounding
 vn_status near_correction_f32(const void *X, const void *F, const void *W, int P, int npts, const int64_t *near_ptr,
                               const int32_t *near_ves, long long *acc, const unsigned *gmax_bits, cudaStream_t st);
+vn_status near_correction_accum(const void *X, const void *F, const void *W, int P, int npts, const int64_t *near_ptr,
+                                const int32_t *near_ves, double2 *accum, vn_precision prec, cudaStream_t st);
 vn_status near_correction_f64(const void *X, const void *F, const void *W, int P, int npts, const int64_t *near_ptr,
                               const int32_t *near_ves, long long *acc, const unsigned long long *gmax_bits,
                               cudaStream_t st);

@@ -444,17 +444,19 @@ constexpr int kP2PThreads = 64;
 constexpr int kP2PSplit = 4;
 __global__ void __launch_bounds__(kP2PThreads)
 fmm_l2p_p2p(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const int *__restrict__ vs,
-            const int *__restrict__ perm, const long long *__restrict__ start, int L, int q,
+            const long long *__restrict__ start, const cplx *__restrict__ tz, const int *__restrict__ tvs,
+            const int *__restrict__ tperm, const long long *__restrict__ tstart, int L, int q,
             const unsigned long long *__restrict__ enc, const cplx *__restrict__ loc, const double *__restrict__ logtab,
             cplx *__restrict__ accum)
-{
+{   // targets (tz, tvs, tperm, tstart) are the sorted sources themselves for vn_farfield_fmm, a separate sorted set
+    // (tvs == nullptr: no vesicle to exclude) for the free-target variant
     __shared__ double tab[kLogTab + kExpTab];
     __shared__ cplx lc[3 * kFmmMaxQ];
     __shared__ double4 src[kP2PThreads];               // (zeta_x, zeta_y, g_x, g_y)
     __shared__ int sves[kP2PThreads];
     constexpr int kRound = kP2PThreads / kP2PSplit;
     const int n = 1 << L, c = blockIdx.x, ix = c / n, iy = c % n;
-    const long long a = start[c], b = start[c + 1];
+    const long long a = tstart[c], b = tstart[c + 1];
     if (a == b) return;
     const int tid = threadIdx.x, slot = tid / kP2PSplit, part = tid % kP2PSplit;
     for (int e = tid; e < kLogTab + kExpTab; e += kP2PThreads) tab[e] = logtab[e];
@@ -471,8 +473,8 @@ fmm_l2p_p2p(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const int 
         int myves = -1;
         double ux = 0.0, uy = 0.0;
         if (live) {
-            z = zs[ti];
-            myves = vs[ti];
+            z = tz[ti];
+            myves = tvs ? tvs[ti] : -1;
         }
         if (live && part == 0) {
             // far field: Horner for value and derivative of the three local expansions
@@ -524,7 +526,7 @@ fmm_l2p_p2p(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const int 
             ux += __shfl_xor_sync(0xffffffffu, ux, m);
             uy += __shfl_xor_sync(0xffffffffu, uy, m);
         }
-        if (live && part == 0) accum[perm[ti]] = make_double2(ux, uy);
+        if (live && part == 0) accum[tperm[ti]] = make_double2(ux, uy);
         __syncthreads();
     }
 }
@@ -574,7 +576,7 @@ static int fmm_levels(long long P, int order)
 }
 
 vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, double mu, int order,
-                       void *U, vn_precision prec, cudaStream_t st)
+                       const int64_t *near_ptr, const int32_t *near_ves, void *U, vn_precision prec, cudaStream_t st)
 {
     const int P = (int)(nves * npts), q = order + 1;
     const int L = fmm_levels(P, order);
@@ -638,13 +640,162 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
         fmm_l2l<<<(unsigned)((work + 127) / 128), 128, 0, st>>>(l, q, tab, loc);
         ++launches;
     }
-    fmm_l2p_p2p<<<ncell, kP2PThreads, 0, st>>>(zs, gs, vs, perm, start, L, q, enc, loc, logtab, accum);
+    fmm_l2p_p2p<<<ncell, kP2PThreads, 0, st>>>(zs, gs, vs, start, zs, vs, perm, start, L, q, enc, loc, logtab, accum);
     profile_mark(st, false);
+    if (near_ptr) {   // row f-1 on top: take the near vesicles' contributions out (they are all in the direct part)
+        const vn_status rc = near_correction_accum(X, F, W, P, (int)npts, near_ptr, near_ves, accum, prec, st);
+        if (rc != VN_OK) { (void)cudaFreeAsync(scr, st); return rc; }
+    }
     const double pref = 1.0 / (4.0 * 3.14159265358979323846 * mu);
     if (prec == VN_F32)
         fmm_finish<float2><<<(P + 127) / 128, 128, 0, st>>>(z, g, cell, P, (int)npts, L, accum, pref, (float2 *)U);
     else
         fmm_finish<double2><<<(P + 127) / 128, 128, 0, st>>>(z, g, cell, P, (int)npts, L, accum, pref, (double2 *)U);
+    count_launch(launches + 2);
+    const cudaError_t e = cudaGetLastError();
+    VN_CUDA(cudaFreeAsync(scr, st));
+    return e == cudaSuccess ? VN_OK : VN_ERR_CUDA;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Free targets by the same method (row f-4, both halves together): the sources build the tree and the local
+// expansions exactly as above, the nt targets are sorted into the same leaves, and every target gets its
+// leaf's local expansions plus the direct sum over the 3 x 3 neighbour leaves.  No vesicle is excluded.
+template <typename real2>
+__global__ void __launch_bounds__(256)
+fmm_load_targets(const real2 *__restrict__ Xt, int nt, cplx *__restrict__ zt, unsigned long long *__restrict__ enc)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    double x = INFINITY, y = INFINITY, X1 = -INFINITY, Y1 = -INFINITY;
+    if (i < nt) {
+        const real2 p = Xt[i];
+        x = X1 = (double)p.x;
+        y = Y1 = (double)p.y;
+        zt[i] = make_double2(x, y);
+    }
+#pragma unroll
+    for (int m = 16; m >= 1; m >>= 1) {
+        x = fmin(x, __shfl_xor_sync(0xffffffffu, x, m));
+        y = fmin(y, __shfl_xor_sync(0xffffffffu, y, m));
+        X1 = fmax(X1, __shfl_xor_sync(0xffffffffu, X1, m));
+        Y1 = fmax(Y1, __shfl_xor_sync(0xffffffffu, Y1, m));
+    }
+    if ((threadIdx.x & 31) == 0 && x <= X1) {
+        atomicMin(enc + 0, enc_f64(x));
+        atomicMin(enc + 1, enc_f64(y));
+        atomicMax(enc + 2, enc_f64(X1));
+        atomicMax(enc + 3, enc_f64(Y1));
+    }
+}
+
+__global__ void __launch_bounds__(256)
+fmm_gather_targets(const int *__restrict__ perm, int nt, const cplx *__restrict__ zt, cplx *__restrict__ zts)
+{
+    const int q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q < nt) zts[q] = zt[perm[q]];
+}
+
+template <typename real2>
+__global__ void __launch_bounds__(256)
+fmm_finish_targets(const cplx *__restrict__ accum, int nt, double prefactor, real2 *__restrict__ Ut)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= nt) return;
+    real2 o;
+    o.x = (decltype(o.x))(prefactor * accum[i].x);
+    o.y = (decltype(o.y))(prefactor * accum[i].y);
+    Ut[i] = o;
+}
+
+vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, const void *F, const void *W, int64_t nves,
+                               int64_t npts, double mu, int order, void *Ut, vn_precision prec, cudaStream_t st)
+{
+    const int P = (int)(nves * npts), nt = (int)nt64, q = order + 1;
+    const int L = fmm_levels(P > nt ? P : nt, order);
+    const int n = 1 << L, ncell = n * n;
+    const long long nbox = level_offset(L + 1);
+    const int nb_scan = (ncell + kScanBlock - 1) / kScanBlock;
+    auto up = [](size_t b) { return (b + 255) & ~(size_t)255; };
+    const size_t b_pt = up(sizeof(cplx) * (size_t)P), b_int = up(sizeof(int) * (size_t)P);
+    const size_t b_tpt = up(sizeof(cplx) * (size_t)nt), b_tint = up(sizeof(int) * (size_t)nt);
+    const size_t b_exp = up(sizeof(cplx) * (size_t)nbox * 3 * q), b_cnt = up(sizeof(int) * (size_t)nbox);
+    const size_t b_ccnt = up(sizeof(int) * (size_t)ncell);
+    const size_t b_start = up(sizeof(long long) * ((size_t)ncell + 1)), b_bs = up(sizeof(long long) * (size_t)nb_scan);
+    const size_t b_tab = up(sizeof(double) * fmm_tables_doubles(q)), b_log = up(sizeof(double) * (kLogTab + kExpTab));
+    const size_t total = 4 * b_pt + 3 * b_int + 3 * b_tpt + 2 * b_tint + 2 * b_exp + b_cnt + b_ccnt + 4 * b_start +
+                         b_bs + b_tab + b_log + 256;
+    char *scr = nullptr;
+    VN_CUDA(cudaMallocAsync((void **)&scr, total, st));
+    char *ptr = scr;
+    auto take = [&](size_t b) { char *r = ptr; ptr += b; return r; };
+    cplx *z = (cplx *)take(b_pt), *g = (cplx *)take(b_pt), *zs = (cplx *)take(b_pt), *gs = (cplx *)take(b_pt);
+    int *cell = (int *)take(b_int), *perm = (int *)take(b_int), *vs = (int *)take(b_int);
+    cplx *zt = (cplx *)take(b_tpt), *zts = (cplx *)take(b_tpt), *accum = (cplx *)take(b_tpt);
+    int *tcell = (int *)take(b_tint), *tperm = (int *)take(b_tint);
+    cplx *mult = (cplx *)take(b_exp), *loc = (cplx *)take(b_exp);
+    int *boxcnt = (int *)take(b_cnt), *tcnt = (int *)take(b_ccnt);
+    long long *start = (long long *)take(b_start), *cursor = (long long *)take(b_start);
+    long long *tstart = (long long *)take(b_start), *tcursor = (long long *)take(b_start), *bsum = (long long *)take(b_bs);
+    double *tab = (double *)take(b_tab), *logtab = (double *)take(b_log);
+    unsigned long long *enc = (unsigned long long *)take(256);
+    int *cnt = boxcnt + level_offset(L);
+
+    VN_CUDA(cudaMemsetAsync(boxcnt, 0, b_cnt + b_ccnt, st));       // boxcnt and tcnt are adjacent
+    fmm_init_bounds<<<1, 1, 0, st>>>(enc);
+    const int gp = (P + 255) / 256, gt = (nt + 255) / 256;
+    if (prec == VN_F32) {
+        fmm_load<float, float2><<<gp, 256, 0, st>>>((const float2 *)X, (const float2 *)F, (const float *)W, P, z, g, enc);
+        fmm_load_targets<float2><<<gt, 256, 0, st>>>((const float2 *)Xt, nt, zt, enc);
+    } else {
+        fmm_load<double, double2><<<gp, 256, 0, st>>>((const double2 *)X, (const double2 *)F, (const double *)W, P, z, g, enc);
+        fmm_load_targets<double2><<<gt, 256, 0, st>>>((const double2 *)Xt, nt, zt, enc);
+    }
+    // sources into leaves
+    fmm_bin<<<gp, 256, 0, st>>>(z, P, L, enc, cell, cnt);
+    scan_block_sums<<<nb_scan, kScanThreads, 0, st>>>(cnt, ncell, bsum);
+    scan_of_sums<<<1, kScanThreads, 0, st>>>(bsum, nb_scan);
+    scan_apply<<<nb_scan, kScanThreads, 0, st>>>(cnt, ncell, bsum, start, cursor);
+    fmm_scatter<<<gp, 256, 0, st>>>(cell, P, cursor, perm);
+    fmm_sort_cells<<<(ncell + 127) / 128, 128, 0, st>>>(start, ncell, perm);
+    fmm_gather<<<gp, 256, 0, st>>>(perm, P, (int)npts, z, g, zs, gs, vs);
+    // targets into the same leaves
+    fmm_bin<<<gt, 256, 0, st>>>(zt, nt, L, enc, tcell, tcnt);
+    scan_block_sums<<<nb_scan, kScanThreads, 0, st>>>(tcnt, ncell, bsum);
+    scan_of_sums<<<1, kScanThreads, 0, st>>>(bsum, nb_scan);
+    scan_apply<<<nb_scan, kScanThreads, 0, st>>>(tcnt, ncell, bsum, tstart, tcursor);
+    fmm_scatter<<<gt, 256, 0, st>>>(tcell, nt, tcursor, tperm);
+    fmm_sort_cells<<<(ncell + 127) / 128, 128, 0, st>>>(tstart, ncell, tperm);
+    fmm_gather_targets<<<gt, 256, 0, st>>>(tperm, nt, zt, zts);
+    fmm_build_tables<<<64, 128, 0, st>>>(q, tab);
+    fmm_build_logtab<<<8, 128, 0, st>>>(logtab);
+    int launches = 20;
+
+    profile_mark(st, true);
+    fmm_p2m<<<(ncell + 3) / 4, 128, 0, st>>>(zs, gs, start, L, q, enc, mult);
+    ++launches;
+    for (int l = L - 1; l >= 2; --l) {
+        const long long work = (1ll << (2 * l)) * q;
+        fmm_m2m<<<(unsigned)((work + 127) / 128), 128, 0, st>>>(l, q, tab, mult, boxcnt);
+        ++launches;
+    }
+    const size_t smem_m2l = sizeof(double) * (size_t)(((q * q + 1) & ~1) + 12 * q);
+    const int thr_m2l = (3 * q + 31) & ~31;
+    for (int l = 2; l <= L; ++l) {
+        fmm_m2l<<<1u << (2 * l), thr_m2l, smem_m2l, st>>>(l, q, tab, enc, mult, boxcnt, loc);
+        ++launches;
+    }
+    for (int l = 3; l <= L; ++l) {
+        const long long work = (1ll << (2 * l)) * q;
+        fmm_l2l<<<(unsigned)((work + 127) / 128), 128, 0, st>>>(l, q, tab, loc);
+        ++launches;
+    }
+    fmm_l2p_p2p<<<ncell, kP2PThreads, 0, st>>>(zs, gs, vs, start, zts, nullptr, tperm, tstart, L, q, enc, loc, logtab, accum);
+    profile_mark(st, false);
+    const double pref = 1.0 / (4.0 * 3.14159265358979323846 * mu);
+    if (prec == VN_F32)
+        fmm_finish_targets<float2><<<gt, 256, 0, st>>>(accum, nt, pref, (float2 *)Ut);
+    else
+        fmm_finish_targets<double2><<<gt, 256, 0, st>>>(accum, nt, pref, (double2 *)Ut);
     count_launch(launches + 2);
     const cudaError_t e = cudaGetLastError();
     VN_CUDA(cudaFreeAsync(scr, st));

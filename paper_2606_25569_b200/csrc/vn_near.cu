@@ -318,6 +318,15 @@ struct SinkFixedF64 {
     }
 };
 
+struct SinkAccum {      // the fast multipole path: plain double accumulators in original point order, one writer per point
+    double2 *accum;
+    __device__ void operator()(int t, double x, double y) const
+    {
+        if (x == 0.0 && y == 0.0) return;
+        accum[t] = make_double2(accum[t].x + x, accum[t].y + y);
+    }
+};
+
 struct SinkFixedF32 {
     long long *acc;
     const unsigned *gmax_bits;
@@ -338,6 +347,21 @@ vn_status near_correction_f64(const void *X, const void *F, const void *W, int P
     near_correction<double, double2, SinkFixedF64><<<(P + 7) / 8, 256, 0, st>>>(
         (const double2 *)X, (const double2 *)F, (const double *)W, P, npts, (const long long *)near_ptr,
         (const int *)near_ves, SinkFixedF64{acc, gmax_bits, P});
+    count_launch(1);
+    return cudaGetLastError() == cudaSuccess ? VN_OK : VN_ERR_CUDA;
+}
+
+vn_status near_correction_accum(const void *X, const void *F, const void *W, int P, int npts, const int64_t *near_ptr,
+                                const int32_t *near_ves, double2 *accum, vn_precision prec, cudaStream_t st)
+{
+    if (prec == VN_F32)
+        near_correction<float, float2, SinkAccum><<<(P + 7) / 8, 256, 0, st>>>(
+            (const float2 *)X, (const float2 *)F, (const float *)W, P, npts, (const long long *)near_ptr,
+            (const int *)near_ves, SinkAccum{accum});
+    else
+        near_correction<double, double2, SinkAccum><<<(P + 7) / 8, 256, 0, st>>>(
+            (const double2 *)X, (const double2 *)F, (const double *)W, P, npts, (const long long *)near_ptr,
+            (const int *)near_ves, SinkAccum{accum});
     count_launch(1);
     return cudaGetLastError() == cudaSuccess ? VN_OK : VN_ERR_CUDA;
 }

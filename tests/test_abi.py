@@ -22,7 +22,7 @@ def test_library_exports_every_declared_symbol():
     names = _declared()
     assert {"vn_farfield", "vn_arclength_weights", "vn_farfield_host", "vn_status_string",
             "vn_version", "vn_launch_count", "vn_near_pairs", "vn_farfield_masked",
-            "vn_farfield_targets", "vn_elastic_force", "vn_redistribute_arclength", "vn_farfield_fmm"} <= set(names)
+            "vn_farfield_targets", "vn_elastic_force", "vn_redistribute_arclength", "vn_farfield_fmm", "vn_farfield_targets_fmm"} <= set(names)
     for n in names:
         assert hasattr(L, n), n
     assert vn.vn_version() >= 100
@@ -65,9 +65,11 @@ def test_argument_validation_needs_no_gpu():
     assert L.vn_redistribute_arclength(p, 2, 2, q, vn.VN_F64, None) == INV               # npts < 3
     assert L.vn_redistribute_arclength(p, 2, 513, q, vn.VN_F64, None) == INV             # npts > 512
     assert L.vn_redistribute_arclength(p, 2, 4, p, vn.VN_F64, None) == INV               # in place
-    assert L.vn_farfield_fmm(p, p, None, 2, 4, 1.0, 12, q, vn.VN_F64, None) == INV       # null W
-    assert L.vn_farfield_fmm(p, p, p, 2, 4, 1.0, 1, q, vn.VN_F64, None) == INV          # order < 2
-    assert L.vn_farfield_fmm(p, p, p, 2, 4, 1.0, 49, q, vn.VN_F64, None) == INV         # order > 48
-    assert L.vn_farfield_fmm(p, p, p, 2, 4, 1.0, 12, p, vn.VN_F64, None) == INV         # U aliases X
+    assert L.vn_farfield_fmm(p, p, None, 2, 4, 1.0, 12, None, None, q, vn.VN_F64, None) == INV       # null W
+    assert L.vn_farfield_fmm(p, p, p, 2, 4, 1.0, 1, None, None, q, vn.VN_F64, None) == INV          # order < 2
+    assert L.vn_farfield_fmm(p, p, p, 2, 4, 1.0, 49, None, None, q, vn.VN_F64, None) == INV         # order > 48
+    assert L.vn_farfield_fmm(p, p, p, 2, 4, 1.0, 12, None, None, p, vn.VN_F64, None) == INV         # U aliases X
+    assert L.vn_farfield_targets_fmm(q, 3, p, p, p, 2, 4, 1.0, 60, q, vn.VN_F64, None) == INV   # order > 48
+    assert L.vn_farfield_targets_fmm(None, 0, p, p, p, 2, 4, 1.0, 12, None, vn.VN_F64, None) == vn.VN_OK
     assert L.vn_farfield_host(p, None, None, 2, 4, 1.0, q, vn.VN_F64) == INV
     assert L.vn_farfield_host(p, p, None, 2, 4, -1.0, q, vn.VN_F64) == INV

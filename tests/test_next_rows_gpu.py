@@ -499,3 +499,37 @@ def test_fmm_single_vesicle_gives_zero():
     # everything the expansions add is taken out again by the own-vesicle correction: zero up to truncation
     scale = np.abs(oracle.farfield_targets(X, F, W, X[0, :1] + 50.0)).max()
     assert np.abs(got.cpu().numpy()).max() <= 1e-9 * max(scale, 1.0) * 700
+
+
+@pytest.mark.parametrize("dtype,order", [(np.float64, 38), (np.float32, 12)])
+def test_fmm_masked_parity(dtype, order):
+    """The paper's DirectSingleLayerIntegral in O(P): FMM + near-field mask against the masked oracle."""
+    X, F, W, mu = crowded(1, 0.94)
+    Xo, Fo, Wo = stored(X, dtype), stored(F, dtype), stored(W, dtype)
+    near = oracle.near_mask(Xo, Wo)
+    ref = oracle.farfield_masked(Xo, Fo, Wo, near, mu)
+    Xd, Fd, Wd = dev(X, dtype), dev(F, dtype), dev(W, dtype)
+    ptr, ves = vn.vn_near_pairs(Xd, Wd)
+    got = vn.vn_farfield_fmm(Xd, Fd, Wd, mu, order, near_ptr=ptr, near_ves=ves)
+    torch.cuda.synchronize()
+    rows = near.sum(1) > 0
+    err = rel_l2(got.cpu().numpy(), ref)
+    err_rows = rel_l2(got.cpu().numpy().reshape(-1, 2)[rows], ref.reshape(-1, 2)[rows])
+    print(f"fmm masked crowded1 {np.dtype(dtype).name} p={order}: rel-L2 {err:.3e} (corrected rows {err_rows:.3e})")
+    assert err <= TOL[dtype] and err_rows <= TOL[dtype]
+
+
+@pytest.mark.parametrize("dtype,order", [(np.float64, 38), (np.float32, 12)])
+@pytest.mark.parametrize("index,nt", [(0, 777), (1, 5000), (3, 100_000)])
+def test_fmm_targets_parity(index, nt, dtype, order):
+    s = inputs.config(index)
+    W = oracle.weights(s.X)
+    xt = grid_targets(s.X, nt, 900 + index)
+    rng = np.random.Generator(np.random.PCG64(905))
+    idx = np.arange(len(xt)) if len(xt) <= 5000 else np.unique(np.concatenate([[0, len(xt) - 1], rng.choice(len(xt), size=1500, replace=False)]))
+    ref = oracle.farfield_targets(stored(s.X, dtype), stored(s.F, dtype), stored(W, dtype), stored(xt, dtype)[idx], s.mu)
+    got = vn.vn_farfield_targets(dev(xt, dtype), dev(s.X, dtype), dev(s.F, dtype), dev(W, dtype), s.mu, fmm_order=order)
+    torch.cuda.synchronize()
+    err = rel_l2(got.cpu().numpy()[idx], ref)
+    print(f"fmm targets config{index} nt={len(xt)} {np.dtype(dtype).name} p={order}: rel-L2 {err:.3e}")
+    assert err <= TOL[dtype]
