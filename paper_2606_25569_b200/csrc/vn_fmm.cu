@@ -75,6 +75,28 @@ __global__ void fmm_init_bounds(unsigned long long *enc)
     enc[2] = enc[3] = 0ull;
 }
 
+// Depth of the tree, chosen ON THE DEVICE once the bounding box is known (no host synchronisation): leaves of
+// about kLeafTarget points, where the points are assumed to fill the bounding RECTANGLE evenly, i.e. a
+// fraction 1/aspect of the root square (a 4:1 channel leaves three quarters of the leaves empty).  The host
+// sizes scratch and grids for L_hi (two levels deeper than a full square needs); kernels of unused levels
+// and leaves return at once.  enc[4] holds the level.
+constexpr double kLeafTarget = 64.0;
+__global__ void fmm_choose_level(unsigned long long *enc, int P, int L_hi)
+{
+    const double ex = dec_f64(enc[2]) - dec_f64(enc[0]), ey = dec_f64(enc[3]) - dec_f64(enc[1]);
+    const double lo = fmin(ex, ey), hi = fmax(ex, ey);
+    double occ = (hi > 0.0 && lo > 0.0) ? lo / hi : 1.0;
+    occ = fmax(occ, 1.0 / 16.0);
+    int L = 2;
+    while (L < L_hi && (double)P / (occ * (double)(1ll << (2 * L))) > kLeafTarget) ++L;
+#ifdef VN_FMM_LEVEL_SHIFT                               // build-time experiment: coarser (-1) or finer (+1) tree
+    L += VN_FMM_LEVEL_SHIFT;
+    L = L < 2 ? 2 : (L > L_hi ? L_hi : L);
+#endif
+    enc[4] = (unsigned long long)L;
+}
+__device__ __forceinline__ int load_level(const unsigned long long *__restrict__ enc) { return (int)enc[4]; }
+
 // positions and densities g = F*W promoted to double (original order), and the bounding box
 template <typename real, typename real2>
 __global__ void __launch_bounds__(256)
@@ -109,13 +131,13 @@ fmm_load(const real2 *__restrict__ X, const real2 *__restrict__ F, const real *_
 
 // leaf box of every point and the population count of the leaves
 __global__ void __launch_bounds__(256)
-fmm_bin(const cplx *__restrict__ z, int P, int L, const unsigned long long *__restrict__ enc, int *__restrict__ cell,
+fmm_bin(const cplx *__restrict__ z, int P, const unsigned long long *__restrict__ enc, int *__restrict__ cell,
         int *__restrict__ cnt)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= P) return;
     const Geom gm = load_geom(enc);
-    const int n = 1 << L;
+    const int n = 1 << load_level(enc);
     const double inv = (double)n / gm.size;
     const int ix = min(max((int)((z[i].x - gm.x0) * inv), 0), n - 1);
     const int iy = min(max((int)((z[i].y - gm.y0) * inv), 0), n - 1);
@@ -235,9 +257,10 @@ __host__ __device__ inline long long level_offset(int l) { return ((1ll << (2 * 
 //   A1_k = sum g_x w^k,  A2_k = sum g_y w^k,  B_k = sum conj(zeta) g w^k.
 constexpr int kFmmMaxQ = 49;          // p <= 48
 __global__ void __launch_bounds__(128)
-fmm_p2m(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const long long *__restrict__ start, int L, int q,
-        const unsigned long long *__restrict__ enc, cplx *__restrict__ mult)
+fmm_p2m(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const long long *__restrict__ start, int q,
+        const unsigned long long *__restrict__ enc, cplx *__restrict__ mult, int *__restrict__ boxcnt)
 {
+    const int L = load_level(enc);
     __shared__ cplx acc[4][3 * kFmmMaxQ];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int n = 1 << L, ncell = n * n;
@@ -249,6 +272,7 @@ fmm_p2m(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const long lon
     for (int e = lane; e < 3 * q; e += 32) acc[warp][e] = make_double2(0.0, 0.0);
     __syncwarp();
     const long long a = start[c], b = start[c + 1];
+    if (lane == 0) boxcnt[level_offset(L) + c] = (int)(b - a);
     for (long long base = a; base < b; base += 32) {
         const long long idx = base + lane;
         cplx w = make_double2(0.0, 0.0), g = make_double2(0.0, 0.0), h = make_double2(0.0, 0.0);
@@ -280,8 +304,10 @@ fmm_p2m(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const long lon
 
 // M2M: parent moments from its four children, levels L-1 down to 2.  One thread per (parent box, k).
 __global__ void __launch_bounds__(128)
-fmm_m2m(int level, int q, const double *__restrict__ tab, cplx *__restrict__ mult, int *__restrict__ boxcnt)
+fmm_m2m(int level, int q, const double *__restrict__ tab, const unsigned long long *__restrict__ enc,
+        cplx *__restrict__ mult, int *__restrict__ boxcnt)
 {
+    if (level >= load_level(enc)) return;
     const FmmTables t = fmm_tables_at(const_cast<double *>(tab), q);
     const int n = 1 << level;
     const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -326,6 +352,7 @@ __global__ void __launch_bounds__(160)
 fmm_m2l(int level, int q, const double *__restrict__ tab, const unsigned long long *__restrict__ enc,
         const cplx *__restrict__ mult, const int *__restrict__ boxcnt, cplx *__restrict__ loc)
 {
+    if (level > load_level(enc)) return;
     extern __shared__ __align__(16) double sm[];
     double *Cb = sm;                                   // [q][q]
     cplx *hat = (cplx *)(sm + ((q * q + 1) & ~1));     // [2][3][q]: double-buffered, one barrier per source
@@ -405,8 +432,10 @@ fmm_m2l(int level, int q, const double *__restrict__ tab, const unsigned long lo
 
 // L2L: child local expansions inherit the parent's.  One thread per (child box, k); child level = `level`.
 __global__ void __launch_bounds__(128)
-fmm_l2l(int level, int q, const double *__restrict__ tab, cplx *__restrict__ loc)
+fmm_l2l(int level, int q, const double *__restrict__ tab, const unsigned long long *__restrict__ enc,
+        cplx *__restrict__ loc)
 {
+    if (level > load_level(enc)) return;
     const FmmTables t = fmm_tables_at(const_cast<double *>(tab), q);
     const int n = 1 << level;
     const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -445,7 +474,7 @@ constexpr int kP2PSplit = 4;
 __global__ void __launch_bounds__(kP2PThreads)
 fmm_l2p_p2p(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const int *__restrict__ vs,
             const long long *__restrict__ start, const cplx *__restrict__ tz, const int *__restrict__ tvs,
-            const int *__restrict__ tperm, const long long *__restrict__ tstart, int L, int q,
+            const int *__restrict__ tperm, const long long *__restrict__ tstart, int q,
             const unsigned long long *__restrict__ enc, const cplx *__restrict__ loc, const double *__restrict__ logtab,
             cplx *__restrict__ accum)
 {   // targets (tz, tvs, tperm, tstart) are the sorted sources themselves for vn_farfield_fmm, a separate sorted set
@@ -455,7 +484,9 @@ fmm_l2p_p2p(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const int 
     __shared__ double4 src[kP2PThreads];               // (zeta_x, zeta_y, g_x, g_y)
     __shared__ int sves[kP2PThreads];
     constexpr int kRound = kP2PThreads / kP2PSplit;
+    const int L = load_level(enc);
     const int n = 1 << L, c = blockIdx.x, ix = c / n, iy = c % n;
+    if (c >= n * n) return;
     const long long a = tstart[c], b = tstart[c + 1];
     if (a == b) return;
     const int tid = threadIdx.x, slot = tid / kP2PSplit, part = tid % kP2PSplit;
@@ -535,11 +566,13 @@ fmm_l2p_p2p(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const int 
 // contribution out again (direct, libm log), scale by 1/(4 pi mu) and store.  One thread per point.
 template <typename real2>
 __global__ void __launch_bounds__(128)
-fmm_finish(const cplx *__restrict__ z, const cplx *__restrict__ g, const int *__restrict__ cell, int P, int npts, int L,
-           const cplx *__restrict__ accum, double prefactor, real2 *__restrict__ U)
+fmm_finish(const cplx *__restrict__ z, const cplx *__restrict__ g, const int *__restrict__ cell, int P, int npts,
+           const unsigned long long *__restrict__ enc, const cplx *__restrict__ accum, double prefactor,
+           real2 *__restrict__ U)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= P) return;
+    const int L = load_level(enc);
     const int n = 1 << L;
     const int ci = cell[i], ix = ci >> L, iy = ci & (n - 1);
     const cplx zi = z[i];
@@ -564,14 +597,11 @@ fmm_finish(const cplx *__restrict__ z, const cplx *__restrict__ g, const int *__
 }
 
 // ------------------------------------------------------------------------------------------------
-static int fmm_levels(long long P, int order)
+static int fmm_levels_max(long long P)
 {
-    // leaves of about 1.5 (p+1) points balance the direct part (9 x leaf pairs per point) against M2L
-    // (27 x 3 (p+1)^2 per box); at least 2 levels (no interaction lists above), at most 10
-    double target = 1.5 * (order + 1);
-    target = target < 16 ? 16 : (target > 96 ? 96 : target);
+    // the deepest tree the device may choose: leaves of kLeafTarget points if only 1/16 of the root square is occupied
     int L = 2;
-    while (L < 10 && (double)P / (double)(1ll << (2 * L)) > target) ++L;
+    while (L < 10 && 16.0 * (double)P / (double)(1ll << (2 * L)) > kLeafTarget) ++L;
     return L;
 }
 
@@ -579,7 +609,7 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
                        const int64_t *near_ptr, const int32_t *near_ves, void *U, vn_precision prec, cudaStream_t st)
 {
     const int P = (int)(nves * npts), q = order + 1;
-    const int L = fmm_levels(P, order);
+    const int L = fmm_levels_max(P);                  // upper bound: the device picks the level (fmm_choose_level)
     const int n = 1 << L, ncell = n * n;
     const long long nbox = level_offset(L + 1);
     const int nb_scan = (ncell + kScanBlock - 1) / kScanBlock;
@@ -588,7 +618,8 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
     const size_t b_exp = up(sizeof(cplx) * (size_t)nbox * 3 * q), b_cnt = up(sizeof(int) * (size_t)nbox);
     const size_t b_start = up(sizeof(long long) * ((size_t)ncell + 1)), b_bs = up(sizeof(long long) * (size_t)nb_scan);
     const size_t b_tab = up(sizeof(double) * fmm_tables_doubles(q)), b_log = up(sizeof(double) * (kLogTab + kExpTab));
-    const size_t total = 5 * b_pt + 3 * b_int + 2 * b_exp + b_cnt + 2 * b_start + b_bs + b_tab + b_log + 256;
+    const size_t b_leaf = up(sizeof(int) * (size_t)ncell);
+    const size_t total = 5 * b_pt + 3 * b_int + 2 * b_exp + b_cnt + b_leaf + 2 * b_start + b_bs + b_tab + b_log + 256;
     char *scr = nullptr;
     VN_CUDA(cudaMallocAsync((void **)&scr, total, st));
     char *ptr = scr;
@@ -597,20 +628,20 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
     cplx *accum = (cplx *)take(b_pt);
     int *cell = (int *)take(b_int), *perm = (int *)take(b_int), *vs = (int *)take(b_int);
     cplx *mult = (cplx *)take(b_exp), *loc = (cplx *)take(b_exp);
-    int *boxcnt = (int *)take(b_cnt);
+    int *boxcnt = (int *)take(b_cnt), *cnt = (int *)take(b_leaf);
     long long *start = (long long *)take(b_start), *cursor = (long long *)take(b_start), *bsum = (long long *)take(b_bs);
     double *tab = (double *)take(b_tab), *logtab = (double *)take(b_log);
     unsigned long long *enc = (unsigned long long *)take(256);
-    int *cnt = boxcnt + level_offset(L);
 
-    VN_CUDA(cudaMemsetAsync(boxcnt, 0, b_cnt, st));
+    VN_CUDA(cudaMemsetAsync(boxcnt, 0, b_cnt + b_leaf, st));      // boxcnt and the leaf counts are adjacent
     fmm_init_bounds<<<1, 1, 0, st>>>(enc);
     const int gp = (P + 255) / 256;
     if (prec == VN_F32)
         fmm_load<float, float2><<<gp, 256, 0, st>>>((const float2 *)X, (const float2 *)F, (const float *)W, P, z, g, enc);
     else
         fmm_load<double, double2><<<gp, 256, 0, st>>>((const double2 *)X, (const double2 *)F, (const double *)W, P, z, g, enc);
-    fmm_bin<<<gp, 256, 0, st>>>(z, P, L, enc, cell, cnt);
+    fmm_choose_level<<<1, 1, 0, st>>>(enc, P, L);
+    fmm_bin<<<gp, 256, 0, st>>>(z, P, enc, cell, cnt);
     scan_block_sums<<<nb_scan, kScanThreads, 0, st>>>(cnt, ncell, bsum);
     scan_of_sums<<<1, kScanThreads, 0, st>>>(bsum, nb_scan);
     scan_apply<<<nb_scan, kScanThreads, 0, st>>>(cnt, ncell, bsum, start, cursor);
@@ -619,14 +650,14 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
     fmm_gather<<<gp, 256, 0, st>>>(perm, P, (int)npts, z, g, zs, gs, vs);
     fmm_build_tables<<<64, 128, 0, st>>>(q, tab);
     fmm_build_logtab<<<8, 128, 0, st>>>(logtab);
-    int launches = 12;
+    int launches = 13;
 
     profile_mark(st, true);
-    fmm_p2m<<<(ncell + 3) / 4, 128, 0, st>>>(zs, gs, start, L, q, enc, mult);
+    fmm_p2m<<<(ncell + 3) / 4, 128, 0, st>>>(zs, gs, start, q, enc, mult, boxcnt);
     ++launches;
     for (int l = L - 1; l >= 2; --l) {
         const long long work = (1ll << (2 * l)) * q;
-        fmm_m2m<<<(unsigned)((work + 127) / 128), 128, 0, st>>>(l, q, tab, mult, boxcnt);
+        fmm_m2m<<<(unsigned)((work + 127) / 128), 128, 0, st>>>(l, q, tab, enc, mult, boxcnt);
         ++launches;
     }
     const size_t smem_m2l = sizeof(double) * (size_t)(((q * q + 1) & ~1) + 12 * q);
@@ -637,10 +668,10 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
     }
     for (int l = 3; l <= L; ++l) {
         const long long work = (1ll << (2 * l)) * q;
-        fmm_l2l<<<(unsigned)((work + 127) / 128), 128, 0, st>>>(l, q, tab, loc);
+        fmm_l2l<<<(unsigned)((work + 127) / 128), 128, 0, st>>>(l, q, tab, enc, loc);
         ++launches;
     }
-    fmm_l2p_p2p<<<ncell, kP2PThreads, 0, st>>>(zs, gs, vs, start, zs, vs, perm, start, L, q, enc, loc, logtab, accum);
+    fmm_l2p_p2p<<<ncell, kP2PThreads, 0, st>>>(zs, gs, vs, start, zs, vs, perm, start, q, enc, loc, logtab, accum);
     profile_mark(st, false);
     if (near_ptr) {   // row f-1 on top: take the near vesicles' contributions out (they are all in the direct part)
         const vn_status rc = near_correction_accum(X, F, W, P, (int)npts, near_ptr, near_ves, accum, prec, st);
@@ -648,9 +679,9 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
     }
     const double pref = 1.0 / (4.0 * 3.14159265358979323846 * mu);
     if (prec == VN_F32)
-        fmm_finish<float2><<<(P + 127) / 128, 128, 0, st>>>(z, g, cell, P, (int)npts, L, accum, pref, (float2 *)U);
+        fmm_finish<float2><<<(P + 127) / 128, 128, 0, st>>>(z, g, cell, P, (int)npts, enc, accum, pref, (float2 *)U);
     else
-        fmm_finish<double2><<<(P + 127) / 128, 128, 0, st>>>(z, g, cell, P, (int)npts, L, accum, pref, (double2 *)U);
+        fmm_finish<double2><<<(P + 127) / 128, 128, 0, st>>>(z, g, cell, P, (int)npts, enc, accum, pref, (double2 *)U);
     count_launch(launches + 2);
     const cudaError_t e = cudaGetLastError();
     VN_CUDA(cudaFreeAsync(scr, st));
@@ -711,7 +742,7 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
                                int64_t npts, double mu, int order, void *Ut, vn_precision prec, cudaStream_t st)
 {
     const int P = (int)(nves * npts), nt = (int)nt64, q = order + 1;
-    const int L = fmm_levels(P > nt ? P : nt, order);
+    const int L = fmm_levels_max(P > nt ? P : nt);    // upper bound: the device picks the level
     const int n = 1 << L, ncell = n * n;
     const long long nbox = level_offset(L + 1);
     const int nb_scan = (ncell + kScanBlock - 1) / kScanBlock;
@@ -722,7 +753,7 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
     const size_t b_ccnt = up(sizeof(int) * (size_t)ncell);
     const size_t b_start = up(sizeof(long long) * ((size_t)ncell + 1)), b_bs = up(sizeof(long long) * (size_t)nb_scan);
     const size_t b_tab = up(sizeof(double) * fmm_tables_doubles(q)), b_log = up(sizeof(double) * (kLogTab + kExpTab));
-    const size_t total = 4 * b_pt + 3 * b_int + 3 * b_tpt + 2 * b_tint + 2 * b_exp + b_cnt + b_ccnt + 4 * b_start +
+    const size_t total = 4 * b_pt + 3 * b_int + 3 * b_tpt + 2 * b_tint + 2 * b_exp + b_cnt + 2 * b_ccnt + 4 * b_start +
                          b_bs + b_tab + b_log + 256;
     char *scr = nullptr;
     VN_CUDA(cudaMallocAsync((void **)&scr, total, st));
@@ -733,14 +764,13 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
     cplx *zt = (cplx *)take(b_tpt), *zts = (cplx *)take(b_tpt), *accum = (cplx *)take(b_tpt);
     int *tcell = (int *)take(b_tint), *tperm = (int *)take(b_tint);
     cplx *mult = (cplx *)take(b_exp), *loc = (cplx *)take(b_exp);
-    int *boxcnt = (int *)take(b_cnt), *tcnt = (int *)take(b_ccnt);
+    int *boxcnt = (int *)take(b_cnt), *cnt = (int *)take(b_ccnt), *tcnt = (int *)take(b_ccnt);
     long long *start = (long long *)take(b_start), *cursor = (long long *)take(b_start);
     long long *tstart = (long long *)take(b_start), *tcursor = (long long *)take(b_start), *bsum = (long long *)take(b_bs);
     double *tab = (double *)take(b_tab), *logtab = (double *)take(b_log);
     unsigned long long *enc = (unsigned long long *)take(256);
-    int *cnt = boxcnt + level_offset(L);
 
-    VN_CUDA(cudaMemsetAsync(boxcnt, 0, b_cnt + b_ccnt, st));       // boxcnt and tcnt are adjacent
+    VN_CUDA(cudaMemsetAsync(boxcnt, 0, b_cnt + 2 * b_ccnt, st));   // boxcnt, cnt and tcnt are adjacent
     fmm_init_bounds<<<1, 1, 0, st>>>(enc);
     const int gp = (P + 255) / 256, gt = (nt + 255) / 256;
     if (prec == VN_F32) {
@@ -750,8 +780,9 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
         fmm_load<double, double2><<<gp, 256, 0, st>>>((const double2 *)X, (const double2 *)F, (const double *)W, P, z, g, enc);
         fmm_load_targets<double2><<<gt, 256, 0, st>>>((const double2 *)Xt, nt, zt, enc);
     }
+    fmm_choose_level<<<1, 1, 0, st>>>(enc, P > nt ? P : nt, L);
     // sources into leaves
-    fmm_bin<<<gp, 256, 0, st>>>(z, P, L, enc, cell, cnt);
+    fmm_bin<<<gp, 256, 0, st>>>(z, P, enc, cell, cnt);
     scan_block_sums<<<nb_scan, kScanThreads, 0, st>>>(cnt, ncell, bsum);
     scan_of_sums<<<1, kScanThreads, 0, st>>>(bsum, nb_scan);
     scan_apply<<<nb_scan, kScanThreads, 0, st>>>(cnt, ncell, bsum, start, cursor);
@@ -759,7 +790,7 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
     fmm_sort_cells<<<(ncell + 127) / 128, 128, 0, st>>>(start, ncell, perm);
     fmm_gather<<<gp, 256, 0, st>>>(perm, P, (int)npts, z, g, zs, gs, vs);
     // targets into the same leaves
-    fmm_bin<<<gt, 256, 0, st>>>(zt, nt, L, enc, tcell, tcnt);
+    fmm_bin<<<gt, 256, 0, st>>>(zt, nt, enc, tcell, tcnt);
     scan_block_sums<<<nb_scan, kScanThreads, 0, st>>>(tcnt, ncell, bsum);
     scan_of_sums<<<1, kScanThreads, 0, st>>>(bsum, nb_scan);
     scan_apply<<<nb_scan, kScanThreads, 0, st>>>(tcnt, ncell, bsum, tstart, tcursor);
@@ -768,14 +799,14 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
     fmm_gather_targets<<<gt, 256, 0, st>>>(tperm, nt, zt, zts);
     fmm_build_tables<<<64, 128, 0, st>>>(q, tab);
     fmm_build_logtab<<<8, 128, 0, st>>>(logtab);
-    int launches = 20;
+    int launches = 21;
 
     profile_mark(st, true);
-    fmm_p2m<<<(ncell + 3) / 4, 128, 0, st>>>(zs, gs, start, L, q, enc, mult);
+    fmm_p2m<<<(ncell + 3) / 4, 128, 0, st>>>(zs, gs, start, q, enc, mult, boxcnt);
     ++launches;
     for (int l = L - 1; l >= 2; --l) {
         const long long work = (1ll << (2 * l)) * q;
-        fmm_m2m<<<(unsigned)((work + 127) / 128), 128, 0, st>>>(l, q, tab, mult, boxcnt);
+        fmm_m2m<<<(unsigned)((work + 127) / 128), 128, 0, st>>>(l, q, tab, enc, mult, boxcnt);
         ++launches;
     }
     const size_t smem_m2l = sizeof(double) * (size_t)(((q * q + 1) & ~1) + 12 * q);
@@ -786,10 +817,10 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
     }
     for (int l = 3; l <= L; ++l) {
         const long long work = (1ll << (2 * l)) * q;
-        fmm_l2l<<<(unsigned)((work + 127) / 128), 128, 0, st>>>(l, q, tab, loc);
+        fmm_l2l<<<(unsigned)((work + 127) / 128), 128, 0, st>>>(l, q, tab, enc, loc);
         ++launches;
     }
-    fmm_l2p_p2p<<<ncell, kP2PThreads, 0, st>>>(zs, gs, vs, start, zts, nullptr, tperm, tstart, L, q, enc, loc, logtab, accum);
+    fmm_l2p_p2p<<<ncell, kP2PThreads, 0, st>>>(zs, gs, vs, start, zts, nullptr, tperm, tstart, q, enc, loc, logtab, accum);
     profile_mark(st, false);
     const double pref = 1.0 / (4.0 * 3.14159265358979323846 * mu);
     if (prec == VN_F32)
