@@ -152,22 +152,23 @@ fmm_scatter(const int *__restrict__ cell, int P, long long *__restrict__ cursor,
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= P) return;
     const long long pos = (long long)atomicAdd((unsigned long long *)(cursor + cell[i]), 1ull);
-    perm[pos] = i;
+    perm[pos] = i;                                     // arbitrary order inside a leaf; fmm_sort_cells fixes it
 }
 
-// the atomic scatter leaves every leaf's points in arbitrary order: sort each segment by point index so that
-// every later sum runs in a fixed order (bitwise reproducible results); then gather the sorted copies
+// the atomic scatter leaves every leaf's points in arbitrary order: order each segment by point index so that
+// every later sum runs in a fixed order (bitwise reproducible results).  One warp per leaf, rank sort: the
+// indices of a segment are distinct, so the rank of an entry is the number of smaller ones.
 __global__ void __launch_bounds__(128)
-fmm_sort_cells(const long long *__restrict__ start, int ncell, int *__restrict__ perm)
+fmm_sort_cells(const long long *__restrict__ start, int ncell, const int *__restrict__ unsorted, int *__restrict__ perm)
 {
-    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    const int c = blockIdx.x * 4 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
     if (c >= ncell) return;
     const long long a = start[c], b = start[c + 1];
-    for (long long i = a + 1; i < b; ++i) {            // insertion sort: segments are a few dozen entries
-        const int v = perm[i];
-        long long j = i - 1;
-        while (j >= a && perm[j] > v) { perm[j + 1] = perm[j]; --j; }
-        perm[j + 1] = v;
+    for (long long i = a + lane; i < b; i += 32) {
+        const int v = unsorted[i];
+        int rank = 0;
+        for (long long j = a; j < b; ++j) rank += unsorted[j] < v;
+        perm[a + rank] = v;
     }
 }
 
@@ -471,6 +472,7 @@ __global__ void fmm_build_logtab(double *tab)
 // The sum goes to accum[original point index] (still without the 1/(4 pi mu)).
 constexpr int kP2PThreads = 64;
 constexpr int kP2PSplit = 4;
+constexpr int kP2PTargets = 4;
 __global__ void __launch_bounds__(kP2PThreads)
 fmm_l2p_p2p(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const int *__restrict__ vs,
             const long long *__restrict__ start, const cplx *__restrict__ tz, const int *__restrict__ tvs,
@@ -497,33 +499,42 @@ fmm_l2p_p2p(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const int 
     const cplx ctr = box_centre(gm, L, ix, iy);
     __syncthreads();
 
-    for (long long t0 = a; t0 < b; t0 += kRound) {
-        const long long ti = t0 + slot;
-        const bool live = ti < b;
-        cplx z = make_double2(0.0, 0.0);
-        int myves = -1;
-        double ux = 0.0, uy = 0.0;
-        if (live) {
-            z = tz[ti];
-            myves = tvs ? tvs[ti] : -1;
-        }
-        if (live && part == 0) {
-            // far field: Horner for value and derivative of the three local expansions
-            const cplx t = make_double2((z.x - ctr.x) * inv_s, (z.y - ctr.y) * inv_s);
-            cplx p1 = lc[q - 1], p2 = lc[2 * q - 1], p3 = lc[3 * q - 1];
-            cplx d1 = make_double2(0.0, 0.0), d2 = d1;
-            for (int l = q - 2; l >= 0; --l) {
-                d1 = cfma(d1, t, p1);
-                d2 = cfma(d2, t, p2);
-                p1 = cfma(p1, t, lc[l]);
-                p2 = cfma(p2, t, lc[q + l]);
-                p3 = cfma(p3, t, lc[2 * q + l]);
+    // a thread owns up to kP2PTargets targets (slot, slot + kRound, ...) and every kP2PSplit-th source of a staged
+    // chunk: the source record is read once for kP2PTargets pairs, which are independent chains
+    for (long long t0 = a; t0 < b; t0 += kRound * kP2PTargets) {
+        cplx z[kP2PTargets];
+        int myves[kP2PTargets];
+        double ux[kP2PTargets], uy[kP2PTargets];
+        bool live[kP2PTargets];
+#pragma unroll
+        for (int r = 0; r < kP2PTargets; ++r) {
+            const long long ti = t0 + slot + r * kRound;
+            live[r] = ti < b;
+            z[r] = make_double2(0.0, 0.0);
+            myves[r] = -2;
+            ux[r] = uy[r] = 0.0;
+            if (live[r]) {
+                z[r] = tz[ti];
+                myves[r] = tvs ? tvs[ti] : -1;
             }
-            // phi = (Phi1' + i Phi2') = (d1 + i d2)/s ;  z conj(phi)
-            const cplx phi = make_double2((d1.x - d2.y) * inv_s, (d1.y + d2.x) * inv_s);
-            const cplx zc = cmul(z, make_double2(phi.x, -phi.y));
-            ux = -p1.x + 0.5 * zc.x - 0.5 * p3.x;
-            uy = -p2.x + 0.5 * zc.y + 0.5 * p3.y;
+            if (live[r] && part == 0) {
+                // far field: Horner for value and derivative of the three local expansions
+                const cplx t = make_double2((z[r].x - ctr.x) * inv_s, (z[r].y - ctr.y) * inv_s);
+                cplx p1 = lc[q - 1], p2 = lc[2 * q - 1], p3 = lc[3 * q - 1];
+                cplx d1 = make_double2(0.0, 0.0), d2 = d1;
+                for (int l = q - 2; l >= 0; --l) {
+                    d1 = cfma(d1, t, p1);
+                    d2 = cfma(d2, t, p2);
+                    p1 = cfma(p1, t, lc[l]);
+                    p2 = cfma(p2, t, lc[q + l]);
+                    p3 = cfma(p3, t, lc[2 * q + l]);
+                }
+                // phi = (Phi1' + i Phi2') = (d1 + i d2)/s ;  z conj(phi)
+                const cplx phi = make_double2((d1.x - d2.y) * inv_s, (d1.y + d2.x) * inv_s);
+                const cplx zc = cmul(z[r], make_double2(phi.x, -phi.y));
+                ux[r] = -p1.x + 0.5 * zc.x - 0.5 * p3.x;
+                uy[r] = -p2.x + 0.5 * zc.y + 0.5 * p3.y;
+            }
         }
         // near field
         for (int bx = max(ix - 1, 0); bx <= min(ix + 1, n - 1); ++bx)
@@ -538,26 +549,32 @@ fmm_l2p_p2p(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const int 
                     }
                     __syncthreads();
                     const int cnt = (int)min((long long)kP2PThreads, sb - s0);
-                    if (live)
-                        for (int j = part; j < cnt; j += kP2PSplit) {
-                            if (sves[j] == myves) continue;
-                            const double4 sj = src[j];
-                            const double rx = z.x - sj.x, ry = z.y - sj.y;
+                    for (int j = part; j < cnt; j += kP2PSplit) {
+                        const double4 sj = src[j];
+                        const int sv = sves[j];
+#pragma unroll
+                        for (int r = 0; r < kP2PTargets; ++r) {
+                            if (sv == myves[r] || !live[r]) continue;
+                            const double rx = z[r].x - sj.x, ry = z[r].y - sj.y;
                             const double r2 = fma(rx, rx, ry * ry);
                             double ml, inv;
                             log_rcp_f64(r2, tab, ml, inv);
                             const double qd = fma(rx, sj.z, ry * sj.w) * inv;
-                            ux = fma(ml, sj.z, fma(qd, rx, ux));
-                            uy = fma(ml, sj.w, fma(qd, ry, uy));
+                            ux[r] = fma(ml, sj.z, fma(qd, rx, ux[r]));
+                            uy[r] = fma(ml, sj.w, fma(qd, ry, uy[r]));
                         }
+                    }
                 }
             }
 #pragma unroll
-        for (int m = 1; m < kP2PSplit; m <<= 1) {
-            ux += __shfl_xor_sync(0xffffffffu, ux, m);
-            uy += __shfl_xor_sync(0xffffffffu, uy, m);
+        for (int r = 0; r < kP2PTargets; ++r) {
+#pragma unroll
+            for (int m = 1; m < kP2PSplit; m <<= 1) {
+                ux[r] += __shfl_xor_sync(0xffffffffu, ux[r], m);
+                uy[r] += __shfl_xor_sync(0xffffffffu, uy[r], m);
+            }
+            if (live[r] && part == 0) accum[tperm[t0 + slot + r * kRound]] = make_double2(ux[r], uy[r]);
         }
-        if (live && part == 0) accum[tperm[ti]] = make_double2(ux, uy);
         __syncthreads();
     }
 }
@@ -645,8 +662,8 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
     scan_block_sums<<<nb_scan, kScanThreads, 0, st>>>(cnt, ncell, bsum);
     scan_of_sums<<<1, kScanThreads, 0, st>>>(bsum, nb_scan);
     scan_apply<<<nb_scan, kScanThreads, 0, st>>>(cnt, ncell, bsum, start, cursor);
-    fmm_scatter<<<gp, 256, 0, st>>>(cell, P, cursor, perm);
-    fmm_sort_cells<<<(ncell + 127) / 128, 128, 0, st>>>(start, ncell, perm);
+    fmm_scatter<<<gp, 256, 0, st>>>(cell, P, cursor, vs);                  // vs doubles as the unsorted buffer
+    fmm_sort_cells<<<(ncell + 3) / 4, 128, 0, st>>>(start, ncell, vs, perm);
     fmm_gather<<<gp, 256, 0, st>>>(perm, P, (int)npts, z, g, zs, gs, vs);
     fmm_build_tables<<<64, 128, 0, st>>>(q, tab);
     fmm_build_logtab<<<8, 128, 0, st>>>(logtab);
@@ -786,16 +803,16 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
     scan_block_sums<<<nb_scan, kScanThreads, 0, st>>>(cnt, ncell, bsum);
     scan_of_sums<<<1, kScanThreads, 0, st>>>(bsum, nb_scan);
     scan_apply<<<nb_scan, kScanThreads, 0, st>>>(cnt, ncell, bsum, start, cursor);
-    fmm_scatter<<<gp, 256, 0, st>>>(cell, P, cursor, perm);
-    fmm_sort_cells<<<(ncell + 127) / 128, 128, 0, st>>>(start, ncell, perm);
+    fmm_scatter<<<gp, 256, 0, st>>>(cell, P, cursor, vs);                  // vs doubles as the unsorted buffer
+    fmm_sort_cells<<<(ncell + 3) / 4, 128, 0, st>>>(start, ncell, vs, perm);
     fmm_gather<<<gp, 256, 0, st>>>(perm, P, (int)npts, z, g, zs, gs, vs);
     // targets into the same leaves
     fmm_bin<<<gt, 256, 0, st>>>(zt, nt, enc, tcell, tcnt);
     scan_block_sums<<<nb_scan, kScanThreads, 0, st>>>(tcnt, ncell, bsum);
     scan_of_sums<<<1, kScanThreads, 0, st>>>(bsum, nb_scan);
     scan_apply<<<nb_scan, kScanThreads, 0, st>>>(tcnt, ncell, bsum, tstart, tcursor);
-    fmm_scatter<<<gt, 256, 0, st>>>(tcell, nt, tcursor, tperm);
-    fmm_sort_cells<<<(ncell + 127) / 128, 128, 0, st>>>(tstart, ncell, tperm);
+    fmm_scatter<<<gt, 256, 0, st>>>(tcell, nt, tcursor, (int *)accum);     // accum doubles as the unsorted buffer
+    fmm_sort_cells<<<(ncell + 3) / 4, 128, 0, st>>>(tstart, ncell, (const int *)accum, tperm);
     fmm_gather_targets<<<gt, 256, 0, st>>>(tperm, nt, zt, zts);
     fmm_build_tables<<<64, 128, 0, st>>>(q, tab);
     fmm_build_logtab<<<8, 128, 0, st>>>(logtab);
