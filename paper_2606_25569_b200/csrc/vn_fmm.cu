@@ -339,96 +339,106 @@ fmm_m2m(int level, int q, const double *__restrict__ tab, const unsigned long lo
 }
 
 // ------------------------------------------------------------------------------------------------
-// M2L: one block per target box of `level`; thread (a, l) = (tid / q, tid % q) owns coefficient l of local
-// expansion a (0, 1: the logarithmic potentials Phi1, Phi2; 2: the Cauchy sum psi).  For every box of the
-// interaction list (children of the parent's neighbours that are not neighbours of the target; offset
-// tau = target - source in box units, rho = 1/tau):
-//   Ahat_k = A_k rho^k / k (k >= 1, log type)      Bhat_k = B_k rho^k (k >= 0)              (staged in shared memory)
+// M2L: one WARP per target box of `level` (four boxes per block), no block barrier inside the loop.  Lane `ln` owns
+// the coefficients l = ln and ln + 32 of all three local expansions (0, 1: the logarithmic potentials Phi1, Phi2;
+// 2: the Cauchy sum psi).  For every box of the interaction list (children of the parent's neighbours that are
+// not neighbours of the target; offset tau = target - source in box units, rho = 1/tau):
+//   Ahat_k = A_k rho^k / k (k >= 1, log type)      Bhat_k = B_k rho^k (k >= 0)        (staged in the warp's shared memory)
 //   b_l += (-1)^(l+1) rho^l ( A_0 / l + sum_{k>=1} C(k+l-1, l) Ahat_k )          l >= 1
 //   b_0 += A_0 (log s - log rho) - sum_{k>=1} Ahat_k
 //   d_l += (-1)^l rho^(l+1) / s * sum_{k>=0} C(k+l, l) Bhat_k ;   d_0 -= conj(A1_0 + i A2_0)   (the g/2 of each source)
-// so the inner loop is a REAL binomial matrix (shared memory, same for every offset and level) times a complex
-// vector: 2 DFMA per entry.
-__global__ void __launch_bounds__(160)
+// so the inner loop is a REAL binomial matrix (shared memory, same for every offset and level) times complex
+// vectors: one matrix entry serves all three expansions (6 DFMA per 8-byte load + 3 broadcasts).
+constexpr int kM2LWarps = 4;
+__global__ void __launch_bounds__(32 * kM2LWarps)
 fmm_m2l(int level, int q, const double *__restrict__ tab, const unsigned long long *__restrict__ enc,
         const cplx *__restrict__ mult, const int *__restrict__ boxcnt, cplx *__restrict__ loc)
 {
     if (level > load_level(enc)) return;
     extern __shared__ __align__(16) double sm[];
-    double *Cb = sm;                                   // [q][q]
-    cplx *hat = (cplx *)(sm + ((q * q + 1) & ~1));     // [2][3][q]: double-buffered, one barrier per source
-    __shared__ cplx A0[2][2];
-    __shared__ int list_src[27], list_off[27], list_n;
+    double *Cb = sm;                                                  // [q][q]
+    const int warp = threadIdx.x >> 5, ln = threadIdx.x & 31;
+    cplx *hat = (cplx *)(sm + ((q * q + 1) & ~1)) + warp * 3 * (q + 1);   // [3][q+1] per warp; hat[a][q] = 0 pads the shifted read
     const FmmTables t = fmm_tables_at(const_cast<double *>(tab), q);
-    const int n = 1 << level;
-    const int box = blockIdx.x, ix = box / n, iy = box % n;
-    const int a = threadIdx.x / q, l = threadIdx.x - a * q;       // blockDim.x = 3 q rounded up to a warp
-    const bool active = a < 3;
     for (int e = threadIdx.x; e < q * q; e += blockDim.x) Cb[e] = t.Cb[e];
-    if (threadIdx.x == 0) {                            // interaction list: non-empty boxes, fixed order
-        const int px = ix >> 1, py = iy >> 1;
-        int cnt = 0;
-        for (int sx = max(0, 2 * (px - 1)); sx < min(n, 2 * (px + 1) + 2); ++sx)
-            for (int sy = max(0, 2 * (py - 1)); sy < min(n, 2 * (py + 1) + 2); ++sy) {
-                if (abs(sx - ix) <= 1 && abs(sy - iy) <= 1) continue;
-                if (boxcnt[level_offset(level) + (long long)sx * n + sy] == 0) continue;
-                list_src[cnt] = sx * n + sy;
-                list_off[cnt] = (ix - sx + 3) * 7 + (iy - sy + 3);
-                ++cnt;
-            }
-        list_n = cnt;
-    }
+    __syncthreads();
+    const int n = 1 << level;
+    const int box = blockIdx.x * kM2LWarps + warp;
+    if (box >= n * n) return;
+    const int ix = box / n, iy = box % n;
     const Geom gm = load_geom(enc);
     const double s = gm.size / (double)n, log_s = log(s);
-    cplx acc = make_double2(0.0, 0.0);
-    const double sgn = (l & 1) ? -1.0 : 1.0;           // (-1)^l
-    __syncthreads();
-    const int ns = list_n;
+    const int l0 = ln, l1 = ln + 32;
+    const bool v0 = l0 < q, v1 = l1 < q;
+    cplx acc[3][2];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) acc[a][0] = acc[a][1] = make_double2(0.0, 0.0);
     const cplx *Mlev = mult + level_offset(level) * (long long)(3 * q);
-    cplx nextA = make_double2(0.0, 0.0);
-    if (active && ns > 0) nextA = Mlev[(long long)list_src[0] * (3 * q) + a * q + l];
-    for (int it = 0; it < ns; ++it) {
-        const int o = list_off[it];
-        const cplx *rho = t.rho + (size_t)o * (q + 1);
-        cplx *hb = hat + (it & 1) * 3 * q;
-        if (active) {
-            cplx v = cmul(nextA, rho[l]);
-            if (a < 2 && l >= 1) v = cscale(v, 1.0 / (double)l);
-            hb[a * q + l] = v;
-            if (a < 2 && l == 0) A0[it & 1][a] = nextA;
-            if (it + 1 < ns) nextA = Mlev[(long long)list_src[it + 1] * (3 * q) + a * q + l];   // prefetch
-        }
-        __syncthreads();
-        if (active) {
-            cplx S = make_double2(0.0, 0.0);
-            const cplx *h = hb + a * q;
-            const cplx a0 = A0[it & 1][a < 2 ? a : 0], a1 = A0[it & 1][1];
-            if (a < 2) {
-                for (int k = 1; k < q; ++k) {
-                    const double c = Cb[(k - 1) * q + l];
-                    S.x = fma(c, h[k].x, S.x);
-                    S.y = fma(c, h[k].y, S.y);
+    const int px = ix >> 1, py = iy >> 1;
+    for (int sx = max(0, 2 * (px - 1)); sx < min(n, 2 * (px + 1) + 2); ++sx)
+        for (int sy = max(0, 2 * (py - 1)); sy < min(n, 2 * (py + 1) + 2); ++sy) {
+            if (abs(sx - ix) <= 1 && abs(sy - iy) <= 1) continue;
+            const long long src = (long long)sx * n + sy;
+            if (boxcnt[level_offset(level) + src] == 0) continue;
+            const int o = (ix - sx + 3) * 7 + (iy - sy + 3);
+            const cplx *rho = t.rho + (size_t)o * (q + 1);
+            const cplx *A = Mlev + src * (3 * q);
+            __syncwarp();                                             // the previous source's hat is consumed
+            for (int k = ln; k <= q; k += 32) {
+                cplx h0 = make_double2(0.0, 0.0), h1 = h0, h2 = h0;
+                if (k < q) {
+                    const cplx r = rho[k];
+                    h0 = cmul(A[k], r);
+                    h1 = cmul(A[q + k], r);
+                    h2 = cmul(A[2 * q + k], r);
+                    if (k >= 1) { const double ik = 1.0 / (double)k; h0 = cscale(h0, ik); h1 = cscale(h1, ik); }
                 }
+                hat[k] = h0;
+                hat[(q + 1) + k] = h1;
+                hat[2 * (q + 1) + k] = h2;
+            }
+            __syncwarp();
+            const cplx A10 = A[0], A20 = A[q];                       // raw zeroth moments (real charges: imaginary part 0)
+            cplx S[3][2];
+#pragma unroll
+            for (int a = 0; a < 3; ++a) S[a][0] = S[a][1] = make_double2(0.0, 0.0);
+            const cplx *h0p = hat + 1, *h1p = hat + (q + 1) + 1, *h2p = hat + 2 * (q + 1);   // log arrays read k + 1
+            for (int k = 0; k < q; ++k) {
+                const double c0 = v0 ? Cb[k * q + l0] : 0.0, c1 = v1 ? Cb[k * q + l1] : 0.0;
+                const cplx e0 = h0p[k], e1 = h1p[k], e2 = h2p[k];     // Ahat1_{k+1}, Ahat2_{k+1}, Bhat_k
+                S[0][0].x = fma(c0, e0.x, S[0][0].x); S[0][0].y = fma(c0, e0.y, S[0][0].y);
+                S[1][0].x = fma(c0, e1.x, S[1][0].x); S[1][0].y = fma(c0, e1.y, S[1][0].y);
+                S[2][0].x = fma(c0, e2.x, S[2][0].x); S[2][0].y = fma(c0, e2.y, S[2][0].y);
+                S[0][1].x = fma(c1, e0.x, S[0][1].x); S[0][1].y = fma(c1, e0.y, S[0][1].y);
+                S[1][1].x = fma(c1, e1.x, S[1][1].x); S[1][1].y = fma(c1, e1.y, S[1][1].y);
+                S[2][1].x = fma(c1, e2.x, S[2][1].x); S[2][1].y = fma(c1, e2.y, S[2][1].y);
+            }
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                const int l = j ? l1 : l0;
+                if (!(j ? v1 : v0)) continue;
+                const double sgn = (l & 1) ? -1.0 : 1.0;              // (-1)^l
                 if (l == 0) {
                     const cplx lr = t.lrho[o];
-                    acc = cadd(acc, make_double2(a0.x * (log_s - lr.x) + a0.y * lr.y - S.x,
-                                                 -a0.x * lr.y + a0.y * (log_s - lr.x) - S.y));
+                    acc[0][j] = cadd(acc[0][j], make_double2(A10.x * (log_s - lr.x) + A10.y * lr.y - S[0][j].x,
+                                                             -A10.x * lr.y + A10.y * (log_s - lr.x) - S[0][j].y));
+                    acc[1][j] = cadd(acc[1][j], make_double2(A20.x * (log_s - lr.x) + A20.y * lr.y - S[1][j].x,
+                                                             -A20.x * lr.y + A20.y * (log_s - lr.x) - S[1][j].y));
                 } else {
-                    const cplx w = cadd(cscale(a0, 1.0 / (double)l), S);
-                    acc = cadd(acc, cscale(cmul(rho[l], w), -sgn));
+                    const double il = 1.0 / (double)l;
+                    acc[0][j] = cadd(acc[0][j], cscale(cmul(rho[l], cadd(cscale(A10, il), S[0][j])), -sgn));
+                    acc[1][j] = cadd(acc[1][j], cscale(cmul(rho[l], cadd(cscale(A20, il), S[1][j])), -sgn));
                 }
-            } else {
-                for (int k = 0; k < q; ++k) {
-                    const double c = Cb[k * q + l];
-                    S.x = fma(c, h[k].x, S.x);
-                    S.y = fma(c, h[k].y, S.y);
-                }
-                acc = cadd(acc, cscale(cmul(rho[l + 1], S), sgn / s));
-                if (l == 0) acc = cadd(acc, make_double2(-(a0.x - a1.y), a0.y + a1.x));   // -conj(A1_0 + i A2_0)
+                acc[2][j] = cadd(acc[2][j], cscale(cmul(rho[l + 1], S[2][j]), sgn / s));
+                if (l == 0) acc[2][j] = cadd(acc[2][j], make_double2(-(A10.x - A20.y), A10.y + A20.x));   // -conj(A1_0 + i A2_0)
             }
         }
+    cplx *out = loc + (level_offset(level) + box) * (long long)(3 * q);
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        if (v0) out[a * q + l0] = acc[a][0];
+        if (v1) out[a * q + l1] = acc[a][1];
     }
-    if (active) loc[(level_offset(level) + box) * (long long)(3 * q) + a * q + l] = acc;
 }
 
 // L2L: child local expansions inherit the parent's.  One thread per (child box, k); child level = `level`.
@@ -677,10 +687,9 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
         fmm_m2m<<<(unsigned)((work + 127) / 128), 128, 0, st>>>(l, q, tab, enc, mult, boxcnt);
         ++launches;
     }
-    const size_t smem_m2l = sizeof(double) * (size_t)(((q * q + 1) & ~1) + 12 * q);
-    const int thr_m2l = (3 * q + 31) & ~31;
+    const size_t smem_m2l = sizeof(double) * (size_t)(((q * q + 1) & ~1) + 2 * kM2LWarps * 3 * (q + 1));
     for (int l = 2; l <= L; ++l) {
-        fmm_m2l<<<1u << (2 * l), thr_m2l, smem_m2l, st>>>(l, q, tab, enc, mult, boxcnt, loc);
+        fmm_m2l<<<((1u << (2 * l)) + kM2LWarps - 1) / kM2LWarps, 32 * kM2LWarps, smem_m2l, st>>>(l, q, tab, enc, mult, boxcnt, loc);
         ++launches;
     }
     for (int l = 3; l <= L; ++l) {
@@ -826,10 +835,9 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
         fmm_m2m<<<(unsigned)((work + 127) / 128), 128, 0, st>>>(l, q, tab, enc, mult, boxcnt);
         ++launches;
     }
-    const size_t smem_m2l = sizeof(double) * (size_t)(((q * q + 1) & ~1) + 12 * q);
-    const int thr_m2l = (3 * q + 31) & ~31;
+    const size_t smem_m2l = sizeof(double) * (size_t)(((q * q + 1) & ~1) + 2 * kM2LWarps * 3 * (q + 1));
     for (int l = 2; l <= L; ++l) {
-        fmm_m2l<<<1u << (2 * l), thr_m2l, smem_m2l, st>>>(l, q, tab, enc, mult, boxcnt, loc);
+        fmm_m2l<<<((1u << (2 * l)) + kM2LWarps - 1) / kM2LWarps, 32 * kM2LWarps, smem_m2l, st>>>(l, q, tab, enc, mult, boxcnt, loc);
         ++launches;
     }
     for (int l = 3; l <= L; ++l) {
