@@ -3,6 +3,7 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 0..4] [--precision f32|f64]
     python bench.py --impl reference ...        # the oracle, as it stands, on the host cores
+    python bench.py --path masked|targets|aux|fmm [--order P] ...   # the NEXT rows, same JSON line
 
 A *step* is one pass of the whole hot path (DESIGN.md rows a-1..a-5: arclength weights, packing,
 pair sum, reduction, scaling) over one batch of synthetic input.  The default workload is

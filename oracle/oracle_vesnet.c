@@ -21,6 +21,9 @@
  *                                d/ds = |dX/dalpha|^-1 d/dalpha                      PAPER.md:161-169 (sec 2.2.1)
  *   near field of a point        distance to the vesicle <= arclength spacing
  *   near vesicles masked out of the direct sum, same mask returned                   PAPER.md:329 (sec 4.1), 426 (Alg. 4 l.4)
+ *   free targets (all vesicles contribute)                                           eq 2.8 summed over every vesicle
+ *   elastic force                f = -kappa_b X_ssss + (sigma X_s)_s                 PAPER.md:123 (eq 2.7)
+ *   redistribution               6x upsampling, arclength, search, linear interp.    PAPER.md:331-335 (sec 4.2)
  *
  * Arithmetic: every term and every accumulator is `long double` (x87 80-bit on
  * x86-64; >= fp64 everywhere), loops are in the order the definition is written,
@@ -32,8 +35,10 @@
  * Stokeslet, S[n] = 0 outside a closed circle / ellipse, closed form for a
  * constant density on a circle, scaling / adjoint identities, brute-force
  * symmetric pair sums, equivariances, circle / ellipse weights and the elliptic
- * integral perimeter, numpy.fft for the derivative.  Nothing here is "parity
- * unpinned".
+ * integral perimeter, numpy.fft for the derivative; near mask against a brute-force
+ * definition; elastic force against circle / warped-circle / ellipse closed forms,
+ * zero net force and a numpy FFT route; redistribution against its fixed point, a
+ * warped circle and a numpy FFT / interp route.  Nothing here is "parity unpinned".
  */
 #include <math.h>
 #include <stdint.h>

@@ -370,6 +370,6 @@ const char *vn_status_string(vn_status s)
     return "unknown status";
 }
 
-int vn_version(void) { return 200; }
+int vn_version(void) { return 300; }
 
 }  // extern "C"
