@@ -194,6 +194,7 @@ def workload_config(args, susp, note=""):
             "pairs_per_evaluation": 512 * 512 * P if args.path == "targets" else susp.pairs,
             "evaluations_per_step": evals,
             "precision": args.precision, "l2": "flushed between timed steps (256 MiB write); inputs < L2",
+            "cuda_graph": bool(getattr(args, "graph", False)),
             "parallelism": f"{args.gpus} independent suspensions (one per GPU)" if args.gpus > 1 else "single GPU",
             "note": note}
 
@@ -307,6 +308,8 @@ def main():
                          "interactions per second so that it compares with --path farfield")
     ap.add_argument("--order", type=int, default=0, help="expansion order of --path fmm (default 12 for f32, 38 for f64); with --path targets a value > 0 "
                          "selects vn_farfield_targets_fmm")
+    ap.add_argument("--graph", action="store_true",
+                    help="capture one step (all its evaluations) into a CUDA graph after the warm-up and time graph replays")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -424,6 +427,23 @@ def main():
     for _ in range(max(args.warmup, 3)):
         step_device()
     torch.cuda.synchronize()
+    step_eager = step_device
+    if args.graph:                                     # every call only enqueues stream-ordered work: capturable
+        cap = torch.cuda.Stream()
+        cap.wait_stream(torch.cuda.current_stream())
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.stream(cap):
+            step_eager()
+            cap.synchronize()
+            n_cap = vn.vn_launch_count()
+            with torch.cuda.graph(graph, stream=cap):
+                step_eager()
+            launches_per_step = vn.vn_launch_count() - n_cap      # kernels recorded into the graph
+        torch.cuda.synchronize()
+        step_device = graph.replay
+        for _ in range(2):
+            step_device()
+        torch.cuda.synchronize()
 
     sampler = ClockSampler(nvml_index(local_rank))
     sampler.start()
@@ -432,6 +452,8 @@ def main():
     n0 = vn.vn_launch_count()
     t_dev = timed(step_device, args.steps, True)
     launches = vn.vn_launch_count() - n0
+    if args.graph:
+        launches = launches_per_step * args.steps            # replayed from the graph, not re-enqueued by the host
     kernel_ms = vn.vn_profile_read()
     vn.vn_profile_enable(False)
     sampler.stop_flag.set()

@@ -27,7 +27,8 @@
  *  - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Device
  *    calls only enqueue work and return; scratch memory is stream-ordered
  *    (cudaMallocAsync / cudaFreeAsync on `stream`), so back-to-back calls on one stream
- *    need no host synchronisation.
+ *    need no host synchronisation and a sequence of calls can be captured into a CUDA graph
+ *    (after one eager call per entry point, which performs the lazy per-device initialisation).
  *  - Errors are return codes only; nothing is printed, thrown or aborted.
  *      VN_ERR_INVALID_ARG  null pointer, nves < 1, npts < 1, nves*npts >= 2^31,
  *                          mu not finite or <= 0, bad enum, misaligned pointer

@@ -238,3 +238,45 @@ def test_launch_counter_moves():
     vn.vn_farfield(dev(s.X, np.float32), dev(s.F, np.float32), dev(W, np.float32))
     torch.cuda.synchronize()
     assert vn.vn_launch_count() >= n0 + 3
+
+
+# ------------------------------------------------------------------------------------- CUDA graphs
+@pytest.mark.parametrize("path", ["farfield", "fmm"])
+def test_sequence_is_graph_capturable(path):
+    """Config 4's pattern (copy positions, weights, evaluation, several times on one stream) captured into a CUDA graph
+    and replayed: every call only enqueues stream-ordered work (incl. its scratch), so the replay is bitwise the
+    eager result."""
+    s, W = problem(1)
+    rng = np.random.Generator(np.random.PCG64(11))
+    seq = [dev(s.X + 1e-3 * rng.standard_normal(s.X.shape), np.float32) for _ in range(3)]
+    Fd = dev(s.F, np.float32)
+    Xd, Wd, Ud = torch.empty_like(seq[0]), torch.empty((s.nves, s.npts), dtype=torch.float32, device="cuda"), torch.empty_like(seq[0])
+    outs = [torch.empty_like(Ud) for _ in seq]
+
+    def run():
+        for x, o in zip(seq, outs):
+            Xd.copy_(x)
+            vn.vn_arclength_weights(Xd, out=Wd)
+            if path == "farfield":
+                vn.vn_farfield(Xd, Fd, Wd, s.mu, out=Ud)
+            else:
+                vn.vn_farfield_fmm(Xd, Fd, Wd, s.mu, 12, out=Ud)
+            o.copy_(Ud)
+
+    run()                                               # eager: also performs every lazy initialisation
+    torch.cuda.synchronize()
+    eager = [o.clone() for o in outs]
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        run()                                           # warm the side stream
+        side.synchronize()
+        with torch.cuda.graph(g, stream=side):
+            run()
+    for o in outs:
+        o.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    for a, b in zip(eager, outs):
+        assert torch.equal(a, b)
