@@ -208,6 +208,16 @@ vn_status vn_redistribute_arclength(const void *X, int64_t nves, int64_t npts, v
 vn_status vn_profile_enable(int enable);
 int64_t vn_profile_read(double *ms, int64_t max_entries);
 
+/* Host-only introspection (no CUDA call, works without a GPU): the work decomposition vn_farfield would use
+ * for nves x npts points when `resident_blocks` blocks of the pair kernel fit on the device at once
+ * (148 SMs x 3 on a B200).  plan[0] = points per super-tile (target block), plan[1] = source tiles per
+ * super-tile, plan[2] = number of super-tiles n_st, plan[3] = chunks per super-tile (grid = n_st * chunks),
+ * plan[4] = points per source tile.  Block (I, c) walks chunk c of the list  { tiles of I itself; tiles of
+ * super-tiles I+1 .. I+S_I (mod n_st) },  S_I = floor((n_st-1)/2) (+1 for I < n_st/2 when n_st is even), which
+ * visits every unordered pair of super-tiles exactly once.  Used by the CPU tests of the host logic. */
+vn_status vn_plan_farfield(int64_t nves, int64_t npts, vn_precision precision, int32_t resident_blocks,
+                           int32_t *plan /* HOST, 5 entries */);
+
 /* Number of kernels of this library launched by the calling process so far
  * (all entry points, all streams).  Used by bench.py to report gpu_launches. */
 int64_t vn_launch_count(void);

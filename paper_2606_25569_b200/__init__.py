@@ -68,6 +68,8 @@ def lib():
         L.vn_farfield_fmm.restype = ci
         L.vn_farfield_targets_fmm.argtypes = [vp, i64, vp, vp, vp, i64, i64, dbl, ci, vp, ci, vp]
         L.vn_farfield_targets_fmm.restype = ci
+        L.vn_plan_farfield.argtypes = [i64, i64, ci, ctypes.c_int32, ctypes.POINTER(ctypes.c_int32)]
+        L.vn_plan_farfield.restype = ci
         L.vn_profile_enable.argtypes = [ci]
         L.vn_profile_enable.restype = ci
         L.vn_profile_read.argtypes = [ctypes.POINTER(dbl), i64]
@@ -324,6 +326,15 @@ def vn_farfield_host(X, F, W=None, mu: float = 1.0, out=None):
     if rc != VN_OK:
         raise VesnetError(rc, "vn_farfield_host")
     return out
+
+
+def vn_plan_farfield(nves: int, npts: int, precision: int = VN_F32, resident_blocks: int = 148 * 3):
+    """Host-only: the work decomposition of vn_farfield as a dict (no GPU needed)."""
+    buf = (ctypes.c_int32 * 5)()
+    rc = lib().vn_plan_farfield(nves, npts, precision, resident_blocks, buf)
+    if rc != VN_OK:
+        raise VesnetError(rc, "vn_plan_farfield")
+    return dict(super_tile=buf[0], tiles_per_super_tile=buf[1], n_super_tiles=buf[2], n_chunks=buf[3], tile=buf[4])
 
 
 def vn_profile_enable(enable: bool) -> None:

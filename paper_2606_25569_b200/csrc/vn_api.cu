@@ -42,6 +42,8 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
                        const int64_t *near_ptr, const int32_t *near_ves, void *U, vn_precision prec, cudaStream_t st);
 vn_status farfield_targets_fmm(const void *Xt, int64_t nt, const void *X, const void *F, const void *W, int64_t nves,
                                int64_t npts, double mu, int order, void *Ut, vn_precision prec, cudaStream_t st);
+void plan_f32(long long P, int slots, int *super_tile, int *sub, SymSplit *sp);
+void plan_f64(long long P, int slots, int *super_tile, int *sub, SymSplit *sp);
 vn_status near_pairs(const void *X, const void *W, int64_t nves, int64_t npts, int64_t *near_ptr,
                      int32_t *near_ves, int64_t capacity, vn_precision prec, cudaStream_t st);
 vn_status arclength_weights(const void *X, int64_t nves, int64_t npts, void *W, vn_precision prec, cudaStream_t st);
@@ -328,6 +330,21 @@ vn_status vn_farfield_host(const void *X, const void *F, const void *W, int64_t 
     if (rc != VN_OK) return rc;
     VN_CUDA(cudaMemcpyAsync(U, dU, bX, cudaMemcpyDeviceToHost, st));
     VN_CUDA(cudaStreamSynchronize(st));
+    return VN_OK;
+}
+
+vn_status vn_plan_farfield(int64_t nves, int64_t npts, vn_precision precision, int32_t resident_blocks, int32_t *plan)
+{
+    if (!plan || resident_blocks < 1 || check_shape(nves, npts, precision) != VN_OK) return VN_ERR_INVALID_ARG;
+    int super_tile = 0, sub = 0;
+    SymSplit sp;
+    if (precision == VN_F32) plan_f32(nves * npts, resident_blocks, &super_tile, &sub, &sp);
+    else plan_f64(nves * npts, resident_blocks, &super_tile, &sub, &sp);
+    plan[0] = super_tile;
+    plan[1] = sub;
+    plan[2] = sp.n_st;
+    plan[3] = sp.n_chunks;
+    plan[4] = kTile;
     return VN_OK;
 }
 

@@ -575,4 +575,12 @@ vn_status farfield_targets_f32(const void *Xt, int64_t nt, const void *X, const 
     return e == cudaSuccess ? VN_OK : VN_ERR_CUDA;
 }
 
+// host-only: the decomposition vn_farfield (fp32) would use with `slots` resident blocks (vn_plan_farfield)
+void plan_f32(long long P, int slots, int *super_tile, int *sub, SymSplit *sp)
+{
+    *super_tile = kST32;
+    *sub = kSub32;
+    *sp = choose_sym_split(P, kST32, slots, VN_F32_MINTILES);
+}
+
 }  // namespace vn

@@ -436,4 +436,12 @@ vn_status farfield_targets_f64(const void *Xt, int64_t nt, const void *X, const 
     return e == cudaSuccess ? VN_OK : VN_ERR_CUDA;
 }
 
+// host-only: the decomposition vn_farfield (fp64) would use with `slots` resident blocks (vn_plan_farfield)
+void plan_f64(long long P, int slots, int *super_tile, int *sub, SymSplit *sp)
+{
+    *super_tile = kST64;
+    *sub = kSub64;
+    *sp = choose_sym_split(P, kST64, slots, VN_F64_MINTILES);
+}
+
 }  // namespace vn

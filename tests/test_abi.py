@@ -22,7 +22,7 @@ def test_library_exports_every_declared_symbol():
     names = _declared()
     assert {"vn_farfield", "vn_arclength_weights", "vn_farfield_host", "vn_status_string",
             "vn_version", "vn_launch_count", "vn_near_pairs", "vn_farfield_masked",
-            "vn_farfield_targets", "vn_elastic_force", "vn_redistribute_arclength", "vn_farfield_fmm", "vn_farfield_targets_fmm"} <= set(names)
+            "vn_farfield_targets", "vn_elastic_force", "vn_redistribute_arclength", "vn_farfield_fmm", "vn_farfield_targets_fmm", "vn_plan_farfield"} <= set(names)
     for n in names:
         assert hasattr(L, n), n
     assert vn.vn_version() >= 100
