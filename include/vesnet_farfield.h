@@ -146,8 +146,8 @@ vn_status vn_farfield_targets(const void *Xt, int64_t nt,
  * `order` = p, the number of terms kept in the multipole / local expansions (2 <= p <= 48); the
  * relative L2 truncation error falls like 0.45^p (measured on the synthetic suspensions: p = 12
  * about 3e-6, p = 20 about 5e-9, p = 38 about 1e-13); vn_farfield stays the exact path.
- * Arithmetic is double inside for both storage precisions, so the VN_F32 result is the double
- * result rounded once.  Uniform quadtree over the bounding square of the points; a strongly
+ * The expansions are double for both storage precisions; the direct part over neighbouring leaves runs
+ * in the storage precision (VN_F32: the same SFU pair arithmetic as vn_farfield, error about 1e-6).  Uniform quadtree over the bounding square of the points; a strongly
  * non-uniform point distribution costs time (crowded leaves), not accuracy.  Results are bitwise
  * reproducible.  Scratch: about 100 * (p+1) bytes per leaf box plus 100 bytes per point.
  * near_ptr / near_ves: NULL for the plain sum (vn_farfield's quantity), or the CSR near-field

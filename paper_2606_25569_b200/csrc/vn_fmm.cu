@@ -14,8 +14,9 @@
 // square, power moments about box centres scaled by the box size, M2M / M2L / L2L in scaled variables, local
 // expansions evaluated at the targets, direct sums over the 3 x 3 neighbour boxes.  The target's own vesicle is
 // excluded as in vn_farfield: the direct part skips it, and what the expansions included of it (own-vesicle
-// points in non-neighbour boxes) is subtracted by a short direct sum.  All arithmetic is double for both storage
-// precisions; the accuracy is set by p (truncation error about 0.45^p relative, measured).
+// points in non-neighbour boxes) is subtracted by a short direct sum.  The expansions are double for both storage
+// precisions, so the accuracy of the far part is set by p alone (truncation error about 0.45^p relative, measured);
+// the direct part runs in the storage precision (fp32: the SFU pair arithmetic of the exact fp32 kernel).
 #include "vn_common.cuh"
 #include "vn_log64.cuh"
 
@@ -483,6 +484,7 @@ __global__ void fmm_build_logtab(double *tab)
 constexpr int kP2PThreads = 64;
 constexpr int kP2PSplit = 4;
 constexpr int kP2PTargets = 4;
+template <bool F32NEAR>
 __global__ void __launch_bounds__(kP2PThreads)
 fmm_l2p_p2p(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const int *__restrict__ vs,
             const long long *__restrict__ start, const cplx *__restrict__ tz, const int *__restrict__ tvs,
@@ -490,8 +492,11 @@ fmm_l2p_p2p(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const int 
             const unsigned long long *__restrict__ enc, const cplx *__restrict__ loc, const double *__restrict__ logtab,
             cplx *__restrict__ accum)
 {   // targets (tz, tvs, tperm, tstart) are the sorted sources themselves for vn_farfield_fmm, a separate sorted set
-    // (tvs == nullptr: no vesicle to exclude) for the free-target variant
-    __shared__ double tab[kLogTab + kExpTab];
+    // (tvs == nullptr: no vesicle to exclude) for the free-target variant.
+    // F32NEAR (fp32 storage): the direct part runs in fp32 with the SFU lg2/rcp, exactly the pair arithmetic of the
+    // exact fp32 kernel (the stored positions and densities ARE floats, so nothing is lost converting them back),
+    // per-chunk float partial sums folded into double accumulators; the expansions stay double.
+    __shared__ double tab[F32NEAR ? 1 : kLogTab + kExpTab];
     __shared__ cplx lc[3 * kFmmMaxQ];
     __shared__ double4 src[kP2PThreads];               // (zeta_x, zeta_y, g_x, g_y)
     __shared__ int sves[kP2PThreads];
@@ -502,7 +507,8 @@ fmm_l2p_p2p(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const int 
     const long long a = tstart[c], b = tstart[c + 1];
     if (a == b) return;
     const int tid = threadIdx.x, slot = tid / kP2PSplit, part = tid % kP2PSplit;
-    for (int e = tid; e < kLogTab + kExpTab; e += kP2PThreads) tab[e] = logtab[e];
+    if (!F32NEAR)
+        for (int e = tid; e < kLogTab + kExpTab; e += kP2PThreads) tab[e] = logtab[e];
     for (int e = tid; e < 3 * q; e += kP2PThreads) lc[e] = loc[(level_offset(L) + c) * (long long)(3 * q) + e];
     const Geom gm = load_geom(enc);
     const double s = gm.size / (double)n, inv_s = 1.0 / s;
@@ -559,19 +565,46 @@ fmm_l2p_p2p(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const int 
                     }
                     __syncthreads();
                     const int cnt = (int)min((long long)kP2PThreads, sb - s0);
-                    for (int j = part; j < cnt; j += kP2PSplit) {
-                        const double4 sj = src[j];
-                        const int sv = sves[j];
+                    if (F32NEAR) {
+                        float fx[kP2PTargets], fy[kP2PTargets], zx[kP2PTargets], zy[kP2PTargets];
 #pragma unroll
                         for (int r = 0; r < kP2PTargets; ++r) {
-                            if (sv == myves[r] || !live[r]) continue;
-                            const double rx = z[r].x - sj.x, ry = z[r].y - sj.y;
-                            const double r2 = fma(rx, rx, ry * ry);
-                            double ml, inv;
-                            log_rcp_f64(r2, tab, ml, inv);
-                            const double qd = fma(rx, sj.z, ry * sj.w) * inv;
-                            ux[r] = fma(ml, sj.z, fma(qd, rx, ux[r]));
-                            uy[r] = fma(ml, sj.w, fma(qd, ry, uy[r]));
+                            fx[r] = fy[r] = 0.f;
+                            zx[r] = (float)z[r].x;
+                            zy[r] = (float)z[r].y;
+                        }
+                        for (int j = part; j < cnt; j += kP2PSplit) {
+                            const double4 sj = src[j];
+                            const float sx = (float)sj.x, sy = (float)sj.y, gx = (float)sj.z, gy = (float)sj.w;
+                            const int sv = sves[j];
+#pragma unroll
+                            for (int r = 0; r < kP2PTargets; ++r) {
+                                if (sv == myves[r] || !live[r]) continue;
+                                const float rx = zx[r] - sx, ry = zy[r] - sy;
+                                const float r2 = fmaf(rx, rx, ry * ry);
+                                const float ml = -0.34657359027997264f * sfu_lg2(r2);
+                                const float qd = fmaf(rx, gx, ry * gy) * sfu_rcp(r2);
+                                fx[r] += fmaf(ml, gx, qd * rx);
+                                fy[r] += fmaf(ml, gy, qd * ry);
+                            }
+                        }
+#pragma unroll
+                        for (int r = 0; r < kP2PTargets; ++r) { ux[r] += (double)fx[r]; uy[r] += (double)fy[r]; }
+                    } else {
+                        for (int j = part; j < cnt; j += kP2PSplit) {
+                            const double4 sj = src[j];
+                            const int sv = sves[j];
+#pragma unroll
+                            for (int r = 0; r < kP2PTargets; ++r) {
+                                if (sv == myves[r] || !live[r]) continue;
+                                const double rx = z[r].x - sj.x, ry = z[r].y - sj.y;
+                                const double r2 = fma(rx, rx, ry * ry);
+                                double ml, inv;
+                                log_rcp_f64(r2, tab, ml, inv);
+                                const double qd = fma(rx, sj.z, ry * sj.w) * inv;
+                                ux[r] = fma(ml, sj.z, fma(qd, rx, ux[r]));
+                                uy[r] = fma(ml, sj.w, fma(qd, ry, uy[r]));
+                            }
                         }
                     }
                 }
@@ -697,7 +730,10 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
         fmm_l2l<<<(unsigned)((work + 127) / 128), 128, 0, st>>>(l, q, tab, enc, loc);
         ++launches;
     }
-    fmm_l2p_p2p<<<ncell, kP2PThreads, 0, st>>>(zs, gs, vs, start, zs, vs, perm, start, q, enc, loc, logtab, accum);
+    if (prec == VN_F32)
+        fmm_l2p_p2p<true><<<ncell, kP2PThreads, 0, st>>>(zs, gs, vs, start, zs, vs, perm, start, q, enc, loc, logtab, accum);
+    else
+        fmm_l2p_p2p<false><<<ncell, kP2PThreads, 0, st>>>(zs, gs, vs, start, zs, vs, perm, start, q, enc, loc, logtab, accum);
     profile_mark(st, false);
     if (near_ptr) {   // row f-1 on top: take the near vesicles' contributions out (they are all in the direct part)
         const vn_status rc = near_correction_accum(X, F, W, P, (int)npts, near_ptr, near_ves, accum, prec, st);
@@ -845,7 +881,10 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
         fmm_l2l<<<(unsigned)((work + 127) / 128), 128, 0, st>>>(l, q, tab, enc, loc);
         ++launches;
     }
-    fmm_l2p_p2p<<<ncell, kP2PThreads, 0, st>>>(zs, gs, vs, start, zts, nullptr, tperm, tstart, q, enc, loc, logtab, accum);
+    if (prec == VN_F32)
+        fmm_l2p_p2p<true><<<ncell, kP2PThreads, 0, st>>>(zs, gs, vs, start, zts, nullptr, tperm, tstart, q, enc, loc, logtab, accum);
+    else
+        fmm_l2p_p2p<false><<<ncell, kP2PThreads, 0, st>>>(zs, gs, vs, start, zts, nullptr, tperm, tstart, q, enc, loc, logtab, accum);
     profile_mark(st, false);
     const double pref = 1.0 / (4.0 * 3.14159265358979323846 * mu);
     if (prec == VN_F32)
