@@ -533,3 +533,28 @@ def test_fmm_targets_parity(index, nt, dtype, order):
     err = rel_l2(got.cpu().numpy()[idx], ref)
     print(f"fmm targets config{index} nt={len(xt)} {np.dtype(dtype).name} p={order}: rel-L2 {err:.3e}")
     assert err <= TOL[dtype]
+
+
+@pytest.mark.parametrize("layout", ["two_clusters", "line", "one_far_outlier"])
+def test_fmm_nonuniform_layouts(layout):
+    """Strongly non-uniform point distributions cost time (crowded leaves), never accuracy."""
+    rng = np.random.Generator(np.random.PCG64({"two_clusters": 501, "line": 502, "one_far_outlier": 503}[layout]))
+    nves, npts = 60, 64
+    al = 2 * np.pi * np.arange(npts) / npts
+    body = np.stack([np.cos(al), 0.5 * np.sin(al)], -1) * 0.3
+    if layout == "two_clusters":
+        cen = np.concatenate([rng.normal(size=(30, 2)) * 2.0, rng.normal(size=(30, 2)) * 2.0 + np.array([400.0, 250.0])])
+    elif layout == "line":
+        cen = np.stack([np.arange(nves) * 0.9, np.zeros(nves)], -1)
+    else:
+        cen = rng.normal(size=(nves, 2)) * 3.0
+        cen[-1] = (5000.0, -3000.0)
+    X = body[None] + cen[:, None, :]
+    F = rng.normal(size=X.shape)
+    W = oracle.weights(X)
+    ref = oracle.farfield(X, F, W, 1.0)
+    got = vn.vn_farfield_fmm(dev(X, np.float64), dev(F, np.float64), dev(W, np.float64), 1.0, 40)
+    torch.cuda.synchronize()
+    err = rel_l2(got.cpu().numpy(), ref)
+    print(f"fmm {layout}: rel-L2 {err:.3e}")
+    assert err <= 1e-11
