@@ -560,7 +560,10 @@ fmm_l2p_p2p(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const int 
                     __syncthreads();
                     if (s0 + tid < sb) {
                         const cplx zz = zs[s0 + tid], gg = gs[s0 + tid];
-                        src[tid] = make_double4(zz.x, zz.y, gg.x, gg.y);
+                        if (F32NEAR)    // the stored values are floats: converted back once per staged source, exactly
+                            reinterpret_cast<float4 *>(src)[tid] = make_float4((float)zz.x, (float)zz.y, (float)gg.x, (float)gg.y);
+                        else
+                            src[tid] = make_double4(zz.x, zz.y, gg.x, gg.y);
                         sves[tid] = vs[s0 + tid];
                     }
                     __syncthreads();
@@ -574,8 +577,8 @@ fmm_l2p_p2p(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const int 
                             zy[r] = (float)z[r].y;
                         }
                         for (int j = part; j < cnt; j += kP2PSplit) {
-                            const double4 sj = src[j];
-                            const float sx = (float)sj.x, sy = (float)sj.y, gx = (float)sj.z, gy = (float)sj.w;
+                            const float4 sj = reinterpret_cast<const float4 *>(src)[j];
+                            const float sx = sj.x, sy = sj.y, gx = sj.z, gy = sj.w;
                             const int sv = sves[j];
 #pragma unroll
                             for (int r = 0; r < kP2PTargets; ++r) {
