@@ -40,7 +40,10 @@
  *    fp32 numbers, and vn_farfield_targets additionally shares one reciprocal between two pairs
  *    (t = rcp(a*b), 1/a = t*b), which needs a*b inside the fp32 normal range, i.e.
  *    1e-9 < |r| < 1e9 in the caller's units.  VN_F64 needs normal doubles whose reciprocal is normal.
- *  - Input values are not validated: NaN/Inf propagate.  Points of DIFFERENT vesicles
+ *  - Input values are not validated.  A non-finite value anywhere in X, F or W makes EVERY output of
+ *    vn_farfield / vn_farfield_masked / vn_farfield_targets NaN (their integer accumulators cannot carry
+ *    NaN/Inf point by point; a free target's own coordinates are not checked); the FMM calls let it
+ *    propagate through their double arithmetic.  Points of DIFFERENT vesicles
  *    are assumed distinct; a coincident cross-vesicle pair gives an unspecified (possibly
  *    non-finite) value at that target only (reading A5).  nves == 1 is valid and yields U == 0.
  */

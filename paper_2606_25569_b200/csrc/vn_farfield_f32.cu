@@ -66,7 +66,9 @@ __global__ void pack_sources_f32(const float2 *__restrict__ X, const float2 *__r
         src[2 * (size_t)s + 0] = make_ulonglong2(pk(y.x, y.x), pk(y.y, y.y));
         src[2 * (size_t)s + 1] = make_ulonglong2(pk(gx, gx), pk(gy, gy));
         m = fabsf(gx) + fabsf(gy);
-        if (!(m <= 3.4028234e38f)) m = __int_as_float(0x7f800000);   // NaN / Inf -> +Inf
+        // a non-finite density or position cannot be carried through the integer accumulators point by point:
+        // flag it (gmax = +Inf) and finish_f32 answers NaN everywhere
+        if (!(m <= 3.4028234e38f) || !(fabsf(y.x) + fabsf(y.y) <= 3.4028234e38f)) m = __int_as_float(0x7f800000);
     }
     const unsigned wm = __reduce_max_sync(0xffffffffu, __float_as_uint(m));
     if ((threadIdx.x & 31) == 0 && wm != 0u) atomicMax(gmax_bits, wm);
@@ -363,6 +365,10 @@ __global__ void finish_f32(const long long *__restrict__ acc, int n, int P, cons
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
+    if (*gmax_bits == 0x7f800000u) {                      // non-finite input somewhere: see pack_sources_f32
+        U[i] = make_float2(__int_as_float(0x7fc00000), __int_as_float(0x7fc00000));
+        return;
+    }
     const double f = prefactor / fixed_scale(*gmax_bits, P);
     const longlong2 v = *reinterpret_cast<const longlong2 *>(acc + 2 * (size_t)i);
     U[i] = make_float2((float)(f * (double)v.x), (float)(f * (double)v.y));

@@ -50,7 +50,10 @@ __global__ void pack_sources_f64(const double2 *__restrict__ X, const double2 *_
         const double gx = f.x * w, gy = f.y * w;
         src[s] = make_double4(y.x, y.y, gx, gy);
         m = fabs(gx) + fabs(gy);
-        if (!(m <= 1.7976931348623157e308)) m = __longlong_as_double(0x7ff0000000000000ll);   // NaN / Inf -> +Inf
+        // a non-finite density or position cannot be carried through the integer accumulators point by point:
+        // flag it (gmax = +Inf) and finish_f64 answers NaN everywhere
+        if (!(m <= 1.7976931348623157e308) || !(fabs(y.x) + fabs(y.y) <= 1.7976931348623157e308))
+            m = __longlong_as_double(0x7ff0000000000000ll);
     }
 #pragma unroll
     for (int k = 16; k >= 1; k >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, k));
@@ -261,6 +264,11 @@ __global__ void finish_f64(const long long *__restrict__ acc, int n, int P, cons
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
+    if (*gmax_bits == 0x7ff0000000000000ull) {            // non-finite input somewhere: see pack_sources_f64
+        const double qnan = __longlong_as_double(0x7ff8000000000000ll);
+        U[i] = make_double2(qnan, qnan);
+        return;
+    }
     const Fixed2 fx = fixed2_scale(*gmax_bits, P);
     const longlong2 a = *reinterpret_cast<const longlong2 *>(acc + 4 * (size_t)i);
     const longlong2 b = *reinterpret_cast<const longlong2 *>(acc + 4 * (size_t)i + 2);

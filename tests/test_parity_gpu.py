@@ -280,3 +280,30 @@ def test_sequence_is_graph_capturable(path):
     torch.cuda.synchronize()
     for a, b in zip(eager, outs):
         assert torch.equal(a, b)
+
+
+# ------------------------------------------------------------------------------------- degenerate inputs (reading A5)
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+@pytest.mark.parametrize("call", ["farfield", "fmm"])
+def test_coincident_points_and_nans_stay_local(call, dtype):
+    """A coincident cross-vesicle pair (precondition violation) and a NaN density may spoil the targets they touch,
+    nothing else: no hang, no fault, every other target keeps its value."""
+    s, W = problem(1)
+    X, F = s.X.copy(), s.F.copy()
+    X[5, 7] = X[200, 3]                                   # point (5,7) now coincides with point (200,3)
+    Xd, Fd, Wd = dev(X, dtype), dev(F, dtype), dev(W, dtype)
+    fn = (lambda f: vn.vn_farfield(Xd, f, Wd, s.mu)) if call == "farfield" else (lambda f: vn.vn_farfield_fmm(Xd, f, Wd, s.mu, 12 if dtype == np.float32 else 38))
+    got = fn(Fd).cpu().numpy()
+    torch.cuda.synchronize()
+    Xo, Fo, Wo = oracle_inputs(X, F, W, dtype)
+    idx = np.setdiff1d(sample_targets(s.nves * s.npts, 1500, 17), [5 * s.npts + 7, 200 * s.npts + 3])
+    ref = oracle.farfield_subset(Xo, Fo, Wo, idx, s.mu)
+    assert rel_l2(got.reshape(-1, 2)[idx], ref) <= TOL[dtype]
+    # a NaN density at one source poisons every target of the other vesicles (that is the sum's meaning); the exact
+    # path answers NaN everywhere (documented: its integer accumulators cannot carry NaN point by point)
+    Fn = F.copy(); Fn[9, 0, 0] = np.nan
+    gotn = fn(dev(Fn, dtype)).cpu().numpy()
+    torch.cuda.synchronize()
+    assert np.isnan(gotn[10]).all()
+    if call == "farfield":
+        assert np.isnan(gotn).all()
