@@ -364,13 +364,12 @@ fmm_m2l(int level, int q, const double *__restrict__ tab, const unsigned long lo
     for (int e = threadIdx.x; e < q * q; e += blockDim.x) Cb[e] = t.Cb[e];
     __syncthreads();
     const int n = 1 << level;
-    const int box = blockIdx.x * kM2LWarps + warp;
-    if (box >= n * n) return;
-    const int ix = box / n, iy = box % n;
     const Geom gm = load_geom(enc);
     const double s = gm.size / (double)n, log_s = log(s);
     const int l0 = ln, l1 = ln + 32;
     const bool v0 = l0 < q, v1 = l1 < q;
+    for (int box = blockIdx.x * kM2LWarps + warp; box < n * n; box += gridDim.x * kM2LWarps) {
+    const int ix = box / n, iy = box % n;
     cplx acc[3][2];
 #pragma unroll
     for (int a = 0; a < 3; ++a) acc[a][0] = acc[a][1] = make_double2(0.0, 0.0);
@@ -440,6 +439,8 @@ fmm_m2l(int level, int q, const double *__restrict__ tab, const unsigned long lo
         if (v0) out[a * q + l0] = acc[a][0];
         if (v1) out[a * q + l1] = acc[a][1];
     }
+    __syncwarp();
+    }   // boxes
 }
 
 // L2L: child local expansions inherit the parent's.  One thread per (child box, k); child level = `level`.
@@ -502,16 +503,19 @@ fmm_l2p_p2p(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const int 
     __shared__ int sves[kP2PThreads];
     constexpr int kRound = kP2PThreads / kP2PSplit;
     const int L = load_level(enc);
-    const int n = 1 << L, c = blockIdx.x, ix = c / n, iy = c % n;
-    if (c >= n * n) return;
-    const long long a = tstart[c], b = tstart[c + 1];
-    if (a == b) return;
+    const int n = 1 << L;
     const int tid = threadIdx.x, slot = tid / kP2PSplit, part = tid % kP2PSplit;
     if (!F32NEAR)
         for (int e = tid; e < kLogTab + kExpTab; e += kP2PThreads) tab[e] = logtab[e];
-    for (int e = tid; e < 3 * q; e += kP2PThreads) lc[e] = loc[(level_offset(L) + c) * (long long)(3 * q) + e];
     const Geom gm = load_geom(enc);
     const double s = gm.size / (double)n, inv_s = 1.0 / s;
+    // the grid is sized by the host for the deepest admissible tree: leaves are walked with a grid stride
+    for (int c = blockIdx.x; c < n * n; c += gridDim.x) {
+    const int ix = c / n, iy = c % n;
+    const long long a = tstart[c], b = tstart[c + 1];
+    if (a == b) continue;
+    __syncthreads();                                   // the previous leaf's lc is consumed
+    for (int e = tid; e < 3 * q; e += kP2PThreads) lc[e] = loc[(level_offset(L) + c) * (long long)(3 * q) + e];
     const cplx ctr = box_centre(gm, L, ix, iy);
     __syncthreads();
 
@@ -623,6 +627,7 @@ fmm_l2p_p2p(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const int 
         }
         __syncthreads();
     }
+    }   // leaves
 }
 
 // own-vesicle points that sit in NON-neighbour leaf boxes of the target went through the expansions: take their
@@ -715,6 +720,7 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
     fmm_build_logtab<<<8, 128, 0, st>>>(logtab);
     int launches = 13;
 
+    const int p2p_grid = ncell < 148 * 64 ? ncell : 148 * 64;      // grid-stride over the leaves the device chose
     profile_mark(st, true);
     fmm_p2m<<<(ncell + 3) / 4, 128, 0, st>>>(zs, gs, start, q, enc, mult, boxcnt);
     ++launches;
@@ -725,7 +731,8 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
     }
     const size_t smem_m2l = sizeof(double) * (size_t)(((q * q + 1) & ~1) + 2 * kM2LWarps * 3 * (q + 1));
     for (int l = 2; l <= L; ++l) {
-        fmm_m2l<<<((1u << (2 * l)) + kM2LWarps - 1) / kM2LWarps, 32 * kM2LWarps, smem_m2l, st>>>(l, q, tab, enc, mult, boxcnt, loc);
+        const unsigned nb = ((1u << (2 * l)) + kM2LWarps - 1) / kM2LWarps;
+        fmm_m2l<<<nb < 148u * 16u ? nb : 148u * 16u, 32 * kM2LWarps, smem_m2l, st>>>(l, q, tab, enc, mult, boxcnt, loc);
         ++launches;
     }
     for (int l = 3; l <= L; ++l) {
@@ -734,9 +741,9 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
         ++launches;
     }
     if (prec == VN_F32)
-        fmm_l2p_p2p<true><<<ncell, kP2PThreads, 0, st>>>(zs, gs, vs, start, zs, vs, perm, start, q, enc, loc, logtab, accum);
+        fmm_l2p_p2p<true><<<p2p_grid, kP2PThreads, 0, st>>>(zs, gs, vs, start, zs, vs, perm, start, q, enc, loc, logtab, accum);
     else
-        fmm_l2p_p2p<false><<<ncell, kP2PThreads, 0, st>>>(zs, gs, vs, start, zs, vs, perm, start, q, enc, loc, logtab, accum);
+        fmm_l2p_p2p<false><<<p2p_grid, kP2PThreads, 0, st>>>(zs, gs, vs, start, zs, vs, perm, start, q, enc, loc, logtab, accum);
     profile_mark(st, false);
     if (near_ptr) {   // row f-1 on top: take the near vesicles' contributions out (they are all in the direct part)
         const vn_status rc = near_correction_accum(X, F, W, P, (int)npts, near_ptr, near_ves, accum, prec, st);
@@ -866,6 +873,7 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
     fmm_build_logtab<<<8, 128, 0, st>>>(logtab);
     int launches = 21;
 
+    const int p2p_grid = ncell < 148 * 64 ? ncell : 148 * 64;      // grid-stride over the leaves the device chose
     profile_mark(st, true);
     fmm_p2m<<<(ncell + 3) / 4, 128, 0, st>>>(zs, gs, start, q, enc, mult, boxcnt);
     ++launches;
@@ -876,7 +884,8 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
     }
     const size_t smem_m2l = sizeof(double) * (size_t)(((q * q + 1) & ~1) + 2 * kM2LWarps * 3 * (q + 1));
     for (int l = 2; l <= L; ++l) {
-        fmm_m2l<<<((1u << (2 * l)) + kM2LWarps - 1) / kM2LWarps, 32 * kM2LWarps, smem_m2l, st>>>(l, q, tab, enc, mult, boxcnt, loc);
+        const unsigned nb = ((1u << (2 * l)) + kM2LWarps - 1) / kM2LWarps;
+        fmm_m2l<<<nb < 148u * 16u ? nb : 148u * 16u, 32 * kM2LWarps, smem_m2l, st>>>(l, q, tab, enc, mult, boxcnt, loc);
         ++launches;
     }
     for (int l = 3; l <= L; ++l) {
@@ -885,9 +894,9 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
         ++launches;
     }
     if (prec == VN_F32)
-        fmm_l2p_p2p<true><<<ncell, kP2PThreads, 0, st>>>(zs, gs, vs, start, zts, nullptr, tperm, tstart, q, enc, loc, logtab, accum);
+        fmm_l2p_p2p<true><<<p2p_grid, kP2PThreads, 0, st>>>(zs, gs, vs, start, zts, nullptr, tperm, tstart, q, enc, loc, logtab, accum);
     else
-        fmm_l2p_p2p<false><<<ncell, kP2PThreads, 0, st>>>(zs, gs, vs, start, zts, nullptr, tperm, tstart, q, enc, loc, logtab, accum);
+        fmm_l2p_p2p<false><<<p2p_grid, kP2PThreads, 0, st>>>(zs, gs, vs, start, zts, nullptr, tperm, tstart, q, enc, loc, logtab, accum);
     profile_mark(st, false);
     const double pref = 1.0 / (4.0 * 3.14159265358979323846 * mu);
     if (prec == VN_F32)
