@@ -482,9 +482,18 @@ __global__ void fmm_build_logtab(double *tab)
 //   far  = -(Re Phi1 + i Re Phi2) + (z/2) conj(Phi1' + i Phi2') - (1/2) conj(psi)   from the box's local expansions
 //   near = direct sum over the points of the 3 x 3 neighbour boxes that belong to OTHER vesicles
 // The sum goes to accum[original point index] (still without the 1/(4 pi mu)).
-constexpr int kP2PThreads = 64;
-constexpr int kP2PSplit = 4;
-constexpr int kP2PTargets = 4;
+#ifndef VN_FMM_P2P_THREADS
+#define VN_FMM_P2P_THREADS 128
+#endif
+#ifndef VN_FMM_P2P_SPLIT
+#define VN_FMM_P2P_SPLIT 4
+#endif
+#ifndef VN_FMM_P2P_TARGETS
+#define VN_FMM_P2P_TARGETS 2
+#endif
+constexpr int kP2PThreads = VN_FMM_P2P_THREADS;
+constexpr int kP2PSplit = VN_FMM_P2P_SPLIT;       // threads that share one target (power of two, <= 32)
+constexpr int kP2PTargets = VN_FMM_P2P_TARGETS;   // targets per thread
 template <bool F32NEAR>
 __global__ void __launch_bounds__(kP2PThreads)
 fmm_l2p_p2p(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const int *__restrict__ vs,
