@@ -307,3 +307,28 @@ def test_coincident_points_and_nans_stay_local(call, dtype):
     assert np.isnan(gotn[10]).all()
     if call == "farfield":
         assert np.isnan(gotn).all()
+
+
+def test_two_streams_interleaved():
+    """Calls enqueued alternately on two streams (different problems, different entry points): scratch is
+    stream-ordered per call, so the results equal the ones computed one after the other."""
+    s1, W1 = problem(1)
+    s0, W0 = problem(0)
+    a = [dev(s1.X, np.float32), dev(s1.F, np.float32), dev(W1, np.float32)]
+    b = [dev(s0.X, np.float64), dev(s0.F, np.float64), dev(W0, np.float64)]
+    ref_a = vn.vn_farfield(*a, s1.mu).clone()
+    ref_b = vn.vn_farfield(*b, s0.mu).clone()
+    ref_f = vn.vn_farfield_fmm(*a, s1.mu, 12).clone()
+    torch.cuda.synchronize()
+    st1, st2 = torch.cuda.Stream(), torch.cuda.Stream()
+    outs = []
+    for _ in range(4):
+        with torch.cuda.stream(st1):
+            ua = vn.vn_farfield(*a, s1.mu)
+            uf = vn.vn_farfield_fmm(*a, s1.mu, 12)
+        with torch.cuda.stream(st2):
+            ub = vn.vn_farfield(*b, s0.mu)
+        outs.append((ua, ub, uf))
+    torch.cuda.synchronize()
+    for ua, ub, uf in outs:
+        assert torch.equal(ua, ref_a) and torch.equal(ub, ref_b) and torch.equal(uf, ref_f)
