@@ -6,6 +6,9 @@
  * networks: "DirectSingleLayerIntegral(X, f)" (Alg. 4 line 3), the
  * O((MN)^2) direct evaluation of the single-layer integral between vesicles that is
  * "done without any approximation" and dominates the time step.
+ * Around it, declared further down: the near-field relation and the masked sum (the paper's
+ * actual DirectSingleLayerIntegral), free targets, a fast multipole evaluation of the same
+ * sums, the elastic force that produces F, and the equal-arclength redistribution.
  *
  * Mathematics (PAPER.md:129-136 eqs 2.8/2.9, :173 trapezoid rule, :140-144 eq 2.10):
  *
