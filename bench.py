@@ -525,14 +525,18 @@ def main():
                                   "pinned host buffers -> device copies -> the path's C-ABI calls -> copy back, synchronised"}
         if args.path == "masked":
             line["config"]["near_pairs"] = n_near
-        if args.path == "targets" and args.order > 0:
-            line["config"]["order"] = args.order
-            line["roofline"]["kernel"] = "fmm kernels (P2M, M2M, M2L, L2L, L2P+P2P)"
-            line["roofline"]["note"] = "approximate algorithm (vn_farfield_targets_fmm): 'achieved' counts the direct sum's interactions"
-        if args.path == "fmm":
-            line["config"]["order"] = fmm_order
-            line["roofline"]["note"] = ("approximate algorithm: 'achieved' counts the interactions of the direct sum it replaces, "
-                                        "not executed work; kernel_ms_avg spans P2M..P2P (all FMM kernels)")
+        if args.path == "fmm" or (args.path == "targets" and args.order > 0):
+            # an approximate O(P) algorithm does not execute the direct sum's interactions: no ALU roofline fraction
+            # is claimed for it; `value` is the direct sum's pair count over the FMM's time ("equivalent" rate)
+            line["config"]["order"] = fmm_order if args.path == "fmm" else args.order
+            rl = line["roofline"]
+            rl["kernel"] = "fmm kernels (P2M, M2M, M2L, L2L, L2P+P2P); kernel_ms_avg spans all of them"
+            rl["equivalent_ginteractions_per_s"] = rl.pop("kernel_ginteractions_per_s", None)
+            for k in ("achieved", "frac", "flop_frac", "frac_at_sampled_clock"):
+                rl[k] = None
+            rl["note"] = ("approximate algorithm (expansion order in config.order): no fraction of the pair kernels' "
+                          "instruction roofline is claimed; see profiles/r1f_fmm_kernels_config4_f64_ncu.md for the "
+                          "FP64-pipe occupancy of its two dominant kernels")
         if world == 1 and not args.no_cpu_baseline:
             v, cores, sample = oracle_rate(susp, np_dtype, 15.0, 4242, args.path)
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
