@@ -275,6 +275,48 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
                 RX(p) = fma2(KA, Ux[p], RX(p));
                 RY(p) = fma2(KA, Uy[p], RY(p));
             }
+        } else if (!both && cnt == kTile && npts % kTile == 0 && base + kST32 <= P) {
+            // a tile of the block's OWN super-tile when vesicles are whole tiles (npts a multiple of 128, the
+            // paper's N = 128): target k of a thread lies in tile k of the super-tile, so its own vesicle is
+            // excluded for ALL lanes alike.  One-directional, unpredicated, packed; the excluded halves (which
+            // also hold the r = 0 self pairs) are discarded after the tile.
+            u64 Ux[NP], Uy[NP];
+#pragma unroll
+            for (int p = 0; p < NP; ++p) Ux[p] = Uy[p] = 0ull;
+#pragma unroll 2
+            for (int j = 0; j < kTile; ++j) {
+                const ulonglong2 yy = ts[2 * j + 0];
+                const ulonglong2 gg = ts[2 * j + 1];
+#pragma unroll
+                for (int p = 0; p < NP; ++p) {
+                    const u64 rx = sub2(tx[p], yy.x);
+                    const u64 ry = sub2(ty[p], yy.y);
+                    const u64 r2 = fma2(rx, rx, mul2(ry, ry));
+                    float a, b, ka, kb;
+                    upk(r2, a, b);
+                    upk(mul2(r2, KA), ka, kb);
+                    const u64 inv = pk(sfu_rcp(ka), sfu_rcp(kb));
+                    const u64 l = pk(sfu_lg2(a), sfu_lg2(b));
+                    const u64 ux = mul2(rx, inv);
+                    const u64 uy = mul2(ry, inv);
+                    const u64 Mxy = mul2(ux, ry);
+                    const u64 Mxx = fma2(ux, rx, l);
+                    const u64 Myy = fma2(uy, ry, l);
+                    Ux[p] = fma2(Mxx, gg.x, fma2(Mxy, gg.y, Ux[p]));
+                    Uy[p] = fma2(Mxy, gg.x, fma2(Myy, gg.y, Uy[p]));
+                }
+            }
+            const int vs_src = first / npts;
+#pragma unroll
+            for (int p = 0; p < NP; ++p) {
+                float x0, x1, y0, y1;
+                upk(Ux[p], x0, x1);
+                upk(Uy[p], y0, y1);
+                if ((base + (2 * p) * kThreads) / npts == vs_src) x0 = y0 = 0.f;
+                if ((base + (2 * p + 1) * kThreads) / npts == vs_src) x1 = y1 = 0.f;
+                RX(p) = fma2(KA, pk(x0, x1), RX(p));
+                RY(p) = fma2(KA, pk(y0, y1), RY(p));
+            }
         } else if (cnt > 0) {
             // predicated path: own-vesicle sources and the ragged tail are skipped per pair
             float ux[T], uy[T];

@@ -202,6 +202,29 @@ farfield_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__
                     atomicAdd((unsigned long long *)(accj + 4 * jb),
                               (unsigned long long)fixed2_word(c[0], fx, lane % kDup));
             }
+        } else if (!both && cnt == kTile && npts % kTile == 0 && base + kST64 <= P) {
+            // a tile of the block's OWN super-tile when vesicles are whole tiles (npts a multiple of 128): target k
+            // of every thread lies in tile k, so "own vesicle" is the same decision for the whole block -- a uniform
+            // skip instead of a per-pair predicate.  One-directional.
+            const int vs_src = first / npts;
+            bool skip[T];
+#pragma unroll
+            for (int k = 0; k < T; ++k) skip[k] = (base + k * kThreads) / npts == vs_src;
+#pragma unroll 2
+            for (int j = 0; j < kTile; ++j) {
+                const double4 sj = ts[j];
+#pragma unroll
+                for (int k = 0; k < T; ++k) {
+                    if (skip[k]) continue;
+                    const double rx = tx[k] - sj.x, ry = ty[k] - sj.y;
+                    const double r2 = fma(rx, rx, ry * ry);
+                    double ml, inv;
+                    log_rcp_f64(r2, tab, ml, inv);
+                    const double qd = fma(rx, sj.z, ry * sj.w) * inv;
+                    Ux[k] = fma(ml, sj.z, fma(qd, rx, Ux[k]));
+                    Uy[k] = fma(ml, sj.w, fma(qd, ry, Uy[k]));
+                }
+            }
         } else if (cnt > 0) {
             // predicated path: own-vesicle sources and the ragged tail are skipped per pair
             int own[T];
