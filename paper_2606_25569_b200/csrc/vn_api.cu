@@ -70,8 +70,8 @@ Split choose_split_for(int n_tb, int n_tiles, int slots, int min_tiles)
 
 // Grid of the symmetric kernels: every super-tile walks a list of about sub*(n_st/2 + 1) source tiles,
 // cut into n_chunks chunks.  The run time is modelled as (waves of resident blocks + 1/2) x (tiles of
-// the longest chunk + 1): the half wave stands for the ragged tail (blocks do not run in lockstep; with
-// only a few blocks per slot the last ones leave SMs idle), the extra tile for the per-block set-up.
+// the longest chunk + 1): the half wave stands for the ragged tail of a multi-wave grid (blocks do not run in
+// lockstep; with only a few blocks per slot the last ones leave SMs idle), the extra tile for the per-block set-up.
 // The chunk count minimising it wins.  Measured on B200: 2000 x 128 fp32 runs 1.5 % faster with 6,500
 // blocks of 39 tiles than with 1,750 blocks of 144 tiles although both fill whole waves.
 SymSplit choose_sym_split(long long P, int super_tile, int slots, int min_tiles)
@@ -87,7 +87,7 @@ SymSplit choose_sym_split(long long P, int super_tile, int slots, int min_tiles)
     auto cost = [&](int c) {
         const long long blocks = (long long)sp.n_st * c;
         const long long waves = (blocks + slots - 1) / slots;
-        return ((double)waves + 0.5) * (double)((list + c - 1) / c + 1);
+        return ((double)waves + (waves > 1 ? 0.5 : 0.0)) * (double)((list + c - 1) / c + 1);   // one wave has no tail
     };
     double best = cost(1);
     sp.n_chunks = 1;
