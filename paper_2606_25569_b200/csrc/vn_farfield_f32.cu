@@ -17,7 +17,7 @@
 // B200): VN_F32_SHARED_RCP=1 lets the two r2 of a packed pair share one reciprocal
 // (t = rcp(KA a b), 1/(KA a) = t b: 9.5 lane-instr + 0.75 SFU) -- 5 % slower here because the FMA pipe,
 // not the SFU, is the bound; VN_F32_MINBLK (resident blocks per SM: 3 = 168 registers, more ILP, beats
-// 4 = 128 registers), VN_F32_BATCH, VN_F32_NP, VN_F32_RSMEM, VN_F32_MINTILES.
+// 4 = 128 registers), VN_F32_BATCH, VN_F32_NP, VN_F32_MINTILES.
 //
 // Cross-block accumulation goes through 64-bit fixed-point atomics (integer addition is associative, so
 // the result is bitwise reproducible whatever the block order); see fixed_scale().
@@ -42,9 +42,6 @@ constexpr int kSub32 = kST32 / kTile;             // source tiles per super-tile
 #endif
 #ifndef VN_F32_SHARED_RCP
 #define VN_F32_SHARED_RCP 0                       // 1: the two r2 of a packed pair share one SFU reciprocal
-#endif
-#ifndef VN_F32_RSMEM
-#define VN_F32_RSMEM 0                            // 1: running sums live in shared memory instead of registers
 #endif
 constexpr int kBatch = VN_F32_BATCH;              // sources per cross-lane reduction batch
 
@@ -169,17 +166,9 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
     const int span_begin = (base / npts) * npts;
     const int span_end = (last_target / npts + 1) * npts;
 
-#if VN_F32_RSMEM
-    __shared__ u64 Rsm[2 * NP][kThreads];
-#define RX(p) Rsm[p][tid]
-#define RY(p) Rsm[NP + (p)][tid]
-#else
     u64 Rx[NP], Ry[NP];   // running sums of  -(ln2/2) A + B  over the tiles of this chunk
-#define RX(p) Rx[p]
-#define RY(p) Ry[p]
-#endif
 #pragma unroll
-    for (int p = 0; p < NP; ++p) RX(p) = RY(p) = 0ull;
+    for (int p = 0; p < NP; ++p) Rx[p] = Ry[p] = 0ull;
     const u64 KA = pk(-0.34657359027997264f, -0.34657359027997264f);   // -(ln 2)/2
 
     for (int i = 0; i < nt; ++i) {
@@ -272,8 +261,8 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
             }
 #pragma unroll
             for (int p = 0; p < NP; ++p) {
-                RX(p) = fma2(KA, Ux[p], RX(p));
-                RY(p) = fma2(KA, Uy[p], RY(p));
+                Rx[p] = fma2(KA, Ux[p], Rx[p]);
+                Ry[p] = fma2(KA, Uy[p], Ry[p]);
             }
         } else if (!both && cnt == kTile && npts % kTile == 0 && base + kST32 <= P) {
             // a tile of the block's OWN super-tile when vesicles are whole tiles (npts a multiple of 128, the
@@ -314,8 +303,8 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
                 upk(Uy[p], y0, y1);
                 if ((base + (2 * p) * kThreads) / npts == vs_src) x0 = y0 = 0.f;
                 if ((base + (2 * p + 1) * kThreads) / npts == vs_src) x1 = y1 = 0.f;
-                RX(p) = fma2(KA, pk(x0, x1), RX(p));
-                RY(p) = fma2(KA, pk(y0, y1), RY(p));
+                Rx[p] = fma2(KA, pk(x0, x1), Rx[p]);
+                Ry[p] = fma2(KA, pk(y0, y1), Ry[p]);
             }
         } else if (cnt > 0) {
             // predicated path: own-vesicle sources and the ragged tail are skipped per pair
@@ -373,8 +362,8 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
             }
 #pragma unroll
             for (int p = 0; p < NP; ++p) {
-                RX(p) = add2(RX(p), pk(ux[2 * p], ux[2 * p + 1]));
-                RY(p) = add2(RY(p), pk(uy[2 * p], uy[2 * p + 1]));
+                Rx[p] = add2(Rx[p], pk(ux[2 * p], ux[2 * p + 1]));
+                Ry[p] = add2(Ry[p], pk(uy[2 * p], uy[2 * p + 1]));
             }
         }
         __syncwarp();
@@ -385,8 +374,8 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
 #pragma unroll
     for (int p = 0; p < NP; ++p) {
         float x0, x1, y0, y1;
-        upk(RX(p), x0, x1);
-        upk(RY(p), y0, y1);
+        upk(Rx[p], x0, x1);
+        upk(Ry[p], y0, y1);
         const int i0 = base + (2 * p) * kThreads + tid;
         const int i1 = i0 + kThreads;
         if (i0 < P) {
