@@ -53,12 +53,12 @@ struct Split {
     int n_chunks;    // source chunks (grid = n_tb * n_chunks)
 };
 
-// Choose the number of source chunks so that the grid fills `slots` resident blocks in whole
-// waves (wave quantisation) while each chunk keeps >= min_tiles tiles.
+// One-directional kernels (free targets): choose the number of source chunks so that the grid fills
+// `slots` resident blocks in whole waves while each chunk keeps >= min_tiles tiles.
 Split choose_split_for(int n_tb, int n_tiles, int slots, int min_tiles);
 
-// Symmetric (both-direction) decomposition of the fp32 kernel: block = (super-tile I, chunk c of I's
-// source-tile list); see vn_farfield_f32.cu.
+// Symmetric (both-direction) decomposition of the pair kernels of both precisions: block = (super-tile I,
+// chunk c of I's source-tile list); see vn_farfield_f32.cu and choose_sym_split() in vn_api.cu.
 struct SymSplit {
     int n_st;        // super-tiles (target blocks)
     int n_tiles;     // source tiles of kTile points
