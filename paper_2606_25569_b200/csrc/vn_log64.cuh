@@ -13,8 +13,8 @@ constexpr int kExpTab = 2048;                 // (1/2) ln2 (E - 1023) for every 
 // no exponent/mantissa surgery on r2 and no integer-to-double conversion (I2F.F64 occupies the FP64 pipe).
 //   t0  = hardware reciprocal seed of r2 (2^-20 accurate, full exponent range)
 //   1/r2 = t0 (1 + d + d^2), d = 1 - r2 t0                                     (one cubic step, 3 DP)
-//   rc  = t0 rounded to 10 mantissa bits = 2^(E-1023) (1 + k/1024);  eps = r2 rc - 1 (one fma; |eps| <= 2^-11 + 2^-19)
-//   -(1/2) ln r2 = (1/2) ln rc - (1/2) log1p(eps),  log1p by its series through eps^4 (next term <= 6e-18), Horner
+//   rc  = t0 truncated to 10 mantissa bits = 2^(E-1023) (1 + k/1024);  eps = r2 rc - 1 (one fma; 0 <= eps < 2^-10)
+//   -(1/2) ln r2 = (1/2) ln rc - (1/2) log1p(eps),  log1p by its series through eps^4 (next term <= 1.8e-16), Horner
 //   (1/2) ln rc = tabE[E] + tab[k]:  tab[k] = (1/2) ln(1 + k/1024), tabE[E] = (1/2) ln2 (E - 1023) for every
 //   exponent field E = 0 .. 2047; both built by every block at start-up (24 KB of shared memory).
 // r2 must be a positive normal double whose reciprocal is normal too (the header's precondition).
@@ -22,7 +22,7 @@ __device__ __forceinline__ void log_rcp_f64(double r2, const double *__restrict_
 {
     double t0;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(t0) : "d"(r2));                // MUFU.RCP64H
-    const int rch = (__double2hiint(t0) + 0x200) & 0xfffffc00;              // round to 10 mantissa bits
+    const int rch = __double2hiint(t0) & 0xfffffc00;                        // truncate to 10 mantissa bits
     const double rc = __hiloint2double(rch, 0);
     const int k = (rch >> 10) & 0x3ff;
     const double base = tab[kLogTab + (rch >> 20)] + tab[k];
