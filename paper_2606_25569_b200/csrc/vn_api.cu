@@ -250,6 +250,7 @@ vn_status vn_farfield_fmm(const void *X, const void *F, const void *W, int64_t n
                           vn_precision precision, void *stream)
 {
     if (misaligned(near_ptr, 8) || misaligned(near_ves, 4)) return VN_ERR_INVALID_ARG;
+    if (order == 0) order = precision == VN_F32 ? 12 : 38;      // the orders that meet 2e-5 / 1e-12
     if (!X || !F || !W || !U) return VN_ERR_INVALID_ARG;
     if (check_shape(nves, npts, precision) != VN_OK) return VN_ERR_INVALID_ARG;
     if (!isfinite(mu) || !(mu > 0.0) || order < 2 || order > 48) return VN_ERR_INVALID_ARG;
@@ -268,6 +269,7 @@ vn_status vn_farfield_targets_fmm(const void *Xt, int64_t nt, const void *X, con
 {
     if (!X || !F || !W) return VN_ERR_INVALID_ARG;
     if (check_shape(nves, npts, precision) != VN_OK) return VN_ERR_INVALID_ARG;
+    if (order == 0) order = precision == VN_F32 ? 12 : 38;
     if (nt < 0 || nt >= (1ll << 31) || order < 2 || order > 48) return VN_ERR_INVALID_ARG;
     if (!isfinite(mu) || !(mu > 0.0)) return VN_ERR_INVALID_ARG;
     if (nt == 0) return VN_OK;

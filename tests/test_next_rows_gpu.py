@@ -585,3 +585,13 @@ def test_fmm_four_million_points():
     err = rel_l2(got.cpu().numpy().reshape(-1, 2)[idx], ref)
     print(f"fmm 32000 x 128 (4.1 M points) float32 p=12: sampled rel-L2 {err:.3e}, {e0.elapsed_time(e1) / 3:.2f} ms per evaluation")
     assert err <= TOL[np.float32]
+
+
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+def test_fmm_default_order_meets_the_tolerance(dtype):
+    s = inputs.config(1)
+    W = oracle.weights(s.X)
+    ref = oracle.farfield(stored(s.X, dtype), stored(s.F, dtype), stored(W, dtype), s.mu)
+    got = vn.vn_farfield_fmm(dev(s.X, dtype), dev(s.F, dtype), dev(W, dtype), s.mu, 0)     # order 0 = default for the precision
+    torch.cuda.synchronize()
+    assert rel_l2(got.cpu().numpy(), ref) <= TOL[dtype]
