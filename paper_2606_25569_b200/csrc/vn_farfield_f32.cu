@@ -38,7 +38,7 @@ constexpr int kSub32 = kST32 / kTile;             // source tiles per super-tile
 #define VN_F32_MINBLK 3
 #endif
 #ifndef VN_F32_MINTILES
-#define VN_F32_MINTILES 4
+#define VN_F32_MINTILES 1
 #endif
 #ifndef VN_F32_SHARED_RCP
 #define VN_F32_SHARED_RCP 0                       // 1: the two r2 of a packed pair share one SFU reciprocal

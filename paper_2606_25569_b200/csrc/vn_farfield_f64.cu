@@ -31,7 +31,7 @@ constexpr int kSub64 = kST64 / kTile;         // source tiles per super-tile: 4
 #define VN_F64_MINBLK 3
 #endif
 #ifndef VN_F64_MINTILES
-#define VN_F64_MINTILES 8
+#define VN_F64_MINTILES 1
 #endif
 constexpr int kBatch64 = VN_F64_BATCH;        // sources per cross-lane reduction batch
 
