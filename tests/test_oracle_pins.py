@@ -522,3 +522,28 @@ def test_redistribute_equivariances():
     d1 = np.abs(Y - X).max()
     d2 = np.abs(oracle.redistribute(Y) - Y).max()
     assert d2 < 2e-2 * d1
+
+
+# ----------------------------------------------------------------------------- complex form (the identity behind row f-4b)
+def test_complex_potential_form_of_the_stokeslet_sum():
+    """With z = x + i y, g = gx + i gy:  sum_j K(z - zeta_j) g_j = -(Re Phi1 + i Re Phi2) + (z/2) conj(Phi1' + i Phi2')
+    - (1/2) conj(psi),  Phi_m = sum g_{m,j} log(z - zeta_j),  psi = sum [conj(zeta_j) g_j / (z - zeta_j) - conj(g_j)].
+    An independent statement of the same sum (two logarithmic potentials and a Cauchy sum, evaluated by brute force
+    with numpy's complex arithmetic): it pins the oracle once more and is the identity vn_farfield_fmm expands."""
+    rng = np.random.default_rng(42)
+    nves, N = 5, 12
+    X = rng.normal(size=(nves, N, 2)) * 0.4 + 3.0 * rng.normal(size=(nves, 1, 2))
+    F = rng.normal(size=(nves, N, 2))
+    W = rng.uniform(0.5, 1.5, size=(nves, N))
+    xt = rng.normal(size=(9, 2)) * 4.0 + np.array([15.0, -2.0])
+    zeta = (X[..., 0] + 1j * X[..., 1]).ravel()
+    g = ((F[..., 0] + 1j * F[..., 1]) * W).ravel()
+    z = xt[:, 0] + 1j * xt[:, 1]
+    dz = z[:, None] - zeta[None, :]
+    Phi1 = (g.real[None, :] * np.log(dz)).sum(1)
+    Phi2 = (g.imag[None, :] * np.log(dz)).sum(1)
+    dPhi = ((g.real + 1j * g.imag)[None, :] / dz).sum(1)                 # Phi1' + i Phi2'
+    psi = (np.conj(zeta)[None, :] * g[None, :] / dz - np.conj(g)[None, :]).sum(1)
+    u = -(Phi1.real + 1j * Phi2.real) + 0.5 * z * np.conj(dPhi) - 0.5 * np.conj(psi)
+    ref = oracle.farfield_targets(X, F, W, xt, mu=1.0) * 4 * np.pi
+    assert np.abs(u - (ref[:, 0] + 1j * ref[:, 1])).max() <= 1e-13
