@@ -1,4 +1,5 @@
-"""Parity of the NEXT rows (DESIGN.md f-1 near-field mask variant, f-4 free targets) with the oracle
+"""Parity of the NEXT rows (DESIGN.md f-1 near-field mask variant, f-2 elastic force, f-3 redistribution, f-4 free
+targets, f-4b fast multipole evaluation) with the oracle
 (run on the B200 box: pytest -m gpu).  Every call goes through the C-ABI library via the binding.
 
 Index work (the near relation) must match the oracle exactly; the decision d^2 <= h^2 is taken in
