@@ -69,30 +69,36 @@ Split choose_split_for(int n_tb, int n_tiles, int slots, int min_tiles)
 }
 
 // Grid of the symmetric kernels: every super-tile walks a list of about sub*(n_st/2 + 1) source tiles,
-// cut into n_chunks chunks.  The run time is modelled as (waves of resident blocks + 1/2) x (tiles of
-// the longest chunk + 1): the half wave stands for the ragged tail of a multi-wave grid (blocks do not run in
-// lockstep; with only a few blocks per slot the last ones leave SMs idle), the extra tile for the per-block set-up.
-// The chunk count minimising it wins.  Measured on B200: 2000 x 128 fp32 runs 1.5 % faster with 6,500
-// blocks of 39 tiles than with 1,750 blocks of 144 tiles although both fill whole waves.
-SymSplit choose_sym_split(long long P, int super_tile, int slots, int min_tiles)
+// cut into n_chunks chunks of t = list/n_chunks tiles.  With W = n_st*list/slots tiles of work per resident-block
+// slot, the run time measured on B200 follows  W (1 + o/t) + b t  tile-times: o = 0.03 tile-times of set-up and
+// flush per block, b = 0.25 for the ragged end of a grid whose blocks do not run in lockstep (the hardware hands
+// out blocks as slots free up, so a multi-wave grid has no wave quantisation worth modelling).  The minimum is at
+// t = sqrt(W o / b) = sqrt(0.12 W): 1 tile per block at 256 x 128 points, 8 at 2000 x 128, 33 at 8000 x 128.
+// Measured, fp32: 256 x 128 0.41 ms with 1-tile blocks against 0.47 ms with 416 blocks of 10 tiles;
+// 1000 x 128 5.66 ms (6 tiles) against 5.72 (13).  max_tiles > 0 caps t (fp64 kernel: its stage refill waits for
+// the slowest warp, which costs about half a tile-time per block once a block has more tiles than stages).
+SymSplit choose_sym_split(long long P, int super_tile, int slots, int min_tiles, int max_tiles)
 {
     SymSplit sp;
     sp.n_st = (int)((P + super_tile - 1) / super_tile);
     sp.n_tiles = (int)((P + kTile - 1) / kTile);
     const int sub = super_tile / kTile;
     const long long list = (long long)sub * (sp.n_st / 2 + 1);     // longest list over the super-tiles
-    long long max_chunks = list / min_tiles;
-    if (max_chunks < 1) max_chunks = 1;
-    if (max_chunks > 256) max_chunks = 256;
-    auto cost = [&](int c) {
-        const long long blocks = (long long)sp.n_st * c;
-        const long long waves = (blocks + slots - 1) / slots;
-        return ((double)waves + (waves > 1 ? 0.5 : 0.0)) * (double)((list + c - 1) / c + 1);   // one wave has no tail
-    };
-    double best = cost(1);
-    sp.n_chunks = 1;
-    for (int c = 2; c <= (int)max_chunks; ++c)
-        if (cost(c) < best * (1.0 - 1e-9)) { best = cost(c); sp.n_chunks = c; }
+    const double W = (double)sp.n_st * (double)list / (double)(slots > 0 ? slots : 1);
+    long long t = (long long)(sqrt(0.12 * W) + 0.5);
+    if (t < min_tiles) t = min_tiles;
+    if (t < 1) t = 1;
+    if (max_tiles > 0 && t > max_tiles) t = max_tiles;
+    if (t > list) t = list;
+    long long c = (list + t - 1) / t;
+    // keep the grid below 2^31 - 1 blocks
+    const long long cmax = 2147483647ll / (sp.n_st > 0 ? sp.n_st : 1);
+    if (c > cmax) c = cmax;
+    if (c < 1) c = 1;
+    sp.n_chunks = (int)c;
+#ifdef VN_SYM_FORCE_CHUNKS
+    sp.n_chunks = VN_SYM_FORCE_CHUNKS;    // tuning builds only
+#endif
     return sp;
 }
 

@@ -64,7 +64,7 @@ struct SymSplit {
     int n_tiles;     // source tiles of kTile points
     int n_chunks;    // chunks of the per-super-tile list (grid = n_st * n_chunks)
 };
-SymSplit choose_sym_split(long long P, int super_tile, int slots, int min_tiles);
+SymSplit choose_sym_split(long long P, int super_tile, int slots, int min_tiles, int max_tiles);
 
 // exclusive scan of int counts into 64-bit offsets (kernels in vn_near.cu, also used by vn_fmm.cu)
 constexpr int kScanThreads = 256;
@@ -116,6 +116,21 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
                      smem_u32(dst)),
                  "l"(src), "r"(bytes), "r"(smem_u32(bar))
                  : "memory");
+}
+
+// Stage hand-back of the tile ring without anybody waiting: every warp counts itself out of stage s when it
+// has read the tile; the warp that makes the count a multiple of the block's warp count was the last one out
+// and refills the stage itself.  (A warp cannot run a whole ring ahead -- the refill it would need is only
+// issued once all warps have left -- so the count identifies the last warp exactly.)  The fences order the
+// warps' shared-memory reads before the bulk copy that overwrites the stage (generic -> async proxy).
+__device__ __forceinline__ bool stage_last_out(int *drained, int warps)   // call from one lane per warp
+{
+    __threadfence_block();
+    const int left = atomicAdd(drained, 1) + 1;
+    if (left % warps != 0) return false;
+    __threadfence_block();
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    return true;
 }
 
 // ---------------------------------------------------------------------------------------------

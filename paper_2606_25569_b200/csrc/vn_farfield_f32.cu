@@ -92,7 +92,7 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
     constexpr int T = 2 * NP;
     __shared__ __align__(128) ulonglong2 tile[kStages][kTile * 2];
     __shared__ __align__(8) u64 full_bar[kStages];
-    __shared__ __align__(8) u64 empty_bar[kStages];
+    __shared__ int drained[kStages];                 // warps that have left each stage (stage_last_out)
 
     const int tid = threadIdx.x;
     const int lane = tid & 31;
@@ -115,7 +115,7 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
 #pragma unroll
         for (int s = 0; s < kStages; ++s) {
             mbar_init(&full_bar[s], 1);
-            mbar_init(&empty_bar[s], kThreads / 32);
+            drained[s] = 0;
         }
         mbar_fence_init();
     }
@@ -173,10 +173,6 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
 
     for (int i = 0; i < nt; ++i) {
         const int s = i % kStages;
-        if (tid == 0 && i >= 1 && i - 1 + kStages < nt) {   // refill the stage drained last iteration
-            mbar_wait(&empty_bar[(i - 1) % kStages], ((i - 1) / kStages) & 1);
-            issue(i - 1 + kStages);
-        }
         mbar_wait(&full_bar[s], (i / kStages) & 1);
 
         const int u = u_begin + i;
@@ -367,7 +363,8 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
             }
         }
         __syncwarp();
-        if (lane == 0) mbar_arrive(&empty_bar[s]);
+        if (lane == 0 && stage_last_out(&drained[s], kThreads / 32) && i + kStages < nt)
+            issue(i + kStages);                      // the last warp out of the stage refills it
     }
 
     // this block's one-directional sums for its own targets
@@ -419,7 +416,7 @@ vn_status farfield_f32(const void *X, const void *F, const void *W, int64_t nves
         VN_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, farfield_f32_kernel<kNP32>, kThreads, 0));
         slots = sms * (occ > 0 ? occ : 1);
     }
-    const SymSplit sp = choose_sym_split(P, kST32, slots, VN_F32_MINTILES);
+    const SymSplit sp = choose_sym_split(P, kST32, slots, VN_F32_MINTILES, 0);
 
     // scratch: packed sources | fixed-point accumulators | gmax
     const size_t b_src = (size_t)P * 32, b_acc = (size_t)P * 16;
@@ -617,7 +614,7 @@ void plan_f32(long long P, int slots, int *super_tile, int *sub, SymSplit *sp)
 {
     *super_tile = kST32;
     *sub = kSub32;
-    *sp = choose_sym_split(P, kST32, slots, VN_F32_MINTILES);
+    *sp = choose_sym_split(P, kST32, slots, VN_F32_MINTILES, 0);
 }
 
 }  // namespace vn

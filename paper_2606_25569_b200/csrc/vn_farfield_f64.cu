@@ -311,7 +311,7 @@ vn_status farfield_f64(const void *X, const void *F, const void *W, int64_t nves
         VN_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, farfield_f64_kernel, kThreads, 0));
         slots = sms * (occ > 0 ? occ : 1);
     }
-    const SymSplit sp = choose_sym_split(P, kST64, slots, VN_F64_MINTILES);
+    const SymSplit sp = choose_sym_split(P, kST64, slots, VN_F64_MINTILES, kStages);
 
     // scratch: packed sources | fixed-point accumulators (hi, lo per component) | gmax
     const size_t b_src = (size_t)P * 32, b_acc = (size_t)P * 32;
@@ -472,7 +472,7 @@ void plan_f64(long long P, int slots, int *super_tile, int *sub, SymSplit *sp)
 {
     *super_tile = kST64;
     *sub = kSub64;
-    *sp = choose_sym_split(P, kST64, slots, VN_F64_MINTILES);
+    *sp = choose_sym_split(P, kST64, slots, VN_F64_MINTILES, kStages);
 }
 
 }  // namespace vn
