@@ -451,6 +451,9 @@ vn_status farfield_f32(const void *X, const void *F, const void *W, int64_t nves
 //   r = x - y; r2 = rx*rx + ry*ry; A += lg2(r2) * g; d = rx*gx + ry*gy; B += (d / r2) * r
 // (2 FADD + 3 FMUL + 6 FFMA + 1.5 MUFU with the shared reciprocal), 8 targets per thread as packed
 // pairs, the same tile ring, per-tile partial sums folded into running sums, fixed-point atomics out.
+#ifndef VN_TGT_LASTOUT
+#define VN_TGT_LASTOUT 0           // 1: stage hand-back by the last warp out (as in the pair kernel)
+#endif
 #ifndef VN_F32_TGT_MINBLK
 #define VN_F32_TGT_MINBLK 4
 #endif
@@ -462,7 +465,11 @@ targets_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict_
     constexpr int T = 2 * NP;
     __shared__ __align__(128) ulonglong2 tile[kStages][kTile * 2];
     __shared__ __align__(8) u64 full_bar[kStages];
+#if VN_TGT_LASTOUT
+    __shared__ int drained[kStages];                 // warps that have left each stage (stage_last_out)
+#else
     __shared__ __align__(8) u64 empty_bar[kStages];
+#endif
 
     const int tid = threadIdx.x;
     const int tb = blockIdx.x / n_chunks;
@@ -474,7 +481,11 @@ targets_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict_
 #pragma unroll
         for (int s = 0; s < kStages; ++s) {
             mbar_init(&full_bar[s], 1);
+#if VN_TGT_LASTOUT
+            drained[s] = 0;
+#else
             mbar_init(&empty_bar[s], kThreads / 32);
+#endif
         }
         mbar_fence_init();
     }
@@ -506,10 +517,12 @@ targets_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict_
 
     for (int i = 0; i < nt; ++i) {
         const int s = i % kStages;
+#if !VN_TGT_LASTOUT
         if (tid == 0 && i >= 1 && i - 1 + kStages < nt) {
             mbar_wait(&empty_bar[(i - 1) % kStages], ((i - 1) / kStages) & 1);
             issue(i - 1 + kStages);
         }
+#endif
         mbar_wait(&full_bar[s], (i / kStages) & 1);
 
         const int cnt = min(kTile, P - (t_begin + i) * kTile);
@@ -551,7 +564,12 @@ targets_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict_
             Ry[p] = add2(Ry[p], fma2(KA, Ay[p], By[p]));
         }
         __syncwarp();
+#if VN_TGT_LASTOUT
+        if ((tid & 31) == 0 && stage_last_out(&drained[s], kThreads / 32) && i + kStages < nt)
+            issue(i + kStages);                      // the last warp out of the stage refills it
+#else
         if ((tid & 31) == 0) mbar_arrive(&empty_bar[s]);
+#endif
     }
 
     const double scale = fixed_scale(*gmax_bits, P);

@@ -30,6 +30,15 @@ constexpr int kSub64 = kST64 / kTile;         // source tiles per super-tile: 4
 #ifndef VN_F64_MINBLK
 #define VN_F64_MINBLK 3
 #endif
+#ifndef VN_F64_LASTOUT
+#define VN_F64_LASTOUT 0          // 1: stage hand-back by the last warp out (as in the fp32 kernel)
+#endif
+#ifndef VN_F64_MAXTILES
+#define VN_F64_MAXTILES kStages   // cap of the chunk length (0: none)
+#endif
+#ifndef VN_TGT_LASTOUT
+#define VN_TGT_LASTOUT 0           // 1: free-target kernel hands stages back by the last warp out
+#endif
 #ifndef VN_F64_MINTILES
 #define VN_F64_MINTILES 1
 #endif
@@ -73,7 +82,11 @@ farfield_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__
     constexpr int kDup = 32 / (2 * B);              // lanes that end up with the same reduced value
     __shared__ __align__(128) double4 tile[kStages][kTile];
     __shared__ __align__(8) u64 full_bar[kStages];
+#if VN_F64_LASTOUT
+    __shared__ int drained[kStages];                 // warps that have left each stage (stage_last_out)
+#else
     __shared__ __align__(8) u64 empty_bar[kStages];
+#endif
     __shared__ double tab[kLogTab + kExpTab];
 
     const int tid = threadIdx.x;
@@ -97,7 +110,11 @@ farfield_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__
 #pragma unroll
         for (int s = 0; s < kStages; ++s) {
             mbar_init(&full_bar[s], 1);
+#if VN_F64_LASTOUT
+            drained[s] = 0;
+#else
             mbar_init(&empty_bar[s], kThreads / 32);
+#endif
         }
         mbar_fence_init();
     }
@@ -143,10 +160,12 @@ farfield_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__
 
     for (int i = 0; i < nt; ++i) {
         const int s = i % kStages;
+#if !VN_F64_LASTOUT
         if (tid == 0 && i >= 1 && i - 1 + kStages < nt) {   // refill the stage drained last iteration
             mbar_wait(&empty_bar[(i - 1) % kStages], ((i - 1) / kStages) & 1);
             issue(i - 1 + kStages);
         }
+#endif
         mbar_wait(&full_bar[s], (i / kStages) & 1);
 
         const int u = u_begin + i;
@@ -267,7 +286,12 @@ farfield_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__
             }
         }
         __syncwarp();
+#if VN_F64_LASTOUT
+        if (lane == 0 && stage_last_out(&drained[s], kThreads / 32) && i + kStages < nt)
+            issue(i + kStages);                      // the last warp out of the stage refills it
+#else
         if (lane == 0) mbar_arrive(&empty_bar[s]);
+#endif
     }
 
     // this block's sums for its own targets
@@ -311,7 +335,7 @@ vn_status farfield_f64(const void *X, const void *F, const void *W, int64_t nves
         VN_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, farfield_f64_kernel, kThreads, 0));
         slots = sms * (occ > 0 ? occ : 1);
     }
-    const SymSplit sp = choose_sym_split(P, kST64, slots, VN_F64_MINTILES, kStages);
+    const SymSplit sp = choose_sym_split(P, kST64, slots, VN_F64_MINTILES, VN_F64_MAXTILES);
 
     // scratch: packed sources | fixed-point accumulators (hi, lo per component) | gmax
     const size_t b_src = (size_t)P * 32, b_acc = (size_t)P * 32;
@@ -352,7 +376,11 @@ targets_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__ 
     constexpr int T = kT64;
     __shared__ __align__(128) double4 tile[kStages][kTile];
     __shared__ __align__(8) u64 full_bar[kStages];
+#if VN_TGT_LASTOUT
+    __shared__ int drained[kStages];                 // warps that have left each stage (stage_last_out)
+#else
     __shared__ __align__(8) u64 empty_bar[kStages];
+#endif
     __shared__ double tab[kLogTab + kExpTab];
 
     const int tid = threadIdx.x;
@@ -365,7 +393,11 @@ targets_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__ 
 #pragma unroll
         for (int s = 0; s < kStages; ++s) {
             mbar_init(&full_bar[s], 1);
+#if VN_TGT_LASTOUT
+            drained[s] = 0;
+#else
             mbar_init(&empty_bar[s], kThreads / 32);
+#endif
         }
         mbar_fence_init();
     }
@@ -396,10 +428,12 @@ targets_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__ 
 
     for (int i = 0; i < nt; ++i) {
         const int s = i % kStages;
+#if !VN_TGT_LASTOUT
         if (tid == 0 && i >= 1 && i - 1 + kStages < nt) {
             mbar_wait(&empty_bar[(i - 1) % kStages], ((i - 1) / kStages) & 1);
             issue(i - 1 + kStages);
         }
+#endif
         mbar_wait(&full_bar[s], (i / kStages) & 1);
         const int cnt = min(kTile, P - (t_begin + i) * kTile);
         const double4 *ts = tile[s];
@@ -418,7 +452,12 @@ targets_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__ 
             }
         }
         __syncwarp();
+#if VN_TGT_LASTOUT
+        if ((tid & 31) == 0 && stage_last_out(&drained[s], kThreads / 32) && i + kStages < nt)
+            issue(i + kStages);                      // the last warp out of the stage refills it
+#else
         if ((tid & 31) == 0) mbar_arrive(&empty_bar[s]);
+#endif
     }
 
     const Fixed2 fx = fixed2_scale(*gmax_bits, P);
@@ -472,7 +511,7 @@ void plan_f64(long long P, int slots, int *super_tile, int *sub, SymSplit *sp)
 {
     *super_tile = kST64;
     *sub = kSub64;
-    *sp = choose_sym_split(P, kST64, slots, VN_F64_MINTILES, kStages);
+    *sp = choose_sym_split(P, kST64, slots, VN_F64_MINTILES, VN_F64_MAXTILES);
 }
 
 }  // namespace vn
