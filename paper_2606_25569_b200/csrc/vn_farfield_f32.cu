@@ -451,11 +451,11 @@ vn_status farfield_f32(const void *X, const void *F, const void *W, int64_t nves
 //   r = x - y; r2 = rx*rx + ry*ry; A += lg2(r2) * g; d = rx*gx + ry*gy; B += (d / r2) * r
 // (2 FADD + 3 FMUL + 6 FFMA + 1.5 MUFU with the shared reciprocal), 8 targets per thread as packed
 // pairs, the same tile ring, per-tile partial sums folded into running sums, fixed-point atomics out.
-#ifndef VN_TGT_LASTOUT
-#define VN_TGT_LASTOUT 0           // 1: stage hand-back by the last warp out (as in the pair kernel)
-#endif
+#ifndef VN_TGT32_LASTOUT
+#define VN_TGT32_LASTOUT 0         // 1: stage hand-back by the last warp out as in the pair kernel; measured
+#endif                             // 2008 against 2178 GInt/s at 2000 x 128 sources, 512 x 512 targets: off
 #ifndef VN_F32_TGT_MINBLK
-#define VN_F32_TGT_MINBLK 4
+#define VN_F32_TGT_MINBLK 3       // measured at 2000 x 128 sources, 512 x 512 targets: 2245 GInt/s against 2229 with 4
 #endif
 template <int NP>
 __global__ void __launch_bounds__(kThreads, VN_F32_TGT_MINBLK)
@@ -465,7 +465,7 @@ targets_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict_
     constexpr int T = 2 * NP;
     __shared__ __align__(128) ulonglong2 tile[kStages][kTile * 2];
     __shared__ __align__(8) u64 full_bar[kStages];
-#if VN_TGT_LASTOUT
+#if VN_TGT32_LASTOUT
     __shared__ int drained[kStages];                 // warps that have left each stage (stage_last_out)
 #else
     __shared__ __align__(8) u64 empty_bar[kStages];
@@ -481,7 +481,7 @@ targets_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict_
 #pragma unroll
         for (int s = 0; s < kStages; ++s) {
             mbar_init(&full_bar[s], 1);
-#if VN_TGT_LASTOUT
+#if VN_TGT32_LASTOUT
             drained[s] = 0;
 #else
             mbar_init(&empty_bar[s], kThreads / 32);
@@ -517,7 +517,7 @@ targets_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict_
 
     for (int i = 0; i < nt; ++i) {
         const int s = i % kStages;
-#if !VN_TGT_LASTOUT
+#if !VN_TGT32_LASTOUT
         if (tid == 0 && i >= 1 && i - 1 + kStages < nt) {
             mbar_wait(&empty_bar[(i - 1) % kStages], ((i - 1) / kStages) & 1);
             issue(i - 1 + kStages);
@@ -541,7 +541,8 @@ targets_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict_
                 float a, b;
                 upk(r2, a, b);
                 const float t = sfu_rcp(a * b);
-                const u64 inv = pk(t * b, t * a);
+                const u64 inv = mul2(pk(t, t), pk(b, a));   // (1/a, 1/b): one packed multiply on the swapped pair
+                                                            // (the swap is register allocation, no instruction)
                 const u64 l = pk(sfu_lg2(a), sfu_lg2(b));
                 Ax[p] = fma2(l, gg.x, Ax[p]);
                 Ay[p] = fma2(l, gg.y, Ay[p]);
@@ -564,7 +565,7 @@ targets_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict_
             Ry[p] = add2(Ry[p], fma2(KA, Ay[p], By[p]));
         }
         __syncwarp();
-#if VN_TGT_LASTOUT
+#if VN_TGT32_LASTOUT
         if ((tid & 31) == 0 && stage_last_out(&drained[s], kThreads / 32) && i + kStages < nt)
             issue(i + kStages);                      // the last warp out of the stage refills it
 #else

@@ -31,14 +31,15 @@ constexpr int kSub64 = kST64 / kTile;         // source tiles per super-tile: 4
 #define VN_F64_MINBLK 3
 #endif
 #ifndef VN_F64_LASTOUT
-#define VN_F64_LASTOUT 0          // 1: stage hand-back by the last warp out (as in the fp32 kernel)
+#define VN_F64_LASTOUT 0          // 1: stage hand-back by the last warp out (as in the fp32 kernel); costs 28 bytes of
+                                  // spills at 3 blocks/SM and measured 965 against 1000 GInt/s at 2000 x 128: off
 #endif
 #ifndef VN_F64_MAXTILES
 #define VN_F64_MAXTILES kStages   // cap of the chunk length (0: none)
 #endif
-#ifndef VN_TGT_LASTOUT
-#define VN_TGT_LASTOUT 0           // 1: free-target kernel hands stages back by the last warp out
-#endif
+#ifndef VN_TGT64_LASTOUT
+#define VN_TGT64_LASTOUT 1         // free-target kernel: the last warp out of a ring stage refills it (stage_last_out);
+#endif                             // measured 719 against 696 GInt/s at 2000 x 128 sources, 512 x 512 targets
 #ifndef VN_F64_MINTILES
 #define VN_F64_MINTILES 1
 #endif
@@ -376,7 +377,7 @@ targets_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__ 
     constexpr int T = kT64;
     __shared__ __align__(128) double4 tile[kStages][kTile];
     __shared__ __align__(8) u64 full_bar[kStages];
-#if VN_TGT_LASTOUT
+#if VN_TGT64_LASTOUT
     __shared__ int drained[kStages];                 // warps that have left each stage (stage_last_out)
 #else
     __shared__ __align__(8) u64 empty_bar[kStages];
@@ -393,7 +394,7 @@ targets_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__ 
 #pragma unroll
         for (int s = 0; s < kStages; ++s) {
             mbar_init(&full_bar[s], 1);
-#if VN_TGT_LASTOUT
+#if VN_TGT64_LASTOUT
             drained[s] = 0;
 #else
             mbar_init(&empty_bar[s], kThreads / 32);
@@ -428,7 +429,7 @@ targets_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__ 
 
     for (int i = 0; i < nt; ++i) {
         const int s = i % kStages;
-#if !VN_TGT_LASTOUT
+#if !VN_TGT64_LASTOUT
         if (tid == 0 && i >= 1 && i - 1 + kStages < nt) {
             mbar_wait(&empty_bar[(i - 1) % kStages], ((i - 1) / kStages) & 1);
             issue(i - 1 + kStages);
@@ -452,7 +453,7 @@ targets_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__ 
             }
         }
         __syncwarp();
-#if VN_TGT_LASTOUT
+#if VN_TGT64_LASTOUT
         if ((tid & 31) == 0 && stage_last_out(&drained[s], kThreads / 32) && i + kStages < nt)
             issue(i + kStages);                      // the last warp out of the stage refills it
 #else
