@@ -30,6 +30,9 @@ constexpr int kSub64 = kST64 / kTile;         // source tiles per super-tile: 4
 #ifndef VN_F64_MINBLK
 #define VN_F64_MINBLK 3
 #endif
+#ifndef VN_F64_GTAB
+#define VN_F64_GTAB 0             // 1: the pair kernel's blocks copy the log tables from scratch (built once per call by
+#endif                            // pack_sources_f64 with the same code) instead of building them
 #ifndef VN_F64_LASTOUT
 #define VN_F64_LASTOUT 0          // 1: stage hand-back by the last warp out (as in the fp32 kernel); costs 28 bytes of
                                   // spills at 3 blocks/SM and measured 965 against 1000 GInt/s at 2000 x 128: off
@@ -49,9 +52,10 @@ constexpr int kBatch64 = VN_F64_BATCH;        // sources per cross-lane reductio
 // (the bit pattern of a non-negative double orders like the double).
 __global__ void pack_sources_f64(const double2 *__restrict__ X, const double2 *__restrict__ F,
                                  const double *__restrict__ W, int P, double4 *__restrict__ src,
-                                 unsigned long long *__restrict__ gmax_bits)
+                                 unsigned long long *__restrict__ gmax_bits, double *__restrict__ gtab)
 {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (gtab) build_log_tables(gtab, s, gridDim.x * blockDim.x);   // once per call, for the pair kernel's blocks
     double m = 0.0;
     if (s < P) {
         const double2 y = X[s];
@@ -76,7 +80,7 @@ __global__ void pack_sources_f64(const double2 *__restrict__ X, const double2 *_
 __global__ void __launch_bounds__(kThreads, VN_F64_MINBLK)
 farfield_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__ X, int P, int npts,
                     int n_tiles, int n_st, int n_chunks, const unsigned long long *__restrict__ gmax_bits,
-                    long long *__restrict__ acc)
+                    long long *__restrict__ acc, const double2 *__restrict__ gtab)
 {
     constexpr int T = kT64;
     constexpr int B = kBatch64;
@@ -119,7 +123,14 @@ farfield_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__
         }
         mbar_fence_init();
     }
+#if VN_F64_GTAB
+    static_assert((kLogTab + kExpTab) % (2 * kThreads) == 0, "table copy assumes whole rounds");
+#pragma unroll
+    for (int k = 0; k < (kLogTab + kExpTab) / (2 * kThreads); ++k)
+        reinterpret_cast<double2 *>(tab)[k * kThreads + tid] = __ldg(gtab + k * kThreads + tid);
+#else
     build_log_tables(tab, tid, kThreads);
+#endif
     __syncthreads();
 
     auto issue = [&](int i) {   // one thread: list entry u_begin + i -> stage i % kStages
@@ -341,16 +352,18 @@ vn_status farfield_f64(const void *X, const void *F, const void *W, int64_t nves
     // scratch: packed sources | fixed-point accumulators (hi, lo per component) | gmax
     const size_t b_src = (size_t)P * 32, b_acc = (size_t)P * 32;
     char *scratch = nullptr;
-    VN_CUDA(cudaMallocAsync((void **)&scratch, b_src + b_acc + 16, st));
+    const size_t b_tab = VN_F64_GTAB ? (size_t)(kLogTab + kExpTab) * sizeof(double) : 0;
+    VN_CUDA(cudaMallocAsync((void **)&scratch, b_src + b_acc + 16 + b_tab, st));
     double4 *src = (double4 *)scratch;
     long long *acc = (long long *)(scratch + b_src);
     unsigned long long *gmax = (unsigned long long *)(scratch + b_src + b_acc);
+    double *gtab = VN_F64_GTAB ? (double *)(scratch + b_src + b_acc + 16) : nullptr;   // 16-byte aligned
     VN_CUDA(cudaMemsetAsync(acc, 0, b_acc + 16, st));
 
-    pack_sources_f64<<<(P + 255) / 256, 256, 0, st>>>((const double2 *)X, (const double2 *)F, (const double *)W, P, src, gmax);
+    pack_sources_f64<<<(P + 255) / 256, 256, 0, st>>>((const double2 *)X, (const double2 *)F, (const double *)W, P, src, gmax, gtab);
     profile_mark(st, true);
     farfield_f64_kernel<<<sp.n_st * sp.n_chunks, kThreads, 0, st>>>(src, (const double2 *)X, P, (int)npts, sp.n_tiles,
-                                                                   sp.n_st, sp.n_chunks, gmax, acc);
+                                                                   sp.n_st, sp.n_chunks, gmax, acc, (const double2 *)gtab);
     profile_mark(st, false);
     if (near_ptr) {   // row f-1: take the near vesicles' contributions out again before the final rounding
         const vn_status rc = near_correction_f64(X, F, W, P, (int)npts, near_ptr, near_ves, acc, gmax, st);
@@ -495,7 +508,7 @@ vn_status farfield_targets_f64(const void *Xt, int64_t nt, const void *X, const 
     unsigned long long *gmax = (unsigned long long *)(scratch + b_src + b_acc);
     VN_CUDA(cudaMemsetAsync(acc, 0, b_acc + 16, st));
 
-    pack_sources_f64<<<(P + 255) / 256, 256, 0, st>>>((const double2 *)X, (const double2 *)F, (const double *)W, P, src, gmax);
+    pack_sources_f64<<<(P + 255) / 256, 256, 0, st>>>((const double2 *)X, (const double2 *)F, (const double *)W, P, src, gmax, nullptr);
     profile_mark(st, true);
     targets_f64_kernel<<<sp.n_tb * sp.n_chunks, kThreads, 0, st>>>(src, (const double2 *)Xt, n, P, sp.n_tiles,
                                                                   sp.n_chunks, gmax, acc);
