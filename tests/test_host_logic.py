@@ -60,3 +60,23 @@ def test_plan_fills_the_device_in_waves():
         if nves >= 2000:
             assert blocks >= 8 * slots
     assert vn.lib().vn_plan_farfield(0, 4, vn.VN_F32, slots, None) == vn.VN_ERR_INVALID_ARG
+
+
+def test_chunk_length_follows_the_measured_model():
+    """choose_sym_split: chunks of t = sqrt(0.12 W) tiles, W = tiles of work per resident-block
+    slot; the fp64 kernel caps t at the ring depth (4 stages)."""
+    slots = 148 * 3
+
+    def tiles_per_chunk(nves, prec):
+        p = vn.vn_plan_farfield(nves, 128, prec, slots)
+        n_st = p["n_super_tiles"]
+        longest = p["tiles_per_super_tile"] * ((n_st - 1) // 2 + (1 if n_st % 2 == 0 else 0) + 1)
+        W = n_st * longest / slots
+        return -(-longest // p["n_chunks"]), W
+
+    for nves in (256, 1000, 2000, 8000):
+        t, W = tiles_per_chunk(nves, vn.VN_F32)
+        assert abs(t - max(1.0, (0.12 * W) ** 0.5)) <= 1.0
+        t64, _ = tiles_per_chunk(nves, vn.VN_F64)
+        assert 1 <= t64 <= 4
+    assert tiles_per_chunk(256, vn.VN_F32)[0] == 1 and tiles_per_chunk(8000, vn.VN_F32)[0] == 33
