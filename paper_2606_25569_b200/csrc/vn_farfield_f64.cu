@@ -31,8 +31,9 @@ constexpr int kSub64 = kST64 / kTile;         // source tiles per super-tile: 4
 #define VN_F64_MINBLK 3
 #endif
 #ifndef VN_F64_GTAB
-#define VN_F64_GTAB 0             // 1: the pair kernel's blocks copy the log tables from scratch (built once per call by
-#endif                            // pack_sources_f64 with the same code) instead of building them
+#define VN_F64_GTAB 1             // the pair kernel's blocks copy the log tables from scratch (built once per call by
+#endif                            // pack_sources_f64 with the same code) instead of building them: +1 % at 2000 x 128,
+                                  // +2.4 % at 256 x 128 (one-tile blocks)
 #ifndef VN_F64_LASTOUT
 #define VN_F64_LASTOUT 0          // 1: stage hand-back by the last warp out (as in the fp32 kernel); costs 28 bytes of
                                   // spills at 3 blocks/SM and measured 965 against 1000 GInt/s at 2000 x 128: off

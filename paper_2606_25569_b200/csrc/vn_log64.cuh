@@ -39,7 +39,8 @@ __device__ __forceinline__ void log_rcp_f64(double r2, const double *__restrict_
     mhalf_log = fma(eps, q, base);
 }
 
-// the two tables of log_rcp_f64, consecutive in shared memory: tab[0 .. kLogTab) and tabE[0 .. kExpTab)
+// the two tables of log_rcp_f64, consecutive in memory (shared, or the scratch copy the pair kernel loads from):
+// tab[0 .. kLogTab) and tabE[0 .. kExpTab)
 __device__ __forceinline__ void build_log_tables(double *tab, int tid, int nthreads)
 {
     for (int k = tid; k < kLogTab; k += nthreads) tab[k] = 0.5 * log1p((double)k * (1.0 / 1024.0));
