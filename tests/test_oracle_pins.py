@@ -547,3 +547,52 @@ def test_complex_potential_form_of_the_stokeslet_sum():
     u = -(Phi1.real + 1j * Phi2.real) + 0.5 * z * np.conj(dPhi) - 0.5 * np.conj(psi)
     ref = oracle.farfield_targets(X, F, W, xt, mu=1.0) * 4 * np.pi
     assert np.abs(u - (ref[:, 0] + 1j * ref[:, 1])).max() <= 1e-13
+
+
+# ----------------------------------------------------------------------------- sharp pins (round 2)
+def test_near_mask_threshold_is_sharp_and_inclusive():
+    """PAPER.md:144 "less than OR EQUAL TO the arclength spacing", :248 |d| <= h.  All coordinates are dyadic
+    rationals, so d^2 and h^2 are exact doubles and the decision at d = h is not a rounding accident:
+    h = 5/16; targets on the axis at h(1 - 1e-6), h, h(1 + 1e-6), 0.95 h, 1.05 h and on the 3-4-5 diagonal
+    (3/16, 4/16) with d = 5/16 = h exactly, each next to its own source point (the sources are 10 apart)."""
+    h = 0.3125
+    offs = [(h * (1 - 1e-6), 0.0, 1), (h, 0.0, 1), (h * (1 + 1e-6), 0.0, 0), (0.95 * h, 0.0, 1), (1.05 * h, 0.0, 0),
+            (0.1875, 0.25, 1), (0.0, -h, 1), (-0.1875, -0.25, 1), (0.1875 + 2.0 ** -20, 0.25, 0),
+            (0.1875 - 2.0 ** -20, 0.25, 1)]
+    n = len(offs)
+    B = np.stack([10.0 * np.arange(n), np.zeros(n)], -1)                # source vesicle: spacing h
+    A = B + np.array([(dx, dy) for dx, dy, _ in offs])                  # target vesicle: tiny spacing of its own
+    X = np.stack([A, B])
+    W = np.stack([np.full(n, 2.0 ** -10), np.full(n, h)])
+    W[1, 3] = 0.25 * h                                                  # h is the LARGEST weight of the vesicle (N1)
+    near = oracle.near_mask(X, W)
+    want = np.array([e for _, _, e in offs], dtype=np.uint8)
+    assert np.array_equal(near[:n, 1], want)
+    assert not near[:n, 0].any() and not near[n:, 1].any()              # never the own vesicle
+    assert not near[n:, 0].any()                                        # A's own spacing 2^-10: B is not near A
+    assert np.array_equal(oracle.near_mask_subset(X, W, np.arange(2 * n)), near)
+    # the spacing is the SOURCE vesicle's: give A the spacing h and B a tiny one, the relation flips
+    near2 = oracle.near_mask(X, W[::-1].copy())
+    assert np.array_equal(near2[n:, 0][[0, 1, 3, 5, 6, 7, 9]], np.ones(7, dtype=np.uint8)) and not near2[:n, 1].any()
+
+
+def test_redistribute_integrates_every_mode_of_the_fine_spectrum():
+    """Reading R2: the arclength is the term-by-term integral of the Fourier series of |X_alpha| on the fine grid,
+    modes k = 1 .. M/2 - 1.  A strong ripple at the coarse grid's highest matched mode (N/2 - 1) puts energy
+    6e-7 / 7e-6 (coefficient / k) into the fine grid's top mode M/2 - 1, so dropping any mode up to the last one
+    moves the arclengths by far more than the 1e-12 this is compared at (numpy FFT / interp route)."""
+    for N, amp in ((12, 0.2), (16, 0.2)):
+        M = 6 * N
+        al = 2 * np.pi * np.arange(N) / N
+        r = 1 + amp * np.cos((N // 2 - 1) * al + 0.3)
+        X = np.stack([r * np.cos(al), 0.7 * r * np.sin(al)], -1)[None] + np.array([0.5, -0.25])
+        # the premise: |shat_k| / k at the top mode is large against the tolerance
+        Xh = np.fft.fft(X[0], axis=0) / N
+        pad = np.zeros((M, 2), dtype=complex)
+        K = (N - 1) // 2
+        pad[:K + 1] = Xh[:K + 1]
+        pad[M - K:] = Xh[N - K:]
+        dXu = np.real(np.fft.ifft(pad * (1j * np.fft.fftfreq(M, 1.0 / M))[:, None], axis=0)) * M
+        sh = np.fft.fft(np.sqrt((dXu ** 2).sum(1))) / M
+        assert abs(sh[M // 2 - 1]) / (M // 2 - 1) > 1e-7
+        assert np.abs(oracle.redistribute(X) - _np_redistribute(X)).max() <= 1e-12
