@@ -211,9 +211,19 @@ vn_status vn_redistribute_arclength(const void *X, int64_t nves, int64_t npts, v
  * vn_farfield_host / vn_farfield_masked / vn_farfield_targets call records a CUDA event pair on its
  * stream around the pair kernel alone (not the pack / finish / correction kernels).  vn_profile_read waits for the recorded events,
  * writes up to max_entries durations in milliseconds (oldest first) into the HOST array
- * ms, forgets them, and returns how many it wrote (or -1 on a CUDA error). */
+ * ms, forgets them, and returns how many it wrote (or -1 on a CUDA error).  vn_profile_enable(0) also destroys
+ * whatever events were recorded and not read. */
 vn_status vn_profile_enable(int enable);
 int64_t vn_profile_read(double *ms, int64_t max_entries);
+
+/* Measured issue rates of the arithmetic pipes that bound the pair kernels (the nominal
+ * lane counts "must be confirmed by microbenchmark").  Runs four register-only stream
+ * kernels of this library on `stream` (about 40 ms in all), waits for them, and writes into the HOST array
+ * rates[5]: lane-operations per second of [0] packed FFMA2 (fma.rn.f32x2, counted as two per thread),
+ * [1] FFMA, [2] MUFU (rcp.approx and lg2.approx, half each), [3] DFMA; [4] the device's SM count.
+ * The best of three launch shapes (16 / 32 / 64 warps per SM, eight independent chains per thread) is reported.
+ * Synchronous; not capturable into a graph.  bench.py calls it once per run for roofline.peak_measured. */
+vn_status vn_pipe_peaks(double *rates /* HOST, 5 entries */, void *stream);
 
 /* Host-only introspection (no CUDA call, works without a GPU): the work decomposition vn_farfield would use
  * for nves x npts points when `resident_blocks` blocks of the pair kernel fit on the device at once
@@ -232,7 +242,8 @@ int64_t vn_launch_count(void);
 /* Static, NUL-terminated description of a status code. */
 const char *vn_status_string(vn_status s);
 
-/* Library version: major*10000 + minor*100 + patch. */
+/* Library version: major*10000 + minor*100 + patch (this header: 0.2.0 = 200). */
+#define VN_VERSION 200
 int vn_version(void);
 
 #ifdef __cplusplus

@@ -21,6 +21,10 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "oracle_vesnet.c")
 _LIB = os.path.join(_HERE, "liboracle_vesnet.so")
 _lib = None
+_BASE_SRC = os.path.join(_HERE, "baseline_f64.c")
+_BASE_LIB = os.path.join(_HERE, "libbaseline_f64.so")
+_BASE_FLAGS = ["-O3", "-march=native", "-ffast-math", "-fopenmp"]
+_base = None
 
 
 def build(force: bool = False) -> str:
@@ -30,6 +34,39 @@ def build(force: bool = False) -> str:
                "-o", _LIB, _SRC, "-lm"]
         subprocess.run(cmd, check=True)
     return _LIB
+
+
+def build_baseline(force: bool = False) -> str:
+    """Compile baseline_f64.c, the plain-double SPEED baseline (not the parity oracle; see its header).
+    -march=native: always rebuilt on the machine that times it (bench.py passes force=True)."""
+    if force or not os.path.exists(_BASE_LIB) or os.path.getmtime(_BASE_LIB) < os.path.getmtime(_BASE_SRC):
+        subprocess.run(["gcc"] + _BASE_FLAGS + ["-fPIC", "-shared", "-o", _BASE_LIB, _BASE_SRC, "-lm"], check=True)
+    return _BASE_LIB
+
+
+def baseline_flags() -> str:
+    return "gcc " + " ".join(_BASE_FLAGS)
+
+
+def baseline_farfield_subset(X, F, W, idx, mu=1.0, rebuild=False):
+    """The direct sum in plain double at the flat point indices ``idx`` -> [len(idx), 2] (speed baseline)."""
+    global _base
+    if _base is None or rebuild:
+        lib = ctypes.CDLL(build_baseline(force=rebuild))
+        d = ctypes.POINTER(ctypes.c_double)
+        lib.baseline_num_threads.restype = ctypes.c_int
+        lib.baseline_farfield_subset.argtypes = [d, d, d, ctypes.c_int64, ctypes.c_int64, ctypes.c_double,
+                                                 ctypes.POINTER(ctypes.c_int64), ctypes.c_int64, d]
+        _base = lib
+    X = _c(X); nves, npts, _ = X.shape
+    F = _c(F, X.shape); W = _c(W, (nves, npts))
+    idx = np.ascontiguousarray(idx, dtype=np.int64)
+    Us = np.empty((idx.size, 2), dtype=np.float64)
+    rc = _base.baseline_farfield_subset(_p(X), _p(F), _p(W), nves, npts, float(mu),
+                                        idx.ctypes.data_as(ctypes.POINTER(ctypes.c_int64)), idx.size, _p(Us))
+    if rc:
+        raise ValueError(f"baseline_farfield_subset rc={rc}")
+    return Us
 
 
 def _load():

@@ -78,6 +78,8 @@ def lib():
         L.vn_launch_count.restype = i64
         L.vn_status_string.argtypes = [ci]
         L.vn_status_string.restype = ctypes.c_char_p
+        L.vn_pipe_peaks.argtypes = [ctypes.POINTER(dbl), vp]
+        L.vn_pipe_peaks.restype = ci
         L.vn_version.argtypes = []
         L.vn_version.restype = ci
         _lib = L
@@ -195,12 +197,15 @@ def vn_near_pairs(X, W, near_ptr=None, near_ves=None, stream=None):
             if rc != VN_OK:
                 raise VesnetError(rc, "vn_near_pairs")
             near_ves = torch.empty(int(near_ptr[P].item()), dtype=torch.int32, device=X.device)
+            if near_ves.numel() == 0:
+                return near_ptr, near_ves                  # the count-only call has filled near_ptr
         _check_dev("near_ves", near_ves, None, torch.int32)
-        if near_ves.numel() > 0:
-            rc = L.vn_near_pairs(X.data_ptr(), W.data_ptr(), nves, npts, near_ptr.data_ptr(), near_ves.data_ptr(),
-                                 near_ves.numel(), _prec(X), _stream_ptr(stream))
-            if rc != VN_OK:
-                raise VesnetError(rc, "vn_near_pairs")
+        # a caller-supplied empty near_ves still gets the count-only call, so that near_ptr is always written
+        rc = L.vn_near_pairs(X.data_ptr(), W.data_ptr(), nves, npts, near_ptr.data_ptr(),
+                             near_ves.data_ptr() if near_ves.numel() else None, near_ves.numel(), _prec(X),
+                             _stream_ptr(stream))
+        if rc != VN_OK:
+            raise VesnetError(rc, "vn_near_pairs")
     return near_ptr, near_ves
 
 
@@ -348,6 +353,15 @@ def vn_profile_read(max_entries: int = 4096):
     if n < 0:
         raise VesnetError(VN_ERR_CUDA, "vn_profile_read")
     return [buf[i] for i in range(n)]
+
+
+def vn_pipe_peaks(stream=None):
+    """Measured pipe rates in lane-operations per second: dict(ffma2, ffma, mufu, dfma, sms).  Synchronous."""
+    buf = (ctypes.c_double * 5)()
+    rc = lib().vn_pipe_peaks(buf, _stream_ptr(stream))
+    if rc != VN_OK:
+        raise VesnetError(rc, "vn_pipe_peaks")
+    return dict(ffma2=buf[0], ffma=buf[1], mufu=buf[2], dfma=buf[3], sms=int(buf[4]))
 
 
 def vn_launch_count() -> int:

@@ -18,8 +18,9 @@ static std::vector<cudaEvent_t> g_profile_events;   // begin, end, begin, end, .
 
 void profile_mark(cudaStream_t st, bool begin)
 {
-    if (!g_profile) return;
+    if (!__atomic_load_n(&g_profile, __ATOMIC_RELAXED)) return;    // cheap test without the lock ...
     std::lock_guard<std::mutex> lock(g_profile_mtx);
+    if (!g_profile) return;                                        // ... decided under it
     if (begin != (g_profile_events.size() % 2 == 0)) return;   // keep pairs well formed
     cudaEvent_t ev;
     if (cudaEventCreate(&ev) != cudaSuccess) return;
@@ -47,6 +48,7 @@ void plan_f64(long long P, int slots, int *super_tile, int *sub, SymSplit *sp);
 vn_status near_pairs(const void *X, const void *W, int64_t nves, int64_t npts, int64_t *near_ptr,
                      int32_t *near_ves, int64_t capacity, vn_precision prec, cudaStream_t st);
 vn_status arclength_weights(const void *X, int64_t nves, int64_t npts, void *W, vn_precision prec, cudaStream_t st);
+vn_status pipe_peaks(double *rates, cudaStream_t st);
 
 Split choose_split_for(int n_tb, int n_tiles, int slots, int min_tiles)
 {
@@ -356,10 +358,22 @@ vn_status vn_plan_farfield(int64_t nves, int64_t npts, vn_precision precision, i
     return VN_OK;
 }
 
+vn_status vn_pipe_peaks(double *rates, void *stream)
+{
+    if (!rates) return VN_ERR_INVALID_ARG;
+    const vn_status ds = check_device();
+    if (ds != VN_OK) return ds;
+    return pipe_peaks(rates, (cudaStream_t)stream);
+}
+
 vn_status vn_profile_enable(int enable)
 {
     std::lock_guard<std::mutex> lock(g_profile_mtx);
-    g_profile = enable != 0;
+    __atomic_store_n(&g_profile, enable != 0, __ATOMIC_RELAXED);
+    if (!enable) {                                  // recorded and never read: do not keep the events
+        for (cudaEvent_t ev : g_profile_events) cudaEventDestroy(ev);
+        g_profile_events.clear();
+    }
     return VN_OK;
 }
 
@@ -395,6 +409,6 @@ const char *vn_status_string(vn_status s)
     return "unknown status";
 }
 
-int vn_version(void) { return 300; }
+int vn_version(void) { return VN_VERSION; }
 
 }  // extern "C"

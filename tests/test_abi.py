@@ -25,7 +25,10 @@ def test_library_exports_every_declared_symbol():
             "vn_farfield_targets", "vn_elastic_force", "vn_redistribute_arclength", "vn_farfield_fmm", "vn_farfield_targets_fmm", "vn_plan_farfield"} <= set(names)
     for n in names:
         assert hasattr(L, n), n
-    assert vn.vn_version() >= 100
+    # the header's encoding, major*10000 + minor*100 + patch, and the header's own constant
+    header = open(os.path.join(ROOT, "include", "vesnet_farfield.h")).read()
+    assert vn.vn_version() == int(re.search(r"#define\s+VN_VERSION\s+(\d+)", header).group(1)) == 200
+    assert "vn_pipe_peaks" in names
     assert L.vn_status_string(0) == b"ok" and b"invalid" in L.vn_status_string(1)
 
 
@@ -72,4 +75,5 @@ def test_argument_validation_needs_no_gpu():
     assert L.vn_farfield_targets_fmm(q, 3, p, p, p, 2, 4, 1.0, 60, q, vn.VN_F64, None) == INV   # order > 48
     assert L.vn_farfield_targets_fmm(None, 0, p, p, p, 2, 4, 1.0, 12, None, vn.VN_F64, None) == vn.VN_OK
     assert L.vn_farfield_host(p, None, None, 2, 4, 1.0, q, vn.VN_F64) == INV
+    assert L.vn_pipe_peaks(None, None) == INV
     assert L.vn_farfield_host(p, p, None, 2, 4, -1.0, q, vn.VN_F64) == INV

@@ -16,14 +16,9 @@ from paper_2606_25569_b200 import inputs
 pytestmark = pytest.mark.gpu
 torch = pytest.importorskip("torch")
 
-TOL = {np.float64: 1e-12, np.float32: 2e-5}
+from parity_util import TOL, check, rel_l2
+
 _cache = {}
-
-
-def rel_l2(a, b):
-    a = np.asarray(a, dtype=np.float64).ravel()
-    b = np.asarray(b, dtype=np.float64).ravel()
-    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
 
 
 def dev(a, dtype):
@@ -179,11 +174,9 @@ def test_farfield_masked_full_parity(case, dtype):
     got = vn.vn_farfield_masked(Xd, Fd, Wd, ptr, ves, mu)
     torch.cuda.synchronize()
     got = got.cpu().numpy()
-    err = rel_l2(got, ref)
     rows = near.sum(1) > 0                                           # the corrected targets on their own
-    err_rows = rel_l2(got.reshape(-1, 2)[rows], ref.reshape(-1, 2)[rows])
-    print(f"masked {case} {np.dtype(dtype).name}: rel-L2 {err:.3e} (corrected rows only {err_rows:.3e}, {rows.sum()} rows)")
-    assert err <= TOL[dtype] and err_rows <= TOL[dtype]
+    check(got, ref, TOL[dtype], f"masked {case} {np.dtype(dtype).name}")
+    check(got.reshape(-1, 2)[rows], ref.reshape(-1, 2)[rows], TOL[dtype], f"masked {case} {np.dtype(dtype).name}, corrected rows only")
     # the mask matters: the unmasked sum differs on those rows by far more than the tolerance
     full = oracle.farfield(Xo, Fo, Wo, mu).reshape(-1, 2)
     assert rel_l2(full[rows], ref.reshape(-1, 2)[rows]) > 1e3 * TOL[dtype]
@@ -221,9 +214,8 @@ def test_farfield_masked_large_sampled(dtype):
     Xo, Fo, Wo = stored(X, dtype), stored(F, dtype), stored(W, dtype)
     rows = oracle.near_mask_subset(Xo, Wo, idx)
     ref = oracle.farfield_masked_subset(Xo, Fo, Wo, idx, rows, mu)
-    err = rel_l2(got.cpu().numpy().reshape(-1, 2)[idx], ref)
-    print(f"masked config3 x0.97 {np.dtype(dtype).name}: {len(hot)} corrected points, sampled rel-L2 {err:.3e}")
-    assert len(hot) > 1000 and err <= TOL[dtype]
+    check(got.cpu().numpy().reshape(-1, 2)[idx], ref, TOL[dtype], f"masked config3 x0.97 {np.dtype(dtype).name}, {len(hot)} corrected points, sampled")
+    assert len(hot) > 1000
 
 
 def test_farfield_masked_deterministic():
@@ -258,9 +250,7 @@ def test_farfield_targets_parity(index, nt, dtype):
     ref = oracle.farfield_targets(stored(s.X, dtype), stored(s.F, dtype), stored(W, dtype), stored(xt, dtype), s.mu)
     got = vn.vn_farfield_targets(dev(xt, dtype), dev(s.X, dtype), dev(s.F, dtype), dev(W, dtype), s.mu)
     torch.cuda.synchronize()
-    err = rel_l2(got.cpu().numpy(), ref)
-    print(f"targets config{index} nt={nt} {np.dtype(dtype).name}: rel-L2 {err:.3e}")
-    assert err <= TOL[dtype]
+    check(got.cpu().numpy(), ref, TOL[dtype], f"targets config{index} nt={nt} {np.dtype(dtype).name}")
 
 
 @pytest.mark.parametrize("dtype", [np.float64, np.float32])
@@ -274,9 +264,7 @@ def test_farfield_targets_large_sampled(dtype):
     rng = np.random.Generator(np.random.PCG64(904))
     idx = np.unique(np.concatenate([[0, 1023, 1024, len(xt) - 1], rng.choice(len(xt), size=1500, replace=False)]))
     ref = oracle.farfield_targets(stored(s.X, dtype), stored(s.F, dtype), stored(W, dtype), stored(xt, dtype)[idx], s.mu)
-    err = rel_l2(got.cpu().numpy()[idx], ref)
-    print(f"targets config3 nt={len(xt)} {np.dtype(dtype).name}: sampled rel-L2 {err:.3e}")
-    assert err <= TOL[dtype]
+    check(got.cpu().numpy()[idx], ref, TOL[dtype], f"targets config3 nt={len(xt)} {np.dtype(dtype).name}, sampled")
 
 
 @pytest.mark.parametrize("dtype", [np.float64, np.float32])
@@ -293,7 +281,7 @@ def test_farfield_targets_on_a_membrane_free_vesicle_equals_farfield(dtype):
     # with a source point)
     b = vn.vn_farfield_targets(Xd[-1].clone(), Xd[:-1].contiguous(), Fd[:-1].contiguous(), Wd[:-1].contiguous(), s.mu)
     torch.cuda.synchronize()
-    assert rel_l2(b.cpu().numpy(), a.cpu().numpy()) <= TOL[dtype]
+    check(b.cpu().numpy(), a.cpu().numpy(), TOL[dtype], f"targets on a force-free vesicle vs farfield {np.dtype(dtype).name}")
 
 
 def test_farfield_targets_empty():
@@ -305,13 +293,20 @@ def test_farfield_targets_empty():
 
 
 # ------------------------------------------------------------------------------------- elastic force (row f-2)
-def force_tol(npts, dtype):
-    """The operator is a fourth spectral derivative: each of the four d/dalpha amplifies the relative
-    rounding noise already present by up to npts/2 (highest retained wavenumber over the O(1)
-    wavenumbers that carry the signal).  The kernel works in double, the oracle in long double, on the
-    same stored inputs: bound 64 eps (npts/2)^4 (64 covers the npts-term sums), plus the rounding of
-    the result to the storage type."""
-    return max(TOL[dtype] if dtype == np.float32 else 0.0, 64 * 2.2e-16 * (npts / 2) ** 4, 1e-12)
+def force_tol(X, sig, kb, dtype):
+    """Empirical conditioning of f = -kappa_b X_ssss + (sigma X_s)_s at this input (the operator is a fourth spectral
+    derivative, so north_star's 1e-12 -- stated for vn_farfield -- does not apply unchanged): the ORACLE is evaluated
+    on X and on X with every vesicle-centred coordinate multiplied by (1 + 2 eps r), r = +-1 at random,
+    eps = 2^-53; the relative L2 change is what one rounding of the input costs.  The kernel differentiates
+    differences to the vesicle's first point in double, i.e. it rounds numbers of the vesicle's size, hence the
+    centred perturbation.  Allowed: 8 x that change (+ 1e-14 for tiny npts; + 2^-23 for rounding the result to
+    float).  At npts = 128 this is about 2e-11 (the bound used in round 1, 64 eps (npts/2)^4, was 2.4e-7)."""
+    Xo, so = stored(X, dtype), stored(sig, dtype)
+    rng = np.random.Generator(np.random.PCG64(12345))
+    c = Xo.mean(1, keepdims=True)
+    Xp = c + (Xo - c) * (1.0 + 2.0 ** -52 * rng.choice([-1.0, 1.0], size=Xo.shape))
+    est = rel_l2(oracle.elastic_force(Xp, so, kb), oracle.elastic_force(Xo, so, kb))
+    return 8.0 * est + 1e-14 + (2.0 ** -23 if dtype == np.float32 else 0.0)
 
 
 def tension(nves, npts, seed):
@@ -332,9 +327,7 @@ def test_elastic_force_parity(index, dtype):
     ref = oracle.elastic_force(stored(s.X, dtype), stored(sig, dtype), kb)
     got = vn.vn_elastic_force(dev(s.X, dtype), dev(sig, dtype), kb)
     torch.cuda.synchronize()
-    err = rel_l2(got.cpu().numpy(), ref)
-    print(f"elastic force config{index} {np.dtype(dtype).name}: rel-L2 {err:.3e} (tolerance {force_tol(s.npts, dtype):.1e})")
-    assert err <= force_tol(s.npts, dtype)
+    check(got.cpu().numpy(), ref, force_tol(s.X, sig, kb, dtype), f"elastic force config{index} {np.dtype(dtype).name}", c_max=4.0)
 
 
 @pytest.mark.parametrize("npts", [3, 8, 31, 32, 33, 100, 129, 257, 1024])
@@ -347,7 +340,7 @@ def test_elastic_force_edge_shapes(npts):
     ref = oracle.elastic_force(X, sig, 1.3)
     got = vn.vn_elastic_force(dev(X, np.float64), dev(sig, np.float64), 1.3)
     torch.cuda.synchronize()
-    assert rel_l2(got.cpu().numpy(), ref) <= force_tol(npts, np.float64)
+    check(got.cpu().numpy(), ref, force_tol(X, sig, 1.3, np.float64), f"elastic force npts={npts}", c_max=4.0)
 
 
 def test_elastic_force_rejects_long_vesicles_and_feeds_farfield():
@@ -363,7 +356,7 @@ def test_elastic_force_rejects_long_vesicles_and_feeds_farfield():
     torch.cuda.synchronize()
     Fo = oracle.elastic_force(s.X, sig.cpu().numpy(), 0.5)
     ref = oracle.farfield(s.X, Fo, oracle.weights(s.X), s.mu)
-    assert rel_l2(Ud.cpu().numpy(), ref) <= force_tol(s.npts, np.float64)
+    check(Ud.cpu().numpy(), ref, 8.0 * force_tol(s.X, sig.cpu().numpy(), 0.5, np.float64), "elastic force -> farfield chain config0")
 
 
 # ------------------------------------------------------------------------------------- equal-arclength redistribution (row f-3)
@@ -371,6 +364,12 @@ def shape_err(got, ref):
     """Error relative to the size of the vesicles (not to their position in the box)."""
     c = ref.mean(1, keepdims=True)
     return float(np.linalg.norm(got - ref) / np.linalg.norm(ref - c))
+
+
+def shape_err_max(got, ref):
+    """Largest point-wise displacement over the rms radius of the vesicles."""
+    c = ref.mean(1, keepdims=True)
+    return float(np.sqrt(((got - ref) ** 2).sum(-1)).max() / np.sqrt(((ref - c) ** 2).sum(-1).mean()))
 
 
 def redistribute_tol(X, dtype):
@@ -391,10 +390,12 @@ def test_redistribute_parity(index, dtype):
     got = vn.vn_redistribute_arclength(dev(X, dtype))
     torch.cuda.synchronize()
     err = shape_err(got.cpu().numpy().astype(np.float64), ref)
+    err_max = shape_err_max(got.cpu().numpy().astype(np.float64), ref)
     W0, W1 = oracle.weights(stored(X, dtype)), oracle.weights(got.cpu().numpy().astype(np.float64))
     print(f"redistribute config{index} {np.dtype(dtype).name}: shape-relative L2 {err:.3e} (tolerance {redistribute_tol(X, dtype):.1e}); "
           f"max/min spacing {np.max(W0.max(1) / W0.min(1)):.3f} -> {np.max(W1.max(1) / W1.min(1)):.4f}")
-    assert err <= redistribute_tol(X, dtype)
+    print(f"redistribute config{index} {np.dtype(dtype).name}: point-wise max {err_max:.3e}")
+    assert err <= redistribute_tol(X, dtype) and err_max <= 4.0 * redistribute_tol(X, dtype)
 
 
 @pytest.mark.parametrize("npts", [3, 4, 5, 8, 31, 33, 100, 129, 257, 512])
@@ -407,7 +408,7 @@ def test_redistribute_edge_shapes(npts):
     ref = oracle.redistribute(X)
     got = vn.vn_redistribute_arclength(dev(X, np.float64))
     torch.cuda.synchronize()
-    assert shape_err(got.cpu().numpy(), ref) <= 1e-12
+    assert shape_err(got.cpu().numpy(), ref) <= 1e-12 and shape_err_max(got.cpu().numpy(), ref) <= 4e-12
 
 
 def test_redistribute_rejects_bad_sizes_and_chains():
@@ -423,13 +424,16 @@ def test_redistribute_rejects_bad_sizes_and_chains():
     torch.cuda.synchronize()
     Xo = oracle.redistribute(s.X)
     ref = oracle.farfield(Xo, s.F, oracle.weights(Xo), s.mu)
-    assert rel_l2(Ud.cpu().numpy(), ref) <= 1e-12
+    check(Ud.cpu().numpy(), ref, 1e-12, "redistribute -> weights -> farfield chain config0")
 
 
 # ------------------------------------------------------------------------------------- fast multipole method (row f-4, second half)
 # vn_farfield_fmm approximates the exact sum; the oracle is still the plain direct sum.  The tolerance follows the
 # truncation error of the expansions, about 0.45^p relative: p = 12 for the fp32 bar (2e-5),
-# p = 38 for the fp64 bar (1e-12).
+# p = 38 for the fp64 bar (1e-12).  Point-wise (max-rel) the truncation error is held to FMM_C x the tolerance: the
+# error of a truncated expansion is largest for the targets closest to the corner of their box, a handful of points,
+# so it exceeds the L2 average by a factor the exact path does not have (measured maxima: DESIGN.md section 7).
+FMM_C = 4.0
 @pytest.mark.parametrize("index,dtype,order", [(0, np.float64, 38), (0, np.float32, 12), (1, np.float64, 38),
                                                 (1, np.float32, 12), (1, np.float64, 12)])
 def test_fmm_full_parity(index, dtype, order):
@@ -438,10 +442,8 @@ def test_fmm_full_parity(index, dtype, order):
     ref = oracle.farfield(stored(s.X, dtype), stored(s.F, dtype), stored(W, dtype), s.mu)
     got = vn.vn_farfield_fmm(dev(s.X, dtype), dev(s.F, dtype), dev(W, dtype), s.mu, order)
     torch.cuda.synchronize()
-    err = rel_l2(got.cpu().numpy(), ref)
     tol = TOL[dtype] if not (dtype == np.float64 and order < 30) else 2e-5
-    print(f"fmm config{index} {np.dtype(dtype).name} p={order}: rel-L2 {err:.3e} (tolerance {tol:.0e})")
-    assert err <= tol
+    check(got.cpu().numpy(), ref, tol, f"fmm config{index} {np.dtype(dtype).name} p={order}", c_max=FMM_C)
 
 
 @pytest.mark.parametrize("index,dtype,order,nsample", [(3, np.float32, 12, 3072), (3, np.float64, 38, 3072),
@@ -455,9 +457,7 @@ def test_fmm_sampled_parity_large(index, dtype, order, nsample):
     ref = oracle.farfield_subset(stored(s.X, dtype), stored(s.F, dtype), stored(W, dtype), idx, s.mu)
     got = vn.vn_farfield_fmm(dev(s.X, dtype), dev(s.F, dtype), dev(W, dtype), s.mu, order)
     torch.cuda.synchronize()
-    err = rel_l2(got.cpu().numpy().reshape(-1, 2)[idx], ref)
-    print(f"fmm config{index} {np.dtype(dtype).name} p={order}: sampled rel-L2 {err:.3e}")
-    assert err <= TOL[dtype]
+    check(got.cpu().numpy().reshape(-1, 2)[idx], ref, TOL[dtype], f"fmm config{index} {np.dtype(dtype).name} p={order} sampled", c_max=FMM_C)
 
 
 def test_fmm_converges_with_order_and_agrees_with_exact_path():
@@ -489,7 +489,7 @@ def test_fmm_edge_shapes(nves, npts):
     got = vn.vn_farfield_fmm(dev(X, np.float64), dev(F, np.float64), dev(W, np.float64), 0.7, 40)
     torch.cuda.synchronize()
     got = got.cpu().numpy()
-    assert np.all(np.isfinite(got)) and rel_l2(got, ref) <= 1e-11
+    check(got, ref, 1e-11, f"fmm edge shape {nves} x {npts}", c_max=FMM_C)
 
 
 def test_fmm_single_vesicle_gives_zero():
@@ -514,10 +514,9 @@ def test_fmm_masked_parity(dtype, order):
     got = vn.vn_farfield_fmm(Xd, Fd, Wd, mu, order, near_ptr=ptr, near_ves=ves)
     torch.cuda.synchronize()
     rows = near.sum(1) > 0
-    err = rel_l2(got.cpu().numpy(), ref)
-    err_rows = rel_l2(got.cpu().numpy().reshape(-1, 2)[rows], ref.reshape(-1, 2)[rows])
-    print(f"fmm masked crowded1 {np.dtype(dtype).name} p={order}: rel-L2 {err:.3e} (corrected rows {err_rows:.3e})")
-    assert err <= TOL[dtype] and err_rows <= TOL[dtype]
+    check(got.cpu().numpy(), ref, TOL[dtype], f"fmm masked crowded1 {np.dtype(dtype).name} p={order}", c_max=FMM_C)
+    check(got.cpu().numpy().reshape(-1, 2)[rows], ref.reshape(-1, 2)[rows], TOL[dtype],
+          f"fmm masked crowded1 {np.dtype(dtype).name} p={order}, corrected rows", c_max=FMM_C)
 
 
 @pytest.mark.parametrize("dtype,order", [(np.float64, 38), (np.float32, 12)])
@@ -531,9 +530,7 @@ def test_fmm_targets_parity(index, nt, dtype, order):
     ref = oracle.farfield_targets(stored(s.X, dtype), stored(s.F, dtype), stored(W, dtype), stored(xt, dtype)[idx], s.mu)
     got = vn.vn_farfield_targets(dev(xt, dtype), dev(s.X, dtype), dev(s.F, dtype), dev(W, dtype), s.mu, fmm_order=order)
     torch.cuda.synchronize()
-    err = rel_l2(got.cpu().numpy()[idx], ref)
-    print(f"fmm targets config{index} nt={len(xt)} {np.dtype(dtype).name} p={order}: rel-L2 {err:.3e}")
-    assert err <= TOL[dtype]
+    check(got.cpu().numpy()[idx], ref, TOL[dtype], f"fmm targets config{index} nt={len(xt)} {np.dtype(dtype).name} p={order}", c_max=FMM_C)
 
 
 @pytest.mark.parametrize("layout", ["two_clusters", "line", "one_far_outlier"])
@@ -556,9 +553,7 @@ def test_fmm_nonuniform_layouts(layout):
     ref = oracle.farfield(X, F, W, 1.0)
     got = vn.vn_farfield_fmm(dev(X, np.float64), dev(F, np.float64), dev(W, np.float64), 1.0, 40)
     torch.cuda.synchronize()
-    err = rel_l2(got.cpu().numpy(), ref)
-    print(f"fmm {layout}: rel-L2 {err:.3e}")
-    assert err <= 1e-11
+    check(got.cpu().numpy(), ref, 1e-11, f"fmm {layout}", c_max=FMM_C)
 
 
 def test_fmm_four_million_points():
@@ -583,9 +578,8 @@ def test_fmm_four_million_points():
         vn.vn_farfield_fmm(Xd, Fd, Wd, s.mu, 12, out=got)
     e1.record()
     e1.synchronize()
-    err = rel_l2(got.cpu().numpy().reshape(-1, 2)[idx], ref)
-    print(f"fmm 32000 x 128 (4.1 M points) float32 p=12: sampled rel-L2 {err:.3e}, {e0.elapsed_time(e1) / 3:.2f} ms per evaluation")
-    assert err <= TOL[np.float32]
+    print(f"fmm 32000 x 128 (4.1 M points) float32 p=12: {e0.elapsed_time(e1) / 3:.2f} ms per evaluation")
+    check(got.cpu().numpy().reshape(-1, 2)[idx], ref, TOL[np.float32], "fmm 32000 x 128 float32 p=12 sampled", c_max=FMM_C)
 
 
 @pytest.mark.parametrize("dtype", [np.float64, np.float32])
@@ -595,4 +589,4 @@ def test_fmm_default_order_meets_the_tolerance(dtype):
     ref = oracle.farfield(stored(s.X, dtype), stored(s.F, dtype), stored(W, dtype), s.mu)
     got = vn.vn_farfield_fmm(dev(s.X, dtype), dev(s.F, dtype), dev(W, dtype), s.mu, 0)     # order 0 = default for the precision
     torch.cuda.synchronize()
-    assert rel_l2(got.cpu().numpy(), ref) <= TOL[dtype]
+    check(got.cpu().numpy(), ref, TOL[dtype], f"fmm default order {np.dtype(dtype).name}", c_max=FMM_C)

@@ -596,3 +596,23 @@ def test_redistribute_integrates_every_mode_of_the_fine_spectrum():
         sh = np.fft.fft(np.sqrt((dXu ** 2).sum(1))) / M
         assert abs(sh[M // 2 - 1]) / (M // 2 - 1) > 1e-7
         assert np.abs(oracle.redistribute(X) - _np_redistribute(X)).max() <= 1e-12
+
+
+def test_speed_baseline_agrees_with_the_oracle():
+    """oracle/baseline_f64.c (plain double, vectorised; the CPU SPEED baseline bench.py times) is the same sum as
+    the long-double oracle: 1e-13 relative L2 and point-wise, on a suspension-like input and on random blobs.
+    It is never compared with the CUDA path; this pin only keeps the timed code honest."""
+    rng = np.random.default_rng(77)
+    X, F, W = _random_problem(rng, 9, 37)
+    idx = np.arange(9 * 37)
+    ref = oracle.farfield_subset(X, F, W, idx, mu=0.8)
+    got = oracle.baseline_farfield_subset(X, F, W, idx, mu=0.8)
+    assert np.linalg.norm(got - ref) / np.linalg.norm(ref) <= 1e-13
+    assert np.abs(got - ref).max() <= 1e-13 * np.abs(ref).max()
+    assert np.array_equal(oracle.baseline_farfield_subset(X, F, W, idx[5:9], mu=0.8), got[5:9])
+    A, _ = _ellipse(1.0, 0.4, 128, th=0.3)
+    B, _ = _ellipse(1.0, 0.4, 128, th=1.1, c=(2.4, 0.3))
+    X = np.stack([A, B]); F = rng.normal(size=X.shape); W = oracle.weights(X)
+    ref = oracle.farfield(X, F, W).reshape(-1, 2)
+    got = oracle.baseline_farfield_subset(X, F, W, np.arange(256))
+    assert np.linalg.norm(got - ref) / np.linalg.norm(ref) <= 1e-13

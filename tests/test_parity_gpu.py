@@ -14,14 +14,9 @@ from paper_2606_25569_b200 import inputs
 pytestmark = pytest.mark.gpu
 torch = pytest.importorskip("torch")
 
-TOL = {np.float64: 1e-12, np.float32: 2e-5}
+from parity_util import TOL, check, rel_l2
+
 _cache = {}
-
-
-def rel_l2(a, b):
-    a = np.asarray(a, dtype=np.float64).ravel()
-    b = np.asarray(b, dtype=np.float64).ravel()
-    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
 
 
 def dev(a, dtype):
@@ -61,14 +56,12 @@ def test_farfield_full_parity(index, dtype):
     Xo, Fo, Wo = oracle_inputs(s.X, s.F, W, dtype)
     ref = oracle.farfield(Xo, Fo, Wo, s.mu)
     got = gpu_farfield(s.X, s.F, W, s.mu, dtype)
-    err = rel_l2(got, ref)
-    print(f"config{index} {np.dtype(dtype).name}: rel-L2 {err:.3e}")
-    assert err <= TOL[dtype]
+    check(got, ref, TOL[dtype], f"farfield config{index} {np.dtype(dtype).name} all targets")
 
 
 # ------------------------------------------------------------------------------------- full-size configs, sampled targets
-@pytest.mark.parametrize("index,dtype,nsample", [(2, np.float32, 4096), (2, np.float64, 4096),
-                                                 (3, np.float32, 3072), (3, np.float64, 3072)])
+@pytest.mark.parametrize("index,dtype,nsample", [(2, np.float32, 8192), (2, np.float64, 8192),
+                                                 (3, np.float32, 16384), (3, np.float64, 16384)])
 def test_farfield_sampled_parity_large(index, dtype, nsample):
     s, W = problem(index)
     P = s.nves * s.npts
@@ -76,44 +69,40 @@ def test_farfield_sampled_parity_large(index, dtype, nsample):
     Xo, Fo, Wo = oracle_inputs(s.X, s.F, W, dtype)
     ref = oracle.farfield_subset(Xo, Fo, Wo, idx, s.mu)
     got = gpu_farfield(s.X, s.F, W, s.mu, dtype).reshape(-1, 2)[idx]
-    err = rel_l2(got, ref)
-    print(f"config{index} {np.dtype(dtype).name}: sampled rel-L2 {err:.3e} over {len(idx)} targets")
-    assert err <= TOL[dtype]
+    check(got, ref, TOL[dtype], f"farfield config{index} {np.dtype(dtype).name} sampled")
 
 
 def test_config4_sequence_fp32():
-    """8,000 x 128, ten consecutive evaluations on one stream reusing the device buffers; the
-    oracle checks calls 0 and 9 on sampled targets, fp64-GPU checks call 0 on ALL targets."""
+    """8,000 x 128, ten consecutive evaluations on one stream reusing the device buffers (BASELINE.json configs[4]).
+    ALL ten calls are compared on ALL 1.02 M targets with the fp64 GPU path on the same fp32-rounded inputs; the
+    oracle checks calls 0, 4 and 9 on 16,384 sampled targets in both precisions, which ties
+    the fp64 GPU path -- and through it every target of every call -- to the oracle."""
     s, W = problem(4)
     P = s.nves * s.npts
-    idx = sample_targets(P, 1024, 260625569 + 100)
+    idx = sample_targets(P, 16384, 260625569 + 100)
     seq = [dev(x, np.float32) for x in s.X_sequence]
     Xd = torch.empty_like(seq[0])
     Fd, Wd = dev(s.F, np.float32), dev(W, np.float32)
     Ud = torch.empty_like(Xd)
-    outs = {}
+    outs = []
     for c in range(10):
         Xd.copy_(seq[c])
         vn.vn_farfield(Xd, Fd, Wd, s.mu, out=Ud)
-        if c in (0, 9):
-            outs[c] = Ud.clone()
+        outs.append(Ud.clone())                    # stream-ordered copy of call c's result; no host synchronisation
     torch.cuda.synchronize()
-    for c in (0, 9):
-        Xo, Fo, Wo = oracle_inputs(s.X_sequence[c], s.F, W, np.float32)
-        ref = oracle.farfield_subset(Xo, Fo, Wo, idx, s.mu)
-        err = rel_l2(outs[c].cpu().numpy().reshape(-1, 2)[idx], ref)
-        print(f"config4 call {c}: sampled rel-L2 {err:.3e}")
-        assert err <= TOL[np.float32]
-    # all targets: fp32 GPU vs fp64 GPU on the same fp32-rounded inputs
-    U64 = vn.vn_farfield(seq[0].double(), Fd.double(), Wd.double(), s.mu)
-    torch.cuda.synchronize()
-    err = rel_l2(outs[0].cpu().numpy(), U64.cpu().numpy())
-    print(f"config4 call 0: fp32 vs fp64 GPU over all targets rel-L2 {err:.3e}")
-    assert err <= TOL[np.float32]
-    # and the fp64 GPU result itself against the oracle on the sample
-    Xo, Fo, Wo = oracle_inputs(s.X_sequence[0], s.F, W, np.float32)
-    ref = oracle.farfield_subset(Xo, Fo, Wo, idx, s.mu)
-    assert rel_l2(U64.cpu().numpy().reshape(-1, 2)[idx], ref) <= TOL[np.float64]
+    F64, W64 = Fd.double(), Wd.double()
+    U64 = torch.empty((s.nves, s.npts, 2), dtype=torch.float64, device="cuda")
+    for c in range(10):
+        vn.vn_farfield(seq[c].double(), F64, W64, s.mu, out=U64)
+        torch.cuda.synchronize()
+        u64 = U64.cpu().numpy()
+        check(outs[c].cpu().numpy(), u64, TOL[np.float32], f"config4 call {c}: fp32 GPU vs fp64 GPU, all targets")
+        if c in (0, 4, 9):
+            Xo, Fo, Wo = oracle_inputs(s.X_sequence[c], s.F, W, np.float32)
+            ref = oracle.farfield_subset(Xo, Fo, Wo, idx, s.mu)
+            check(outs[c].cpu().numpy().reshape(-1, 2)[idx], ref, TOL[np.float32], f"config4 call {c}: fp32 GPU vs oracle, sampled")
+            check(u64.reshape(-1, 2)[idx], ref, TOL[np.float64], f"config4 call {c}: fp64 GPU vs oracle, sampled")
+    assert not torch.equal(outs[0], outs[9])       # the positions really moved between calls
 
 
 # ------------------------------------------------------------------------------------- edge shapes
@@ -134,8 +123,8 @@ def test_edge_shapes(nves, npts, dtype):
     Xo, Fo, Wo = oracle_inputs(X, F, W, dtype)
     ref = oracle.farfield(Xo, Fo, Wo, mu)
     got = gpu_farfield(X, F, W, mu, dtype)
-    assert got.shape == ref.shape and np.all(np.isfinite(got))
-    assert rel_l2(got, ref) <= TOL[dtype]
+    assert got.shape == ref.shape
+    check(got, ref, TOL[dtype], f"edge shape {nves} x {npts} {np.dtype(dtype).name}")
 
 
 @pytest.mark.parametrize("dtype", [np.float64, np.float32])
@@ -166,9 +155,7 @@ def test_arclength_weights_parity(index, dtype):
     ref = oracle.weights(Xo)
     got = vn.vn_arclength_weights(dev(s.X, dtype))
     torch.cuda.synchronize()
-    err = rel_l2(got.cpu().numpy(), ref)
-    print(f"weights config{index} {np.dtype(dtype).name}: rel-L2 {err:.3e}")
-    assert err <= TOL[dtype]
+    check(got.cpu().numpy(), ref, TOL[dtype], f"weights config{index} {np.dtype(dtype).name}", vec=1)
 
 
 @pytest.mark.parametrize("npts", [1, 2, 3, 8, 31, 32, 33, 100, 129, 257, 1500])
@@ -182,7 +169,7 @@ def test_arclength_weights_edge_shapes(npts):
     if npts <= 2:
         assert np.abs(got).max() < 1e-12          # only the mean and the dropped Nyquist mode exist
     else:
-        assert rel_l2(got, ref) <= 1e-12
+        check(got, ref, 1e-12, f"weights npts={npts}", vec=1)
 
 
 # ------------------------------------------------------------------------------------- whole path, host buffers
@@ -195,13 +182,13 @@ def test_host_entry_point_whole_path(dtype):
     Xo, Fo = X.astype(np.float64), F.astype(np.float64)
     idx = sample_targets(s.nves * s.npts, 2048, 3)
     ref = oracle.farfield_subset(Xo, Fo, oracle.weights(Xo), idx, s.mu)
-    assert rel_l2(got.reshape(-1, 2)[idx], ref) <= TOL[dtype]
+    check(got.reshape(-1, 2)[idx], ref, TOL[dtype], f"host entry {np.dtype(dtype).name} (device weights)")
     # pinned torch tensors and caller-supplied weights
     Xp, Fp = torch.from_numpy(X).pin_memory(), torch.from_numpy(F).pin_memory()
     Wp = torch.from_numpy(oracle.weights(Xo).astype(dtype)).pin_memory()
     Up = torch.empty_like(Xp).pin_memory()
     vn.vn_farfield_host(Xp, Fp, Wp, s.mu, out=Up)
-    assert rel_l2(Up.numpy().reshape(-1, 2)[idx], ref) <= TOL[dtype]
+    check(Up.numpy().reshape(-1, 2)[idx], ref, TOL[dtype], f"host entry {np.dtype(dtype).name} (caller weights)")
 
 
 # ------------------------------------------------------------------------------------- determinism, streams
@@ -298,7 +285,7 @@ def test_coincident_points_and_nans_stay_local(call, dtype):
     Xo, Fo, Wo = oracle_inputs(X, F, W, dtype)
     idx = np.setdiff1d(sample_targets(s.nves * s.npts, 1500, 17), [5 * s.npts + 7, 200 * s.npts + 3])
     ref = oracle.farfield_subset(Xo, Fo, Wo, idx, s.mu)
-    assert rel_l2(got.reshape(-1, 2)[idx], ref) <= TOL[dtype]
+    check(got.reshape(-1, 2)[idx], ref, TOL[dtype], f"coincident pair elsewhere, {call} {np.dtype(dtype).name}")
     # a NaN density at one source poisons every target of the other vesicles (that is the sum's meaning); the exact
     # path answers NaN everywhere (documented: its integer accumulators cannot carry NaN point by point)
     Fn = F.copy(); Fn[9, 0, 0] = np.nan
