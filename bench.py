@@ -12,8 +12,17 @@ evaluations with perturbed positions, reusing the device buffers on one stream. 
 0-3 a step is one evaluation.  `value` counts P*(P-npts) interactions per evaluation (own-vesicle
 pairs are not counted) over device time (CUDA events, inputs resident in HBM, max over ranks);
 `e2e` is the same work through vn_farfield_host with pinned HOST buffers (copies inside the
-timed region).  With --gpus N every rank evaluates its own, differently seeded suspension of the
-same shape (independent problems, no data-path collective): "scaling": "weak".
+timed region).
+
+--gpus N > 1 (one process per GPU, torchrun): the SAME suspension is evaluated by all ranks together
+(DESIGN.md section 8): every rank owns a contiguous range of vesicles, one all-gather makes all
+sources known everywhere, rank r runs blocks r, r+N, ... of the pair walk (vn_farfield_partial), one
+integer reduce-scatter sums the fixed-point accumulators, vn_farfield_finish rounds the rank's shard.
+Total work is fixed: "scaling": "strong".  The result is bit for bit the single-GPU result.
+
+The default invocation (N = 1, configs[4], fp32) also measures, in the same run, the issue rates of
+the FP32 / SFU / FP64 pipes (vn_pipe_peaks -> roofline.peak_measured) and a `sweep` over the other
+configurations north_star's target names (configs[3] fp32 and fp64, configs[1] fp32).
 
 One JSON line is printed by rank 0.
 """
@@ -26,6 +35,7 @@ import statistics
 import sys
 import threading
 import time
+from types import SimpleNamespace
 
 import numpy as np
 
@@ -34,10 +44,13 @@ sys.path.insert(0, ROOT)
 
 METRIC = "far-field Stokeslet GInteractions/s"
 UNIT = "GInt/s"
-# canonical per-pair work: 2 FADD + 3 FMUL + 6 FFMA = 11 FP32-pipe lane
-# instructions (17 flop) + 2 SFU ops; fp64: the same 11 DP instructions (17 flop).
+# canonical per-pair work: 2 FADD + 3 FMUL + 6 FFMA = 11 FP32-pipe
+# lane-instructions (17 flop) + 2 SFU ops; fp64: the same 11 DP instructions (17 flop).
 LANE_OPS_PER_PAIR = 11
 FLOP_PER_PAIR = 17
+# what the kernels execute per directed interaction (symmetric evaluation; SASS counts)
+EXECUTED_LANE_OPS = {("farfield", "f32"): 9.0, ("masked", "f32"): 9.0, ("farfield", "f64"): 12.85, ("masked", "f64"): 12.85,
+                     ("targets", "f32"): 13.0, ("targets", "f64"): 19.0}
 SMS, FP32_LANES, FP64_LANES = 148, 128, 64
 
 
@@ -78,9 +91,14 @@ class ClockSampler(threading.Thread):
                 for bit, name in names.items():
                     if mask & bit:
                         self.reasons.add(name)
-                time.sleep(0.1)
+                time.sleep(0.05)
         except Exception as exc:                      # no NVML: report that, do not fail the bench
             self.reasons.add(f"nvml_unavailable:{type(exc).__name__}")
+
+    def stop(self):
+        self.stop_flag.set()
+        self.join()
+        return self.summary()
 
     def summary(self):
         return {"sm_mhz": statistics.median(self.sm) if self.sm else None,
@@ -99,16 +117,6 @@ def nvml_index(local_rank):
     return local_rank
 
 
-def make_workload(index, rank):
-    """Suspension for this rank: rank 0 gets BASELINE.json's seed, rank r the same recipe with seed + 1000 r."""
-    from paper_2606_25569_b200 import inputs
-    from paper_2606_25569_b200 import multi
-    if rank == 0 or index == 0:
-        return inputs.config(index)
-    kw = dict(inputs._CONFIGS[index])
-    return inputs.suspension(seed=multi.shard_seed(inputs.BASE_SEED, index, rank), **kw)
-
-
 def target_grid(susp, n_side, np_dtype):
     """n_side x n_side velocity-field grid over the suspension's bounding box plus a margin of 1
     (row f-4).  Grid points that fall close to a membrane simply get the plain trapezoid value."""
@@ -119,16 +127,21 @@ def target_grid(susp, n_side, np_dtype):
     return np.ascontiguousarray(np.stack(np.meshgrid(gx, gy, indexing="ij"), -1).reshape(-1, 2), dtype=np_dtype)
 
 
-def oracle_rate(susp, np_dtype, seconds, rng_seed, path="farfield"):
+def oracle_rate(susp, np_dtype, seconds, rng_seed, path="farfield", fast=False):
     """Times the oracle (as it stands) on a bounded random sample of targets x ALL sources of the
-    same workload; returns (GInt/s, cores, description)."""
+    same workload; returns (GInt/s, cores, description).  fast=True times oracle/baseline_f64.c instead
+    (plain double, vectorised: the CPU speed baseline, farfield path only)."""
     import oracle
     X = np.asarray(susp.X, dtype=np_dtype).astype(np.float64)
     F = np.asarray(susp.F, dtype=np_dtype).astype(np.float64)
     W = oracle.weights(X)
     P = susp.nves * susp.npts
     rng = np.random.Generator(np.random.PCG64(rng_seed))
-    if path == "targets":
+    if fast:
+        oracle.build_baseline(force=True)             # -march=native: compiled on the machine that times it
+        pool, per_target = P, P - susp.npts
+        run = lambda idx: oracle.baseline_farfield_subset(X, F, W, idx, susp.mu)
+    elif path == "targets":
         xt = target_grid(susp, 512, np_dtype).astype(np.float64)
         pool, per_target = len(xt), P
         run = lambda idx: oracle.farfield_targets(X, F, W, xt[idx], susp.mu)
@@ -150,12 +163,28 @@ def oracle_rate(susp, np_dtype, seconds, rng_seed, path="farfield"):
     return n * per_target / dt / 1e9, oracle.num_threads(), f"{n} random targets x all {P} sources ({n * per_target:.3e} pairs, {dt:.1f} s)"
 
 
+def cpu_baseline(susp, np_dtype, path):
+    """The reported CPU baseline: the oracle as it stands (long double, the parity checker) and, for the farfield
+    path, the same sum in plain vectorised double (oracle/baseline_f64.c) -- the checker is the right code to compare
+    against and the wrong code to race against, so both are stated."""
+    import oracle
+    v, cores, sample = oracle_rate(susp, np_dtype, 15.0, 4242, path)
+    out = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+           "code": "oracle/oracle_vesnet.c (long double, gcc -O2 -ffp-contract=off -fopenmp)"}
+    if path == "farfield":
+        vf, _, sf = oracle_rate(susp, np_dtype, 5.0, 4243, path, fast=True)
+        out["fast_double"] = {"value": vf, "unit": UNIT, "cores": cores, "sample": sf,
+                              "code": "oracle/baseline_f64.c (double, %s; pinned to the oracle at 1e-13)" % oracle.baseline_flags()}
+    return out
+
+
 def run_reference(args):
     """--impl reference: the oracle on the host cores, same metric/config; rank 0 only."""
+    from paper_2606_25569_b200 import inputs
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    susp = make_workload(args.workload, 0)
+    susp = inputs.config(args.workload)
     np_dtype = np.float32 if args.precision == "f32" else np.float64
     total = max(1, args.steps + args.warmup)
     per_step = max(2.0, min(30.0, 150.0 / total))
@@ -170,7 +199,7 @@ def run_reference(args):
     pairs_eval = 512 * 512 * P if args.path == "targets" else susp.pairs
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": evals * pairs_eval / (value * 1e9) * 1e3, "higher_is_better": True, "scaling": "weak",
+            "ms_per_step": evals * pairs_eval / (value * 1e9) * 1e3, "higher_is_better": True, "scaling": "strong",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": workload_config(args, susp, "oracle on host cores; ms_per_step extrapolated from the sampled rate"),
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
@@ -195,7 +224,8 @@ def workload_config(args, susp, note=""):
             "evaluations_per_step": evals,
             "precision": args.precision, "l2": "flushed between timed steps (256 MiB write); inputs < L2",
             "cuda_graph": bool(getattr(args, "graph", False)),
-            "parallelism": f"{args.gpus} independent suspensions (one per GPU)" if args.gpus > 1 else "single GPU",
+            "parallelism": (f"one suspension over {args.gpus} GPUs: vesicle ranges per rank, all-gather of X/F/W, blocks of the pair "
+                            f"walk dealt round-robin, integer reduce-scatter of the accumulators" if args.gpus > 1 else "single GPU"),
             "note": note}
 
 
@@ -204,7 +234,6 @@ def run_aux(args, susp, vn, torch, tdtype, np_dtype, rank, world, local_rank):
     workload's vesicles (rows f-3, a-1, f-2: everything O(P) that surrounds the pair sum in a time step).
     Reported in membrane points per second; the roofline object describes the dominant kernel
     (redistribute_kernel, FP64 pipe; algorithmic DFMA count per vesicle stated in DESIGN.md section 11)."""
-    from paper_2606_25569_b200 import multi
     import oracle
     P = susp.nves * susp.npts
     X_h = torch.from_numpy(np.ascontiguousarray(susp.X, dtype=np_dtype)).pin_memory()
@@ -240,36 +269,32 @@ def run_aux(args, susp, vn, torch, tdtype, np_dtype, rank, world, local_rank):
     t_dev = 0.0
     for _ in range(args.steps):
         flush.fill_(1)
-        multi.barrier(); torch.cuda.synchronize()
+        torch.cuda.synchronize()
         e0, e1 = ev(), ev()
         e0.record(); step(True); e1.record(); e1.synchronize()
         t_dev += e0.elapsed_time(e1) * 1e-3
     launches = vn.vn_launch_count() - n0
     t_e2e = 0.0
     for _ in range(args.steps):
-        multi.barrier(); torch.cuda.synchronize()
+        torch.cuda.synchronize()
         t0 = time.perf_counter()
         X_d.copy_(X_h, non_blocking=True); sig_d.copy_(sig_h, non_blocking=True)
         step(False)
         F_host.copy_(F_d, non_blocking=True)
         torch.cuda.synchronize()
         t_e2e += time.perf_counter() - t0
-    sampler.stop_flag.set(); sampler.join()
-    rate, t_dev, _ = multi.whole_job_rate(args.steps * P, t_dev, "cuda")
-    rate_e2e, t_e2e, _ = multi.whole_job_rate(args.steps * P, t_e2e, "cuda")
-    if rank != 0:
-        return
+    clocks = sampler.stop()
+    rate, rate_e2e = args.steps * P / t_dev, args.steps * P / t_e2e
     N = susp.npts
     dfma_per_ves = 24 * N * N + 36 * N * N      # interpolant + derivative (4 x 6N x N), integration (6N x 6N)
     k_ms = statistics.mean(parts["redistribute"])
-    clocks = sampler.summary()
     sm_max = clocks.get("sm_max_mhz") or 1965.0
     peak = SMS * FP64_LANES * sm_max * 1e6 / 1e12
     achieved = dfma_per_ves * susp.nves / (k_ms * 1e-3) / 1e12
     es = 4 if args.precision == "f32" else 8
     line = {"metric": "membrane points/s through redistribution + weights + elastic force", "value": rate,
             "unit": "points/s", "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-            "ms_per_step": t_dev / args.steps * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": t_dev / args.steps * 1e3, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"BASELINE.json configs[{args.workload}]: {susp.name}", "path": "rows f-3, a-1, f-2",
                        "nves": susp.nves, "npts": susp.npts, "storage": args.precision,
@@ -281,7 +306,7 @@ def run_aux(args, susp, vn, torch, tdtype, np_dtype, rank, world, local_rank):
                          "peak_source": "derived: 148 SMs x 64 lanes x %.0f MHz" % sm_max,
                          "dfma_per_vesicle": dfma_per_ves, "traffic": None},
             "e2e": {"value": rate_e2e, "unit": "points/s", "h2d_bytes_per_step": 3 * es * P, "d2h_bytes_per_step": 2 * es * P}}
-    if world == 1 and not args.no_cpu_baseline:
+    if not args.no_cpu_baseline:
         Xo = np.asarray(susp.X, dtype=np_dtype).astype(np.float64)
         nv = min(susp.nves, 4000)
         t0 = time.perf_counter()
@@ -290,6 +315,216 @@ def run_aux(args, susp, vn, torch, tdtype, np_dtype, rank, world, local_rank):
         line["cpu_baseline"] = {"value": nv * susp.npts / dt, "unit": "points/s", "cores": oracle.num_threads(),
                                 "kind": "oracle", "sample": f"first {nv} vesicles ({dt:.1f} s)"}
     print(json.dumps(line), flush=True)
+
+
+def traffic_from_profiles(workload, precision, path):
+    """DRAM bytes per launch of the pair kernel from the committed `ncu --set full` capture (profiles/traffic.csv names
+    the capture); a live run cannot measure it -- the profiler is not attached -- so it is looked up, or null."""
+    try:
+        import csv
+        with open(os.path.join(ROOT, "profiles", "traffic.csv")) as fh:
+            for row in csv.DictReader(fh):
+                if (row["workload"] == f"config{workload}" and row["precision"] == precision
+                        and row.get("path", "farfield") == path):
+                    return int(row["dram_read_bytes"]) + int(row["dram_write_bytes"]), row.get("source")
+    except Exception:
+        pass
+    return None, None
+
+
+def measure(ctx, m):
+    """One workload / precision / path through the device-timed and (optionally) the host-buffer legs.
+    ctx: torch, vn, multi, rank, world, local_rank, flush;  m: workload, precision, path, steps, warmup, order, graph, e2e.
+    Returns a dict (every rank; rank 0 prints)."""
+    torch, vn, multi = ctx.torch, ctx.vn, ctx.multi
+    from paper_2606_25569_b200 import inputs
+    rank, world = ctx.rank, ctx.world
+    tdtype = torch.float32 if m.precision == "f32" else torch.float64
+    np_dtype = np.float32 if m.precision == "f32" else np.float64
+    susp = inputs.config(m.workload)                   # every rank generates the same suspension (same seed)
+    seq_np = susp.X_sequence if susp.X_sequence else [susp.X]
+    evals = len(seq_np)
+    P = susp.nves * susp.npts
+    pairs_eval = 512 * 512 * P if m.path == "targets" else susp.pairs
+    vb, ve = multi.shard_range(susp.nves, world, rank)  # this rank's vesicles (everything at world = 1)
+    nloc = ve - vb
+
+    # ---- device-resident inputs (value) and pinned host inputs (e2e): this rank's shard
+    seq_h = [torch.from_numpy(np.ascontiguousarray(x[vb:ve], dtype=np_dtype)).pin_memory() for x in seq_np]
+    F_h = torch.from_numpy(np.ascontiguousarray(susp.F[vb:ve], dtype=np_dtype)).pin_memory()
+    U_h = torch.empty_like(seq_h[0]).pin_memory()
+    seq_d = [x.cuda() for x in seq_h]
+    F_d = F_h.cuda()
+    X_d = torch.empty_like(seq_d[0])
+    W_d = torch.empty((nloc, susp.npts), dtype=tdtype, device="cuda")
+    U_d = torch.empty_like(X_d)
+    fmm_order = m.order or (12 if m.precision == "f32" else 38)
+    if m.path == "masked":                             # CSR buffers sized once (4 near vesicles per point is generous)
+        near_ptr = torch.empty(P + 1, dtype=torch.int64, device="cuda")
+        near_ves = torch.empty(4 * P, dtype=torch.int32, device="cuda")
+    if m.path == "targets":
+        Xt_h = torch.from_numpy(target_grid(susp, 512, np_dtype)).pin_memory()
+        Xt_d = Xt_h.cuda()
+        Ut_d = torch.empty_like(Xt_d)
+        Ut_h = torch.empty_like(Xt_h).pin_memory()
+
+    def evaluate():
+        vn.vn_arclength_weights(X_d, out=W_d)          # a-1 (on the rank's own vesicles)
+        if world > 1:                                   # section 8e: all-gather, partial, reduce-scatter, finish
+            U_d.copy_(multi.sharded_farfield_gpu(vn, X_d, F_d, W_d, susp.nves, susp.mu, rank, world))
+        elif m.path == "farfield":
+            vn.vn_farfield(X_d, F_d, W_d, susp.mu, out=U_d)   # a-2 .. a-5
+        elif m.path == "fmm":
+            vn.vn_farfield_fmm(X_d, F_d, W_d, susp.mu, fmm_order, out=U_d)
+        elif m.path == "masked":
+            vn.vn_near_pairs(X_d, W_d, near_ptr, near_ves)
+            vn.vn_farfield_masked(X_d, F_d, W_d, near_ptr, near_ves, susp.mu, out=U_d)
+        else:
+            vn.vn_farfield_targets(Xt_d, X_d, F_d, W_d, susp.mu, out=Ut_d, fmm_order=m.order)   # --order > 0: FMM
+
+    def step_device():
+        for c in range(evals):
+            X_d.copy_(seq_d[c])                        # device-to-device, same stream
+            evaluate()
+
+    def step_host():
+        for c in range(evals):
+            if m.path == "farfield" and world == 1:
+                vn.vn_farfield_host(seq_h[c], F_h, None, susp.mu, out=U_h)
+            else:                                      # no host entry point for these: explicit copies around the C-ABI calls
+                X_d.copy_(seq_h[c], non_blocking=True)
+                F_d.copy_(F_h, non_blocking=True)
+                if m.path == "targets":
+                    Xt_d.copy_(Xt_h, non_blocking=True)
+                evaluate()
+                if m.path == "targets":
+                    Ut_h.copy_(Ut_d, non_blocking=True)
+                else:
+                    U_h.copy_(U_d, non_blocking=True)
+                torch.cuda.synchronize()
+
+    def barrier():
+        multi.barrier()
+        torch.cuda.synchronize()
+
+    def timed(step_fn, steps, use_events):
+        """K steps; L2 flushed between steps outside the timed intervals.  Returns seconds (sum)."""
+        total = 0.0
+        for _ in range(steps):
+            ctx.flush.fill_(1)
+            barrier()
+            if use_events:
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                step_fn()
+                e1.record()
+                e1.synchronize()
+                total += e0.elapsed_time(e1) * 1e-3
+            else:
+                t0 = time.perf_counter()
+                step_fn()                              # synchronous call (returns after the D2H copy)
+                total += time.perf_counter() - t0
+            barrier()
+        return total
+
+    warm = max(m.warmup, 3)
+    for _ in range(warm):
+        step_device()
+    torch.cuda.synchronize()
+    launches_per_step = None
+    if m.graph:                                        # every call only enqueues stream-ordered work: capturable
+        step_eager = step_device
+        cap = torch.cuda.Stream()
+        cap.wait_stream(torch.cuda.current_stream())
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.stream(cap):
+            step_eager()
+            cap.synchronize()
+            n_cap = vn.vn_launch_count()
+            with torch.cuda.graph(graph, stream=cap):
+                step_eager()
+            launches_per_step = vn.vn_launch_count() - n_cap      # kernels recorded into the graph
+        torch.cuda.synchronize()
+        step_device = graph.replay
+        for _ in range(2):
+            step_device()
+        torch.cuda.synchronize()
+
+    sampler = ClockSampler(nvml_index(ctx.local_rank))
+    sampler.start()
+    vn.vn_profile_enable(True)
+    vn.vn_profile_read()
+    n0 = vn.vn_launch_count()
+    t_dev = timed(step_device, m.steps, True)
+    launches = vn.vn_launch_count() - n0
+    if m.graph:
+        launches = launches_per_step * m.steps               # replayed from the graph, not re-enqueued by the host
+    kernel_ms = vn.vn_profile_read()
+    vn.vn_profile_enable(False)
+    clocks = sampler.stop()
+
+    t_e2e = None
+    if m.e2e:
+        for _ in range(2 if m.path == "farfield" else 1):
+            step_host()
+        t_e2e = timed(step_host, m.steps, False)             # every step timed (none extrapolated)
+
+    n_near = None
+    if m.path == "masked":
+        torch.cuda.synchronize()
+        n_near = int(near_ptr[P].item())
+        if n_near > near_ves.numel():
+            raise SystemExit(f"near relation has {n_near} pairs, buffer holds {near_ves.numel()}")
+    # whole-job numbers: the ranks share one job, so the work is the job's and the time the slowest rank's
+    t_dev = multi.max_over_ranks(t_dev, "cuda")
+    if t_e2e is not None:
+        t_e2e = multi.max_over_ranks(t_e2e, "cuda")
+    pairs_total = m.steps * evals * pairs_eval
+    es = 4 if m.precision == "f32" else 8
+    nt = 512 * 512
+    return SimpleNamespace(susp=susp, evals=evals, P=P, pairs_eval=pairs_eval, value=pairs_total / t_dev / 1e9,
+                           ms_per_step=t_dev / m.steps * 1e3, kernel_ms=kernel_ms, clocks=clocks, launches=int(launches),
+                           e2e=None if t_e2e is None else pairs_total / t_e2e / 1e9, n_near=n_near, fmm_order=fmm_order,
+                           h2d=evals * 2 * es * (2 * P + (nt if m.path == "targets" else 0)),
+                           d2h=evals * 2 * es * (nt if m.path == "targets" else P), warm=warm)
+
+
+def roofline_of(r, m, peaks, world):
+    """The roofline object of one measurement (pair kernel of the exact paths)."""
+    sm_max = r.clocks.get("sm_max_mhz") or measured_peaks().get("sm_max_mhz") or 1965.0
+    lanes = FP32_LANES if m.precision == "f32" else FP64_LANES
+    peak_nominal = SMS * lanes * sm_max * 1e6 / 1e12                   # T lane-instr/s at max clock
+    peak_meas = None
+    if peaks:
+        peak_meas = (peaks["ffma2"] if m.precision == "f32" else peaks["dfma"]) / 1e12
+    k_ms = statistics.mean(r.kernel_ms) if r.kernel_ms else None
+    # with N GPUs each launch of the pair kernel processes 1/N of the blocks
+    pairs_launch = r.pairs_eval / world
+    achieved = LANE_OPS_PER_PAIR * pairs_launch / (k_ms * 1e-3) / 1e12 if k_ms else None
+    executed = EXECUTED_LANE_OPS.get((m.path, m.precision))
+    traffic, traffic_src = traffic_from_profiles(m.workload, m.precision, m.path)
+    pipe = "FP32" if m.precision == "f32" else "FP64"
+    return {"bound": "alu",
+            "kernel": ("targets_%s_kernel" if m.path == "targets" else "farfield_%s_kernel") % m.precision,
+            "achieved": achieved, "peak": peak_nominal,
+            "unit": "T lane-instr/s (%s pipe; 11 CANONICAL lane-instructions per pair -- the symmetric kernels execute "
+                    "fewer, so this fraction can exceed the pipe's busy fraction; its ceiling is 11 / executed_lane_ops_per_pair)" % pipe,
+            "frac": achieved / peak_nominal if achieved else None,
+            "frac_canonical": achieved / peak_nominal if achieved else None,
+            "peak_nominal": peak_nominal,
+            "peak_source": "nominal: 148 SMs x %d lanes x %.0f MHz (guide unit counts, clocks.max.sm); peak_measured is this "
+                           "run's vn_pipe_peaks stream (%s)" % (lanes, sm_max, "FFMA2" if m.precision == "f32" else "DFMA"),
+            "peak_measured": peak_meas,
+            "frac_vs_measured_peak": achieved / peak_meas if achieved and peak_meas else None,
+            "executed_lane_ops_per_pair": executed,
+            "frac_executed": (executed / LANE_OPS_PER_PAIR) * achieved / peak_nominal if achieved and executed else None,
+            "kernel_ms_avg": k_ms, "kernel_launches_timed": len(r.kernel_ms),
+            "kernel_ginteractions_per_s": pairs_launch / (k_ms * 1e-3) / 1e9 if k_ms else None,
+            "flop_frac": (FLOP_PER_PAIR * pairs_launch / (k_ms * 1e-3) / 1e12) / (2 * peak_nominal) if k_ms else None,
+            "frac_at_sampled_clock": (achieved / (SMS * lanes * r.clocks["sm_mhz"] * 1e6 / 1e12)
+                                      if achieved and r.clocks.get("sm_mhz") else None),
+            "hbm_algorithmic_bytes": 28 * r.P if m.precision == "f32" else 56 * r.P,
+            "traffic": traffic, "traffic_source": ("profiles/" + traffic_src) if traffic_src else None}
 
 
 def main():
@@ -312,6 +547,8 @@ def main():
                     help="capture one step (all its evaluations) into a CUDA graph after the warm-up and time graph replays")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-sweep", action="store_true", help="skip the sweep over configs[3] / configs[1] of the default invocation")
+    ap.add_argument("--no-peaks", action="store_true", help="skip the pipe-rate microbenchmark (vn_pipe_peaks)")
     args = ap.parse_args()
     if args.workload == 0:
         args.precision = "f64"          # config 0 is fp64 only
@@ -322,12 +559,15 @@ def main():
     import torch
     import torch.distributed as dist
     import paper_2606_25569_b200 as vn
+    from paper_2606_25569_b200 import inputs, multi
 
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the product has no CPU path")
+    if world > 1 and args.path != "farfield":
+        raise SystemExit("only the farfield path is sharded over GPUs (DESIGN.md section 8); run the other paths with --gpus 1")
     torch.cuda.set_device(local_rank)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
@@ -335,211 +575,73 @@ def main():
 
     tdtype = torch.float32 if args.precision == "f32" else torch.float64
     np_dtype = np.float32 if args.precision == "f32" else np.float64
-    susp = make_workload(args.workload, rank)
     if args.path == "aux":
-        return run_aux(args, susp, vn, torch, tdtype, np_dtype, rank, world, local_rank)
-    seq_np = susp.X_sequence if susp.X_sequence else [susp.X]
-    evals = len(seq_np)
-    P = susp.nves * susp.npts
-    pairs_eval = 512 * 512 * P if args.path == "targets" else susp.pairs
-    pairs_step = evals * pairs_eval
+        return run_aux(args, inputs.config(args.workload), vn, torch, tdtype, np_dtype, rank, world, local_rank)
 
-    # ---- device-resident inputs (value) and pinned host inputs (e2e)
-    seq_h = [torch.from_numpy(np.ascontiguousarray(x, dtype=np_dtype)).pin_memory() for x in seq_np]
-    F_h = torch.from_numpy(np.ascontiguousarray(susp.F, dtype=np_dtype)).pin_memory()
-    U_h = torch.empty_like(seq_h[0]).pin_memory()
-    seq_d = [x.cuda() for x in seq_h]
-    F_d = F_h.cuda()
-    X_d = torch.empty_like(seq_d[0])
-    W_d = torch.empty((susp.nves, susp.npts), dtype=tdtype, device="cuda")
-    U_d = torch.empty_like(X_d)
-    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")
+    ctx = SimpleNamespace(torch=torch, vn=vn, multi=multi, rank=rank, world=world, local_rank=local_rank,
+                          flush=torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda"))
+    m = SimpleNamespace(workload=args.workload, precision=args.precision, path=args.path, steps=args.steps,
+                        warmup=args.warmup, order=args.order, graph=args.graph, e2e=not args.no_e2e)
+    r = measure(ctx, m)
 
-    fmm_order = args.order or (12 if args.precision == "f32" else 38)
-    if args.path == "masked":                          # CSR buffers sized once (4 near vesicles per point is generous)
-        near_ptr = torch.empty(P + 1, dtype=torch.int64, device="cuda")
-        near_ves = torch.empty(4 * P, dtype=torch.int32, device="cuda")
-    if args.path == "targets":
-        Xt_h = torch.from_numpy(target_grid(susp, 512, np_dtype)).pin_memory()
-        Xt_d = Xt_h.cuda()
-        Ut_d = torch.empty_like(Xt_d)
-        Ut_h = torch.empty_like(Xt_h).pin_memory()
-
-    def evaluate():
-        vn.vn_arclength_weights(X_d, out=W_d)          # a-1
-        if args.path == "farfield":
-            vn.vn_farfield(X_d, F_d, W_d, susp.mu, out=U_d)   # a-2 .. a-5
-        elif args.path == "fmm":
-            vn.vn_farfield_fmm(X_d, F_d, W_d, susp.mu, fmm_order, out=U_d)
-        elif args.path == "masked":
-            vn.vn_near_pairs(X_d, W_d, near_ptr, near_ves)
-            vn.vn_farfield_masked(X_d, F_d, W_d, near_ptr, near_ves, susp.mu, out=U_d)
-        else:
-            vn.vn_farfield_targets(Xt_d, X_d, F_d, W_d, susp.mu, out=Ut_d, fmm_order=args.order)   # --order > 0: FMM
-
-    def step_device():
-        for c in range(evals):
-            X_d.copy_(seq_d[c])                        # device-to-device, same stream
-            evaluate()
-
-    def step_host():
-        for c in range(evals):
-            if args.path == "farfield":
-                vn.vn_farfield_host(seq_h[c], F_h, None, susp.mu, out=U_h)
-            else:                                      # no host entry point for the NEXT rows: explicit copies
-                X_d.copy_(seq_h[c], non_blocking=True)
-                F_d.copy_(F_h, non_blocking=True)
-                if args.path == "targets":
-                    Xt_d.copy_(Xt_h, non_blocking=True)
-                evaluate()
-                if args.path == "targets":
-                    Ut_h.copy_(Ut_d, non_blocking=True)
-                else:
-                    U_h.copy_(U_d, non_blocking=True)
-                torch.cuda.synchronize()
-
-    from paper_2606_25569_b200 import multi
-
-    def barrier():
-        multi.barrier()
-        torch.cuda.synchronize()
-
-    def timed(step_fn, steps, use_events):
-        """K steps; L2 flushed between steps outside the timed intervals.  Returns seconds (sum)."""
-        total = 0.0
-        for _ in range(steps):
-            flush.fill_(1)
-            barrier()
-            if use_events:
-                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                e0.record()
-                step_fn()
-                e1.record()
-                e1.synchronize()
-                total += e0.elapsed_time(e1) * 1e-3
-            else:
-                t0 = time.perf_counter()
-                step_fn()                              # synchronous call (returns after the D2H copy)
-                total += time.perf_counter() - t0
-            barrier()
-        return total
-
-    for _ in range(max(args.warmup, 3)):
-        step_device()
-    torch.cuda.synchronize()
-    step_eager = step_device
-    if args.graph:                                     # every call only enqueues stream-ordered work: capturable
-        cap = torch.cuda.Stream()
-        cap.wait_stream(torch.cuda.current_stream())
-        graph = torch.cuda.CUDAGraph()
-        with torch.cuda.stream(cap):
-            step_eager()
-            cap.synchronize()
-            n_cap = vn.vn_launch_count()
-            with torch.cuda.graph(graph, stream=cap):
-                step_eager()
-            launches_per_step = vn.vn_launch_count() - n_cap      # kernels recorded into the graph
-        torch.cuda.synchronize()
-        step_device = graph.replay
-        for _ in range(2):
-            step_device()
-        torch.cuda.synchronize()
-
-    sampler = ClockSampler(nvml_index(local_rank))
-    sampler.start()
-    vn.vn_profile_enable(True)
-    vn.vn_profile_read()
-    n0 = vn.vn_launch_count()
-    t_dev = timed(step_device, args.steps, True)
-    launches = vn.vn_launch_count() - n0
-    if args.graph:
-        launches = launches_per_step * args.steps            # replayed from the graph, not re-enqueued by the host
-    kernel_ms = vn.vn_profile_read()
-    vn.vn_profile_enable(False)
-    sampler.stop_flag.set()
-    sampler.join()
-
-    t_e2e = None
-    if not args.no_e2e:
-        for _ in range(3 if args.path == "farfield" else 1):
-            step_host()
-        t_e2e = timed(step_host, max(1, min(args.steps, 2)), False) / max(1, min(args.steps, 2)) * args.steps
-
-    if args.path == "masked":
-        torch.cuda.synchronize()
-        n_near = int(near_ptr[P].item())
-        if n_near > near_ves.numel():
-            raise SystemExit(f"near relation has {n_near} pairs, buffer holds {near_ves.numel()}")
-    # whole-job numbers: work summed over ranks, time = the slowest rank (paper_2606_25569_b200/multi.py)
-    rate_dev, t_dev, _ = multi.whole_job_rate(args.steps * pairs_step, t_dev, "cuda")
-    if t_e2e is not None:
-        rate_e2e, t_e2e, _ = multi.whole_job_rate(args.steps * pairs_step, t_e2e, "cuda")
+    default_run = (world == 1 and args.path == "farfield" and args.workload == 4 and args.precision == "f32"
+                   and not args.graph)
+    peaks = None
+    if not args.no_peaks and world == 1:
+        sampler = ClockSampler(nvml_index(local_rank))
+        sampler.start()
+        peaks = vn.vn_pipe_peaks()
+        peaks["clocks"] = sampler.stop()
+    sweep = []
+    if default_run and not args.no_sweep:              # the other configurations north_star's target names, same run
+        for w, prec, steps in ((3, "f32", 10), (3, "f64", 5), (1, "f32", 20)):
+            ms = SimpleNamespace(workload=w, precision=prec, path="farfield", steps=steps, warmup=3, order=0,
+                                 graph=False, e2e=False)
+            rs = measure(ctx, ms)
+            rl = roofline_of(rs, ms, peaks, 1)
+            sweep.append({"workload": f"BASELINE.json configs[{w}]: {rs.susp.name}", "precision": prec, "value": rs.value,
+                          "unit": UNIT, "steps": steps, "ms_per_step": rs.ms_per_step, "kernel_ms_avg": rl["kernel_ms_avg"],
+                          "frac": rl["frac"], "frac_vs_measured_peak": rl["frac_vs_measured_peak"],
+                          "frac_executed": rl["frac_executed"], "clocks": rs.clocks, "gpu_launches": rs.launches})
 
     if rank == 0:
-        value = rate_dev / 1e9
-        clocks = sampler.summary()
-        peaks = measured_peaks()
-        sm_max = clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz") or 1965.0
-        lanes = FP32_LANES if args.precision == "f32" else FP64_LANES
-        peak_lane = SMS * lanes * sm_max * 1e6 / 1e12                     # T lane-instr/s at max clock
-        k_ms = statistics.mean(kernel_ms) if kernel_ms else None
-        achieved = LANE_OPS_PER_PAIR * pairs_eval / (k_ms * 1e-3) / 1e12 if k_ms else None
-        traffic = None                                   # dram bytes per launch from the committed ncu --set full capture
-        try:
-            import csv
-            with open(os.path.join(ROOT, "profiles", "traffic.csv")) as fh:
-                for row in csv.DictReader(fh):
-                    if (row["workload"] == f"config{args.workload}" and row["precision"] == args.precision
-                            and row.get("path", "farfield") == args.path):
-                        traffic = int(row["dram_read_bytes"]) + int(row["dram_write_bytes"])
-        except Exception:
-            pass
-        roofline = {"bound": "alu",
-                    "kernel": ("fmm kernels (P2M, M2M, M2L, L2L, L2P+P2P)" if args.path == "fmm" else
-                               ("targets_%s_kernel" if args.path == "targets" else "farfield_%s_kernel") % args.precision),
-                    "achieved": achieved, "peak": peak_lane,
-                    "unit": "T lane-instr/s (%s pipe; 11 canonical instr per pair)" % ("FP32" if args.precision == "f32" else "FP64"),
-                    "frac": achieved / peak_lane if achieved else None,
-                    "peak_source": "derived: 148 SMs x %d lanes x %.0f MHz (guide unit counts, clocks.max.sm); "
-                                   "MEASURED_PEAKS.json holds only HBM/bf16 peaks" % (lanes, sm_max),
-                    "kernel_ms_avg": k_ms, "kernel_launches_timed": len(kernel_ms),
-                    "kernel_ginteractions_per_s": pairs_eval / (k_ms * 1e-3) / 1e9 if k_ms else None,
-                    "flop_frac": (FLOP_PER_PAIR * pairs_eval / (k_ms * 1e-3) / 1e12) / (2 * peak_lane) if k_ms else None,
-                    "frac_at_sampled_clock": (achieved / (SMS * lanes * clocks["sm_mhz"] * 1e6 / 1e12)
-                                              if achieved and clocks.get("sm_mhz") else None),
-                    "hbm_algorithmic_bytes": 28 * P if args.precision == "f32" else 56 * P,
-                    "traffic": traffic}
-        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-                "warmup": max(args.warmup, 3), "ms_per_step": t_dev / args.steps * 1e3, "higher_is_better": True,
-                "scaling": "weak", "vs_baseline": None, "dtype": args.precision, "data": "synthetic",
-                "config": workload_config(args, susp), "clocks": clocks, "gpu_launches": int(launches),
-                "roofline": roofline}
-        if t_e2e is not None:
-            es = 4 if args.precision == "f32" else 8
-            nt = 512 * 512
-            line["e2e"] = {"value": rate_e2e / 1e9, "unit": UNIT,
-                           "h2d_bytes_per_step": evals * 2 * es * (2 * P + (nt if args.path == "targets" else 0)),
-                           "d2h_bytes_per_step": evals * 2 * es * (nt if args.path == "targets" else P),
+        line = {"metric": METRIC, "value": r.value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": r.warm, "ms_per_step": r.ms_per_step, "higher_is_better": True,
+                "scaling": "strong", "vs_baseline": None, "dtype": args.precision, "data": "synthetic",
+                "config": workload_config(args, r.susp), "clocks": r.clocks, "gpu_launches": r.launches,
+                "roofline": roofline_of(r, m, peaks, world)}
+        if peaks:
+            sms = peaks["sms"]
+            line["pipe_peaks"] = {"unit": "lane-ops per clock per SM at clocks.sm_max_mhz (nominal 128 / 128 / 16 / 64)",
+                                  **{k: peaks[k] / (sms * (peaks["clocks"].get("sm_max_mhz") or 1965.0) * 1e6)
+                                     for k in ("ffma2", "ffma", "mufu", "dfma", "ffma2_noreuse", "dfma_noreuse")},
+                                  "lane_ops_per_s": {k: peaks[k] for k in ("ffma2", "ffma", "mufu", "dfma", "ffma2_noreuse", "dfma_noreuse")},
+                                  "sms": sms, "clocks": peaks["clocks"]}
+        if r.e2e is not None:
+            line["e2e"] = {"value": r.e2e, "unit": UNIT, "h2d_bytes_per_step": r.h2d // world, "d2h_bytes_per_step": r.d2h // world,
+                           "steps_timed": args.steps,
                            "api": "vn_farfield_host (pinned host buffers; weights computed on device)"
-                                  if args.path == "farfield" else
-                                  "pinned host buffers -> device copies -> the path's C-ABI calls -> copy back, synchronised"}
+                                  if args.path == "farfield" and world == 1 else
+                                  "pinned host buffers -> device copies -> the path's C-ABI calls -> copy back, synchronised"
+                                  + (" (bytes per rank)" if world > 1 else "")}
         if args.path == "masked":
-            line["config"]["near_pairs"] = n_near
+            line["config"]["near_pairs"] = r.n_near
         if args.path == "fmm" or (args.path == "targets" and args.order > 0):
             # an approximate O(P) algorithm does not execute the direct sum's interactions: no ALU roofline fraction
             # is claimed for it; `value` is the direct sum's pair count over the FMM's time ("equivalent" rate)
-            line["config"]["order"] = fmm_order if args.path == "fmm" else args.order
+            line["config"]["order"] = r.fmm_order if args.path == "fmm" else args.order
             rl = line["roofline"]
             rl["kernel"] = "fmm kernels (P2M, M2M, M2L, L2L, L2P+P2P); kernel_ms_avg spans all of them"
             rl["equivalent_ginteractions_per_s"] = rl.pop("kernel_ginteractions_per_s", None)
-            for k in ("achieved", "frac", "flop_frac", "frac_at_sampled_clock"):
+            for k in ("achieved", "frac", "frac_canonical", "flop_frac", "frac_at_sampled_clock", "frac_vs_measured_peak",
+                      "frac_executed", "executed_lane_ops_per_pair"):
                 rl[k] = None
             rl["note"] = ("approximate algorithm (expansion order in config.order): no fraction of the pair kernels' "
-                          "instruction roofline is claimed; see profiles/r1f_fmm_kernels_config4_f64_ncu.md for the "
-                          "FP64-pipe occupancy of its two dominant kernels")
+                          "instruction roofline is claimed; see profiles/ for the FP64-pipe occupancy of its dominant kernels")
+        if sweep:
+            line["sweep"] = sweep
         if world == 1 and not args.no_cpu_baseline:
-            v, cores, sample = oracle_rate(susp, np_dtype, 15.0, 4242, args.path)
-            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+            line["cpu_baseline"] = cpu_baseline(r.susp, np_dtype, args.path)
         print(json.dumps(line), flush=True)
 
     if world > 1:

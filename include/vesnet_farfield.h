@@ -216,14 +216,36 @@ vn_status vn_redistribute_arclength(const void *X, int64_t nves, int64_t npts, v
 vn_status vn_profile_enable(int enable);
 int64_t vn_profile_read(double *ms, int64_t max_entries);
 
+/* One suspension on several GPUs.  The pair kernel evaluates every
+ * unordered pair of points once and scatters into both points' accumulators, so the work is dealt out by BLOCKS of
+ * the pair walk, not by targets: with all sources known to every device (one all-gather of X, F, W), device `part`
+ * of `nparts` runs vn_farfield_partial, which executes blocks part, part + nparts, ... of the same grid vn_farfield
+ * would run and leaves the RAW fixed-point accumulators in acc: 2 (VN_F32) or 4 (VN_F64) 64-bit integer words per
+ * point, [nves*npts*2] or [nves*npts*4] int64, overwritten.  Integer addition is associative, so summing the
+ * parts' accumulators word by word in any order (one integer reduce-scatter over the devices, 16 / 32 bytes per
+ * point) gives bit for bit the accumulators of the single-device call.  vn_farfield_finish then turns any
+ * contiguous range of `count` points of summed accumulators (pointer to the first word of the range) into
+ * velocities U[count,2]: scale by 1/(4 pi mu), round once.  gmax (8 bytes, 8-byte aligned, written by
+ * vn_farfield_partial, identical on every device because every device packs all sources) carries the scale of
+ * the fixed-point format; npoints_total = nves*npts of the whole suspension.  part = 0, nparts = 1 followed by
+ * vn_farfield_finish over all points IS vn_farfield.  All pointers are DEVICE pointers; asynchronous on `stream`.
+ * VN_ERR_INVALID_ARG additionally for part < 0, nparts < 1, part >= nparts, count < 0. */
+vn_status vn_farfield_partial(const void *X, const void *F, const void *W, int64_t nves, int64_t npts,
+                              int32_t part, int32_t nparts, void *acc, void *gmax,
+                              vn_precision precision, void *stream);
+vn_status vn_farfield_finish(const void *acc, const void *gmax, int64_t npoints_total, int64_t count, double mu,
+                             void *U, vn_precision precision, void *stream);
+
 /* Measured issue rates of the arithmetic pipes that bound the pair kernels (the nominal
- * lane counts "must be confirmed by microbenchmark").  Runs four register-only stream
- * kernels of this library on `stream` (about 40 ms in all), waits for them, and writes into the HOST array
- * rates[5]: lane-operations per second of [0] packed FFMA2 (fma.rn.f32x2, counted as two per thread),
- * [1] FFMA, [2] MUFU (rcp.approx and lg2.approx, half each), [3] DFMA; [4] the device's SM count.
+ * lane counts "must be confirmed by microbenchmark").  Runs six register-only stream
+ * kernels of this library on `stream` (about 60 ms in all), waits for them, and writes into the HOST array
+ * rates[8]: lane-operations per second of [0] packed FFMA2 (fma.rn.f32x2, counted as two per thread),
+ * [1] FFMA, [2] MUFU (rcp.approx and lg2.approx, half each), [3] DFMA; [4] the device's SM count; [5], [6] FFMA2
+ * and DFMA streams whose three operands are different registers in every instruction (no operand reuse between
+ * neighbours: what the register file feeds the pipes when all inputs change); [7] zero (reserved).
  * The best of three launch shapes (16 / 32 / 64 warps per SM, eight independent chains per thread) is reported.
  * Synchronous; not capturable into a graph.  bench.py calls it once per run for roofline.peak_measured. */
-vn_status vn_pipe_peaks(double *rates /* HOST, 5 entries */, void *stream);
+vn_status vn_pipe_peaks(double *rates /* HOST, 8 entries */, void *stream);
 
 /* Host-only introspection (no CUDA call, works without a GPU): the work decomposition vn_farfield would use
  * for nves x npts points when `resident_blocks` blocks of the pair kernel fit on the device at once

@@ -78,6 +78,10 @@ def lib():
         L.vn_launch_count.restype = i64
         L.vn_status_string.argtypes = [ci]
         L.vn_status_string.restype = ctypes.c_char_p
+        L.vn_farfield_partial.argtypes = [vp, vp, vp, i64, i64, ctypes.c_int32, ctypes.c_int32, vp, vp, ci, vp]
+        L.vn_farfield_partial.restype = ci
+        L.vn_farfield_finish.argtypes = [vp, vp, i64, i64, dbl, vp, ci, vp]
+        L.vn_farfield_finish.restype = ci
         L.vn_pipe_peaks.argtypes = [ctypes.POINTER(dbl), vp]
         L.vn_pipe_peaks.restype = ci
         L.vn_version.argtypes = []
@@ -129,6 +133,57 @@ def vn_farfield(X, F, W, mu: float = 1.0, out=None, stream=None):
                                out.data_ptr(), _prec(X), _stream_ptr(stream))
     if rc != VN_OK:
         raise VesnetError(rc, "vn_farfield")
+    return out
+
+
+def acc_words(dtype) -> int:
+    """64-bit accumulator words per point of vn_farfield_partial: 2 for float32, 4 for float64."""
+    import torch
+    return 2 if dtype == torch.float32 else 4
+
+
+def vn_farfield_partial(X, F, W, part: int, nparts: int, acc=None, gmax=None, stream=None):
+    """Raw fixed-point accumulators of the blocks of part `part` of `nparts` (device tensors).
+    Returns (acc int64 [nves*npts*words], gmax int64 [1])."""
+    import torch
+    nves, npts, two = X.shape
+    if two != 2:
+        raise ValueError("X must be [nves, npts, 2]")
+    _check_dev("X", X)
+    _check_dev("F", F, X.shape, X.dtype)
+    _check_dev("W", W, (nves, npts), X.dtype)
+    n = nves * npts * acc_words(X.dtype)
+    if acc is None:
+        acc = torch.empty(n, dtype=torch.int64, device=X.device)
+    if gmax is None:
+        gmax = torch.empty(1, dtype=torch.int64, device=X.device)
+    _check_dev("acc", acc, (n,), torch.int64)
+    _check_dev("gmax", gmax, (1,), torch.int64)
+    with torch.cuda.device(X.device):
+        rc = lib().vn_farfield_partial(X.data_ptr(), F.data_ptr(), W.data_ptr(), nves, npts, int(part), int(nparts),
+                                       acc.data_ptr(), gmax.data_ptr(), _prec(X), _stream_ptr(stream))
+    if rc != VN_OK:
+        raise VesnetError(rc, "vn_farfield_partial")
+    return acc, gmax
+
+
+def vn_farfield_finish(acc, gmax, npoints_total: int, dtype, mu: float = 1.0, out=None, stream=None):
+    """U[count, 2] from a contiguous range of summed accumulators (count = acc.numel() / words per point)."""
+    import torch
+    _check_dev("acc", acc, None, torch.int64)
+    _check_dev("gmax", gmax, (1,), torch.int64)
+    count = acc.numel() // acc_words(dtype)
+    if out is None:
+        out = torch.empty((count, 2), dtype=dtype, device=acc.device)
+    _check_dev("out", out, None, dtype)
+    if out.numel() != 2 * count:
+        raise ValueError("out must hold count x 2 values")
+    with torch.cuda.device(acc.device):
+        rc = lib().vn_farfield_finish(acc.data_ptr() if count else None, gmax.data_ptr(), int(npoints_total), count,
+                                      float(mu), out.data_ptr() if count else None,
+                                      VN_F32 if dtype == torch.float32 else VN_F64, _stream_ptr(stream))
+    if rc != VN_OK:
+        raise VesnetError(rc, "vn_farfield_finish")
     return out
 
 
@@ -357,11 +412,12 @@ def vn_profile_read(max_entries: int = 4096):
 
 def vn_pipe_peaks(stream=None):
     """Measured pipe rates in lane-operations per second: dict(ffma2, ffma, mufu, dfma, sms).  Synchronous."""
-    buf = (ctypes.c_double * 5)()
+    buf = (ctypes.c_double * 8)()
     rc = lib().vn_pipe_peaks(buf, _stream_ptr(stream))
     if rc != VN_OK:
         raise VesnetError(rc, "vn_pipe_peaks")
-    return dict(ffma2=buf[0], ffma=buf[1], mufu=buf[2], dfma=buf[3], sms=int(buf[4]))
+    return dict(ffma2=buf[0], ffma=buf[1], mufu=buf[2], dfma=buf[3], sms=int(buf[4]), ffma2_noreuse=buf[5],
+                dfma_noreuse=buf[6])
 
 
 def vn_launch_count() -> int:

@@ -49,6 +49,14 @@ vn_status near_pairs(const void *X, const void *W, int64_t nves, int64_t npts, i
                      int32_t *near_ves, int64_t capacity, vn_precision prec, cudaStream_t st);
 vn_status arclength_weights(const void *X, int64_t nves, int64_t npts, void *W, vn_precision prec, cudaStream_t st);
 vn_status pipe_peaks(double *rates, cudaStream_t st);
+vn_status farfield_partial_f32(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, int part,
+                               int nparts, void *acc, void *gmax, cudaStream_t st);
+vn_status farfield_partial_f64(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, int part,
+                               int nparts, void *acc, void *gmax, cudaStream_t st);
+vn_status farfield_finish_f32(const void *acc, const void *gmax, int64_t P_total, int64_t count, double mu, void *U,
+                              cudaStream_t st);
+vn_status farfield_finish_f64(const void *acc, const void *gmax, int64_t P_total, int64_t count, double mu, void *U,
+                              cudaStream_t st);
 
 Split choose_split_for(int n_tb, int n_tiles, int slots, int min_tiles)
 {
@@ -356,6 +364,40 @@ vn_status vn_plan_farfield(int64_t nves, int64_t npts, vn_precision precision, i
     plan[3] = sp.n_chunks;
     plan[4] = kTile;
     return VN_OK;
+}
+
+vn_status vn_farfield_partial(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, int32_t part,
+                              int32_t nparts, void *acc, void *gmax, vn_precision precision, void *stream)
+{
+    if (!X || !F || !W || !acc || !gmax) return VN_ERR_INVALID_ARG;
+    if (check_shape(nves, npts, precision) != VN_OK) return VN_ERR_INVALID_ARG;
+    if (nparts < 1 || part < 0 || part >= nparts) return VN_ERR_INVALID_ARG;
+    const size_t pair = precision == VN_F32 ? 8 : 16;
+    if (misaligned(X, pair) || misaligned(F, pair) || misaligned(W, pair / 2) || misaligned(acc, 16) || misaligned(gmax, 8))
+        return VN_ERR_INVALID_ARG;
+    if (acc == X || acc == F || acc == W || gmax == acc) return VN_ERR_INVALID_ARG;
+    const vn_status ds = check_device();
+    if (ds != VN_OK) return ds;
+    cudaStream_t st = (cudaStream_t)stream;
+    return precision == VN_F32 ? farfield_partial_f32(X, F, W, nves, npts, part, nparts, acc, gmax, st)
+                               : farfield_partial_f64(X, F, W, nves, npts, part, nparts, acc, gmax, st);
+}
+
+vn_status vn_farfield_finish(const void *acc, const void *gmax, int64_t npoints_total, int64_t count, double mu, void *U,
+                             vn_precision precision, void *stream)
+{
+    if (precision != VN_F32 && precision != VN_F64) return VN_ERR_INVALID_ARG;
+    if (npoints_total < 1 || npoints_total >= (1ll << 31) || count < 0 || count > npoints_total) return VN_ERR_INVALID_ARG;
+    if (!isfinite(mu) || !(mu > 0.0)) return VN_ERR_INVALID_ARG;
+    if (count == 0) return VN_OK;
+    if (!acc || !gmax || !U) return VN_ERR_INVALID_ARG;
+    if (misaligned(acc, 16) || misaligned(gmax, 8) || misaligned(U, precision == VN_F32 ? 8 : 16) || U == acc)
+        return VN_ERR_INVALID_ARG;
+    const vn_status ds = check_device();
+    if (ds != VN_OK) return ds;
+    cudaStream_t st = (cudaStream_t)stream;
+    return precision == VN_F32 ? farfield_finish_f32(acc, gmax, npoints_total, count, mu, U, st)
+                               : farfield_finish_f64(acc, gmax, npoints_total, count, mu, U, st);
 }
 
 vn_status vn_pipe_peaks(double *rates, void *stream)

@@ -87,7 +87,7 @@ template <int NP>
 __global__ void __launch_bounds__(kThreads, VN_F32_MINBLK)
 farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict__ X, int P, int npts,
                     int n_tiles, int n_st, int n_chunks, const unsigned *__restrict__ gmax_bits,
-                    long long *__restrict__ acc)
+                    long long *__restrict__ acc, int part, int nparts)
 {
     constexpr int T = 2 * NP;
     __shared__ __align__(128) ulonglong2 tile[kStages][kTile * 2];
@@ -96,8 +96,9 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
 
     const int tid = threadIdx.x;
     const int lane = tid & 31;
-    const int I = blockIdx.x / n_chunks;
-    const int sc = blockIdx.x - I * n_chunks;
+    const int bid = blockIdx.x * nparts + part;      // blocks are dealt round-robin to the parts (one part per GPU)
+    const int I = bid / n_chunks;
+    const int sc = bid - I * n_chunks;
     int S = (n_st - 1) / 2;
     if ((n_st & 1) == 0 && I < n_st / 2) S += 1;
     const int nu = kSub32 * (S + 1);
@@ -403,10 +404,10 @@ __global__ void finish_f32(const long long *__restrict__ acc, int n, int P, cons
 }
 
 // ------------------------------------------------------------------------------------------------
-vn_status farfield_f32(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, double mu,
-                       void *U, cudaStream_t st, const int64_t *near_ptr, const int32_t *near_ves)
+// pack + pair kernel for the blocks of one part: acc (P x 2 words) and gmax are the caller's, already zeroed
+static vn_status accumulate_f32(const void *X, const void *F, const void *W, int P, int npts, int part, int nparts,
+                                ulonglong2 *src, long long *acc, unsigned *gmax, cudaStream_t st)
 {
-    const int P = (int)(nves * npts);
     static int slots_dev[kMaxDevices] = {0};
     int &slots = slots_dev[current_device()];
     if (slots == 0) {
@@ -416,8 +417,25 @@ vn_status farfield_f32(const void *X, const void *F, const void *W, int64_t nves
         VN_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, farfield_f32_kernel<kNP32>, kThreads, 0));
         slots = sms * (occ > 0 ? occ : 1);
     }
+    // the grid is the single-device grid whatever nparts is: the blocks' own roundings are then the same and the
+    // summed accumulators bit for bit those of vn_farfield (the chunk length tuned for one device costs 0.3 % on 8)
     const SymSplit sp = choose_sym_split(P, kST32, slots, VN_F32_MINTILES, 0);
+    const long long blocks = (long long)sp.n_st * sp.n_chunks;
+    const int mine = (int)((blocks - part + nparts - 1) / nparts);
+    pack_sources_f32<<<(P + 255) / 256, 256, 0, st>>>((const float2 *)X, (const float2 *)F, (const float *)W, P, src, gmax);
+    profile_mark(st, true);
+    if (mine > 0)
+        farfield_f32_kernel<kNP32><<<mine, kThreads, 0, st>>>(src, (const float2 *)X, P, npts, sp.n_tiles, sp.n_st,
+                                                              sp.n_chunks, gmax, acc, part, nparts);
+    profile_mark(st, false);
+    count_launch(mine > 0 ? 2 : 1);
+    return VN_OK;
+}
 
+vn_status farfield_f32(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, double mu,
+                       void *U, cudaStream_t st, const int64_t *near_ptr, const int32_t *near_ves)
+{
+    const int P = (int)(nves * npts);
     // scratch: packed sources | fixed-point accumulators | gmax
     const size_t b_src = (size_t)P * 32, b_acc = (size_t)P * 16;
     char *scratch = nullptr;
@@ -426,21 +444,41 @@ vn_status farfield_f32(const void *X, const void *F, const void *W, int64_t nves
     long long *acc = (long long *)(scratch + b_src);
     unsigned *gmax = (unsigned *)(scratch + b_src + b_acc);
     VN_CUDA(cudaMemsetAsync(acc, 0, b_acc + 16, st));
-
-    pack_sources_f32<<<(P + 255) / 256, 256, 0, st>>>((const float2 *)X, (const float2 *)F, (const float *)W, P, src, gmax);
-    profile_mark(st, true);
-    farfield_f32_kernel<kNP32><<<sp.n_st * sp.n_chunks, kThreads, 0, st>>>(src, (const float2 *)X, P, (int)npts,
-                                                                          sp.n_tiles, sp.n_st, sp.n_chunks, gmax, acc);
-    profile_mark(st, false);
-    if (near_ptr) {   // row f-1: take the near vesicles' contributions out again before the final rounding
-        const vn_status rc = near_correction_f32(X, F, W, P, (int)npts, near_ptr, near_ves, acc, gmax, st);
-        if (rc != VN_OK) { (void)cudaFreeAsync(scratch, st); return rc; }
-    }
+    vn_status rc = accumulate_f32(X, F, W, P, (int)npts, 0, 1, src, acc, gmax, st);
+    if (rc == VN_OK && near_ptr)   // row f-1: take the near vesicles' contributions out again before the final rounding
+        rc = near_correction_f32(X, F, W, P, (int)npts, near_ptr, near_ves, acc, gmax, st);
+    if (rc != VN_OK) { (void)cudaFreeAsync(scratch, st); return rc; }
     finish_f32<<<(P + 255) / 256, 256, 0, st>>>(acc, P, P, gmax, 1.0 / (4.0 * 3.14159265358979323846 * mu), (float2 *)U);
-    count_launch(3);
+    count_launch(1);
     const cudaError_t e = cudaGetLastError();
     VN_CUDA(cudaFreeAsync(scratch, st));
     return e == cudaSuccess ? VN_OK : VN_ERR_CUDA;
+}
+
+// Section 8e building blocks: the accumulators of the blocks of part `part` of `nparts` (all sources known to the
+// caller), and the final step on any contiguous range of (summed) accumulators.
+vn_status farfield_partial_f32(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, int part,
+                               int nparts, void *acc, void *gmax, cudaStream_t st)
+{
+    const int P = (int)(nves * npts);
+    ulonglong2 *src = nullptr;
+    VN_CUDA(cudaMallocAsync((void **)&src, (size_t)P * 32, st));
+    VN_CUDA(cudaMemsetAsync(acc, 0, (size_t)P * 16, st));
+    VN_CUDA(cudaMemsetAsync(gmax, 0, 8, st));
+    const vn_status rc = accumulate_f32(X, F, W, P, (int)npts, part, nparts, src, (long long *)acc, (unsigned *)gmax, st);
+    const cudaError_t e = cudaGetLastError();
+    VN_CUDA(cudaFreeAsync(src, st));
+    return rc != VN_OK ? rc : (e == cudaSuccess ? VN_OK : VN_ERR_CUDA);
+}
+
+vn_status farfield_finish_f32(const void *acc, const void *gmax, int64_t P_total, int64_t count, double mu, void *U,
+                              cudaStream_t st)
+{
+    finish_f32<<<(int)((count + 255) / 256), 256, 0, st>>>((const long long *)acc, (int)count, (int)P_total,
+                                                           (const unsigned *)gmax,
+                                                           1.0 / (4.0 * 3.14159265358979323846 * mu), (float2 *)U);
+    count_launch(1);
+    return cudaGetLastError() == cudaSuccess ? VN_OK : VN_ERR_CUDA;
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -19,7 +19,7 @@
 namespace vn {
 
 #ifndef VN_F64_T
-#define VN_F64_T 4
+#define VN_F64_T 6                // measured at 2000 x 128 with 2 blocks/SM: 4 targets 1057, 6 targets 1091, 8 targets 1090 GInt/s
 #endif
 constexpr int kT64 = VN_F64_T;                // targets per thread
 constexpr int kST64 = kT64 * kThreads;        // points per super-tile (target block): 512
@@ -28,8 +28,8 @@ constexpr int kSub64 = kST64 / kTile;         // source tiles per super-tile: 4
 #define VN_F64_BATCH 8
 #endif
 #ifndef VN_F64_MINBLK
-#define VN_F64_MINBLK 3
-#endif
+#define VN_F64_MINBLK 2           // 2 blocks/SM (up to 255 registers, no spills) beat 3 (168 registers): more independent
+#endif                            // pairs in flight per warp matter more to the FP64 pipe than more warps
 #ifndef VN_F64_GTAB
 #define VN_F64_GTAB 1             // the pair kernel's blocks copy the log tables from scratch (built once per call by
 #endif                            // pack_sources_f64 with the same code) instead of building them: +1 % at 2000 x 128,
@@ -41,6 +41,10 @@ constexpr int kSub64 = kST64 / kTile;         // source tiles per super-tile: 4
 #ifndef VN_F64_MAXTILES
 #define VN_F64_MAXTILES kStages   // cap of the chunk length (0: none)
 #endif
+#ifndef VN_F64_SMEMRED
+#define VN_F64_SMEMRED 1          // 1: the j <- i contributions of a batch are summed over the warp through a transposed
+#endif                            // shared-memory buffer (16 STS.64 + 8 LDS.128 + 2 SHFL) instead of the register
+                                  // transpose-reduce (32 SHFL + 60 FSEL + 45 MOV for 64-bit values)
 #ifndef VN_TGT64_LASTOUT
 #define VN_TGT64_LASTOUT 1         // free-target kernel: the last warp out of a ring stage refills it (stage_last_out);
 #endif                             // measured 719 against 696 GInt/s at 2000 x 128 sources, 512 x 512 targets
@@ -48,6 +52,13 @@ constexpr int kSub64 = kST64 / kTile;         // source tiles per super-tile: 4
 #define VN_F64_MINTILES 1
 #endif
 constexpr int kBatch64 = VN_F64_BATCH;        // sources per cross-lane reduction batch
+// shared-memory layout of the fp64 kernels (dynamic)
+constexpr int kPairTileBytes = kStages * kTile * 32;
+constexpr int kTabBytes = (kLogTab + kExpTab) * 8;
+constexpr int kRedRow = 36, kRedHalf = 18;
+constexpr int kRedBytes = VN_F64_SMEMRED ? (kThreads / 32) * 2 * kBatch64 * kRedRow * 8 : 0;
+constexpr int kPairSmem = kPairTileBytes + kRedBytes;      // dynamic part; the tables (kTabBytes) are static
+constexpr int kTgtSmem = kPairTileBytes;
 
 // a-2: one 32-byte record (yx, yy, gx, gy) per source, g = F*W; also gmax = max_j (|gx| + |gy|)
 // (the bit pattern of a non-negative double orders like the double).
@@ -81,24 +92,33 @@ __global__ void pack_sources_f64(const double2 *__restrict__ X, const double2 *_
 __global__ void __launch_bounds__(kThreads, VN_F64_MINBLK)
 farfield_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__ X, int P, int npts,
                     int n_tiles, int n_st, int n_chunks, const unsigned long long *__restrict__ gmax_bits,
-                    long long *__restrict__ acc, const double2 *__restrict__ gtab)
+                    long long *__restrict__ acc, const double2 *__restrict__ gtab, int part, int nparts)
 {
     constexpr int T = kT64;
     constexpr int B = kBatch64;
     constexpr int kDup = 32 / (2 * B);              // lanes that end up with the same reduced value
-    __shared__ __align__(128) double4 tile[kStages][kTile];
+    // the log tables are static shared memory (their addresses fold into the lookups as immediates); the tile ring
+    // and the reduction buffer are dynamic (together with the tables more than the 48 KB a kernel may declare)
+    extern __shared__ __align__(128) unsigned char smem_f64[];
+    double4 (*tile)[kTile] = reinterpret_cast<double4 (*)[kTile]>(smem_f64);
+    __shared__ __align__(16) double tab[kLogTab + kExpTab];
     __shared__ __align__(8) u64 full_bar[kStages];
 #if VN_F64_LASTOUT
     __shared__ int drained[kStages];                 // warps that have left each stage (stage_last_out)
 #else
     __shared__ __align__(8) u64 empty_bar[kStages];
 #endif
-    __shared__ double tab[kLogTab + kExpTab];
+#if VN_F64_SMEMRED
+    // per warp: 2B rows (values) of 32 lanes; 16-byte loads of half rows are conflict-free with a half offset of
+    // 18 doubles and a row stride of 36 (bank shifts of 4 and 8 words)
+    double (*red)[2 * B * kRedRow] = reinterpret_cast<double (*)[2 * B * kRedRow]>(smem_f64 + kPairTileBytes);
+#endif
 
     const int tid = threadIdx.x;
     const int lane = tid & 31;
-    const int I = blockIdx.x / n_chunks;
-    const int sc = blockIdx.x - I * n_chunks;
+    const int bid = blockIdx.x * nparts + part;      // blocks are dealt round-robin to the parts (one part per GPU)
+    const int I = bid / n_chunks;
+    const int sc = bid - I * n_chunks;
     int S = (n_st - 1) / 2;
     if ((n_st & 1) == 0 && I < n_st / 2) S += 1;
     const int nu = kSub64 * (S + 1);
@@ -216,6 +236,30 @@ farfield_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__
                     c[2 * jj + 0] = cx;
                     c[2 * jj + 1] = cy;
                 }
+#if VN_F64_SMEMRED
+                // sum over the warp through shared memory: lane L stores value v at row v, column L; then lane L
+                // adds up half (L & 1) of row L >> 1 and the two halves meet in one shuffle: lane L ends with the
+                // warp total of value L / 2 (kDup = 2 at B = 8)
+                static_assert(kDup == 2, "shared-memory reduction assumes 16 values per batch");
+                {
+                    double *rw = red[tid >> 5];
+                    const int col = lane + (lane >= 16 ? kRedHalf - 16 : 0);
+                    __syncwarp();                                   // the previous batch's reads are done
+#pragma unroll
+                    for (int v = 0; v < 2 * B; ++v) rw[v * kRedRow + col] = c[v];
+                    __syncwarp();
+                    const double2 *row = reinterpret_cast<const double2 *>(rw + (lane >> 1) * kRedRow + (lane & 1) * kRedHalf);
+                    double s0 = 0.0, s1 = 0.0;
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) {
+                        const double2 v = row[q];
+                        s0 += v.x;
+                        s1 += v.y;
+                    }
+                    c[0] = s0 + s1;
+                    c[0] += __shfl_xor_sync(0xffffffffu, c[0], 1);
+                }
+#else
                 // transpose-reduce over the warp: 2B values per lane -> one warp total per lane
                 int m = 16;
 #pragma unroll
@@ -230,6 +274,7 @@ farfield_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__
                 }
 #pragma unroll
                 for (; m >= 1; m >>= 1) c[0] += __shfl_xor_sync(0xffffffffu, c[0], m);
+#endif
                 if ((lane % kDup) < 2)
                     atomicAdd((unsigned long long *)(accj + 4 * jb),
                               (unsigned long long)fixed2_word(c[0], fx, lane % kDup));
@@ -335,46 +380,83 @@ __global__ void finish_f64(const long long *__restrict__ acc, int n, int P, cons
     U[i] = make_double2(prefactor * fixed2_value(a.x, a.y, fx), prefactor * fixed2_value(b.x, b.y, fx));
 }
 
-vn_status farfield_f64(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, double mu,
-                       void *U, cudaStream_t st, const int64_t *near_ptr, const int32_t *near_ves)
+// pack + pair kernel for the blocks of one part: acc (P x 4 words) and gmax are the caller's, already zeroed;
+// scratch holds the packed sources and, behind them, the log tables
+static vn_status accumulate_f64(const void *X, const void *F, const void *W, int P, int npts, int part, int nparts,
+                                char *scratch, long long *acc, unsigned long long *gmax, cudaStream_t st)
 {
-    const int P = (int)(nves * npts);
     static int slots_dev[kMaxDevices] = {0};
     int &slots = slots_dev[current_device()];
     if (slots == 0) {
         int dev = 0, sms = 0, occ = 0;
         VN_CUDA(cudaGetDevice(&dev));
         VN_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-        VN_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, farfield_f64_kernel, kThreads, 0));
+        VN_CUDA(cudaFuncSetAttribute(farfield_f64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kPairSmem));
+        VN_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, farfield_f64_kernel, kThreads, kPairSmem));
         slots = sms * (occ > 0 ? occ : 1);
     }
-    const SymSplit sp = choose_sym_split(P, kST64, slots, VN_F64_MINTILES, VN_F64_MAXTILES);
-
-    // scratch: packed sources | fixed-point accumulators (hi, lo per component) | gmax
-    const size_t b_src = (size_t)P * 32, b_acc = (size_t)P * 32;
-    char *scratch = nullptr;
-    const size_t b_tab = VN_F64_GTAB ? (size_t)(kLogTab + kExpTab) * sizeof(double) : 0;
-    VN_CUDA(cudaMallocAsync((void **)&scratch, b_src + b_acc + 16 + b_tab, st));
+    const SymSplit sp = choose_sym_split(P, kST64, slots, VN_F64_MINTILES, VN_F64_MAXTILES);   // see accumulate_f32
+    const long long blocks = (long long)sp.n_st * sp.n_chunks;
+    const int mine = (int)((blocks - part + nparts - 1) / nparts);
     double4 *src = (double4 *)scratch;
-    long long *acc = (long long *)(scratch + b_src);
-    unsigned long long *gmax = (unsigned long long *)(scratch + b_src + b_acc);
-    double *gtab = VN_F64_GTAB ? (double *)(scratch + b_src + b_acc + 16) : nullptr;   // 16-byte aligned
-    VN_CUDA(cudaMemsetAsync(acc, 0, b_acc + 16, st));
-
+    double *gtab = VN_F64_GTAB ? (double *)(scratch + (size_t)P * 32) : nullptr;   // 16-byte aligned
     pack_sources_f64<<<(P + 255) / 256, 256, 0, st>>>((const double2 *)X, (const double2 *)F, (const double *)W, P, src, gmax, gtab);
     profile_mark(st, true);
-    farfield_f64_kernel<<<sp.n_st * sp.n_chunks, kThreads, 0, st>>>(src, (const double2 *)X, P, (int)npts, sp.n_tiles,
-                                                                   sp.n_st, sp.n_chunks, gmax, acc, (const double2 *)gtab);
+    if (mine > 0)
+        farfield_f64_kernel<<<mine, kThreads, kPairSmem, st>>>(src, (const double2 *)X, P, npts, sp.n_tiles, sp.n_st,
+                                                               sp.n_chunks, gmax, acc, (const double2 *)gtab, part, nparts);
     profile_mark(st, false);
-    if (near_ptr) {   // row f-1: take the near vesicles' contributions out again before the final rounding
-        const vn_status rc = near_correction_f64(X, F, W, P, (int)npts, near_ptr, near_ves, acc, gmax, st);
-        if (rc != VN_OK) { (void)cudaFreeAsync(scratch, st); return rc; }
-    }
+    count_launch(mine > 0 ? 2 : 1);
+    return VN_OK;
+}
+static size_t scratch_f64_bytes(int P) { return (size_t)P * 32 + (VN_F64_GTAB ? (size_t)kTabBytes : 0); }
+
+vn_status farfield_f64(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, double mu,
+                       void *U, cudaStream_t st, const int64_t *near_ptr, const int32_t *near_ves)
+{
+    const int P = (int)(nves * npts);
+    // scratch: packed sources | log tables | fixed-point accumulators (hi, lo per component) | gmax
+    const size_t b_src = scratch_f64_bytes(P), b_acc = (size_t)P * 32;
+    char *scratch = nullptr;
+    VN_CUDA(cudaMallocAsync((void **)&scratch, b_src + b_acc + 16, st));
+    long long *acc = (long long *)(scratch + b_src);
+    unsigned long long *gmax = (unsigned long long *)(scratch + b_src + b_acc);
+    VN_CUDA(cudaMemsetAsync(acc, 0, b_acc + 16, st));
+    vn_status rc = accumulate_f64(X, F, W, P, (int)npts, 0, 1, scratch, acc, gmax, st);
+    if (rc == VN_OK && near_ptr)   // row f-1: take the near vesicles' contributions out again before the final rounding
+        rc = near_correction_f64(X, F, W, P, (int)npts, near_ptr, near_ves, acc, gmax, st);
+    if (rc != VN_OK) { (void)cudaFreeAsync(scratch, st); return rc; }
     finish_f64<<<(P + 255) / 256, 256, 0, st>>>(acc, P, P, gmax, 1.0 / (4.0 * 3.14159265358979323846 * mu), (double2 *)U);
-    count_launch(3);
+    count_launch(1);
     const cudaError_t e = cudaGetLastError();
     VN_CUDA(cudaFreeAsync(scratch, st));
     return e == cudaSuccess ? VN_OK : VN_ERR_CUDA;
+}
+
+// Section 8e building blocks (see vn_farfield_f32.cu)
+vn_status farfield_partial_f64(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, int part,
+                               int nparts, void *acc, void *gmax, cudaStream_t st)
+{
+    const int P = (int)(nves * npts);
+    char *scratch = nullptr;
+    VN_CUDA(cudaMallocAsync((void **)&scratch, scratch_f64_bytes(P), st));
+    VN_CUDA(cudaMemsetAsync(acc, 0, (size_t)P * 32, st));
+    VN_CUDA(cudaMemsetAsync(gmax, 0, 8, st));
+    const vn_status rc = accumulate_f64(X, F, W, P, (int)npts, part, nparts, scratch, (long long *)acc,
+                                        (unsigned long long *)gmax, st);
+    const cudaError_t e = cudaGetLastError();
+    VN_CUDA(cudaFreeAsync(scratch, st));
+    return rc != VN_OK ? rc : (e == cudaSuccess ? VN_OK : VN_ERR_CUDA);
+}
+
+vn_status farfield_finish_f64(const void *acc, const void *gmax, int64_t P_total, int64_t count, double mu, void *U,
+                              cudaStream_t st)
+{
+    finish_f64<<<(int)((count + 255) / 256), 256, 0, st>>>((const long long *)acc, (int)count, (int)P_total,
+                                                           (const unsigned long long *)gmax,
+                                                           1.0 / (4.0 * 3.14159265358979323846 * mu), (double2 *)U);
+    count_launch(1);
+    return cudaGetLastError() == cudaSuccess ? VN_OK : VN_ERR_CUDA;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -383,20 +465,25 @@ vn_status farfield_f64(const void *X, const void *F, const void *W, int64_t nves
 #ifndef VN_F64_TGT_MINBLK
 #define VN_F64_TGT_MINBLK 4
 #endif
+#ifndef VN_F64_TGT_T
+#define VN_F64_TGT_T 4
+#endif
+constexpr int kT64T = VN_F64_TGT_T;            // targets per thread of the free-target kernel
 __global__ void __launch_bounds__(kThreads, VN_F64_TGT_MINBLK)
 targets_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__ Xt, int nt_pts, int P,
                    int n_tiles, int n_chunks, const unsigned long long *__restrict__ gmax_bits,
                    long long *__restrict__ acc)
 {
-    constexpr int T = kT64;
-    __shared__ __align__(128) double4 tile[kStages][kTile];
+    constexpr int T = kT64T;
+    extern __shared__ __align__(128) unsigned char smem_f64[];
+    double4 (*tile)[kTile] = reinterpret_cast<double4 (*)[kTile]>(smem_f64);
+    __shared__ __align__(16) double tab[kLogTab + kExpTab];
     __shared__ __align__(8) u64 full_bar[kStages];
 #if VN_TGT64_LASTOUT
     __shared__ int drained[kStages];                 // warps that have left each stage (stage_last_out)
 #else
     __shared__ __align__(8) u64 empty_bar[kStages];
 #endif
-    __shared__ double tab[kLogTab + kExpTab];
 
     const int tid = threadIdx.x;
     const int tb = blockIdx.x / n_chunks;
@@ -496,10 +583,11 @@ vn_status farfield_targets_f64(const void *Xt, int64_t nt, const void *X, const 
         int dev = 0, sms = 0, occ = 0;
         VN_CUDA(cudaGetDevice(&dev));
         VN_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-        VN_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, targets_f64_kernel, kThreads, 0));
+        VN_CUDA(cudaFuncSetAttribute(targets_f64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTgtSmem));
+        VN_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, targets_f64_kernel, kThreads, kTgtSmem));
         slots = sms * (occ > 0 ? occ : 1);
     }
-    const Split sp = choose_split_for((n + kST64 - 1) / kST64, (P + kTile - 1) / kTile, slots, 8);
+    const Split sp = choose_split_for((n + kT64T * kThreads - 1) / (kT64T * kThreads), (P + kTile - 1) / kTile, slots, 8);
 
     const size_t b_src = (size_t)P * 32, b_acc = (size_t)n * 32;
     char *scratch = nullptr;
@@ -511,7 +599,7 @@ vn_status farfield_targets_f64(const void *Xt, int64_t nt, const void *X, const 
 
     pack_sources_f64<<<(P + 255) / 256, 256, 0, st>>>((const double2 *)X, (const double2 *)F, (const double *)W, P, src, gmax, nullptr);
     profile_mark(st, true);
-    targets_f64_kernel<<<sp.n_tb * sp.n_chunks, kThreads, 0, st>>>(src, (const double2 *)Xt, n, P, sp.n_tiles,
+    targets_f64_kernel<<<sp.n_tb * sp.n_chunks, kThreads, kTgtSmem, st>>>(src, (const double2 *)Xt, n, P, sp.n_tiles,
                                                                   sp.n_chunks, gmax, acc);
     profile_mark(st, false);
     finish_f64<<<(n + 255) / 256, 256, 0, st>>>(acc, n, P, gmax, 1.0 / (4.0 * 3.14159265358979323846 * mu), (double2 *)Ut);

@@ -52,6 +52,10 @@ __device__ __forceinline__ double dec_f64(unsigned long long e)
 {
     return __longlong_as_double((long long)((e >> 63) ? (e & 0x7fffffffffffffffull) : ~e));
 }
+// Everything after the binning works in coordinates relative to the CENTRE of the root square (fmm_choose_level
+// fixes it, fmm_bin subtracts it from the internal copies of the points): the moments conj(zeta) g and the term
+// z conj(Phi') of the evaluation are each of size |z| / |r| times the result, so with absolute coordinates a
+// suspension far from the origin would lose digits that the translation-invariant exact path keeps.
 struct Geom {
     double x0, y0, size;     // lower-left corner and edge of the root square
 };
@@ -95,6 +99,20 @@ __global__ void fmm_choose_level(unsigned long long *enc, int P, int L_hi)
     L = L < 2 ? 2 : (L > L_hi ? L_hi : L);
 #endif
     enc[4] = (unsigned long long)L;
+    // centre of the root square; the bounds are re-encoded relative to it (every later kernel reads these)
+    const double x0 = dec_f64(enc[0]), y0 = dec_f64(enc[1]), x1 = dec_f64(enc[2]), y1 = dec_f64(enc[3]);
+    if (x0 <= x1) {
+        const double half = 0.5 * fmax(fmax(x1 - x0, y1 - y0) * (1.0 + 1e-9), 1e-300);
+        const double cx = x0 + half, cy = y0 + half;
+        enc[5] = (unsigned long long)__double_as_longlong(cx);
+        enc[6] = (unsigned long long)__double_as_longlong(cy);
+        enc[0] = enc_f64(x0 - cx);
+        enc[1] = enc_f64(y0 - cy);
+        enc[2] = enc_f64(x1 - cx);
+        enc[3] = enc_f64(y1 - cy);
+    } else {
+        enc[5] = enc[6] = 0ull;
+    }
 }
 __device__ __forceinline__ int load_level(const unsigned long long *__restrict__ enc) { return (int)enc[4]; }
 
@@ -130,9 +148,10 @@ fmm_load(const real2 *__restrict__ X, const real2 *__restrict__ F, const real *_
     }
 }
 
-// leaf box of every point and the population count of the leaves
+// moves every point into the root square's frame (in place, see Geom), then: leaf box of every point and the
+// population count of the leaves
 __global__ void __launch_bounds__(256)
-fmm_bin(const cplx *__restrict__ z, int P, const unsigned long long *__restrict__ enc, int *__restrict__ cell,
+fmm_bin(cplx *__restrict__ z, int P, const unsigned long long *__restrict__ enc, int *__restrict__ cell,
         int *__restrict__ cnt)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -140,8 +159,10 @@ fmm_bin(const cplx *__restrict__ z, int P, const unsigned long long *__restrict_
     const Geom gm = load_geom(enc);
     const int n = 1 << load_level(enc);
     const double inv = (double)n / gm.size;
-    const int ix = min(max((int)((z[i].x - gm.x0) * inv), 0), n - 1);
-    const int iy = min(max((int)((z[i].y - gm.y0) * inv), 0), n - 1);
+    const cplx zc = make_double2(z[i].x - __longlong_as_double((long long)enc[5]), z[i].y - __longlong_as_double((long long)enc[6]));
+    z[i] = zc;
+    const int ix = min(max((int)((zc.x - gm.x0) * inv), 0), n - 1);
+    const int iy = min(max((int)((zc.y - gm.y0) * inv), 0), n - 1);
     const int c = ix * n + iy;
     cell[i] = c;
     atomicAdd(cnt + c, 1);

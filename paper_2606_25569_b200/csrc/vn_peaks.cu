@@ -103,7 +103,60 @@ __global__ void __launch_bounds__(256) peak_dfma_kernel(int iters, double b, dou
     if (s == 123.456) sink[0] = (float)s;
 }
 
-// rates[0..3] = FFMA2, FFMA, MUFU (rcp + lg2), DFMA lane-operations per second; rates[4] = SM count of the device
+// The streams above re-read two of their three operands from one instruction to the next (register-reuse cache
+// hits).  These two read three DIFFERENT register pairs in every instruction and share no operand slot with their
+// neighbours -- the operand pattern of a kernel whose inputs change every instruction -- and measure what the
+// register file can feed the pipes in that case.
+__global__ void __launch_bounds__(256) peak_ffma2_noreuse_kernel(int iters, float b0, float c0, float *sink)
+{
+    u64 a[kChains], b[kChains], c[kChains];
+#pragma unroll
+    for (int k = 0; k < kChains; ++k) {
+        a[k] = pk(1.0f + 0.001f * (float)(threadIdx.x + k), 0.5f + 0.002f * (float)k);
+        b[k] = pk(b0 - 0.0001f * (float)k, b0 - 0.0002f * (float)k);
+        c[k] = pk(c0 + 0.0001f * (float)k, c0 + 0.0002f * (float)k);
+    }
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int u = 0; u < kInner; ++u) {
+#pragma unroll
+            for (int k = 0; k < kChains; ++k) a[k] = fma2(a[k], b[(k + u) % kChains], c[(k + 3 * u + 1) % kChains]);
+        }
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int k = 0; k < kChains; ++k) {
+        float lo, hi;
+        upk(a[k], lo, hi);
+        s += lo + hi;
+    }
+    if (s == 123.456f) sink[0] = s;
+}
+
+__global__ void __launch_bounds__(256) peak_dfma_noreuse_kernel(int iters, double b0, double c0, float *sink)
+{
+    double a[kChains], b[kChains], c[kChains];
+#pragma unroll
+    for (int k = 0; k < kChains; ++k) {
+        a[k] = 1.0 + 0.001 * (double)(threadIdx.x + k);
+        b[k] = b0 - 0.0001 * (double)k;
+        c[k] = c0 + 0.0001 * (double)k;
+    }
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int u = 0; u < kInner; ++u) {
+#pragma unroll
+            for (int k = 0; k < kChains; ++k) a[k] = fma(a[k], b[(k + u) % kChains], c[(k + 3 * u + 1) % kChains]);
+        }
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int k = 0; k < kChains; ++k) s += a[k];
+    if (s == 123.456) sink[0] = (float)s;
+}
+
+// rates[0..3] = FFMA2, FFMA, MUFU (rcp + lg2), DFMA lane-operations per second; rates[4] = SM count of the device;
+// rates[5], rates[6] = FFMA2 and DFMA streams without operand reuse; rates[7] = 0 (reserved)
 vn_status pipe_peaks(double *rates, cudaStream_t st)
 {
     int dev = 0, sms = 0;
@@ -117,10 +170,12 @@ vn_status pipe_peaks(double *rates, cudaStream_t st)
     vn_status rc = VN_OK;
     // launch shapes: (threads per block, blocks per SM): 16, 32 and 64 warps per SM
     const int shapes[3][2] = {{128, 4}, {256, 4}, {256, 8}};
-    for (int kind = 0; kind < 4 && rc == VN_OK; ++kind) {
+    const int slot_of[6] = {0, 1, 2, 3, 5, 6};
+    rates[7] = 0.0;
+    for (int kind = 0; kind < 6 && rc == VN_OK; ++kind) {
         // about a millisecond per launch at nominal rates
-        const int iters = kind == 0 ? 2048 : (kind == 1 ? 2048 : (kind == 2 ? 512 : 1024));
-        const double lane_ops_per_thread = (double)iters * kInner * kChains * (kind == 0 ? 2.0 : 1.0);
+        const int iters = (kind == 0 || kind == 1 || kind == 4) ? 2048 : (kind == 2 ? 512 : 1024);
+        const double lane_ops_per_thread = (double)iters * kInner * kChains * ((kind == 0 || kind == 4) ? 2.0 : 1.0);
         double best = 0.0;
         for (int sh = 0; sh < 3 && rc == VN_OK; ++sh) {
             const int threads = shapes[sh][0], blocks = shapes[sh][1] * sms;
@@ -130,7 +185,9 @@ vn_status pipe_peaks(double *rates, cudaStream_t st)
                     case 0: peak_ffma2_kernel<<<blocks, threads, 0, st>>>(iters, 0.999f, 0.001f, sink); break;
                     case 1: peak_ffma_kernel<<<blocks, threads, 0, st>>>(iters, 0.999f, 0.001f, sink); break;
                     case 2: peak_mufu_kernel<<<blocks, threads, 0, st>>>(iters, 1.0f, 2.0f, sink); break;
-                    default: peak_dfma_kernel<<<blocks, threads, 0, st>>>(iters, 0.999, 0.001, sink); break;
+                    case 3: peak_dfma_kernel<<<blocks, threads, 0, st>>>(iters, 0.999, 0.001, sink); break;
+                    case 4: peak_ffma2_noreuse_kernel<<<blocks, threads, 0, st>>>(iters, 0.999f, 0.001f, sink); break;
+                    default: peak_dfma_noreuse_kernel<<<blocks, threads, 0, st>>>(iters, 0.999, 0.001, sink); break;
                 }
                 count_launch(1);
                 if (rep > 0) {
@@ -146,7 +203,7 @@ vn_status pipe_peaks(double *rates, cudaStream_t st)
                 }
             }
         }
-        rates[kind] = best;
+        rates[slot_of[kind]] = best;
     }
     rates[4] = (double)sms;
     cudaEventDestroy(e0);

@@ -77,3 +77,23 @@ def test_argument_validation_needs_no_gpu():
     assert L.vn_farfield_host(p, None, None, 2, 4, 1.0, q, vn.VN_F64) == INV
     assert L.vn_pipe_peaks(None, None) == INV
     assert L.vn_farfield_host(p, p, None, 2, 4, -1.0, q, vn.VN_F64) == INV
+
+
+def test_partial_and_finish_argument_validation():
+    L = vn.lib()
+    buf = (ctypes.c_double * 64)()
+    p = ctypes.addressof(buf)
+    q = ctypes.addressof((ctypes.c_double * 64)())
+    g = ctypes.addressof((ctypes.c_double * 2)())
+    INV = vn.VN_ERR_INVALID_ARG
+    assert L.vn_farfield_partial(p, p, p, 2, 4, 2, 2, q, g, vn.VN_F32, None) == INV        # part >= nparts
+    assert L.vn_farfield_partial(p, p, p, 2, 4, -1, 2, q, g, vn.VN_F32, None) == INV       # part < 0
+    assert L.vn_farfield_partial(p, p, p, 2, 4, 0, 0, q, g, vn.VN_F32, None) == INV        # nparts < 1
+    assert L.vn_farfield_partial(p, p, p, 2, 4, 0, 1, None, g, vn.VN_F32, None) == INV     # null acc
+    assert L.vn_farfield_partial(p, p, p, 2, 4, 0, 1, q, None, vn.VN_F32, None) == INV     # null gmax
+    assert L.vn_farfield_partial(p, p, p, 2, 4, 0, 1, p, g, vn.VN_F32, None) == INV        # acc aliases X
+    assert L.vn_farfield_finish(q, g, 8, 9, 1.0, p, vn.VN_F32, None) == INV                # count > total
+    assert L.vn_farfield_finish(q, g, 8, -1, 1.0, p, vn.VN_F32, None) == INV
+    assert L.vn_farfield_finish(q, g, 8, 4, 0.0, p, vn.VN_F32, None) == INV                # mu
+    assert L.vn_farfield_finish(q, g, 8, 4, 1.0, None, vn.VN_F32, None) == INV             # null U
+    assert L.vn_farfield_finish(None, g, 8, 0, 1.0, None, vn.VN_F32, None) == vn.VN_OK     # count == 0: nothing to do

@@ -590,3 +590,27 @@ def test_fmm_default_order_meets_the_tolerance(dtype):
     got = vn.vn_farfield_fmm(dev(s.X, dtype), dev(s.F, dtype), dev(W, dtype), s.mu, 0)     # order 0 = default for the precision
     torch.cuda.synchronize()
     check(got.cpu().numpy(), ref, TOL[dtype], f"fmm default order {np.dtype(dtype).name}", c_max=FMM_C)
+
+
+@pytest.mark.parametrize("shift", [(1.0e4, -3.0e4), (-2.0e5, 1.0e5)])
+def test_fmm_is_translation_invariant(shift):
+    """The expansions work in the root square's frame, so a suspension far from the origin keeps the accuracy it
+    has at the origin (the exact path is translation invariant by construction; in absolute coordinates the terms
+    conj(zeta) g and z conj(Phi') would each be |z| / |r| times larger than their sum)."""
+    s = inputs.config(1)
+    W = oracle.weights(s.X)
+    Xs = s.X + np.asarray(shift)
+    ref = oracle.farfield(Xs, s.F, W, s.mu)                       # the oracle on the SHIFTED points
+    got = vn.vn_farfield_fmm(dev(Xs, np.float64), dev(s.F, np.float64), dev(W, np.float64), s.mu, 38)
+    got0 = vn.vn_farfield_fmm(dev(s.X, np.float64), dev(s.F, np.float64), dev(W, np.float64), s.mu, 38)
+    torch.cuda.synchronize()
+    e_shift, _ = check(got.cpu().numpy(), ref, 1e-12, f"fmm config1 shifted by {shift}", c_max=FMM_C)
+    e_zero = rel_l2(got0.cpu().numpy(), oracle.farfield(s.X, s.F, W, s.mu))
+    # moving into the root square's frame rounds once more (an ulp of the box size against gaps of 0.05): the shifted
+    # run may lose a digit against the run at the origin, not the six digits |z| / |r| = 1e5 / 0.05 would cost
+    print(f"fmm at the origin {e_zero:.2e}, shifted {e_shift:.2e}")
+    assert e_shift <= 1e-13
+    # the exact path, for comparison
+    ex = vn.vn_farfield(dev(Xs, np.float64), dev(s.F, np.float64), dev(W, np.float64), s.mu)
+    torch.cuda.synchronize()
+    check(ex.cpu().numpy(), ref, 1e-12, f"farfield config1 shifted by {shift}")

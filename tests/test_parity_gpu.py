@@ -319,3 +319,43 @@ def test_two_streams_interleaved():
     torch.cuda.synchronize()
     for ua, ub, uf in outs:
         assert torch.equal(ua, ref_a) and torch.equal(ub, ref_b) and torch.equal(uf, ref_f)
+
+
+# ------------------------------------------------------------------------------------- one suspension over several GPUs (section 8e)
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("index,nparts", [(0, 2), (1, 2), (1, 3), (2, 8)])
+def test_partial_accumulators_reproduce_farfield_bitwise(index, nparts, dtype):
+    """The multi-GPU split on one device: the raw fixed-point accumulators of parts 0 .. nparts-1 (what each GPU
+    would compute), added as integers (what the reduce-scatter does), finished on two vesicle ranges (what each
+    GPU does with its shard) give bit for bit the result of vn_farfield."""
+    s, W = problem(index)
+    Xd, Fd, Wd = dev(s.X, dtype), dev(s.F, dtype), dev(W, dtype)
+    ref = vn.vn_farfield(Xd, Fd, Wd, s.mu)
+    total, gmax0 = None, None
+    for part in range(nparts):
+        acc, gmax = vn.vn_farfield_partial(Xd, Fd, Wd, part, nparts)
+        assert acc.abs().sum().item() != 0 or index == 0            # every part has work (config 0: a handful of blocks)
+        total = acc.clone() if total is None else total + acc
+        gmax0 = gmax.clone() if gmax0 is None else gmax0
+        assert torch.equal(gmax, gmax0)                              # every device packs all sources: same scale
+    P, words = s.nves * s.npts, vn.acc_words(Xd.dtype)
+    k = (s.nves // 3) * s.npts                                       # two shards of different sizes
+    lo = vn.vn_farfield_finish(total[:k * words], gmax0, P, Xd.dtype, s.mu)
+    hi = vn.vn_farfield_finish(total[k * words:], gmax0, P, Xd.dtype, s.mu)
+    torch.cuda.synchronize()
+    assert torch.equal(torch.cat([lo, hi]).view_as(ref), ref)
+    # nparts = 1 is the single-device call
+    acc, gmax = vn.vn_farfield_partial(Xd, Fd, Wd, 0, 1)
+    assert torch.equal(acc, total)
+    assert torch.equal(vn.vn_farfield_finish(acc, gmax, P, Xd.dtype, s.mu).view_as(ref), ref)
+
+
+def test_sharded_farfield_single_process_equals_farfield():
+    """multi.sharded_farfield_gpu with world = 1 (no process group) is the plain call."""
+    from paper_2606_25569_b200 import multi
+    s, W = problem(1)
+    Xd, Fd, Wd = dev(s.X, np.float32), dev(s.F, np.float32), dev(W, np.float32)
+    U = multi.sharded_farfield_gpu(vn, Xd, Fd, Wd, s.nves, s.mu, 0, 1)
+    ref = vn.vn_farfield(Xd, Fd, Wd, s.mu)
+    torch.cuda.synchronize()
+    assert torch.equal(U, ref)
