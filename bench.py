@@ -358,7 +358,7 @@ def measure(ctx, m):
     X_d = torch.empty_like(seq_d[0])
     W_d = torch.empty((nloc, susp.npts), dtype=tdtype, device="cuda")
     U_d = torch.empty_like(X_d)
-    fmm_order = m.order or (12 if m.precision == "f32" else 38)
+    fmm_order = m.order or (14 if m.precision == "f32" else 38)
     if m.path == "masked":                             # CSR buffers sized once (4 near vesicles per point is generous)
         near_ptr = torch.empty(P + 1, dtype=torch.int64, device="cuda")
         near_ves = torch.empty(4 * P, dtype=torch.int32, device="cuda")
@@ -541,7 +541,7 @@ def main():
                          "aux: the O(P) rows around the sum (f-3 redistribution, a-1 weights, f-2 elastic force), "
                          "reported in points/s; fmm: vn_farfield_fmm (approximate, O(P)), reported in the direct sum's "
                          "interactions per second so that it compares with --path farfield")
-    ap.add_argument("--order", type=int, default=0, help="expansion order of --path fmm (default 12 for f32, 38 for f64); with --path targets a value > 0 "
+    ap.add_argument("--order", type=int, default=0, help="expansion order of --path fmm (default 14 for f32, 38 for f64); with --path targets a value > 0 "
                          "selects vn_farfield_targets_fmm")
     ap.add_argument("--graph", action="store_true",
                     help="capture one step (all its evaluations) into a CUDA graph after the warm-up and time graph replays")

@@ -45,8 +45,9 @@
  *    1e-9 < |r| < 1e9 in the caller's units.  VN_F64 needs normal doubles whose reciprocal is normal.
  *  - Input values are not validated.  A non-finite value anywhere in X, F or W makes EVERY output of
  *    vn_farfield / vn_farfield_masked / vn_farfield_targets NaN (their integer accumulators cannot carry
- *    NaN/Inf point by point; a free target's own coordinates are not checked); the FMM calls let it
- *    propagate through their double arithmetic.  Points of DIFFERENT vesicles
+ *    NaN/Inf point by point; a free target's own coordinates are not checked); the FMM calls, and vn_farfield
+ *    for suspensions of at most 1,024 points (one launch, plain floating-point sums), let it propagate
+ *    through their arithmetic: at least every output the value contributes to is non-finite.  Points of DIFFERENT vesicles
  *    are assumed distinct; a coincident cross-vesicle pair gives an unspecified (possibly
  *    non-finite) value at that target only (reading A5).  nves == 1 is valid and yields U == 0.
  */
@@ -71,7 +72,9 @@ typedef enum { VN_F32 = 0, VN_F64 = 1 } vn_precision;
 /* Far-field single-layer potential at every membrane point, own vesicle excluded
  * (north_star).  All pointers are DEVICE pointers.
  * Steps run on the device: pack g = F*W, pair sum over all other vesicles' points,
- * two-level accumulation, scale by 1/(4 pi mu), store.  U is overwritten. */
+ * two-level accumulation, scale by 1/(4 pi mu), store.  U is overwritten.
+ * Suspensions of at most 1,024 points take a single-launch kernel without scratch memory
+ * (one-directional sums, no atomics); larger ones the symmetric pair kernels. */
 vn_status vn_farfield(const void *X, const void *F, const void *W,
                       int64_t nves, int64_t npts, double mu,
                       void *U, vn_precision precision, void *stream);
@@ -150,9 +153,12 @@ vn_status vn_farfield_targets(const void *Xt, int64_t nt,
  * ... will make it scale as O(M), but an applicable GPU implementation is beyond the scope of this
  * paper"; Greengard & Rokhlin 1987 cited PAPER.md:173).  It is an APPROXIMATION:
  * `order` = p, the number of terms kept in the multipole / local expansions (2 <= p <= 48, or 0 for
- * the default that meets vn_farfield's tolerance: 12 for VN_F32, 38 for VN_F64); the
+ * the default that meets vn_farfield's tolerance: 14 for VN_F32, 38 for VN_F64); the
  * relative L2 truncation error falls like 0.45^p (measured on the synthetic suspensions: p = 12
- * about 3e-6, p = 20 about 5e-9, p = 38 about 1e-13); vn_farfield stays the exact path.
+ * about 3e-6, p = 20 about 5e-9, p = 38 about 1e-13) and the largest point-wise error, relative to the largest
+ * velocity, is about 15 times that (targets near the corner of their leaf box): 8e-5 at p = 12, 1.7e-5 at the
+ * default p = 14; vn_farfield stays the exact path.  The expansions are formed in the frame of the root square's
+ * centre, so the accuracy does not depend on where the suspension sits.
  * The expansions are double for both storage precisions; the direct part over neighbouring leaves runs
  * in the storage precision (VN_F32: the same SFU pair arithmetic as vn_farfield, error about 1e-6).  Uniform quadtree over the bounding square of the points; a strongly
  * non-uniform point distribution costs time (crowded leaves), not accuracy.  Results are bitwise
@@ -235,6 +241,17 @@ vn_status vn_farfield_partial(const void *X, const void *F, const void *W, int64
                               vn_precision precision, void *stream);
 vn_status vn_farfield_finish(const void *acc, const void *gmax, int64_t npoints_total, int64_t count, double mu,
                              void *U, vn_precision precision, void *stream);
+
+/* Self-check of the pair kernels' shared-memory ring (stands in for compute-sanitizer's
+ * racecheck / initcheck, which cannot be run on the development pool).  Computes what vn_farfield computes, always
+ * with the symmetric pair kernels (whatever the size), in a verification build of them: every source record a warp
+ * reads from a ring stage is compared, bit for bit, with its original in global memory, so a stage refilled by the
+ * bulk copy while a warp still reads it, or read before its copy has landed, is counted; and the scratch memory is
+ * filled with 0xFF bytes before use, so a read of scratch that no kernel wrote shows in U.  Synchronous: waits for
+ * `stream`, then writes the number of mismatching record reads into the HOST variable *mismatches (0 = clean).
+ * U (DEVICE, overwritten) must equal vn_farfield's U bit for bit when the suspension has more than 1,024 points. */
+vn_status vn_selfcheck(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, double mu,
+                       void *U, vn_precision precision, void *stream, int64_t *mismatches /* HOST */);
 
 /* Measured issue rates of the arithmetic pipes that bound the pair kernels (the nominal
  * lane counts "must be confirmed by microbenchmark").  Runs six register-only stream

@@ -82,6 +82,8 @@ def lib():
         L.vn_farfield_partial.restype = ci
         L.vn_farfield_finish.argtypes = [vp, vp, i64, i64, dbl, vp, ci, vp]
         L.vn_farfield_finish.restype = ci
+        L.vn_selfcheck.argtypes = [vp, vp, vp, i64, i64, dbl, vp, ci, vp, ctypes.POINTER(i64)]
+        L.vn_selfcheck.restype = ci
         L.vn_pipe_peaks.argtypes = [ctypes.POINTER(dbl), vp]
         L.vn_pipe_peaks.restype = ci
         L.vn_version.argtypes = []
@@ -187,8 +189,9 @@ def vn_farfield_finish(acc, gmax, npoints_total: int, dtype, mu: float = 1.0, ou
     return out
 
 
-def vn_farfield_fmm(X, F, W, mu: float = 1.0, order: int = 12, out=None, stream=None, near_ptr=None, near_ves=None):
-    """The far-field sum by the fast multipole method with `order` expansion terms (approximate, O(P));
+def vn_farfield_fmm(X, F, W, mu: float = 1.0, order: int = 0, out=None, stream=None, near_ptr=None, near_ves=None):
+    """The far-field sum by the fast multipole method with `order` expansion terms (approximate, O(P); 0 = the
+    default for the precision: 14 for float32, 38 for float64);
     with the CSR relation of vn_near_pairs the near vesicles' contributions are zeroed as in vn_farfield_masked."""
     import torch
     nves, npts, two = X.shape
@@ -408,6 +411,28 @@ def vn_profile_read(max_entries: int = 4096):
     if n < 0:
         raise VesnetError(VN_ERR_CUDA, "vn_profile_read")
     return [buf[i] for i in range(n)]
+
+
+def vn_selfcheck(X, F, W, mu: float = 1.0, out=None, stream=None):
+    """vn_farfield through the verification build of the pair kernels (ring reads compared with global memory, scratch
+    poisoned).  Returns (U, mismatches); synchronous."""
+    import torch
+    nves, npts, two = X.shape
+    if two != 2:
+        raise ValueError("X must be [nves, npts, 2]")
+    _check_dev("X", X)
+    _check_dev("F", F, X.shape, X.dtype)
+    _check_dev("W", W, (nves, npts), X.dtype)
+    if out is None:
+        out = torch.empty_like(X)
+    _check_dev("out", out, X.shape, X.dtype)
+    n = ctypes.c_int64(-1)
+    with torch.cuda.device(X.device):
+        rc = lib().vn_selfcheck(X.data_ptr(), F.data_ptr(), W.data_ptr(), nves, npts, float(mu), out.data_ptr(),
+                                _prec(X), _stream_ptr(stream), ctypes.byref(n))
+    if rc != VN_OK:
+        raise VesnetError(rc, "vn_selfcheck")
+    return out, int(n.value)
 
 
 def vn_pipe_peaks(stream=None):

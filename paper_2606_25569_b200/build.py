@@ -11,7 +11,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libvesnet_farfield.so")
-SOURCES = ["vn_api.cu", "vn_farfield_f32.cu", "vn_farfield_f64.cu", "vn_weights.cu", "vn_near.cu", "vn_force.cu", "vn_redistribute.cu", "vn_fmm.cu", "vn_peaks.cu"]
+SOURCES = ["vn_api.cu", "vn_farfield_f32.cu", "vn_farfield_f64.cu", "vn_weights.cu", "vn_near.cu", "vn_force.cu", "vn_redistribute.cu", "vn_fmm.cu", "vn_peaks.cu", "vn_farfield_small.cu"]
 HEADERS = [os.path.join(CSRC, "vn_common.cuh"), os.path.join(CSRC, "vn_log64.cuh"),
            os.path.join(os.path.dirname(HERE), "include", "vesnet_farfield.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",

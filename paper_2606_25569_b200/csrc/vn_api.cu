@@ -49,6 +49,12 @@ vn_status near_pairs(const void *X, const void *W, int64_t nves, int64_t npts, i
                      int32_t *near_ves, int64_t capacity, vn_precision prec, cudaStream_t st);
 vn_status arclength_weights(const void *X, int64_t nves, int64_t npts, void *W, vn_precision prec, cudaStream_t st);
 vn_status pipe_peaks(double *rates, cudaStream_t st);
+vn_status farfield_selfcheck_f32(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, double mu,
+                                 void *U, unsigned long long *mismatches, cudaStream_t st);
+vn_status farfield_selfcheck_f64(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, double mu,
+                                 void *U, unsigned long long *mismatches, cudaStream_t st);
+vn_status farfield_small(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, double mu, void *U,
+                         vn_precision prec, cudaStream_t st);
 vn_status farfield_partial_f32(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, int part,
                                int nparts, void *acc, void *gmax, cudaStream_t st);
 vn_status farfield_partial_f64(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, int part,
@@ -135,6 +141,15 @@ static vn_status check_device()
     return ok ? VN_OK : VN_ERR_UNSUPPORTED;
 }
 
+// vn_farfield proper: the single-launch kernel for tiny suspensions, the symmetric pair kernels otherwise
+static vn_status farfield_dispatch(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, double mu,
+                                   void *U, vn_precision prec, cudaStream_t st)
+{
+    if (nves * npts <= kSmallPoints) return farfield_small(X, F, W, nves, npts, mu, U, prec, st);
+    return prec == VN_F32 ? farfield_f32(X, F, W, nves, npts, mu, U, st, nullptr, nullptr)
+                          : farfield_f64(X, F, W, nves, npts, mu, U, st, nullptr, nullptr);
+}
+
 static bool misaligned(const void *p, size_t a) { return ((uintptr_t)p % a) != 0; }
 
 static vn_status check_shape(int64_t nves, int64_t npts, vn_precision prec)
@@ -163,9 +178,7 @@ vn_status vn_farfield(const void *X, const void *F, const void *W, int64_t nves,
     if (U == X || U == F || U == W) return VN_ERR_INVALID_ARG;
     const vn_status ds = check_device();
     if (ds != VN_OK) return ds;
-    cudaStream_t st = (cudaStream_t)stream;
-    return precision == VN_F32 ? farfield_f32(X, F, W, nves, npts, mu, U, st, nullptr, nullptr)
-                               : farfield_f64(X, F, W, nves, npts, mu, U, st, nullptr, nullptr);
+    return farfield_dispatch(X, F, W, nves, npts, mu, U, precision, (cudaStream_t)stream);
 }
 
 vn_status vn_near_pairs(const void *X, const void *W, int64_t nves, int64_t npts, int64_t *near_ptr,
@@ -266,7 +279,7 @@ vn_status vn_farfield_fmm(const void *X, const void *F, const void *W, int64_t n
                           vn_precision precision, void *stream)
 {
     if (misaligned(near_ptr, 8) || misaligned(near_ves, 4)) return VN_ERR_INVALID_ARG;
-    if (order == 0) order = precision == VN_F32 ? 12 : 38;      // the orders that meet 2e-5 / 1e-12
+    if (order == 0) order = precision == VN_F32 ? 14 : 38;      // the orders that meet 2e-5 / 1e-12, point-wise too
     if (!X || !F || !W || !U) return VN_ERR_INVALID_ARG;
     if (check_shape(nves, npts, precision) != VN_OK) return VN_ERR_INVALID_ARG;
     if (!isfinite(mu) || !(mu > 0.0) || order < 2 || order > 48) return VN_ERR_INVALID_ARG;
@@ -285,7 +298,7 @@ vn_status vn_farfield_targets_fmm(const void *Xt, int64_t nt, const void *X, con
 {
     if (!X || !F || !W) return VN_ERR_INVALID_ARG;
     if (check_shape(nves, npts, precision) != VN_OK) return VN_ERR_INVALID_ARG;
-    if (order == 0) order = precision == VN_F32 ? 12 : 38;
+    if (order == 0) order = precision == VN_F32 ? 14 : 38;
     if (nt < 0 || nt >= (1ll << 31) || order < 2 || order > 48) return VN_ERR_INVALID_ARG;
     if (!isfinite(mu) || !(mu > 0.0)) return VN_ERR_INVALID_ARG;
     if (nt == 0) return VN_OK;
@@ -310,30 +323,31 @@ vn_status vn_farfield_host(const void *X, const void *F, const void *W, int64_t 
     const vn_status ds = check_device();
     if (ds != VN_OK) return ds;
 
-    // process-wide cached device buffers and stream, grown on demand
+    // cached device buffer and stream PER DEVICE, grown on demand, kept for the life of the process (a caller that
+    // switches devices finds each device's own cache again; nothing is dropped or leaked on a switch)
+    struct HostCache {
+        cudaStream_t st = nullptr;
+        char *buf = nullptr;
+        size_t cap = 0;
+    };
     static std::mutex mtx;
-    static cudaStream_t st = nullptr;
-    static char *buf = nullptr;
-    static size_t cap = 0;
-    static int owner = -1;                          // device the cached stream and buffer belong to
+    static HostCache cache[kMaxDevices];
     std::lock_guard<std::mutex> lock(mtx);
-    if (owner != current_device()) {                // first call, or the caller switched devices: start afresh
-        st = nullptr; buf = nullptr; cap = 0;       // (the old device's stream and buffer are left to that context)
-        owner = current_device();
-    }
-    if (!st) VN_CUDA(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking));
+    HostCache &hc = cache[current_device()];
+    if (!hc.st) VN_CUDA(cudaStreamCreateWithFlags(&hc.st, cudaStreamNonBlocking));
+    cudaStream_t st = hc.st;
     const size_t P = (size_t)(nves * npts);
     const size_t es = precision == VN_F32 ? 4 : 8;
     const size_t bX = 2 * es * P, bW = es * P;
     auto up = [](size_t b) { return (b + 255) & ~(size_t)255; };
     const size_t need = 3 * up(bX) + up(bW);
-    if (need > cap) {
-        if (buf) VN_CUDA(cudaFree(buf));
-        buf = nullptr; cap = 0;
-        VN_CUDA(cudaMalloc((void **)&buf, need));
-        cap = need;
+    if (need > hc.cap) {
+        if (hc.buf) VN_CUDA(cudaFree(hc.buf));
+        hc.buf = nullptr; hc.cap = 0;
+        VN_CUDA(cudaMalloc((void **)&hc.buf, need));
+        hc.cap = need;
     }
-    char *dX = buf, *dF = dX + up(bX), *dU = dF + up(bX), *dW = dU + up(bX);
+    char *dX = hc.buf, *dF = dX + up(bX), *dU = dF + up(bX), *dW = dU + up(bX);
     VN_CUDA(cudaMemcpyAsync(dX, X, bX, cudaMemcpyHostToDevice, st));
     VN_CUDA(cudaMemcpyAsync(dF, F, bX, cudaMemcpyHostToDevice, st));
     vn_status rc;
@@ -343,8 +357,7 @@ vn_status vn_farfield_host(const void *X, const void *F, const void *W, int64_t 
         rc = arclength_weights(dX, nves, npts, dW, precision, st);
         if (rc != VN_OK) return rc;
     }
-    rc = precision == VN_F32 ? farfield_f32(dX, dF, dW, nves, npts, mu, dU, st, nullptr, nullptr)
-                             : farfield_f64(dX, dF, dW, nves, npts, mu, dU, st, nullptr, nullptr);
+    rc = farfield_dispatch(dX, dF, dW, nves, npts, mu, dU, precision, st);
     if (rc != VN_OK) return rc;
     VN_CUDA(cudaMemcpyAsync(U, dU, bX, cudaMemcpyDeviceToHost, st));
     VN_CUDA(cudaStreamSynchronize(st));
@@ -398,6 +411,34 @@ vn_status vn_farfield_finish(const void *acc, const void *gmax, int64_t npoints_
     cudaStream_t st = (cudaStream_t)stream;
     return precision == VN_F32 ? farfield_finish_f32(acc, gmax, npoints_total, count, mu, U, st)
                                : farfield_finish_f64(acc, gmax, npoints_total, count, mu, U, st);
+}
+
+vn_status vn_selfcheck(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, double mu, void *U,
+                       vn_precision precision, void *stream, int64_t *mismatches)
+{
+    if (!X || !F || !W || !U || !mismatches) return VN_ERR_INVALID_ARG;
+    if (check_shape(nves, npts, precision) != VN_OK) return VN_ERR_INVALID_ARG;
+    if (!isfinite(mu) || !(mu > 0.0)) return VN_ERR_INVALID_ARG;
+    const size_t pair = precision == VN_F32 ? 8 : 16;
+    if (misaligned(X, pair) || misaligned(F, pair) || misaligned(U, pair) || misaligned(W, pair / 2))
+        return VN_ERR_INVALID_ARG;
+    if (U == X || U == F || U == W) return VN_ERR_INVALID_ARG;
+    const vn_status ds = check_device();
+    if (ds != VN_OK) return ds;
+    cudaStream_t st = (cudaStream_t)stream;
+    unsigned long long *d_count = nullptr;
+    VN_CUDA(cudaMallocAsync((void **)&d_count, 8, st));
+    VN_CUDA(cudaMemsetAsync(d_count, 0, 8, st));
+    const vn_status rc = precision == VN_F32 ? farfield_selfcheck_f32(X, F, W, nves, npts, mu, U, d_count, st)
+                                             : farfield_selfcheck_f64(X, F, W, nves, npts, mu, U, d_count, st);
+    unsigned long long h_count = 0;
+    const cudaError_t e1 = cudaMemcpyAsync(&h_count, d_count, 8, cudaMemcpyDeviceToHost, st);
+    const cudaError_t e2 = cudaStreamSynchronize(st);
+    (void)cudaFreeAsync(d_count, st);
+    if (rc != VN_OK) return rc;
+    if (e1 != cudaSuccess || e2 != cudaSuccess) { (void)cudaGetLastError(); return VN_ERR_CUDA; }
+    *mismatches = (int64_t)h_count;
+    return VN_OK;
 }
 
 vn_status vn_pipe_peaks(double *rates, void *stream)

@@ -15,6 +15,7 @@ typedef unsigned long long u64;
 constexpr int kThreads = 128;      // threads per block in the pair kernels (4 warps)
 constexpr int kTile = 128;         // sources per shared-memory tile
 constexpr int kStages = 4;         // tiles in flight per block
+constexpr int kSmallPoints = 1024; // vn_farfield of at most this many points is ONE launch (vn_farfield_small.cu)
 
 // ---------------------------------------------------------------------------------------------
 // launch bookkeeping (vn_launch_count)

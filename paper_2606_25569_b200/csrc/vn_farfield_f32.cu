@@ -83,11 +83,14 @@ __global__ void pack_sources_f32(const float2 *__restrict__ X, const float2 *__r
 // 1-D bulk async copies (TMA) that complete on mbarriers.  A tile that cannot contain points of the
 // block's own vesicles takes the fast path (no predicate); tiles that overlap them and a ragged last
 // tile take the predicated path.
-template <int NP>
+// CHECK = true (vn_selfcheck): every record read from the ring is compared with its original in global memory and
+// mismatches are counted -- a stage refilled while a warp still reads it, or read before its copy has landed, shows
+// up as a non-zero count (the tool this replaces, compute-sanitizer's racecheck, is not available on the pool).
+template <int NP, bool CHECK>
 __global__ void __launch_bounds__(kThreads, VN_F32_MINBLK)
 farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict__ X, int P, int npts,
                     int n_tiles, int n_st, int n_chunks, const unsigned *__restrict__ gmax_bits,
-                    long long *__restrict__ acc, int part, int nparts)
+                    long long *__restrict__ acc, int part, int nparts, unsigned long long *__restrict__ mismatches)
 {
     constexpr int T = 2 * NP;
     __shared__ __align__(128) ulonglong2 tile[kStages][kTile * 2];
@@ -181,6 +184,10 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
         const int first = tile_of(u) * kTile;
         const int cnt = min(kTile, P - first);
         const ulonglong2 *ts = tile[s];
+        auto verify = [&](int j, const ulonglong2 &yy, const ulonglong2 &gg) {      // CHECK builds only
+            const ulonglong2 oy = __ldcg(src + 2 * (size_t)(first + j)), og = __ldcg(src + 2 * (size_t)(first + j) + 1);
+            if (oy.x != yy.x || oy.y != yy.y || og.x != gg.x || og.y != gg.y) atomicAdd(mismatches, 1ull);
+        };
         const bool fast = both && (first >= span_end || first + kTile <= span_begin) && (cnt == kTile);
         if (fast) {
             // per-tile partial sums (two-level accumulation), in units of -(ln2/2): U' = U / KA
@@ -196,6 +203,7 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
                 for (int jj = 0; jj < kBatch; ++jj) {
                     const ulonglong2 yy = ts[2 * (jb + jj) + 0];   // (yx,yx) (yy,yy)
                     const ulonglong2 gg = ts[2 * (jb + jj) + 1];   // (gx,gx) (gy,gy)
+                    if (CHECK) verify(jb + jj, yy, gg);
                     u64 rx[NP], ry[NP], l[NP], inv[NP];
 #pragma unroll
                     for (int p = 0; p < NP; ++p) {
@@ -273,6 +281,7 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
             for (int j = 0; j < kTile; ++j) {
                 const ulonglong2 yy = ts[2 * j + 0];
                 const ulonglong2 gg = ts[2 * j + 1];
+                if (CHECK) verify(j, yy, gg);
 #pragma unroll
                 for (int p = 0; p < NP; ++p) {
                     const u64 rx = sub2(tx[p], yy.x);
@@ -316,6 +325,7 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
             for (int j = 0; j < cnt; ++j) {
                 const ulonglong2 yy = ts[2 * j + 0];
                 const ulonglong2 gg = ts[2 * j + 1];
+                if (CHECK) verify(j, yy, gg);
                 float sx, sy, gx, gy, dum;
                 upk(yy.x, sx, dum);
                 upk(yy.y, sy, dum);
@@ -406,7 +416,8 @@ __global__ void finish_f32(const long long *__restrict__ acc, int n, int P, cons
 // ------------------------------------------------------------------------------------------------
 // pack + pair kernel for the blocks of one part: acc (P x 2 words) and gmax are the caller's, already zeroed
 static vn_status accumulate_f32(const void *X, const void *F, const void *W, int P, int npts, int part, int nparts,
-                                ulonglong2 *src, long long *acc, unsigned *gmax, cudaStream_t st)
+                                ulonglong2 *src, long long *acc, unsigned *gmax, cudaStream_t st,
+                                unsigned long long *mismatches = nullptr)
 {
     static int slots_dev[kMaxDevices] = {0};
     int &slots = slots_dev[current_device()];
@@ -414,7 +425,7 @@ static vn_status accumulate_f32(const void *X, const void *F, const void *W, int
         int dev = 0, sms = 0, occ = 0;
         VN_CUDA(cudaGetDevice(&dev));
         VN_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-        VN_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, farfield_f32_kernel<kNP32>, kThreads, 0));
+        VN_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, farfield_f32_kernel<kNP32, false>, kThreads, 0));
         slots = sms * (occ > 0 ? occ : 1);
     }
     // the grid is the single-device grid whatever nparts is: the blocks' own roundings are then the same and the
@@ -424,9 +435,12 @@ static vn_status accumulate_f32(const void *X, const void *F, const void *W, int
     const int mine = (int)((blocks - part + nparts - 1) / nparts);
     pack_sources_f32<<<(P + 255) / 256, 256, 0, st>>>((const float2 *)X, (const float2 *)F, (const float *)W, P, src, gmax);
     profile_mark(st, true);
-    if (mine > 0)
-        farfield_f32_kernel<kNP32><<<mine, kThreads, 0, st>>>(src, (const float2 *)X, P, npts, sp.n_tiles, sp.n_st,
-                                                              sp.n_chunks, gmax, acc, part, nparts);
+    if (mine > 0 && !mismatches)
+        farfield_f32_kernel<kNP32, false><<<mine, kThreads, 0, st>>>(src, (const float2 *)X, P, npts, sp.n_tiles, sp.n_st,
+                                                                     sp.n_chunks, gmax, acc, part, nparts, nullptr);
+    else if (mine > 0)
+        farfield_f32_kernel<kNP32, true><<<mine, kThreads, 0, st>>>(src, (const float2 *)X, P, npts, sp.n_tiles, sp.n_st,
+                                                                    sp.n_chunks, gmax, acc, part, nparts, mismatches);
     profile_mark(st, false);
     count_launch(mine > 0 ? 2 : 1);
     return VN_OK;
@@ -447,6 +461,29 @@ vn_status farfield_f32(const void *X, const void *F, const void *W, int64_t nves
     vn_status rc = accumulate_f32(X, F, W, P, (int)npts, 0, 1, src, acc, gmax, st);
     if (rc == VN_OK && near_ptr)   // row f-1: take the near vesicles' contributions out again before the final rounding
         rc = near_correction_f32(X, F, W, P, (int)npts, near_ptr, near_ves, acc, gmax, st);
+    if (rc != VN_OK) { (void)cudaFreeAsync(scratch, st); return rc; }
+    finish_f32<<<(P + 255) / 256, 256, 0, st>>>(acc, P, P, gmax, 1.0 / (4.0 * 3.14159265358979323846 * mu), (float2 *)U);
+    count_launch(1);
+    const cudaError_t e = cudaGetLastError();
+    VN_CUDA(cudaFreeAsync(scratch, st));
+    return e == cudaSuccess ? VN_OK : VN_ERR_CUDA;
+}
+
+// vn_selfcheck: the general path with poisoned scratch (every byte 0xFF before use: a read of scratch that nothing
+// wrote shows up in the result) and the ring verification of the CHECK kernel; *mismatches (device) is incremented.
+vn_status farfield_selfcheck_f32(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, double mu,
+                                 void *U, unsigned long long *mismatches, cudaStream_t st)
+{
+    const int P = (int)(nves * npts);
+    const size_t b_src = (size_t)P * 32, b_acc = (size_t)P * 16;
+    char *scratch = nullptr;
+    VN_CUDA(cudaMallocAsync((void **)&scratch, b_src + b_acc + 16, st));
+    VN_CUDA(cudaMemsetAsync(scratch, 0xFF, b_src + b_acc + 16, st));
+    ulonglong2 *src = (ulonglong2 *)scratch;
+    long long *acc = (long long *)(scratch + b_src);
+    unsigned *gmax = (unsigned *)(scratch + b_src + b_acc);
+    VN_CUDA(cudaMemsetAsync(acc, 0, b_acc + 16, st));
+    const vn_status rc = accumulate_f32(X, F, W, P, (int)npts, 0, 1, src, acc, gmax, st, mismatches);
     if (rc != VN_OK) { (void)cudaFreeAsync(scratch, st); return rc; }
     finish_f32<<<(P + 255) / 256, 256, 0, st>>>(acc, P, P, gmax, 1.0 / (4.0 * 3.14159265358979323846 * mu), (float2 *)U);
     count_launch(1);
@@ -492,6 +529,9 @@ vn_status farfield_finish_f32(const void *acc, const void *gmax, int64_t P_total
 #ifndef VN_TGT32_LASTOUT
 #define VN_TGT32_LASTOUT 0         // 1: stage hand-back by the last warp out as in the pair kernel; measured
 #endif                             // 2008 against 2178 GInt/s at 2000 x 128 sources, 512 x 512 targets: off
+#ifndef VN_TGT32_LOCAL_FIX
+#define VN_TGT32_LOCAL_FIX 1       // a bad distance spoils its own target only (one check per tile, see the kernel)
+#endif
 #ifndef VN_F32_TGT_MINBLK
 #define VN_F32_TGT_MINBLK 3       // measured at 2000 x 128 sources, 512 x 512 targets: 2245 GInt/s against 2229 with 4
 #endif
@@ -597,6 +637,50 @@ targets_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict_
 #pragma unroll 1
             for (int j = 0; j < cnt; ++j) pair(j);
         }
+#if VN_TGT32_LOCAL_FIX
+        {   // The shared reciprocal t = rcp(a b) turns into Inf or 0 when a*b leaves the fp32 normal range (a target on
+            // top of a source, |r| beyond 1e-9 .. 1e9) and then spoils BOTH targets of the packed pair.  One sum over
+            // the tile's partial sums detects it (NaN / Inf is sticky); the warp then redoes this tile with one
+            // reciprocal per pair, so that only the target that owns the bad distance keeps a non-finite value.
+            u64 chk = add2(add2(Ax[0], Ay[0]), add2(Bx[0], By[0]));
+#pragma unroll
+            for (int p = 1; p < NP; ++p) chk = add2(chk, add2(add2(Ax[p], Ay[p]), add2(Bx[p], By[p])));
+            float c0, c1;
+            upk(chk, c0, c1);
+            if (__any_sync(0xffffffffu, !(fabsf(c0 + c1) <= 3.4028234e38f))) {
+#pragma unroll
+                for (int p = 0; p < NP; ++p) {        // unrolled: a dynamic index would move the arrays to local memory
+                    float x0, x1, y0, y1;
+                    upk(tx[p], x0, x1);
+                    upk(ty[p], y0, y1);
+                    float a[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};      // (Ax, Ay, Bx, By) of the two targets
+#pragma unroll 1
+                    for (int j = 0; j < cnt; ++j) {
+                        float sx, sy, gx, gy, dum;
+                        upk(ts[2 * j + 0].x, sx, dum);
+                        upk(ts[2 * j + 0].y, sy, dum);
+                        upk(ts[2 * j + 1].x, gx, dum);
+                        upk(ts[2 * j + 1].y, gy, dum);
+#pragma unroll
+                        for (int h = 0; h < 2; ++h) {
+                            const float rx = (h ? x1 : x0) - sx, ry = (h ? y1 : y0) - sy;
+                            const float r2 = fmaf(rx, rx, ry * ry);
+                            const float l = sfu_lg2(r2);
+                            const float q = fmaf(rx, gx, ry * gy) * sfu_rcp(r2);
+                            a[h][0] = fmaf(l, gx, a[h][0]);
+                            a[h][1] = fmaf(l, gy, a[h][1]);
+                            a[h][2] = fmaf(q, rx, a[h][2]);
+                            a[h][3] = fmaf(q, ry, a[h][3]);
+                        }
+                    }
+                    Ax[p] = pk(a[0][0], a[1][0]);
+                    Ay[p] = pk(a[0][1], a[1][1]);
+                    Bx[p] = pk(a[0][2], a[1][2]);
+                    By[p] = pk(a[0][3], a[1][3]);
+                }
+            }
+        }
+#endif
 #pragma unroll
         for (int p = 0; p < NP; ++p) {
             Rx[p] = add2(Rx[p], fma2(KA, Ax[p], Bx[p]));

@@ -89,10 +89,13 @@ __global__ void pack_sources_f64(const double2 *__restrict__ X, const double2 *_
 // a-3 / a-4: pair kernel; block (I, c) = super-tile I as targets x chunk c of I's list of source tiles
 // (own super-tile one-directional with the own vesicle predicated out, then the tiles of super-tiles
 // I+1 .. I+S_I in both directions) -- the same walk as farfield_f32_kernel.
+// CHECK = true (vn_selfcheck): ring verification as in farfield_f32_kernel.
+template <bool CHECK>
 __global__ void __launch_bounds__(kThreads, VN_F64_MINBLK)
 farfield_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__ X, int P, int npts,
                     int n_tiles, int n_st, int n_chunks, const unsigned long long *__restrict__ gmax_bits,
-                    long long *__restrict__ acc, const double2 *__restrict__ gtab, int part, int nparts)
+                    long long *__restrict__ acc, const double2 *__restrict__ gtab, int part, int nparts,
+                    unsigned long long *__restrict__ mismatches)
 {
     constexpr int T = kT64;
     constexpr int B = kBatch64;
@@ -206,6 +209,13 @@ farfield_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__
         const int first = tile_of(u) * kTile;
         const int cnt = min(kTile, P - first);
         const double4 *ts = tile[s];
+        auto verify = [&](int j, const double4 &sj) {                                // CHECK builds only
+            const double2 *o = reinterpret_cast<const double2 *>(src + first + j);
+            const double2 oa = __ldcg(o), ob = __ldcg(o + 1);
+            if (__double_as_longlong(oa.x) != __double_as_longlong(sj.x) || __double_as_longlong(oa.y) != __double_as_longlong(sj.y) ||
+                __double_as_longlong(ob.x) != __double_as_longlong(sj.z) || __double_as_longlong(ob.y) != __double_as_longlong(sj.w))
+                atomicAdd(mismatches, 1ull);
+        };
         const bool fast = both && (first >= span_end || first + kTile <= span_begin) && (cnt == kTile);
         if (fast) {
             // lane L ends a batch holding the warp total of value L / kDup (value = 2*source + component);
@@ -217,6 +227,7 @@ farfield_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__
 #pragma unroll
                 for (int jj = 0; jj < B; ++jj) {
                     const double4 sj = ts[jb + jj];
+                    if (CHECK) verify(jb + jj, sj);
                     double cx = 0.0, cy = 0.0;
 #pragma unroll
                     for (int k = 0; k < T; ++k) {
@@ -290,6 +301,7 @@ farfield_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__
 #pragma unroll 2
             for (int j = 0; j < kTile; ++j) {
                 const double4 sj = ts[j];
+                if (CHECK) verify(j, sj);
 #pragma unroll
                 for (int k = 0; k < T; ++k) {
                     if (skip[k]) continue;
@@ -310,6 +322,7 @@ farfield_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__
 #pragma unroll 1
             for (int j = 0; j < cnt; ++j) {
                 const double4 sj = ts[j];
+                if (CHECK) verify(j, sj);
                 const int jg = first + j;
                 double cx = 0.0, cy = 0.0;
 #pragma unroll
@@ -383,7 +396,8 @@ __global__ void finish_f64(const long long *__restrict__ acc, int n, int P, cons
 // pack + pair kernel for the blocks of one part: acc (P x 4 words) and gmax are the caller's, already zeroed;
 // scratch holds the packed sources and, behind them, the log tables
 static vn_status accumulate_f64(const void *X, const void *F, const void *W, int P, int npts, int part, int nparts,
-                                char *scratch, long long *acc, unsigned long long *gmax, cudaStream_t st)
+                                char *scratch, long long *acc, unsigned long long *gmax, cudaStream_t st,
+                                unsigned long long *mismatches = nullptr)
 {
     static int slots_dev[kMaxDevices] = {0};
     int &slots = slots_dev[current_device()];
@@ -391,8 +405,9 @@ static vn_status accumulate_f64(const void *X, const void *F, const void *W, int
         int dev = 0, sms = 0, occ = 0;
         VN_CUDA(cudaGetDevice(&dev));
         VN_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-        VN_CUDA(cudaFuncSetAttribute(farfield_f64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kPairSmem));
-        VN_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, farfield_f64_kernel, kThreads, kPairSmem));
+        VN_CUDA(cudaFuncSetAttribute(farfield_f64_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kPairSmem));
+        VN_CUDA(cudaFuncSetAttribute(farfield_f64_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kPairSmem));
+        VN_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, farfield_f64_kernel<false>, kThreads, kPairSmem));
         slots = sms * (occ > 0 ? occ : 1);
     }
     const SymSplit sp = choose_sym_split(P, kST64, slots, VN_F64_MINTILES, VN_F64_MAXTILES);   // see accumulate_f32
@@ -402,9 +417,12 @@ static vn_status accumulate_f64(const void *X, const void *F, const void *W, int
     double *gtab = VN_F64_GTAB ? (double *)(scratch + (size_t)P * 32) : nullptr;   // 16-byte aligned
     pack_sources_f64<<<(P + 255) / 256, 256, 0, st>>>((const double2 *)X, (const double2 *)F, (const double *)W, P, src, gmax, gtab);
     profile_mark(st, true);
-    if (mine > 0)
-        farfield_f64_kernel<<<mine, kThreads, kPairSmem, st>>>(src, (const double2 *)X, P, npts, sp.n_tiles, sp.n_st,
-                                                               sp.n_chunks, gmax, acc, (const double2 *)gtab, part, nparts);
+    if (mine > 0 && !mismatches)
+        farfield_f64_kernel<false><<<mine, kThreads, kPairSmem, st>>>(src, (const double2 *)X, P, npts, sp.n_tiles, sp.n_st,
+                                                                      sp.n_chunks, gmax, acc, (const double2 *)gtab, part, nparts, nullptr);
+    else if (mine > 0)
+        farfield_f64_kernel<true><<<mine, kThreads, kPairSmem, st>>>(src, (const double2 *)X, P, npts, sp.n_tiles, sp.n_st,
+                                                                     sp.n_chunks, gmax, acc, (const double2 *)gtab, part, nparts, mismatches);
     profile_mark(st, false);
     count_launch(mine > 0 ? 2 : 1);
     return VN_OK;
@@ -425,6 +443,27 @@ vn_status farfield_f64(const void *X, const void *F, const void *W, int64_t nves
     vn_status rc = accumulate_f64(X, F, W, P, (int)npts, 0, 1, scratch, acc, gmax, st);
     if (rc == VN_OK && near_ptr)   // row f-1: take the near vesicles' contributions out again before the final rounding
         rc = near_correction_f64(X, F, W, P, (int)npts, near_ptr, near_ves, acc, gmax, st);
+    if (rc != VN_OK) { (void)cudaFreeAsync(scratch, st); return rc; }
+    finish_f64<<<(P + 255) / 256, 256, 0, st>>>(acc, P, P, gmax, 1.0 / (4.0 * 3.14159265358979323846 * mu), (double2 *)U);
+    count_launch(1);
+    const cudaError_t e = cudaGetLastError();
+    VN_CUDA(cudaFreeAsync(scratch, st));
+    return e == cudaSuccess ? VN_OK : VN_ERR_CUDA;
+}
+
+// vn_selfcheck (see farfield_selfcheck_f32)
+vn_status farfield_selfcheck_f64(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, double mu,
+                                 void *U, unsigned long long *mismatches, cudaStream_t st)
+{
+    const int P = (int)(nves * npts);
+    const size_t b_src = scratch_f64_bytes(P), b_acc = (size_t)P * 32;
+    char *scratch = nullptr;
+    VN_CUDA(cudaMallocAsync((void **)&scratch, b_src + b_acc + 16, st));
+    VN_CUDA(cudaMemsetAsync(scratch, 0xFF, b_src + b_acc + 16, st));
+    long long *acc = (long long *)(scratch + b_src);
+    unsigned long long *gmax = (unsigned long long *)(scratch + b_src + b_acc);
+    VN_CUDA(cudaMemsetAsync(acc, 0, b_acc + 16, st));
+    const vn_status rc = accumulate_f64(X, F, W, P, (int)npts, 0, 1, scratch, acc, gmax, st, mismatches);
     if (rc != VN_OK) { (void)cudaFreeAsync(scratch, st); return rc; }
     finish_f64<<<(P + 255) / 256, 256, 0, st>>>(acc, P, P, gmax, 1.0 / (4.0 * 3.14159265358979323846 * mu), (double2 *)U);
     count_launch(1);

@@ -374,8 +374,11 @@ fmm_m2m(int level, int q, const double *__restrict__ tab, const unsigned long lo
 constexpr int kM2LWarps = 4;
 __global__ void __launch_bounds__(32 * kM2LWarps)
 fmm_m2l(int level, int q, const double *__restrict__ tab, const unsigned long long *__restrict__ enc,
-        const cplx *__restrict__ mult, const int *__restrict__ boxcnt, cplx *__restrict__ loc)
-{
+        const cplx *__restrict__ mult, const int *__restrict__ boxcnt, const int *__restrict__ tboxcnt,
+        cplx *__restrict__ loc)
+{   // tboxcnt: population of the TARGET boxes (the sources' own counts for vn_farfield_fmm; nullptr when the targets
+    // are a separate set and every box may hold some): a box without targets needs no local expansion -- in a 4:1
+    // channel three quarters of the root square's boxes are empty
     if (level > load_level(enc)) return;
     extern __shared__ __align__(16) double sm[];
     double *Cb = sm;                                                  // [q][q]
@@ -390,6 +393,7 @@ fmm_m2l(int level, int q, const double *__restrict__ tab, const unsigned long lo
     const int l0 = ln, l1 = ln + 32;
     const bool v0 = l0 < q, v1 = l1 < q;
     for (int box = blockIdx.x * kM2LWarps + warp; box < n * n; box += gridDim.x * kM2LWarps) {
+    if (tboxcnt && tboxcnt[level_offset(level) + box] == 0) continue;
     const int ix = box / n, iy = box % n;
     cplx acc[3][2];
 #pragma unroll
@@ -467,7 +471,7 @@ fmm_m2l(int level, int q, const double *__restrict__ tab, const unsigned long lo
 // L2L: child local expansions inherit the parent's.  One thread per (child box, k); child level = `level`.
 __global__ void __launch_bounds__(128)
 fmm_l2l(int level, int q, const double *__restrict__ tab, const unsigned long long *__restrict__ enc,
-        cplx *__restrict__ loc)
+        const int *__restrict__ tboxcnt, cplx *__restrict__ loc)
 {
     if (level > load_level(enc)) return;
     const FmmTables t = fmm_tables_at(const_cast<double *>(tab), q);
@@ -475,6 +479,7 @@ fmm_l2l(int level, int q, const double *__restrict__ tab, const unsigned long lo
     const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (e >= (long long)n * n * q) return;
     const int box = (int)(e / q), k = (int)(e % q);
+    if (tboxcnt && tboxcnt[level_offset(level) + box] == 0) return;      // no targets below this box (see fmm_m2l)
     const int ix = box / n, iy = box % n, c = 2 * (ix & 1) + (iy & 1);
     const cplx *par = loc + (level_offset(level - 1) + (long long)(ix >> 1) * (n >> 1) + (iy >> 1)) * (long long)(3 * q);
     const cplx *row = t.T + ((size_t)c * q + k) * q;
@@ -762,12 +767,12 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
     const size_t smem_m2l = sizeof(double) * (size_t)(((q * q + 1) & ~1) + 2 * kM2LWarps * 3 * (q + 1));
     for (int l = 2; l <= L; ++l) {
         const unsigned nb = ((1u << (2 * l)) + kM2LWarps - 1) / kM2LWarps;
-        fmm_m2l<<<nb < 148u * 16u ? nb : 148u * 16u, 32 * kM2LWarps, smem_m2l, st>>>(l, q, tab, enc, mult, boxcnt, loc);
+        fmm_m2l<<<nb < 148u * 16u ? nb : 148u * 16u, 32 * kM2LWarps, smem_m2l, st>>>(l, q, tab, enc, mult, boxcnt, boxcnt, loc);
         ++launches;
     }
     for (int l = 3; l <= L; ++l) {
         const long long work = (1ll << (2 * l)) * q;
-        fmm_l2l<<<(unsigned)((work + 127) / 128), 128, 0, st>>>(l, q, tab, enc, loc);
+        fmm_l2l<<<(unsigned)((work + 127) / 128), 128, 0, st>>>(l, q, tab, enc, boxcnt, loc);
         ++launches;
     }
     if (prec == VN_F32)
@@ -915,12 +920,12 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
     const size_t smem_m2l = sizeof(double) * (size_t)(((q * q + 1) & ~1) + 2 * kM2LWarps * 3 * (q + 1));
     for (int l = 2; l <= L; ++l) {
         const unsigned nb = ((1u << (2 * l)) + kM2LWarps - 1) / kM2LWarps;
-        fmm_m2l<<<nb < 148u * 16u ? nb : 148u * 16u, 32 * kM2LWarps, smem_m2l, st>>>(l, q, tab, enc, mult, boxcnt, loc);
+        fmm_m2l<<<nb < 148u * 16u ? nb : 148u * 16u, 32 * kM2LWarps, smem_m2l, st>>>(l, q, tab, enc, mult, boxcnt, nullptr, loc);
         ++launches;
     }
     for (int l = 3; l <= L; ++l) {
         const long long work = (1ll << (2 * l)) * q;
-        fmm_l2l<<<(unsigned)((work + 127) / 128), 128, 0, st>>>(l, q, tab, enc, loc);
+        fmm_l2l<<<(unsigned)((work + 127) / 128), 128, 0, st>>>(l, q, tab, enc, nullptr, loc);
         ++launches;
     }
     if (prec == VN_F32)
