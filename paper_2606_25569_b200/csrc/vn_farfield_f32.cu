@@ -44,6 +44,9 @@ constexpr int kSub32 = kST32 / kTile;             // source tiles per super-tile
 #define VN_F32_SHARED_RCP 0                       // 1: the two r2 of a packed pair share one SFU reciprocal
 #endif
 constexpr int kBatch = VN_F32_BATCH;              // sources per cross-lane reduction batch
+#ifndef VN_F32_SMEMRED
+#define VN_F32_SMEMRED 0                          // 0: register transpose-reduce (shuffles); 1: transposed shared-memory
+#endif                                            // buffer; 2: the same, summed while the next batch is computed
 
 // ------------------------------------------------------------------------------------------------
 // a-2: g = F*W, packed with the position into one 32-byte record per source, every value
@@ -96,6 +99,10 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
     __shared__ __align__(128) ulonglong2 tile[kStages][kTile * 2];
     __shared__ __align__(8) u64 full_bar[kStages];
     __shared__ int drained[kStages];                 // warps that have left each stage (stage_last_out)
+#if VN_F32_SMEMRED
+    constexpr int kRedRow = 40, kRedHalf = 20;       // floats: 16-byte loads of half rows are conflict-free
+    __shared__ __align__(16) float red[kThreads / 32][2 * kBatch * kRedRow];
+#endif
 
     const int tid = threadIdx.x;
     const int lane = tid & 31;
@@ -196,9 +203,8 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
             for (int p = 0; p < NP; ++p) Ux[p] = Uy[p] = 0ull;
             constexpr int kDup = 32 / (2 * kBatch);       // lanes that end a batch with the same warp total
             long long *accj = acc + 2 * (size_t)first + lane / kDup;
-#pragma unroll 1
-            for (int jb = 0; jb < kTile; jb += kBatch) {
-                float c[2 * kBatch];              // this thread's contributions to the batch's sources
+            // this thread's contributions c[2 jj], c[2 jj + 1] to the sources jb .. jb + kBatch - 1 (and its own sums Ux, Uy)
+            auto batch = [&](int jb, float (&c)[2 * kBatch]) {
 #pragma unroll
                 for (int jj = 0; jj < kBatch; ++jj) {
                     const ulonglong2 yy = ts[2 * (jb + jj) + 0];   // (yx,yx) (yy,yy)
@@ -247,6 +253,69 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
                     upk(cUy, lo, hi);
                     c[2 * jj + 1] = lo + hi;
                 }
+            };
+#if VN_F32_SMEMRED == 2
+            // The c values of a batch are parked in a transposed shared-memory buffer and summed over the warp
+            // while the NEXT batch is computed: the loads are issued before that batch's arithmetic and nothing
+            // of it depends on them, so the reduction's latency chain hides behind 576 packed instructions
+            // instead of ending every batch.
+            static_assert(kDup == 2, "shared-memory reduction assumes 16 values per batch");
+            float *rw = red[tid >> 5];
+            const int col = lane + (lane >= 16 ? kRedHalf - 16 : 0);
+            const float4 *row = reinterpret_cast<const float4 *>(rw + (lane >> 1) * kRedRow + (lane & 1) * kRedHalf);
+            auto park = [&](const float (&c)[2 * kBatch]) {
+                __syncwarp();                                       // every lane has read the previous batch's rows
+#pragma unroll
+                for (int v = 0; v < 2 * kBatch; ++v) rw[v * kRedRow + col] = c[v];
+            };
+            auto total = [&](const float4 &q0, const float4 &q1, const float4 &q2, const float4 &q3) {
+                float t = ((q0.x + q0.y) + (q0.z + q0.w)) + ((q1.x + q1.y) + (q1.z + q1.w)) +
+                          (((q2.x + q2.y) + (q2.z + q2.w)) + ((q3.x + q3.y) + (q3.z + q3.w)));
+                t += __shfl_xor_sync(0xffffffffu, t, 1);
+                return t;
+            };
+            {
+                float c[2 * kBatch];
+                batch(0, c);
+                park(c);
+            }
+#pragma unroll 1
+            for (int jb = kBatch; jb < kTile; jb += kBatch) {
+                __syncwarp();                                       // the parked rows are complete
+                const float4 q0 = row[0], q1 = row[1], q2 = row[2], q3 = row[3];
+                float c[2 * kBatch];
+                batch(jb, c);
+                const float t = total(q0, q1, q2, q3);
+                if (lane % kDup == 0) red_fixed(accj + 2 * (jb - kBatch), t * -0.34657359027997264f, scale);
+                park(c);
+            }
+            {
+                __syncwarp();
+                const float4 q0 = row[0], q1 = row[1], q2 = row[2], q3 = row[3];
+                const float t = total(q0, q1, q2, q3);
+                if (lane % kDup == 0) red_fixed(accj + 2 * (kTile - kBatch), t * -0.34657359027997264f, scale);
+            }
+#else
+#pragma unroll 1
+            for (int jb = 0; jb < kTile; jb += kBatch) {
+                float c[2 * kBatch];              // this thread's contributions to the batch's sources
+                batch(jb, c);
+#if VN_F32_SMEMRED == 1
+                static_assert(kDup == 2, "shared-memory reduction assumes 16 values per batch");
+                {
+                    float *rw = red[tid >> 5];
+                    const int col = lane + (lane >= 16 ? kRedHalf - 16 : 0);
+                    __syncwarp();                                   // the previous batch's reads are done
+#pragma unroll
+                    for (int v = 0; v < 2 * kBatch; ++v) rw[v * kRedRow + col] = c[v];
+                    __syncwarp();
+                    const float4 *row = reinterpret_cast<const float4 *>(rw + (lane >> 1) * kRedRow + (lane & 1) * kRedHalf);
+                    const float4 q0 = row[0], q1 = row[1], q2 = row[2], q3 = row[3];
+                    c[0] = ((q0.x + q0.y) + (q0.z + q0.w)) + ((q1.x + q1.y) + (q1.z + q1.w)) +
+                           (((q2.x + q2.y) + (q2.z + q2.w)) + ((q3.x + q3.y) + (q3.z + q3.w)));
+                    c[0] += __shfl_xor_sync(0xffffffffu, c[0], 1);
+                }
+#else
                 // transpose-reduce over the warp: 16 values per lane -> lane L ends with the warp
                 // total of value L / kDup; 16 shuffles instead of 16 x 5 at kBatch = 8.
                 int m = 16;
@@ -262,8 +331,10 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
                 }
 #pragma unroll
                 for (; m >= 1; m >>= 1) c[0] += __shfl_xor_sync(0xffffffffu, c[0], m);
+#endif
                 if (lane % kDup == 0) red_fixed(accj + 2 * jb, c[0] * -0.34657359027997264f, scale);
             }
+#endif
 #pragma unroll
             for (int p = 0; p < NP; ++p) {
                 Rx[p] = fma2(KA, Ux[p], Rx[p]);
