@@ -44,9 +44,17 @@ constexpr int kSub32 = kST32 / kTile;             // source tiles per super-tile
 #define VN_F32_SHARED_RCP 0                       // 1: the two r2 of a packed pair share one SFU reciprocal
 #endif
 constexpr int kBatch = VN_F32_BATCH;              // sources per cross-lane reduction batch
+#ifndef VN_F32_RED_UNROLL
+#define VN_F32_RED_UNROLL 1                       // batches per scheduling region of the deferred-reduction loop: 3, 5, 15 measured
+#endif                                            // -10 %, -27 %, -36 % at 2000 x 128 (13 KB of SASS per batch: instruction cache)
+constexpr int kRedUnroll = VN_F32_RED_UNROLL;
 #ifndef VN_F32_SMEMRED
-#define VN_F32_SMEMRED 0                          // 0: register transpose-reduce (shuffles); 1: transposed shared-memory
-#endif                                            // buffer; 2: the same, summed while the next batch is computed
+#define VN_F32_SMEMRED 2                          // how the j <- i contributions of a batch are summed over the warp.
+#endif                                            // 0: register transpose-reduce (16 shuffles); 1: transposed shared-memory
+                                                  // buffer; 2: the same, summed while the NEXT batch is computed; 3: as 2 with
+                                                  // the packed pairs parked as they are.  Measured at 8000 x 128 / 2000 x 128 /
+                                                  // 256 x 128 (GInt/s): 0: 2942 / 2905 / 2203, 1: 2971 / 2938 / 2233,
+                                                  // 2: 3078 / 3046 / 2295, 3: 2987 / 2955 / 2246
 
 // ------------------------------------------------------------------------------------------------
 // a-2: g = F*W, packed with the position into one 32-byte record per source, every value
@@ -99,7 +107,10 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
     __shared__ __align__(128) ulonglong2 tile[kStages][kTile * 2];
     __shared__ __align__(8) u64 full_bar[kStages];
     __shared__ int drained[kStages];                 // warps that have left each stage (stage_last_out)
-#if VN_F32_SMEMRED
+#if VN_F32_SMEMRED == 3
+    constexpr int kRedRow = 72, kRedHalf = 36;       // 64 floats per row (both halves of every lane's packed pair)
+    __shared__ __align__(16) float red[kThreads / 32][2 * kBatch * kRedRow];
+#elif VN_F32_SMEMRED
     constexpr int kRedRow = 40, kRedHalf = 20;       // floats: 16-byte loads of half rows are conflict-free
     __shared__ __align__(16) float red[kThreads / 32][2 * kBatch * kRedRow];
 #endif
@@ -204,7 +215,7 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
             constexpr int kDup = 32 / (2 * kBatch);       // lanes that end a batch with the same warp total
             long long *accj = acc + 2 * (size_t)first + lane / kDup;
             // this thread's contributions c[2 jj], c[2 jj + 1] to the sources jb .. jb + kBatch - 1 (and its own sums Ux, Uy)
-            auto batch = [&](int jb, float (&c)[2 * kBatch]) {
+            auto batch = [&](int jb, u64 (&cp)[2 * kBatch]) {
 #pragma unroll
                 for (int jj = 0; jj < kBatch; ++jj) {
                     const ulonglong2 yy = ts[2 * (jb + jj) + 0];   // (yx,yx) (yy,yy)
@@ -247,14 +258,63 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
                         Ux[p] = fma2(Mxy, gg.y, Ux[p]);
                         Uy[p] = fma2(Mxy, gg.x, Uy[p]);
                     }
-                    float lo, hi;
-                    upk(cUx, lo, hi);
-                    c[2 * jj + 0] = lo + hi;
-                    upk(cUy, lo, hi);
-                    c[2 * jj + 1] = lo + hi;
+                    cp[2 * jj + 0] = cUx;       // both targets of the packed pair still side by side
+                    cp[2 * jj + 1] = cUy;
                 }
             };
-#if VN_F32_SMEMRED == 2
+            auto fold = [&](const u64 (&cp)[2 * kBatch], float (&c)[2 * kBatch]) {
+#pragma unroll
+                for (int v = 0; v < 2 * kBatch; ++v) {
+                    float lo, hi;
+                    upk(cp[v], lo, hi);
+                    c[v] = lo + hi;
+                }
+            };
+#if VN_F32_SMEMRED == 3
+            // As mode 2, but the packed pairs are parked as they are (STS.64): the lo + hi additions move out of the
+            // batch's arithmetic into the deferred sum (32 floats per lane instead of 16).
+            static_assert(kDup == 2, "shared-memory reduction assumes 16 values per batch");
+            float *rw = red[tid >> 5];
+            const int col = 2 * lane + (lane >= 16 ? kRedHalf - 32 : 0);
+            const float4 *row = reinterpret_cast<const float4 *>(rw + (lane >> 1) * kRedRow + (lane & 1) * kRedHalf);
+            auto park = [&](const u64 (&cp)[2 * kBatch]) {
+                __syncwarp();                                       // every lane has read the previous batch's rows
+#pragma unroll
+                for (int v = 0; v < 2 * kBatch; ++v) *reinterpret_cast<u64 *>(rw + v * kRedRow + col) = cp[v];
+            };
+            auto sum4 = [](const float4 &q) { return (q.x + q.y) + (q.z + q.w); };
+            auto total = [&](const float4 (&q)[8]) {
+                float t = ((sum4(q[0]) + sum4(q[1])) + (sum4(q[2]) + sum4(q[3]))) +
+                          ((sum4(q[4]) + sum4(q[5])) + (sum4(q[6]) + sum4(q[7])));
+                t += __shfl_xor_sync(0xffffffffu, t, 1);
+                return t;
+            };
+            {
+                u64 cp[2 * kBatch];
+                batch(0, cp);
+                park(cp);
+            }
+#pragma unroll kRedUnroll
+            for (int jb = kBatch; jb < kTile; jb += kBatch) {
+                __syncwarp();                                       // the parked rows are complete
+                float4 q[8];
+#pragma unroll
+                for (int e = 0; e < 8; ++e) q[e] = row[e];
+                u64 cp[2 * kBatch];
+                batch(jb, cp);
+                const float t = total(q);
+                if (lane % kDup == 0) red_fixed(accj + 2 * (jb - kBatch), t * -0.34657359027997264f, scale);
+                park(cp);
+            }
+            {
+                __syncwarp();
+                float4 q[8];
+#pragma unroll
+                for (int e = 0; e < 8; ++e) q[e] = row[e];
+                const float t = total(q);
+                if (lane % kDup == 0) red_fixed(accj + 2 * (kTile - kBatch), t * -0.34657359027997264f, scale);
+            }
+#elif VN_F32_SMEMRED == 2
             // The c values of a batch are parked in a transposed shared-memory buffer and summed over the warp
             // while the NEXT batch is computed: the loads are issued before that batch's arithmetic and nothing
             // of it depends on them, so the reduction's latency chain hides behind 576 packed instructions
@@ -275,16 +335,20 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
                 return t;
             };
             {
+                u64 cp[2 * kBatch];
                 float c[2 * kBatch];
-                batch(0, c);
+                batch(0, cp);
+                fold(cp, c);
                 park(c);
             }
-#pragma unroll 1
+#pragma unroll kRedUnroll
             for (int jb = kBatch; jb < kTile; jb += kBatch) {
                 __syncwarp();                                       // the parked rows are complete
                 const float4 q0 = row[0], q1 = row[1], q2 = row[2], q3 = row[3];
+                u64 cp[2 * kBatch];
                 float c[2 * kBatch];
-                batch(jb, c);
+                batch(jb, cp);
+                fold(cp, c);
                 const float t = total(q0, q1, q2, q3);
                 if (lane % kDup == 0) red_fixed(accj + 2 * (jb - kBatch), t * -0.34657359027997264f, scale);
                 park(c);
@@ -298,8 +362,10 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
 #else
 #pragma unroll 1
             for (int jb = 0; jb < kTile; jb += kBatch) {
+                u64 cp[2 * kBatch];
                 float c[2 * kBatch];              // this thread's contributions to the batch's sources
-                batch(jb, c);
+                batch(jb, cp);
+                fold(cp, c);
 #if VN_F32_SMEMRED == 1
                 static_assert(kDup == 2, "shared-memory reduction assumes 16 values per batch");
                 {

@@ -221,9 +221,8 @@ farfield_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__
             // lane L ends a batch holding the warp total of value L / kDup (value = 2*source + component);
             // sub-lane 0 adds its high word, sub-lane 1 its low word
             long long *accj = acc + 4 * (size_t)first + 2 * (lane / kDup) + (lane % kDup);
-#pragma unroll 1
-            for (int jb = 0; jb < kTile; jb += B) {
-                double c[2 * B];
+            // this thread's contributions c[2 jj], c[2 jj + 1] to the sources jb .. jb + B - 1 (and its own sums Ux, Uy)
+            auto batch = [&](int jb, double (&c)[2 * B]) {
 #pragma unroll
                 for (int jj = 0; jj < B; ++jj) {
                     const double4 sj = ts[jb + jj];
@@ -247,7 +246,58 @@ farfield_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__
                     c[2 * jj + 0] = cx;
                     c[2 * jj + 1] = cy;
                 }
-#if VN_F64_SMEMRED
+            };
+#if VN_F64_SMEMRED == 2
+            // The c values of a batch are parked in the transposed shared-memory buffer and summed over the warp while
+            // the NEXT batch is computed (loads issued before that batch's arithmetic, nothing of it depends on them).
+            static_assert(kDup == 2, "shared-memory reduction assumes 16 values per batch");
+            double *rw = red[tid >> 5];
+            const int col = lane + (lane >= 16 ? kRedHalf - 16 : 0);
+            const double2 *row = reinterpret_cast<const double2 *>(rw + (lane >> 1) * kRedRow + (lane & 1) * kRedHalf);
+            auto park = [&](const double (&c)[2 * B]) {
+                __syncwarp();                                       // every lane has read the previous batch's rows
+#pragma unroll
+                for (int v = 0; v < 2 * B; ++v) rw[v * kRedRow + col] = c[v];
+            };
+            auto total = [&](const double2 (&q)[8]) {
+                double t = (((q[0].x + q[0].y) + (q[1].x + q[1].y)) + ((q[2].x + q[2].y) + (q[3].x + q[3].y))) +
+                           (((q[4].x + q[4].y) + (q[5].x + q[5].y)) + ((q[6].x + q[6].y) + (q[7].x + q[7].y)));
+                t += __shfl_xor_sync(0xffffffffu, t, 1);
+                return t;
+            };
+            {
+                double c[2 * B];
+                batch(0, c);
+                park(c);
+            }
+#pragma unroll 1
+            for (int jb = B; jb < kTile; jb += B) {
+                __syncwarp();                                       // the parked rows are complete
+                double2 q[8];
+#pragma unroll
+                for (int e = 0; e < 8; ++e) q[e] = row[e];
+                double c[2 * B];
+                batch(jb, c);
+                const double t = total(q);
+                if ((lane % kDup) < 2)
+                    atomicAdd((unsigned long long *)(accj + 4 * (jb - B)), (unsigned long long)fixed2_word(t, fx, lane % kDup));
+                park(c);
+            }
+            {
+                __syncwarp();
+                double2 q[8];
+#pragma unroll
+                for (int e = 0; e < 8; ++e) q[e] = row[e];
+                const double t = total(q);
+                if ((lane % kDup) < 2)
+                    atomicAdd((unsigned long long *)(accj + 4 * (kTile - B)), (unsigned long long)fixed2_word(t, fx, lane % kDup));
+            }
+#else
+#pragma unroll 1
+            for (int jb = 0; jb < kTile; jb += B) {
+                double c[2 * B];
+                batch(jb, c);
+#if VN_F64_SMEMRED == 1
                 // sum over the warp through shared memory: lane L stores value v at row v, column L; then lane L
                 // adds up half (L & 1) of row L >> 1 and the two halves meet in one shuffle: lane L ends with the
                 // warp total of value L / 2 (kDup = 2 at B = 8)
@@ -290,6 +340,7 @@ farfield_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__
                     atomicAdd((unsigned long long *)(accj + 4 * jb),
                               (unsigned long long)fixed2_word(c[0], fx, lane % kDup));
             }
+#endif
         } else if (!both && cnt == kTile && npts % kTile == 0 && base + kST64 <= P) {
             // a tile of the block's OWN super-tile when vesicles are whole tiles (npts a multiple of 128): target k
             // of every thread lies in tile k, so "own vesicle" is the same decision for the whole block -- a uniform
