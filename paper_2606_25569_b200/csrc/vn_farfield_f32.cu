@@ -111,7 +111,14 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
     constexpr int kRedRow = 72, kRedHalf = 36;       // 64 floats per row (both halves of every lane's packed pair)
     __shared__ __align__(16) float red[kThreads / 32][2 * kBatch * kRedRow];
 #elif VN_F32_SMEMRED
-    constexpr int kRedRow = 40, kRedHalf = 20;       // floats: 16-byte loads of half rows are conflict-free
+#ifndef VN_F32_REDROW
+#define VN_F32_REDROW 40          // row stride and half-row offset in floats.  40 / 20: the 16-byte loads of half rows are
+#define VN_F32_REDHALF 20         // conflict-free, the 4-byte stores of lanes 16-19 share banks with lanes 0-3 (2-way, 20 %
+#endif                            // of the kernel's shared-memory wavefronts are replays); 36 / 16 is conflict-free for both
+                                  // and measured 0.5 % SLOWER (3063 against 3079 GInt/s at 8000 x 128), as was a double-buffered
+                                  // variant with one __syncwarp per batch (2991): the kernel's speed follows ptxas's schedule,
+                                  // not the shared-memory traffic (8 % of the LSU pipe)
+    constexpr int kRedRow = VN_F32_REDROW, kRedHalf = VN_F32_REDHALF;
     __shared__ __align__(16) float red[kThreads / 32][2 * kBatch * kRedRow];
 #endif
 
