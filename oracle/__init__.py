@@ -14,6 +14,7 @@ from __future__ import annotations
 import ctypes
 import os
 import subprocess
+import zlib
 
 import numpy as np
 
@@ -36,11 +37,30 @@ def build(force: bool = False) -> str:
     return _LIB
 
 
+def _cpu_stamp() -> str:
+    """Identifies the instruction set of this machine (-march=native binaries must not travel between machines)."""
+    try:
+        with open("/proc/cpuinfo") as fh:
+            for line in fh:
+                if line.startswith("flags"):
+                    return str(zlib.crc32(line.split(":", 1)[1].strip().encode()))
+    except OSError:
+        pass
+    return "unknown"
+
+
 def build_baseline(force: bool = False) -> str:
     """Compile baseline_f64.c, the plain-double SPEED baseline (not the parity oracle; see its header).
-    -march=native: always rebuilt on the machine that times it (bench.py passes force=True)."""
-    if force or not os.path.exists(_BASE_LIB) or os.path.getmtime(_BASE_LIB) < os.path.getmtime(_BASE_SRC):
+    -march=native: rebuilt whenever the library was made on a machine with another instruction set (the in-tree .so
+    travels to the GPU box with the snapshot), and always on the machine that times it (bench.py passes force=True)."""
+    stamp_file = _BASE_LIB + ".cpu"
+    stamp = _cpu_stamp()
+    old = open(stamp_file).read().strip() if os.path.exists(stamp_file) else ""
+    if (force or old != stamp or not os.path.exists(_BASE_LIB)
+            or os.path.getmtime(_BASE_LIB) < os.path.getmtime(_BASE_SRC)):
         subprocess.run(["gcc"] + _BASE_FLAGS + ["-fPIC", "-shared", "-o", _BASE_LIB, _BASE_SRC, "-lm"], check=True)
+        with open(stamp_file, "w") as fh:
+            fh.write(stamp)
     return _BASE_LIB
 
 

@@ -48,6 +48,9 @@ constexpr int kBatch = VN_F32_BATCH;              // sources per cross-lane redu
 #define VN_F32_RED_UNROLL 1                       // batches per scheduling region of the deferred-reduction loop: 3, 5, 15 measured
 #endif                                            // -10 %, -27 %, -36 % at 2000 x 128 (13 KB of SASS per batch: instruction cache)
 constexpr int kRedUnroll = VN_F32_RED_UNROLL;
+#ifndef VN_F32_PREFETCH
+#define VN_F32_PREFETCH 0                         // 1 (mode 2 only): the first source record of a batch is loaded a batch ahead
+#endif
 #ifndef VN_F32_SMEMRED
 #define VN_F32_SMEMRED 2                          // how the j <- i contributions of a batch are summed over the warp.
 #endif                                            // 0: register transpose-reduce (16 shuffles); 1: transposed shared-memory
@@ -222,11 +225,19 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
             constexpr int kDup = 32 / (2 * kBatch);       // lanes that end a batch with the same warp total
             long long *accj = acc + 2 * (size_t)first + lane / kDup;
             // this thread's contributions c[2 jj], c[2 jj + 1] to the sources jb .. jb + kBatch - 1 (and its own sums Ux, Uy)
+#if VN_F32_PREFETCH
+            ulonglong2 pre_y = ts[0], pre_g = ts[1];      // the first source of the next batch, loaded a batch ahead
+#endif
             auto batch = [&](int jb, u64 (&cp)[2 * kBatch]) {
 #pragma unroll
                 for (int jj = 0; jj < kBatch; ++jj) {
+#if VN_F32_PREFETCH
+                    const ulonglong2 yy = jj == 0 ? pre_y : ts[2 * (jb + jj) + 0];
+                    const ulonglong2 gg = jj == 0 ? pre_g : ts[2 * (jb + jj) + 1];
+#else
                     const ulonglong2 yy = ts[2 * (jb + jj) + 0];   // (yx,yx) (yy,yy)
                     const ulonglong2 gg = ts[2 * (jb + jj) + 1];   // (gx,gx) (gy,gy)
+#endif
                     if (CHECK) verify(jb + jj, yy, gg);
                     u64 rx[NP], ry[NP], l[NP], inv[NP];
 #pragma unroll
@@ -345,6 +356,10 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
                 u64 cp[2 * kBatch];
                 float c[2 * kBatch];
                 batch(0, cp);
+#if VN_F32_PREFETCH
+                pre_y = ts[2 * kBatch + 0];
+                pre_g = ts[2 * kBatch + 1];
+#endif
                 fold(cp, c);
                 park(c);
             }
@@ -355,6 +370,13 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
                 u64 cp[2 * kBatch];
                 float c[2 * kBatch];
                 batch(jb, cp);
+#if VN_F32_PREFETCH
+                {
+                    const int jn = min(jb + kBatch, kTile - 1);     // (the last batch of a tile prefetches a record it will not use)
+                    pre_y = ts[2 * jn + 0];
+                    pre_g = ts[2 * jn + 1];
+                }
+#endif
                 fold(cp, c);
                 const float t = total(q0, q1, q2, q3);
                 if (lane % kDup == 0) red_fixed(accj + 2 * (jb - kBatch), t * -0.34657359027997264f, scale);
