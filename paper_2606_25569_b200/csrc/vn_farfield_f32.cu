@@ -49,7 +49,8 @@ constexpr int kBatch = VN_F32_BATCH;              // sources per cross-lane redu
 #endif                                            // -10 %, -27 %, -36 % at 2000 x 128 (13 KB of SASS per batch: instruction cache)
 constexpr int kRedUnroll = VN_F32_RED_UNROLL;
 #ifndef VN_F32_PREFETCH
-#define VN_F32_PREFETCH 0                         // 1 (mode 2 only): the first source record of a batch is loaded a batch ahead
+#define VN_F32_PREFETCH 0                         // 1 (mode 2 only): the first source record of a batch is loaded a batch ahead;
+                                                  // measured 3043 against 3079 GInt/s at 8000 x 128: off
 #endif
 #ifndef VN_F32_SMEMRED
 #define VN_F32_SMEMRED 2                          // how the j <- i contributions of a batch are summed over the warp.
