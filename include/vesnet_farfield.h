@@ -40,9 +40,11 @@
  *      VN_ERR_CUDA         a CUDA runtime call failed (allocation, launch)
  *    Argument checks happen before any CUDA call, so they work without a GPU.
  *  - VN_F32 uses the SFU approximations rcp/lg2 (flush-to-zero): squared distances must be normal
- *    fp32 numbers, and vn_farfield_targets additionally shares one reciprocal between two pairs
- *    (t = rcp(a*b), 1/a = t*b), which needs a*b inside the fp32 normal range, i.e.
- *    1e-9 < |r| < 1e9 in the caller's units.  VN_F64 needs normal doubles whose reciprocal is normal.
+ *    fp32 numbers.  vn_farfield_targets additionally shares one reciprocal between two pairs
+ *    (t = rcp(a*b), 1/a = t*b), which is exact only while a*b stays inside the fp32 normal range
+ *    (1e-9 < |r| < 1e9 in the caller's units); a tile in which that fails (a target on top of a source,
+ *    say) is detected and redone with one reciprocal per pair, so that a bad distance spoils the value of
+ *    its own target only.  VN_F64 needs normal doubles whose reciprocal is normal.
  *  - Input values are not validated.  A non-finite value anywhere in X, F or W makes EVERY output of
  *    vn_farfield / vn_farfield_masked / vn_farfield_targets NaN (their integer accumulators cannot carry
  *    NaN/Inf point by point; a free target's own coordinates are not checked); the FMM calls, and vn_farfield

@@ -44,7 +44,11 @@ constexpr int kSub64 = kST64 / kTile;         // source tiles per super-tile: 4
 #ifndef VN_F64_SMEMRED
 #define VN_F64_SMEMRED 1          // 1: the j <- i contributions of a batch are summed over the warp through a transposed
 #endif                            // shared-memory buffer (16 STS.64 + 8 LDS.128 + 2 SHFL) instead of the register
-                                  // transpose-reduce (32 SHFL + 60 FSEL + 45 MOV for 64-bit values)
+                                  // transpose-reduce (0: 32 SHFL + 60 FSEL + 45 MOV for 64-bit values); 2, 3: the sum
+                                  // deferred behind the next batch as in the fp32 kernel -- no gain here (pair kernel at
+                                  // 2000 x 128: 59.93 ms with 1, 62.05 with 2 (two call sites of the batch cost an address
+                                  // add per table lookup), 60.12 with 3): the FP64 pipe, not the reduction chain, is what
+                                  // the two warps per scheduler wait for
 #ifndef VN_TGT64_LASTOUT
 #define VN_TGT64_LASTOUT 1         // free-target kernel: the last warp out of a ring stage refills it (stage_last_out);
 #endif                             // measured 719 against 696 GInt/s at 2000 x 128 sources, 512 x 512 targets
@@ -247,7 +251,36 @@ farfield_f64_kernel(const double4 *__restrict__ src, const double2 *__restrict__
                     c[2 * jj + 1] = cy;
                 }
             };
-#if VN_F64_SMEMRED == 2
+#if VN_F64_SMEMRED == 3
+            // as mode 2, with ONE call site of the batch arithmetic (the first trip has nothing parked yet)
+            static_assert(kDup == 2, "shared-memory reduction assumes 16 values per batch");
+            double *rw = red[tid >> 5];
+            const int col = lane + (lane >= 16 ? kRedHalf - 16 : 0);
+            const double2 *row = reinterpret_cast<const double2 *>(rw + (lane >> 1) * kRedRow + (lane & 1) * kRedHalf);
+#pragma unroll 1
+            for (int jb = 0; jb <= kTile; jb += B) {
+                __syncwarp();                                       // the parked rows are complete
+                double2 q[8];
+                if (jb > 0) {
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) q[e] = row[e];
+                }
+                double c[2 * B];
+                if (jb < kTile) batch(jb, c);
+                if (jb > 0) {
+                    double t = (((q[0].x + q[0].y) + (q[1].x + q[1].y)) + ((q[2].x + q[2].y) + (q[3].x + q[3].y))) +
+                               (((q[4].x + q[4].y) + (q[5].x + q[5].y)) + ((q[6].x + q[6].y) + (q[7].x + q[7].y)));
+                    t += __shfl_xor_sync(0xffffffffu, t, 1);
+                    if ((lane % kDup) < 2)
+                        atomicAdd((unsigned long long *)(accj + 4 * (jb - B)), (unsigned long long)fixed2_word(t, fx, lane % kDup));
+                }
+                if (jb < kTile) {
+                    __syncwarp();                                   // every lane has read the previous batch's rows
+#pragma unroll
+                    for (int v = 0; v < 2 * B; ++v) rw[v * kRedRow + col] = c[v];
+                }
+            }
+#elif VN_F64_SMEMRED == 2
             // The c values of a batch are parked in the transposed shared-memory buffer and summed over the warp while
             // the NEXT batch is computed (loads issued before that batch's arithmetic, nothing of it depends on them).
             static_assert(kDup == 2, "shared-memory reduction assumes 16 values per batch");
