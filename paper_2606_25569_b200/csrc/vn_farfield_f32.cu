@@ -48,6 +48,10 @@ constexpr int kBatch = VN_F32_BATCH;              // sources per cross-lane redu
 #define VN_F32_RED_UNROLL 1                       // batches per scheduling region of the deferred-reduction loop: 3, 5, 15 measured
 #endif                                            // -10 %, -27 %, -36 % at 2000 x 128 (13 KB of SASS per batch: instruction cache)
 constexpr int kRedUnroll = VN_F32_RED_UNROLL;
+#ifndef VN_F32_DIAG_NOMUFU
+#define VN_F32_DIAG_NOMUFU 0                      // DIAGNOSTIC builds only (wrong results): bit 0 drops the SFU operations of the
+#endif                                            // fast loop, bit 1 its j <- i reduction; measured at 8000 x 128: 3240 / 3133 /
+                                                  // 3327 GInt/s for 1 / 2 / 3 against 3079
 #ifndef VN_F32_PREFETCH
 #define VN_F32_PREFETCH 0                         // 1 (mode 2 only): the first source record of a batch is loaded a batch ahead;
                                                   // measured 3043 against 3079 GInt/s at 8000 x 128: off
@@ -254,9 +258,17 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
 #else
                         float ka, kb;
                         upk(mul2(r2, KA), ka, kb);
+#if VN_F32_DIAG_NOMUFU & 1   // diagnostic build only (wrong results): how fast is the loop without its SFU operations?
+                        inv[p] = pk(ka, kb);
+#else
                         inv[p] = pk(sfu_rcp(ka), sfu_rcp(kb));                       // 1/(KA r2)
 #endif
+#endif
+#if VN_F32_DIAG_NOMUFU & 1
+                        l[p] = r2;
+#else
                         l[p] = pk(sfu_lg2(a), sfu_lg2(b));
+#endif
                     }
                     u64 cUx = 0ull, cUy = 0ull;
 #pragma unroll
@@ -378,10 +390,16 @@ farfield_f32_kernel(const ulonglong2 *__restrict__ src, const float2 *__restrict
                     pre_g = ts[2 * jn + 1];
                 }
 #endif
+#if VN_F32_DIAG_NOMUFU & 2       // diagnostic build only (wrong results): the loop without the j <- i reduction
+#pragma unroll
+                for (int v = 0; v < 2 * kBatch; ++v) Ux[v % NP] = add2(Ux[v % NP], cp[v]);
+                (void)q0; (void)q1; (void)q2; (void)q3; (void)c;
+#else
                 fold(cp, c);
                 const float t = total(q0, q1, q2, q3);
                 if (lane % kDup == 0) red_fixed(accj + 2 * (jb - kBatch), t * -0.34657359027997264f, scale);
                 park(c);
+#endif
             }
             {
                 __syncwarp();
