@@ -3,7 +3,7 @@ one process per GPU.
 
 The pair kernel evaluates every unordered pair of points once and scatters into BOTH points' accumulators, so the
 work cannot be cut by targets without giving up the symmetry (a target-sharded split evaluates every cross-shard
-pair twice: 10.75 instead of 9.0 FP32 lane-instructions per interaction at N = 8).  It is cut by BLOCKS of the
+pair twice: 12.5 instead of 9.0 FP32 lane-instructions per interaction at N = 8).  It is cut by BLOCKS of the
 pair walk instead:
 
     1. every rank owns a contiguous range of vesicles (its shard of X, F, W and of the result U);
@@ -16,12 +16,13 @@ pair walk instead:
 
 Integer addition is associative, so the result is bit for bit the single-GPU result whatever N is, and the 2x saving
 of the symmetric evaluation is kept.  At 8,000 x 128 (fp32): 20 MB gathered + 16 MB reduce-scattered per rank against
-357 ms / N of arithmetic -- tens of microseconds on NVLink 5 / NVSwitch; the collectives are NCCL's (there is nothing
+340 ms / N of arithmetic -- tens of microseconds on NVLink 5 / NVSwitch; the collectives are NCCL's (there is nothing
 to overlap them with: step 2 must finish before, step 4 can only start after, the kernel).
 
 `sharded_farfield` is written against two callables (the accumulate and the finish step) so that the CPU tests can
 drive the same partition / gather / reduce logic with the oracle as the evaluator (tests/test_multi_gloo.py);
-`sharded_farfield_gpu` binds it to the library.  Backend-agnostic: NCCL on GPUs, gloo in the CPU tests.
+`sharded_farfield_gpu` binds it to the library.  Backend-agnostic: NCCL on GPUs, gloo in the tests (CPU tensors, or
+CUDA tensors staged through host memory: tests/test_multi_gpu.py runs several ranks' real kernels on one GPU).
 """
 from __future__ import annotations
 
@@ -76,6 +77,11 @@ def shard_range(nves: int, world: int, rank: int):
     return min(rank * s, nves), min((rank + 1) * s, nves)
 
 
+def _staged(d, t):
+    """gloo moves host memory only: a CUDA tensor goes through a host copy there (tests); NCCL takes it as it is."""
+    return d.get_backend() == "gloo" and t.is_cuda
+
+
 def all_gather_shards(local, nves: int, world: int):
     """local: this rank's shard [n_local, ...] -> the whole array [nves, ...] on every rank.  Shards are padded to
     the common size ceil(nves / world) for the collective and the padding is cut off again."""
@@ -87,6 +93,10 @@ def all_gather_shards(local, nves: int, world: int):
     if local.shape[0] != s:
         pad = torch.zeros((s - local.shape[0],) + tuple(local.shape[1:]), dtype=local.dtype, device=local.device)
         local = torch.cat([local, pad], 0)
+    if _staged(d, local):
+        host = torch.empty((world * s,) + tuple(local.shape[1:]), dtype=local.dtype)
+        d.all_gather_into_tensor(host, local.contiguous().cpu())
+        return host[:nves].to(local.device)
     full = torch.empty((world * s,) + tuple(local.shape[1:]), dtype=local.dtype, device=local.device)
     d.all_gather_into_tensor(full, local.contiguous())
     return full[:nves]
@@ -95,7 +105,7 @@ def all_gather_shards(local, nves: int, world: int):
 def reduce_scatter_sum(full, nves: int, per_vesicle: int, world: int, rank: int):
     """full: integer accumulators of ALL vesicles [nves * per_vesicle] computed by this rank -> the sum over ranks of
     this rank's own vesicles [n_local * per_vesicle].  One reduce-scatter where the backend has it (NCCL); gloo has
-    none, there it is an all-reduce followed by the slice (CPU tests only)."""
+    none, there it is an all-reduce followed by the slice (tests only)."""
     import torch
     d = _dist()
     b, e = shard_range(nves, world, rank)
@@ -103,6 +113,10 @@ def reduce_scatter_sum(full, nves: int, per_vesicle: int, world: int, rank: int)
         return full[b * per_vesicle:e * per_vesicle]
     s = shard_size(nves, world)
     if d.get_backend() == "gloo":
+        if full.is_cuda:
+            host = full.cpu()
+            d.all_reduce(host, op=d.ReduceOp.SUM)
+            return host[b * per_vesicle:e * per_vesicle].to(full.device)
         d.all_reduce(full, op=d.ReduceOp.SUM)
         return full[b * per_vesicle:e * per_vesicle]
     if world * s != nves:
