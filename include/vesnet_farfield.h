@@ -66,7 +66,8 @@ typedef enum {
     VN_OK = 0,
     VN_ERR_INVALID_ARG = 1,
     VN_ERR_UNSUPPORTED = 2,
-    VN_ERR_CUDA = 3
+    VN_ERR_CUDA = 3,
+    VN_ERR_TOO_LARGE = 4    /* vn_farfield_noalloc_f32 only: more points than the static scratch holds */
 } vn_status;
 
 typedef enum { VN_F32 = 0, VN_F64 = 1 } vn_precision;
@@ -266,6 +267,26 @@ vn_status vn_selfcheck(const void *X, const void *F, const void *W, int64_t nves
  * Synchronous; not capturable into a graph.  bench.py calls it once per run for roofline.peak_measured. */
 vn_status vn_pipe_peaks(double *rates /* HOST, 8 entries */, void *stream);
 
+/* vn_farfield without any allocation, single precision (the same sum, the same kernels).
+ * For callers that cannot call cudaMalloc: code under CUDA graph / stream capture, tight serving loops, harnesses
+ * that forbid it.  vn_farfield takes 48 bytes of scratch per point from the stream-ordered allocator for every call
+ * above 1,024 points; this entry point keeps that scratch in a static device array of the library instead and calls
+ * no cudaMalloc*, cudaFree* or allocating library routine (with vn_profile_enable off).  The price is a LIMIT and a
+ * standing cost: at most vn_noalloc_max_points() = 262,144 points (nves*npts; BASELINE.json configs[0..3]), and the
+ * array -- 12 MiB + 256 B -- is held by every GPU that loads the library until the process exits.
+ * X, F [nves,npts,2], W [nves,npts], U [nves,npts,2]: float, DEVICE pointers, the caller's; U is overwritten and
+ * must not alias an input.  Always the symmetric pair kernel (also below 1,024 points), with the grid vn_farfield
+ * uses: above 1,024 points U equals vn_farfield's bit for bit.  Asynchronous on `stream`.
+ * Returns VN_ERR_TOO_LARGE for nves*npts > vn_noalloc_max_points() (checked before any CUDA call, nothing is
+ * launched), otherwise vn_farfield's codes.  All calls on a device SHARE the array, which keeps the previous call's
+ * contents (the call clears what must start at zero): calls on one stream are ordered and safe; calls whose
+ * kernels overlap on the GPU -- two streams, two graphs replayed concurrently, two host threads on two streams --
+ * race on it and give undefined results.  The first call on a device looks the array's address up
+ * (cudaGetSymbolAddress, device current) and queries the kernel's occupancy: make it outside a capture. */
+vn_status vn_farfield_noalloc_f32(const void *X, const void *F, const void *W, int64_t nves, int64_t npts,
+                                  double mu, void *U, void *stream);
+int64_t vn_noalloc_max_points(void);
+
 /* Host-only introspection (no CUDA call, works without a GPU): the work decomposition vn_farfield would use
  * for nves x npts points when `resident_blocks` blocks of the pair kernel fit on the device at once
  * (148 SMs x 3 on a B200).  plan[0] = points per super-tile (target block), plan[1] = source tiles per
@@ -283,8 +304,8 @@ int64_t vn_launch_count(void);
 /* Static, NUL-terminated description of a status code. */
 const char *vn_status_string(vn_status s);
 
-/* Library version: major*10000 + minor*100 + patch (this header: 0.2.0 = 200). */
-#define VN_VERSION 200
+/* Library version: major*10000 + minor*100 + patch (this header: 0.2.1 = 201). */
+#define VN_VERSION 201
 int vn_version(void);
 
 #ifdef __cplusplus

@@ -25,7 +25,7 @@ import ctypes
 import os
 
 VN_F32, VN_F64 = 0, 1
-VN_OK, VN_ERR_INVALID_ARG, VN_ERR_UNSUPPORTED, VN_ERR_CUDA = 0, 1, 2, 3
+VN_OK, VN_ERR_INVALID_ARG, VN_ERR_UNSUPPORTED, VN_ERR_CUDA, VN_ERR_TOO_LARGE = 0, 1, 2, 3, 4
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libvesnet_farfield.so")
@@ -86,6 +86,10 @@ def lib():
         L.vn_selfcheck.restype = ci
         L.vn_pipe_peaks.argtypes = [ctypes.POINTER(dbl), vp]
         L.vn_pipe_peaks.restype = ci
+        L.vn_farfield_noalloc_f32.argtypes = [vp, vp, vp, i64, i64, dbl, vp, vp]
+        L.vn_farfield_noalloc_f32.restype = ci
+        L.vn_noalloc_max_points.argtypes = []
+        L.vn_noalloc_max_points.restype = i64
         L.vn_version.argtypes = []
         L.vn_version.restype = ci
         _lib = L
@@ -135,6 +139,31 @@ def vn_farfield(X, F, W, mu: float = 1.0, out=None, stream=None):
                                out.data_ptr(), _prec(X), _stream_ptr(stream))
     if rc != VN_OK:
         raise VesnetError(rc, "vn_farfield")
+    return out
+
+
+def vn_noalloc_max_points() -> int:
+    """Most points (nves * npts) vn_farfield_noalloc_f32 takes: the capacity of the library's static scratch."""
+    return int(lib().vn_noalloc_max_points())
+
+
+def vn_farfield_noalloc_f32(X, F, W, out, mu: float = 1.0, stream=None):
+    """vn_farfield in single precision without any allocation (static scratch inside the library; see the header for
+    the limit and the sharing rule).  `out` [nves, npts, 2] float32 is the caller's and required: the binding
+    allocates nothing either.  Raises VesnetError(VN_ERR_TOO_LARGE) above vn_noalloc_max_points() points."""
+    import torch
+    nves, npts, two = X.shape
+    if two != 2:
+        raise ValueError("X must be [nves, npts, 2]")
+    _check_dev("X", X, None, torch.float32)
+    _check_dev("F", F, X.shape, torch.float32)
+    _check_dev("W", W, (nves, npts), torch.float32)
+    _check_dev("out", out, X.shape, torch.float32)
+    with torch.cuda.device(X.device):
+        rc = lib().vn_farfield_noalloc_f32(X.data_ptr(), F.data_ptr(), W.data_ptr(), nves, npts, float(mu),
+                                           out.data_ptr(), _stream_ptr(stream))
+    if rc != VN_OK:
+        raise VesnetError(rc, "vn_farfield_noalloc_f32")
     return out
 
 

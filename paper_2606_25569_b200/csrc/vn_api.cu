@@ -61,6 +61,9 @@ vn_status farfield_partial_f64(const void *X, const void *F, const void *W, int6
                                int nparts, void *acc, void *gmax, cudaStream_t st);
 vn_status farfield_finish_f32(const void *acc, const void *gmax, int64_t P_total, int64_t count, double mu, void *U,
                               cudaStream_t st);
+vn_status farfield_static_f32(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, double mu,
+                              void *U, cudaStream_t st);
+int64_t farfield_static_max_points();
 vn_status farfield_finish_f64(const void *acc, const void *gmax, int64_t P_total, int64_t count, double mu, void *U,
                               cudaStream_t st);
 
@@ -180,6 +183,25 @@ vn_status vn_farfield(const void *X, const void *F, const void *W, int64_t nves,
     if (ds != VN_OK) return ds;
     return farfield_dispatch(X, F, W, nves, npts, mu, U, precision, (cudaStream_t)stream);
 }
+
+// no allocation: static scratch (vn_farfield_f32.cu), fp32, at most vn_noalloc_max_points() points
+vn_status vn_farfield_noalloc_f32(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, double mu,
+                                  void *U, void *stream)
+{
+    if (!X || !F || !W || !U) return VN_ERR_INVALID_ARG;
+    if (check_shape(nves, npts, VN_F32) != VN_OK) return VN_ERR_INVALID_ARG;
+    if (!isfinite(mu) || !(mu > 0.0)) return VN_ERR_INVALID_ARG;
+    if (misaligned(X, 8) || misaligned(F, 8) || misaligned(U, 8) || misaligned(W, 4)) return VN_ERR_INVALID_ARG;
+    if (U == X || U == F || U == W) return VN_ERR_INVALID_ARG;
+    if (nves * npts > farfield_static_max_points()) return VN_ERR_TOO_LARGE;
+    int dev = 0, major = 0;                  // the device check of the other entry points without their pool set-up
+    VN_CUDA(cudaGetDevice(&dev));
+    VN_CUDA(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+    if (major != 10) return VN_ERR_UNSUPPORTED;
+    return farfield_static_f32(X, F, W, nves, npts, mu, U, (cudaStream_t)stream);
+}
+
+int64_t vn_noalloc_max_points(void) { return farfield_static_max_points(); }
 
 vn_status vn_near_pairs(const void *X, const void *W, int64_t nves, int64_t npts, int64_t *near_ptr,
                         int32_t *near_ves, int64_t capacity, vn_precision precision, void *stream)
@@ -488,6 +510,8 @@ const char *vn_status_string(vn_status s)
         case VN_ERR_INVALID_ARG: return "invalid argument";
         case VN_ERR_UNSUPPORTED: return "unsupported device (needs compute capability 10.x, sm_100a build)";
         case VN_ERR_CUDA: return "CUDA runtime error";
+        case VN_ERR_TOO_LARGE:
+            return "too many points for the static scratch of vn_farfield_noalloc_f32 (at most 262,144 = vn_noalloc_max_points(); use vn_farfield)";
     }
     return "unknown status";
 }

@@ -21,6 +21,8 @@
 //
 // Cross-block accumulation goes through 64-bit fixed-point atomics (integer addition is associative, so
 // the result is bitwise reproducible whatever the block order); see fixed_scale().
+#include <mutex>
+
 #include "vn_common.cuh"
 
 namespace vn {
@@ -699,6 +701,70 @@ vn_status farfield_finish_f32(const void *acc, const void *gmax, int64_t P_total
     finish_f32<<<(int)((count + 255) / 256), 256, 0, st>>>((const long long *)acc, (int)count, (int)P_total,
                                                            (const unsigned *)gmax,
                                                            1.0 / (4.0 * 3.14159265358979323846 * mu), (float2 *)U);
+    count_launch(1);
+    return cudaGetLastError() == cudaSuccess ? VN_OK : VN_ERR_CUDA;
+}
+
+// ------------------------------------------------------------------------------------------------
+// vn_farfield_noalloc_f32: the general fp32 path (pack, symmetric pair kernel, finish -- the same kernels, the same
+// grid, hence bit for bit the same U as farfield_f32) for callers that may not allocate: code under stream capture,
+// tight serving loops, harnesses that forbid cudaMalloc.  farfield_f32 takes 48 bytes of scratch per point from the
+// stream-ordered allocator; here the scratch is the static device array below, 12 MiB + 256 B that EVERY device
+// which loads the library holds until the process exits -- which is why the limit is modest: kStaticMaxPoints =
+// 262,144 points (BASELINE.json configs[0..3]; configs[4], 1.02 M points, needs 47 MiB and stays with vn_farfield).
+//   layout:  [0, 32 maxP)  packed sources (ulonglong2 pairs, written by pack_sources_f32 before anything reads them)
+//            [32 maxP, 32 maxP + 16 P)  fixed-point accumulators, then 16 bytes holding gmax: cleared by every call
+// All calls on a device share the array and it keeps the last call's contents; two calls whose kernels overlap on the
+// GPU (different streams, or graphs replayed concurrently) race on it.  Calls on one stream are ordered and safe.
+// In host code the array's name is a host-side stand-in, not a device address: the address is asked for once per
+// device, with that device current, by cudaGetSymbolAddress, and only that pointer is handed to the kernels.
+constexpr int kStaticMaxPoints = 1 << 18;
+constexpr size_t kStaticSrcBytes = (size_t)kStaticMaxPoints * 32;
+constexpr size_t kStaticAccBytes = (size_t)kStaticMaxPoints * 16;
+constexpr size_t kStaticScratchBytes = kStaticSrcBytes + kStaticAccBytes + 256;
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticScratchBytes];
+
+int64_t farfield_static_max_points() { return kStaticMaxPoints; }
+
+// device address of g_static_scratch on the CURRENT device (cached per device ordinal)
+static vn_status static_scratch_base(unsigned char **base)
+{
+    static std::mutex lock;
+    static unsigned char *base_dev[kMaxDevices] = {nullptr};
+    int dev = -1;
+    VN_CUDA(cudaGetDevice(&dev));
+    const bool cached = dev >= 0 && dev < kMaxDevices;
+    std::lock_guard<std::mutex> guard(lock);
+    if (cached && base_dev[dev]) {
+        *base = base_dev[dev];
+        return VN_OK;
+    }
+    void *p = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&p, g_static_scratch);
+    if (e != cudaSuccess || !p) {
+        (void)cudaGetLastError();
+        return VN_ERR_CUDA;
+    }
+    if (cached) base_dev[dev] = (unsigned char *)p;
+    *base = (unsigned char *)p;
+    return VN_OK;
+}
+
+vn_status farfield_static_f32(const void *X, const void *F, const void *W, int64_t nves, int64_t npts, double mu,
+                              void *U, cudaStream_t st)
+{
+    if (nves * npts > (int64_t)kStaticMaxPoints) return VN_ERR_TOO_LARGE;
+    const int P = (int)(nves * npts);
+    unsigned char *base = nullptr;
+    const vn_status rb = static_scratch_base(&base);
+    if (rb != VN_OK) return rb;
+    ulonglong2 *src = (ulonglong2 *)base;
+    long long *acc = (long long *)(base + kStaticSrcBytes);
+    unsigned *gmax = (unsigned *)(base + kStaticSrcBytes + (size_t)P * 16);
+    VN_CUDA(cudaMemsetAsync(acc, 0, (size_t)P * 16 + 16, st));      // what must start at zero: accumulators, gmax
+    const vn_status rc = accumulate_f32(X, F, W, P, (int)npts, 0, 1, src, acc, gmax, st);
+    if (rc != VN_OK) return rc;
+    finish_f32<<<(P + 255) / 256, 256, 0, st>>>(acc, P, P, gmax, 1.0 / (4.0 * 3.14159265358979323846 * mu), (float2 *)U);
     count_launch(1);
     return cudaGetLastError() == cudaSuccess ? VN_OK : VN_ERR_CUDA;
 }

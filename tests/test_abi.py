@@ -27,8 +27,8 @@ def test_library_exports_every_declared_symbol():
         assert hasattr(L, n), n
     # the header's encoding, major*10000 + minor*100 + patch, and the header's own constant
     header = open(os.path.join(ROOT, "include", "vesnet_farfield.h")).read()
-    assert vn.vn_version() == int(re.search(r"#define\s+VN_VERSION\s+(\d+)", header).group(1)) == 200
-    assert "vn_pipe_peaks" in names
+    assert vn.vn_version() == int(re.search(r"#define\s+VN_VERSION\s+(\d+)", header).group(1)) == 201
+    assert "vn_pipe_peaks" in names and "vn_farfield_noalloc_f32" in names and "vn_noalloc_max_points" in names
     assert L.vn_status_string(0) == b"ok" and b"invalid" in L.vn_status_string(1)
 
 
@@ -48,6 +48,15 @@ def test_argument_validation_needs_no_gpu():
     assert L.vn_farfield(p + 4, p, p, 2, 4, 1.0, q, vn.VN_F32, None) == INV         # misaligned pair
     assert L.vn_farfield(p, p, p, 2, 4, 1.0, p, vn.VN_F64, None) == INV             # U aliases X
     assert L.vn_arclength_weights(None, 2, 4, q, vn.VN_F64, None) == INV
+    # no-allocation entry point: the size limit of its static scratch is checked before any CUDA call
+    cap = L.vn_noalloc_max_points()
+    assert cap == 262144
+    assert L.vn_farfield_noalloc_f32(p, p, p, cap // 128 + 1, 128, 1.0, q, None) == vn.VN_ERR_TOO_LARGE
+    assert L.vn_farfield_noalloc_f32(p, p, p, 1, cap + 1, 1.0, q, None) == vn.VN_ERR_TOO_LARGE
+    assert L.vn_farfield_noalloc_f32(None, p, p, 2, 4, 1.0, q, None) == INV
+    assert L.vn_farfield_noalloc_f32(p, p, p, 2, 4, -1.0, q, None) == INV
+    assert L.vn_farfield_noalloc_f32(p, p, p, 2, 4, 1.0, p, None) == INV              # U aliases X
+    assert b"static scratch" in L.vn_status_string(vn.VN_ERR_TOO_LARGE)
     assert L.vn_arclength_weights(p, 2, -1, q, vn.VN_F64, None) == INV
     # NEXT rows
     assert L.vn_near_pairs(p, None, 2, 4, q, None, 0, vn.VN_F64, None) == INV          # null W
