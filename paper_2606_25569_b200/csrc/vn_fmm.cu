@@ -468,6 +468,141 @@ fmm_m2l(int level, int q, const double *__restrict__ tab, const unsigned long lo
     }   // boxes
 }
 
+// M2L for q <= 16 (orders up to 15: the defaults, 12 in double and 14 in single precision, live here).  fmm_m2l gives
+// a lane the coefficients l and l + 32: with q = 15 half of its DFMAs multiply padding and 17 of 32 lanes carry
+// none.  Here a HALF-warp owns a source box -- lane = (half, l), two sources of the interaction list in flight per warp --
+// and three more things change: the list (up to 27 non-empty boxes of the 6 x 6 parent-neighbour region) is built by the
+// lanes in parallel (one round of boxcnt loads instead of 27 dependent ones), the next pair's moments are fetched into
+// registers before the current pair's matrix-vector loop (the L2 latency of a source box hides behind the previous
+// one's arithmetic), and the two halves' sums meet in one shuffle at the end.  Same formulas as fmm_m2l; the order in
+// which the sources are added differs (fixed, so the result is still reproducible run to run).
+constexpr int kM2LHalfQ = 16;
+__global__ void __launch_bounds__(32 * kM2LWarps)
+fmm_m2l_half(int level, int q, const double *__restrict__ tab, const unsigned long long *__restrict__ enc,
+             const cplx *__restrict__ mult, const int *__restrict__ boxcnt, const int *__restrict__ tboxcnt,
+             cplx *__restrict__ loc)
+{
+    if (level > load_level(enc)) return;
+    extern __shared__ __align__(16) double sm[];
+    double *Cb = sm;                                                  // [q][q]
+    const int warp = threadIdx.x >> 5, ln = threadIdx.x & 31, half = ln >> 4, l = ln & 15;
+    const int hstride = 3 * (q + 1) + 1;                              // odd number of 16-byte words: the halves' broadcasts fall in different banks
+    cplx *hat = (cplx *)(sm + ((q * q + 1) & ~1)) + (warp * 2 + half) * hstride;   // [3][q+1] per half; hat[a][q] = 0 pads the shifted read
+    int *list = (int *)((cplx *)(sm + ((q * q + 1) & ~1)) + kM2LWarps * 2 * hstride) + warp * 32;
+    const FmmTables t = fmm_tables_at(const_cast<double *>(tab), q);
+    for (int e = threadIdx.x; e < q * q; e += blockDim.x) Cb[e] = t.Cb[e];
+    if (l < 3) hat[l * (q + 1) + q] = make_double2(0.0, 0.0);
+    __syncthreads();
+    const int n = 1 << level;
+    const Geom gm = load_geom(enc);
+    const double s = gm.size / (double)n, log_s = log(s), inv_s = 1.0 / s;
+    const bool v = l < q;
+    const double sgn = (l & 1) ? -1.0 : 1.0, il = l > 0 ? 1.0 / (double)l : 0.0;
+    const long long lev0 = level_offset(level);
+    const cplx *Mlev = mult + lev0 * (long long)(3 * q);
+    for (int box = blockIdx.x * kM2LWarps + warp; box < n * n; box += gridDim.x * kM2LWarps) {
+        if (tboxcnt && tboxcnt[lev0 + box] == 0) continue;
+        const int ix = box / n, iy = box % n, px = ix >> 1, py = iy >> 1;
+        // interaction list: children of the parent's neighbours that are not neighbours of the box and hold sources
+        __syncwarp();
+        int nlist = 0;
+#pragma unroll
+        for (int r = 0; r < 2; ++r) {
+            const int e = ln + 32 * r;
+            bool ok = false;
+            int entry = 0;
+            if (e < 36) {
+                const int sx = 2 * (px - 1) + e / 6, sy = 2 * (py - 1) + e % 6;
+                if (sx >= 0 && sx < n && sy >= 0 && sy < n && !(abs(sx - ix) <= 1 && abs(sy - iy) <= 1)) {
+                    const int src = sx * n + sy;
+                    ok = boxcnt[lev0 + src] != 0;
+                    entry = src | (((ix - sx + 3) * 7 + (iy - sy + 3)) << 24);
+                }
+            }
+            const unsigned m = __ballot_sync(0xffffffffu, ok);
+            if (ok) list[nlist + __popc(m & ((1u << ln) - 1u))] = entry;
+            nlist += __popc(m);
+        }
+        __syncwarp();
+        cplx acc0 = make_double2(0.0, 0.0), acc1 = acc0, acc2 = acc0;
+        // moments of the half's next source (coefficient l of the three expansions) and its offset
+        cplx a0, a1, a2;
+        int o;
+        auto fetch = [&](int idx) {
+            a0 = a1 = a2 = make_double2(0.0, 0.0);
+            o = 24;                                                    // tau = 0: rho = lrho = 0, an absent source adds nothing
+            if (idx < nlist) {
+                const int entry = list[idx];
+                o = entry >> 24;
+                if (v) {
+                    const cplx *A = Mlev + (long long)(entry & 0xffffff) * (3 * q);
+                    a0 = A[l];
+                    a1 = A[q + l];
+                    a2 = A[2 * q + l];
+                }
+            }
+        };
+        fetch(half);
+        for (int i = 0; i < nlist; i += 2) {
+            const cplx *rho = t.rho + (size_t)o * (q + 1);
+            const int o_now = o;
+            __syncwarp();                                             // the previous pair's hat is consumed
+            if (v) {
+                const cplx r = __ldg(&rho[l]);
+                cplx h0 = cmul(a0, r), h1 = cmul(a1, r);
+                if (l >= 1) { h0 = cscale(h0, il); h1 = cscale(h1, il); }
+                hat[l] = h0;
+                hat[(q + 1) + l] = h1;
+                hat[2 * (q + 1) + l] = cmul(a2, r);
+            }
+            fetch(i + 2 + half);                                      // in flight during the loop below
+            __syncwarp();
+            const cplx A10 = hat[0], A20 = hat[q + 1];                // rho^0 = 1: the raw zeroth moments
+            cplx S0 = make_double2(0.0, 0.0), S1 = S0, S2 = S0;
+            const cplx *h0p = hat + 1, *h1p = hat + (q + 1) + 1, *h2p = hat + 2 * (q + 1);   // log arrays read k + 1
+            const double *Cl = Cb + (v ? l : 0);
+#pragma unroll 5
+            for (int k = 0; k < q; ++k) {
+                const double c0 = Cl[k * q];
+                const cplx e0 = h0p[k], e1 = h1p[k], e2 = h2p[k];     // Ahat1_{k+1}, Ahat2_{k+1}, Bhat_k
+                S0.x = fma(c0, e0.x, S0.x); S0.y = fma(c0, e0.y, S0.y);
+                S1.x = fma(c0, e1.x, S1.x); S1.y = fma(c0, e1.y, S1.y);
+                S2.x = fma(c0, e2.x, S2.x); S2.y = fma(c0, e2.y, S2.y);
+            }
+            if (v) {
+                if (l == 0) {
+                    const cplx lr = t.lrho[o_now];
+                    acc0 = cadd(acc0, make_double2(A10.x * (log_s - lr.x) + A10.y * lr.y - S0.x,
+                                                   -A10.x * lr.y + A10.y * (log_s - lr.x) - S0.y));
+                    acc1 = cadd(acc1, make_double2(A20.x * (log_s - lr.x) + A20.y * lr.y - S1.x,
+                                                   -A20.x * lr.y + A20.y * (log_s - lr.x) - S1.y));
+                    acc2 = cadd(acc2, make_double2(-(A10.x - A20.y), A10.y + A20.x));       // -conj(A1_0 + i A2_0)
+                } else {
+                    const cplx rl = cscale(__ldg(&rho[l]), -sgn);
+                    acc0 = cfma(rl, cadd(cscale(A10, il), S0), acc0);
+                    acc1 = cfma(rl, cadd(cscale(A20, il), S1), acc1);
+                }
+                acc2 = cfma(cscale(__ldg(&rho[l + 1]), sgn * inv_s), S2, acc2);
+            }
+        }
+        // the two halves' sums
+        acc0.x += __shfl_xor_sync(0xffffffffu, acc0.x, 16); acc0.y += __shfl_xor_sync(0xffffffffu, acc0.y, 16);
+        acc1.x += __shfl_xor_sync(0xffffffffu, acc1.x, 16); acc1.y += __shfl_xor_sync(0xffffffffu, acc1.y, 16);
+        acc2.x += __shfl_xor_sync(0xffffffffu, acc2.x, 16); acc2.y += __shfl_xor_sync(0xffffffffu, acc2.y, 16);
+        if (v && half == 0) {
+            cplx *out = loc + (lev0 + box) * (long long)(3 * q);
+            out[l] = acc0;
+            out[q + l] = acc1;
+            out[2 * q + l] = acc2;
+        }
+    }   // boxes
+}
+static size_t m2l_half_smem(int q)
+{
+    return sizeof(double) * (size_t)((q * q + 1) & ~1) + sizeof(cplx) * (size_t)(kM2LWarps * 2 * (3 * (q + 1) + 1)) +
+           sizeof(int) * (size_t)(kM2LWarps * 32);
+}
+
 // L2L: child local expansions inherit the parent's.  One thread per (child box, k); child level = `level`.
 __global__ void __launch_bounds__(128)
 fmm_l2l(int level, int q, const double *__restrict__ tab, const unsigned long long *__restrict__ enc,
@@ -767,7 +902,10 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
     const size_t smem_m2l = sizeof(double) * (size_t)(((q * q + 1) & ~1) + 2 * kM2LWarps * 3 * (q + 1));
     for (int l = 2; l <= L; ++l) {
         const unsigned nb = ((1u << (2 * l)) + kM2LWarps - 1) / kM2LWarps;
-        fmm_m2l<<<nb < 148u * 16u ? nb : 148u * 16u, 32 * kM2LWarps, smem_m2l, st>>>(l, q, tab, enc, mult, boxcnt, boxcnt, loc);
+        if (q <= kM2LHalfQ)
+            fmm_m2l_half<<<nb < 148u * 16u ? nb : 148u * 16u, 32 * kM2LWarps, m2l_half_smem(q), st>>>(l, q, tab, enc, mult, boxcnt, boxcnt, loc);
+        else
+            fmm_m2l<<<nb < 148u * 16u ? nb : 148u * 16u, 32 * kM2LWarps, smem_m2l, st>>>(l, q, tab, enc, mult, boxcnt, boxcnt, loc);
         ++launches;
     }
     for (int l = 3; l <= L; ++l) {
@@ -920,7 +1058,10 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
     const size_t smem_m2l = sizeof(double) * (size_t)(((q * q + 1) & ~1) + 2 * kM2LWarps * 3 * (q + 1));
     for (int l = 2; l <= L; ++l) {
         const unsigned nb = ((1u << (2 * l)) + kM2LWarps - 1) / kM2LWarps;
-        fmm_m2l<<<nb < 148u * 16u ? nb : 148u * 16u, 32 * kM2LWarps, smem_m2l, st>>>(l, q, tab, enc, mult, boxcnt, nullptr, loc);
+        if (q <= kM2LHalfQ)
+            fmm_m2l_half<<<nb < 148u * 16u ? nb : 148u * 16u, 32 * kM2LWarps, m2l_half_smem(q), st>>>(l, q, tab, enc, mult, boxcnt, nullptr, loc);
+        else
+            fmm_m2l<<<nb < 148u * 16u ? nb : 148u * 16u, 32 * kM2LWarps, smem_m2l, st>>>(l, q, tab, enc, mult, boxcnt, nullptr, loc);
         ++launches;
     }
     for (int l = 3; l <= L; ++l) {
