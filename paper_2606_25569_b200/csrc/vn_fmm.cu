@@ -800,6 +800,167 @@ fmm_l2p_p2p(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const int 
     }   // leaves
 }
 
+// L2P + P2P for single-precision storage, the version the fp32 calls run (fmm_l2p_p2p<true> above is its plain
+// predecessor, kept as the readable statement of the same sum).  What changes is the shape of the work, not the sum:
+//  * a thread owns TWO targets as the halves of packed fp32 pairs (FADD2 / FMUL2 / FFMA2, the arithmetic of the exact
+//    fp32 kernels): per source and target pair 11 packed instructions + 4 MUFU instead of 2 x 14 scalar ones;
+//  * the own-vesicle exclusion costs no branch: the two SFU results of an excluded pair are replaced by zeros (a
+//    select each), which removes both of its terms -- also for the self pair, whose lg2 / rcp are infinite;
+//  * the leaf's n targets are dealt out evenly: rounds of at most 128 targets, ceil(n_r / 2) slots of two targets,
+//    floor(128 / slots) threads per slot each taking every split-th source (n = 62: 31 slots x 4 threads; n = 100:
+//    50 x 2), the partial sums meeting in a fixed order through shared memory -- no power-of-two quantisation;
+//  * the three columns of the 3 x 3 neighbourhood are three contiguous index ranges (leaves are stored column by
+//    column): they are staged as ONE list in chunks of 512 sources, two barriers per chunk instead of two per box;
+//  * the far field (Horner of the three local expansions, double) is evaluated by one thread per target, all
+//    threads busy, instead of by every fourth thread.
+// Per-chunk float partial sums are folded into double accumulators as before.
+constexpr int kP2PChunk = 512;
+__global__ void __launch_bounds__(128)
+fmm_l2p_p2p_packed(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const int *__restrict__ vs,
+                   const long long *__restrict__ start, const cplx *__restrict__ tz, const int *__restrict__ tvs,
+                   const int *__restrict__ tperm, const long long *__restrict__ tstart, int q,
+                   const unsigned long long *__restrict__ enc, const cplx *__restrict__ loc, cplx *__restrict__ accum)
+{
+    constexpr int kT = 128;
+    __shared__ cplx lc[3 * kFmmMaxQ];
+    __shared__ float4 sxy[kP2PChunk];                  // (x, x, y, y): both halves of a packed operand
+    __shared__ float4 sgg[kP2PChunk];                  // (gx, gx, gy, gy)
+    __shared__ int sves[kP2PChunk];
+    __shared__ cplx far[kT];
+    __shared__ double4 red[kT];
+    const int L = load_level(enc);
+    const int n = 1 << L;
+    const int tid = threadIdx.x;
+    const Geom gm = load_geom(enc);
+    const double s = gm.size / (double)n, inv_s = 1.0 / s;
+    for (int c = blockIdx.x; c < n * n; c += gridDim.x) {
+        const long long a = tstart[c], b = tstart[c + 1];
+        if (a == b) continue;
+        const int ix = c / n, iy = c % n;
+        __syncthreads();                               // the previous leaf's lc is consumed
+        for (int e = tid; e < 3 * q; e += kT) lc[e] = loc[(level_offset(L) + c) * (long long)(3 * q) + e];
+        const cplx ctr = box_centre(gm, L, ix, iy);
+        // the neighbourhood's sources: one contiguous index range per column
+        long long cs[3];
+        int clen[3];
+        const int by0 = max(iy - 1, 0), by1 = min(iy + 1, n - 1);
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const int bx = ix - 1 + k;
+            cs[k] = 0;
+            clen[k] = 0;
+            if (bx >= 0 && bx < n) {
+                cs[k] = start[bx * n + by0];
+                clen[k] = (int)(start[bx * n + by1 + 1] - cs[k]);
+            }
+        }
+        const int total = clen[0] + clen[1] + clen[2];
+        const int nt = (int)(b - a);
+        const int rounds = (nt + kT - 1) / kT, per_round = (nt + rounds - 1) / rounds;
+        for (int r = 0; r < rounds; ++r) {
+            const long long t0 = a + (long long)r * per_round;
+            const int cnt_t = (int)min((long long)per_round, b - t0);
+            const int slots = (cnt_t + 1) >> 1;
+            const int split = kT / slots;
+            const int slot = tid / split, part = tid - slot * split;
+            const bool active = slot < slots;
+            const bool has_b = active && slot + slots < cnt_t;
+            __syncthreads();                           // lc is loaded; the previous round's far / red are consumed
+            if (tid < cnt_t) {
+                // far field: Horner for value and derivative of the three local expansions
+                const cplx z = tz[t0 + tid];
+                const cplx t = make_double2((z.x - ctr.x) * inv_s, (z.y - ctr.y) * inv_s);
+                cplx p1 = lc[q - 1], p2 = lc[2 * q - 1], p3 = lc[3 * q - 1];
+                cplx d1 = make_double2(0.0, 0.0), d2 = d1;
+                for (int l = q - 2; l >= 0; --l) {
+                    d1 = cfma(d1, t, p1);
+                    d2 = cfma(d2, t, p2);
+                    p1 = cfma(p1, t, lc[l]);
+                    p2 = cfma(p2, t, lc[q + l]);
+                    p3 = cfma(p3, t, lc[2 * q + l]);
+                }
+                // phi = (Phi1' + i Phi2') = (d1 + i d2)/s ;  z conj(phi)
+                const cplx phi = make_double2((d1.x - d2.y) * inv_s, (d1.y + d2.x) * inv_s);
+                const cplx zc = cmul(z, make_double2(phi.x, -phi.y));
+                far[tid] = make_double2(-p1.x + 0.5 * zc.x - 0.5 * p3.x, -p2.x + 0.5 * zc.y + 0.5 * p3.y);
+            }
+            // the slot's two targets (a dead second half repeats the first and is never stored)
+            u64 zx2 = 0, zy2 = 0;
+            int va = -2, vb = -2;
+            if (active) {
+                const cplx za = tz[t0 + slot], zb = tz[t0 + (has_b ? slot + slots : slot)];
+                zx2 = pk((float)za.x, (float)zb.x);
+                zy2 = pk((float)za.y, (float)zb.y);
+                va = tvs ? tvs[t0 + slot] : -1;
+                vb = has_b ? (tvs ? tvs[t0 + slot + slots] : -1) : -2;
+            }
+            double uxa = 0.0, uya = 0.0, uxb = 0.0, uyb = 0.0;
+            for (int f0 = 0; f0 < total; f0 += kP2PChunk) {
+                __syncthreads();
+                const int cnt = min(kP2PChunk, total - f0);
+                for (int e = tid; e < cnt; e += kT) {
+                    int f = f0 + e;
+                    long long idx;
+                    if (f < clen[0]) idx = cs[0] + f;
+                    else if (f < clen[0] + clen[1]) idx = cs[1] + (f - clen[0]);
+                    else idx = cs[2] + (f - clen[0] - clen[1]);
+                    const cplx zz = zs[idx], gg = gs[idx];           // the stored values are floats: converted back exactly
+                    const float x = (float)zz.x, y = (float)zz.y, gx = (float)gg.x, gy = (float)gg.y;
+                    sxy[e] = make_float4(x, x, y, y);
+                    sgg[e] = make_float4(gx, gx, gy, gy);
+                    sves[e] = vs[idx];
+                }
+                __syncthreads();
+                if (active) {
+                    u64 fxl = 0, fyl = 0, fxq = 0, fyq = 0;           // packed (a, b): sum lg2 g  and  sum qd r
+#pragma unroll 2
+                    for (int j = part; j < cnt; j += split) {
+                        const ulonglong2 pxy = *reinterpret_cast<const ulonglong2 *>(&sxy[j]);
+                        const ulonglong2 pgg = *reinterpret_cast<const ulonglong2 *>(&sgg[j]);
+                        const int sv = sves[j];
+                        const u64 rx = sub2(zx2, pxy.x), ry = sub2(zy2, pxy.y);
+                        const u64 r2 = fma2(rx, rx, mul2(ry, ry));
+                        float r2a, r2b;
+                        upk(r2, r2a, r2b);
+                        const float lga = sv != va ? sfu_lg2(r2a) : 0.f, lgb = sv != vb ? sfu_lg2(r2b) : 0.f;
+                        const float iva = sv != va ? sfu_rcp(r2a) : 0.f, ivb = sv != vb ? sfu_rcp(r2b) : 0.f;
+                        const u64 lg = pk(lga, lgb);
+                        const u64 qd = mul2(fma2(rx, pgg.x, mul2(ry, pgg.y)), pk(iva, ivb));
+                        fxl = fma2(lg, pgg.x, fxl);
+                        fyl = fma2(lg, pgg.y, fyl);
+                        fxq = fma2(qd, rx, fxq);
+                        fyq = fma2(qd, ry, fyq);
+                    }
+                    float la, lb, qa, qb;
+                    upk(fxl, la, lb);
+                    upk(fxq, qa, qb);
+                    uxa += (double)fmaf(-0.34657359027997264f, la, qa);     // -ln(r) = -(ln 2 / 2) lg2(r^2)
+                    uxb += (double)fmaf(-0.34657359027997264f, lb, qb);
+                    upk(fyl, la, lb);
+                    upk(fyq, qa, qb);
+                    uya += (double)fmaf(-0.34657359027997264f, la, qa);
+                    uyb += (double)fmaf(-0.34657359027997264f, lb, qb);
+                }
+            }
+            red[tid] = make_double4(uxa, uya, uxb, uyb);
+            __syncthreads();
+            if (active && part == 0) {
+                double4 u = red[tid];
+                for (int p = 1; p < split; ++p) {
+                    const double4 w = red[tid + p];
+                    u.x += w.x; u.y += w.y; u.z += w.z; u.w += w.w;
+                }
+                const cplx fa = far[slot];
+                accum[tperm[t0 + slot]] = make_double2(u.x + fa.x, u.y + fa.y);
+                if (has_b) {
+                    const cplx fb = far[slot + slots];
+                    accum[tperm[t0 + slot + slots]] = make_double2(u.z + fb.x, u.w + fb.y);
+                }
+            }
+        }
+    }   // leaves
+}
+
 // own-vesicle points that sit in NON-neighbour leaf boxes of the target went through the expansions: take their
 // contribution out again (direct, libm log), scale by 1/(4 pi mu) and store.  One thread per point.
 template <typename real2>
@@ -914,7 +1075,7 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
         ++launches;
     }
     if (prec == VN_F32)
-        fmm_l2p_p2p<true><<<p2p_grid, kP2PThreads, 0, st>>>(zs, gs, vs, start, zs, vs, perm, start, q, enc, loc, logtab, accum);
+        fmm_l2p_p2p_packed<<<p2p_grid, 128, 0, st>>>(zs, gs, vs, start, zs, vs, perm, start, q, enc, loc, accum);
     else
         fmm_l2p_p2p<false><<<p2p_grid, kP2PThreads, 0, st>>>(zs, gs, vs, start, zs, vs, perm, start, q, enc, loc, logtab, accum);
     profile_mark(st, false);
@@ -1070,7 +1231,7 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
         ++launches;
     }
     if (prec == VN_F32)
-        fmm_l2p_p2p<true><<<p2p_grid, kP2PThreads, 0, st>>>(zs, gs, vs, start, zts, nullptr, tperm, tstart, q, enc, loc, logtab, accum);
+        fmm_l2p_p2p_packed<<<p2p_grid, 128, 0, st>>>(zs, gs, vs, start, zts, nullptr, tperm, tstart, q, enc, loc, accum);
     else
         fmm_l2p_p2p<false><<<p2p_grid, kP2PThreads, 0, st>>>(zs, gs, vs, start, zts, nullptr, tperm, tstart, q, enc, loc, logtab, accum);
     profile_mark(st, false);
