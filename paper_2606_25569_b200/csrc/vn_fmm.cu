@@ -209,8 +209,9 @@ fmm_gather(const int *__restrict__ perm, int P, int npts, const cplx *__restrict
 // ------------------------------------------------------------------------------------------------
 // translation tables for order p (q = p + 1 coefficients), built once per call on the device:
 //   Cb[n][l]   = C(n + l, l)                                    (real, q x q)          -- M2L
-//   S[c][k][m] = C(k, m) delta_c^(k-m) 2^-m   (m <= k)          (complex, 4 x q x q)   -- M2M, child c -> parent
-//   T[c][m][k] = 2^-m C(k, m) delta_c^(k-m)   (k >= m)          (complex, 4 x q x q)   -- L2L, parent -> child c
+//   S(c; k, m) = C(k, m) delta_c^(k-m) 2^-m   (m <= k, else 0)  (complex, 4 x q x q)   -- M2M, child c -> parent, output k
+//   T(c; k, m) = 2^-k C(m, k) delta_c^(m-k)   (m >= k, else 0)  (complex, 4 x q x q)   -- L2L, parent -> child c, output k
+//   both stored [c][m][k], the OUTPUT index fastest: the lanes of a warp own consecutive k and read consecutive words
 //   rho[t][n]  = tau_t^-n, n = 0 .. q;  lrho[t] = log(1/tau_t)  (complex, 49 offsets tau = dx + i dy, |dx|,|dy| <= 3)
 // delta_c = ((a - 1/2) + i (b - 1/2)) / 2 is the child's centre in the parent's scaled variable, c = 2 a + b.
 struct FmmTables {
@@ -255,8 +256,8 @@ __global__ void fmm_build_tables(int q, double *base)
         cplx s = make_double2(0.0, 0.0), u = make_double2(0.0, 0.0);
         if (m <= k) s = cscale(cpowi(d, k - m), binom(k, m) * exp2(-(double)m));       // S[c][k][m]
         if (k <= m) u = cscale(cpowi(d, m - k), binom(m, k) * exp2(-(double)k));       // T[c][k][m]: row = child index k
-        t.S[e] = s;
-        t.T[e] = u;
+        t.S[((size_t)c * q + m) * q + k] = s;
+        t.T[((size_t)c * q + m) * q + k] = u;
     }
     for (int e = tid; e < 49 * (q + 1); e += nthreads) {
         const int o = e / (q + 1), n = e % (q + 1);
@@ -325,40 +326,72 @@ fmm_p2m(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const long lon
     for (int e = lane; e < 3 * q; e += 32) out[e] = acc[warp][e];
 }
 
-// M2M: parent moments from its four children, levels L-1 down to 2.  One thread per (parent box, k).
-__global__ void __launch_bounds__(128)
+// M2M: parent moments from its four children, levels L-1 down to 2.  One WARP per parent box: the children's
+// moments are staged in the warp's shared memory with coalesced loads (one round trip to L2 instead of one per term),
+// then work item (k, h) -- output coefficient k, child pair h -- sums S(c; k, m) A_c[m] over m and the pair's two
+// children; 2 q items are dealt to the lanes (q = 15: 30 of 32 lanes busy), the table is read with the output
+// index fastest (coalesced, L1-resident), the children's coefficients are shared-memory broadcasts, and the two
+// pairs' partial sums meet through shared memory.
+constexpr int kShiftWarps = 4;
+__global__ void __launch_bounds__(32 * kShiftWarps)
 fmm_m2m(int level, int q, const double *__restrict__ tab, const unsigned long long *__restrict__ enc,
         cplx *__restrict__ mult, int *__restrict__ boxcnt)
 {
     if (level >= load_level(enc)) return;
+    extern __shared__ __align__(16) double sm[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    cplx *ch = (cplx *)sm + warp * (12 * q + 3 * q);               // [4][3][q] children | [3][q] second pair's partial sums
+    cplx *part = ch + 12 * q;
     const FmmTables t = fmm_tables_at(const_cast<double *>(tab), q);
     const int n = 1 << level;
-    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= (long long)n * n * q) return;
-    const int box = (int)(e / q), k = (int)(e % q);
-    const int ix = box / n, iy = box % n;
-    cplx s1 = make_double2(0.0, 0.0), s2 = s1, s3 = s1;
-    int cnt = 0;
-    for (int c = 0; c < 4; ++c) {
-        const long long child = level_offset(level + 1) + (long long)(2 * ix + (c >> 1)) * (2 * n) + (2 * iy + (c & 1));
-        const int cc = boxcnt[child];
-        cnt += cc;
-        if (cc == 0) continue;
-        const cplx *A = mult + child * (long long)(3 * q);
-        const cplx *row = t.S + ((size_t)c * q + k) * q;
-        for (int m = 0; m <= k; ++m) {
-            const cplx sm = row[m];
-            s1 = cfma(sm, A[m], s1);
-            s2 = cfma(sm, A[q + m], s2);
-            s3 = cfma(sm, A[2 * q + m], s3);
+    for (int box = blockIdx.x * kShiftWarps + warp; box < n * n; box += gridDim.x * kShiftWarps) {
+        const int ix = box / n, iy = box % n;
+        const long long child0 = level_offset(level + 1) + (long long)(2 * ix) * (2 * n) + 2 * iy;
+        // children c = 2 a + b sit at child0 + a * 2n + b
+        const int cc = lane < 4 ? boxcnt[child0 + (long long)(lane >> 1) * (2 * n) + (lane & 1)] : 0;
+        const unsigned have = __ballot_sync(0xffffffffu, cc != 0) & 0xfu;
+        int cnt = cc;
+        cnt += __shfl_xor_sync(0xffffffffu, cnt, 1);
+        cnt += __shfl_xor_sync(0xffffffffu, cnt, 2);
+        __syncwarp();                                               // the previous box's staging is consumed
+        for (int e = lane; e < 12 * q; e += 32) {
+            const int c = e / (3 * q);
+            ch[e] = ((have >> c) & 1u) ? mult[(child0 + (long long)(c >> 1) * (2 * n) + (c & 1)) * (long long)(3 * q) + (e - c * 3 * q)]
+                                       : make_double2(0.0, 0.0);
         }
+        __syncwarp();
+        cplx *out = mult + (level_offset(level) + box) * (long long)(3 * q);
+        for (int w0 = 0; w0 < 2 * q; w0 += 32) {
+            const int w = w0 + lane;
+            const bool live = w < 2 * q;
+            const int h = live && w >= q ? 1 : 0, k = live ? w - h * q : 0;
+            cplx s1 = make_double2(0.0, 0.0), s2 = s1, s3 = s1;
+            for (int c = 2 * h; c < 2 * h + 2; ++c) {
+                if (!((have >> c) & 1u)) continue;
+                const cplx *A = ch + c * 3 * q;
+                const cplx *col = t.S + (size_t)c * q * q + k;
+#pragma unroll 4
+                for (int m = 0; m < q; ++m) {                       // entries with m > k are zero
+                    const cplx sm_ = __ldg(&col[(size_t)m * q]);
+                    s1 = cfma(sm_, A[m], s1);
+                    s2 = cfma(sm_, A[q + m], s2);
+                    s3 = cfma(sm_, A[2 * q + m], s3);
+                }
+            }
+            if (live && h == 1) { part[k] = s1; part[q + k] = s2; part[2 * q + k] = s3; }
+            __syncwarp();
+            if (live && h == 0) {
+                // the second pair's item (k, 1) is item q + k: it was computed in this round or is computed in a later one
+                out[k] = s1; out[q + k] = s2; out[2 * q + k] = s3;
+            }
+        }
+        __syncwarp();
+        // add the second pair's partial sums (all items are done)
+        for (int e = lane; e < 3 * q; e += 32) out[e] = cadd(out[e], part[e]);
+        if (lane == 0) boxcnt[level_offset(level) + box] = cnt;
     }
-    cplx *out = mult + (level_offset(level) + box) * (long long)(3 * q);
-    out[k] = s1;
-    out[q + k] = s2;
-    out[2 * q + k] = s3;
-    if (k == 0) boxcnt[level_offset(level) + box] = cnt;
 }
+static size_t shift_smem(int q) { return sizeof(cplx) * (size_t)(kShiftWarps * 15 * q); }
 
 // ------------------------------------------------------------------------------------------------
 // M2L: one WARP per target box of `level` (four boxes per block), no block barrier inside the loop.  Lane `ln` owns
@@ -478,11 +511,11 @@ fmm_m2l(int level, int q, const double *__restrict__ tab, const unsigned long lo
 // which the sources are added differs (fixed, so the result is still reproducible run to run).
 constexpr int kM2LHalfQ = 16;
 __global__ void __launch_bounds__(32 * kM2LWarps)
-fmm_m2l_half(int level, int q, const double *__restrict__ tab, const unsigned long long *__restrict__ enc,
+fmm_m2l_half(int q, const double *__restrict__ tab, const unsigned long long *__restrict__ enc,
              const cplx *__restrict__ mult, const int *__restrict__ boxcnt, const int *__restrict__ tboxcnt,
              cplx *__restrict__ loc)
 {
-    if (level > load_level(enc)) return;
+    const int L = load_level(enc);
     extern __shared__ __align__(16) double sm[];
     double *Cb = sm;                                                  // [q][q]
     const int warp = threadIdx.x >> 5, ln = threadIdx.x & 31, half = ln >> 4, l = ln & 15;
@@ -493,14 +526,22 @@ fmm_m2l_half(int level, int q, const double *__restrict__ tab, const unsigned lo
     for (int e = threadIdx.x; e < q * q; e += blockDim.x) Cb[e] = t.Cb[e];
     if (l < 3) hat[l * (q + 1) + q] = make_double2(0.0, 0.0);
     __syncthreads();
-    const int n = 1 << level;
     const Geom gm = load_geom(enc);
-    const double s = gm.size / (double)n, log_s = log(s), inv_s = 1.0 / s;
+    const double log_size = log(gm.size);
     const bool v = l < q;
     const double sgn = (l & 1) ? -1.0 : 1.0, il = l > 0 ? 1.0 / (double)l : 0.0;
-    const long long lev0 = level_offset(level);
-    const cplx *Mlev = mult + lev0 * (long long)(3 * q);
-    for (int box = blockIdx.x * kM2LWarps + warp; box < n * n; box += gridDim.x * kM2LWarps) {
+    // the boxes of ALL levels 2 .. L in one launch, deepest level first (M2L of a level needs the multipoles only, not
+    // the other levels' local expansions; L2L adds the parents' afterwards): the small upper levels overlap with the
+    // tail of the deepest one instead of costing a launch each
+    const long long total = level_offset(L + 1) - level_offset(2);
+    for (long long gi = (long long)blockIdx.x * kM2LWarps + warp; gi < total; gi += (long long)gridDim.x * kM2LWarps) {
+        int level = L;
+        long long rem = gi;
+        while (rem >= (1ll << (2 * level))) { rem -= 1ll << (2 * level); --level; }
+        const int box = (int)rem, n = 1 << level;
+        const double s = gm.size / (double)n, inv_s = 1.0 / s, log_s = fma(-(double)level, 0.693147180559945309417, log_size);
+        const long long lev0 = level_offset(level);
+        const cplx *Mlev = mult + lev0 * (long long)(3 * q);
         if (tboxcnt && tboxcnt[lev0 + box] == 0) continue;
         const int ix = box / n, iy = box % n, px = ix >> 1, py = iy >> 1;
         // interaction list: children of the parent's neighbours that are not neighbours of the box and hold sources
@@ -603,32 +644,47 @@ static size_t m2l_half_smem(int q)
            sizeof(int) * (size_t)(kM2LWarps * 32);
 }
 
-// L2L: child local expansions inherit the parent's.  One thread per (child box, k); child level = `level`.
-__global__ void __launch_bounds__(128)
+// L2L: child local expansions inherit the parent's; child level = `level`.  One WARP per PARENT box: the parent's
+// expansion is staged once for its four children, work item (c, k) -- child c, output coefficient k -- sums
+// T(c; k, m) par[m] over m >= k; 4 q items are dealt to the lanes.
+__global__ void __launch_bounds__(32 * kShiftWarps)
 fmm_l2l(int level, int q, const double *__restrict__ tab, const unsigned long long *__restrict__ enc,
         const int *__restrict__ tboxcnt, cplx *__restrict__ loc)
 {
     if (level > load_level(enc)) return;
+    extern __shared__ __align__(16) double sm[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    cplx *par = (cplx *)sm + warp * 3 * q;
     const FmmTables t = fmm_tables_at(const_cast<double *>(tab), q);
-    const int n = 1 << level;
-    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= (long long)n * n * q) return;
-    const int box = (int)(e / q), k = (int)(e % q);
-    if (tboxcnt && tboxcnt[level_offset(level) + box] == 0) return;      // no targets below this box (see fmm_m2l)
-    const int ix = box / n, iy = box % n, c = 2 * (ix & 1) + (iy & 1);
-    const cplx *par = loc + (level_offset(level - 1) + (long long)(ix >> 1) * (n >> 1) + (iy >> 1)) * (long long)(3 * q);
-    const cplx *row = t.T + ((size_t)c * q + k) * q;
-    cplx s1 = make_double2(0.0, 0.0), s2 = s1, s3 = s1;
-    for (int m = k; m < q; ++m) {
-        const cplx tm = row[m];
-        s1 = cfma(tm, par[m], s1);
-        s2 = cfma(tm, par[q + m], s2);
-        s3 = cfma(tm, par[2 * q + m], s3);
+    const int n = 1 << level, np = n >> 1;
+    for (int pbox = blockIdx.x * kShiftWarps + warp; pbox < np * np; pbox += gridDim.x * kShiftWarps) {
+        if (tboxcnt && tboxcnt[level_offset(level - 1) + pbox] == 0) continue;   // no targets below the parent (see fmm_m2l)
+        const int px = pbox / np, py = pbox % np;
+        const long long child0 = level_offset(level) + (long long)(2 * px) * n + 2 * py;
+        const int tc = (lane < 4 && tboxcnt) ? tboxcnt[child0 + (long long)(lane >> 1) * n + (lane & 1)] : 1;
+        const unsigned have = __ballot_sync(0xffffffffu, tc != 0) & 0xfu;
+        __syncwarp();
+        const cplx *src = loc + (level_offset(level - 1) + pbox) * (long long)(3 * q);
+        for (int e = lane; e < 3 * q; e += 32) par[e] = src[e];
+        __syncwarp();
+        for (int w = lane; w < 4 * q; w += 32) {
+            const int c = w / q, k = w - c * q;
+            if (!((have >> c) & 1u)) continue;
+            const cplx *col = t.T + (size_t)c * q * q + k;
+            cplx s1 = make_double2(0.0, 0.0), s2 = s1, s3 = s1;
+#pragma unroll 4
+            for (int m = k; m < q; ++m) {
+                const cplx tm = __ldg(&col[(size_t)m * q]);
+                s1 = cfma(tm, par[m], s1);
+                s2 = cfma(tm, par[q + m], s2);
+                s3 = cfma(tm, par[2 * q + m], s3);
+            }
+            cplx *out = loc + (child0 + (long long)(c >> 1) * n + (c & 1)) * (long long)(3 * q);
+            out[k] = cadd(out[k], s1);
+            out[q + k] = cadd(out[q + k], s2);
+            out[2 * q + k] = cadd(out[2 * q + k], s3);
+        }
     }
-    cplx *out = loc + (level_offset(level) + box) * (long long)(3 * q);
-    out[k] = cadd(out[k], s1);
-    out[q + k] = cadd(out[q + k], s2);
-    out[2 * q + k] = cadd(out[2 * q + k], s3);
 }
 
 // the two tables of log_rcp_f64 in global memory (built once per call, copied to shared memory by every block)
@@ -1056,22 +1112,25 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
     fmm_p2m<<<(ncell + 3) / 4, 128, 0, st>>>(zs, gs, start, q, enc, mult, boxcnt);
     ++launches;
     for (int l = L - 1; l >= 2; --l) {
-        const long long work = (1ll << (2 * l)) * q;
-        fmm_m2m<<<(unsigned)((work + 127) / 128), 128, 0, st>>>(l, q, tab, enc, mult, boxcnt);
+        const unsigned nb = ((1u << (2 * l)) + kShiftWarps - 1) / kShiftWarps;          // a warp per parent box
+        fmm_m2m<<<nb < 148u * 16u ? nb : 148u * 16u, 32 * kShiftWarps, shift_smem(q), st>>>(l, q, tab, enc, mult, boxcnt);
         ++launches;
     }
     const size_t smem_m2l = sizeof(double) * (size_t)(((q * q + 1) & ~1) + 2 * kM2LWarps * 3 * (q + 1));
-    for (int l = 2; l <= L; ++l) {
-        const unsigned nb = ((1u << (2 * l)) + kM2LWarps - 1) / kM2LWarps;
-        if (q <= kM2LHalfQ)
-            fmm_m2l_half<<<nb < 148u * 16u ? nb : 148u * 16u, 32 * kM2LWarps, m2l_half_smem(q), st>>>(l, q, tab, enc, mult, boxcnt, boxcnt, loc);
-        else
-            fmm_m2l<<<nb < 148u * 16u ? nb : 148u * 16u, 32 * kM2LWarps, smem_m2l, st>>>(l, q, tab, enc, mult, boxcnt, boxcnt, loc);
+    if (q <= kM2LHalfQ) {              // all levels in one launch
+        const long long nb = (level_offset(L + 1) - level_offset(2) + kM2LWarps - 1) / kM2LWarps;
+        fmm_m2l_half<<<(unsigned)(nb < 148 * 16 ? nb : 148 * 16), 32 * kM2LWarps, m2l_half_smem(q), st>>>(q, tab, enc, mult, boxcnt, boxcnt, loc);
         ++launches;
+    } else {
+        for (int l = 2; l <= L; ++l) {
+            const unsigned nb = ((1u << (2 * l)) + kM2LWarps - 1) / kM2LWarps;
+            fmm_m2l<<<nb < 148u * 16u ? nb : 148u * 16u, 32 * kM2LWarps, smem_m2l, st>>>(l, q, tab, enc, mult, boxcnt, boxcnt, loc);
+            ++launches;
+        }
     }
     for (int l = 3; l <= L; ++l) {
-        const long long work = (1ll << (2 * l)) * q;
-        fmm_l2l<<<(unsigned)((work + 127) / 128), 128, 0, st>>>(l, q, tab, enc, boxcnt, loc);
+        const unsigned nb = ((1u << (2 * (l - 1))) + kShiftWarps - 1) / kShiftWarps;    // a warp per parent box
+        fmm_l2l<<<nb < 148u * 16u ? nb : 148u * 16u, 32 * kShiftWarps, shift_smem(q), st>>>(l, q, tab, enc, boxcnt, loc);
         ++launches;
     }
     if (prec == VN_F32)
@@ -1212,22 +1271,25 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
     fmm_p2m<<<(ncell + 3) / 4, 128, 0, st>>>(zs, gs, start, q, enc, mult, boxcnt);
     ++launches;
     for (int l = L - 1; l >= 2; --l) {
-        const long long work = (1ll << (2 * l)) * q;
-        fmm_m2m<<<(unsigned)((work + 127) / 128), 128, 0, st>>>(l, q, tab, enc, mult, boxcnt);
+        const unsigned nb = ((1u << (2 * l)) + kShiftWarps - 1) / kShiftWarps;          // a warp per parent box
+        fmm_m2m<<<nb < 148u * 16u ? nb : 148u * 16u, 32 * kShiftWarps, shift_smem(q), st>>>(l, q, tab, enc, mult, boxcnt);
         ++launches;
     }
     const size_t smem_m2l = sizeof(double) * (size_t)(((q * q + 1) & ~1) + 2 * kM2LWarps * 3 * (q + 1));
-    for (int l = 2; l <= L; ++l) {
-        const unsigned nb = ((1u << (2 * l)) + kM2LWarps - 1) / kM2LWarps;
-        if (q <= kM2LHalfQ)
-            fmm_m2l_half<<<nb < 148u * 16u ? nb : 148u * 16u, 32 * kM2LWarps, m2l_half_smem(q), st>>>(l, q, tab, enc, mult, boxcnt, nullptr, loc);
-        else
-            fmm_m2l<<<nb < 148u * 16u ? nb : 148u * 16u, 32 * kM2LWarps, smem_m2l, st>>>(l, q, tab, enc, mult, boxcnt, nullptr, loc);
+    if (q <= kM2LHalfQ) {              // all levels in one launch
+        const long long nb = (level_offset(L + 1) - level_offset(2) + kM2LWarps - 1) / kM2LWarps;
+        fmm_m2l_half<<<(unsigned)(nb < 148 * 16 ? nb : 148 * 16), 32 * kM2LWarps, m2l_half_smem(q), st>>>(q, tab, enc, mult, boxcnt, nullptr, loc);
         ++launches;
+    } else {
+        for (int l = 2; l <= L; ++l) {
+            const unsigned nb = ((1u << (2 * l)) + kM2LWarps - 1) / kM2LWarps;
+            fmm_m2l<<<nb < 148u * 16u ? nb : 148u * 16u, 32 * kM2LWarps, smem_m2l, st>>>(l, q, tab, enc, mult, boxcnt, nullptr, loc);
+            ++launches;
+        }
     }
     for (int l = 3; l <= L; ++l) {
-        const long long work = (1ll << (2 * l)) * q;
-        fmm_l2l<<<(unsigned)((work + 127) / 128), 128, 0, st>>>(l, q, tab, enc, nullptr, loc);
+        const unsigned nb = ((1u << (2 * (l - 1))) + kShiftWarps - 1) / kShiftWarps;    // a warp per parent box
+        fmm_l2l<<<nb < 148u * 16u ? nb : 148u * 16u, 32 * kShiftWarps, shift_smem(q), st>>>(l, q, tab, enc, nullptr, loc);
         ++launches;
     }
     if (prec == VN_F32)
