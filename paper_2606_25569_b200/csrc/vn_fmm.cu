@@ -17,6 +17,10 @@
 // points in non-neighbour boxes) is subtracted by a short direct sum.  The expansions are double for both storage
 // precisions, so the accuracy of the far part is set by p alone (truncation error about 0.45^p relative, measured);
 // the direct part runs in the storage precision (fp32: the SFU pair arithmetic of the exact fp32 kernel).
+#ifdef VN_FMM_TIMING
+#include <cstdio>
+#endif
+
 #include "vn_common.cuh"
 #include "vn_log64.cuh"
 
@@ -326,6 +330,75 @@ fmm_p2m(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const long lon
     for (int e = lane; e < 3 * q; e += 32) out[e] = acc[warp][e];
 }
 
+// P2M for q <= 16.  fmm_p2m reduces every power over the lanes (60 shuffles per coefficient and 32 sources); here
+// the sum runs the other way round: for 32 sources at a time lane j writes the powers w_j^0 .. w_j^(q-1) of ITS source
+// into the warp's shared memory (row stride odd in 16-byte words: conflict-free both ways), then lane (half, k) adds up
+// coefficient k over the sources j = half, half + 2, ... -- a 16-byte load of the power and two broadcasts (g, conj(zeta) g)
+// per 8 DFMA, no shuffles -- and the two halves meet once per leaf.
+constexpr int kP2MWarps = 4;
+__global__ void __launch_bounds__(32 * kP2MWarps)
+fmm_p2m_half(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const long long *__restrict__ start, int q,
+             const unsigned long long *__restrict__ enc, cplx *__restrict__ mult, int *__restrict__ boxcnt)
+{
+    const int L = load_level(enc);
+    extern __shared__ __align__(16) double sm[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, half = lane >> 4, k = lane & 15;
+    const int stride = q | 1;
+    cplx *pw = (cplx *)sm + warp * (32 * stride + 64);               // [32][stride] powers | [32] g | [32] conj(zeta) g
+    cplx *sg = pw + 32 * stride, *sh = sg + 32;
+    const int n = 1 << L, ncell = n * n;
+    const Geom gm = load_geom(enc);
+    const double s = gm.size / (double)n, inv_s = 1.0 / s;
+    const bool v = k < q;
+    for (int c = blockIdx.x * kP2MWarps + warp; c < ncell; c += gridDim.x * kP2MWarps) {
+        const long long a = start[c], b = start[c + 1];
+        if (lane == 0) boxcnt[level_offset(L) + c] = (int)(b - a);
+        cplx *out = mult + (level_offset(L) + c) * (long long)(3 * q);
+        if (a == b) {                                                // the upper levels read the moments of empty leaves too
+            for (int e = lane; e < 3 * q; e += 32) out[e] = make_double2(0.0, 0.0);
+            continue;
+        }
+        const cplx ctr = box_centre(gm, L, c / n, c % n);
+        cplx a1 = make_double2(0.0, 0.0), a2 = a1, bb = a1;          // A1_k, A2_k, B_k (this half's sources)
+        for (long long base = a; base < b; base += 32) {
+            const long long idx = base + lane;
+            const int cnt = (int)min(32ll, b - base);
+            __syncwarp();                                            // the previous 32 sources are consumed
+            if (idx < b) {
+                const cplx zt = zs[idx], g = gs[idx];
+                const cplx w = make_double2((zt.x - ctr.x) * inv_s, (zt.y - ctr.y) * inv_s);
+                sg[lane] = g;
+                sh[lane] = cmul(make_double2(zt.x, -zt.y), g);      // conj(zeta) g
+                cplx p = make_double2(1.0, 0.0);
+                cplx *row = pw + lane * stride;
+                for (int kk = 0; kk < q; ++kk) {
+                    row[kk] = p;
+                    p = cmul(p, w);
+                }
+            }
+            __syncwarp();
+            if (v) {
+#pragma unroll 4
+                for (int j = half; j < cnt; j += 2) {
+                    const cplx p = pw[j * stride + k], g = sg[j], h = sh[j];
+                    a1.x = fma(g.x, p.x, a1.x); a1.y = fma(g.x, p.y, a1.y);
+                    a2.x = fma(g.y, p.x, a2.x); a2.y = fma(g.y, p.y, a2.y);
+                    bb = cfma(h, p, bb);
+                }
+            }
+        }
+        a1.x += __shfl_xor_sync(0xffffffffu, a1.x, 16); a1.y += __shfl_xor_sync(0xffffffffu, a1.y, 16);
+        a2.x += __shfl_xor_sync(0xffffffffu, a2.x, 16); a2.y += __shfl_xor_sync(0xffffffffu, a2.y, 16);
+        bb.x += __shfl_xor_sync(0xffffffffu, bb.x, 16); bb.y += __shfl_xor_sync(0xffffffffu, bb.y, 16);
+        if (v && half == 0) {
+            out[k] = a1;
+            out[q + k] = a2;
+            out[2 * q + k] = bb;
+        }
+    }
+}
+static size_t p2m_half_smem(int q) { return sizeof(cplx) * (size_t)(kP2MWarps * (32 * (q | 1) + 64)); }
+
 // M2M: parent moments from its four children, levels L-1 down to 2.  One WARP per parent box: the children's
 // moments are staged in the warp's shared memory with coalesced loads (one round trip to L2 instead of one per term),
 // then work item (k, h) -- output coefficient k, child pair h -- sums S(c; k, m) A_c[m] over m and the pair's two
@@ -333,6 +406,26 @@ fmm_p2m(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const long lon
 // index fastest (coalesced, L1-resident), the children's coefficients are shared-memory broadcasts, and the two
 // pairs' partial sums meet through shared memory.
 constexpr int kShiftWarps = 4;
+constexpr int kShiftStageQ = 16;
+// dst[e] = src[e], e = first, first + stride, ... < count, with eight loads in flight per thread: written as
+// dst[e] = src[e] in a loop, every load waits for the previous store (the compiler cannot rule out aliasing), and
+// the kernels of the small upper levels are nothing but such latencies in a row
+__device__ __forceinline__ void stage_cplx(cplx *dst, const cplx *src, int first, int stride, int count)
+{
+    for (int e0 = first; e0 < count; e0 += 8 * stride) {
+        cplx tmp[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            const int e = e0 + i * stride;
+            if (e < count) tmp[i] = src[e];
+        }
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            const int e = e0 + i * stride;
+            if (e < count) dst[e] = tmp[i];
+        }
+    }
+}
 __global__ void __launch_bounds__(32 * kShiftWarps)
 fmm_m2m(int level, int q, const double *__restrict__ tab, const unsigned long long *__restrict__ enc,
         cplx *__restrict__ mult, int *__restrict__ boxcnt)
@@ -340,9 +433,18 @@ fmm_m2m(int level, int q, const double *__restrict__ tab, const unsigned long lo
     if (level >= load_level(enc)) return;
     extern __shared__ __align__(16) double sm[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    cplx *ch = (cplx *)sm + warp * (12 * q + 3 * q);               // [4][3][q] children | [3][q] second pair's partial sums
+    cplx *ch = (cplx *)sm + warp * (12 * q + 6 * q);               // [4][3][q] children | [2][3][q] the child pairs' partial sums
     cplx *part = ch + 12 * q;
     const FmmTables t = fmm_tables_at(const_cast<double *>(tab), q);
+    // the table: in shared memory up to kShiftStageQ (every launch starts with a cold L1: read through it, the
+    // 4 q loads of a work item would each wait for L2), straight from global memory above
+    const cplx *Stab = t.S;
+    if (q <= kShiftStageQ) {
+        cplx *st = (cplx *)sm + kShiftWarps * 18 * q;
+        stage_cplx(st, t.S, threadIdx.x, blockDim.x, 4 * q * q);
+        Stab = st;
+        __syncthreads();
+    }
     const int n = 1 << level;
     for (int box = blockIdx.x * kShiftWarps + warp; box < n * n; box += gridDim.x * kShiftWarps) {
         const int ix = box / n, iy = box % n;
@@ -354,11 +456,9 @@ fmm_m2m(int level, int q, const double *__restrict__ tab, const unsigned long lo
         cnt += __shfl_xor_sync(0xffffffffu, cnt, 1);
         cnt += __shfl_xor_sync(0xffffffffu, cnt, 2);
         __syncwarp();                                               // the previous box's staging is consumed
-        for (int e = lane; e < 12 * q; e += 32) {
-            const int c = e / (3 * q);
-            ch[e] = ((have >> c) & 1u) ? mult[(child0 + (long long)(c >> 1) * (2 * n) + (c & 1)) * (long long)(3 * q) + (e - c * 3 * q)]
-                                       : make_double2(0.0, 0.0);
-        }
+        for (int c = 0; c < 4; ++c)                                 // children without sources are skipped below, not staged
+            if ((have >> c) & 1u)
+                stage_cplx(ch + c * 3 * q, mult + (child0 + (long long)(c >> 1) * (2 * n) + (c & 1)) * (long long)(3 * q), lane, 32, 3 * q);
         __syncwarp();
         cplx *out = mult + (level_offset(level) + box) * (long long)(3 * q);
         for (int w0 = 0; w0 < 2 * q; w0 += 32) {
@@ -369,29 +469,26 @@ fmm_m2m(int level, int q, const double *__restrict__ tab, const unsigned long lo
             for (int c = 2 * h; c < 2 * h + 2; ++c) {
                 if (!((have >> c) & 1u)) continue;
                 const cplx *A = ch + c * 3 * q;
-                const cplx *col = t.S + (size_t)c * q * q + k;
+                const cplx *col = Stab + (size_t)c * q * q + k;
 #pragma unroll 4
                 for (int m = 0; m < q; ++m) {                       // entries with m > k are zero
-                    const cplx sm_ = __ldg(&col[(size_t)m * q]);
+                    const cplx sm_ = col[(size_t)m * q];
                     s1 = cfma(sm_, A[m], s1);
                     s2 = cfma(sm_, A[q + m], s2);
                     s3 = cfma(sm_, A[2 * q + m], s3);
                 }
             }
-            if (live && h == 1) { part[k] = s1; part[q + k] = s2; part[2 * q + k] = s3; }
-            __syncwarp();
-            if (live && h == 0) {
-                // the second pair's item (k, 1) is item q + k: it was computed in this round or is computed in a later one
-                out[k] = s1; out[q + k] = s2; out[2 * q + k] = s3;
+            if (live) {
+                cplx *mine = part + h * 3 * q;
+                mine[k] = s1; mine[q + k] = s2; mine[2 * q + k] = s3;
             }
         }
         __syncwarp();
-        // add the second pair's partial sums (all items are done)
-        for (int e = lane; e < 3 * q; e += 32) out[e] = cadd(out[e], part[e]);
+        for (int e = lane; e < 3 * q; e += 32) out[e] = cadd(part[e], part[3 * q + e]);
         if (lane == 0) boxcnt[level_offset(level) + box] = cnt;
     }
 }
-static size_t shift_smem(int q) { return sizeof(cplx) * (size_t)(kShiftWarps * 15 * q); }
+static size_t shift_smem(int q) { return sizeof(cplx) * (size_t)(kShiftWarps * 18 * q + (q <= kShiftStageQ ? 4 * q * q : 0)); }
 
 // ------------------------------------------------------------------------------------------------
 // M2L: one WARP per target box of `level` (four boxes per block), no block barrier inside the loop.  Lane `ln` owns
@@ -656,6 +753,13 @@ fmm_l2l(int level, int q, const double *__restrict__ tab, const unsigned long lo
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     cplx *par = (cplx *)sm + warp * 3 * q;
     const FmmTables t = fmm_tables_at(const_cast<double *>(tab), q);
+    const cplx *Ttab = t.T;                                         // staged like the table of fmm_m2m
+    if (q <= kShiftStageQ) {
+        cplx *st = (cplx *)sm + kShiftWarps * 18 * q;
+        stage_cplx(st, t.T, threadIdx.x, blockDim.x, 4 * q * q);
+        Ttab = st;
+        __syncthreads();
+    }
     const int n = 1 << level, np = n >> 1;
     for (int pbox = blockIdx.x * kShiftWarps + warp; pbox < np * np; pbox += gridDim.x * kShiftWarps) {
         if (tboxcnt && tboxcnt[level_offset(level - 1) + pbox] == 0) continue;   // no targets below the parent (see fmm_m2l)
@@ -664,25 +768,24 @@ fmm_l2l(int level, int q, const double *__restrict__ tab, const unsigned long lo
         const int tc = (lane < 4 && tboxcnt) ? tboxcnt[child0 + (long long)(lane >> 1) * n + (lane & 1)] : 1;
         const unsigned have = __ballot_sync(0xffffffffu, tc != 0) & 0xfu;
         __syncwarp();
-        const cplx *src = loc + (level_offset(level - 1) + pbox) * (long long)(3 * q);
-        for (int e = lane; e < 3 * q; e += 32) par[e] = src[e];
+        stage_cplx(par, loc + (level_offset(level - 1) + pbox) * (long long)(3 * q), lane, 32, 3 * q);
         __syncwarp();
         for (int w = lane; w < 4 * q; w += 32) {
             const int c = w / q, k = w - c * q;
             if (!((have >> c) & 1u)) continue;
-            const cplx *col = t.T + (size_t)c * q * q + k;
-            cplx s1 = make_double2(0.0, 0.0), s2 = s1, s3 = s1;
+            const cplx *col = Ttab + (size_t)c * q * q + k;
+            cplx *out = loc + (child0 + (long long)(c >> 1) * n + (c & 1)) * (long long)(3 * q);
+            cplx s1 = out[k], s2 = out[q + k], s3 = out[2 * q + k];      // the child's own M2L part, in flight during the sum
 #pragma unroll 4
             for (int m = k; m < q; ++m) {
-                const cplx tm = __ldg(&col[(size_t)m * q]);
+                const cplx tm = col[(size_t)m * q];
                 s1 = cfma(tm, par[m], s1);
                 s2 = cfma(tm, par[q + m], s2);
                 s3 = cfma(tm, par[2 * q + m], s3);
             }
-            cplx *out = loc + (child0 + (long long)(c >> 1) * n + (c & 1)) * (long long)(3 * q);
-            out[k] = cadd(out[k], s1);
-            out[q + k] = cadd(out[q + k], s2);
-            out[2 * q + k] = cadd(out[2 * q + k], s3);
+            out[k] = s1;
+            out[q + k] = s2;
+            out[2 * q + k] = s3;
         }
     }
 }
@@ -1052,6 +1155,41 @@ fmm_finish(const cplx *__restrict__ z, const cplx *__restrict__ g, const int *__
 }
 
 // ------------------------------------------------------------------------------------------------
+// -DVN_FMM_TIMING (diagnostic builds only): device time of every phase of vn_farfield_fmm, printed to stderr per call
+#ifdef VN_FMM_TIMING
+struct FmmTimer {
+    cudaStream_t st;
+    cudaEvent_t ev[40];
+    const char *name[40];
+    int n = 0;
+    explicit FmmTimer(cudaStream_t s) : st(s) { tick("start"); }
+    void tick(const char *what)
+    {
+        if (n >= 40) return;
+        cudaEventCreate(&ev[n]);
+        cudaEventRecord(ev[n], st);
+        name[n++] = what;
+    }
+    ~FmmTimer()
+    {
+        cudaEventSynchronize(ev[n - 1]);
+        float total = 0.f;
+        cudaEventElapsedTime(&total, ev[0], ev[n - 1]);
+        fprintf(stderr, "fmm phases (us):");
+        for (int i = 1; i < n; ++i) {
+            float ms = 0.f;
+            cudaEventElapsedTime(&ms, ev[i - 1], ev[i]);
+            fprintf(stderr, " %s %.1f", name[i], ms * 1e3f);
+        }
+        fprintf(stderr, " | total %.1f\n", total * 1e3f);
+        for (int i = 0; i < n; ++i) cudaEventDestroy(ev[i]);
+    }
+};
+#define FMM_TICK(what) fmm_timer.tick(what)
+#else
+#define FMM_TICK(what) ((void)0)
+#endif
+
 static int fmm_levels_max(long long P)
 {
     // the deepest tree the device may choose: leaves of kLeafTarget points if only 1/16 of the root square is occupied
@@ -1088,6 +1226,9 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
     double *tab = (double *)take(b_tab), *logtab = (double *)take(b_log);
     unsigned long long *enc = (unsigned long long *)take(256);
 
+#ifdef VN_FMM_TIMING
+    FmmTimer fmm_timer(st);
+#endif
     VN_CUDA(cudaMemsetAsync(boxcnt, 0, b_cnt + b_leaf, st));      // boxcnt and the leaf counts are adjacent
     fmm_init_bounds<<<1, 1, 0, st>>>(enc);
     const int gp = (P + 255) / 256;
@@ -1095,28 +1236,37 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
         fmm_load<float, float2><<<gp, 256, 0, st>>>((const float2 *)X, (const float2 *)F, (const float *)W, P, z, g, enc);
     else
         fmm_load<double, double2><<<gp, 256, 0, st>>>((const double2 *)X, (const double2 *)F, (const double *)W, P, z, g, enc);
+    FMM_TICK("load");
     fmm_choose_level<<<1, 1, 0, st>>>(enc, P, L);
     fmm_bin<<<gp, 256, 0, st>>>(z, P, enc, cell, cnt);
     scan_block_sums<<<nb_scan, kScanThreads, 0, st>>>(cnt, ncell, bsum);
     scan_of_sums<<<1, kScanThreads, 0, st>>>(bsum, nb_scan);
     scan_apply<<<nb_scan, kScanThreads, 0, st>>>(cnt, ncell, bsum, start, cursor);
+    FMM_TICK("bin+scan");
     fmm_scatter<<<gp, 256, 0, st>>>(cell, P, cursor, vs);                  // vs doubles as the unsorted buffer
     fmm_sort_cells<<<(ncell + 3) / 4, 128, 0, st>>>(start, ncell, vs, perm);
     fmm_gather<<<gp, 256, 0, st>>>(perm, P, (int)npts, z, g, zs, gs, vs);
+    FMM_TICK("sort+gather");
     fmm_build_tables<<<64, 128, 0, st>>>(q, tab);
     fmm_build_logtab<<<8, 128, 0, st>>>(logtab);
     int launches = 13;
 
     const int p2p_grid = ncell < 148 * 64 ? ncell : 148 * 64;      // grid-stride over the leaves the device chose
+    FMM_TICK("tables");
     profile_mark(st, true);
-    fmm_p2m<<<(ncell + 3) / 4, 128, 0, st>>>(zs, gs, start, q, enc, mult, boxcnt);
+    if (q <= kM2LHalfQ)
+        fmm_p2m_half<<<(ncell + kP2MWarps - 1) / kP2MWarps < 148 * 16 ? (ncell + kP2MWarps - 1) / kP2MWarps : 148 * 16, 32 * kP2MWarps, p2m_half_smem(q), st>>>(zs, gs, start, q, enc, mult, boxcnt);
+    else
+        fmm_p2m<<<(ncell + 3) / 4, 128, 0, st>>>(zs, gs, start, q, enc, mult, boxcnt);
     ++launches;
+    FMM_TICK("p2m");
     for (int l = L - 1; l >= 2; --l) {
         const unsigned nb = ((1u << (2 * l)) + kShiftWarps - 1) / kShiftWarps;          // a warp per parent box
         fmm_m2m<<<nb < 148u * 16u ? nb : 148u * 16u, 32 * kShiftWarps, shift_smem(q), st>>>(l, q, tab, enc, mult, boxcnt);
         ++launches;
     }
     const size_t smem_m2l = sizeof(double) * (size_t)(((q * q + 1) & ~1) + 2 * kM2LWarps * 3 * (q + 1));
+    FMM_TICK("m2m");
     if (q <= kM2LHalfQ) {              // all levels in one launch
         const long long nb = (level_offset(L + 1) - level_offset(2) + kM2LWarps - 1) / kM2LWarps;
         fmm_m2l_half<<<(unsigned)(nb < 148 * 16 ? nb : 148 * 16), 32 * kM2LWarps, m2l_half_smem(q), st>>>(q, tab, enc, mult, boxcnt, boxcnt, loc);
@@ -1128,16 +1278,19 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
             ++launches;
         }
     }
+    FMM_TICK("m2l");
     for (int l = 3; l <= L; ++l) {
         const unsigned nb = ((1u << (2 * (l - 1))) + kShiftWarps - 1) / kShiftWarps;    // a warp per parent box
         fmm_l2l<<<nb < 148u * 16u ? nb : 148u * 16u, 32 * kShiftWarps, shift_smem(q), st>>>(l, q, tab, enc, boxcnt, loc);
         ++launches;
     }
+    FMM_TICK("l2l");
     if (prec == VN_F32)
         fmm_l2p_p2p_packed<<<p2p_grid, 128, 0, st>>>(zs, gs, vs, start, zs, vs, perm, start, q, enc, loc, accum);
     else
         fmm_l2p_p2p<false><<<p2p_grid, kP2PThreads, 0, st>>>(zs, gs, vs, start, zs, vs, perm, start, q, enc, loc, logtab, accum);
     profile_mark(st, false);
+    FMM_TICK("l2p+p2p");
     if (near_ptr) {   // row f-1 on top: take the near vesicles' contributions out (they are all in the direct part)
         const vn_status rc = near_correction_accum(X, F, W, P, (int)npts, near_ptr, near_ves, accum, prec, st);
         if (rc != VN_OK) { (void)cudaFreeAsync(scr, st); return rc; }
@@ -1148,6 +1301,7 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
     else
         fmm_finish<double2><<<(P + 127) / 128, 128, 0, st>>>(z, g, cell, P, (int)npts, enc, accum, pref, (double2 *)U);
     count_launch(launches + 2);
+    FMM_TICK("finish");
     const cudaError_t e = cudaGetLastError();
     VN_CUDA(cudaFreeAsync(scr, st));
     return e == cudaSuccess ? VN_OK : VN_ERR_CUDA;
@@ -1268,7 +1422,10 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
 
     const int p2p_grid = ncell < 148 * 64 ? ncell : 148 * 64;      // grid-stride over the leaves the device chose
     profile_mark(st, true);
-    fmm_p2m<<<(ncell + 3) / 4, 128, 0, st>>>(zs, gs, start, q, enc, mult, boxcnt);
+    if (q <= kM2LHalfQ)
+        fmm_p2m_half<<<(ncell + kP2MWarps - 1) / kP2MWarps < 148 * 16 ? (ncell + kP2MWarps - 1) / kP2MWarps : 148 * 16, 32 * kP2MWarps, p2m_half_smem(q), st>>>(zs, gs, start, q, enc, mult, boxcnt);
+    else
+        fmm_p2m<<<(ncell + 3) / 4, 128, 0, st>>>(zs, gs, start, q, enc, mult, boxcnt);
     ++launches;
     for (int l = L - 1; l >= 2; --l) {
         const unsigned nb = ((1u << (2 * l)) + kShiftWarps - 1) / kShiftWarps;          // a warp per parent box
