@@ -120,23 +120,12 @@ __global__ void fmm_choose_level(unsigned long long *enc, int P, int L_hi)
 }
 __device__ __forceinline__ int load_level(const unsigned long long *__restrict__ enc) { return (int)enc[4]; }
 
-// positions and densities g = F*W promoted to double (original order), and the bounding box
-template <typename real, typename real2>
-__global__ void __launch_bounds__(256)
-fmm_load(const real2 *__restrict__ X, const real2 *__restrict__ F, const real *__restrict__ W, int P,
-         cplx *__restrict__ z, cplx *__restrict__ g, unsigned long long *__restrict__ enc)
+// bounding box of a block's points: per-thread extremes -> warp shuffles -> shared memory -> FOUR atomics per block
+// (one set per warp was 128 K serialised 64-bit atomics on four addresses at a million points: 80 of the kernel's 96 us)
+__device__ __forceinline__ void bounds_commit(double x, double y, double X1, double Y1, unsigned long long *__restrict__ enc)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    double x = INFINITY, y = INFINITY, X1 = -INFINITY, Y1 = -INFINITY;
-    if (i < P) {
-        const real2 p = X[i];
-        const real2 f = F[i];
-        const real w = W[i];
-        x = X1 = (double)p.x;
-        y = Y1 = (double)p.y;
-        z[i] = make_double2(x, y);
-        g[i] = make_double2((double)(f.x * w), (double)(f.y * w));   // product in the storage precision, as in the exact path
-    }
+    __shared__ double red[4][32];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = (blockDim.x + 31) >> 5;
 #pragma unroll
     for (int m = 16; m >= 1; m >>= 1) {
         x = fmin(x, __shfl_xor_sync(0xffffffffu, x, m));
@@ -144,12 +133,49 @@ fmm_load(const real2 *__restrict__ X, const real2 *__restrict__ F, const real *_
         X1 = fmax(X1, __shfl_xor_sync(0xffffffffu, X1, m));
         Y1 = fmax(Y1, __shfl_xor_sync(0xffffffffu, Y1, m));
     }
-    if ((threadIdx.x & 31) == 0 && x <= X1) {
+    if (lane == 0) { red[0][warp] = x; red[1][warp] = y; red[2][warp] = X1; red[3][warp] = Y1; }
+    __syncthreads();
+    if (warp != 0) return;
+    x = lane < nw ? red[0][lane] : INFINITY;
+    y = lane < nw ? red[1][lane] : INFINITY;
+    X1 = lane < nw ? red[2][lane] : -INFINITY;
+    Y1 = lane < nw ? red[3][lane] : -INFINITY;
+#pragma unroll
+    for (int m = 16; m >= 1; m >>= 1) {
+        x = fmin(x, __shfl_xor_sync(0xffffffffu, x, m));
+        y = fmin(y, __shfl_xor_sync(0xffffffffu, y, m));
+        X1 = fmax(X1, __shfl_xor_sync(0xffffffffu, X1, m));
+        Y1 = fmax(Y1, __shfl_xor_sync(0xffffffffu, Y1, m));
+    }
+    if (lane == 0 && x <= X1) {
         atomicMin(enc + 0, enc_f64(x));
         atomicMin(enc + 1, enc_f64(y));
         atomicMax(enc + 2, enc_f64(X1));
         atomicMax(enc + 3, enc_f64(Y1));
     }
+}
+constexpr int kLoadBlocks = 148 * 8;      // grid-stride: at most this many blocks commit a bounding box
+
+// positions and densities g = F*W promoted to double (original order), and the bounding box
+template <typename real, typename real2>
+__global__ void __launch_bounds__(256)
+fmm_load(const real2 *__restrict__ X, const real2 *__restrict__ F, const real *__restrict__ W, int P,
+         cplx *__restrict__ z, cplx *__restrict__ g, unsigned long long *__restrict__ enc)
+{
+    double x = INFINITY, y = INFINITY, X1 = -INFINITY, Y1 = -INFINITY;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < P; i += gridDim.x * blockDim.x) {
+        const real2 p = X[i];
+        const real2 f = F[i];
+        const real w = W[i];
+        const double px = (double)p.x, py = (double)p.y;
+        x = fmin(x, px);
+        y = fmin(y, py);
+        X1 = fmax(X1, px);
+        Y1 = fmax(Y1, py);
+        z[i] = make_double2(px, py);
+        g[i] = make_double2((double)(f.x * w), (double)(f.y * w));   // product in the storage precision, as in the exact path
+    }
+    bounds_commit(x, y, X1, Y1, enc);
 }
 
 // moves every point into the root square's frame (in place, see Geom), then: leaf box of every point and the
@@ -187,9 +213,28 @@ fmm_scatter(const int *__restrict__ cell, int P, long long *__restrict__ cursor,
 __global__ void __launch_bounds__(128)
 fmm_sort_cells(const long long *__restrict__ start, int ncell, const int *__restrict__ unsorted, int *__restrict__ perm)
 {
-    const int c = blockIdx.x * 4 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    constexpr int kBuf = 256;                          // leaves up to this size are ranked out of shared memory
+    __shared__ int buf[4][kBuf];
+    const int w = threadIdx.x >> 5, c = blockIdx.x * 4 + w, lane = threadIdx.x & 31;
     if (c >= ncell) return;
     const long long a = start[c], b = start[c + 1];
+    const int m = (int)(b - a);
+    if (m <= 1) {
+        if (m == 1 && lane == 0) perm[a] = unsorted[a];
+        return;
+    }
+    if (m <= kBuf) {
+        for (int i = lane; i < m; i += 32) buf[w][i] = unsorted[a + i];
+        __syncwarp();
+        for (int i = lane; i < m; i += 32) {
+            const int v = buf[w][i];
+            int rank = 0;
+#pragma unroll 8
+            for (int j = 0; j < m; ++j) rank += buf[w][j] < v;
+            perm[a + rank] = v;
+        }
+        return;
+    }
     for (long long i = a + lane; i < b; i += 32) {
         const int v = unsorted[i];
         int rank = 0;
@@ -1121,37 +1166,75 @@ fmm_l2p_p2p_packed(const cplx *__restrict__ zs, const cplx *__restrict__ gs, con
 }
 
 // own-vesicle points that sit in NON-neighbour leaf boxes of the target went through the expansions: take their
-// contribution out again (direct, libm log), scale by 1/(4 pi mu) and store.  One thread per point.
-template <typename real2>
-__global__ void __launch_bounds__(128)
-fmm_finish(const cplx *__restrict__ z, const cplx *__restrict__ g, const int *__restrict__ cell, int P, int npts,
+// contribution out again, scale by 1/(4 pi mu) and store.  One block per vesicle: its points (position, density, leaf)
+// are staged in shared memory once and every thread walks them for its own point -- consecutive points of a membrane
+// sit in the same or adjacent leaves, so a warp's neighbour tests agree and the few direct terms are not divergent.
+// F32 (single-precision storage): the terms are evaluated with the SFU pair arithmetic of the fp32 kernels (the
+// positions and densities are floats; the correction is a small part of the sum); double: libm log and a division.
+constexpr int kFinThreads = 128;
+constexpr int kFinChunk = 256;
+template <typename real2, bool F32>
+__global__ void __launch_bounds__(kFinThreads)
+fmm_finish(const cplx *__restrict__ z, const cplx *__restrict__ g, const int *__restrict__ cell, int nves, int npts,
            const unsigned long long *__restrict__ enc, const cplx *__restrict__ accum, double prefactor,
            real2 *__restrict__ U)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= P) return;
+    __shared__ cplx sz[kFinChunk], sg[kFinChunk];
+    __shared__ int sc[kFinChunk];
     const int L = load_level(enc);
-    const int n = 1 << L;
-    const int ci = cell[i], ix = ci >> L, iy = ci & (n - 1);
-    const cplx zi = z[i];
-    const int v0 = (i / npts) * npts;
-    double cx = 0.0, cy = 0.0;
-    for (int j = v0; j < v0 + npts; ++j) {
-        const int cj = cell[j];
-        if (abs((cj >> L) - ix) <= 1 && abs((cj & (n - 1)) - iy) <= 1) continue;
-        const cplx gj = g[j];
-        const double rx = zi.x - z[j].x, ry = zi.y - z[j].y;
-        const double r2 = rx * rx + ry * ry;
-        const double ml = -0.5 * log(r2);
-        const double qd = (rx * gj.x + ry * gj.y) / r2;
-        cx += ml * gj.x + qd * rx;
-        cy += ml * gj.y + qd * ry;
+    const int n = 1 << L, tid = threadIdx.x;
+    for (int ves = blockIdx.x; ves < nves; ves += gridDim.x) {
+        const long long v0 = (long long)ves * npts;
+        for (int t0 = 0; t0 < npts; t0 += kFinThreads) {
+            const bool live = t0 + tid < npts;
+            const long long i = v0 + (live ? t0 + tid : 0);
+            const cplx zi = z[i];
+            const int ci = cell[i], ix = ci >> L, iy = ci & (n - 1);
+            double cx = 0.0, cy = 0.0;
+            for (int s0 = 0; s0 < npts; s0 += kFinChunk) {
+                const int cnt = min(kFinChunk, npts - s0);
+                __syncthreads();
+                for (int e = tid; e < cnt; e += kFinThreads) {
+                    sz[e] = z[v0 + s0 + e];
+                    sg[e] = g[v0 + s0 + e];
+                    sc[e] = cell[v0 + s0 + e];
+                }
+                __syncthreads();
+                if (!live) continue;
+                float fx = 0.f, fy = 0.f;
+                for (int j = 0; j < cnt; ++j) {
+                    const int cj = sc[j];
+                    if (abs((cj >> L) - ix) <= 1 && abs((cj & (n - 1)) - iy) <= 1) continue;   // in the direct part: masked there
+                    const cplx zj = sz[j], gj = sg[j];
+                    if (F32) {
+                        const float rx = (float)(zi.x - zj.x), ry = (float)(zi.y - zj.y);
+                        const float gx = (float)gj.x, gy = (float)gj.y;
+                        const float r2 = fmaf(rx, rx, ry * ry);
+                        const float ml = -0.34657359027997264f * sfu_lg2(r2);
+                        const float qd = fmaf(rx, gx, ry * gy) * sfu_rcp(r2);
+                        fx += fmaf(ml, gx, qd * rx);
+                        fy += fmaf(ml, gy, qd * ry);
+                    } else {
+                        const double rx = zi.x - zj.x, ry = zi.y - zj.y;
+                        const double r2 = rx * rx + ry * ry;
+                        const double ml = -0.5 * log(r2);
+                        const double qd = (rx * gj.x + ry * gj.y) / r2;
+                        cx += ml * gj.x + qd * rx;
+                        cy += ml * gj.y + qd * ry;
+                    }
+                }
+                cx += (double)fx;
+                cy += (double)fy;
+            }
+            if (live) {
+                const cplx u = accum[i];
+                real2 o;
+                o.x = (decltype(o.x))(prefactor * (u.x - cx));
+                o.y = (decltype(o.y))(prefactor * (u.y - cy));
+                U[i] = o;
+            }
+        }
     }
-    const cplx u = accum[i];
-    real2 o;
-    o.x = (decltype(o.x))(prefactor * (u.x - cx));
-    o.y = (decltype(o.y))(prefactor * (u.y - cy));
-    U[i] = o;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -1233,9 +1316,9 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
     fmm_init_bounds<<<1, 1, 0, st>>>(enc);
     const int gp = (P + 255) / 256;
     if (prec == VN_F32)
-        fmm_load<float, float2><<<gp, 256, 0, st>>>((const float2 *)X, (const float2 *)F, (const float *)W, P, z, g, enc);
+        fmm_load<float, float2><<<gp < kLoadBlocks ? gp : kLoadBlocks, 256, 0, st>>>((const float2 *)X, (const float2 *)F, (const float *)W, P, z, g, enc);
     else
-        fmm_load<double, double2><<<gp, 256, 0, st>>>((const double2 *)X, (const double2 *)F, (const double *)W, P, z, g, enc);
+        fmm_load<double, double2><<<gp < kLoadBlocks ? gp : kLoadBlocks, 256, 0, st>>>((const double2 *)X, (const double2 *)F, (const double *)W, P, z, g, enc);
     FMM_TICK("load");
     fmm_choose_level<<<1, 1, 0, st>>>(enc, P, L);
     fmm_bin<<<gp, 256, 0, st>>>(z, P, enc, cell, cnt);
@@ -1297,9 +1380,9 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
     }
     const double pref = 1.0 / (4.0 * 3.14159265358979323846 * mu);
     if (prec == VN_F32)
-        fmm_finish<float2><<<(P + 127) / 128, 128, 0, st>>>(z, g, cell, P, (int)npts, enc, accum, pref, (float2 *)U);
+        fmm_finish<float2, true><<<(unsigned)(nves < 148 * 64 ? nves : 148 * 64), kFinThreads, 0, st>>>(z, g, cell, (int)nves, (int)npts, enc, accum, pref, (float2 *)U);
     else
-        fmm_finish<double2><<<(P + 127) / 128, 128, 0, st>>>(z, g, cell, P, (int)npts, enc, accum, pref, (double2 *)U);
+        fmm_finish<double2, false><<<(unsigned)(nves < 148 * 64 ? nves : 148 * 64), kFinThreads, 0, st>>>(z, g, cell, (int)nves, (int)npts, enc, accum, pref, (double2 *)U);
     count_launch(launches + 2);
     FMM_TICK("finish");
     const cudaError_t e = cudaGetLastError();
@@ -1315,27 +1398,17 @@ template <typename real2>
 __global__ void __launch_bounds__(256)
 fmm_load_targets(const real2 *__restrict__ Xt, int nt, cplx *__restrict__ zt, unsigned long long *__restrict__ enc)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
     double x = INFINITY, y = INFINITY, X1 = -INFINITY, Y1 = -INFINITY;
-    if (i < nt) {
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < nt; i += gridDim.x * blockDim.x) {
         const real2 p = Xt[i];
-        x = X1 = (double)p.x;
-        y = Y1 = (double)p.y;
-        zt[i] = make_double2(x, y);
+        const double px = (double)p.x, py = (double)p.y;
+        x = fmin(x, px);
+        y = fmin(y, py);
+        X1 = fmax(X1, px);
+        Y1 = fmax(Y1, py);
+        zt[i] = make_double2(px, py);
     }
-#pragma unroll
-    for (int m = 16; m >= 1; m >>= 1) {
-        x = fmin(x, __shfl_xor_sync(0xffffffffu, x, m));
-        y = fmin(y, __shfl_xor_sync(0xffffffffu, y, m));
-        X1 = fmax(X1, __shfl_xor_sync(0xffffffffu, X1, m));
-        Y1 = fmax(Y1, __shfl_xor_sync(0xffffffffu, Y1, m));
-    }
-    if ((threadIdx.x & 31) == 0 && x <= X1) {
-        atomicMin(enc + 0, enc_f64(x));
-        atomicMin(enc + 1, enc_f64(y));
-        atomicMax(enc + 2, enc_f64(X1));
-        atomicMax(enc + 3, enc_f64(Y1));
-    }
+    bounds_commit(x, y, X1, Y1, enc);
 }
 
 __global__ void __launch_bounds__(256)
@@ -1393,11 +1466,11 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
     fmm_init_bounds<<<1, 1, 0, st>>>(enc);
     const int gp = (P + 255) / 256, gt = (nt + 255) / 256;
     if (prec == VN_F32) {
-        fmm_load<float, float2><<<gp, 256, 0, st>>>((const float2 *)X, (const float2 *)F, (const float *)W, P, z, g, enc);
-        fmm_load_targets<float2><<<gt, 256, 0, st>>>((const float2 *)Xt, nt, zt, enc);
+        fmm_load<float, float2><<<gp < kLoadBlocks ? gp : kLoadBlocks, 256, 0, st>>>((const float2 *)X, (const float2 *)F, (const float *)W, P, z, g, enc);
+        fmm_load_targets<float2><<<gt < kLoadBlocks ? gt : kLoadBlocks, 256, 0, st>>>((const float2 *)Xt, nt, zt, enc);
     } else {
-        fmm_load<double, double2><<<gp, 256, 0, st>>>((const double2 *)X, (const double2 *)F, (const double *)W, P, z, g, enc);
-        fmm_load_targets<double2><<<gt, 256, 0, st>>>((const double2 *)Xt, nt, zt, enc);
+        fmm_load<double, double2><<<gp < kLoadBlocks ? gp : kLoadBlocks, 256, 0, st>>>((const double2 *)X, (const double2 *)F, (const double *)W, P, z, g, enc);
+        fmm_load_targets<double2><<<gt < kLoadBlocks ? gt : kLoadBlocks, 256, 0, st>>>((const double2 *)Xt, nt, zt, enc);
     }
     fmm_choose_level<<<1, 1, 0, st>>>(enc, P > nt ? P : nt, L);
     // sources into leaves
