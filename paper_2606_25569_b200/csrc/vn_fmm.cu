@@ -213,7 +213,7 @@ fmm_scatter(const int *__restrict__ cell, int P, long long *__restrict__ cursor,
 __global__ void __launch_bounds__(128)
 fmm_sort_cells(const long long *__restrict__ start, int ncell, const int *__restrict__ unsorted, int *__restrict__ perm)
 {
-    constexpr int kBuf = 256;                          // leaves up to this size are ranked out of shared memory
+    constexpr int kBuf = 256;                          // leaves up to this size are sorted in shared memory
     __shared__ int buf[4][kBuf];
     const int w = threadIdx.x >> 5, c = blockIdx.x * 4 + w, lane = threadIdx.x & 31;
     if (c >= ncell) return;
@@ -223,16 +223,24 @@ fmm_sort_cells(const long long *__restrict__ start, int ncell, const int *__rest
         if (m == 1 && lane == 0) perm[a] = unsorted[a];
         return;
     }
-    if (m <= kBuf) {
-        for (int i = lane; i < m; i += 32) buf[w][i] = unsorted[a + i];
+    if (m <= kBuf) {                                   // bitonic network in the warp's shared memory (indices are distinct)
+        int n2 = 2;
+        while (n2 < m) n2 <<= 1;
+        for (int i = lane; i < n2; i += 32) buf[w][i] = i < m ? unsorted[a + i] : 0x7fffffff;
         __syncwarp();
-        for (int i = lane; i < m; i += 32) {
-            const int v = buf[w][i];
-            int rank = 0;
-#pragma unroll 8
-            for (int j = 0; j < m; ++j) rank += buf[w][j] < v;
-            perm[a + rank] = v;
-        }
+        for (int k = 2; k <= n2; k <<= 1)
+            for (int j = k >> 1; j > 0; j >>= 1) {
+                for (int t = lane; t < (n2 >> 1); t += 32) {
+                    const int i = ((t & ~(j - 1)) << 1) | (t & (j - 1));      // lower index of pair t at distance j
+                    const int x = buf[w][i], y = buf[w][i + j];
+                    if ((x > y) == ((i & k) == 0)) {
+                        buf[w][i] = y;
+                        buf[w][i + j] = x;
+                    }
+                }
+                __syncwarp();
+            }
+        for (int i = lane; i < m; i += 32) perm[a + i] = buf[w][i];
         return;
     }
     for (long long i = a + lane; i < b; i += 32) {
@@ -444,13 +452,12 @@ fmm_p2m_half(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const lon
 }
 static size_t p2m_half_smem(int q) { return sizeof(cplx) * (size_t)(kP2MWarps * (32 * (q | 1) + 64)); }
 
-// M2M: parent moments from its four children, levels L-1 down to 2.  One WARP per parent box: the children's
-// moments are staged in the warp's shared memory with coalesced loads (one round trip to L2 instead of one per term),
-// then work item (k, h) -- output coefficient k, child pair h -- sums S(c; k, m) A_c[m] over m and the pair's two
-// children; 2 q items are dealt to the lanes (q = 15: 30 of 32 lanes busy), the table is read with the output
-// index fastest (coalesced, L1-resident), the children's coefficients are shared-memory broadcasts, and the two
-// pairs' partial sums meet through shared memory.
-constexpr int kShiftWarps = 4;
+// M2M: parent moments from its four children, levels L-1 down to 2.  One BLOCK per parent box (grid-stride): the
+// children's moments are staged in shared memory with coalesced loads (one round trip to L2 instead of one per term),
+// then thread (c, a, k) -- child c, expansion a, output coefficient k: 12 q work items -- sums S(c; k, m) A_c,a[m]
+// over m <= k, and q threads per expansion add the four children's parts.  The upper levels have a handful of boxes:
+// what counts there is how little one thread does in a row, not the instruction total.
+constexpr int kShiftThreads = 192;        // 12 q = 180 work items at q = 15
 constexpr int kShiftStageQ = 16;
 // dst[e] = src[e], e = first, first + stride, ... < count, with eight loads in flight per thread: written as
 // dst[e] = src[e] in a loop, every load waits for the previous store (the compiler cannot rule out aliasing), and
@@ -471,69 +478,59 @@ __device__ __forceinline__ void stage_cplx(cplx *dst, const cplx *src, int first
         }
     }
 }
-__global__ void __launch_bounds__(32 * kShiftWarps)
+__global__ void __launch_bounds__(kShiftThreads)
 fmm_m2m(int level, int q, const double *__restrict__ tab, const unsigned long long *__restrict__ enc,
         cplx *__restrict__ mult, int *__restrict__ boxcnt)
 {
     if (level >= load_level(enc)) return;
     extern __shared__ __align__(16) double sm[];
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    cplx *ch = (cplx *)sm + warp * (12 * q + 6 * q);               // [4][3][q] children | [2][3][q] the child pairs' partial sums
-    cplx *part = ch + 12 * q;
+    cplx *ch = (cplx *)sm;                                           // [4][3][q] children's moments
+    cplx *part = ch + 12 * q;                                        // [4][3][q] their contributions to the parent
+    __shared__ int scnt[4];
     const FmmTables t = fmm_tables_at(const_cast<double *>(tab), q);
     // the table: in shared memory up to kShiftStageQ (every launch starts with a cold L1: read through it, the
-    // 4 q loads of a work item would each wait for L2), straight from global memory above
+    // loads of a work item would each wait for L2), straight from global memory above
     const cplx *Stab = t.S;
     if (q <= kShiftStageQ) {
-        cplx *st = (cplx *)sm + kShiftWarps * 18 * q;
+        cplx *st = part + 12 * q;
         stage_cplx(st, t.S, threadIdx.x, blockDim.x, 4 * q * q);
         Stab = st;
-        __syncthreads();
     }
-    const int n = 1 << level;
-    for (int box = blockIdx.x * kShiftWarps + warp; box < n * n; box += gridDim.x * kShiftWarps) {
+    const int n = 1 << level, tid = threadIdx.x;
+    for (int box = blockIdx.x; box < n * n; box += gridDim.x) {
         const int ix = box / n, iy = box % n;
         const long long child0 = level_offset(level + 1) + (long long)(2 * ix) * (2 * n) + 2 * iy;
         // children c = 2 a + b sit at child0 + a * 2n + b
-        const int cc = lane < 4 ? boxcnt[child0 + (long long)(lane >> 1) * (2 * n) + (lane & 1)] : 0;
-        const unsigned have = __ballot_sync(0xffffffffu, cc != 0) & 0xfu;
-        int cnt = cc;
-        cnt += __shfl_xor_sync(0xffffffffu, cnt, 1);
-        cnt += __shfl_xor_sync(0xffffffffu, cnt, 2);
-        __syncwarp();                                               // the previous box's staging is consumed
-        for (int c = 0; c < 4; ++c)                                 // children without sources are skipped below, not staged
-            if ((have >> c) & 1u)
-                stage_cplx(ch + c * 3 * q, mult + (child0 + (long long)(c >> 1) * (2 * n) + (c & 1)) * (long long)(3 * q), lane, 32, 3 * q);
-        __syncwarp();
-        cplx *out = mult + (level_offset(level) + box) * (long long)(3 * q);
-        for (int w0 = 0; w0 < 2 * q; w0 += 32) {
-            const int w = w0 + lane;
-            const bool live = w < 2 * q;
-            const int h = live && w >= q ? 1 : 0, k = live ? w - h * q : 0;
-            cplx s1 = make_double2(0.0, 0.0), s2 = s1, s3 = s1;
-            for (int c = 2 * h; c < 2 * h + 2; ++c) {
-                if (!((have >> c) & 1u)) continue;
-                const cplx *A = ch + c * 3 * q;
+        __syncthreads();                                             // the previous box is written out
+        if (tid < 4) scnt[tid] = boxcnt[child0 + (long long)(tid >> 1) * (2 * n) + (tid & 1)];
+        __syncthreads();
+        for (int c = 0; c < 4; ++c)                                  // children without sources are skipped below, not staged
+            if (scnt[c] != 0)
+                stage_cplx(ch + c * 3 * q, mult + (child0 + (long long)(c >> 1) * (2 * n) + (c & 1)) * (long long)(3 * q), tid, kShiftThreads, 3 * q);
+        __syncthreads();
+        for (int w = tid; w < 12 * q; w += kShiftThreads) {
+            const int c = w / (3 * q), k = w % q;                    // w = (c * 3 + a) * q + k
+            cplx s0 = make_double2(0.0, 0.0), s1 = s0;               // two chains: even and odd m
+            if (scnt[c] != 0) {
+                const cplx *A = ch + (w - k);
                 const cplx *col = Stab + (size_t)c * q * q + k;
-#pragma unroll 4
-                for (int m = 0; m < q; ++m) {                       // entries with m > k are zero
-                    const cplx sm_ = col[(size_t)m * q];
-                    s1 = cfma(sm_, A[m], s1);
-                    s2 = cfma(sm_, A[q + m], s2);
-                    s3 = cfma(sm_, A[2 * q + m], s3);
+                int m = 0;
+                for (; m + 1 <= k; m += 2) {
+                    s0 = cfma(col[(size_t)m * q], A[m], s0);
+                    s1 = cfma(col[(size_t)(m + 1) * q], A[m + 1], s1);
                 }
+                if (m <= k) s0 = cfma(col[(size_t)m * q], A[m], s0);
             }
-            if (live) {
-                cplx *mine = part + h * 3 * q;
-                mine[k] = s1; mine[q + k] = s2; mine[2 * q + k] = s3;
-            }
+            part[w] = cadd(s0, s1);
         }
-        __syncwarp();
-        for (int e = lane; e < 3 * q; e += 32) out[e] = cadd(part[e], part[3 * q + e]);
-        if (lane == 0) boxcnt[level_offset(level) + box] = cnt;
+        __syncthreads();
+        cplx *out = mult + (level_offset(level) + box) * (long long)(3 * q);
+        for (int e = tid; e < 3 * q; e += kShiftThreads)
+            out[e] = cadd(cadd(part[e], part[3 * q + e]), cadd(part[6 * q + e], part[9 * q + e]));
+        if (tid == 0) boxcnt[level_offset(level) + box] = scnt[0] + scnt[1] + scnt[2] + scnt[3];
     }
 }
-static size_t shift_smem(int q) { return sizeof(cplx) * (size_t)(kShiftWarps * 18 * q + (q <= kShiftStageQ ? 4 * q * q : 0)); }
+static size_t shift_smem(int q) { return sizeof(cplx) * (size_t)(24 * q + (q <= kShiftStageQ ? 4 * q * q : 0)); }
 
 // ------------------------------------------------------------------------------------------------
 // M2L: one WARP per target box of `level` (four boxes per block), no block barrier inside the loop.  Lane `ln` owns
@@ -786,51 +783,47 @@ static size_t m2l_half_smem(int q)
            sizeof(int) * (size_t)(kM2LWarps * 32);
 }
 
-// L2L: child local expansions inherit the parent's; child level = `level`.  One WARP per PARENT box: the parent's
-// expansion is staged once for its four children, work item (c, k) -- child c, output coefficient k -- sums
-// T(c; k, m) par[m] over m >= k; 4 q items are dealt to the lanes.
-__global__ void __launch_bounds__(32 * kShiftWarps)
+// L2L: child local expansions inherit the parent's; child level = `level`.  One BLOCK per PARENT box (grid-stride):
+// the parent's expansion is staged once for its four children, thread (c, a, k) -- child c, expansion a, output
+// coefficient k -- adds sum_{m >= k} T(c; k, m) par_a[m] to the child's own M2L part.
+__global__ void __launch_bounds__(kShiftThreads)
 fmm_l2l(int level, int q, const double *__restrict__ tab, const unsigned long long *__restrict__ enc,
         const int *__restrict__ tboxcnt, cplx *__restrict__ loc)
 {
     if (level > load_level(enc)) return;
     extern __shared__ __align__(16) double sm[];
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    cplx *par = (cplx *)sm + warp * 3 * q;
+    cplx *par = (cplx *)sm;                                          // [3][q]
+    __shared__ int scnt[4];
     const FmmTables t = fmm_tables_at(const_cast<double *>(tab), q);
-    const cplx *Ttab = t.T;                                         // staged like the table of fmm_m2m
+    const cplx *Ttab = t.T;                                          // staged like the table of fmm_m2m
     if (q <= kShiftStageQ) {
-        cplx *st = (cplx *)sm + kShiftWarps * 18 * q;
+        cplx *st = par + 24 * q;
         stage_cplx(st, t.T, threadIdx.x, blockDim.x, 4 * q * q);
         Ttab = st;
-        __syncthreads();
     }
-    const int n = 1 << level, np = n >> 1;
-    for (int pbox = blockIdx.x * kShiftWarps + warp; pbox < np * np; pbox += gridDim.x * kShiftWarps) {
+    const int n = 1 << level, np = n >> 1, tid = threadIdx.x;
+    for (int pbox = blockIdx.x; pbox < np * np; pbox += gridDim.x) {
         if (tboxcnt && tboxcnt[level_offset(level - 1) + pbox] == 0) continue;   // no targets below the parent (see fmm_m2l)
         const int px = pbox / np, py = pbox % np;
         const long long child0 = level_offset(level) + (long long)(2 * px) * n + 2 * py;
-        const int tc = (lane < 4 && tboxcnt) ? tboxcnt[child0 + (long long)(lane >> 1) * n + (lane & 1)] : 1;
-        const unsigned have = __ballot_sync(0xffffffffu, tc != 0) & 0xfu;
-        __syncwarp();
-        stage_cplx(par, loc + (level_offset(level - 1) + pbox) * (long long)(3 * q), lane, 32, 3 * q);
-        __syncwarp();
-        for (int w = lane; w < 4 * q; w += 32) {
-            const int c = w / q, k = w - c * q;
-            if (!((have >> c) & 1u)) continue;
+        __syncthreads();
+        if (tid < 4) scnt[tid] = tboxcnt ? tboxcnt[child0 + (long long)(tid >> 1) * n + (tid & 1)] : 1;
+        stage_cplx(par, loc + (level_offset(level - 1) + pbox) * (long long)(3 * q), tid, kShiftThreads, 3 * q);
+        __syncthreads();
+        for (int w = tid; w < 12 * q; w += kShiftThreads) {
+            const int c = w / (3 * q), r = w - c * 3 * q, k = r % q;  // r = a * q + k
+            if (scnt[c] == 0) continue;
+            cplx *out = loc + (child0 + (long long)(c >> 1) * n + (c & 1)) * (long long)(3 * q) + r;
+            cplx s0 = *out, s1 = make_double2(0.0, 0.0);              // the child's own M2L part, in flight during the sum
+            const cplx *A = par + (r - k);
             const cplx *col = Ttab + (size_t)c * q * q + k;
-            cplx *out = loc + (child0 + (long long)(c >> 1) * n + (c & 1)) * (long long)(3 * q);
-            cplx s1 = out[k], s2 = out[q + k], s3 = out[2 * q + k];      // the child's own M2L part, in flight during the sum
-#pragma unroll 4
-            for (int m = k; m < q; ++m) {
-                const cplx tm = col[(size_t)m * q];
-                s1 = cfma(tm, par[m], s1);
-                s2 = cfma(tm, par[q + m], s2);
-                s3 = cfma(tm, par[2 * q + m], s3);
+            int m = k;
+            for (; m + 1 < q; m += 2) {
+                s0 = cfma(col[(size_t)m * q], A[m], s0);
+                s1 = cfma(col[(size_t)(m + 1) * q], A[m + 1], s1);
             }
-            out[k] = s1;
-            out[q + k] = s2;
-            out[2 * q + k] = s3;
+            if (m < q) s0 = cfma(col[(size_t)m * q], A[m], s0);
+            *out = cadd(s0, s1);
         }
     }
 }
@@ -1344,8 +1337,8 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
     ++launches;
     FMM_TICK("p2m");
     for (int l = L - 1; l >= 2; --l) {
-        const unsigned nb = ((1u << (2 * l)) + kShiftWarps - 1) / kShiftWarps;          // a warp per parent box
-        fmm_m2m<<<nb < 148u * 16u ? nb : 148u * 16u, 32 * kShiftWarps, shift_smem(q), st>>>(l, q, tab, enc, mult, boxcnt);
+        const unsigned nb = 1u << (2 * l);                                               // a block per parent box
+        fmm_m2m<<<nb < 148u * 4u ? nb : 148u * 4u, kShiftThreads, shift_smem(q), st>>>(l, q, tab, enc, mult, boxcnt);
         ++launches;
     }
     const size_t smem_m2l = sizeof(double) * (size_t)(((q * q + 1) & ~1) + 2 * kM2LWarps * 3 * (q + 1));
@@ -1363,8 +1356,8 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
     }
     FMM_TICK("m2l");
     for (int l = 3; l <= L; ++l) {
-        const unsigned nb = ((1u << (2 * (l - 1))) + kShiftWarps - 1) / kShiftWarps;    // a warp per parent box
-        fmm_l2l<<<nb < 148u * 16u ? nb : 148u * 16u, 32 * kShiftWarps, shift_smem(q), st>>>(l, q, tab, enc, boxcnt, loc);
+        const unsigned nb = 1u << (2 * (l - 1));                                         // a block per parent box
+        fmm_l2l<<<nb < 148u * 4u ? nb : 148u * 4u, kShiftThreads, shift_smem(q), st>>>(l, q, tab, enc, boxcnt, loc);
         ++launches;
     }
     FMM_TICK("l2l");
@@ -1501,8 +1494,8 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
         fmm_p2m<<<(ncell + 3) / 4, 128, 0, st>>>(zs, gs, start, q, enc, mult, boxcnt);
     ++launches;
     for (int l = L - 1; l >= 2; --l) {
-        const unsigned nb = ((1u << (2 * l)) + kShiftWarps - 1) / kShiftWarps;          // a warp per parent box
-        fmm_m2m<<<nb < 148u * 16u ? nb : 148u * 16u, 32 * kShiftWarps, shift_smem(q), st>>>(l, q, tab, enc, mult, boxcnt);
+        const unsigned nb = 1u << (2 * l);                                               // a block per parent box
+        fmm_m2m<<<nb < 148u * 4u ? nb : 148u * 4u, kShiftThreads, shift_smem(q), st>>>(l, q, tab, enc, mult, boxcnt);
         ++launches;
     }
     const size_t smem_m2l = sizeof(double) * (size_t)(((q * q + 1) & ~1) + 2 * kM2LWarps * 3 * (q + 1));
@@ -1518,8 +1511,8 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
         }
     }
     for (int l = 3; l <= L; ++l) {
-        const unsigned nb = ((1u << (2 * (l - 1))) + kShiftWarps - 1) / kShiftWarps;    // a warp per parent box
-        fmm_l2l<<<nb < 148u * 16u ? nb : 148u * 16u, 32 * kShiftWarps, shift_smem(q), st>>>(l, q, tab, enc, nullptr, loc);
+        const unsigned nb = 1u << (2 * (l - 1));                                         // a block per parent box
+        fmm_l2l<<<nb < 148u * 4u ? nb : 148u * 4u, kShiftThreads, shift_smem(q), st>>>(l, q, tab, enc, nullptr, loc);
         ++launches;
     }
     if (prec == VN_F32)
