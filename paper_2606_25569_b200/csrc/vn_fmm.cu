@@ -78,20 +78,25 @@ __device__ __forceinline__ cplx box_centre(const Geom &g, int level, int ix, int
     return make_double2(fma((double)ix + 0.5, s, g.x0), fma((double)iy + 0.5, s, g.y0));
 }
 
-__global__ void fmm_init_bounds(unsigned long long *enc)
-{
-    enc[0] = enc[1] = ~0ull;
-    enc[2] = enc[3] = 0ull;
-}
-
+// enc[0..3] while the bounding box is being collected: ~enc(xmin), ~enc(ymin), enc(xmax), enc(ymax), all four
+// growing under atomicMax from ZERO, so that the one memset that clears the counters initialises them too;
+// enc[8] counts the blocks of the load kernels that have committed their box.  fmm_choose_level (run by the last of
+// those blocks) turns them into the final form: plain encodings relative to the centre of the root square.
 // Depth of the tree, chosen ON THE DEVICE once the bounding box is known (no host synchronisation): leaves of
 // about kLeafTarget points, where the points are assumed to fill the bounding RECTANGLE evenly, i.e. a
 // fraction 1/aspect of the root square (a 4:1 channel leaves three quarters of the leaves empty).  The host
 // sizes scratch and grids for L_hi (two levels deeper than a full square needs); kernels of unused levels
 // and leaves return at once.  enc[4] holds the level.
 constexpr double kLeafTarget = 64.0;
-__global__ void fmm_choose_level(unsigned long long *enc, int P, int L_hi)
+__device__ void fmm_choose_level(volatile unsigned long long *enc, int P, int L_hi)
 {
+    if (enc[2] == 0ull) {                               // no finite point at all: an empty box, as before
+        enc[0] = ~0ull;
+        enc[1] = ~0ull;
+    } else {
+        enc[0] = ~enc[0];
+        enc[1] = ~enc[1];
+    }
     const double ex = dec_f64(enc[2]) - dec_f64(enc[0]), ey = dec_f64(enc[3]) - dec_f64(enc[1]);
     const double lo = fmin(ex, ey), hi = fmax(ex, ey);
     double occ = (hi > 0.0 && lo > 0.0) ? lo / hi : 1.0;
@@ -115,15 +120,18 @@ __global__ void fmm_choose_level(unsigned long long *enc, int P, int L_hi)
         enc[2] = enc_f64(x1 - cx);
         enc[3] = enc_f64(y1 - cy);
     } else {
-        enc[5] = enc[6] = 0ull;
+        enc[5] = 0ull;
+        enc[6] = 0ull;
     }
 }
 __device__ __forceinline__ int load_level(const unsigned long long *__restrict__ enc) { return (int)enc[4]; }
 
 // bounding box of a block's points: per-thread extremes -> warp shuffles -> shared memory -> FOUR atomics per block
 // (one set per warp was 128 K serialised 64-bit atomics on four addresses at a million points: 80 of the kernel's 96 us)
-__device__ __forceinline__ void bounds_commit(double x, double y, double X1, double Y1, unsigned long long *__restrict__ enc)
-{
+__device__ __forceinline__ void bounds_commit(double x, double y, double X1, double Y1, unsigned long long *enc,
+                                              unsigned tickets, int P_level, int L_hi)
+{   // tickets: blocks of ALL load kernels of the call (sources, and targets where they are a separate set); the block
+    // that draws the last one knows the whole box and fixes level and centre (no launch of its own for that)
     __shared__ double red[4][32];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = (blockDim.x + 31) >> 5;
 #pragma unroll
@@ -147,11 +155,17 @@ __device__ __forceinline__ void bounds_commit(double x, double y, double X1, dou
         X1 = fmax(X1, __shfl_xor_sync(0xffffffffu, X1, m));
         Y1 = fmax(Y1, __shfl_xor_sync(0xffffffffu, Y1, m));
     }
-    if (lane == 0 && x <= X1) {
-        atomicMin(enc + 0, enc_f64(x));
-        atomicMin(enc + 1, enc_f64(y));
+    if (lane != 0) return;
+    if (x <= X1) {
+        atomicMax(enc + 0, ~enc_f64(x));
+        atomicMax(enc + 1, ~enc_f64(y));
         atomicMax(enc + 2, enc_f64(X1));
         atomicMax(enc + 3, enc_f64(Y1));
+    }
+    __threadfence();
+    if (atomicAdd(enc + 8, 1ull) == (unsigned long long)tickets - 1ull) {
+        __threadfence();
+        fmm_choose_level(enc, P_level, L_hi);
     }
 }
 constexpr int kLoadBlocks = 148 * 8;      // grid-stride: at most this many blocks commit a bounding box
@@ -160,7 +174,7 @@ constexpr int kLoadBlocks = 148 * 8;      // grid-stride: at most this many bloc
 template <typename real, typename real2>
 __global__ void __launch_bounds__(256)
 fmm_load(const real2 *__restrict__ X, const real2 *__restrict__ F, const real *__restrict__ W, int P,
-         cplx *__restrict__ z, cplx *__restrict__ g, unsigned long long *__restrict__ enc)
+         cplx *__restrict__ z, cplx *__restrict__ g, unsigned long long *enc, unsigned tickets, int P_level, int L_hi)
 {
     double x = INFINITY, y = INFINITY, X1 = -INFINITY, Y1 = -INFINITY;
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < P; i += gridDim.x * blockDim.x) {
@@ -175,7 +189,7 @@ fmm_load(const real2 *__restrict__ X, const real2 *__restrict__ F, const real *_
         z[i] = make_double2(px, py);
         g[i] = make_double2((double)(f.x * w), (double)(f.y * w));   // product in the storage precision, as in the exact path
     }
-    bounds_commit(x, y, X1, Y1, enc);
+    bounds_commit(x, y, X1, Y1, enc, tickets, P_level, L_hi);
 }
 
 // moves every point into the root square's frame (in place, see Geom), then: leaf box of every point and the
@@ -271,6 +285,7 @@ fmm_gather(const int *__restrict__ perm, int P, int npts, const cplx *__restrict
 //   both stored [c][m][k], the OUTPUT index fastest: the lanes of a warp own consecutive k and read consecutive words
 //   rho[t][n]  = tau_t^-n, n = 0 .. q;  lrho[t] = log(1/tau_t)  (complex, 49 offsets tau = dx + i dy, |dx|,|dy| <= 3)
 // delta_c = ((a - 1/2) + i (b - 1/2)) / 2 is the child's centre in the parent's scaled variable, c = 2 a + b.
+constexpr int kTableBlocks = 64;
 struct FmmTables {
     double *Cb;
     cplx *S, *T, *rho, *lrho;
@@ -299,10 +314,15 @@ __device__ __forceinline__ cplx cpowi(cplx a, int n)
     for (int i = 0; i < n; ++i) r = cmul(r, a);
     return r;
 }
-__global__ void fmm_build_tables(int q, double *base)
-{
+__global__ void fmm_build_tables(int q, double *base, double *logtab)
+{   // blocks beyond kTableBlocks (launched only when logtab is wanted: double-precision storage) build the two tables
+    // of log_rcp_f64 in global memory, which every block of the direct part copies to its shared memory
+    if (blockIdx.x >= kTableBlocks) {
+        build_log_tables(logtab, (blockIdx.x - kTableBlocks) * blockDim.x + threadIdx.x, (gridDim.x - kTableBlocks) * blockDim.x);
+        return;
+    }
     const FmmTables t = fmm_tables_at(base, q);
-    const int nthreads = gridDim.x * blockDim.x, tid = blockIdx.x * blockDim.x + threadIdx.x;
+    const int nthreads = kTableBlocks * blockDim.x, tid = blockIdx.x * blockDim.x + threadIdx.x;
     for (int e = tid; e < q * q; e += nthreads) {
         const int n = e / q, l = e % q;
         t.Cb[e] = binom(n + l, l);
@@ -649,7 +669,10 @@ fmm_m2l(int level, int q, const double *__restrict__ tab, const unsigned long lo
 // one's arithmetic), and the two halves' sums meet in one shuffle at the end.  Same formulas as fmm_m2l; the order in
 // which the sources are added differs (fixed, so the result is still reproducible run to run).
 constexpr int kM2LHalfQ = 16;
-__global__ void __launch_bounds__(32 * kM2LWarps)
+#ifndef VN_FMM_M2L_MINBLK
+#define VN_FMM_M2L_MINBLK 4
+#endif
+__global__ void __launch_bounds__(32 * kM2LWarps, VN_FMM_M2L_MINBLK)
 fmm_m2l_half(int q, const double *__restrict__ tab, const unsigned long long *__restrict__ enc,
              const cplx *__restrict__ mult, const int *__restrict__ boxcnt, const int *__restrict__ tboxcnt,
              cplx *__restrict__ loc)
@@ -826,12 +849,6 @@ fmm_l2l(int level, int q, const double *__restrict__ tab, const unsigned long lo
             *out = cadd(s0, s1);
         }
     }
-}
-
-// the two tables of log_rcp_f64 in global memory (built once per call, copied to shared memory by every block)
-__global__ void fmm_build_logtab(double *tab)
-{
-    build_log_tables(tab, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -1297,23 +1314,21 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
     cplx *accum = (cplx *)take(b_pt);
     int *cell = (int *)take(b_int), *perm = (int *)take(b_int), *vs = (int *)take(b_int);
     cplx *mult = (cplx *)take(b_exp), *loc = (cplx *)take(b_exp);
+    unsigned long long *enc = (unsigned long long *)take(256);
     int *boxcnt = (int *)take(b_cnt), *cnt = (int *)take(b_leaf);
     long long *start = (long long *)take(b_start), *cursor = (long long *)take(b_start), *bsum = (long long *)take(b_bs);
     double *tab = (double *)take(b_tab), *logtab = (double *)take(b_log);
-    unsigned long long *enc = (unsigned long long *)take(256);
 
 #ifdef VN_FMM_TIMING
     FmmTimer fmm_timer(st);
 #endif
-    VN_CUDA(cudaMemsetAsync(boxcnt, 0, b_cnt + b_leaf, st));      // boxcnt and the leaf counts are adjacent
-    fmm_init_bounds<<<1, 1, 0, st>>>(enc);
-    const int gp = (P + 255) / 256;
-    if (prec == VN_F32)
-        fmm_load<float, float2><<<gp < kLoadBlocks ? gp : kLoadBlocks, 256, 0, st>>>((const float2 *)X, (const float2 *)F, (const float *)W, P, z, g, enc);
+    VN_CUDA(cudaMemsetAsync(enc, 0, 256 + b_cnt + b_leaf, st));   // the bounding box, boxcnt and the leaf counts are adjacent
+    const int gp = (P + 255) / 256, gl = gp < kLoadBlocks ? gp : kLoadBlocks;
+    if (prec == VN_F32)                                            // the last block to finish also fixes level and centre
+        fmm_load<float, float2><<<gl, 256, 0, st>>>((const float2 *)X, (const float2 *)F, (const float *)W, P, z, g, enc, gl, P, L);
     else
-        fmm_load<double, double2><<<gp < kLoadBlocks ? gp : kLoadBlocks, 256, 0, st>>>((const double2 *)X, (const double2 *)F, (const double *)W, P, z, g, enc);
+        fmm_load<double, double2><<<gl, 256, 0, st>>>((const double2 *)X, (const double2 *)F, (const double *)W, P, z, g, enc, gl, P, L);
     FMM_TICK("load");
-    fmm_choose_level<<<1, 1, 0, st>>>(enc, P, L);
     fmm_bin<<<gp, 256, 0, st>>>(z, P, enc, cell, cnt);
     scan_block_sums<<<nb_scan, kScanThreads, 0, st>>>(cnt, ncell, bsum);
     scan_of_sums<<<1, kScanThreads, 0, st>>>(bsum, nb_scan);
@@ -1323,9 +1338,8 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
     fmm_sort_cells<<<(ncell + 3) / 4, 128, 0, st>>>(start, ncell, vs, perm);
     fmm_gather<<<gp, 256, 0, st>>>(perm, P, (int)npts, z, g, zs, gs, vs);
     FMM_TICK("sort+gather");
-    fmm_build_tables<<<64, 128, 0, st>>>(q, tab);
-    fmm_build_logtab<<<8, 128, 0, st>>>(logtab);
-    int launches = 13;
+    fmm_build_tables<<<kTableBlocks + (prec == VN_F32 ? 0 : 8), 128, 0, st>>>(q, tab, logtab);   // log tables: double only
+    int launches = 10;
 
     const int p2p_grid = ncell < 148 * 64 ? ncell : 148 * 64;      // grid-stride over the leaves the device chose
     FMM_TICK("tables");
@@ -1389,7 +1403,8 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
 // leaf's local expansions plus the direct sum over the 3 x 3 neighbour leaves.  No vesicle is excluded.
 template <typename real2>
 __global__ void __launch_bounds__(256)
-fmm_load_targets(const real2 *__restrict__ Xt, int nt, cplx *__restrict__ zt, unsigned long long *__restrict__ enc)
+fmm_load_targets(const real2 *__restrict__ Xt, int nt, cplx *__restrict__ zt, unsigned long long *enc, unsigned tickets,
+                 int P_level, int L_hi)
 {
     double x = INFINITY, y = INFINITY, X1 = -INFINITY, Y1 = -INFINITY;
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < nt; i += gridDim.x * blockDim.x) {
@@ -1401,7 +1416,7 @@ fmm_load_targets(const real2 *__restrict__ Xt, int nt, cplx *__restrict__ zt, un
         Y1 = fmax(Y1, py);
         zt[i] = make_double2(px, py);
     }
-    bounds_commit(x, y, X1, Y1, enc);
+    bounds_commit(x, y, X1, Y1, enc, tickets, P_level, L_hi);
 }
 
 __global__ void __launch_bounds__(256)
@@ -1449,23 +1464,24 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
     cplx *zt = (cplx *)take(b_tpt), *zts = (cplx *)take(b_tpt), *accum = (cplx *)take(b_tpt);
     int *tcell = (int *)take(b_tint), *tperm = (int *)take(b_tint);
     cplx *mult = (cplx *)take(b_exp), *loc = (cplx *)take(b_exp);
+    unsigned long long *enc = (unsigned long long *)take(256);
     int *boxcnt = (int *)take(b_cnt), *cnt = (int *)take(b_ccnt), *tcnt = (int *)take(b_ccnt);
     long long *start = (long long *)take(b_start), *cursor = (long long *)take(b_start);
     long long *tstart = (long long *)take(b_start), *tcursor = (long long *)take(b_start), *bsum = (long long *)take(b_bs);
     double *tab = (double *)take(b_tab), *logtab = (double *)take(b_log);
-    unsigned long long *enc = (unsigned long long *)take(256);
 
-    VN_CUDA(cudaMemsetAsync(boxcnt, 0, b_cnt + 2 * b_ccnt, st));   // boxcnt, cnt and tcnt are adjacent
-    fmm_init_bounds<<<1, 1, 0, st>>>(enc);
+    VN_CUDA(cudaMemsetAsync(enc, 0, 256 + b_cnt + 2 * b_ccnt, st));   // the bounding box, boxcnt, cnt and tcnt are adjacent
     const int gp = (P + 255) / 256, gt = (nt + 255) / 256;
+    const int gl = gp < kLoadBlocks ? gp : kLoadBlocks, glt = gt < kLoadBlocks ? gt : kLoadBlocks;
+    const int Plev = P > nt ? P : nt;
+    // sources and targets share one box: the last block of the two kernels together fixes level and centre
     if (prec == VN_F32) {
-        fmm_load<float, float2><<<gp < kLoadBlocks ? gp : kLoadBlocks, 256, 0, st>>>((const float2 *)X, (const float2 *)F, (const float *)W, P, z, g, enc);
-        fmm_load_targets<float2><<<gt < kLoadBlocks ? gt : kLoadBlocks, 256, 0, st>>>((const float2 *)Xt, nt, zt, enc);
+        fmm_load<float, float2><<<gl, 256, 0, st>>>((const float2 *)X, (const float2 *)F, (const float *)W, P, z, g, enc, gl + glt, Plev, L);
+        fmm_load_targets<float2><<<glt, 256, 0, st>>>((const float2 *)Xt, nt, zt, enc, gl + glt, Plev, L);
     } else {
-        fmm_load<double, double2><<<gp < kLoadBlocks ? gp : kLoadBlocks, 256, 0, st>>>((const double2 *)X, (const double2 *)F, (const double *)W, P, z, g, enc);
-        fmm_load_targets<double2><<<gt < kLoadBlocks ? gt : kLoadBlocks, 256, 0, st>>>((const double2 *)Xt, nt, zt, enc);
+        fmm_load<double, double2><<<gl, 256, 0, st>>>((const double2 *)X, (const double2 *)F, (const double *)W, P, z, g, enc, gl + glt, Plev, L);
+        fmm_load_targets<double2><<<glt, 256, 0, st>>>((const double2 *)Xt, nt, zt, enc, gl + glt, Plev, L);
     }
-    fmm_choose_level<<<1, 1, 0, st>>>(enc, P > nt ? P : nt, L);
     // sources into leaves
     fmm_bin<<<gp, 256, 0, st>>>(z, P, enc, cell, cnt);
     scan_block_sums<<<nb_scan, kScanThreads, 0, st>>>(cnt, ncell, bsum);
@@ -1482,9 +1498,8 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
     fmm_scatter<<<gt, 256, 0, st>>>(tcell, nt, tcursor, (int *)accum);     // accum doubles as the unsorted buffer
     fmm_sort_cells<<<(ncell + 3) / 4, 128, 0, st>>>(tstart, ncell, (const int *)accum, tperm);
     fmm_gather_targets<<<gt, 256, 0, st>>>(tperm, nt, zt, zts);
-    fmm_build_tables<<<64, 128, 0, st>>>(q, tab);
-    fmm_build_logtab<<<8, 128, 0, st>>>(logtab);
-    int launches = 21;
+    fmm_build_tables<<<kTableBlocks + (prec == VN_F32 ? 0 : 8), 128, 0, st>>>(q, tab, logtab);   // log tables: double only
+    int launches = 18;
 
     const int p2p_grid = ncell < 148 * 64 ? ncell : 148 * 64;      // grid-stride over the leaves the device chose
     profile_mark(st, true);
