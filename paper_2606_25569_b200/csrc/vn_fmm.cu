@@ -482,6 +482,8 @@ constexpr int kShiftStageQ = 16;
 // dst[e] = src[e], e = first, first + stride, ... < count, with eight loads in flight per thread: written as
 // dst[e] = src[e] in a loop, every load waits for the previous store (the compiler cannot rule out aliasing), and
 // the kernels of the small upper levels are nothing but such latencies in a row
+// (loads go to L2, not through L1: the multi-level launches read what other blocks wrote earlier in the same launch)
+__device__ __forceinline__ cplx ldcg_cplx(const cplx *p) { return __ldcg(p); }
 __device__ __forceinline__ void stage_cplx(cplx *dst, const cplx *src, int first, int stride, int count)
 {
     for (int e0 = first; e0 < count; e0 += 8 * stride) {
@@ -489,7 +491,7 @@ __device__ __forceinline__ void stage_cplx(cplx *dst, const cplx *src, int first
 #pragma unroll
         for (int i = 0; i < 8; ++i) {
             const int e = e0 + i * stride;
-            if (e < count) tmp[i] = src[e];
+            if (e < count) tmp[i] = ldcg_cplx(src + e);
         }
 #pragma unroll
         for (int i = 0; i < 8; ++i) {
@@ -498,16 +500,32 @@ __device__ __forceinline__ void stage_cplx(cplx *dst, const cplx *src, int first
         }
     }
 }
-__global__ void __launch_bounds__(kShiftThreads)
-fmm_m2m(int level, int q, const double *__restrict__ tab, const unsigned long long *__restrict__ enc,
-        cplx *__restrict__ mult, int *__restrict__ boxcnt)
+// Several levels in ONE launch: the levels below the top two have a few hundred boxes at most, a launch each is mostly
+// launch latency.  All blocks of the grid meet at a counter between two levels; the host sizes such a grid so that
+// every block is resident (occupancy query), otherwise the blocks that spin would wait for blocks that cannot start.
+__device__ __forceinline__ void grid_barrier(unsigned long long *counter, unsigned long long target)
 {
-    if (level >= load_level(enc)) return;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        atomicAdd(counter, 1ull);
+        while (*(volatile unsigned long long *)counter < target) { }
+        __threadfence();
+    }
+    __syncthreads();
+}
+// levels L - d_first, L - d_first - 1, ..., max(L - d_last, 2)  (L = the tree's depth, chosen on the device)
+__global__ void __launch_bounds__(kShiftThreads)
+fmm_m2m(int d_first, int d_last, int q, const double *__restrict__ tab, unsigned long long *enc,
+        cplx *mult, int *boxcnt)
+{
+    const int L = load_level(enc);
     extern __shared__ __align__(16) double sm[];
     cplx *ch = (cplx *)sm;                                           // [4][3][q] children's moments
     cplx *part = ch + 12 * q;                                        // [4][3][q] their contributions to the parent
     __shared__ int scnt[4];
     const FmmTables t = fmm_tables_at(const_cast<double *>(tab), q);
+    if (L - d_first < 2) return;                                     // nothing to do (uniform over the grid)
     // the table: in shared memory up to kShiftStageQ (every launch starts with a cold L1: read through it, the
     // loads of a work item would each wait for L2), straight from global memory above
     const cplx *Stab = t.S;
@@ -516,13 +534,17 @@ fmm_m2m(int level, int q, const double *__restrict__ tab, const unsigned long lo
         stage_cplx(st, t.S, threadIdx.x, blockDim.x, 4 * q * q);
         Stab = st;
     }
-    const int n = 1 << level, tid = threadIdx.x;
+    const int tid = threadIdx.x;
+    unsigned long long arrivals = 0;
+    for (int level = L - d_first; level >= 2 && level >= L - d_last; --level) {
+    if (level != L - d_first) grid_barrier(enc + 9, arrivals += gridDim.x);   // the level below is complete
+    const int n = 1 << level;
     for (int box = blockIdx.x; box < n * n; box += gridDim.x) {
         const int ix = box / n, iy = box % n;
         const long long child0 = level_offset(level + 1) + (long long)(2 * ix) * (2 * n) + 2 * iy;
         // children c = 2 a + b sit at child0 + a * 2n + b
         __syncthreads();                                             // the previous box is written out
-        if (tid < 4) scnt[tid] = boxcnt[child0 + (long long)(tid >> 1) * (2 * n) + (tid & 1)];
+        if (tid < 4) scnt[tid] = __ldcg(boxcnt + child0 + (long long)(tid >> 1) * (2 * n) + (tid & 1));
         __syncthreads();
         for (int c = 0; c < 4; ++c)                                  // children without sources are skipped below, not staged
             if (scnt[c] != 0)
@@ -549,6 +571,30 @@ fmm_m2m(int level, int q, const double *__restrict__ tab, const unsigned long lo
             out[e] = cadd(cadd(part[e], part[3 * q + e]), cadd(part[6 * q + e], part[9 * q + e]));
         if (tid == 0) boxcnt[level_offset(level) + box] = scnt[0] + scnt[1] + scnt[2] + scnt[3];
     }
+    }   // levels
+}
+static size_t shift_smem(int q);
+__global__ void fmm_l2l(int d_hi, int d_lo, int q, const double *__restrict__ tab, unsigned long long *enc,
+                        const int *__restrict__ tboxcnt, cplx *loc);
+// blocks of the multi-level launches of fmm_m2m / fmm_l2l: all resident at once (see grid_barrier), at most two per SM
+static int shift_resident_blocks(int q)
+{
+    static int q_dev[kMaxDevices] = {0}, blocks_dev[kMaxDevices] = {0};
+    const int d = current_device();
+    if (q_dev[d] != q || blocks_dev[d] == 0) {
+        int dev = 0, sms = 0, o1 = 0, o2 = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess ||
+            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o1, fmm_m2m, kShiftThreads, shift_smem(q)) != cudaSuccess ||
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o2, fmm_l2l, kShiftThreads, shift_smem(q)) != cudaSuccess) {
+            (void)cudaGetLastError();
+            return 1;                                  // a single block needs nobody else to be resident
+        }
+        const int occ = o1 < o2 ? o1 : o2;
+        blocks_dev[d] = occ < 1 ? 1 : sms * (occ < 2 ? occ : 2);
+        q_dev[d] = q;
+    }
+    return blocks_dev[d];
 }
 static size_t shift_smem(int q) { return sizeof(cplx) * (size_t)(24 * q + (q <= kShiftStageQ ? 4 * q * q : 0)); }
 
@@ -809,11 +855,14 @@ static size_t m2l_half_smem(int q)
 // L2L: child local expansions inherit the parent's; child level = `level`.  One BLOCK per PARENT box (grid-stride):
 // the parent's expansion is staged once for its four children, thread (c, a, k) -- child c, expansion a, output
 // coefficient k -- adds sum_{m >= k} T(c; k, m) par_a[m] to the child's own M2L part.
+// child levels max(3, L - d_hi), ..., L - d_lo  top-down, a grid barrier between two of them
 __global__ void __launch_bounds__(kShiftThreads)
-fmm_l2l(int level, int q, const double *__restrict__ tab, const unsigned long long *__restrict__ enc,
-        const int *__restrict__ tboxcnt, cplx *__restrict__ loc)
+fmm_l2l(int d_hi, int d_lo, int q, const double *__restrict__ tab, unsigned long long *enc,
+        const int *__restrict__ tboxcnt, cplx *loc)
 {
-    if (level > load_level(enc)) return;
+    const int L = load_level(enc);
+    const int l_first = max(3, L - d_hi), l_end = L - d_lo;
+    if (l_first > l_end) return;
     extern __shared__ __align__(16) double sm[];
     cplx *par = (cplx *)sm;                                          // [3][q]
     __shared__ int scnt[4];
@@ -824,7 +873,11 @@ fmm_l2l(int level, int q, const double *__restrict__ tab, const unsigned long lo
         stage_cplx(st, t.T, threadIdx.x, blockDim.x, 4 * q * q);
         Ttab = st;
     }
-    const int n = 1 << level, np = n >> 1, tid = threadIdx.x;
+    const int tid = threadIdx.x;
+    unsigned long long arrivals = 0;
+    for (int level = l_first; level <= l_end; ++level) {
+    if (level != l_first) grid_barrier(enc + 10, arrivals += gridDim.x);      // the level above is complete
+    const int n = 1 << level, np = n >> 1;
     for (int pbox = blockIdx.x; pbox < np * np; pbox += gridDim.x) {
         if (tboxcnt && tboxcnt[level_offset(level - 1) + pbox] == 0) continue;   // no targets below the parent (see fmm_m2l)
         const int px = pbox / np, py = pbox % np;
@@ -837,7 +890,7 @@ fmm_l2l(int level, int q, const double *__restrict__ tab, const unsigned long lo
             const int c = w / (3 * q), r = w - c * 3 * q, k = r % q;  // r = a * q + k
             if (scnt[c] == 0) continue;
             cplx *out = loc + (child0 + (long long)(c >> 1) * n + (c & 1)) * (long long)(3 * q) + r;
-            cplx s0 = *out, s1 = make_double2(0.0, 0.0);              // the child's own M2L part, in flight during the sum
+            cplx s0 = ldcg_cplx(out), s1 = make_double2(0.0, 0.0);    // the child's own M2L part, in flight during the sum
             const cplx *A = par + (r - k);
             const cplx *col = Ttab + (size_t)c * q * q + k;
             int m = k;
@@ -849,6 +902,7 @@ fmm_l2l(int level, int q, const double *__restrict__ tab, const unsigned long lo
             *out = cadd(s0, s1);
         }
     }
+    }   // levels
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -1350,10 +1404,14 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
         fmm_p2m<<<(ncell + 3) / 4, 128, 0, st>>>(zs, gs, start, q, enc, mult, boxcnt);
     ++launches;
     FMM_TICK("p2m");
-    for (int l = L - 1; l >= 2; --l) {
-        const unsigned nb = 1u << (2 * l);                                               // a block per parent box
-        fmm_m2m<<<nb < 148u * 4u ? nb : 148u * 4u, kShiftThreads, shift_smem(q), st>>>(l, q, tab, enc, mult, boxcnt);
+    if (L >= 3) {     // the level above the leaves with a full grid, all levels above it in one launch of resident blocks
+        const unsigned nb = 1u << (2 * (L - 1));
+        fmm_m2m<<<nb < 148u * 4u ? nb : 148u * 4u, kShiftThreads, shift_smem(q), st>>>(1, 1, q, tab, enc, mult, boxcnt);
         ++launches;
+        if (L >= 4) {
+            fmm_m2m<<<shift_resident_blocks(q), kShiftThreads, shift_smem(q), st>>>(2, 99, q, tab, enc, mult, boxcnt);
+            ++launches;
+        }
     }
     const size_t smem_m2l = sizeof(double) * (size_t)(((q * q + 1) & ~1) + 2 * kM2LWarps * 3 * (q + 1));
     FMM_TICK("m2m");
@@ -1369,9 +1427,13 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
         }
     }
     FMM_TICK("m2l");
-    for (int l = 3; l <= L; ++l) {
-        const unsigned nb = 1u << (2 * (l - 1));                                         // a block per parent box
-        fmm_l2l<<<nb < 148u * 4u ? nb : 148u * 4u, kShiftThreads, shift_smem(q), st>>>(l, q, tab, enc, boxcnt, loc);
+    if (L >= 3) {     // levels 3 .. L - 1 in one launch of resident blocks, the leaf level with a full grid
+        if (L >= 4) {
+            fmm_l2l<<<shift_resident_blocks(q), kShiftThreads, shift_smem(q), st>>>(99, 1, q, tab, enc, boxcnt, loc);
+            ++launches;
+        }
+        const unsigned nb = 1u << (2 * (L - 1));
+        fmm_l2l<<<nb < 148u * 4u ? nb : 148u * 4u, kShiftThreads, shift_smem(q), st>>>(0, 0, q, tab, enc, boxcnt, loc);
         ++launches;
     }
     FMM_TICK("l2l");
@@ -1508,10 +1570,14 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
     else
         fmm_p2m<<<(ncell + 3) / 4, 128, 0, st>>>(zs, gs, start, q, enc, mult, boxcnt);
     ++launches;
-    for (int l = L - 1; l >= 2; --l) {
-        const unsigned nb = 1u << (2 * l);                                               // a block per parent box
-        fmm_m2m<<<nb < 148u * 4u ? nb : 148u * 4u, kShiftThreads, shift_smem(q), st>>>(l, q, tab, enc, mult, boxcnt);
+    if (L >= 3) {     // the level above the leaves with a full grid, all levels above it in one launch of resident blocks
+        const unsigned nb = 1u << (2 * (L - 1));
+        fmm_m2m<<<nb < 148u * 4u ? nb : 148u * 4u, kShiftThreads, shift_smem(q), st>>>(1, 1, q, tab, enc, mult, boxcnt);
         ++launches;
+        if (L >= 4) {
+            fmm_m2m<<<shift_resident_blocks(q), kShiftThreads, shift_smem(q), st>>>(2, 99, q, tab, enc, mult, boxcnt);
+            ++launches;
+        }
     }
     const size_t smem_m2l = sizeof(double) * (size_t)(((q * q + 1) & ~1) + 2 * kM2LWarps * 3 * (q + 1));
     if (q <= kM2LHalfQ) {              // all levels in one launch
@@ -1525,9 +1591,13 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
             ++launches;
         }
     }
-    for (int l = 3; l <= L; ++l) {
-        const unsigned nb = 1u << (2 * (l - 1));                                         // a block per parent box
-        fmm_l2l<<<nb < 148u * 4u ? nb : 148u * 4u, kShiftThreads, shift_smem(q), st>>>(l, q, tab, enc, nullptr, loc);
+    if (L >= 3) {     // levels 3 .. L - 1 in one launch of resident blocks, the leaf level with a full grid
+        if (L >= 4) {
+            fmm_l2l<<<shift_resident_blocks(q), kShiftThreads, shift_smem(q), st>>>(99, 1, q, tab, enc, nullptr, loc);
+            ++launches;
+        }
+        const unsigned nb = 1u << (2 * (L - 1));
+        fmm_l2l<<<nb < 148u * 4u ? nb : 148u * 4u, kShiftThreads, shift_smem(q), st>>>(0, 0, q, tab, enc, nullptr, loc);
         ++launches;
     }
     if (prec == VN_F32)
