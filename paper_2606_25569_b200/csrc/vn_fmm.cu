@@ -286,13 +286,16 @@ fmm_gather(const int *__restrict__ perm, int P, int npts, const cplx *__restrict
 //   T(c; k, m) = 2^-k C(m, k) delta_c^(m-k)   (m >= k, else 0)  (complex, 4 x q x q)   -- L2L, parent -> child c, output k
 //   both stored [c][m][k], the OUTPUT index fastest: the lanes of a warp own consecutive k and read consecutive words
 //   rho[t][n]  = tau_t^-n, n = 0 .. q;  lrho[t] = log(1/tau_t)  (complex, 49 offsets tau = dx + i dy, |dx|,|dy| <= 3)
+//   coef[t][5][q]: the per-offset factors of fmm_m2l_half, one load each instead of a few operations per source:
+//     [0][k] = rho^k / k (k >= 1), 1 (k = 0)   [1][k] = rho^k        (scaling of the source's moments)
+//     [2][l] = -(-1)^l rho^l (l >= 1), -1 (l = 0)      [3][l] = [2][l] / l (l >= 1), -lrho (l = 0)      [4][l] = (-1)^l rho^(l+1)
 // delta_c = ((a - 1/2) + i (b - 1/2)) / 2 is the child's centre in the parent's scaled variable, c = 2 a + b.
 constexpr int kTableBlocks = 64;
 struct FmmTables {
     double *Cb;
-    cplx *S, *T, *rho, *lrho;
+    cplx *S, *T, *rho, *lrho, *coef;
 };
-__host__ __device__ inline size_t fmm_tables_doubles(int q) { return (((size_t)q * q + 1) & ~(size_t)1) + 2 * (size_t)(8 * q * q) + 2 * (size_t)(49 * (q + 1)) + 2 * 49; }
+__host__ __device__ inline size_t fmm_tables_doubles(int q) { return (((size_t)q * q + 1) & ~(size_t)1) + 2 * (size_t)(8 * q * q) + 2 * (size_t)(49 * (q + 1)) + 2 * 49 + 2 * (size_t)(49 * 5 * q); }
 __host__ __device__ inline FmmTables fmm_tables_at(double *base, int q)
 {
     FmmTables t;
@@ -301,6 +304,7 @@ __host__ __device__ inline FmmTables fmm_tables_at(double *base, int q)
     t.T = t.S + 4 * q * q;
     t.rho = t.T + 4 * q * q;
     t.lrho = t.rho + 49 * (q + 1);
+    t.coef = t.lrho + 49;
     return t;
 }
 __device__ __forceinline__ double binom(int n, int l)
@@ -344,10 +348,19 @@ __global__ void fmm_build_tables(int q, double *base, double *logtab)
         cplx r = make_double2(0.0, 0.0);
         if (tau.x != 0.0 || tau.y != 0.0) r = cpowi(crcp(tau), n);
         t.rho[e] = r;
-        if (n == 0) {
-            cplx lr = make_double2(0.0, 0.0);
-            if (tau.x != 0.0 || tau.y != 0.0) lr = make_double2(-0.5 * log(tau.x * tau.x + tau.y * tau.y), -atan2(tau.y, tau.x));
-            t.lrho[o] = lr;
+        cplx lr = make_double2(0.0, 0.0);
+        if (tau.x != 0.0 || tau.y != 0.0) lr = make_double2(-0.5 * log(tau.x * tau.x + tau.y * tau.y), -atan2(tau.y, tau.x));
+        if (n == 0) t.lrho[o] = lr;
+        if (n < q) {
+            const double sg = (n & 1) ? -1.0 : 1.0, in = n > 0 ? 1.0 / (double)n : 0.0;
+            cplx rn1 = make_double2(0.0, 0.0);                      // rho^(n+1)
+            if (tau.x != 0.0 || tau.y != 0.0) rn1 = cmul(r, crcp(tau));
+            cplx *c = t.coef + (size_t)o * 5 * q;
+            c[0 * q + n] = n > 0 ? cscale(r, in) : make_double2(1.0, 0.0);
+            c[1 * q + n] = r;
+            c[2 * q + n] = n > 0 ? cscale(r, -sg) : make_double2(-1.0, 0.0);
+            c[3 * q + n] = n > 0 ? cscale(r, -sg * in) : make_double2(-lr.x, -lr.y);
+            c[4 * q + n] = cscale(rn1, sg);
         }
     }
 }
@@ -739,7 +752,7 @@ fmm_m2l_half(int q, const double *__restrict__ tab, const unsigned long long *__
     const Geom gm = load_geom(enc);
     const double log_size = log(gm.size);
     const bool v = l < q;
-    const double sgn = (l & 1) ? -1.0 : 1.0, il = l > 0 ? 1.0 / (double)l : 0.0;
+    const int lv = v ? l : 0;                                        // lanes beyond q compute column 0 and store nothing
     // the boxes of ALL levels 2 .. L in one launch, deepest level first (M2L of a level needs the multipoles only, not
     // the other levels' local expansions; L2L adds the parents' afterwards): the small upper levels overlap with the
     // tail of the deepest one instead of costing a launch each
@@ -776,42 +789,43 @@ fmm_m2l_half(int q, const double *__restrict__ tab, const unsigned long long *__
         }
         __syncwarp();
         cplx acc0 = make_double2(0.0, 0.0), acc1 = acc0, acc2 = acc0;
-        // moments of the half's next source (coefficient l of the three expansions) and its offset
-        cplx a0, a1, a2;
-        int o;
+        cplx sumA1 = acc0, sumA2 = acc0;                               // zeroth moments of the half's sources, for the l = 0 terms
+        // the half's next source: coefficient l of its three expansions and the two factors that scale them
+        cplx a0, a1, a2, cpre, cpreB;
+        const cplx *cf;
         auto fetch = [&](int idx) {
             a0 = a1 = a2 = make_double2(0.0, 0.0);
-            o = 24;                                                    // tau = 0: rho = lrho = 0, an absent source adds nothing
+            int o = 24;                                                // tau = 0: all factors 0 or harmless, an absent source adds nothing
+            const cplx *A = Mlev;
             if (idx < nlist) {
                 const int entry = list[idx];
                 o = entry >> 24;
-                if (v) {
-                    const cplx *A = Mlev + (long long)(entry & 0xffffff) * (3 * q);
-                    a0 = A[l];
-                    a1 = A[q + l];
-                    a2 = A[2 * q + l];
-                }
+                A = Mlev + (long long)(entry & 0xffffff) * (3 * q);
             }
+            cf = t.coef + (size_t)o * 5 * q + lv;
+            if (v && idx < nlist) {
+                a0 = A[l];
+                a1 = A[q + l];
+                a2 = A[2 * q + l];
+            }
+            cpre = __ldg(cf);
+            cpreB = __ldg(cf + q);
         };
         fetch(half);
         for (int i = 0; i < nlist; i += 2) {
-            const cplx *rho = t.rho + (size_t)o * (q + 1);
-            const int o_now = o;
             __syncwarp();                                             // the previous pair's hat is consumed
             if (v) {
-                const cplx r = __ldg(&rho[l]);
-                cplx h0 = cmul(a0, r), h1 = cmul(a1, r);
-                if (l >= 1) { h0 = cscale(h0, il); h1 = cscale(h1, il); }
-                hat[l] = h0;
-                hat[(q + 1) + l] = h1;
-                hat[2 * (q + 1) + l] = cmul(a2, r);
+                hat[l] = cmul(a0, cpre);                               // Ahat1_k = A1_k rho^k / k
+                hat[(q + 1) + l] = cmul(a1, cpre);
+                hat[2 * (q + 1) + l] = cmul(a2, cpreB);                // Bhat_k = B_k rho^k
             }
+            const cplx cS = __ldg(cf + 2 * q), cA = __ldg(cf + 3 * q), c2 = __ldg(cf + 4 * q);   // used after the loop below
             fetch(i + 2 + half);                                      // in flight during the loop below
             __syncwarp();
             const cplx A10 = hat[0], A20 = hat[q + 1];                // rho^0 = 1: the raw zeroth moments
             cplx S0 = make_double2(0.0, 0.0), S1 = S0, S2 = S0;
             const cplx *h0p = hat + 1, *h1p = hat + (q + 1) + 1, *h2p = hat + 2 * (q + 1);   // log arrays read k + 1
-            const double *Cl = Cb + (v ? l : 0);
+            const double *Cl = Cb + lv;
 #pragma unroll 5
             for (int k = 0; k < q; ++k) {
                 const double c0 = Cl[k * q];
@@ -820,21 +834,19 @@ fmm_m2l_half(int q, const double *__restrict__ tab, const unsigned long long *__
                 S1.x = fma(c0, e1.x, S1.x); S1.y = fma(c0, e1.y, S1.y);
                 S2.x = fma(c0, e2.x, S2.x); S2.y = fma(c0, e2.y, S2.y);
             }
-            if (v) {
-                if (l == 0) {
-                    const cplx lr = t.lrho[o_now];
-                    acc0 = cadd(acc0, make_double2(A10.x * (log_s - lr.x) + A10.y * lr.y - S0.x,
-                                                   -A10.x * lr.y + A10.y * (log_s - lr.x) - S0.y));
-                    acc1 = cadd(acc1, make_double2(A20.x * (log_s - lr.x) + A20.y * lr.y - S1.x,
-                                                   -A20.x * lr.y + A20.y * (log_s - lr.x) - S1.y));
-                    acc2 = cadd(acc2, make_double2(-(A10.x - A20.y), A10.y + A20.x));       // -conj(A1_0 + i A2_0)
-                } else {
-                    const cplx rl = cscale(__ldg(&rho[l]), -sgn);
-                    acc0 = cfma(rl, cadd(cscale(A10, il), S0), acc0);
-                    acc1 = cfma(rl, cadd(cscale(A20, il), S1), acc1);
-                }
-                acc2 = cfma(cscale(__ldg(&rho[l + 1]), sgn * inv_s), S2, acc2);
-            }
+            // b_l += cS (A_0 / l + S) for l >= 1, b_0 += A_0 (log s - log rho) - S: cA = cS / l resp. -log rho, the log s
+            // part and the -conj(A1_0 + i A2_0) of d_0 follow from the sums of the zeroth moments once per box
+            acc0 = cfma(cS, S0, cfma(cA, A10, acc0));
+            acc1 = cfma(cS, S1, cfma(cA, A20, acc1));
+            acc2 = cfma(c2, S2, acc2);
+            sumA1 = cadd(sumA1, A10);
+            sumA2 = cadd(sumA2, A20);
+        }
+        {
+            const double z0 = l == 0 ? 1.0 : 0.0;                     // the l = 0 terms, without a branch
+            acc0 = make_double2(fma(z0 * log_s, sumA1.x, acc0.x), fma(z0 * log_s, sumA1.y, acc0.y));
+            acc1 = make_double2(fma(z0 * log_s, sumA2.x, acc1.x), fma(z0 * log_s, sumA2.y, acc1.y));
+            acc2 = make_double2(fma(acc2.x, inv_s, -z0 * (sumA1.x - sumA2.y)), fma(acc2.y, inv_s, z0 * (sumA1.y + sumA2.x)));
         }
         // the two halves' sums
         acc0.x += __shfl_xor_sync(0xffffffffu, acc0.x, 16); acc0.y += __shfl_xor_sync(0xffffffffu, acc0.y, 16);
