@@ -225,18 +225,22 @@ fmm_scatter(const int *__restrict__ cell, int P, long long *__restrict__ cursor,
 // every later sum runs in a fixed order (bitwise reproducible results).  One warp per leaf, rank sort: the
 // indices of a segment are distinct, so the rank of an entry is the number of smaller ones.
 __global__ void __launch_bounds__(128)
-fmm_sort_cells(const long long *__restrict__ start, int ncell, const int *__restrict__ unsorted, int *__restrict__ perm)
-{
+fmm_sort_cells(const long long *__restrict__ start, const unsigned long long *__restrict__ enc,
+               const int *__restrict__ unsorted, int *__restrict__ perm)
+{   // the leaves of the level the device chose, walked with a grid stride: a grid sized for the deepest admissible
+    // tree is mostly blocks without a leaf (61 K of 65 K at a million points), and scheduling those cost 40 us
     constexpr int kBuf = 256;                          // leaves up to this size are sorted in shared memory
     __shared__ int buf[4][kBuf];
-    const int w = threadIdx.x >> 5, c = blockIdx.x * 4 + w, lane = threadIdx.x & 31;
-    if (c >= ncell) return;
+    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int ncell = 1 << (2 * load_level(enc));
+    for (int c = blockIdx.x * 4 + w; c < ncell; c += gridDim.x * 4) {
     const long long a = start[c], b = start[c + 1];
     const int m = (int)(b - a);
     if (m <= 1) {
         if (m == 1 && lane == 0) perm[a] = unsorted[a];
-        return;
+        continue;
     }
+    __syncwarp();                                      // the previous leaf's buffer is written out
     if (m <= kBuf) {                                   // bitonic network in the warp's shared memory (indices are distinct)
         int n2 = 2;
         while (n2 < m) n2 <<= 1;
@@ -255,7 +259,7 @@ fmm_sort_cells(const long long *__restrict__ start, int ncell, const int *__rest
                 __syncwarp();
             }
         for (int i = lane; i < m; i += 32) perm[a + i] = buf[w][i];
-        return;
+        continue;
     }
     for (long long i = a + lane; i < b; i += 32) {
         const int v = unsorted[i];
@@ -263,6 +267,7 @@ fmm_sort_cells(const long long *__restrict__ start, int ncell, const int *__rest
         for (long long j = a; j < b; ++j) rank += unsorted[j] < v;
         perm[a + rank] = v;
     }
+    }   // leaves
 }
 
 __global__ void __launch_bounds__(256)
@@ -1262,17 +1267,45 @@ fmm_finish(const cplx *__restrict__ z, const cplx *__restrict__ g, const int *__
 {
     __shared__ cplx sz[kFinChunk], sg[kFinChunk];
     __shared__ int sc[kFinChunk];
+    __shared__ int box[4];                              // leaf bounding box of the vesicle: min ix, min iy, max ix, max iy
     const int L = load_level(enc);
     const int n = 1 << L, tid = threadIdx.x;
     for (int ves = blockIdx.x; ves < nves; ves += gridDim.x) {
         const long long v0 = (long long)ves * npts;
+        // a point has something to take out only if some point of its vesicle lies two or more leaves away: most
+        // vesicles fit in 2 x 2 leaves, and in a wider one only the points of the outer leaves qualify
+        __syncthreads();
+        if (tid < 2) box[tid] = n;
+        else if (tid < 4) box[tid] = -1;
+        __syncthreads();
+        {
+            int x0 = n, y0 = n, x1 = -1, y1 = -1;
+            for (int e = tid; e < npts; e += kFinThreads) {
+                const int cj = cell[v0 + e], jx = cj >> L, jy = cj & (n - 1);
+                x0 = min(x0, jx); y0 = min(y0, jy); x1 = max(x1, jx); y1 = max(y1, jy);
+            }
+#pragma unroll
+            for (int m = 16; m >= 1; m >>= 1) {
+                x0 = min(x0, __shfl_xor_sync(0xffffffffu, x0, m));
+                y0 = min(y0, __shfl_xor_sync(0xffffffffu, y0, m));
+                x1 = max(x1, __shfl_xor_sync(0xffffffffu, x1, m));
+                y1 = max(y1, __shfl_xor_sync(0xffffffffu, y1, m));
+            }
+            if ((tid & 31) == 0) {
+                atomicMin(&box[0], x0); atomicMin(&box[1], y0); atomicMax(&box[2], x1); atomicMax(&box[3], y1);
+            }
+        }
+        __syncthreads();
+        const int bx0 = box[0], by0 = box[1], bx1 = box[2], by1 = box[3];
+        const bool compact = bx1 - bx0 <= 1 && by1 - by0 <= 1;      // every pair of its points is a neighbour pair
         for (int t0 = 0; t0 < npts; t0 += kFinThreads) {
             const bool live = t0 + tid < npts;
             const long long i = v0 + (live ? t0 + tid : 0);
             const cplx zi = z[i];
             const int ci = cell[i], ix = ci >> L, iy = ci & (n - 1);
+            const bool mine = live && (ix - bx0 > 1 || bx1 - ix > 1 || iy - by0 > 1 || by1 - iy > 1);
             double cx = 0.0, cy = 0.0;
-            for (int s0 = 0; s0 < npts; s0 += kFinChunk) {
+            for (int s0 = 0; s0 < npts && !compact; s0 += kFinChunk) {
                 const int cnt = min(kFinChunk, npts - s0);
                 __syncthreads();
                 for (int e = tid; e < cnt; e += kFinThreads) {
@@ -1281,7 +1314,7 @@ fmm_finish(const cplx *__restrict__ z, const cplx *__restrict__ g, const int *__
                     sc[e] = cell[v0 + s0 + e];
                 }
                 __syncthreads();
-                if (!live) continue;
+                if (!mine) continue;
                 float fx = 0.f, fy = 0.f;
                 for (int j = 0; j < cnt; ++j) {
                     const int cj = sc[j];
@@ -1407,7 +1440,7 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
     scan_apply<<<nb_scan, kScanThreads, 0, st>>>(cnt, ncell, bsum, start, cursor);
     FMM_TICK("bin+scan");
     fmm_scatter<<<gp, 256, 0, st>>>(cell, P, cursor, vs);                  // vs doubles as the unsorted buffer
-    fmm_sort_cells<<<(ncell + 3) / 4, 128, 0, st>>>(start, ncell, vs, perm);
+    fmm_sort_cells<<<(ncell + 3) / 4 < 148 * 16 ? (ncell + 3) / 4 : 148 * 16, 128, 0, st>>>(start, enc, vs, perm);
     fmm_gather<<<gp, 256, 0, st>>>(perm, P, (int)npts, z, g, zs, gs, vs, prec == VN_F32 ? srcf : nullptr);
     FMM_TICK("sort+gather");
     fmm_build_tables<<<kTableBlocks + (prec == VN_F32 ? 0 : 8), 128, 0, st>>>(q, tab, logtab);   // log tables: double only
@@ -1569,7 +1602,7 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
     scan_of_sums<<<1, kScanThreads, 0, st>>>(bsum, nb_scan);
     scan_apply<<<nb_scan, kScanThreads, 0, st>>>(cnt, ncell, bsum, start, cursor);
     fmm_scatter<<<gp, 256, 0, st>>>(cell, P, cursor, vs);                  // vs doubles as the unsorted buffer
-    fmm_sort_cells<<<(ncell + 3) / 4, 128, 0, st>>>(start, ncell, vs, perm);
+    fmm_sort_cells<<<(ncell + 3) / 4 < 148 * 16 ? (ncell + 3) / 4 : 148 * 16, 128, 0, st>>>(start, enc, vs, perm);
     fmm_gather<<<gp, 256, 0, st>>>(perm, P, (int)npts, z, g, zs, gs, vs, prec == VN_F32 ? srcf : nullptr);
     // targets into the same leaves
     fmm_bin<<<gt, 256, 0, st>>>(zt, nt, enc, tcell, tcnt);
@@ -1577,7 +1610,7 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
     scan_of_sums<<<1, kScanThreads, 0, st>>>(bsum, nb_scan);
     scan_apply<<<nb_scan, kScanThreads, 0, st>>>(tcnt, ncell, bsum, tstart, tcursor);
     fmm_scatter<<<gt, 256, 0, st>>>(tcell, nt, tcursor, (int *)accum);     // accum doubles as the unsorted buffer
-    fmm_sort_cells<<<(ncell + 3) / 4, 128, 0, st>>>(tstart, ncell, (const int *)accum, tperm);
+    fmm_sort_cells<<<(ncell + 3) / 4 < 148 * 16 ? (ncell + 3) / 4 : 148 * 16, 128, 0, st>>>(tstart, enc, (const int *)accum, tperm);
     fmm_gather_targets<<<gt, 256, 0, st>>>(tperm, nt, zt, zts);
     fmm_build_tables<<<kTableBlocks + (prec == VN_F32 ? 0 : 8), 128, 0, st>>>(q, tab, logtab);   // log tables: double only
     int launches = 18;
