@@ -499,6 +499,10 @@ static size_t p2m_half_smem(int q) { return sizeof(cplx) * (size_t)(kP2MWarps * 
 // what counts there is how little one thread does in a row, not the instruction total.
 constexpr int kShiftThreads = 192;        // 12 q = 180 work items at q = 15
 constexpr int kShiftStageQ = 16;
+#ifndef VN_FMM_SHIFT_WAVE
+#define VN_FMM_SHIFT_WAVE 4
+#endif
+constexpr unsigned kShiftWave = VN_FMM_SHIFT_WAVE;   // blocks per SM of the single-level launches (grid-stride over the boxes)
 // dst[e] = src[e], e = first, first + stride, ... < count, with eight loads in flight per thread: written as
 // dst[e] = src[e] in a loop, every load waits for the previous store (the compiler cannot rule out aliasing), and
 // the kernels of the small upper levels are nothing but such latencies in a row
@@ -1457,7 +1461,7 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
     FMM_TICK("p2m");
     if (L >= 3) {     // the level above the leaves with a full grid, all levels above it in one launch of resident blocks
         const unsigned nb = 1u << (2 * (L - 1));
-        fmm_m2m<<<nb < 148u * 4u ? nb : 148u * 4u, kShiftThreads, shift_smem(q), st>>>(1, 1, q, tab, enc, mult, boxcnt);
+        fmm_m2m<<<nb < 148u * kShiftWave ? nb : 148u * kShiftWave, kShiftThreads, shift_smem(q), st>>>(1, 1, q, tab, enc, mult, boxcnt);
         ++launches;
         if (L >= 4) {
             fmm_m2m<<<shift_resident_blocks(q), kShiftThreads, shift_smem(q), st>>>(2, 99, q, tab, enc, mult, boxcnt);
@@ -1484,7 +1488,7 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
             ++launches;
         }
         const unsigned nb = 1u << (2 * (L - 1));
-        fmm_l2l<<<nb < 148u * 4u ? nb : 148u * 4u, kShiftThreads, shift_smem(q), st>>>(0, 0, q, tab, enc, boxcnt, loc);
+        fmm_l2l<<<nb < 148u * kShiftWave ? nb : 148u * kShiftWave, kShiftThreads, shift_smem(q), st>>>(0, 0, q, tab, enc, boxcnt, loc);
         ++launches;
     }
     FMM_TICK("l2l");
@@ -1624,7 +1628,7 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
     ++launches;
     if (L >= 3) {     // the level above the leaves with a full grid, all levels above it in one launch of resident blocks
         const unsigned nb = 1u << (2 * (L - 1));
-        fmm_m2m<<<nb < 148u * 4u ? nb : 148u * 4u, kShiftThreads, shift_smem(q), st>>>(1, 1, q, tab, enc, mult, boxcnt);
+        fmm_m2m<<<nb < 148u * kShiftWave ? nb : 148u * kShiftWave, kShiftThreads, shift_smem(q), st>>>(1, 1, q, tab, enc, mult, boxcnt);
         ++launches;
         if (L >= 4) {
             fmm_m2m<<<shift_resident_blocks(q), kShiftThreads, shift_smem(q), st>>>(2, 99, q, tab, enc, mult, boxcnt);
@@ -1649,7 +1653,7 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
             ++launches;
         }
         const unsigned nb = 1u << (2 * (L - 1));
-        fmm_l2l<<<nb < 148u * 4u ? nb : 148u * 4u, kShiftThreads, shift_smem(q), st>>>(0, 0, q, tab, enc, nullptr, loc);
+        fmm_l2l<<<nb < 148u * kShiftWave ? nb : 148u * kShiftWave, kShiftThreads, shift_smem(q), st>>>(0, 0, q, tab, enc, nullptr, loc);
         ++launches;
     }
     if (prec == VN_F32)

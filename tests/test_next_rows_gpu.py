@@ -496,6 +496,40 @@ def test_fmm_edge_shapes(nves, npts):
     check(got, ref, 1e-11, f"fmm edge shape {nves} x {npts}", c_max=FMM_C)
 
 
+@pytest.mark.parametrize("order", [14, 15])
+@pytest.mark.parametrize("nves,npts", [(2, 1), (3, 2), (7, 3), (5, 33), (3, 129), (37, 128), (11, 1000), (1030, 1), (3, 2049), (300, 64)])
+def test_fmm_edge_shapes_single_precision(nves, npts, order):
+    """The kernels only the fp32 calls run (packed direct part, half-warp P2M / M2L: q = order + 1 <= 16) on the same
+    ragged shapes, at the default order and at the largest order of that path (q = 16: every lane of a half-warp
+    carries a coefficient).  A structural test -- an indexing fault gives errors of order one --, so the bound is
+    the fp32 tolerance times 5: random clouds put points of different vesicles closer than a suspension does."""
+    rng = np.random.Generator(np.random.PCG64(1000 * nves + npts))
+    X = rng.normal(size=(nves, npts, 2)) * 0.3 + 4.0 * rng.normal(size=(nves, 1, 2))
+    F = rng.normal(size=(nves, npts, 2))
+    W = rng.uniform(0.5, 1.5, size=(nves, npts))
+    ref = oracle.farfield(stored(X, np.float32), stored(F, np.float32), stored(W, np.float32), 0.7)
+    got = vn.vn_farfield_fmm(dev(X, np.float32), dev(F, np.float32), dev(W, np.float32), 0.7, order)
+    torch.cuda.synchronize()
+    check(got.cpu().numpy(), ref, 5 * TOL[np.float32], f"fmm fp32 edge shape {nves} x {npts} p={order}", c_max=FMM_C)
+
+
+def test_fmm_orders_across_the_kernel_switch_single_precision():
+    """Orders 13 .. 18 at config 1 in fp32: q = order + 1 <= 16 runs the half-warp kernels, above that the general ones;
+    all of them must sit at the fp32 bar against the exact fp32 path, and low orders must be visibly worse."""
+    s = inputs.config(1)
+    W = oracle.weights(s.X)
+    Xd, Fd, Wd = dev(s.X, np.float32), dev(s.F, np.float32), dev(W, np.float32)
+    exact = vn.vn_farfield(Xd, Fd, Wd, s.mu).cpu().numpy()
+    errs = {}
+    for order in (2, 6, 13, 14, 15, 16, 17, 18):
+        got = vn.vn_farfield_fmm(Xd, Fd, Wd, s.mu, order)
+        torch.cuda.synchronize()
+        errs[order] = rel_l2(got.cpu().numpy(), exact)
+    print("fmm fp32 vs exact fp32 path, config1:", " ".join(f"p={o}: {e:.2e}" for o, e in errs.items()))
+    assert errs[2] > errs[6] > errs[13] and errs[2] > 1e-3
+    assert all(errs[o] <= TOL[np.float32] for o in (14, 15, 16, 17, 18))
+
+
 def test_fmm_single_vesicle_gives_zero():
     rng = np.random.Generator(np.random.PCG64(5))
     X = rng.normal(size=(1, 700, 2)); F = rng.normal(size=(1, 700, 2)); W = rng.uniform(0.5, 1.5, size=(1, 700))
