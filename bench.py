@@ -21,8 +21,9 @@ integer reduce-scatter sums the fixed-point accumulators, vn_farfield_finish rou
 Total work is fixed: "scaling": "strong".  The result is bit for bit the single-GPU result.
 
 The default invocation (N = 1, configs[4], fp32) also measures, in the same run, the issue rates of
-the FP32 / SFU / FP64 pipes (vn_pipe_peaks -> roofline.peak_measured) and a `sweep` over the other
-configurations north_star's target names (configs[3] fp32 and fp64, configs[1] fp32).
+the FP32 / SFU / FP64 pipes (vn_pipe_peaks -> roofline.peak_measured), a `sweep` over the other
+configurations north_star's target names (configs[3] fp32 and fp64, configs[1] fp32), and `next_rows`: the fast
+multipole evaluation of the same sum (row f-4b) at configs[4] and configs[3].
 
 One JSON line is printed by rank 0.
 """
@@ -332,6 +333,9 @@ def traffic_from_profiles(workload, precision, path):
     return None, None
 
 
+_SUSPENSIONS = {}          # workload index -> generated suspension (the default run measures several paths on configs[4])
+
+
 def measure(ctx, m):
     """One workload / precision / path through the device-timed and (optionally) the host-buffer legs.
     ctx: torch, vn, multi, rank, world, local_rank, flush;  m: workload, precision, path, steps, warmup, order, graph, e2e.
@@ -341,7 +345,7 @@ def measure(ctx, m):
     rank, world = ctx.rank, ctx.world
     tdtype = torch.float32 if m.precision == "f32" else torch.float64
     np_dtype = np.float32 if m.precision == "f32" else np.float64
-    susp = inputs.config(m.workload)                   # every rank generates the same suspension (same seed)
+    susp = _SUSPENSIONS.get(m.workload) or _SUSPENSIONS.setdefault(m.workload, inputs.config(m.workload))   # same seed on every rank
     seq_np = susp.X_sequence if susp.X_sequence else [susp.X]
     evals = len(seq_np)
     P = susp.nves * susp.npts
@@ -604,6 +608,19 @@ def main():
                           "frac": rl["frac"], "frac_vs_measured_peak": rl["frac_vs_measured_peak"],
                           "frac_executed": rl["frac_executed"], "clocks": rs.clocks, "gpu_launches": rs.launches})
 
+    next_rows = []
+    if default_run and not args.no_sweep:              # row f-4b in the same run: the O(P) evaluation of the same sum
+        for w, steps in ((4, 3), (3, 10)):
+            ms = SimpleNamespace(workload=w, precision="f32", path="fmm", steps=steps, warmup=3, order=0,
+                                 graph=False, e2e=False)
+            rs = measure(ctx, ms)
+            evals = len(rs.susp.X_sequence) if rs.susp.X_sequence else 1
+            next_rows.append({"row": "f-4b vn_farfield_fmm (approximate, O(P))", "workload": f"BASELINE.json configs[{w}]: {rs.susp.name}",
+                              "precision": "f32", "order": rs.fmm_order, "steps": steps, "ms_per_step": rs.ms_per_step,
+                              "evaluations_per_step": evals, "ms_per_evaluation": rs.ms_per_step / evals,
+                              "equivalent_value": rs.value, "unit": UNIT + " (the direct sum's pair count over this time)",
+                              "clocks": rs.clocks, "gpu_launches": rs.launches})
+
     if rank == 0:
         line = {"metric": METRIC, "value": r.value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": r.warm, "ms_per_step": r.ms_per_step, "higher_is_better": True,
@@ -640,6 +657,8 @@ def main():
                           "instruction roofline is claimed; see profiles/ for the FP64-pipe occupancy of its dominant kernels")
         if sweep:
             line["sweep"] = sweep
+        if next_rows:
+            line["next_rows"] = next_rows
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(r.susp, np_dtype, args.path)
         print(json.dumps(line), flush=True)

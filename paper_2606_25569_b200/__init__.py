@@ -117,9 +117,33 @@ def _check_dev(name, t, shape=None, dtype=None):
 
 
 def _stream_ptr(stream):
+    """cudaStream_t of `stream`, or of torch's current stream on the current device (the bindings make the tensors'
+    device current first).  The raw-handle query costs 0.3 us where building a torch.cuda.Stream object costs 3."""
     import torch
-    s = torch.cuda.current_stream() if stream is None else stream
-    return ctypes.c_void_p(s.cuda_stream)
+    if stream is not None:
+        return ctypes.c_void_p(stream.cuda_stream)
+    raw = getattr(torch._C, "_cuda_getCurrentRawStream", None)
+    if raw is not None:
+        return ctypes.c_void_p(raw(torch.cuda.current_device()))
+    return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+class _NoGuard:
+    def __enter__(self):
+        return None
+
+    def __exit__(self, *exc):
+        return False
+
+
+_NO_GUARD = _NoGuard()
+
+
+def _on(device):
+    """Context that makes `device` current for the call -- nothing at all when it already is (every call of a
+    single-GPU process; torch.cuda.device() costs 3 us to enter and leave, a tenth of a small problem's step)."""
+    import torch
+    return _NO_GUARD if device.index == torch.cuda.current_device() else torch.cuda.device(device)
 
 
 def vn_farfield(X, F, W, mu: float = 1.0, out=None, stream=None):
@@ -134,7 +158,7 @@ def vn_farfield(X, F, W, mu: float = 1.0, out=None, stream=None):
     if out is None:
         out = torch.empty_like(X)
     _check_dev("out", out, X.shape, X.dtype)
-    with torch.cuda.device(X.device):
+    with _on(X.device):
         rc = lib().vn_farfield(X.data_ptr(), F.data_ptr(), W.data_ptr(), nves, npts, float(mu),
                                out.data_ptr(), _prec(X), _stream_ptr(stream))
     if rc != VN_OK:
@@ -159,7 +183,7 @@ def vn_farfield_noalloc_f32(X, F, W, out, mu: float = 1.0, stream=None):
     _check_dev("F", F, X.shape, torch.float32)
     _check_dev("W", W, (nves, npts), torch.float32)
     _check_dev("out", out, X.shape, torch.float32)
-    with torch.cuda.device(X.device):
+    with _on(X.device):
         rc = lib().vn_farfield_noalloc_f32(X.data_ptr(), F.data_ptr(), W.data_ptr(), nves, npts, float(mu),
                                            out.data_ptr(), _stream_ptr(stream))
     if rc != VN_OK:
@@ -190,7 +214,7 @@ def vn_farfield_partial(X, F, W, part: int, nparts: int, acc=None, gmax=None, st
         gmax = torch.empty(1, dtype=torch.int64, device=X.device)
     _check_dev("acc", acc, (n,), torch.int64)
     _check_dev("gmax", gmax, (1,), torch.int64)
-    with torch.cuda.device(X.device):
+    with _on(X.device):
         rc = lib().vn_farfield_partial(X.data_ptr(), F.data_ptr(), W.data_ptr(), nves, npts, int(part), int(nparts),
                                        acc.data_ptr(), gmax.data_ptr(), _prec(X), _stream_ptr(stream))
     if rc != VN_OK:
@@ -209,7 +233,7 @@ def vn_farfield_finish(acc, gmax, npoints_total: int, dtype, mu: float = 1.0, ou
     _check_dev("out", out, None, dtype)
     if out.numel() != 2 * count:
         raise ValueError("out must hold count x 2 values")
-    with torch.cuda.device(acc.device):
+    with _on(acc.device):
         rc = lib().vn_farfield_finish(acc.data_ptr() if count else None, gmax.data_ptr(), int(npoints_total), count,
                                       float(mu), out.data_ptr() if count else None,
                                       VN_F32 if dtype == torch.float32 else VN_F64, _stream_ptr(stream))
@@ -232,7 +256,7 @@ def vn_farfield_fmm(X, F, W, mu: float = 1.0, order: int = 0, out=None, stream=N
     if out is None:
         out = torch.empty_like(X)
     _check_dev("out", out, X.shape, X.dtype)
-    with torch.cuda.device(X.device):
+    with _on(X.device):
         if near_ptr is not None:
             _check_dev("near_ptr", near_ptr, (nves * npts + 1,), torch.int64)
             _check_dev("near_ves", near_ves, None, torch.int32)
@@ -255,7 +279,7 @@ def vn_arclength_weights(X, out=None, stream=None):
     if out is None:
         out = torch.empty((nves, npts), dtype=X.dtype, device=X.device)
     _check_dev("out", out, (nves, npts), X.dtype)
-    with torch.cuda.device(X.device):
+    with _on(X.device):
         rc = lib().vn_arclength_weights(X.data_ptr(), nves, npts, out.data_ptr(), _prec(X), _stream_ptr(stream))
     if rc != VN_OK:
         raise VesnetError(rc, "vn_arclength_weights")
@@ -277,7 +301,7 @@ def vn_near_pairs(X, W, near_ptr=None, near_ves=None, stream=None):
         near_ptr = torch.empty(P + 1, dtype=torch.int64, device=X.device)
     _check_dev("near_ptr", near_ptr, (P + 1,), torch.int64)
     L = lib()
-    with torch.cuda.device(X.device):
+    with _on(X.device):
         if near_ves is None:
             rc = L.vn_near_pairs(X.data_ptr(), W.data_ptr(), nves, npts, near_ptr.data_ptr(), None, 0,
                                  _prec(X), _stream_ptr(stream))
@@ -310,7 +334,7 @@ def vn_farfield_masked(X, F, W, near_ptr, near_ves, mu: float = 1.0, out=None, s
     if out is None:
         out = torch.empty_like(X)
     _check_dev("out", out, X.shape, X.dtype)
-    with torch.cuda.device(X.device):
+    with _on(X.device):
         rc = lib().vn_farfield_masked(X.data_ptr(), F.data_ptr(), W.data_ptr(), nves, npts, float(mu),
                                       near_ptr.data_ptr(), near_ves.data_ptr() if near_ves.numel() else None,
                                       out.data_ptr(), _prec(X), _stream_ptr(stream))
@@ -333,7 +357,7 @@ def vn_farfield_targets(Xt, X, F, W, mu: float = 1.0, out=None, stream=None, fmm
     if out is None:
         out = torch.empty_like(Xt)
     _check_dev("out", out, Xt.shape, X.dtype)
-    with torch.cuda.device(X.device):
+    with _on(X.device):
         pt, po = (Xt.data_ptr(), out.data_ptr()) if Xt.numel() else (None, None)
         if fmm_order > 0:
             rc = lib().vn_farfield_targets_fmm(pt, Xt.shape[0], X.data_ptr(), F.data_ptr(), W.data_ptr(), nves, npts,
@@ -357,7 +381,7 @@ def vn_elastic_force(X, sigma, kappa_b: float = 1.0, out=None, stream=None):
     if out is None:
         out = torch.empty_like(X)
     _check_dev("out", out, X.shape, X.dtype)
-    with torch.cuda.device(X.device):
+    with _on(X.device):
         rc = lib().vn_elastic_force(X.data_ptr(), sigma.data_ptr(), nves, npts, float(kappa_b), out.data_ptr(),
                                     _prec(X), _stream_ptr(stream))
     if rc != VN_OK:
@@ -375,7 +399,7 @@ def vn_redistribute_arclength(X, out=None, stream=None):
     if out is None:
         out = torch.empty_like(X)
     _check_dev("out", out, X.shape, X.dtype)
-    with torch.cuda.device(X.device):
+    with _on(X.device):
         rc = lib().vn_redistribute_arclength(X.data_ptr(), nves, npts, out.data_ptr(), _prec(X), _stream_ptr(stream))
     if rc != VN_OK:
         raise VesnetError(rc, "vn_redistribute_arclength")
@@ -456,7 +480,7 @@ def vn_selfcheck(X, F, W, mu: float = 1.0, out=None, stream=None):
         out = torch.empty_like(X)
     _check_dev("out", out, X.shape, X.dtype)
     n = ctypes.c_int64(-1)
-    with torch.cuda.device(X.device):
+    with _on(X.device):
         rc = lib().vn_selfcheck(X.data_ptr(), F.data_ptr(), W.data_ptr(), nves, npts, float(mu), out.data_ptr(),
                                 _prec(X), _stream_ptr(stream), ctypes.byref(n))
     if rc != VN_OK:

@@ -13,25 +13,35 @@
 namespace vn {
 
 // c[m] = D_{j, j-m}: first column of the circulant, m = 0 .. N-1.
+__device__ __forceinline__ double weights_coeff(int m, int N)
+{
+    if (m == 0) return 0.0;
+    const double a = (double)m / (double)N;              // angle / pi
+    const double sn = sinpi(a), cs = cospi(a);
+    const double sign = (m & 1) ? -1.0 : 1.0;
+    return (N & 1) ? 0.5 * sign / sn : 0.5 * sign * cs / sn;
+}
 __global__ void weights_table(int N, double *__restrict__ c)
 {
     const int m = blockIdx.x * blockDim.x + threadIdx.x;
-    if (m >= N) return;
-    double v = 0.0;
-    if (m > 0) {
-        const double a = (double)m / (double)N;          // angle / pi
-        const double sn = sinpi(a), cs = cospi(a);
-        const double sign = (m & 1) ? -1.0 : 1.0;
-        v = (N & 1) ? 0.5 * sign / sn : 0.5 * sign * cs / sn;
-    }
-    c[m] = v;
+    if (m < N) c[m] = weights_coeff(m, N);
 }
+// Up to kLocalTable points per vesicle every block builds the column itself, in shared memory (N / 128 coefficients
+// per thread against 2 N FMAs of its own work): no table kernel and no scratch allocation around the call, which at
+// 16 x 32 points cost more than the weights.
+constexpr int kLocalTable = 1024;
 
-template <typename real, typename real2>
+template <typename real, typename real2, bool LOCAL>
 __global__ void __launch_bounds__(128)
-weights_kernel(const real2 *__restrict__ X, int N, const double *__restrict__ c, real *__restrict__ W)
+weights_kernel(const real2 *__restrict__ X, int N, const double *__restrict__ cg, real *__restrict__ W)
 {
     __shared__ double sx[128], sy[128];
+    __shared__ double sc[LOCAL ? kLocalTable : 1];
+    const double *c = cg;
+    if (LOCAL) {
+        for (int m = threadIdx.x; m < N; m += 128) sc[m] = weights_coeff(m, N);
+        c = sc;                                          // the first barrier of the loop below orders these writes
+    }
     const int v = blockIdx.y;
     const int j = blockIdx.x * 128 + threadIdx.x;
     const real2 *Xv = X + (size_t)v * N;
@@ -52,7 +62,7 @@ weights_kernel(const real2 *__restrict__ X, int N, const double *__restrict__ c,
             int m = j - k0;                    // (j - k) mod N, walks down as k walks up
             if (m < 0) m += N;
             for (int q = 0; q < cnt; ++q) {
-                const double cm = __ldg(c + m);
+                const double cm = LOCAL ? c[m] : __ldg(c + m);
                 dx = fma(cm, sx[q], dx);
                 dy = fma(cm, sy[q], dy);
                 m = (m == 0) ? N - 1 : m - 1;
@@ -66,23 +76,29 @@ weights_kernel(const real2 *__restrict__ X, int N, const double *__restrict__ c,
 vn_status arclength_weights(const void *X, int64_t nves, int64_t npts, void *W, vn_precision prec, cudaStream_t st)
 {
     const int N = (int)npts;
+    const bool local = N <= kLocalTable;
     double *c = nullptr;
-    VN_CUDA(cudaMallocAsync((void **)&c, sizeof(double) * (size_t)N, st));
-    weights_table<<<(N + 127) / 128, 128, 0, st>>>(N, c);
+    if (!local) {
+        VN_CUDA(cudaMallocAsync((void **)&c, sizeof(double) * (size_t)N, st));
+        weights_table<<<(N + 127) / 128, 128, 0, st>>>(N, c);
+        count_launch(1);
+    }
     // grid.y is limited to 65535: walk the vesicles in slabs
     const int jb = (N + 127) / 128;
     for (int64_t v0 = 0; v0 < nves; v0 += 65535) {
         const int nv = (int)((nves - v0) < 65535 ? (nves - v0) : 65535);
         const dim3 grid(jb, nv);
-        if (prec == VN_F32)
-            weights_kernel<float, float2><<<grid, 128, 0, st>>>((const float2 *)X + v0 * N, N, c, (float *)W + v0 * N);
-        else
-            weights_kernel<double, double2><<<grid, 128, 0, st>>>((const double2 *)X + v0 * N, N, c, (double *)W + v0 * N);
+        if (prec == VN_F32) {
+            if (local) weights_kernel<float, float2, true><<<grid, 128, 0, st>>>((const float2 *)X + v0 * N, N, c, (float *)W + v0 * N);
+            else weights_kernel<float, float2, false><<<grid, 128, 0, st>>>((const float2 *)X + v0 * N, N, c, (float *)W + v0 * N);
+        } else {
+            if (local) weights_kernel<double, double2, true><<<grid, 128, 0, st>>>((const double2 *)X + v0 * N, N, c, (double *)W + v0 * N);
+            else weights_kernel<double, double2, false><<<grid, 128, 0, st>>>((const double2 *)X + v0 * N, N, c, (double *)W + v0 * N);
+        }
         count_launch(1);
     }
-    count_launch(1);
     const cudaError_t e = cudaGetLastError();
-    VN_CUDA(cudaFreeAsync(c, st));
+    if (!local) VN_CUDA(cudaFreeAsync(c, st));
     return e == cudaSuccess ? VN_OK : VN_ERR_CUDA;
 }
 
