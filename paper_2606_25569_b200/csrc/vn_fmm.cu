@@ -498,7 +498,7 @@ static size_t p2m_half_smem(int q) { return sizeof(cplx) * (size_t)(kP2MWarps * 
 // over m <= k, and q threads per expansion add the four children's parts.  The upper levels have a handful of boxes:
 // what counts there is how little one thread does in a row, not the instruction total.
 constexpr int kShiftThreads = 192;        // 12 q = 180 work items at q = 15
-constexpr int kShiftStageQ = 16;
+constexpr int kShiftStageQ = 49;     // = kFmmMaxQ: always (172 KB of dynamic shared memory at the largest order, opted into below)
 #ifndef VN_FMM_SHIFT_WAVE
 #define VN_FMM_SHIFT_WAVE 4
 #endif
@@ -607,7 +607,10 @@ static int shift_resident_blocks(int q)
     const int d = current_device();
     if (q_dev[d] != q || blocks_dev[d] == 0) {
         int dev = 0, sms = 0, o1 = 0, o2 = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess ||
+        const int max_smem = (int)shift_smem(kFmmMaxQ);              // the table in shared memory at any order: beyond 48 KB
+        if (cudaFuncSetAttribute(fmm_m2m, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem) != cudaSuccess ||
+            cudaFuncSetAttribute(fmm_l2l, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem) != cudaSuccess ||
+            cudaGetDevice(&dev) != cudaSuccess ||
             cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
             cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o1, fmm_m2m, kShiftThreads, shift_smem(q)) != cudaSuccess ||
             cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o2, fmm_l2l, kShiftThreads, shift_smem(q)) != cudaSuccess) {
@@ -635,42 +638,71 @@ static size_t shift_smem(int q) { return sizeof(cplx) * (size_t)(24 * q + (q <= 
 // vectors: one matrix entry serves all three expansions (6 DFMA per 8-byte load + 3 broadcasts).
 constexpr int kM2LWarps = 4;
 __global__ void __launch_bounds__(32 * kM2LWarps)
-fmm_m2l(int level, int q, const double *__restrict__ tab, const unsigned long long *__restrict__ enc,
+fmm_m2l(int q, const double *__restrict__ tab, const unsigned long long *__restrict__ enc,
         const cplx *__restrict__ mult, const int *__restrict__ boxcnt, const int *__restrict__ tboxcnt,
         cplx *__restrict__ loc)
 {   // tboxcnt: population of the TARGET boxes (the sources' own counts for vn_farfield_fmm; nullptr when the targets
     // are a separate set and every box may hold some): a box without targets needs no local expansion -- in a 4:1
-    // channel three quarters of the root square's boxes are empty
-    if (level > load_level(enc)) return;
+    // channel three quarters of the root square's boxes are empty.
+    // The boxes of ALL levels 2 .. L in one launch, deepest level first, and the interaction list built by the lanes
+    // in parallel, as in fmm_m2l_half below.  Coefficients 32 .. q - 1 (q > 32: a few lanes' second coefficient) are
+    // not carried through the loop by every lane -- half of its DFMAs would multiply padding -- but summed afterwards
+    // by (coefficient, quarter of the k range) work items and met through shared memory.
+    const int L = load_level(enc);
     extern __shared__ __align__(16) double sm[];
     double *Cb = sm;                                                  // [q][q]
     const int warp = threadIdx.x >> 5, ln = threadIdx.x & 31;
-    cplx *hat = (cplx *)(sm + ((q * q + 1) & ~1)) + warp * 3 * (q + 1);   // [3][q+1] per warp; hat[a][q] = 0 pads the shifted read
+    cplx *hat = (cplx *)(sm + ((q * q + 1) & ~1)) + warp * (3 * (q + 1) + 96);   // [3][q+1] per warp; hat[a][q] = 0 pads the shifted read
+    cplx *red = hat + 3 * (q + 1);                                    // [32][3] partial sums of the coefficients >= 32
+    int *list = (int *)((cplx *)(sm + ((q * q + 1) & ~1)) + kM2LWarps * (3 * (q + 1) + 96)) + warp * 32;
     const FmmTables t = fmm_tables_at(const_cast<double *>(tab), q);
     for (int e = threadIdx.x; e < q * q; e += blockDim.x) Cb[e] = t.Cb[e];
     __syncthreads();
-    const int n = 1 << level;
     const Geom gm = load_geom(enc);
-    const double s = gm.size / (double)n, log_s = log(s);
+    const double log_size = log(gm.size);
     const int l0 = ln, l1 = ln + 32;
     const bool v0 = l0 < q, v1 = l1 < q;
-    for (int box = blockIdx.x * kM2LWarps + warp; box < n * n; box += gridDim.x * kM2LWarps) {
-    if (tboxcnt && tboxcnt[level_offset(level) + box] == 0) continue;
-    const int ix = box / n, iy = box % n;
+    const int nb = q > 32 ? q - 32 : 0, nchunk = nb ? 32 / nb : 0, kper = nb ? (q + nchunk - 1) / nchunk : 0;
+    const long long total = level_offset(L + 1) - level_offset(2);
+    for (long long gi = (long long)blockIdx.x * kM2LWarps + warp; gi < total; gi += (long long)gridDim.x * kM2LWarps) {
+    int level = L;
+    long long rem = gi;
+    while (rem >= (1ll << (2 * level))) { rem -= 1ll << (2 * level); --level; }
+    const int box = (int)rem, n = 1 << level;
+    const double s = gm.size / (double)n, log_s = fma(-(double)level, 0.693147180559945309417, log_size);
+    const long long lev0 = level_offset(level);
+    if (tboxcnt && tboxcnt[lev0 + box] == 0) continue;
+    const int ix = box / n, iy = box % n, px = ix >> 1, py = iy >> 1;
+    __syncwarp();
+    int nlist = 0;
+#pragma unroll
+    for (int r = 0; r < 2; ++r) {
+        const int e = ln + 32 * r;
+        bool ok = false;
+        int entry = 0;
+        if (e < 36) {
+            const int sx = 2 * (px - 1) + e / 6, sy = 2 * (py - 1) + e % 6;
+            if (sx >= 0 && sx < n && sy >= 0 && sy < n && !(abs(sx - ix) <= 1 && abs(sy - iy) <= 1)) {
+                const int src = sx * n + sy;
+                ok = boxcnt[lev0 + src] != 0;
+                entry = src | (((ix - sx + 3) * 7 + (iy - sy + 3)) << 24);
+            }
+        }
+        const unsigned m = __ballot_sync(0xffffffffu, ok);
+        if (ok) list[nlist + __popc(m & ((1u << ln) - 1u))] = entry;
+        nlist += __popc(m);
+    }
+    __syncwarp();
     cplx acc[3][2];
 #pragma unroll
     for (int a = 0; a < 3; ++a) acc[a][0] = acc[a][1] = make_double2(0.0, 0.0);
-    const cplx *Mlev = mult + level_offset(level) * (long long)(3 * q);
-    const int px = ix >> 1, py = iy >> 1;
-    for (int sx = max(0, 2 * (px - 1)); sx < min(n, 2 * (px + 1) + 2); ++sx)
-        for (int sy = max(0, 2 * (py - 1)); sy < min(n, 2 * (py + 1) + 2); ++sy) {
-            if (abs(sx - ix) <= 1 && abs(sy - iy) <= 1) continue;
-            const long long src = (long long)sx * n + sy;
-            if (boxcnt[level_offset(level) + src] == 0) continue;
-            const int o = (ix - sx + 3) * 7 + (iy - sy + 3);
+    const cplx *Mlev = mult + lev0 * (long long)(3 * q);
+    for (int i = 0; i < nlist; ++i) {
+            const int entry = list[i];
+            const int o = entry >> 24;
             const cplx *rho = t.rho + (size_t)o * (q + 1);
-            const cplx *A = Mlev + src * (3 * q);
-            __syncwarp();                                             // the previous source's hat is consumed
+            const cplx *A = Mlev + (long long)(entry & 0xffffff) * (3 * q);
+            __syncwarp();                                             // the previous source's hat and red are consumed
             for (int k = ln; k <= q; k += 32) {
                 cplx h0 = make_double2(0.0, 0.0), h1 = h0, h2 = h0;
                 if (k < q) {
@@ -690,15 +722,42 @@ fmm_m2l(int level, int q, const double *__restrict__ tab, const unsigned long lo
 #pragma unroll
             for (int a = 0; a < 3; ++a) S[a][0] = S[a][1] = make_double2(0.0, 0.0);
             const cplx *h0p = hat + 1, *h1p = hat + (q + 1) + 1, *h2p = hat + 2 * (q + 1);   // log arrays read k + 1
-            for (int k = 0; k < q; ++k) {
-                const double c0 = v0 ? Cb[k * q + l0] : 0.0, c1 = v1 ? Cb[k * q + l1] : 0.0;
-                const cplx e0 = h0p[k], e1 = h1p[k], e2 = h2p[k];     // Ahat1_{k+1}, Ahat2_{k+1}, Bhat_k
-                S[0][0].x = fma(c0, e0.x, S[0][0].x); S[0][0].y = fma(c0, e0.y, S[0][0].y);
-                S[1][0].x = fma(c0, e1.x, S[1][0].x); S[1][0].y = fma(c0, e1.y, S[1][0].y);
-                S[2][0].x = fma(c0, e2.x, S[2][0].x); S[2][0].y = fma(c0, e2.y, S[2][0].y);
-                S[0][1].x = fma(c1, e0.x, S[0][1].x); S[0][1].y = fma(c1, e0.y, S[0][1].y);
-                S[1][1].x = fma(c1, e1.x, S[1][1].x); S[1][1].y = fma(c1, e1.y, S[1][1].y);
-                S[2][1].x = fma(c1, e2.x, S[2][1].x); S[2][1].y = fma(c1, e2.y, S[2][1].y);
+            {
+                const double *Cl = Cb + (v0 ? l0 : 0);
+#pragma unroll 4
+                for (int k = 0; k < q; ++k) {
+                    const double c0 = Cl[k * q];
+                    const cplx e0 = h0p[k], e1 = h1p[k], e2 = h2p[k];     // Ahat1_{k+1}, Ahat2_{k+1}, Bhat_k
+                    S[0][0].x = fma(c0, e0.x, S[0][0].x); S[0][0].y = fma(c0, e0.y, S[0][0].y);
+                    S[1][0].x = fma(c0, e1.x, S[1][0].x); S[1][0].y = fma(c0, e1.y, S[1][0].y);
+                    S[2][0].x = fma(c0, e2.x, S[2][0].x); S[2][0].y = fma(c0, e2.y, S[2][0].y);
+                }
+            }
+            if (nb) {                                                 // coefficients 32 .. q - 1: item (coefficient j, chunk c of the k range)
+                cplx T0 = make_double2(0.0, 0.0), T1 = T0, T2 = T0;
+                if (ln < nchunk * nb) {
+                    const int c = ln / nb, j = ln - c * nb;
+                    const double *Cl = Cb + 32 + j;
+                    const int k1 = min(q, (c + 1) * kper);
+                    for (int k = c * kper; k < k1; ++k) {
+                        const double c1 = Cl[k * q];
+                        const cplx e0 = h0p[k], e1 = h1p[k], e2 = h2p[k];
+                        T0.x = fma(c1, e0.x, T0.x); T0.y = fma(c1, e0.y, T0.y);
+                        T1.x = fma(c1, e1.x, T1.x); T1.y = fma(c1, e1.y, T1.y);
+                        T2.x = fma(c1, e2.x, T2.x); T2.y = fma(c1, e2.y, T2.y);
+                    }
+                }
+                red[ln * 3 + 0] = T0;
+                red[ln * 3 + 1] = T1;
+                red[ln * 3 + 2] = T2;
+                __syncwarp();
+                if (v1)
+                    for (int c = 0; c < nchunk; ++c) {
+                        const cplx *pr = red + (ln + c * nb) * 3;
+                        S[0][1] = cadd(S[0][1], pr[0]);
+                        S[1][1] = cadd(S[1][1], pr[1]);
+                        S[2][1] = cadd(S[2][1], pr[2]);
+                    }
             }
 #pragma unroll
             for (int j = 0; j < 2; ++j) {
@@ -720,7 +779,7 @@ fmm_m2l(int level, int q, const double *__restrict__ tab, const unsigned long lo
                 if (l == 0) acc[2][j] = cadd(acc[2][j], make_double2(-(A10.x - A20.y), A10.y + A20.x));   // -conj(A1_0 + i A2_0)
             }
         }
-    cplx *out = loc + (level_offset(level) + box) * (long long)(3 * q);
+    cplx *out = loc + (lev0 + box) * (long long)(3 * q);
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
         if (v0) out[a * q + l0] = acc[a][0];
@@ -728,6 +787,11 @@ fmm_m2l(int level, int q, const double *__restrict__ tab, const unsigned long lo
     }
     __syncwarp();
     }   // boxes
+}
+static size_t m2l_smem(int q)
+{
+    return sizeof(double) * (size_t)((q * q + 1) & ~1) + sizeof(cplx) * (size_t)(kM2LWarps * (3 * (q + 1) + 96)) +
+           sizeof(int) * (size_t)(kM2LWarps * 32);
 }
 
 // M2L for q <= 16 (orders up to 15: the defaults, 12 in double and 14 in single precision, live here).  fmm_m2l gives
@@ -1459,32 +1523,30 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
         fmm_p2m<<<(ncell + 3) / 4, 128, 0, st>>>(zs, gs, start, q, enc, mult, boxcnt);
     ++launches;
     FMM_TICK("p2m");
+    const int resident = L >= 3 ? shift_resident_blocks(q) : 1;     // also opts the two kernels into their shared memory
     if (L >= 3) {     // the level above the leaves with a full grid, all levels above it in one launch of resident blocks
         const unsigned nb = 1u << (2 * (L - 1));
         fmm_m2m<<<nb < 148u * kShiftWave ? nb : 148u * kShiftWave, kShiftThreads, shift_smem(q), st>>>(1, 1, q, tab, enc, mult, boxcnt);
         ++launches;
         if (L >= 4) {
-            fmm_m2m<<<shift_resident_blocks(q), kShiftThreads, shift_smem(q), st>>>(2, 99, q, tab, enc, mult, boxcnt);
+            fmm_m2m<<<resident, kShiftThreads, shift_smem(q), st>>>(2, 99, q, tab, enc, mult, boxcnt);
             ++launches;
         }
     }
-    const size_t smem_m2l = sizeof(double) * (size_t)(((q * q + 1) & ~1) + 2 * kM2LWarps * 3 * (q + 1));
     FMM_TICK("m2m");
     if (q <= kM2LHalfQ) {              // all levels in one launch
         const long long nb = (level_offset(L + 1) - level_offset(2) + kM2LWarps - 1) / kM2LWarps;
         fmm_m2l_half<<<(unsigned)(nb < 148 * 16 ? nb : 148 * 16), 32 * kM2LWarps, m2l_half_smem(q), st>>>(q, tab, enc, mult, boxcnt, boxcnt, loc);
         ++launches;
     } else {
-        for (int l = 2; l <= L; ++l) {
-            const unsigned nb = ((1u << (2 * l)) + kM2LWarps - 1) / kM2LWarps;
-            fmm_m2l<<<nb < 148u * 16u ? nb : 148u * 16u, 32 * kM2LWarps, smem_m2l, st>>>(l, q, tab, enc, mult, boxcnt, boxcnt, loc);
-            ++launches;
-        }
+        const long long nb = (level_offset(L + 1) - level_offset(2) + kM2LWarps - 1) / kM2LWarps;
+        fmm_m2l<<<(unsigned)(nb < 148 * 16 ? nb : 148 * 16), 32 * kM2LWarps, m2l_smem(q), st>>>(q, tab, enc, mult, boxcnt, boxcnt, loc);
+        ++launches;
     }
     FMM_TICK("m2l");
     if (L >= 3) {     // levels 3 .. L - 1 in one launch of resident blocks, the leaf level with a full grid
         if (L >= 4) {
-            fmm_l2l<<<shift_resident_blocks(q), kShiftThreads, shift_smem(q), st>>>(99, 1, q, tab, enc, boxcnt, loc);
+            fmm_l2l<<<resident, kShiftThreads, shift_smem(q), st>>>(99, 1, q, tab, enc, boxcnt, loc);
             ++launches;
         }
         const unsigned nb = 1u << (2 * (L - 1));
@@ -1626,30 +1688,28 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
     else
         fmm_p2m<<<(ncell + 3) / 4, 128, 0, st>>>(zs, gs, start, q, enc, mult, boxcnt);
     ++launches;
+    const int resident = L >= 3 ? shift_resident_blocks(q) : 1;     // also opts the two kernels into their shared memory
     if (L >= 3) {     // the level above the leaves with a full grid, all levels above it in one launch of resident blocks
         const unsigned nb = 1u << (2 * (L - 1));
         fmm_m2m<<<nb < 148u * kShiftWave ? nb : 148u * kShiftWave, kShiftThreads, shift_smem(q), st>>>(1, 1, q, tab, enc, mult, boxcnt);
         ++launches;
         if (L >= 4) {
-            fmm_m2m<<<shift_resident_blocks(q), kShiftThreads, shift_smem(q), st>>>(2, 99, q, tab, enc, mult, boxcnt);
+            fmm_m2m<<<resident, kShiftThreads, shift_smem(q), st>>>(2, 99, q, tab, enc, mult, boxcnt);
             ++launches;
         }
     }
-    const size_t smem_m2l = sizeof(double) * (size_t)(((q * q + 1) & ~1) + 2 * kM2LWarps * 3 * (q + 1));
     if (q <= kM2LHalfQ) {              // all levels in one launch
         const long long nb = (level_offset(L + 1) - level_offset(2) + kM2LWarps - 1) / kM2LWarps;
         fmm_m2l_half<<<(unsigned)(nb < 148 * 16 ? nb : 148 * 16), 32 * kM2LWarps, m2l_half_smem(q), st>>>(q, tab, enc, mult, boxcnt, nullptr, loc);
         ++launches;
     } else {
-        for (int l = 2; l <= L; ++l) {
-            const unsigned nb = ((1u << (2 * l)) + kM2LWarps - 1) / kM2LWarps;
-            fmm_m2l<<<nb < 148u * 16u ? nb : 148u * 16u, 32 * kM2LWarps, smem_m2l, st>>>(l, q, tab, enc, mult, boxcnt, nullptr, loc);
-            ++launches;
-        }
+        const long long nb = (level_offset(L + 1) - level_offset(2) + kM2LWarps - 1) / kM2LWarps;
+        fmm_m2l<<<(unsigned)(nb < 148 * 16 ? nb : 148 * 16), 32 * kM2LWarps, m2l_smem(q), st>>>(q, tab, enc, mult, boxcnt, nullptr, loc);
+        ++launches;
     }
     if (L >= 3) {     // levels 3 .. L - 1 in one launch of resident blocks, the leaf level with a full grid
         if (L >= 4) {
-            fmm_l2l<<<shift_resident_blocks(q), kShiftThreads, shift_smem(q), st>>>(99, 1, q, tab, enc, nullptr, loc);
+            fmm_l2l<<<resident, kShiftThreads, shift_smem(q), st>>>(99, 1, q, tab, enc, nullptr, loc);
             ++launches;
         }
         const unsigned nb = 1u << (2 * (L - 1));
