@@ -374,75 +374,30 @@ __global__ void fmm_build_tables(int q, double *base, double *logtab)
 __host__ __device__ inline long long level_offset(int l) { return ((1ll << (2 * l)) - 1) / 3; }
 
 // ------------------------------------------------------------------------------------------------
-// P2M: one warp per leaf box.  Moments about the box centre in the scaled variable w = (zeta - c)/s:
+// P2M: moments about the box centre in the scaled variable w = (zeta - c)/s:
 //   A1_k = sum g_x w^k,  A2_k = sum g_y w^k,  B_k = sum conj(zeta) g w^k.
 constexpr int kFmmMaxQ = 49;          // p <= 48
-__global__ void __launch_bounds__(128)
-fmm_p2m(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const long long *__restrict__ start, int q,
-        const unsigned long long *__restrict__ enc, cplx *__restrict__ mult, int *__restrict__ boxcnt)
-{
-    const int L = load_level(enc);
-    __shared__ cplx acc[4][3 * kFmmMaxQ];
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int n = 1 << L, ncell = n * n;
-    const int c = blockIdx.x * 4 + warp;
-    if (c >= ncell) return;
-    const Geom gm = load_geom(enc);
-    const double s = gm.size / (double)n, inv_s = 1.0 / s;
-    const cplx ctr = box_centre(gm, L, c / n, c % n);
-    for (int e = lane; e < 3 * q; e += 32) acc[warp][e] = make_double2(0.0, 0.0);
-    __syncwarp();
-    const long long a = start[c], b = start[c + 1];
-    if (lane == 0) boxcnt[level_offset(L) + c] = (int)(b - a);
-    for (long long base = a; base < b; base += 32) {
-        const long long idx = base + lane;
-        cplx w = make_double2(0.0, 0.0), g = make_double2(0.0, 0.0), h = make_double2(0.0, 0.0);
-        if (idx < b) {
-            const cplx zt = zs[idx];
-            g = gs[idx];
-            w = make_double2((zt.x - ctr.x) * inv_s, (zt.y - ctr.y) * inv_s);
-            h = cmul(make_double2(zt.x, -zt.y), g);                  // conj(zeta) g
-        }
-        cplx pw = make_double2(1.0, 0.0);
-        for (int k = 0; k < q; ++k) {
-            double v[6] = {g.x * pw.x, g.x * pw.y, g.y * pw.x, g.y * pw.y, fma(h.x, pw.x, -h.y * pw.y), fma(h.x, pw.y, h.y * pw.x)};
-#pragma unroll
-            for (int m = 16; m >= 1; m >>= 1)
-#pragma unroll
-                for (int e = 0; e < 6; ++e) v[e] += __shfl_xor_sync(0xffffffffu, v[e], m);
-            if (lane == 0) {
-                acc[warp][k] = cadd(acc[warp][k], make_double2(v[0], v[1]));
-                acc[warp][q + k] = cadd(acc[warp][q + k], make_double2(v[2], v[3]));
-                acc[warp][2 * q + k] = cadd(acc[warp][2 * q + k], make_double2(v[4], v[5]));
-            }
-            pw = cmul(pw, w);
-        }
-    }
-    __syncwarp();
-    cplx *out = mult + (level_offset(L) + c) * (long long)(3 * q);
-    for (int e = lane; e < 3 * q; e += 32) out[e] = acc[warp][e];
-}
-
-// P2M for q <= 16.  fmm_p2m reduces every power over the lanes (60 shuffles per coefficient and 32 sources); here
-// the sum runs the other way round: for 32 sources at a time lane j writes the powers w_j^0 .. w_j^(q-1) of ITS source
-// into the warp's shared memory (row stride odd in 16-byte words: conflict-free both ways), then lane (half, k) adds up
-// coefficient k over the sources j = half, half + 2, ... -- a 16-byte load of the power and two broadcasts (g, conj(zeta) g)
-// per 8 DFMA, no shuffles -- and the two halves meet once per leaf.
+// One warp per leaf box, no shuffles (a reduction of every power over the lanes costs 60 shuffles per coefficient and
+// 32 sources): the sum runs the other way round: for 32 sources at a time lane j writes 16 consecutive powers of
+// ITS source into the warp's shared memory (row stride 17 sixteen-byte words: conflict-free both ways), then lane
+// (half, k) adds up coefficient 16 g + k over the sources j = half, half + 2, ... -- a 16-byte load of the power and
+// two broadcasts (g, conj(zeta) g) per 8 DFMA -- group g = 0 .. ceil(q / 16) - 1 after group, the power recurrence
+// carried on in a register; the two halves meet once per leaf.
 constexpr int kP2MWarps = 4;
+constexpr int kP2MGroups = (kFmmMaxQ + 15) / 16;       // 4
 __global__ void __launch_bounds__(32 * kP2MWarps)
-fmm_p2m_half(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const long long *__restrict__ start, int q,
+fmm_p2m(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const long long *__restrict__ start, int q,
              const unsigned long long *__restrict__ enc, cplx *__restrict__ mult, int *__restrict__ boxcnt)
 {
     const int L = load_level(enc);
-    extern __shared__ __align__(16) double sm[];
+    constexpr int stride = 17;
+    __shared__ cplx pws[kP2MWarps][32 * stride + 64];                 // [32][17] powers | [32] g | [32] conj(zeta) g
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, half = lane >> 4, k = lane & 15;
-    const int stride = q | 1;
-    cplx *pw = (cplx *)sm + warp * (32 * stride + 64);               // [32][stride] powers | [32] g | [32] conj(zeta) g
-    cplx *sg = pw + 32 * stride, *sh = sg + 32;
+    cplx *pw = pws[warp], *sg = pw + 32 * stride, *sh = sg + 32;
     const int n = 1 << L, ncell = n * n;
     const Geom gm = load_geom(enc);
     const double s = gm.size / (double)n, inv_s = 1.0 / s;
-    const bool v = k < q;
+    const int ng = (q + 15) >> 4;
     for (int c = blockIdx.x * kP2MWarps + warp; c < ncell; c += gridDim.x * kP2MWarps) {
         const long long a = start[c], b = start[c + 1];
         if (lane == 0) boxcnt[level_offset(L) + c] = (int)(b - a);
@@ -452,45 +407,60 @@ fmm_p2m_half(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const lon
             continue;
         }
         const cplx ctr = box_centre(gm, L, c / n, c % n);
-        cplx a1 = make_double2(0.0, 0.0), a2 = a1, bb = a1;          // A1_k, A2_k, B_k (this half's sources)
+        cplx a1[kP2MGroups], a2[kP2MGroups], bb[kP2MGroups];         // A1, A2, B of coefficient 16 g + k (this half's sources)
+#pragma unroll
+        for (int g = 0; g < kP2MGroups; ++g) a1[g] = a2[g] = bb[g] = make_double2(0.0, 0.0);
         for (long long base = a; base < b; base += 32) {
             const long long idx = base + lane;
             const int cnt = (int)min(32ll, b - base);
+            cplx w = make_double2(0.0, 0.0), p = make_double2(1.0, 0.0);
             __syncwarp();                                            // the previous 32 sources are consumed
             if (idx < b) {
                 const cplx zt = zs[idx], g = gs[idx];
-                const cplx w = make_double2((zt.x - ctr.x) * inv_s, (zt.y - ctr.y) * inv_s);
+                w = make_double2((zt.x - ctr.x) * inv_s, (zt.y - ctr.y) * inv_s);
                 sg[lane] = g;
                 sh[lane] = cmul(make_double2(zt.x, -zt.y), g);      // conj(zeta) g
-                cplx p = make_double2(1.0, 0.0);
-                cplx *row = pw + lane * stride;
-                for (int kk = 0; kk < q; ++kk) {
-                    row[kk] = p;
-                    p = cmul(p, w);
-                }
             }
-            __syncwarp();
-            if (v) {
+#pragma unroll
+            for (int g = 0; g < kP2MGroups; ++g) {
+                if (g < ng) {
+                    if (g > 0) __syncwarp();                         // the previous group's powers are consumed
+                    cplx *row = pw + lane * stride;
 #pragma unroll 4
-                for (int j = half; j < cnt; j += 2) {
-                    const cplx p = pw[j * stride + k], g = sg[j], h = sh[j];
-                    a1.x = fma(g.x, p.x, a1.x); a1.y = fma(g.x, p.y, a1.y);
-                    a2.x = fma(g.y, p.x, a2.x); a2.y = fma(g.y, p.y, a2.y);
-                    bb = cfma(h, p, bb);
+                    for (int kk = 0; kk < 16; ++kk) {
+                        row[kk] = p;
+                        p = cmul(p, w);
+                    }
+                    __syncwarp();
+                    if (16 * g + k < q) {
+#pragma unroll 4
+                        for (int j = half; j < cnt; j += 2) {
+                            const cplx pp = pw[j * stride + k], g2 = sg[j], h = sh[j];
+                            a1[g].x = fma(g2.x, pp.x, a1[g].x); a1[g].y = fma(g2.x, pp.y, a1[g].y);
+                            a2[g].x = fma(g2.y, pp.x, a2[g].x); a2[g].y = fma(g2.y, pp.y, a2[g].y);
+                            bb[g] = cfma(h, pp, bb[g]);
+                        }
+                    }
                 }
             }
         }
-        a1.x += __shfl_xor_sync(0xffffffffu, a1.x, 16); a1.y += __shfl_xor_sync(0xffffffffu, a1.y, 16);
-        a2.x += __shfl_xor_sync(0xffffffffu, a2.x, 16); a2.y += __shfl_xor_sync(0xffffffffu, a2.y, 16);
-        bb.x += __shfl_xor_sync(0xffffffffu, bb.x, 16); bb.y += __shfl_xor_sync(0xffffffffu, bb.y, 16);
-        if (v && half == 0) {
-            out[k] = a1;
-            out[q + k] = a2;
-            out[2 * q + k] = bb;
+#pragma unroll
+        for (int g = 0; g < kP2MGroups; ++g) {
+            if (g < ng) {
+                cplx x1 = a1[g], x2 = a2[g], xb = bb[g];
+                x1.x += __shfl_xor_sync(0xffffffffu, x1.x, 16); x1.y += __shfl_xor_sync(0xffffffffu, x1.y, 16);
+                x2.x += __shfl_xor_sync(0xffffffffu, x2.x, 16); x2.y += __shfl_xor_sync(0xffffffffu, x2.y, 16);
+                xb.x += __shfl_xor_sync(0xffffffffu, xb.x, 16); xb.y += __shfl_xor_sync(0xffffffffu, xb.y, 16);
+                const int kq = 16 * g + k;
+                if (kq < q && half == 0) {
+                    out[kq] = x1;
+                    out[q + kq] = x2;
+                    out[2 * q + kq] = xb;
+                }
+            }
         }
     }
 }
-static size_t p2m_half_smem(int q) { return sizeof(cplx) * (size_t)(kP2MWarps * (32 * (q | 1) + 64)); }
 
 // M2M: parent moments from its four children, levels L-1 down to 2.  One BLOCK per parent box (grid-stride): the
 // children's moments are staged in shared memory with coalesced loads (one round trip to L2 instead of one per term),
@@ -993,172 +963,16 @@ fmm_l2l(int d_hi, int d_lo, int q, const double *__restrict__ tab, unsigned long
 }
 
 // ------------------------------------------------------------------------------------------------
-// L2P + P2P: one block per leaf box; kP2PSplit threads share one target (each takes every kP2PSplit-th source,
-// fixed-order shuffle reduction), targets in rounds of kP2PThreads / kP2PSplit.
+// ------------------------------------------------------------------------------------------------
+// L2P + P2P: one block of 128 threads per leaf box (grid-stride).
 //   far  = -(Re Phi1 + i Re Phi2) + (z/2) conj(Phi1' + i Phi2') - (1/2) conj(psi)   from the box's local expansions
 //   near = direct sum over the points of the 3 x 3 neighbour boxes that belong to OTHER vesicles
-// The sum goes to accum[original point index] (still without the 1/(4 pi mu)).
-#ifndef VN_FMM_P2P_THREADS
-#define VN_FMM_P2P_THREADS 128
-#endif
-#ifndef VN_FMM_P2P_SPLIT
-#define VN_FMM_P2P_SPLIT 4
-#endif
-#ifndef VN_FMM_P2P_TARGETS
-#define VN_FMM_P2P_TARGETS 2
-#endif
-constexpr int kP2PThreads = VN_FMM_P2P_THREADS;
-constexpr int kP2PSplit = VN_FMM_P2P_SPLIT;       // threads that share one target (power of two, <= 32)
-constexpr int kP2PTargets = VN_FMM_P2P_TARGETS;   // targets per thread
-template <bool F32NEAR>
-__global__ void __launch_bounds__(kP2PThreads)
-fmm_l2p_p2p(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const int *__restrict__ vs,
-            const long long *__restrict__ start, const cplx *__restrict__ tz, const int *__restrict__ tvs,
-            const int *__restrict__ tperm, const long long *__restrict__ tstart, int q,
-            const unsigned long long *__restrict__ enc, const cplx *__restrict__ loc, const double *__restrict__ logtab,
-            cplx *__restrict__ accum)
-{   // targets (tz, tvs, tperm, tstart) are the sorted sources themselves for vn_farfield_fmm, a separate sorted set
-    // (tvs == nullptr: no vesicle to exclude) for the free-target variant.
-    // F32NEAR (fp32 storage): the direct part runs in fp32 with the SFU lg2/rcp, exactly the pair arithmetic of the
-    // exact fp32 kernel (the stored positions and densities ARE floats, so nothing is lost converting them back),
-    // per-chunk float partial sums folded into double accumulators; the expansions stay double.
-    __shared__ double tab[F32NEAR ? 1 : kLogTab + kExpTab];
-    __shared__ cplx lc[3 * kFmmMaxQ];
-    __shared__ double4 src[kP2PThreads];               // (zeta_x, zeta_y, g_x, g_y)
-    __shared__ int sves[kP2PThreads];
-    constexpr int kRound = kP2PThreads / kP2PSplit;
-    const int L = load_level(enc);
-    const int n = 1 << L;
-    const int tid = threadIdx.x, slot = tid / kP2PSplit, part = tid % kP2PSplit;
-    if (!F32NEAR)
-        for (int e = tid; e < kLogTab + kExpTab; e += kP2PThreads) tab[e] = logtab[e];
-    const Geom gm = load_geom(enc);
-    const double s = gm.size / (double)n, inv_s = 1.0 / s;
-    // the grid is sized by the host for the deepest admissible tree: leaves are walked with a grid stride
-    for (int c = blockIdx.x; c < n * n; c += gridDim.x) {
-    const int ix = c / n, iy = c % n;
-    const long long a = tstart[c], b = tstart[c + 1];
-    if (a == b) continue;
-    __syncthreads();                                   // the previous leaf's lc is consumed
-    for (int e = tid; e < 3 * q; e += kP2PThreads) lc[e] = loc[(level_offset(L) + c) * (long long)(3 * q) + e];
-    const cplx ctr = box_centre(gm, L, ix, iy);
-    __syncthreads();
-
-    // a thread owns up to kP2PTargets targets (slot, slot + kRound, ...) and every kP2PSplit-th source of a staged
-    // chunk: the source record is read once for kP2PTargets pairs, which are independent chains
-    for (long long t0 = a; t0 < b; t0 += kRound * kP2PTargets) {
-        cplx z[kP2PTargets];
-        int myves[kP2PTargets];
-        double ux[kP2PTargets], uy[kP2PTargets];
-        bool live[kP2PTargets];
-#pragma unroll
-        for (int r = 0; r < kP2PTargets; ++r) {
-            const long long ti = t0 + slot + r * kRound;
-            live[r] = ti < b;
-            z[r] = make_double2(0.0, 0.0);
-            myves[r] = -2;
-            ux[r] = uy[r] = 0.0;
-            if (live[r]) {
-                z[r] = tz[ti];
-                myves[r] = tvs ? tvs[ti] : -1;
-            }
-            if (live[r] && part == 0) {
-                // far field: Horner for value and derivative of the three local expansions
-                const cplx t = make_double2((z[r].x - ctr.x) * inv_s, (z[r].y - ctr.y) * inv_s);
-                cplx p1 = lc[q - 1], p2 = lc[2 * q - 1], p3 = lc[3 * q - 1];
-                cplx d1 = make_double2(0.0, 0.0), d2 = d1;
-                for (int l = q - 2; l >= 0; --l) {
-                    d1 = cfma(d1, t, p1);
-                    d2 = cfma(d2, t, p2);
-                    p1 = cfma(p1, t, lc[l]);
-                    p2 = cfma(p2, t, lc[q + l]);
-                    p3 = cfma(p3, t, lc[2 * q + l]);
-                }
-                // phi = (Phi1' + i Phi2') = (d1 + i d2)/s ;  z conj(phi)
-                const cplx phi = make_double2((d1.x - d2.y) * inv_s, (d1.y + d2.x) * inv_s);
-                const cplx zc = cmul(z[r], make_double2(phi.x, -phi.y));
-                ux[r] = -p1.x + 0.5 * zc.x - 0.5 * p3.x;
-                uy[r] = -p2.x + 0.5 * zc.y + 0.5 * p3.y;
-            }
-        }
-        // near field
-        for (int bx = max(ix - 1, 0); bx <= min(ix + 1, n - 1); ++bx)
-            for (int by = max(iy - 1, 0); by <= min(iy + 1, n - 1); ++by) {
-                const long long sa = start[bx * n + by], sb = start[bx * n + by + 1];
-                for (long long s0 = sa; s0 < sb; s0 += kP2PThreads) {
-                    __syncthreads();
-                    if (s0 + tid < sb) {
-                        const cplx zz = zs[s0 + tid], gg = gs[s0 + tid];
-                        if (F32NEAR)    // the stored values are floats: converted back once per staged source, exactly
-                            reinterpret_cast<float4 *>(src)[tid] = make_float4((float)zz.x, (float)zz.y, (float)gg.x, (float)gg.y);
-                        else
-                            src[tid] = make_double4(zz.x, zz.y, gg.x, gg.y);
-                        sves[tid] = vs[s0 + tid];
-                    }
-                    __syncthreads();
-                    const int cnt = (int)min((long long)kP2PThreads, sb - s0);
-                    if (F32NEAR) {
-                        float fx[kP2PTargets], fy[kP2PTargets], zx[kP2PTargets], zy[kP2PTargets];
-#pragma unroll
-                        for (int r = 0; r < kP2PTargets; ++r) {
-                            fx[r] = fy[r] = 0.f;
-                            zx[r] = (float)z[r].x;
-                            zy[r] = (float)z[r].y;
-                        }
-                        for (int j = part; j < cnt; j += kP2PSplit) {
-                            const float4 sj = reinterpret_cast<const float4 *>(src)[j];
-                            const float sx = sj.x, sy = sj.y, gx = sj.z, gy = sj.w;
-                            const int sv = sves[j];
-#pragma unroll
-                            for (int r = 0; r < kP2PTargets; ++r) {
-                                if (sv == myves[r] || !live[r]) continue;
-                                const float rx = zx[r] - sx, ry = zy[r] - sy;
-                                const float r2 = fmaf(rx, rx, ry * ry);
-                                const float ml = -0.34657359027997264f * sfu_lg2(r2);
-                                const float qd = fmaf(rx, gx, ry * gy) * sfu_rcp(r2);
-                                fx[r] += fmaf(ml, gx, qd * rx);
-                                fy[r] += fmaf(ml, gy, qd * ry);
-                            }
-                        }
-#pragma unroll
-                        for (int r = 0; r < kP2PTargets; ++r) { ux[r] += (double)fx[r]; uy[r] += (double)fy[r]; }
-                    } else {
-                        for (int j = part; j < cnt; j += kP2PSplit) {
-                            const double4 sj = src[j];
-                            const int sv = sves[j];
-#pragma unroll
-                            for (int r = 0; r < kP2PTargets; ++r) {
-                                if (sv == myves[r] || !live[r]) continue;
-                                const double rx = z[r].x - sj.x, ry = z[r].y - sj.y;
-                                const double r2 = fma(rx, rx, ry * ry);
-                                double ml, inv;
-                                log_rcp_f64(r2, tab, ml, inv);
-                                const double qd = fma(rx, sj.z, ry * sj.w) * inv;
-                                ux[r] = fma(ml, sj.z, fma(qd, rx, ux[r]));
-                                uy[r] = fma(ml, sj.w, fma(qd, ry, uy[r]));
-                            }
-                        }
-                    }
-                }
-            }
-#pragma unroll
-        for (int r = 0; r < kP2PTargets; ++r) {
-#pragma unroll
-            for (int m = 1; m < kP2PSplit; m <<= 1) {
-                ux[r] += __shfl_xor_sync(0xffffffffu, ux[r], m);
-                uy[r] += __shfl_xor_sync(0xffffffffu, uy[r], m);
-            }
-            if (live[r] && part == 0) accum[tperm[t0 + slot + r * kRound]] = make_double2(ux[r], uy[r]);
-        }
-        __syncthreads();
-    }
-    }   // leaves
-}
-
-// L2P + P2P for single-precision storage, the version the fp32 calls run (fmm_l2p_p2p<true> above is its plain
-// predecessor, kept as the readable statement of the same sum).  What changes is the shape of the work, not the sum:
-//  * a thread owns TWO targets as the halves of packed fp32 pairs (FADD2 / FMUL2 / FFMA2, the arithmetic of the exact
-//    fp32 kernels): per source and target pair 11 packed instructions + 4 MUFU instead of 2 x 14 scalar ones;
+// The sum goes to accum[original point index] (still without the 1/(4 pi mu)).  Targets (tz, tvs, tperm, tstart) are
+// the sorted sources themselves for vn_farfield_fmm, a separate sorted set (tvs == nullptr: no vesicle to exclude)
+// for the free-target variant.  The shape of the work:
+//  * a thread owns TWO targets.  Single-precision storage: as the halves of packed fp32 pairs (FADD2 / FMUL2 / FFMA2
+//    and the SFU lg2 / rcp, the arithmetic of the exact fp32 kernels on the stored floats): per source and target pair
+//    11 packed instructions + 4 MUFU; per-chunk float partial sums folded into double accumulators;
 //  * the own-vesicle exclusion costs no branch: the two SFU results of an excluded pair are replaced by zeros (a
 //    select each), which removes both of its terms -- also for the self pair, whose lg2 / rcp are infinite;
 //  * the leaf's n targets are dealt out evenly: rounds of at most 128 targets, ceil(n_r / 2) slots of two targets,
@@ -1168,28 +982,42 @@ fmm_l2p_p2p(const cplx *__restrict__ zs, const cplx *__restrict__ gs, const int 
 //    column): they are staged as ONE list in chunks of 1,024 sources (a typical neighbourhood in one: measured 3.5 %
 //    faster than 512), two barriers per chunk instead of two per box;
 //  * the far field (Horner of the three local expansions, double) is evaluated by one thread per target, all
-//    threads busy, instead of by every fourth thread.
-// Per-chunk float partial sums are folded into double accumulators as before.
+//    threads busy.
 #ifndef VN_FMM_P2P_CHUNK
 #define VN_FMM_P2P_CHUNK 1024
 #endif
 constexpr int kP2PChunk = VN_FMM_P2P_CHUNK;
+#ifndef VN_FMM_P2P_CHUNK64
+#define VN_FMM_P2P_CHUNK64 256
+#endif
+constexpr int kP2PChunk64 = VN_FMM_P2P_CHUNK64;
+// F64 = true: the same deal of the work for double-precision storage -- a thread's two targets are two independent
+// scalar chains through log_rcp_f64 (its 32 KB of tables in front of the source records, records of (x, y) and
+// (gx, gy) doubles, 512 per chunk), the exclusion again a select on (log, 1 / r^2); sums run in double throughout.
+template <bool F64> __host__ __device__ constexpr int p2p_chunk() { return F64 ? kP2PChunk64 : kP2PChunk; }
+template <bool F64> __host__ __device__ constexpr size_t p2p_smem() { return (F64 ? sizeof(double) * (kLogTab + kExpTab) : 0) + (size_t)p2p_chunk<F64>() * 36; }
+template <bool F64>
 __global__ void __launch_bounds__(128)
-fmm_l2p_p2p_packed(const float4 *__restrict__ srcf, const int *__restrict__ vs,
+fmm_l2p_p2p_packed(const float4 *__restrict__ srcf, const cplx *__restrict__ zs, const cplx *__restrict__ gs,
+                   const double *__restrict__ logtab, const int *__restrict__ vs,
                    const long long *__restrict__ start, const cplx *__restrict__ tz, const int *__restrict__ tvs,
                    const int *__restrict__ tperm, const long long *__restrict__ tstart, int q,
                    const unsigned long long *__restrict__ enc, const cplx *__restrict__ loc, cplx *__restrict__ accum)
 {
-    constexpr int kT = 128;
+    constexpr int kT = 128, kChunk = p2p_chunk<F64>();
     __shared__ cplx lc[3 * kFmmMaxQ];
-    __shared__ float4 sxy[kP2PChunk];                  // (x, x, y, y): both halves of a packed operand
-    __shared__ float4 sgg[kP2PChunk];                  // (gx, gx, gy, gy)
-    __shared__ int sves[kP2PChunk];
+    extern __shared__ __align__(16) unsigned char p2p_sm[];
+    double *tab = reinterpret_cast<double *>(p2p_sm);                                  // F64 only
+    float4 *sxy = reinterpret_cast<float4 *>(p2p_sm + (F64 ? sizeof(double) * (kLogTab + kExpTab) : 0));
+    float4 *sgg = sxy + kChunk;                        // fp32: (x, x, y, y) and (gx, gx, gy, gy), both halves of a packed operand
+    int *sves = reinterpret_cast<int *>(sgg + kChunk); // fp64: the same 16 bytes hold (x, y) and (gx, gy) as doubles
     __shared__ cplx far[kT];
     __shared__ double4 red[kT];
     const int L = load_level(enc);
     const int n = 1 << L;
     const int tid = threadIdx.x;
+    if (F64)
+        for (int e = tid; e < kLogTab + kExpTab; e += kT) tab[e] = logtab[e];      // ordered by the barriers of the first leaf
     const Geom gm = load_geom(enc);
     const double s = gm.size / (double)n, inv_s = 1.0 / s;
     for (int c = blockIdx.x; c < n * n; c += gridDim.x) {
@@ -1245,31 +1073,62 @@ fmm_l2p_p2p_packed(const float4 *__restrict__ srcf, const int *__restrict__ vs,
             }
             // the slot's two targets (a dead second half repeats the first and is never stored)
             u64 zx2 = 0, zy2 = 0;
+            cplx za = make_double2(0.0, 0.0), zb = za;
             int va = -2, vb = -2;
             if (active) {
-                const cplx za = tz[t0 + slot], zb = tz[t0 + (has_b ? slot + slots : slot)];
+                za = tz[t0 + slot];
+                zb = tz[t0 + (has_b ? slot + slots : slot)];
                 zx2 = pk((float)za.x, (float)zb.x);
                 zy2 = pk((float)za.y, (float)zb.y);
                 va = tvs ? tvs[t0 + slot] : -1;
                 vb = has_b ? (tvs ? tvs[t0 + slot + slots] : -1) : -2;
             }
             double uxa = 0.0, uya = 0.0, uxb = 0.0, uyb = 0.0;
-            for (int f0 = 0; f0 < total; f0 += kP2PChunk) {
+            for (int f0 = 0; f0 < total; f0 += kChunk) {
                 __syncthreads();
-                const int cnt = min(kP2PChunk, total - f0);
+                const int cnt = min(kChunk, total - f0);
                 for (int e = tid; e < cnt; e += kT) {
                     int f = f0 + e;
                     long long idx;
                     if (f < clen[0]) idx = cs[0] + f;
                     else if (f < clen[0] + clen[1]) idx = cs[1] + (f - clen[0]);
                     else idx = cs[2] + (f - clen[0] - clen[1]);
-                    const float4 v = srcf[idx];                      // (x, y, gx, gy): the stored values, floats to begin with
-                    sxy[e] = make_float4(v.x, v.x, v.y, v.y);
-                    sgg[e] = make_float4(v.z, v.z, v.w, v.w);
+                    if (F64) {
+                        reinterpret_cast<cplx *>(sxy)[e] = zs[idx];
+                        reinterpret_cast<cplx *>(sgg)[e] = gs[idx];
+                    } else {
+                        const float4 v = srcf[idx];                  // (x, y, gx, gy): the stored values, floats to begin with
+                        sxy[e] = make_float4(v.x, v.x, v.y, v.y);
+                        sgg[e] = make_float4(v.z, v.z, v.w, v.w);
+                    }
                     sves[e] = vs[idx];
                 }
                 __syncthreads();
-                if (active) {
+                if (active && F64) {
+                    for (int j = part; j < cnt; j += split) {
+                        const cplx pz = reinterpret_cast<const cplx *>(sxy)[j], pg = reinterpret_cast<const cplx *>(sgg)[j];
+                        const int sv = sves[j];
+                        {
+                            const double rx = za.x - pz.x, ry = za.y - pz.y;
+                            double ml, inv;
+                            log_rcp_f64(fma(rx, rx, ry * ry), tab, ml, inv);
+                            if (sv == va) { ml = 0.0; inv = 0.0; }
+                            const double qd = fma(rx, pg.x, ry * pg.y) * inv;
+                            uxa = fma(ml, pg.x, fma(qd, rx, uxa));
+                            uya = fma(ml, pg.y, fma(qd, ry, uya));
+                        }
+                        {
+                            const double rx = zb.x - pz.x, ry = zb.y - pz.y;
+                            double ml, inv;
+                            log_rcp_f64(fma(rx, rx, ry * ry), tab, ml, inv);
+                            if (sv == vb) { ml = 0.0; inv = 0.0; }
+                            const double qd = fma(rx, pg.x, ry * pg.y) * inv;
+                            uxb = fma(ml, pg.x, fma(qd, rx, uxb));
+                            uyb = fma(ml, pg.y, fma(qd, ry, uyb));
+                        }
+                    }
+                }
+                if (active && !F64) {
                     u64 fxl = 0, fyl = 0, fxq = 0, fyq = 0;           // packed (a, b): sum lg2 g  and  sum qd r
 #pragma unroll 2
                     for (int j = part; j < cnt; j += split) {
@@ -1455,6 +1314,18 @@ struct FmmTimer {
 #define FMM_TICK(what) ((void)0)
 #endif
 
+// the double-precision direct part keeps the 32 KB log tables next to its source records: beyond the 48 KB default
+static vn_status p2p_f64_prepare()
+{
+    static bool done_dev[kMaxDevices] = {false};
+    bool &done = done_dev[current_device()];
+    if (!done) {
+        VN_CUDA(cudaFuncSetAttribute(fmm_l2p_p2p_packed<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p2p_smem<true>()));
+        done = true;
+    }
+    return VN_OK;
+}
+
 static int fmm_levels_max(long long P)
 {
     // the deepest tree the device may choose: leaves of kLeafTarget points if only 1/16 of the root square is occupied
@@ -1517,10 +1388,7 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
     const int p2p_grid = ncell < 148 * 64 ? ncell : 148 * 64;      // grid-stride over the leaves the device chose
     FMM_TICK("tables");
     profile_mark(st, true);
-    if (q <= kM2LHalfQ)
-        fmm_p2m_half<<<(ncell + kP2MWarps - 1) / kP2MWarps < 148 * 16 ? (ncell + kP2MWarps - 1) / kP2MWarps : 148 * 16, 32 * kP2MWarps, p2m_half_smem(q), st>>>(zs, gs, start, q, enc, mult, boxcnt);
-    else
-        fmm_p2m<<<(ncell + 3) / 4, 128, 0, st>>>(zs, gs, start, q, enc, mult, boxcnt);
+    fmm_p2m<<<(ncell + kP2MWarps - 1) / kP2MWarps < 148 * 16 ? (ncell + kP2MWarps - 1) / kP2MWarps : 148 * 16, 32 * kP2MWarps, 0, st>>>(zs, gs, start, q, enc, mult, boxcnt);
     ++launches;
     FMM_TICK("p2m");
     const int resident = L >= 3 ? shift_resident_blocks(q) : 1;     // also opts the two kernels into their shared memory
@@ -1555,9 +1423,9 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
     }
     FMM_TICK("l2l");
     if (prec == VN_F32)
-        fmm_l2p_p2p_packed<<<p2p_grid, 128, 0, st>>>(srcf, vs, start, zs, vs, perm, start, q, enc, loc, accum);
-    else
-        fmm_l2p_p2p<false><<<p2p_grid, kP2PThreads, 0, st>>>(zs, gs, vs, start, zs, vs, perm, start, q, enc, loc, logtab, accum);
+        fmm_l2p_p2p_packed<false><<<p2p_grid, 128, p2p_smem<false>(), st>>>(srcf, zs, gs, logtab, vs, start, zs, vs, perm, start, q, enc, loc, accum);
+    else if (p2p_f64_prepare() == VN_OK)
+        fmm_l2p_p2p_packed<true><<<p2p_grid, 128, p2p_smem<true>(), st>>>(srcf, zs, gs, logtab, vs, start, zs, vs, perm, start, q, enc, loc, accum);
     profile_mark(st, false);
     FMM_TICK("l2p+p2p");
     if (near_ptr) {   // row f-1 on top: take the near vesicles' contributions out (they are all in the direct part)
@@ -1683,10 +1551,7 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
 
     const int p2p_grid = ncell < 148 * 64 ? ncell : 148 * 64;      // grid-stride over the leaves the device chose
     profile_mark(st, true);
-    if (q <= kM2LHalfQ)
-        fmm_p2m_half<<<(ncell + kP2MWarps - 1) / kP2MWarps < 148 * 16 ? (ncell + kP2MWarps - 1) / kP2MWarps : 148 * 16, 32 * kP2MWarps, p2m_half_smem(q), st>>>(zs, gs, start, q, enc, mult, boxcnt);
-    else
-        fmm_p2m<<<(ncell + 3) / 4, 128, 0, st>>>(zs, gs, start, q, enc, mult, boxcnt);
+    fmm_p2m<<<(ncell + kP2MWarps - 1) / kP2MWarps < 148 * 16 ? (ncell + kP2MWarps - 1) / kP2MWarps : 148 * 16, 32 * kP2MWarps, 0, st>>>(zs, gs, start, q, enc, mult, boxcnt);
     ++launches;
     const int resident = L >= 3 ? shift_resident_blocks(q) : 1;     // also opts the two kernels into their shared memory
     if (L >= 3) {     // the level above the leaves with a full grid, all levels above it in one launch of resident blocks
@@ -1717,9 +1582,9 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
         ++launches;
     }
     if (prec == VN_F32)
-        fmm_l2p_p2p_packed<<<p2p_grid, 128, 0, st>>>(srcf, vs, start, zts, nullptr, tperm, tstart, q, enc, loc, accum);
-    else
-        fmm_l2p_p2p<false><<<p2p_grid, kP2PThreads, 0, st>>>(zs, gs, vs, start, zts, nullptr, tperm, tstart, q, enc, loc, logtab, accum);
+        fmm_l2p_p2p_packed<false><<<p2p_grid, 128, p2p_smem<false>(), st>>>(srcf, zs, gs, logtab, vs, start, zts, nullptr, tperm, tstart, q, enc, loc, accum);
+    else if (p2p_f64_prepare() == VN_OK)
+        fmm_l2p_p2p_packed<true><<<p2p_grid, 128, p2p_smem<true>(), st>>>(srcf, zs, gs, logtab, vs, start, zts, nullptr, tperm, tstart, q, enc, loc, accum);
     profile_mark(st, false);
     const double pref = 1.0 / (4.0 * 3.14159265358979323846 * mu);
     if (prec == VN_F32)
