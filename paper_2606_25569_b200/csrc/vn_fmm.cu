@@ -593,6 +593,24 @@ static int shift_resident_blocks(int q)
     }
     return blocks_dev[d];
 }
+// The multi-level launches go through the cooperative-launch attribute: the driver then starts the grid only when all
+// of its blocks fit at once -- also next to kernels of other streams -- which is what grid_barrier needs (a plain
+// launch of a correctly sized grid is safe only as long as nothing else occupies the device).
+template <typename... Params, typename... Args>
+static cudaError_t launch_resident(void (*kernel)(Params...), int blocks, size_t smem, cudaStream_t st, Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)blocks);
+    cfg.blockDim = dim3(kShiftThreads);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeCooperative;
+    attr[0].val.cooperative = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, static_cast<Params>(args)...);
+}
 static size_t shift_smem(int q) { return sizeof(cplx) * (size_t)(24 * q + (q <= kShiftStageQ ? 4 * q * q : 0)); }
 
 // ------------------------------------------------------------------------------------------------
@@ -1397,7 +1415,7 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
         fmm_m2m<<<nb < 148u * kShiftWave ? nb : 148u * kShiftWave, kShiftThreads, shift_smem(q), st>>>(1, 1, q, tab, enc, mult, boxcnt);
         ++launches;
         if (L >= 4) {
-            fmm_m2m<<<resident, kShiftThreads, shift_smem(q), st>>>(2, 99, q, tab, enc, mult, boxcnt);
+            (void)launch_resident(fmm_m2m, resident, shift_smem(q), st, 2, 99, q, tab, enc, mult, boxcnt);
             ++launches;
         }
     }
@@ -1414,7 +1432,7 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
     FMM_TICK("m2l");
     if (L >= 3) {     // levels 3 .. L - 1 in one launch of resident blocks, the leaf level with a full grid
         if (L >= 4) {
-            fmm_l2l<<<resident, kShiftThreads, shift_smem(q), st>>>(99, 1, q, tab, enc, boxcnt, loc);
+            (void)launch_resident(fmm_l2l, resident, shift_smem(q), st, 99, 1, q, tab, enc, boxcnt, loc);
             ++launches;
         }
         const unsigned nb = 1u << (2 * (L - 1));
@@ -1559,7 +1577,7 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
         fmm_m2m<<<nb < 148u * kShiftWave ? nb : 148u * kShiftWave, kShiftThreads, shift_smem(q), st>>>(1, 1, q, tab, enc, mult, boxcnt);
         ++launches;
         if (L >= 4) {
-            fmm_m2m<<<resident, kShiftThreads, shift_smem(q), st>>>(2, 99, q, tab, enc, mult, boxcnt);
+            (void)launch_resident(fmm_m2m, resident, shift_smem(q), st, 2, 99, q, tab, enc, mult, boxcnt);
             ++launches;
         }
     }
@@ -1574,7 +1592,7 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
     }
     if (L >= 3) {     // levels 3 .. L - 1 in one launch of resident blocks, the leaf level with a full grid
         if (L >= 4) {
-            fmm_l2l<<<resident, kShiftThreads, shift_smem(q), st>>>(99, 1, q, tab, enc, nullptr, loc);
+            (void)launch_resident(fmm_l2l, resident, shift_smem(q), st, 99, 1, q, tab, enc, (const int *)nullptr, loc);
             ++launches;
         }
         const unsigned nb = 1u << (2 * (L - 1));

@@ -530,6 +530,29 @@ def test_fmm_orders_across_the_kernel_switch_single_precision():
     assert all(errs[o] <= TOL[np.float32] for o in (14, 15, 16, 17, 18))
 
 
+@pytest.mark.parametrize("dtype,order", [(np.float32, 14), (np.float64, 38)])
+def test_fmm_calls_on_two_streams_at_once(dtype, order):
+    """The multi-level M2M / L2L launches hold a grid barrier, i.e. need all their blocks resident at once; they are
+    launched with the cooperative attribute, so two evaluations in flight on two streams must neither deadlock nor
+    disturb each other (at p = 38 one such grid fills the device)."""
+    s = inputs.config(2)
+    W = oracle.weights(s.X)
+    Xd, Fd, Wd = dev(s.X, dtype), dev(s.F, dtype), dev(W, dtype)
+    F2 = Fd.flip(0).contiguous()
+    ref1 = vn.vn_farfield_fmm(Xd, Fd, Wd, s.mu, order).clone()
+    ref2 = vn.vn_farfield_fmm(Xd, F2, Wd, s.mu, order).clone()
+    torch.cuda.synchronize()
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    out1, out2 = torch.empty_like(ref1), torch.empty_like(ref2)
+    for _ in range(5):
+        with torch.cuda.stream(s1):
+            vn.vn_farfield_fmm(Xd, Fd, Wd, s.mu, order, out=out1)
+        with torch.cuda.stream(s2):
+            vn.vn_farfield_fmm(Xd, F2, Wd, s.mu, order, out=out2)
+    torch.cuda.synchronize()
+    assert torch.equal(out1, ref1) and torch.equal(out2, ref2)
+
+
 def test_fmm_single_vesicle_gives_zero():
     rng = np.random.Generator(np.random.PCG64(5))
     X = rng.normal(size=(1, 700, 2)); F = rng.normal(size=(1, 700, 2)); W = rng.uniform(0.5, 1.5, size=(1, 700))
