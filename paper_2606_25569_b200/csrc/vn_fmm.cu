@@ -170,14 +170,21 @@ __device__ __forceinline__ void bounds_commit(double x, double y, double X1, dou
 }
 constexpr int kLoadBlocks = 148 * 8;      // grid-stride: at most this many blocks commit a bounding box
 
+__device__ void fmm_build_tables(int block, int q, double *base, double *logtab);
+
 // positions and densities g = F*W promoted to double (original order), and the bounding box
 template <typename real, typename real2>
 __global__ void __launch_bounds__(256)
 fmm_load(const real2 *__restrict__ X, const real2 *__restrict__ F, const real *__restrict__ W, int P,
-         cplx *__restrict__ z, cplx *__restrict__ g, unsigned long long *enc, unsigned tickets, int P_level, int L_hi)
-{
+         cplx *__restrict__ z, cplx *__restrict__ g, unsigned long long *enc, unsigned tickets, int P_level, int L_hi,
+         int load_blocks, int q, double *tab, double *logtab)
+{   // blocks load_blocks .. gridDim.x - 1 build the translation tables (fmm_build_tables) and touch no point
+    if ((int)blockIdx.x >= load_blocks) {
+        fmm_build_tables((int)blockIdx.x - load_blocks, q, tab, logtab);
+        return;
+    }
     double x = INFINITY, y = INFINITY, X1 = -INFINITY, Y1 = -INFINITY;
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < P; i += gridDim.x * blockDim.x) {
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < P; i += load_blocks * blockDim.x) {
         const real2 p = X[i];
         const real2 f = F[i];
         const real w = W[i];
@@ -224,11 +231,32 @@ fmm_scatter(const int *__restrict__ cell, int P, long long *__restrict__ cursor,
 // the atomic scatter leaves every leaf's points in arbitrary order: order each segment by point index so that
 // every later sum runs in a fixed order (bitwise reproducible results).  One warp per leaf, rank sort: the
 // indices of a segment are distinct, so the rank of an entry is the number of smaller ones.
+// ... and the leaf's points are gathered into the sorted arrays by the warp that has just sorted them (no launch of
+// its own, no second pass over perm): sources (z, g -> zs, gs, vesicle index vs, float record srcf) or free targets.
+struct GatherArgs {
+    const cplx *z, *g;          // original order (g == nullptr: free targets, positions only)
+    cplx *zs, *gs;
+    int *vs;
+    float4 *srcf;               // nullable
+    int npts;
+};
+__device__ __forceinline__ void gather_one(const GatherArgs &ga, long long pos, int i)
+{
+    const cplx zi = ga.z[i];
+    ga.zs[pos] = zi;
+    if (ga.g) {
+        const cplx gi = ga.g[i];
+        ga.gs[pos] = gi;
+        ga.vs[pos] = i / ga.npts;
+        if (ga.srcf) ga.srcf[pos] = make_float4((float)zi.x, (float)zi.y, (float)gi.x, (float)gi.y);
+    }
+}
 __global__ void __launch_bounds__(128)
 fmm_sort_cells(const long long *__restrict__ start, const unsigned long long *__restrict__ enc,
-               const int *__restrict__ unsorted, int *__restrict__ perm)
+               const int *unsorted, int *__restrict__ perm, GatherArgs ga)
 {   // the leaves of the level the device chose, walked with a grid stride: a grid sized for the deepest admissible
-    // tree is mostly blocks without a leaf (61 K of 65 K at a million points), and scheduling those cost 40 us
+    // tree is mostly blocks without a leaf (61 K of 65 K at a million points), and scheduling those cost 40 us.
+    // `unsorted` may be ga.vs (the sources' scatter buffer): a leaf's entries are all read before any is written.
     constexpr int kBuf = 256;                          // leaves up to this size are sorted in shared memory
     __shared__ int buf[4][kBuf];
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -237,7 +265,11 @@ fmm_sort_cells(const long long *__restrict__ start, const unsigned long long *__
     const long long a = start[c], b = start[c + 1];
     const int m = (int)(b - a);
     if (m <= 1) {
-        if (m == 1 && lane == 0) perm[a] = unsorted[a];
+        if (m == 1 && lane == 0) {
+            const int v = unsorted[a];
+            perm[a] = v;
+            gather_one(ga, a, v);
+        }
         continue;
     }
     __syncwarp();                                      // the previous leaf's buffer is written out
@@ -258,7 +290,11 @@ fmm_sort_cells(const long long *__restrict__ start, const unsigned long long *__
                 }
                 __syncwarp();
             }
-        for (int i = lane; i < m; i += 32) perm[a + i] = buf[w][i];
+        for (int i = lane; i < m; i += 32) {
+            const int v = buf[w][i];
+            perm[a + i] = v;
+            gather_one(ga, a + i, v);
+        }
         continue;
     }
     for (long long i = a + lane; i < b; i += 32) {
@@ -267,22 +303,11 @@ fmm_sort_cells(const long long *__restrict__ start, const unsigned long long *__
         for (long long j = a; j < b; ++j) rank += unsorted[j] < v;
         perm[a + rank] = v;
     }
+    __syncwarp();                                      // the leaf's perm is complete (and `unsorted` no longer read)
+    for (long long i = a + lane; i < b; i += 32) gather_one(ga, i, perm[i]);
     }   // leaves
 }
 
-__global__ void __launch_bounds__(256)
-fmm_gather(const int *__restrict__ perm, int P, int npts, const cplx *__restrict__ z, const cplx *__restrict__ g,
-           cplx *__restrict__ zs, cplx *__restrict__ gs, int *__restrict__ vs, float4 *__restrict__ srcf)
-{   // srcf (single-precision storage only): the source record (x, y, gx, gy) of the direct part, as floats again
-    const int q = blockIdx.x * blockDim.x + threadIdx.x;
-    if (q >= P) return;
-    const int i = perm[q];
-    const cplx zi = z[i], gi = g[i];
-    zs[q] = zi;
-    gs[q] = gi;
-    vs[q] = i / npts;
-    if (srcf) srcf[q] = make_float4((float)zi.x, (float)zi.y, (float)gi.x, (float)gi.y);
-}
 
 // ------------------------------------------------------------------------------------------------
 // translation tables for order p (q = p + 1 coefficients), built once per call on the device:
@@ -295,7 +320,8 @@ fmm_gather(const int *__restrict__ perm, int P, int npts, const cplx *__restrict
 //     [0][k] = rho^k / k (k >= 1), 1 (k = 0)   [1][k] = rho^k        (scaling of the source's moments)
 //     [2][l] = -(-1)^l rho^l (l >= 1), -1 (l = 0)      [3][l] = [2][l] / l (l >= 1), -lrho (l = 0)      [4][l] = (-1)^l rho^(l+1)
 // delta_c = ((a - 1/2) + i (b - 1/2)) / 2 is the child's centre in the parent's scaled variable, c = 2 a + b.
-constexpr int kTableBlocks = 64;
+constexpr int kTableBlocks = 32;        // of 256 threads (fmm_load's block size)
+constexpr int kLogTabBlocks = 4;
 struct FmmTables {
     double *Cb;
     cplx *S, *T, *rho, *lrho, *coef;
@@ -325,15 +351,18 @@ __device__ __forceinline__ cplx cpowi(cplx a, int n)
     for (int i = 0; i < n; ++i) r = cmul(r, a);
     return r;
 }
-__global__ void fmm_build_tables(int q, double *base, double *logtab)
-{   // blocks beyond kTableBlocks (launched only when logtab is wanted: double-precision storage) build the two tables
-    // of log_rcp_f64 in global memory, which every block of the direct part copies to its shared memory
-    if (blockIdx.x >= kTableBlocks) {
-        build_log_tables(logtab, (blockIdx.x - kTableBlocks) * blockDim.x + threadIdx.x, (gridDim.x - kTableBlocks) * blockDim.x);
+// Run by kTableBlocks (+ kLogTabBlocks) extra blocks of fmm_load -- the tables depend on the order only, so they
+// are built beside the first pass over the points instead of in a launch of their own; `block` counts from 0.
+// Blocks beyond kTableBlocks (present only when logtab is wanted: double-precision storage) build the two tables
+// of log_rcp_f64 in global memory, which every block of the direct part copies to its shared memory.
+__device__ void fmm_build_tables(int block, int q, double *base, double *logtab)
+{
+    if (block >= kTableBlocks) {
+        build_log_tables(logtab, (block - kTableBlocks) * blockDim.x + threadIdx.x, kLogTabBlocks * blockDim.x);
         return;
     }
     const FmmTables t = fmm_tables_at(base, q);
-    const int nthreads = kTableBlocks * blockDim.x, tid = blockIdx.x * blockDim.x + threadIdx.x;
+    const int nthreads = kTableBlocks * blockDim.x, tid = block * blockDim.x + threadIdx.x;
     for (int e = tid; e < q * q; e += nthreads) {
         const int n = e / q, l = e % q;
         t.Cb[e] = binom(n + l, l);
@@ -1387,9 +1416,9 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
     VN_CUDA(cudaMemsetAsync(enc, 0, 256 + b_cnt + b_leaf, st));   // the bounding box, boxcnt and the leaf counts are adjacent
     const int gp = (P + 255) / 256, gl = gp < kLoadBlocks ? gp : kLoadBlocks;
     if (prec == VN_F32)                                            // the last block to finish also fixes level and centre
-        fmm_load<float, float2><<<gl, 256, 0, st>>>((const float2 *)X, (const float2 *)F, (const float *)W, P, z, g, enc, gl, P, L);
-    else
-        fmm_load<double, double2><<<gl, 256, 0, st>>>((const double2 *)X, (const double2 *)F, (const double *)W, P, z, g, enc, gl, P, L);
+        fmm_load<float, float2><<<gl + kTableBlocks, 256, 0, st>>>((const float2 *)X, (const float2 *)F, (const float *)W, P, z, g, enc, gl, P, L, gl, q, tab, nullptr);
+    else                                                           // log tables: double only
+        fmm_load<double, double2><<<gl + kTableBlocks + kLogTabBlocks, 256, 0, st>>>((const double2 *)X, (const double2 *)F, (const double *)W, P, z, g, enc, gl, P, L, gl, q, tab, logtab);
     FMM_TICK("load");
     fmm_bin<<<gp, 256, 0, st>>>(z, P, enc, cell, cnt);
     scan_block_sums<<<nb_scan, kScanThreads, 0, st>>>(cnt, ncell, bsum);
@@ -1397,11 +1426,12 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
     scan_apply<<<nb_scan, kScanThreads, 0, st>>>(cnt, ncell, bsum, start, cursor);
     FMM_TICK("bin+scan");
     fmm_scatter<<<gp, 256, 0, st>>>(cell, P, cursor, vs);                  // vs doubles as the unsorted buffer
-    fmm_sort_cells<<<(ncell + 3) / 4 < 148 * 16 ? (ncell + 3) / 4 : 148 * 16, 128, 0, st>>>(start, enc, vs, perm);
-    fmm_gather<<<gp, 256, 0, st>>>(perm, P, (int)npts, z, g, zs, gs, vs, prec == VN_F32 ? srcf : nullptr);
+    {
+        const GatherArgs ga = {z, g, zs, gs, vs, prec == VN_F32 ? srcf : nullptr, (int)npts};
+        fmm_sort_cells<<<(ncell + 3) / 4 < 148 * 16 ? (ncell + 3) / 4 : 148 * 16, 128, 0, st>>>(start, enc, vs, perm, ga);
+    }
     FMM_TICK("sort+gather");
-    fmm_build_tables<<<kTableBlocks + (prec == VN_F32 ? 0 : 8), 128, 0, st>>>(q, tab, logtab);   // log tables: double only
-    int launches = 10;
+    int launches = 8;
 
     const int p2p_grid = ncell < 148 * 64 ? ncell : 148 * 64;      // grid-stride over the leaves the device chose
     FMM_TICK("tables");
@@ -1484,12 +1514,6 @@ fmm_load_targets(const real2 *__restrict__ Xt, int nt, cplx *__restrict__ zt, un
     bounds_commit(x, y, X1, Y1, enc, tickets, P_level, L_hi);
 }
 
-__global__ void __launch_bounds__(256)
-fmm_gather_targets(const int *__restrict__ perm, int nt, const cplx *__restrict__ zt, cplx *__restrict__ zts)
-{
-    const int q = blockIdx.x * blockDim.x + threadIdx.x;
-    if (q < nt) zts[q] = zt[perm[q]];
-}
 
 template <typename real2>
 __global__ void __launch_bounds__(256)
@@ -1542,10 +1566,10 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
     const int Plev = P > nt ? P : nt;
     // sources and targets share one box: the last block of the two kernels together fixes level and centre
     if (prec == VN_F32) {
-        fmm_load<float, float2><<<gl, 256, 0, st>>>((const float2 *)X, (const float2 *)F, (const float *)W, P, z, g, enc, gl + glt, Plev, L);
+        fmm_load<float, float2><<<gl + kTableBlocks, 256, 0, st>>>((const float2 *)X, (const float2 *)F, (const float *)W, P, z, g, enc, gl + glt, Plev, L, gl, q, tab, nullptr);
         fmm_load_targets<float2><<<glt, 256, 0, st>>>((const float2 *)Xt, nt, zt, enc, gl + glt, Plev, L);
     } else {
-        fmm_load<double, double2><<<gl, 256, 0, st>>>((const double2 *)X, (const double2 *)F, (const double *)W, P, z, g, enc, gl + glt, Plev, L);
+        fmm_load<double, double2><<<gl + kTableBlocks + kLogTabBlocks, 256, 0, st>>>((const double2 *)X, (const double2 *)F, (const double *)W, P, z, g, enc, gl + glt, Plev, L, gl, q, tab, logtab);
         fmm_load_targets<double2><<<glt, 256, 0, st>>>((const double2 *)Xt, nt, zt, enc, gl + glt, Plev, L);
     }
     // sources into leaves
@@ -1554,18 +1578,21 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
     scan_of_sums<<<1, kScanThreads, 0, st>>>(bsum, nb_scan);
     scan_apply<<<nb_scan, kScanThreads, 0, st>>>(cnt, ncell, bsum, start, cursor);
     fmm_scatter<<<gp, 256, 0, st>>>(cell, P, cursor, vs);                  // vs doubles as the unsorted buffer
-    fmm_sort_cells<<<(ncell + 3) / 4 < 148 * 16 ? (ncell + 3) / 4 : 148 * 16, 128, 0, st>>>(start, enc, vs, perm);
-    fmm_gather<<<gp, 256, 0, st>>>(perm, P, (int)npts, z, g, zs, gs, vs, prec == VN_F32 ? srcf : nullptr);
+    {
+        const GatherArgs ga = {z, g, zs, gs, vs, prec == VN_F32 ? srcf : nullptr, (int)npts};
+        fmm_sort_cells<<<(ncell + 3) / 4 < 148 * 16 ? (ncell + 3) / 4 : 148 * 16, 128, 0, st>>>(start, enc, vs, perm, ga);
+    }
     // targets into the same leaves
     fmm_bin<<<gt, 256, 0, st>>>(zt, nt, enc, tcell, tcnt);
     scan_block_sums<<<nb_scan, kScanThreads, 0, st>>>(tcnt, ncell, bsum);
     scan_of_sums<<<1, kScanThreads, 0, st>>>(bsum, nb_scan);
     scan_apply<<<nb_scan, kScanThreads, 0, st>>>(tcnt, ncell, bsum, tstart, tcursor);
     fmm_scatter<<<gt, 256, 0, st>>>(tcell, nt, tcursor, (int *)accum);     // accum doubles as the unsorted buffer
-    fmm_sort_cells<<<(ncell + 3) / 4 < 148 * 16 ? (ncell + 3) / 4 : 148 * 16, 128, 0, st>>>(tstart, enc, (const int *)accum, tperm);
-    fmm_gather_targets<<<gt, 256, 0, st>>>(tperm, nt, zt, zts);
-    fmm_build_tables<<<kTableBlocks + (prec == VN_F32 ? 0 : 8), 128, 0, st>>>(q, tab, logtab);   // log tables: double only
-    int launches = 18;
+    {
+        const GatherArgs ga = {zt, nullptr, zts, nullptr, nullptr, nullptr, 1};
+        fmm_sort_cells<<<(ncell + 3) / 4 < 148 * 16 ? (ncell + 3) / 4 : 148 * 16, 128, 0, st>>>(tstart, enc, (const int *)accum, tperm, ga);
+    }
+    int launches = 15;
 
     const int p2p_grid = ncell < 148 * 64 ? ncell : 148 * 64;      // grid-stride over the leaves the device chose
     profile_mark(st, true);
