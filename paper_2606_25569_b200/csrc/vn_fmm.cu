@@ -537,6 +537,30 @@ __device__ __forceinline__ void grid_barrier(unsigned long long *counter, unsign
     }
     __syncthreads();
 }
+constexpr int kM2MPre = (12 * kFmmMaxQ + kShiftThreads - 1) / kShiftThreads;   // children's coefficients per thread
+__device__ __forceinline__ void m2m_prefetch(cplx (&pre)[kM2MPre], int &pre_cnt, int box, int nn, int n, int level, int q,
+                                             int tid, const cplx *mult, const int *boxcnt)
+{
+    if (box >= nn) return;
+    const int ix = box / n, iy = box % n;
+    const long long child0 = level_offset(level + 1) + (long long)(2 * ix) * (2 * n) + 2 * iy;   // child c = 2 a + b at child0 + a * 2n + b
+#pragma unroll
+    for (int r = 0; r < kM2MPre; ++r) {
+        const int e = min(tid + r * kShiftThreads, 12 * q - 1);     // surplus slots reload the last element (never stored)
+        const int c = e / (3 * q);
+        pre[r] = ldcg_cplx(mult + (child0 + (long long)(c >> 1) * (2 * n) + (c & 1)) * (long long)(3 * q) + (e - c * 3 * q));
+    }
+    if (tid < 4) pre_cnt = __ldcg(boxcnt + child0 + (long long)(tid >> 1) * (2 * n) + (tid & 1));
+}
+__device__ __forceinline__ void m2m_commit(const cplx (&pre)[kM2MPre], int pre_cnt, int q, int tid, cplx *ch, int *scnt)
+{   // the prefetched box becomes the current one
+#pragma unroll
+    for (int r = 0; r < kM2MPre; ++r) {
+        const int e = tid + r * kShiftThreads;
+        if (e < 12 * q) ch[e] = pre[r];
+    }
+    if (tid < 4) scnt[tid] = pre_cnt;
+}
 // levels L - d_first, L - d_first - 1, ..., max(L - d_last, 2)  (L = the tree's depth, chosen on the device)
 __global__ void __launch_bounds__(kShiftThreads)
 fmm_m2m(int d_first, int d_last, int q, const double *__restrict__ tab, unsigned long long *enc,
@@ -561,22 +585,23 @@ fmm_m2m(int d_first, int d_last, int q, const double *__restrict__ tab, unsigned
     unsigned long long arrivals = 0;
     for (int level = L - d_first; level >= 2 && level >= L - d_last; --level) {
     if (level != L - d_first) grid_barrier(enc + 9, arrivals += gridDim.x);   // the level below is complete
-    const int n = 1 << level;
-    for (int box = blockIdx.x; box < n * n; box += gridDim.x) {
-        const int ix = box / n, iy = box % n;
-        const long long child0 = level_offset(level + 1) + (long long)(2 * ix) * (2 * n) + 2 * iy;
-        // children c = 2 a + b sit at child0 + a * 2n + b
-        __syncthreads();                                             // the previous box is written out
-        if (tid < 4) scnt[tid] = __ldcg(boxcnt + child0 + (long long)(tid >> 1) * (2 * n) + (tid & 1));
-        __syncthreads();
-        for (int c = 0; c < 4; ++c)                                  // children without sources are skipped below, not staged
-            if (scnt[c] != 0)
-                stage_cplx(ch + c * 3 * q, mult + (child0 + (long long)(c >> 1) * (2 * n) + (c & 1)) * (long long)(3 * q), tid, kShiftThreads, 3 * q);
-        __syncthreads();
+    const int n = 1 << level, nn = n * n;
+    // The block's boxes one after the other, the NEXT box's children (and their counts) in flight while this one is
+    // computed: per box two barriers and no exposed round trip to L2 (the first version waited for the counts, then
+    // for the children, then wrote: 2.6 us per box, 18 us for the 4,096 parents above a million points' leaves).
+    // Children without sources hold zero moments (fmm_p2m and this kernel write them): all four are always loaded.
+    cplx pre[kM2MPre] = {};
+    int pre_cnt = 0;
+    __syncthreads();                                                 // the previous level's last box is written out
+    m2m_prefetch(pre, pre_cnt, blockIdx.x, nn, n, level, q, tid, mult, boxcnt);
+    m2m_commit(pre, pre_cnt, q, tid, ch, scnt);
+    __syncthreads();
+    for (int box = blockIdx.x; box < nn; box += gridDim.x) {
+        m2m_prefetch(pre, pre_cnt, box + gridDim.x, nn, n, level, q, tid, mult, boxcnt);
         for (int w = tid; w < 12 * q; w += kShiftThreads) {
             const int c = w / (3 * q), k = w % q;                    // w = (c * 3 + a) * q + k
             cplx s0 = make_double2(0.0, 0.0), s1 = s0;               // two chains: even and odd m
-            if (scnt[c] != 0) {
+            if (scnt[c] != 0) {                                      // a child without sources adds nothing (a 4:1 channel: most)
                 const cplx *A = ch + (w - k);
                 const cplx *col = Stab + (size_t)c * q * q + k;
                 int m = 0;
@@ -588,11 +613,14 @@ fmm_m2m(int d_first, int d_last, int q, const double *__restrict__ tab, unsigned
             }
             part[w] = cadd(s0, s1);
         }
-        __syncthreads();
+        const int cnt_box = scnt[0] + scnt[1] + scnt[2] + scnt[3];
+        __syncthreads();                                             // part is complete, ch and scnt are consumed
         cplx *out = mult + (level_offset(level) + box) * (long long)(3 * q);
         for (int e = tid; e < 3 * q; e += kShiftThreads)
             out[e] = cadd(cadd(part[e], part[3 * q + e]), cadd(part[6 * q + e], part[9 * q + e]));
-        if (tid == 0) boxcnt[level_offset(level) + box] = scnt[0] + scnt[1] + scnt[2] + scnt[3];
+        if (tid == 0) boxcnt[level_offset(level) + box] = cnt_box;
+        m2m_commit(pre, pre_cnt, q, tid, ch, scnt);
+        __syncthreads();                                             // ch holds the next box, part is consumed
     }
     }   // levels
 }
