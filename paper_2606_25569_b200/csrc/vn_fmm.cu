@@ -1426,6 +1426,9 @@ vn_status farfield_fmm(const void *X, const void *F, const void *W, int64_t nves
     const size_t total = 6 * b_pt + 3 * b_int + 2 * b_exp + b_cnt + b_leaf + 2 * b_start + b_bs + b_tab + b_log + 256;
     char *scr = nullptr;
     VN_CUDA(cudaMallocAsync((void **)&scr, total, st));
+#ifdef VN_FMM_POISON    // diagnostic builds: every byte of scratch 0xFF (NaN) before use -- a read of something no kernel wrote shows in U
+    VN_CUDA(cudaMemsetAsync(scr, 0xFF, total, st));
+#endif
     char *ptr = scr;
     auto take = [&](size_t b) { char *r = ptr; ptr += b; return r; };
     cplx *z = (cplx *)take(b_pt), *g = (cplx *)take(b_pt), *zs = (cplx *)take(b_pt), *gs = (cplx *)take(b_pt);
@@ -1574,6 +1577,9 @@ vn_status farfield_targets_fmm(const void *Xt, int64_t nt64, const void *X, cons
                          b_bs + b_tab + b_log + 256;
     char *scr = nullptr;
     VN_CUDA(cudaMallocAsync((void **)&scr, total, st));
+#ifdef VN_FMM_POISON    // diagnostic builds: every byte of scratch 0xFF (NaN) before use -- a read of something no kernel wrote shows in U
+    VN_CUDA(cudaMemsetAsync(scr, 0xFF, total, st));
+#endif
     char *ptr = scr;
     auto take = [&](size_t b) { char *r = ptr; ptr += b; return r; };
     cplx *z = (cplx *)take(b_pt), *g = (cplx *)take(b_pt), *zs = (cplx *)take(b_pt), *gs = (cplx *)take(b_pt);
