@@ -165,7 +165,9 @@ vn_status vn_farfield_targets(const void *Xt, int64_t nt,
  * The expansions are double for both storage precisions; the direct part over neighbouring leaves runs
  * in the storage precision (VN_F32: the same SFU pair arithmetic as vn_farfield, error about 1e-6).  Uniform quadtree over the bounding square of the points; a strongly
  * non-uniform point distribution costs time (crowded leaves), not accuracy.  Results are bitwise
- * reproducible.  Scratch: about 100 * (p+1) bytes per leaf box plus 100 bytes per point.
+ * reproducible.  Scratch: about 100 * (p+1) bytes per leaf box plus 120 bytes per point.  Stream-ordered and
+ * capturable into a graph like the other calls; two of its kernels hold a grid-wide barrier and are launched with
+ * the cooperative attribute (calls in flight on several streams at once are safe).
  * near_ptr / near_ves: NULL for the plain sum (vn_farfield's quantity), or the CSR near-field
  * relation of vn_near_pairs: then the listed vesicles' contributions are zeroed as in
  * vn_farfield_masked (the paper's DirectSingleLayerIntegral in O(P)). */
