@@ -432,3 +432,37 @@ def test_ring_selfcheck_is_clean(case, dtype):
     ref = vn.vn_farfield_finish(acc, gmax, X.shape[0] * X.shape[1], Xd.dtype, mu).view_as(U)
     torch.cuda.synchronize()
     assert torch.equal(U, ref)
+
+
+def test_prepared_calls_equal_the_plain_binding():
+    """prepare_arclength_weights / prepare_farfield marshal once; every call must be the plain binding's result, on
+    the current stream and on another one."""
+    s, _ = problem(1)
+    X = dev(s.X, np.float32)
+    F = dev(s.F, np.float32)
+    W = torch.empty(X.shape[:2], dtype=X.dtype, device=X.device)
+    U = torch.empty_like(X)
+    w = vn.prepare_arclength_weights(X, W)
+    f = vn.prepare_farfield(X, F, W, U, s.mu)
+    assert w() is W and f() is U
+    torch.cuda.synchronize()
+    W_ref = vn.vn_arclength_weights(X)
+    U_ref = vn.vn_farfield(X, F, W_ref, s.mu)
+    torch.cuda.synchronize()
+    assert torch.equal(W, W_ref) and torch.equal(U, U_ref)
+    side = torch.cuda.Stream()
+    U.zero_()
+    torch.cuda.synchronize()
+    with torch.cuda.stream(side):
+        w()
+        f()
+    side.synchronize()
+    assert torch.equal(U, U_ref)
+    with pytest.raises(ValueError):
+        vn.prepare_farfield(X, F, W[:, :-1].contiguous(), U)
+    U2 = torch.empty_like(X)
+    m = vn.prepare_farfield_fmm(X, F, W, U2, s.mu, 14)
+    assert m() is U2
+    ref = vn.vn_farfield_fmm(X, F, W, s.mu, 14)
+    torch.cuda.synchronize()
+    assert torch.equal(U2, ref)
